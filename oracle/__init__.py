@@ -1,0 +1,13 @@
+"""CPU oracle for the constrained-decoding step -- TEST INFRASTRUCTURE.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference legs may import this package.  See oracle_cd.c.
+"""
+from .oracle_cd import (  # noqa: F401
+    OracleError,
+    build,
+    compact,
+    decode_loop,
+    step,
+    validate,
+)

@@ -1,0 +1,226 @@
+/*
+ * oracle_cd.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, single-threaded CPU definition of the batched type-constrained
+ * decoding step (BASELINE.json north_star).  It
+ * exists so that the CUDA path can be checked against something that a reader
+ * can compare with the text by eye.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may build, load or call it.
+ * It shares no code, header, table or helper with paper_2606_31808_b200/ and
+ * neither side includes the other.
+ *
+ * What the paper fixes:
+ *   - every LM-function generation is restricted to the strings of its
+ *     return_type / options set ("constrained decoding ... guaranteeing
+ *     adherence to datatype structures", section 2.3);
+ *   - the restriction is applied as a mask at the decoding level (section 7,
+ *     L458);
+ *   - one database row in, one value out (section 2.3.2);
+ *   - finished sequences leave the batch (continuous batching, section 4.2,
+ *     L412-L414).
+ * The paper gives no kernel, layout or equation for the step; the precise
+ * definition below is BASELINE.json north_star's: masked max /
+ * argmax with ties to the lowest token id, masked logsumexp, CSR transition,
+ * accept test, stable early-exit compaction.
+ *
+ * Representation choices made ON PURPOSE differently from the GPU path: the
+ * oracle never builds a bitmask; membership is "token appears in the state's
+ * CSR row"; transition lookup is a linear scan; sums are double precision in
+ * ascending token order.
+ *
+ * Pins: tests/test_oracle_pins.py (library log_softmax/argmax on the all-ones
+ * automaton, closed forms, brute force on tiny vocabularies, trie language
+ * enumeration, hand-computed config c0, invariants).
+ * Parity unpinned: log-prob / lse values when an allowed logit is +inf
+ * -- only "token is the lowest-id +inf" is defined.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+enum { ORC_OK = 0, ORC_ERR_ARG = 1, ORC_ERR_AUTOMATON = 2, ORC_ERR_DEAD_STATE = 3 };
+enum { ORC_F32 = 0, ORC_BF16 = 1 };
+
+/* O1: what a valid automaton is. */
+int orc_validate(int32_t V, int32_t S, int32_t start, const int64_t *row_ptr, const int32_t *tok,
+                 const int32_t *next, const uint8_t *accepting)
+{
+    if (V <= 0 || S <= 0 || !row_ptr || !accepting) return ORC_ERR_ARG;
+    if (start < 0 || start >= S) return ORC_ERR_AUTOMATON;
+    if (row_ptr[0] != 0) return ORC_ERR_AUTOMATON;
+    for (int32_t s = 0; s < S; ++s)
+        if (row_ptr[s + 1] < row_ptr[s]) return ORC_ERR_AUTOMATON;
+    if (row_ptr[S] > 0 && (!tok || !next)) return ORC_ERR_ARG;
+    for (int32_t s = 0; s < S; ++s) {
+        for (int64_t j = row_ptr[s]; j < row_ptr[s + 1]; ++j) {
+            if (tok[j] < 0 || tok[j] >= V) return ORC_ERR_AUTOMATON;
+            if (next[j] < 0 || next[j] >= S) return ORC_ERR_AUTOMATON;
+            if (j > row_ptr[s] && tok[j] <= tok[j - 1]) return ORC_ERR_AUTOMATON;
+        }
+    }
+    /* argmax over the empty set is undefined: a state with no way out must accept */
+    for (int32_t s = 0; s < S; ++s)
+        if (row_ptr[s + 1] == row_ptr[s] && !accepting[s]) return ORC_ERR_DEAD_STATE;
+    return ORC_OK;
+}
+
+/* O2.2: widen a stored logit to fp32 exactly; NaN is read as -inf (G6). */
+static float widen(const void *row, int dtype, int64_t t)
+{
+    float x;
+    if (dtype == ORC_BF16) {
+        uint32_t bits = ((uint32_t)((const uint16_t *)row)[t]) << 16;
+        memcpy(&x, &bits, 4);
+    } else {
+        x = ((const float *)row)[t];
+    }
+    if (x != x) x = -INFINITY;
+    return x;
+}
+
+/*
+ * O2: one constrained step for n active rows.  The logits row of slot i is
+ * logits + row_map[i]*ld (row_map == NULL -> i).  state[] is updated in place.
+ */
+int orc_step(int32_t V, int32_t S, const int64_t *row_ptr, const int32_t *tok, const int32_t *next,
+             const uint8_t *accepting, const void *logits, int dtype, int64_t ld,
+             const int32_t *row_map, int32_t *state, int32_t n, int32_t *token_out,
+             double *logprob_out, double *lse_out, uint8_t *done_out)
+{
+    if (n < 0 || ld < V || (dtype != ORC_F32 && dtype != ORC_BF16)) return ORC_ERR_ARG;
+    const int64_t esz = dtype == ORC_BF16 ? 2 : 4;
+    for (int32_t i = 0; i < n; ++i) {
+        const int32_t s = state[i];
+        if (s < 0 || s >= S) return ORC_ERR_ARG;
+        /* O2.1: accepted rows never advance */
+        if (accepting[s]) {
+            token_out[i] = -1;
+            logprob_out[i] = 0.0;
+            lse_out[i] = 0.0;
+            done_out[i] = 1;
+            continue;
+        }
+        const int64_t r = row_map ? (int64_t)row_map[i] : (int64_t)i;
+        const char *row = (const char *)logits + r * ld * esz;
+        const int64_t lo = row_ptr[s], hi = row_ptr[s + 1];
+
+        /* O2.3: m = max over allowed, t* = lowest id attaining it (ascending
+           scan, replace on strictly greater only).  If every allowed logit is
+           -inf the lowest allowed id is kept (G6). */
+        float m = -INFINITY;
+        int32_t tstar = tok[lo];
+        for (int64_t j = lo; j < hi; ++j) {
+            const float x = widen(row, dtype, tok[j]);
+            if (x > m) {
+                m = x;
+                tstar = tok[j];
+            }
+        }
+
+        /* O2.4: sum over allowed of exp(x - m), double, ascending id */
+        double sum = 0.0;
+        for (int64_t j = lo; j < hi; ++j) {
+            const float x = widen(row, dtype, tok[j]);
+            if (x == -INFINITY) continue; /* contributes exactly 0 */
+            sum += exp((double)x - (double)m);
+        }
+        if (m == -INFINITY) {
+            lse_out[i] = -INFINITY;
+            logprob_out[i] = -INFINITY;
+        } else {
+            lse_out[i] = (double)m + log(sum);
+            logprob_out[i] = -log(sum); /* log p(t*) = x_t* - lse = -log(sum); never m - lse */
+        }
+
+        /* O2.5: transition by linear scan, then the accept test */
+        int32_t ns = -1;
+        for (int64_t j = lo; j < hi; ++j)
+            if (tok[j] == tstar) {
+                ns = next[j];
+                break;
+            }
+        token_out[i] = tstar;
+        state[i] = ns;
+        done_out[i] = accepting[ns] ? 1 : 0;
+    }
+    return ORC_OK;
+}
+
+/* O3: stable removal of finished rows.  row_ids_in == NULL means 0..n-1. */
+int orc_compact(const uint8_t *done, const int32_t *row_ids_in, const int32_t *state_in, int32_t n,
+                int32_t *row_ids_out, int32_t *state_out, int32_t *n_active_out)
+{
+    if (n < 0) return ORC_ERR_ARG;
+    int32_t k = 0;
+    for (int32_t i = 0; i < n; ++i) {
+        if (done[i]) continue;
+        row_ids_out[k] = row_ids_in ? row_ids_in[i] : i;
+        if (state_in && state_out) state_out[k] = state_in[i];
+        ++k;
+    }
+    *n_active_out = k;
+    return ORC_OK;
+}
+
+/*
+ * O4: the whole loop.  step_logits[k] is a [B, ld] array indexed by ORIGINAL
+ * row id.  tokens_out is [B, max_steps], -1 padded.  n_active_hist (optional,
+ * [max_steps]) receives the number of rows each step processed.
+ */
+int orc_decode_loop(int32_t V, int32_t S, int32_t start, const int64_t *row_ptr, const int32_t *tok,
+                    const int32_t *next, const uint8_t *accepting, const void *const *step_logits,
+                    int dtype, int64_t ld, int32_t B, int32_t max_steps, int32_t *tokens_out,
+                    int32_t *len_out, int32_t *final_state_out, double *sum_logprob_out,
+                    uint8_t *done_out, int32_t *n_active_hist)
+{
+    if (B < 0 || max_steps < 0) return ORC_ERR_ARG;
+    int32_t *ids = (int32_t *)malloc(sizeof(int32_t) * (size_t)(B + 1) * 6);
+    double *lp = (double *)malloc(sizeof(double) * (size_t)(B + 1) * 2);
+    uint8_t *dn = (uint8_t *)malloc((size_t)B + 1);
+    if (!ids || !lp || !dn) {
+        free(ids); free(lp); free(dn);
+        return ORC_ERR_ARG;
+    }
+    int32_t *st = ids + (B + 1), *ids2 = ids + 2 * (B + 1), *st2 = ids + 3 * (B + 1),
+            *tk = ids + 4 * (B + 1);
+    double *lse = lp + (B + 1);
+    for (int32_t r = 0; r < B; ++r) {
+        for (int32_t k = 0; k < max_steps; ++k) tokens_out[(int64_t)r * max_steps + k] = -1;
+        len_out[r] = 0;
+        final_state_out[r] = start;
+        sum_logprob_out[r] = 0.0;
+        done_out[r] = accepting[start] ? 1 : 0; /* G13 */
+    }
+    if (n_active_hist)
+        for (int32_t k = 0; k < max_steps; ++k) n_active_hist[k] = 0;
+    int32_t n = 0;
+    if (!accepting[start])
+        for (int32_t r = 0; r < B; ++r) {
+            ids[n] = r;
+            st[n] = start;
+            ++n;
+        }
+    int rc = ORC_OK;
+    for (int32_t k = 0; k < max_steps && n > 0; ++k) {
+        if (n_active_hist) n_active_hist[k] = n;
+        rc = orc_step(V, S, row_ptr, tok, next, accepting, step_logits[k], dtype, ld, ids, st, n, tk,
+                      lp, lse, dn);
+        if (rc != ORC_OK) break;
+        for (int32_t i = 0; i < n; ++i) {
+            const int32_t r = ids[i];
+            tokens_out[(int64_t)r * max_steps + k] = tk[i];
+            len_out[r] = k + 1;
+            final_state_out[r] = st[i];
+            sum_logprob_out[r] += lp[i];
+            done_out[r] = dn[i];
+        }
+        int32_t n2 = 0;
+        orc_compact(dn, ids, st, n, ids2, st2, &n2);
+        memcpy(ids, ids2, sizeof(int32_t) * (size_t)n2);
+        memcpy(st, st2, sizeof(int32_t) * (size_t)n2);
+        n = n2;
+    }
+    free(ids); free(lp); free(dn);
+    return rc;
+}

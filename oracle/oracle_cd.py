@@ -1,0 +1,166 @@
+"""ctypes loader for oracle_cd.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Argument marshalling only: every number the oracle reports is computed in
+oracle_cd.c (plain C, single thread, double accumulation).
+This module shares nothing with paper_2606_31808_b200/ and must never be
+imported from it.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import List, Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle_cd.c")
+_SO = os.path.join(_HERE, "liboracle_cd.so")
+_lib = None
+
+F32, BF16 = 0, 1
+OK, ERR_ARG, ERR_AUTOMATON, ERR_DEAD_STATE = 0, 1, 2, 3
+
+
+class OracleError(RuntimeError):
+    def __init__(self, code: int):
+        super().__init__(f"oracle status {code}")
+        self.code = code
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 the oracle into oracle/liboracle_cd.so (no -ffast-math: the
+    summation order and exp/log are the definition)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        tmp = _SO + f".tmp{os.getpid()}"
+        subprocess.check_call(
+            ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"]
+        )
+        os.replace(tmp, _SO)
+    return _SO
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.orc_validate.restype = C.c_int
+        _lib.orc_step.restype = C.c_int
+        _lib.orc_compact.restype = C.c_int
+        _lib.orc_decode_loop.restype = C.c_int
+    return _lib
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _csr(aut):
+    """aut: anything with V, S, start, row_ptr, tok, next, accepting (torch or numpy)."""
+    def np_(x, dt):
+        if hasattr(x, "detach"):
+            x = x.detach().cpu().numpy()
+        return np.ascontiguousarray(np.asarray(x, dtype=dt))
+    return (
+        int(aut.V), int(aut.S), int(aut.start),
+        np_(aut.row_ptr, np.int64), np_(aut.tok, np.int32), np_(aut.next, np.int32),
+        np_(aut.accepting, np.uint8),
+    )
+
+
+def _logits_np(x) -> Tuple[np.ndarray, int]:
+    """[rows, ld] logits (torch fp32 / bf16 tensor, or numpy float32 / uint16
+    holding bf16 bits) -> contiguous numpy array + dtype code.  Bytes are
+    passed through untouched."""
+    if hasattr(x, "detach"):
+        import torch
+        x = x.detach().cpu().contiguous()
+        if x.dtype == torch.bfloat16:
+            return x.view(torch.int16).numpy().view(np.uint16), BF16
+        if x.dtype == torch.float32:
+            return x.numpy(), F32
+        raise TypeError(f"unsupported logits dtype {x.dtype}")
+    x = np.ascontiguousarray(x)
+    if x.dtype == np.uint16:
+        return x, BF16
+    if x.dtype == np.float32:
+        return x, F32
+    raise TypeError(f"unsupported logits dtype {x.dtype}")
+
+
+def validate(aut) -> int:
+    V, S, start, rp, tok, nxt, acc = _csr(aut)
+    return int(_load().orc_validate(C.c_int32(V), C.c_int32(S), C.c_int32(start), _p(rp), _p(tok), _p(nxt), _p(acc)))
+
+
+def step(aut, logits, state: Sequence[int], row_map: Optional[Sequence[int]] = None):
+    """One constrained step (O2).  Returns (token i32[n], logprob f64[n],
+    lse f64[n], done u8[n], new_state i32[n])."""
+    V, S, start, rp, tok, nxt, acc = _csr(aut)
+    x, dt = _logits_np(logits)
+    assert x.ndim == 2
+    ld = x.shape[1]
+    st = np.ascontiguousarray(np.asarray(state, dtype=np.int32)).copy()
+    n = st.shape[0]
+    rm = None if row_map is None else np.ascontiguousarray(np.asarray(row_map, dtype=np.int32))
+    if rm is not None:
+        assert rm.shape[0] == n and (n == 0 or (rm.min() >= 0 and rm.max() < x.shape[0]))
+    else:
+        assert n <= x.shape[0]
+    token = np.empty(n, np.int32)
+    lp = np.empty(n, np.float64)
+    lse = np.empty(n, np.float64)
+    done = np.empty(n, np.uint8)
+    rc = _load().orc_step(
+        C.c_int32(V), C.c_int32(S), _p(rp), _p(tok), _p(nxt), _p(acc), _p(x), C.c_int(dt),
+        C.c_int64(ld), _p(rm), _p(st), C.c_int32(n), _p(token), _p(lp), _p(lse), _p(done))
+    if rc != OK:
+        raise OracleError(rc)
+    return token, lp, lse, done, st
+
+
+def compact(done, row_ids=None, state=None):
+    """Stable compaction (O3).  Returns (row_ids_out i32[k], state_out i32[k] or None, k)."""
+    dn = np.ascontiguousarray(np.asarray(done, dtype=np.uint8))
+    n = dn.shape[0]
+    ri = None if row_ids is None else np.ascontiguousarray(np.asarray(row_ids, dtype=np.int32))
+    si = None if state is None else np.ascontiguousarray(np.asarray(state, dtype=np.int32))
+    ro = np.empty(n, np.int32)
+    so = None if si is None else np.empty(n, np.int32)
+    k = C.c_int32(0)
+    rc = _load().orc_compact(_p(dn), _p(ri), _p(si), C.c_int32(n), _p(ro), _p(so), C.byref(k))
+    if rc != OK:
+        raise OracleError(rc)
+    return ro[: k.value].copy(), (None if so is None else so[: k.value].copy()), int(k.value)
+
+
+def decode_loop(aut, step_logits: List, max_steps: Optional[int] = None):
+    """The whole loop (O4).  step_logits[k] is [B, ld] indexed by original row
+    id.  Returns dict(tokens i32[B,max_steps], len, final_state, sum_logprob
+    f64, done u8, n_active_hist i32[max_steps])."""
+    V, S, start, rp, tok, nxt, acc = _csr(aut)
+    max_steps = len(step_logits) if max_steps is None else max_steps
+    assert len(step_logits) >= max_steps
+    arrs = [_logits_np(x) for x in step_logits[:max_steps]]
+    if max_steps:
+        B, ld = arrs[0][0].shape
+        dt = arrs[0][1]
+        assert all(a.shape == (B, ld) and d == dt for a, d in arrs)
+    else:
+        B, ld, dt = 0, V, F32
+    ptrs = (C.c_void_p * max(1, max_steps))(*[a.ctypes.data for a, _ in arrs])
+    tokens = np.empty((B, max_steps), np.int32)
+    ln = np.empty(B, np.int32)
+    fs = np.empty(B, np.int32)
+    slp = np.empty(B, np.float64)
+    done = np.empty(B, np.uint8)
+    hist = np.zeros(max(1, max_steps), np.int32)
+    rc = _load().orc_decode_loop(
+        C.c_int32(V), C.c_int32(S), C.c_int32(start), _p(rp), _p(tok), _p(nxt), _p(acc), ptrs,
+        C.c_int(dt), C.c_int64(ld), C.c_int32(B), C.c_int32(max_steps), _p(tokens), _p(ln), _p(fs),
+        _p(slp), _p(done), _p(hist))
+    if rc != OK:
+        raise OracleError(rc)
+    return dict(tokens=tokens, len=ln, final_state=fs, sum_logprob=slp, done=done,
+                n_active_hist=hist[:max_steps])
