@@ -1,0 +1,200 @@
+/*
+ * cd.h -- C ABI of the B200 (sm_100a) batched type-constrained decoding step.
+ *
+ * What this library computes.  A local-LM query engine applies an LM function
+ * with a typed output (boolean, one value of an option set, a regex-shaped
+ * value) to every row of a table, one row per prompt (section 2.3.2,
+ * L93-L106), and restricts every generation to the strings of that type by
+ * masking the logits at each decoding step (section 2.3 "Constrained
+ * Decoding", L61; section 7).  Finished sequences leave the running
+ * batch (continuous batching, section 4.2).  The paper delegates
+ * the step to third-party engines and gives no kernel; the operation is fixed
+ * by BASELINE.json north_star:
+ *
+ *   for each active row i with automaton state s_i and logits row x_i[0..V):
+ *     A   = { t : state s_i has a transition on token t }     (allowed set)
+ *     m   = max_{t in A} x_i[t]                                (NaN read as -inf)
+ *     t*  = min { t in A : x_i[t] == m }                       (ties -> lowest id)
+ *     lse = m + log sum_{t in A} exp(x_i[t] - m)               (fp32 accumulate)
+ *     logprob = -log sum_{t in A} exp(x_i[t] - m)              (= x_i[t*] - lse)
+ *     s_i' = next(s_i, t*)     via the per-state sorted CSR of (token, next)
+ *     done_i = accepting[s_i']
+ *   then rows with done_i = 1 are removed from the active list, order kept.
+ *
+ * Conventions
+ *   - every entry point returns a cd_status and never throws or aborts; on
+ *     error *out arguments are untouched and cd_last_error() (thread local)
+ *     describes the failure;
+ *   - "DEVICE pointer": memory of the device the automaton was compiled for,
+ *     owned by the caller, alive until the stream reaches the call's work;
+ *     "HOST pointer": ordinary host memory, read/written before return unless
+ *     stated otherwise;
+ *   - cd_step, cd_transition and cd_compact are asynchronous on `cuda_stream`
+ *     (a cudaStream_t passed as void*; NULL = legacy default stream) and do
+ *     not synchronise with the host; cd_decode_loop* synchronise the stream
+ *     once before returning;
+ *   - a handle is immutable after cd_compile_*.  It may be used from several
+ *     streams and host threads at once: scratch memory is kept per
+ *     (handle, stream) and created on the first call that uses that stream
+ *     (that first call allocates and therefore synchronises; cd_reserve does
+ *     it ahead of time, e.g. before CUDA-graph capture);
+ *   - logits rows start 16-byte aligned: the base pointer is 16-byte aligned
+ *     and ld_elems * sizeof(element) is a multiple of 16; ld_elems >= V.
+ *   - there is no CPU fallback: without a CUDA device every call fails with
+ *     CD_ERR_CUDA.
+ */
+#ifndef CD_H_
+#define CD_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define CD_API __attribute__((visibility("default")))
+#else
+#define CD_API
+#endif
+
+typedef struct cd_dfa cd_dfa_t; /* opaque; owns device memory */
+
+typedef enum {
+    CD_OK = 0,
+    CD_ERR_ARG = 1,        /* bad argument: null pointer, negative size, misalignment, ld < V ... */
+    CD_ERR_AUTOMATON = 2,  /* malformed CSR                                      */
+    CD_ERR_DEAD_STATE = 3, /* a non-accepting state has no transition: argmax over the empty set  */
+    CD_ERR_CUDA = 4,       /* a CUDA runtime call failed (message in cd_last_error)               */
+    CD_ERR_OOM = 5,        /* host or device allocation failed                                    */
+    CD_ERR_INTERNAL = 6    /* a device-side consistency check failed (state out of range, chosen
+                              token missing from the CSR); only cd_decode_loop* can report it     */
+} cd_status;
+
+typedef enum { CD_F32 = 0, CD_BF16 = 1 } cd_dtype;
+
+/*
+ * Automaton store (types -> grammar).
+ * HOST pointers in, device image out.  The CSR lists, for every state s, the
+ * pairs (tok[j], next[j]) for j in [row_ptr[s], row_ptr[s+1]); tok must be
+ * strictly increasing inside a state.  The device image holds the CSR, the
+ * accepting flags and a packed allowed-token bitmask [S][ceil(V/32) padded to a
+ * multiple of 4 words]: bit (t & 31) of word (t >> 5) of row s is set iff state s
+ * has a transition on t; pad bits are zero.
+ * Errors: CD_ERR_ARG (V < 1, S < 1, null pointer, bad device), CD_ERR_AUTOMATON
+ * (row_ptr not non-decreasing from 0, token or next state out of range, tokens
+ * not strictly increasing, start out of range), CD_ERR_DEAD_STATE, CD_ERR_OOM,
+ * CD_ERR_CUDA.  The input arrays are not referenced after return.
+ */
+CD_API cd_status cd_compile_dfa(int32_t V, int32_t S, int32_t start, const int64_t* row_ptr /*[S+1]*/,
+                         const int32_t* tok /*[nnz]*/, const int32_t* next /*[nnz]*/,
+                         const uint8_t* accepting /*[S]*/, int device, cd_dfa_t** out);
+
+/*
+ * Sugar for boolean / option-set types (PAPER.md L61 `options`, L110-L133):
+ * builds the trie automaton of K labels given as token-id sequences
+ * label_tok[label_ptr[k] .. label_ptr[k+1]) (HOST pointers) and compiles it.
+ * State 0 is the root, states are numbered in insertion order, one accepting
+ * leaf per label.  Labels must be non-empty, distinct and prefix-free
+ * (SURVEY 8(c) G5), else CD_ERR_AUTOMATON.
+ */
+CD_API cd_status cd_compile_trie(int32_t V, int32_t K, const int64_t* label_ptr /*[K+1]*/,
+                          const int32_t* label_tok, int device, cd_dfa_t** out);
+
+/* Releases the device image and every per-stream scratch area.  NULL is a no-op.
+   The caller makes sure no work using the handle is still in flight. */
+CD_API void cd_free_dfa(cd_dfa_t* dfa);
+
+/* Shape of a compiled automaton; any out pointer may be NULL. */
+CD_API cd_status cd_dfa_info(const cd_dfa_t* dfa, int32_t* V, int32_t* S, int32_t* start, int64_t* nnz,
+                      int64_t* mask_bytes);
+
+/* Creates (or grows) the scratch area of (dfa, cuda_stream) for up to max_rows
+   rows, so that later calls on that stream neither allocate nor synchronise. */
+CD_API cd_status cd_reserve(const cd_dfa_t* dfa, int32_t max_rows, void* cuda_stream);
+
+/*
+ * One constrained step for n active rows: fused allowed-mask
+ * read, masked max/argmax, masked logsumexp, CSR transition and accept test, one
+ * kernel launch.  All pointers are DEVICE pointers.
+ *   logits      [rows, ld_elems] of `dtype`; the row of active slot i is
+ *               logits + row_map[i] * ld_elems (row_map == NULL -> row i)
+ *   state       [n] in/out: automaton state of slot i, replaced by the next state
+ *   token_out   [n] chosen token id; -1 for a slot whose state is already accepting
+ *   logprob_out [n] log-probability of the chosen token under the masked softmax
+ *   lse_out     [n] masked logsumexp (may be NULL)
+ *   done_out    [n] 1 iff the new state is accepting
+ * A slot whose state is already accepting does not advance: state unchanged,
+ * token -1, logprob 0, lse 0, done 1.  If every allowed logit is -inf (or NaN)
+ * the lowest allowed id is chosen and logprob = lse = -inf.  With an allowed
+ * +inf logit the lowest such id is chosen; logprob / lse are unspecified.
+ * n == 0 is valid and launches nothing.
+ */
+CD_API cd_status cd_step(const cd_dfa_t* dfa, const void* logits, cd_dtype dtype, int64_t ld_elems,
+                  const int32_t* row_map, int32_t* state, int32_t n, int32_t* token_out,
+                  float* logprob_out, float* lse_out, uint8_t* done_out, void* cuda_stream);
+
+/*
+ * Transition lookup on its own for callers that pick tokens
+ * themselves: state[i] <- next(state[i], token[i]); done_out[i] = accepting[new
+ * state].  A slot with token[i] < 0 or whose state has no transition on token[i]
+ * keeps its state and reports done_out[i] = accepting[state[i]].  DEVICE pointers.
+ */
+CD_API cd_status cd_transition(const cd_dfa_t* dfa, const int32_t* token, int32_t* state, int32_t n,
+                        uint8_t* done_out, void* cuda_stream);
+
+/*
+ * Early-exit compaction (finished sequences leave the batch,
+ * PAPER.md L412): stable partition keeping the slots with done[i] == 0.
+ * Out-of-place.  DEVICE pointers.
+ *   row_ids_in  [n] or NULL (NULL -> ids 0..n-1)
+ *   state_in    [n] or NULL (then state_out is not written)
+ *   row_ids_out [n], state_out [n]: first n_active entries are written
+ *   n_active_out device int32
+ */
+CD_API cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, const int32_t* state_in,
+                     int32_t n, int32_t* row_ids_out, int32_t* state_out, int32_t* n_active_out,
+                     void* cuda_stream);
+
+/*
+ * The whole loop: every row starts in the start state; for
+ * k = 0 .. max_steps-1 the active rows take one cd_step on step_logits[k]
+ * (DEVICE pointers in a HOST array; each [B, ld_elems], indexed by ORIGINAL row
+ * id) and finished rows are compacted away.  The active count stays on the
+ * device; the stream is synchronised once before returning.  Outputs are DEVICE
+ * pointers indexed by original row id:
+ *   tokens_out      [B, max_steps] chosen tokens, -1 padded
+ *   len_out         [B] tokens generated
+ *   final_state_out [B]
+ *   sum_logprob_out [B] sum of the chosen tokens' log-probs (fp32)
+ *   done_out        [B] 1 iff the row reached an accepting state (0 = truncated)
+ * If the start state is accepting every row is done with len 0.
+ */
+CD_API cd_status cd_decode_loop(const cd_dfa_t* dfa, const void* const* step_logits, cd_dtype dtype,
+                         int64_t ld_elems, int32_t B, int32_t max_steps, int32_t* tokens_out,
+                         int32_t* len_out, int32_t* final_state_out, float* sum_logprob_out,
+                         uint8_t* done_out, void* cuda_stream);
+
+/*
+ * Same loop with HOST buffers end to end: step_logits_host[k] are HOST arrays
+ * (pinned memory lets the copies overlap the kernels), the five outputs are
+ * HOST arrays.  Host-to-device copies of step k+1 overlap the kernels of step
+ * k through device staging buffers kept in the (handle, stream) scratch area;
+ * copying stops as soon as no row is active.
+ */
+CD_API cd_status cd_decode_loop_host(const cd_dfa_t* dfa, const void* const* step_logits_host,
+                              cd_dtype dtype, int64_t ld_elems, int32_t B, int32_t max_steps,
+                              int32_t* tokens_out, int32_t* len_out, int32_t* final_state_out,
+                              float* sum_logprob_out, uint8_t* done_out, void* cuda_stream);
+
+/* Number of kernel launches this library has enqueued from the calling thread's
+   process so far (monotone; used by bench.py to report gpu_launches). */
+CD_API int64_t cd_launch_count(void);
+
+/* Message of the last failure on the calling thread ("" if none). */
+CD_API const char* cd_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CD_H_ */

@@ -1,0 +1,24 @@
+"""B200-native batched type-constrained decoding step (arxiv/paper_2606_31808 hot path).
+
+Thin Python binding over the C-ABI library libcd.so (include/cd.h): argument
+marshalling only, every step of the path runs in the CUDA kernels under
+csrc/.  PyTorch is used for device memory and streams, nothing else.  There is
+no CPU fallback: if libcd.so is missing or no CUDA device is present the calls
+raise.
+"""
+from .binding import (  # noqa: F401
+    BF16,
+    F32,
+    CdError,
+    Dfa,
+    compact,
+    compile_dfa,
+    compile_trie,
+    decode_loop,
+    decode_loop_host,
+    launch_count,
+    lib,
+    lib_path,
+    step,
+    transition,
+)

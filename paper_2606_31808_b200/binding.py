@@ -1,0 +1,271 @@
+"""ctypes binding with the same names as include/cd.h (argument marshalling only)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import List, Optional, Sequence
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(HERE, "libcd.so")
+_lib = None
+
+F32, BF16 = 0, 1
+STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_STATE",
+          4: "CD_ERR_CUDA", 5: "CD_ERR_OOM", 6: "CD_ERR_INTERNAL"}
+
+# every symbol include/cd.h declares (tests check the .so exports each of them)
+SYMBOLS = (
+    "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_reserve", "cd_step",
+    "cd_transition", "cd_compact", "cd_decode_loop", "cd_decode_loop_host", "cd_launch_count",
+    "cd_last_error",
+)
+
+
+class CdError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{STATUS.get(code, code)}: {msg}")
+        self.code = code
+
+
+def lib_path() -> str:
+    return _SO
+
+
+def lib():
+    """Loads libcd.so; fails loudly when it has not been built (no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise RuntimeError(
+                f"{_SO} is missing: build it with `python -m paper_2606_31808_b200.build` "
+                "(nvcc, sm_100a). There is no CPU fallback.")
+        L = C.CDLL(_SO)
+        for name in SYMBOLS:
+            getattr(L, name)
+        L.cd_last_error.restype = C.c_char_p
+        L.cd_launch_count.restype = C.c_int64
+        L.cd_free_dfa.restype = None
+        L.cd_free_dfa.argtypes = [C.c_void_p]
+        for name in SYMBOLS:
+            if name not in ("cd_last_error", "cd_launch_count", "cd_free_dfa"):
+                getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise CdError(rc, lib().cd_last_error().decode("utf-8", "replace"))
+
+
+def launch_count() -> int:
+    return int(lib().cd_launch_count())
+
+
+def _host(x, dtype) -> torch.Tensor:
+    t = torch.as_tensor(x).detach().to("cpu", dtype).contiguous()
+    return t
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return C.c_void_p(None) if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream(device) -> C.c_void_p:
+    return C.c_void_p(torch.cuda.current_stream(device).cuda_stream)
+
+
+def _dt(t: torch.Tensor) -> int:
+    if t.dtype == torch.bfloat16:
+        return BF16
+    if t.dtype == torch.float32:
+        return F32
+    raise TypeError(f"logits must be float32 or bfloat16, got {t.dtype}")
+
+
+def _dev_tensor(t: torch.Tensor, dtype, name: str, device) -> torch.Tensor:
+    if t.dtype != dtype or not t.is_cuda or not t.is_contiguous() or t.device != device:
+        raise TypeError(f"{name}: expected contiguous {dtype} tensor on {device}")
+    return t
+
+
+class Dfa:
+    """Owner of a cd_dfa_t* handle."""
+
+    def __init__(self, handle: int, device: torch.device):
+        self._h = C.c_void_p(handle)
+        self.device = device
+        V, S, start = C.c_int32(), C.c_int32(), C.c_int32()
+        nnz, mb = C.c_int64(), C.c_int64()
+        _check(lib().cd_dfa_info(self._h, C.byref(V), C.byref(S), C.byref(start), C.byref(nnz), C.byref(mb)))
+        self.V, self.S, self.start, self.nnz, self.mask_bytes = V.value, S.value, start.value, nnz.value, mb.value
+
+    def reserve(self, max_rows: int):
+        _check(lib().cd_reserve(self._h, C.c_int32(max_rows), _stream(self.device)))
+
+    def close(self):
+        if self._h:
+            lib().cd_free_dfa(self._h)
+            self._h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _device_index(device) -> torch.device:
+    d = torch.device(device)
+    if d.type != "cuda":
+        raise ValueError("device must be a CUDA device")
+    return torch.device("cuda", d.index if d.index is not None else torch.cuda.current_device())
+
+
+def compile_dfa(V: int, S: int, start: int, row_ptr, tok, next, accepting, device="cuda") -> Dfa:
+    """cd_compile_dfa: host CSR in, device automaton store out."""
+    L = lib()
+    rp, tk = _host(row_ptr, torch.int64), _host(tok, torch.int32)
+    nx, ac = _host(next, torch.int32), _host(accepting, torch.uint8)
+    if rp.numel() != S + 1 or ac.numel() != S or tk.numel() != nx.numel():
+        raise ValueError("CSR array lengths do not match S / nnz")
+    if S >= 0 and rp.numel() > 0 and int(rp[-1]) > tk.numel():
+        raise ValueError("row_ptr[S] exceeds len(tok)")
+    dev_index = 0
+    dev = None
+    if torch.cuda.is_available():
+        dev = _device_index(device)
+        dev_index = dev.index
+    out = C.c_void_p()
+    _check(L.cd_compile_dfa(C.c_int32(V), C.c_int32(S), C.c_int32(start), _ptr(rp), _ptr(tk), _ptr(nx),
+                            _ptr(ac), C.c_int(dev_index), C.byref(out)))
+    return Dfa(out.value, dev)
+
+
+def compile_trie(V: int, labels: Sequence[Sequence[int]], device="cuda") -> Dfa:
+    """cd_compile_trie: option-set / boolean types as a trie over token-id labels."""
+    L = lib()
+    ptr = [0]
+    flat: List[int] = []
+    for lab in labels:
+        flat.extend(int(t) for t in lab)
+        ptr.append(len(flat))
+    lp = torch.tensor(ptr, dtype=torch.int64)
+    lt = torch.tensor(flat, dtype=torch.int32)
+    dev_index = 0
+    dev = None
+    if torch.cuda.is_available():
+        dev = _device_index(device)
+        dev_index = dev.index
+    out = C.c_void_p()
+    _check(L.cd_compile_trie(C.c_int32(V), C.c_int32(len(labels)), _ptr(lp), _ptr(lt), C.c_int(dev_index),
+                             C.byref(out)))
+    return Dfa(out.value, dev)
+
+
+def step(dfa: Dfa, logits: torch.Tensor, state: torch.Tensor, row_map: Optional[torch.Tensor] = None,
+         n: Optional[int] = None, want_lse: bool = True):
+    """cd_step on torch's current stream.  state (int32, device) is updated in
+    place.  Returns (token i32[n], logprob f32[n], lse f32[n] or None, done u8[n])."""
+    dev = dfa.device
+    if logits.dim() != 2 or not logits.is_cuda or logits.stride(1) != 1:
+        raise TypeError("logits must be a 2-D CUDA tensor with unit inner stride")
+    _dev_tensor(state, torch.int32, "state", dev)
+    n = state.numel() if n is None else n
+    if row_map is not None:
+        _dev_tensor(row_map, torch.int32, "row_map", dev)
+    token = torch.empty(n, dtype=torch.int32, device=dev)
+    logprob = torch.empty(n, dtype=torch.float32, device=dev)
+    lse = torch.empty(n, dtype=torch.float32, device=dev) if want_lse else None
+    done = torch.empty(n, dtype=torch.uint8, device=dev)
+    _check(lib().cd_step(dfa._h, _ptr(logits), C.c_int(_dt(logits)), C.c_int64(logits.stride(0)), _ptr(row_map),
+                         _ptr(state), C.c_int32(n), _ptr(token), _ptr(logprob), _ptr(lse), _ptr(done),
+                         _stream(dev)))
+    return token, logprob, lse, done
+
+
+def transition(dfa: Dfa, token: torch.Tensor, state: torch.Tensor):
+    """cd_transition: state updated in place; returns done u8[n]."""
+    dev = dfa.device
+    _dev_tensor(token, torch.int32, "token", dev)
+    _dev_tensor(state, torch.int32, "state", dev)
+    n = state.numel()
+    done = torch.empty(n, dtype=torch.uint8, device=dev)
+    _check(lib().cd_transition(dfa._h, _ptr(token), _ptr(state), C.c_int32(n), _ptr(done), _stream(dev)))
+    return done
+
+
+def compact(done: torch.Tensor, row_ids: Optional[torch.Tensor] = None, state: Optional[torch.Tensor] = None,
+            n: Optional[int] = None):
+    """cd_compact.  Returns (row_ids_out i32[n], state_out i32[n] or None,
+    n_active device int32[1]); only the first n_active entries are meaningful."""
+    dev = done.device
+    _dev_tensor(done, torch.uint8, "done", dev)
+    n = done.numel() if n is None else n
+    if row_ids is not None:
+        _dev_tensor(row_ids, torch.int32, "row_ids", dev)
+    if state is not None:
+        _dev_tensor(state, torch.int32, "state", dev)
+    ro = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+    so = torch.empty(max(n, 1), dtype=torch.int32, device=dev) if state is not None else None
+    na = torch.empty(1, dtype=torch.int32, device=dev)
+    with torch.cuda.device(dev):
+        _check(lib().cd_compact(_ptr(done), _ptr(row_ids), _ptr(state), C.c_int32(n), _ptr(ro), _ptr(so), _ptr(na),
+                                _stream(dev)))
+    return ro, so, na
+
+
+def _loop_outputs(B: int, max_steps: int, device, pin: bool = False):
+    kw = dict(device=device)
+    if pin:
+        kw = dict(device="cpu", pin_memory=True)
+    return dict(
+        tokens=torch.empty((B, max_steps), dtype=torch.int32, **kw),
+        len=torch.empty(B, dtype=torch.int32, **kw),
+        final_state=torch.empty(B, dtype=torch.int32, **kw),
+        sum_logprob=torch.empty(B, dtype=torch.float32, **kw),
+        done=torch.empty(B, dtype=torch.uint8, **kw),
+    )
+
+
+def decode_loop(dfa: Dfa, step_logits: Sequence[torch.Tensor], max_steps: Optional[int] = None, out=None):
+    """cd_decode_loop: step_logits[k] are [B, ld] CUDA tensors indexed by original
+    row id.  Returns dict(tokens, len, final_state, sum_logprob, done) of device
+    tensors.  Synchronises the current stream once."""
+    dev = dfa.device
+    max_steps = len(step_logits) if max_steps is None else max_steps
+    if max_steps > len(step_logits):
+        raise ValueError("fewer step buffers than max_steps")
+    if max_steps == 0:
+        raise ValueError("max_steps must be >= 1 here (B is taken from the step buffers)")
+    x0 = step_logits[0]
+    B, ld, dt = x0.shape[0], x0.stride(0), _dt(x0)
+    for x in step_logits[:max_steps]:
+        if x.dim() != 2 or not x.is_cuda or x.stride(1) != 1 or x.shape[0] != B or x.stride(0) != ld or _dt(x) != dt:
+            raise TypeError("step_logits must share shape, stride and dtype")
+    ptrs = (C.c_void_p * max_steps)(*[x.data_ptr() for x in step_logits[:max_steps]])
+    out = _loop_outputs(B, max_steps, dev) if out is None else out
+    _check(lib().cd_decode_loop(dfa._h, ptrs, C.c_int(dt), C.c_int64(ld), C.c_int32(B), C.c_int32(max_steps),
+                                _ptr(out["tokens"]), _ptr(out["len"]), _ptr(out["final_state"]),
+                                _ptr(out["sum_logprob"]), _ptr(out["done"]), _stream(dev)))
+    return out
+
+
+def decode_loop_host(dfa: Dfa, step_logits_host: Sequence[torch.Tensor], max_steps: Optional[int] = None, out=None):
+    """cd_decode_loop_host: HOST tensors in (pinned memory overlaps the copies),
+    HOST tensors out; host<->device copies happen inside the call."""
+    dev = dfa.device
+    max_steps = len(step_logits_host) if max_steps is None else max_steps
+    x0 = step_logits_host[0]
+    B, ld, dt = x0.shape[0], x0.stride(0), _dt(x0)
+    for x in step_logits_host[:max_steps]:
+        if x.is_cuda or x.dim() != 2 or x.stride(1) != 1 or x.shape[0] != B or x.stride(0) != ld or _dt(x) != dt:
+            raise TypeError("step_logits_host must be host tensors sharing shape, stride and dtype")
+    ptrs = (C.c_void_p * max_steps)(*[x.data_ptr() for x in step_logits_host[:max_steps]])
+    out = _loop_outputs(B, max_steps, dev, pin=True) if out is None else out
+    _check(lib().cd_decode_loop_host(dfa._h, ptrs, C.c_int(dt), C.c_int64(ld), C.c_int32(B), C.c_int32(max_steps),
+                                     _ptr(out["tokens"]), _ptr(out["len"]), _ptr(out["final_state"]),
+                                     _ptr(out["sum_logprob"]), _ptr(out["done"]), _stream(dev)))
+    return out

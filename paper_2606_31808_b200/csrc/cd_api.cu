@@ -1,0 +1,682 @@
+// cd_api.cu -- the C ABI of include/cd.h: validation, automaton store, scratch management and
+// kernel launches.  No torch types, no CPU fallback: every step of the path runs in the
+// kernels of cd_step.cuh / cd_aux.cuh.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <map>
+#include <mutex>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/cd.h"
+#include "cd_aux.cuh"
+#include "cd_common.cuh"
+#include "cd_step.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+std::atomic<long long> g_launches{0};
+
+cd_status fail(cd_status st, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return st;
+}
+
+#define CU(call)                                                                             \
+    do {                                                                                     \
+        cudaError_t e__ = (call);                                                            \
+        if (e__ != cudaSuccess) {                                                            \
+            const cd_status st__ = (e__ == cudaErrorMemoryAllocation) ? CD_ERR_OOM : CD_ERR_CUDA; \
+            return fail(st__, "%s -> %s (%s:%d)", #call, cudaGetErrorString(e__), __FILE__, __LINE__); \
+        }                                                                                    \
+    } while (0)
+
+constexpr int STEP_WARPS = 8;
+constexpr int STEP_STAGES = 4;
+
+// Per (handle, stream) scratch.  Operations on one stream are ordered, so one area per stream
+// is race free; distinct streams get distinct areas.
+struct Scratch {
+    int cap_rows = 0;
+    long long cap_units = 0;
+    int4* partials = nullptr;
+    int* tickets = nullptr;
+    int* ctrs = nullptr;  // [0] work, [1] finished warps, [2] sticky errors, [3] spare
+    // decode loop
+    int* row_ids[2] = {nullptr, nullptr};
+    int* state[2] = {nullptr, nullptr};
+    int* n_active = nullptr;  // [2]
+    int* token = nullptr;
+    float* logprob = nullptr;
+    uint8_t* done = nullptr;
+    // host-buffer loop
+    void* stage[2] = {nullptr, nullptr};
+    size_t stage_bytes = 0;
+    int* out_i32 = nullptr;  // device copies of the host outputs
+    size_t out_bytes = 0;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr};
+    cudaEvent_t ev_consumed[2] = {nullptr, nullptr};
+    int* h_pinned = nullptr;  // [4] pinned host ints
+
+    void release() {
+        cudaFree(partials); cudaFree(tickets); cudaFree(ctrs);
+        for (int i = 0; i < 2; ++i) { cudaFree(row_ids[i]); cudaFree(state[i]); cudaFree(stage[i]); }
+        cudaFree(n_active); cudaFree(token); cudaFree(logprob); cudaFree(done); cudaFree(out_i32);
+        if (copy_stream) cudaStreamDestroy(copy_stream);
+        for (int i = 0; i < 2; ++i) {
+            if (ev_copied[i]) cudaEventDestroy(ev_copied[i]);
+            if (ev_consumed[i]) cudaEventDestroy(ev_consumed[i]);
+        }
+        if (h_pinned) cudaFreeHost(h_pinned);
+        *this = Scratch();
+    }
+};
+
+}  // namespace
+
+struct cd_dfa {
+    cd::DfaDev dev{};
+    int device = 0;
+    int start = 0;
+    int start_accepting = 0;
+    long long nnz = 0;
+    int num_sms = 0;
+    void* d_mask = nullptr;
+    void* d_row_ptr = nullptr;
+    void* d_tok = nullptr;
+    void* d_next = nullptr;
+    void* d_acc = nullptr;
+    std::mutex mu;
+    std::map<cudaStream_t, Scratch> scratch;
+};
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+template <int DT>
+constexpr int tile_tok() { return cd::TILE_BYTES / (DT == cd::DT_BF16 ? 2 : 4); }
+
+int tiles_per_row(int V, int dtype) {
+    const int tt = cd::TILE_BYTES / (dtype == CD_BF16 ? 2 : 4);
+    return (V + tt - 1) / tt;
+}
+
+int step_grid(const cd_dfa* d, long long n_upper, int dtype) {
+    const long long tiles = n_upper * tiles_per_row(d->dev.V, dtype);
+    long long g = (tiles + 1) / 2;  // few rows: still spread the tiles over many SMs
+    if (g < 1) g = 1;
+    if (g > d->num_sms) g = d->num_sms;
+    return (int)g;
+}
+
+// Upper bound of n' * P(n') over n' <= n for the largest grid (mirrors cd::tiles_per_unit):
+// unclamped tiles-per-unit gives n'P <= 4*warps + n'; clamped at TPU_MAX gives n' * ceil(T/16).
+long long step_units_cap(const cd_dfa* d, long long n) {
+    const int T = tiles_per_row(d->dev.V, CD_BF16) > tiles_per_row(d->dev.V, CD_F32)
+                      ? tiles_per_row(d->dev.V, CD_BF16)
+                      : tiles_per_row(d->dev.V, CD_F32);
+    const long long warps = (long long)d->num_sms * STEP_WARPS;
+    const long long a = warps * cd::UNITS_PER_WARP + n;
+    const long long b = n * ((T + cd::TPU_MAX - 1) / cd::TPU_MAX + 1);
+    // small grids (few rows) use fewer warps, hence fewer units: still below a
+    return (a > b ? a : b) + 64;
+}
+
+cd_status get_scratch(const cd_dfa* cd_, cudaStream_t stream, int rows, bool loop_bufs, Scratch** out) {
+    cd_dfa* d = const_cast<cd_dfa*>(cd_);
+    std::lock_guard<std::mutex> lk(d->mu);
+    Scratch& s = d->scratch[stream];
+    if (rows < 1) rows = 1;
+    if (s.cap_rows < rows) {
+        // growing: wait for the work that still uses the old buffers
+        if (s.cap_rows > 0) CU(cudaStreamSynchronize(stream));
+        int sticky[4] = {0, 0, 0, 0};
+        Scratch old = s;
+        s.cap_rows = 0;
+        const long long units = step_units_cap(d, rows);
+        CU(cudaMalloc(&s.partials, sizeof(int4) * units));
+        CU(cudaMalloc(&s.tickets, sizeof(int) * (size_t)rows));
+        CU(cudaMalloc(&s.ctrs, sizeof(int) * 4));
+        CU(cudaMemset(s.tickets, 0, sizeof(int) * (size_t)rows));
+        CU(cudaMemcpy(s.ctrs, sticky, sizeof sticky, cudaMemcpyHostToDevice));
+        for (int i = 0; i < 2; ++i) {
+            CU(cudaMalloc(&s.row_ids[i], sizeof(int) * (size_t)rows));
+            CU(cudaMalloc(&s.state[i], sizeof(int) * (size_t)rows));
+        }
+        CU(cudaMalloc(&s.n_active, sizeof(int) * 2));
+        CU(cudaMalloc(&s.token, sizeof(int) * (size_t)rows));
+        CU(cudaMalloc(&s.logprob, sizeof(float) * (size_t)rows));
+        CU(cudaMalloc(&s.done, (size_t)rows));
+        s.cap_units = units;
+        s.cap_rows = rows;
+        // keep the host-loop resources, drop the old step buffers
+        old.stage[0] = old.stage[1] = nullptr; old.out_i32 = nullptr; old.copy_stream = nullptr;
+        old.ev_copied[0] = old.ev_copied[1] = old.ev_consumed[0] = old.ev_consumed[1] = nullptr;
+        old.h_pinned = nullptr;
+        old.release();
+    }
+    (void)loop_bufs;
+    *out = &s;
+    return CD_OK;
+}
+
+cd_status check_dtype(cd_dtype dt) {
+    if (dt != CD_F32 && dt != CD_BF16) return fail(CD_ERR_ARG, "dtype must be CD_F32 or CD_BF16");
+    return CD_OK;
+}
+
+template <int DT>
+cd_status launch_step_t(const cd::StepArgs& a, int grid, cudaStream_t stream) {
+    auto kern = cd::step_kernel<DT, STEP_WARPS, STEP_STAGES>;
+    const size_t smem = sizeof(cd::WarpRing<STEP_STAGES>) * STEP_WARPS;
+    static thread_local int configured_dev[2] = {-1, -1};
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    if (configured_dev[DT] != dev) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured_dev[DT] = dev;
+    }
+    kern<<<grid, STEP_WARPS * 32, smem, stream>>>(a);
+    CU(cudaGetLastError());
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return CD_OK;
+}
+
+// n_upper bounds the active count; n_dev (device int) overrides n inside the kernel.
+cd_status launch_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype dtype, long long ld,
+                      const int* row_map, int* state, int n_upper, const int* n_dev, int* token_out,
+                      float* logprob_out, float* lse_out, uint8_t* done_out, cudaStream_t stream) {
+    cd::StepArgs a{};
+    a.dfa = d->dev;
+    a.logits = static_cast<const unsigned char*>(logits);
+    a.ld_bytes = ld * (dtype == CD_BF16 ? 2 : 4);
+    a.row_map = row_map;
+    a.state = state;
+    a.n = n_upper;
+    a.n_dev = n_dev;
+    a.token_out = token_out;
+    a.logprob_out = logprob_out;
+    a.lse_out = lse_out;
+    a.done_out = done_out;
+    a.partials = s->partials;
+    a.tickets = s->tickets;
+    a.ctrs = s->ctrs;
+    const int grid = step_grid(d, n_upper, dtype);
+    return dtype == CD_BF16 ? launch_step_t<cd::DT_BF16>(a, grid, stream)
+                            : launch_step_t<cd::DT_F32>(a, grid, stream);
+}
+
+cd_status check_logits_layout(const cd_dfa* d, const void* logits, cd_dtype dtype, long long ld) {
+    const long long sz = dtype == CD_BF16 ? 2 : 4;
+    if (!logits) return fail(CD_ERR_ARG, "logits is NULL");
+    if (ld < d->dev.V) return fail(CD_ERR_ARG, "ld_elems (%lld) < V (%d)", ld, d->dev.V);
+    if ((reinterpret_cast<uintptr_t>(logits) & 15) != 0) return fail(CD_ERR_ARG, "logits base is not 16-byte aligned");
+    if ((ld * sz) % 16 != 0) return fail(CD_ERR_ARG, "row stride ld_elems*%lld is not a multiple of 16 bytes", sz);
+    return CD_OK;
+}
+
+cd_status compile_impl(int32_t V, int32_t S, int32_t start, const int64_t* row_ptr, const int32_t* tok,
+                       const int32_t* next, const uint8_t* accepting, int device, cd_dfa_t** out) {
+    if (!out) return fail(CD_ERR_ARG, "out is NULL");
+    if (V < 1 || S < 1) return fail(CD_ERR_ARG, "V and S must be >= 1 (V=%d S=%d)", V, S);
+    if (!row_ptr || !accepting) return fail(CD_ERR_ARG, "row_ptr / accepting is NULL");
+    // ---- validation
+    if (start < 0 || start >= S) return fail(CD_ERR_AUTOMATON, "start state %d outside [0,%d)", start, S);
+    if (row_ptr[0] != 0) return fail(CD_ERR_AUTOMATON, "row_ptr[0] = %lld, expected 0", (long long)row_ptr[0]);
+    for (int32_t s = 0; s < S; ++s)
+        if (row_ptr[s + 1] < row_ptr[s]) return fail(CD_ERR_AUTOMATON, "row_ptr decreases at state %d", s);
+    const long long nnz = row_ptr[S];
+    if (nnz > 0 && (!tok || !next)) return fail(CD_ERR_ARG, "tok / next is NULL with nnz = %lld", nnz);
+    for (int32_t s = 0; s < S; ++s) {
+        for (long long j = row_ptr[s]; j < row_ptr[s + 1]; ++j) {
+            if (tok[j] < 0 || tok[j] >= V) return fail(CD_ERR_AUTOMATON, "state %d: token %d outside [0,%d)", s, tok[j], V);
+            if (next[j] < 0 || next[j] >= S) return fail(CD_ERR_AUTOMATON, "state %d: next state %d outside [0,%d)", s, next[j], S);
+            if (j > row_ptr[s] && tok[j] <= tok[j - 1]) return fail(CD_ERR_AUTOMATON, "state %d: tokens not strictly increasing", s);
+        }
+    }
+    for (int32_t s = 0; s < S; ++s)
+        if (row_ptr[s + 1] == row_ptr[s] && !accepting[s])
+            return fail(CD_ERR_DEAD_STATE, "state %d is not accepting and has no transition", s);
+
+    int ndev = 0;
+    CU(cudaGetDeviceCount(&ndev));
+    if (device < 0 || device >= ndev) return fail(CD_ERR_ARG, "device %d outside [0,%d)", device, ndev);
+    DeviceGuard guard(device);
+    if (!guard.ok) return fail(CD_ERR_CUDA, "cannot select device %d", device);
+
+    cd_dfa* d = new (std::nothrow) cd_dfa();
+    if (!d) return fail(CD_ERR_OOM, "host allocation failed");
+    d->device = device;
+    d->start = start;
+    d->start_accepting = accepting[start] ? 1 : 0;
+    d->nnz = nnz;
+    cudaDeviceProp prop;
+    cudaError_t e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) { delete d; return fail(CD_ERR_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e)); }
+    d->num_sms = prop.multiProcessorCount;
+    const int W = (V + 31) / 32;
+    const int Wpad = (W + 3) & ~3;
+    const size_t mask_bytes = (size_t)S * Wpad * 4;
+    cd_status st = CD_OK;
+    auto alloc = [&](void** p, size_t bytes) {
+        if (st != CD_OK) return;
+        cudaError_t e2 = cudaMalloc(p, bytes ? bytes : 16);
+        if (e2 != cudaSuccess)
+            st = fail(e2 == cudaErrorMemoryAllocation ? CD_ERR_OOM : CD_ERR_CUDA, "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e2));
+    };
+    alloc(&d->d_mask, mask_bytes);
+    alloc(&d->d_row_ptr, sizeof(long long) * (size_t)(S + 1));
+    alloc(&d->d_tok, sizeof(int) * (size_t)nnz);
+    alloc(&d->d_next, sizeof(int) * (size_t)nnz);
+    alloc(&d->d_acc, (size_t)S);
+    auto copy = [&](void* dst, const void* src, size_t bytes) {
+        if (st != CD_OK || bytes == 0) return;
+        cudaError_t e2 = cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice);
+        if (e2 != cudaSuccess) st = fail(CD_ERR_CUDA, "cudaMemcpy H2D: %s", cudaGetErrorString(e2));
+    };
+    static_assert(sizeof(long long) == sizeof(int64_t), "row_ptr width");
+    copy(d->d_row_ptr, row_ptr, sizeof(long long) * (size_t)(S + 1));
+    copy(d->d_tok, tok, sizeof(int) * (size_t)nnz);
+    copy(d->d_next, next, sizeof(int) * (size_t)nnz);
+    copy(d->d_acc, accepting, (size_t)S);
+    if (st == CD_OK) {
+        cudaError_t e2 = cudaMemset(d->d_mask, 0, mask_bytes);
+        if (e2 == cudaSuccess && nnz > 0) {
+            const int threads = 256;
+            long long blocks = ((long long)S * 32 + threads - 1) / threads;
+            if (blocks > 65535) blocks = 65535;
+            cd::build_mask_kernel<<<(int)blocks, threads>>>(static_cast<const long long*>(d->d_row_ptr),
+                                                           static_cast<const int*>(d->d_tok), S, Wpad,
+                                                           static_cast<uint32_t*>(d->d_mask));
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            e2 = cudaGetLastError();
+            if (e2 == cudaSuccess) e2 = cudaDeviceSynchronize();
+        }
+        if (e2 != cudaSuccess) st = fail(CD_ERR_CUDA, "mask build: %s", cudaGetErrorString(e2));
+    }
+    if (st != CD_OK) {
+        cudaFree(d->d_mask); cudaFree(d->d_row_ptr); cudaFree(d->d_tok); cudaFree(d->d_next); cudaFree(d->d_acc);
+        delete d;
+        return st;
+    }
+    d->dev.V = V;
+    d->dev.S = S;
+    d->dev.W = W;
+    d->dev.Wpad = Wpad;
+    d->dev.mask = static_cast<const uint32_t*>(d->d_mask);
+    d->dev.row_ptr = static_cast<const long long*>(d->d_row_ptr);
+    d->dev.tok = static_cast<const int*>(d->d_tok);
+    d->dev.next = static_cast<const int*>(d->d_next);
+    d->dev.accepting = static_cast<const uint8_t*>(d->d_acc);
+    *out = d;
+    return CD_OK;
+}
+
+cd_status launch_compact(bool record, const cd::CompactArgs& a, cudaStream_t stream) {
+    if (record)
+        cd::compact_kernel<true><<<1, 1024, 0, stream>>>(a);
+    else
+        cd::compact_kernel<false><<<1, 1024, 0, stream>>>(a);
+    CU(cudaGetLastError());
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return CD_OK;
+}
+
+cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, int* tokens_out, int* len_out,
+                           int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream) {
+    long long work = (long long)B * (max_steps > 0 ? max_steps : 1);
+    long long blocks = (work + 255) / 256;
+    if (blocks < 1) blocks = 1;
+    if (blocks > 4096) blocks = 4096;
+    cd::loop_init_kernel<<<(int)blocks, 256, 0, stream>>>(B, max_steps, d->start, d->start_accepting, s->row_ids[0],
+                                                          s->state[0], s->n_active, tokens_out, len_out,
+                                                          final_state_out, sum_logprob_out, done_out);
+    CU(cudaGetLastError());
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return CD_OK;
+}
+
+// One loop iteration k on `logits` ([B, ld], original row ids): step + record/compact.
+cd_status enqueue_loop_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype dtype, long long ld, int B,
+                            int k, int max_steps, int* tokens_out, int* len_out, int* final_state_out,
+                            float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream) {
+    const int cur = k & 1, nxt = cur ^ 1;
+    cd_status st = launch_step(d, s, logits, dtype, ld, s->row_ids[cur], s->state[cur], B, s->n_active + cur,
+                               s->token, s->logprob, nullptr, s->done, stream);
+    if (st != CD_OK) return st;
+    cd::CompactArgs c{};
+    c.done = s->done;
+    c.row_ids_in = s->row_ids[cur];
+    c.state_in = s->state[cur];
+    c.n = B;
+    c.n_dev = s->n_active + cur;
+    c.row_ids_out = s->row_ids[nxt];
+    c.state_out = s->state[nxt];
+    c.n_active_out = s->n_active + nxt;
+    c.token = s->token;
+    c.logprob = s->logprob;
+    c.step = k;
+    c.max_steps = max_steps;
+    c.tokens_out = tokens_out;
+    c.len_out = len_out;
+    c.final_state_out = final_state_out;
+    c.sum_logprob_out = sum_logprob_out;
+    c.done_row_out = done_out;
+    return launch_compact(true, c, stream);
+}
+
+cd_status check_sticky_errors(Scratch* s, cudaStream_t stream) {
+    int h[4] = {0, 0, 0, 0};
+    CU(cudaMemcpyAsync(h, s->ctrs, sizeof h, cudaMemcpyDeviceToHost, stream));
+    CU(cudaStreamSynchronize(stream));
+    if (h[2] != 0) {
+        int zero = 0;
+        cudaMemcpyAsync(s->ctrs + 2, &zero, sizeof zero, cudaMemcpyHostToDevice, stream);
+        cudaStreamSynchronize(stream);
+        return fail(CD_ERR_INTERNAL, "%d device-side consistency failures (state out of range or token missing from CSR)", h[2]);
+    }
+    return CD_OK;
+}
+
+}  // namespace
+
+// =============================================================================== C ABI
+extern "C" {
+
+const char* cd_last_error(void) { return g_err.c_str(); }
+
+int64_t cd_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+cd_status cd_compile_dfa(int32_t V, int32_t S, int32_t start, const int64_t* row_ptr, const int32_t* tok,
+                         const int32_t* next, const uint8_t* accepting, int device, cd_dfa_t** out) {
+    try {
+        return compile_impl(V, S, start, row_ptr, tok, next, accepting, device, out);
+    } catch (const std::bad_alloc&) {
+        return fail(CD_ERR_OOM, "host allocation failed");
+    } catch (...) {
+        return fail(CD_ERR_INTERNAL, "unexpected exception");
+    }
+}
+
+cd_status cd_compile_trie(int32_t V, int32_t K, const int64_t* label_ptr, const int32_t* label_tok, int device,
+                          cd_dfa_t** out) {
+    try {
+        if (!out || !label_ptr) return fail(CD_ERR_ARG, "NULL argument");
+        if (V < 1 || K < 1) return fail(CD_ERR_ARG, "V and K must be >= 1");
+        if (label_ptr[0] != 0) return fail(CD_ERR_AUTOMATON, "label_ptr[0] must be 0");
+        if (label_ptr[K] > 0 && !label_tok) return fail(CD_ERR_ARG, "label_tok is NULL");
+        // trie in insertion order; children kept sorted per node
+        std::vector<std::map<int, int>> child(1);
+        std::vector<uint8_t> leaf(1, 0);
+        for (int k = 0; k < K; ++k) {
+            const long long lo = label_ptr[k], hi = label_ptr[k + 1];
+            if (hi <= lo) return fail(CD_ERR_AUTOMATON, "label %d is empty", k);
+            int node = 0;
+            for (long long j = lo; j < hi; ++j) {
+                const int t = label_tok[j];
+                if (t < 0 || t >= V) return fail(CD_ERR_AUTOMATON, "label %d: token %d outside [0,%d)", k, t, V);
+                if (leaf[node]) return fail(CD_ERR_AUTOMATON, "label %d extends another label (not prefix-free)", k);
+                auto it = child[node].find(t);
+                if (it == child[node].end()) {
+                    const int nn = (int)child.size();
+                    child[node][t] = nn;
+                    child.emplace_back();
+                    leaf.push_back(0);
+                    node = nn;
+                } else {
+                    node = it->second;
+                }
+            }
+            if (leaf[node] || !child[node].empty())
+                return fail(CD_ERR_AUTOMATON, "label %d duplicates or is a prefix of another label", k);
+            leaf[node] = 1;
+        }
+        const int S = (int)child.size();
+        std::vector<int64_t> rp(S + 1, 0);
+        std::vector<int32_t> tk, nx;
+        for (int s = 0; s < S; ++s) {
+            for (auto& kv : child[s]) {
+                tk.push_back(kv.first);
+                nx.push_back(kv.second);
+            }
+            rp[s + 1] = (int64_t)tk.size();
+        }
+        return compile_impl(V, S, 0, rp.data(), tk.data(), nx.data(), leaf.data(), device, out);
+    } catch (const std::bad_alloc&) {
+        return fail(CD_ERR_OOM, "host allocation failed");
+    } catch (...) {
+        return fail(CD_ERR_INTERNAL, "unexpected exception");
+    }
+}
+
+void cd_free_dfa(cd_dfa_t* d) {
+    if (!d) return;
+    DeviceGuard guard(d->device);
+    for (auto& kv : d->scratch) kv.second.release();
+    cudaFree(d->d_mask); cudaFree(d->d_row_ptr); cudaFree(d->d_tok); cudaFree(d->d_next); cudaFree(d->d_acc);
+    delete d;
+}
+
+cd_status cd_dfa_info(const cd_dfa_t* d, int32_t* V, int32_t* S, int32_t* start, int64_t* nnz, int64_t* mask_bytes) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (V) *V = d->dev.V;
+    if (S) *S = d->dev.S;
+    if (start) *start = d->start;
+    if (nnz) *nnz = d->nnz;
+    if (mask_bytes) *mask_bytes = (int64_t)d->dev.S * d->dev.Wpad * 4;
+    return CD_OK;
+}
+
+cd_status cd_reserve(const cd_dfa_t* d, int32_t max_rows, void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (max_rows < 0) return fail(CD_ERR_ARG, "max_rows < 0");
+    DeviceGuard guard(d->device);
+    Scratch* s = nullptr;
+    return get_scratch(d, static_cast<cudaStream_t>(cuda_stream), max_rows, true, &s);
+}
+
+cd_status cd_step(const cd_dfa_t* d, const void* logits, cd_dtype dtype, int64_t ld_elems, const int32_t* row_map,
+                  int32_t* state, int32_t n, int32_t* token_out, float* logprob_out, float* lse_out,
+                  uint8_t* done_out, void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (n < 0) return fail(CD_ERR_ARG, "n < 0");
+    cd_status st = check_dtype(dtype);
+    if (st != CD_OK) return st;
+    if (n == 0) return CD_OK;
+    if (!state || !token_out || !logprob_out || !done_out) return fail(CD_ERR_ARG, "NULL output / state pointer");
+    st = check_logits_layout(d, logits, dtype, ld_elems);
+    if (st != CD_OK) return st;
+    if ((long long)n * tiles_per_row(d->dev.V, dtype) >= 0x7FFFFFFFLL)
+        return fail(CD_ERR_ARG, "n * tiles_per_row overflows the unit index");
+    DeviceGuard guard(d->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* s = nullptr;
+    st = get_scratch(d, stream, n, false, &s);
+    if (st != CD_OK) return st;
+    return launch_step(d, s, logits, dtype, ld_elems, row_map, state, n, nullptr, token_out, logprob_out, lse_out,
+                       done_out, stream);
+}
+
+cd_status cd_transition(const cd_dfa_t* d, const int32_t* token, int32_t* state, int32_t n, uint8_t* done_out,
+                        void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (n < 0) return fail(CD_ERR_ARG, "n < 0");
+    if (n == 0) return CD_OK;
+    if (!token || !state || !done_out) return fail(CD_ERR_ARG, "NULL pointer");
+    DeviceGuard guard(d->device);
+    const int threads = 256;
+    long long blocks = ((long long)n * 32 + threads - 1) / threads;
+    if (blocks > 8192) blocks = 8192;
+    cd::transition_kernel<<<(int)blocks, threads, 0, static_cast<cudaStream_t>(cuda_stream)>>>(d->dev, token, state, n,
+                                                                                              done_out);
+    CU(cudaGetLastError());
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return CD_OK;
+}
+
+cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, const int32_t* state_in, int32_t n,
+                     int32_t* row_ids_out, int32_t* state_out, int32_t* n_active_out, void* cuda_stream) {
+    if (n < 0) return fail(CD_ERR_ARG, "n < 0");
+    if (!n_active_out) return fail(CD_ERR_ARG, "n_active_out is NULL");
+    if (n > 0 && (!done || !row_ids_out)) return fail(CD_ERR_ARG, "NULL pointer");
+    if (n > 0 && state_in && !state_out) return fail(CD_ERR_ARG, "state_in given without state_out");
+    cd::CompactArgs c{};
+    c.done = done;
+    c.row_ids_in = row_ids_in;
+    c.state_in = state_in;
+    c.n = n;
+    c.row_ids_out = row_ids_out;
+    c.state_out = state_out;
+    c.n_active_out = n_active_out;
+    return launch_compact(false, c, static_cast<cudaStream_t>(cuda_stream));
+}
+
+cd_status cd_decode_loop(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
+                         int32_t B, int32_t max_steps, int32_t* tokens_out, int32_t* len_out,
+                         int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out, void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (B < 0 || max_steps < 0) return fail(CD_ERR_ARG, "B / max_steps < 0");
+    cd_status st = check_dtype(dtype);
+    if (st != CD_OK) return st;
+    if (B == 0) return CD_OK;
+    if (!len_out || !final_state_out || !sum_logprob_out || !done_out || (max_steps > 0 && !tokens_out))
+        return fail(CD_ERR_ARG, "NULL output pointer");
+    if (max_steps > 0 && !step_logits) return fail(CD_ERR_ARG, "step_logits is NULL");
+    if (!d->start_accepting)
+        for (int k = 0; k < max_steps; ++k) {
+            st = check_logits_layout(d, step_logits[k], dtype, ld_elems);
+            if (st != CD_OK) return st;
+        }
+    DeviceGuard guard(d->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* s = nullptr;
+    st = get_scratch(d, stream, B, true, &s);
+    if (st != CD_OK) return st;
+    st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream);
+    if (st != CD_OK) return st;
+    if (!d->start_accepting)
+        for (int k = 0; k < max_steps; ++k) {
+            st = enqueue_loop_step(d, s, step_logits[k], dtype, ld_elems, B, k, max_steps, tokens_out, len_out,
+                                   final_state_out, sum_logprob_out, done_out, stream);
+            if (st != CD_OK) return st;
+        }
+    return check_sticky_errors(s, stream);
+}
+
+cd_status cd_decode_loop_host(const cd_dfa_t* d, const void* const* step_logits_host, cd_dtype dtype,
+                              int64_t ld_elems, int32_t B, int32_t max_steps, int32_t* tokens_out, int32_t* len_out,
+                              int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out,
+                              void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (B < 0 || max_steps < 0) return fail(CD_ERR_ARG, "B / max_steps < 0");
+    cd_status st = check_dtype(dtype);
+    if (st != CD_OK) return st;
+    if (B == 0) return CD_OK;
+    if (!len_out || !final_state_out || !sum_logprob_out || !done_out || (max_steps > 0 && !tokens_out))
+        return fail(CD_ERR_ARG, "NULL output pointer");
+    if (max_steps > 0 && !step_logits_host) return fail(CD_ERR_ARG, "step_logits_host is NULL");
+    const long long sz = dtype == CD_BF16 ? 2 : 4;
+    if (ld_elems < d->dev.V) return fail(CD_ERR_ARG, "ld_elems < V");
+    if ((ld_elems * sz) % 16 != 0) return fail(CD_ERR_ARG, "row stride is not a multiple of 16 bytes");
+    for (int k = 0; k < max_steps; ++k)
+        if (!step_logits_host[k]) return fail(CD_ERR_ARG, "step_logits_host[%d] is NULL", k);
+
+    DeviceGuard guard(d->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* s = nullptr;
+    st = get_scratch(d, stream, B, true, &s);
+    if (st != CD_OK) return st;
+
+    // staging + device copies of the outputs, kept in the scratch area
+    const size_t step_bytes = (size_t)B * (size_t)ld_elems * (size_t)sz;
+    if (s->stage_bytes < step_bytes) {
+        CU(cudaStreamSynchronize(stream));
+        for (int i = 0; i < 2; ++i) { cudaFree(s->stage[i]); s->stage[i] = nullptr; }
+        s->stage_bytes = 0;
+        for (int i = 0; i < 2; ++i) CU(cudaMalloc(&s->stage[i], step_bytes));
+        s->stage_bytes = step_bytes;
+    }
+    const size_t n_tok = (size_t)B * (size_t)(max_steps > 0 ? max_steps : 1);
+    const size_t out_bytes = sizeof(int) * (n_tok + 3 * (size_t)B) + (size_t)B + 64;
+    if (s->out_bytes < out_bytes) {
+        CU(cudaStreamSynchronize(stream));
+        cudaFree(s->out_i32); s->out_i32 = nullptr; s->out_bytes = 0;
+        CU(cudaMalloc(&s->out_i32, out_bytes));
+        s->out_bytes = out_bytes;
+    }
+    if (!s->copy_stream) {
+        CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CU(cudaEventCreateWithFlags(&s->ev_copied[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&s->ev_consumed[i], cudaEventDisableTiming));
+        }
+        CU(cudaMallocHost(&s->h_pinned, sizeof(int) * 4));
+    }
+    int* d_tokens = s->out_i32;
+    int* d_len = d_tokens + n_tok;
+    int* d_fs = d_len + B;
+    float* d_slp = reinterpret_cast<float*>(d_fs + B);
+    uint8_t* d_done = reinterpret_cast<uint8_t*>(d_slp + B);
+
+    st = launch_loop_init(d, s, B, max_steps, d_tokens, d_len, d_fs, d_slp, d_done, stream);
+    if (st != CD_OK) return st;
+    if (!d->start_accepting && max_steps > 0) {
+        // copy of step k+1 (copy stream) overlaps the kernels of step k (compute stream)
+        CU(cudaEventRecord(s->ev_consumed[0], stream));  // staging free from here on
+        CU(cudaEventRecord(s->ev_consumed[1], stream));
+        CU(cudaStreamWaitEvent(s->copy_stream, s->ev_consumed[0], 0));
+        CU(cudaMemcpyAsync(s->stage[0], step_logits_host[0], step_bytes, cudaMemcpyHostToDevice, s->copy_stream));
+        CU(cudaEventRecord(s->ev_copied[0], s->copy_stream));
+        for (int k = 0; k < max_steps; ++k) {
+            const int cur = k & 1, nxt = cur ^ 1;
+            if (k + 1 < max_steps) {
+                CU(cudaStreamWaitEvent(s->copy_stream, s->ev_consumed[nxt], 0));
+                CU(cudaMemcpyAsync(s->stage[nxt], step_logits_host[k + 1], step_bytes, cudaMemcpyHostToDevice,
+                                   s->copy_stream));
+                CU(cudaEventRecord(s->ev_copied[nxt], s->copy_stream));
+            }
+            CU(cudaStreamWaitEvent(stream, s->ev_copied[cur], 0));
+            st = enqueue_loop_step(d, s, s->stage[cur], dtype, ld_elems, B, k, max_steps, d_tokens, d_len, d_fs, d_slp,
+                                   d_done, stream);
+            if (st != CD_OK) return st;
+            CU(cudaEventRecord(s->ev_consumed[cur], stream));
+            // early exit of the host loop: stop copying once nothing is active
+            CU(cudaMemcpyAsync(s->h_pinned, s->n_active + nxt, sizeof(int), cudaMemcpyDeviceToHost, stream));
+            CU(cudaStreamSynchronize(stream));
+            if (s->h_pinned[0] == 0) break;
+        }
+        CU(cudaStreamSynchronize(s->copy_stream));
+    }
+    if (max_steps > 0)
+        CU(cudaMemcpyAsync(tokens_out, d_tokens, sizeof(int) * (size_t)B * max_steps, cudaMemcpyDeviceToHost, stream));
+    CU(cudaMemcpyAsync(len_out, d_len, sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, stream));
+    CU(cudaMemcpyAsync(final_state_out, d_fs, sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, stream));
+    CU(cudaMemcpyAsync(sum_logprob_out, d_slp, sizeof(float) * (size_t)B, cudaMemcpyDeviceToHost, stream));
+    CU(cudaMemcpyAsync(done_out, d_done, (size_t)B, cudaMemcpyDeviceToHost, stream));
+    return check_sticky_errors(s, stream);
+}
+
+}  // extern "C"

@@ -1,0 +1,154 @@
+// cd_common.cuh -- device-side structs and sm_100a PTX helpers shared by the kernels.
+// Part of the product path (never included by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace cd {
+
+constexpr unsigned FULL = 0xFFFFFFFFu;
+constexpr int DT_F32 = 0;
+constexpr int DT_BF16 = 1;
+
+// Device image of a compiled automaton.
+struct DfaDev {
+    int V;                     // vocabulary size
+    int S;                     // number of states
+    int W;                     // ceil(V / 32) mask words that carry bits
+    int Wpad;                  // mask row stride in words, multiple of 4 (16 B rows), pad = 0
+    const uint32_t* mask;      // [S][Wpad], LSB-first: token t <-> bit (t & 31) of word (t >> 5)
+    const long long* row_ptr;  // [S + 1]
+    const int* tok;            // [nnz] strictly increasing inside a state
+    const int* next;           // [nnz]
+    const uint8_t* accepting;  // [S]
+};
+
+// ---------------------------------------------------------------- PTX helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+
+__device__ __forceinline__ void fence_mbar_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+
+__device__ __forceinline__ void fence_proxy_async_smem() {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes)
+                 : "memory");
+}
+
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t"
+        "}" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+
+// 1-D bulk async copy global -> shared (TMA engine, SASS UBLKCP), completion on an mbarrier.
+// dst, src 16-byte aligned; bytes a positive multiple of 16.
+__device__ __forceinline__ void bulk_g2s_hint(uint32_t dst, const void* src, uint32_t bytes,
+                                              uint32_t bar, uint64_t policy) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint "
+        "[%0], [%1], %2, [%3], %4;" ::"r"(dst),
+        "l"(src), "r"(bytes), "r"(bar), "l"(policy)
+        : "memory");
+}
+
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+        "l"(src), "r"(bytes), "r"(bar)
+        : "memory");
+}
+
+// ---------------------------------------------------------------- online softmax pieces
+// (m, s, idx): running masked maximum, sum of exp(x - m) over the allowed elements seen so
+// far, lowest token id attaining m.  Elements are presented in ascending token id per lane,
+// so "replace on strictly greater" keeps the lowest id (north_star: ties -> lowest token id).
+__device__ __forceinline__ void online_update(float& m, float& s, int& idx, float x, int t) {
+    if (x > m) {
+        s = s * __expf(m - x) + 1.0f;  // m = -inf: exp(-inf) = 0
+        m = x;
+        idx = t;
+    } else if (x > -INFINITY) {  // x = -inf contributes exactly 0 (and m may still be -inf)
+        s += __expf(x - m);
+    }
+}
+
+// Merge two partial results; equal maxima keep the lower token id whatever the order.
+__device__ __forceinline__ void online_combine(float& m, float& s, int& idx, float m2, float s2, int i2) {
+    const bool take2 = (m2 > m) || (m2 == m && i2 < idx);
+    const float mw = take2 ? m2 : m, ml = take2 ? m : m2;
+    const float sw = take2 ? s2 : s, sl = take2 ? s : s2;
+    const float f = (ml == -INFINITY) ? 0.0f : __expf(ml - mw);
+    s = fmaf(sl, f, sw);
+    m = mw;
+    idx = take2 ? i2 : idx;
+}
+
+__device__ __forceinline__ void warp_combine(float& m, float& s, int& idx) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const float m2 = __shfl_xor_sync(FULL, m, o);
+        const float s2 = __shfl_xor_sync(FULL, s, o);
+        const int i2 = __shfl_xor_sync(FULL, idx, o);
+        online_combine(m, s, idx, m2, s2, i2);
+    }
+}
+
+// ---------------------------------------------------------------- CSR transition lookup
+// Warp-cooperative 32-ary search of `token` in the sorted CSR row tok[lo, hi): every round the
+// 32 lanes probe 32 split points, so a 5,243-entry row (configs[3]) takes 2 rounds + 1 final
+// compare instead of 13 dependent probes.  Returns the position or -1.  All lanes return the
+// same value.
+__device__ __forceinline__ long long warp_csr_find(const int* __restrict__ tok, long long lo,
+                                                   long long hi, int token, int lane) {
+    while (hi - lo > 32) {
+        const long long step = (hi - lo + 31) >> 5;
+        const long long q = lo + (long long)lane * step;
+        const bool le = (q < hi) && (__ldg(tok + q) <= token);
+        const unsigned b = __ballot_sync(FULL, le);
+        if (b == 0) return -1;  // token below the first entry
+        const int c = __popc(b);
+        lo = lo + (long long)(c - 1) * step;
+        hi = (lo + step < hi) ? lo + step : hi;
+    }
+    const long long q = lo + lane;
+    const bool eq = (q < hi) && (__ldg(tok + q) == token);
+    const unsigned b = __ballot_sync(FULL, eq);
+    return b ? lo + (__ffs(b) - 1) : -1;
+}
+
+}  // namespace cd

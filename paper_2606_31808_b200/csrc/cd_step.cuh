@@ -1,0 +1,308 @@
+// cd_step.cuh -- the fused constrained step (include/cd.h cd_step).
+//
+// Design (B200-first; the paper gives no kernel):
+//   * The step is one streaming pass over the logits, so it is HBM-bound: the job is to keep
+//     enough bytes in flight and to waste no issue slots.  Every WARP owns a private ring of
+//     STAGES shared-memory slots that it fills itself with 1-D bulk async copies (TMA engine,
+//     cp.async.bulk -> SASS UBLKCP) completing on per-slot mbarriers: a 4 KiB logits tile
+//     and the matching piece of the state's allowed-token bitmask land together.  No register
+//     staging, no block-wide barriers, WARPS*STAGES*4 KiB in flight per SM.
+//   * Work unit = (active slot, part of the row).  Units are handed out by one global atomic
+//     counter (dynamic balance across the 148 SMs; the two dies do not run at the same speed),
+//     the number of tiles per unit is derived on the device from the number of active rows, so
+//     the same launch shape serves a full batch and the few-rows tail of an early-exit loop
+//     without any host read of the active count.
+//   * Per tile a lane walks the set bits of its mask words and updates an online
+//     (max, sum-exp, argmax) triple; only allowed elements cost arithmetic.
+//   * Unit results of a row are merged by whichever warp finishes the row's last unit (ticket
+//     counter per slot); that warp also does the CSR transition (32-ary warp search), the
+//     accept test and the output writes, while the other warps keep streaming.
+//   * Tickets and the work counter are self-resetting, so a launch needs no memset.
+#pragma once
+#include "cd_common.cuh"
+
+namespace cd {
+
+constexpr int TILE_BYTES = 4096;      // logits bytes per tile
+constexpr int MASK_SLOT_BYTES = 256;  // bf16: 2048 tokens -> 256 B of mask; fp32: 1024 -> 128 B
+constexpr int TPU_MAX = 16;           // at most 16 tiles (64 KiB) per unit
+constexpr int UNITS_PER_WARP = 4;     // aim for >= 4 units per warp when rows are few
+
+constexpr int FLAG_FIRST = 1;   // first tile of its unit: reset the lane accumulators
+constexpr int FLAG_LAST = 2;    // last tile of its unit: reduce and publish
+constexpr int FLAG_ACCEPT = 4;  // pseudo tile of a slot whose state already accepts (no copy)
+constexpr int FLAG_BADSTATE = 8;
+
+struct StepArgs {
+    DfaDev dfa;
+    const unsigned char* logits;
+    long long ld_bytes;
+    const int* row_map;
+    int* state;
+    int n;
+    const int* n_dev;  // if non-null the active count is read from the device
+    int* token_out;
+    float* logprob_out;
+    float* lse_out;
+    uint8_t* done_out;
+    // scratch (per handle+stream)
+    int4* partials;  // [units] {m bits, s bits, idx, -}
+    int* tickets;    // [rows], zero between launches
+    int* ctrs;       // [0] work counter, [1] finished warps, [2] sticky error count
+};
+
+struct __align__(16) TileMeta {
+    int slot;
+    int tile;   // tile index inside the row
+    int flags;  // FLAG_* | part << 8
+    int st;     // automaton state of the slot
+};
+
+template <int STAGES>
+struct __align__(128) WarpRing {
+    unsigned char logits[STAGES][TILE_BYTES];
+    unsigned char mask[STAGES][MASK_SLOT_BYTES];
+    TileMeta meta[STAGES];
+    unsigned long long bar[STAGES];
+};
+
+// tiles per unit for n active rows (host mirrors this in cd_api.cu: step_units_cap)
+__host__ __device__ inline int tiles_per_unit(long long n, int tiles_per_row, long long total_warps) {
+    long long t = (n * tiles_per_row + total_warps * UNITS_PER_WARP - 1) / (total_warps * UNITS_PER_WARP);
+    if (t < 1) t = 1;
+    if (t > TPU_MAX) t = TPU_MAX;
+    return (int)t;
+}
+
+template <int DT>
+__device__ __forceinline__ float tile_elem(const unsigned char* tile, int e) {
+    float x;
+    if (DT == DT_BF16) {
+        x = __uint_as_float(((uint32_t) reinterpret_cast<const uint16_t*>(tile)[e]) << 16);
+    } else {
+        x = reinterpret_cast<const float*>(tile)[e];
+    }
+    return fmaxf(x, -INFINITY);  // NaN -> -inf
+}
+
+// Row finished: (m, s, idx) is the merged result of all its units.  Warp-uniform.
+__device__ __forceinline__ void finalize_row(const StepArgs& a, int slot, int st, float m, float s,
+                                             int idx, int lane) {
+    const long long lo = __ldg(a.dfa.row_ptr + st), hi = __ldg(a.dfa.row_ptr + st + 1);
+    int token;
+    float lp, lse;
+    if (m == -INFINITY) {  // every allowed logit is -inf: lowest allowed id (G6)
+        token = __ldg(a.dfa.tok + lo);
+        lp = -INFINITY;
+        lse = -INFINITY;
+    } else {
+        token = idx;
+        const float L = logf(s);
+        lp = -L;  // log p(t*) = x_t* - lse = -log(sum); never m - lse (cancellation)
+        lse = m + L;
+    }
+    const long long j = warp_csr_find(a.dfa.tok, lo, hi, token, lane);
+    if (lane == 0) {
+        int ns = st;
+        if (j >= 0) {
+            ns = __ldg(a.dfa.next + j);
+        } else {
+            atomicAdd(a.ctrs + 2, 1);
+        }
+        a.state[slot] = ns;
+        a.token_out[slot] = token;
+        a.logprob_out[slot] = lp;
+        if (a.lse_out) a.lse_out[slot] = lse;
+        a.done_out[slot] = __ldg(a.dfa.accepting + ns) ? 1 : 0;
+    }
+}
+
+template <int DT, int WARPS, int STAGES>
+__global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
+    constexpr int SZ = (DT == DT_BF16) ? 2 : 4;
+    constexpr int TILE_TOK = TILE_BYTES / SZ;
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    WarpRing<STAGES>& ring = reinterpret_cast<WarpRing<STAGES>*>(smem_raw)[warp];
+
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) mbar_init(smem_u32(&ring.bar[s]), 1);
+        fence_mbar_init();
+    }
+    __syncwarp();
+
+    const int n = a.n_dev ? __ldg(a.n_dev) : a.n;
+    const int V = a.dfa.V;
+    const int tiles_per_row = (V + TILE_TOK - 1) / TILE_TOK;
+    const long long total_warps = (long long)gridDim.x * WARPS;
+    const int tpu = tiles_per_unit(n, tiles_per_row, total_warps);
+    const int P = (tiles_per_row + tpu - 1) / tpu;  // units per row
+    const int total_units = n * P;
+    const uint64_t pol_stream = l2_policy_evict_first();
+
+    // ---------------- issue side (warp-uniform state)
+    int next_u_l0 = 0;  // prefetched unit id, valid in lane 0
+    if (lane == 0) next_u_l0 = atomicAdd(a.ctrs + 0, 1);
+    bool exhausted = false;
+    int iss_tile = 0, iss_end = 0, iss_first = 0;
+    int iss_slot = 0, iss_part = 0, iss_st = 0;
+    const unsigned char* iss_row = nullptr;
+    const unsigned char* iss_mask = nullptr;
+    unsigned issued = 0, consumed = 0;
+
+    auto issue_one = [&]() -> bool {
+        if (iss_tile >= iss_end) {
+            if (exhausted) return false;
+            const int u = __shfl_sync(FULL, next_u_l0, 0);
+            if (u >= total_units) {
+                exhausted = true;
+                return false;
+            }
+            if (lane == 0) next_u_l0 = atomicAdd(a.ctrs + 0, 1);
+            iss_slot = u / P;
+            iss_part = u - iss_slot * P;
+            iss_st = a.state[iss_slot];  // updated only after every unit of the slot has arrived
+            const bool bad = (iss_st < 0) || (iss_st >= a.dfa.S);
+            const bool acc = !bad && (__ldg(a.dfa.accepting + iss_st) != 0);
+            if (bad || acc) {
+                const int stage = issued % STAGES;
+                if (lane == 0) {
+                    ring.meta[stage] = TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (iss_part << 8), iss_st};
+                    mbar_arrive(smem_u32(&ring.bar[stage]));
+                }
+                ++issued;
+                iss_tile = iss_end = 0;
+                return true;
+            }
+            const long long r = a.row_map ? (long long)__ldg(a.row_map + iss_slot) : (long long)iss_slot;
+            iss_row = a.logits + r * a.ld_bytes;
+            iss_mask = reinterpret_cast<const unsigned char*>(a.dfa.mask + (long long)iss_st * a.dfa.Wpad);
+            iss_first = iss_part * tpu;
+            iss_tile = iss_first;
+            iss_end = min(iss_first + tpu, tiles_per_row);
+        }
+        const int stage = issued % STAGES;
+        const int t0 = iss_tile * TILE_TOK;
+        const int ntok = min(TILE_TOK, V - t0);
+        const uint32_t bytes = (uint32_t)ntok * SZ;
+        const uint32_t bulk = bytes & ~15u;
+        const uint32_t mbytes = (uint32_t)(((ntok + 31) >> 5) * 4 + 15) & ~15u;
+        const unsigned char* src = iss_row + (long long)iss_tile * TILE_BYTES;
+        if (bulk < bytes) {  // < 16 trailing bytes (V*SZ not a multiple of 16): plain loads
+            const int e = (int)(bulk / SZ) + lane;
+            if (e < ntok) {
+                if (DT == DT_BF16)
+                    reinterpret_cast<uint16_t*>(ring.logits[stage])[e] = reinterpret_cast<const uint16_t*>(src)[e];
+                else
+                    reinterpret_cast<float*>(ring.logits[stage])[e] = reinterpret_cast<const float*>(src)[e];
+            }
+        }
+        if (lane == 0) {
+            int fl = (iss_part << 8);
+            if (iss_tile == iss_first) fl |= FLAG_FIRST;
+            if (iss_tile + 1 == iss_end) fl |= FLAG_LAST;
+            ring.meta[stage] = TileMeta{iss_slot, iss_tile, fl, iss_st};
+            const uint32_t bar = smem_u32(&ring.bar[stage]);
+            mbar_arrive_expect_tx(bar, bulk + mbytes);
+            if (bulk) bulk_g2s_hint(smem_u32(ring.logits[stage]), src, bulk, bar, pol_stream);
+            bulk_g2s(smem_u32(ring.mask[stage]), iss_mask + (long long)iss_tile * (TILE_TOK / 8), mbytes, bar);
+        }
+        ++issued;
+        ++iss_tile;
+        return true;
+    };
+
+#pragma unroll 1
+    for (int k = 0; k < STAGES; ++k)
+        if (!issue_one()) break;
+
+    // ---------------- consume side
+    float m = -INFINITY, s = 0.0f;
+    int idx = 0x7FFFFFFF;
+
+#pragma unroll 1
+    while (consumed < issued) {
+        const int stage = consumed % STAGES;
+        mbar_wait(smem_u32(&ring.bar[stage]), (consumed / STAGES) & 1);
+        __syncwarp();
+        const TileMeta mt = ring.meta[stage];
+        const int part = mt.flags >> 8;
+
+        if (mt.flags & (FLAG_ACCEPT | FLAG_BADSTATE)) {
+            // accepted rows never advance
+            if (part == 0 && lane == 0) {
+                a.token_out[mt.slot] = -1;
+                a.logprob_out[mt.slot] = 0.0f;
+                if (a.lse_out) a.lse_out[mt.slot] = 0.0f;
+                a.done_out[mt.slot] = 1;
+                if (mt.flags & FLAG_BADSTATE) atomicAdd(a.ctrs + 2, 1);
+            }
+        } else {
+            if (mt.flags & FLAG_FIRST) {
+                m = -INFINITY;
+                s = 0.0f;
+                idx = 0x7FFFFFFF;
+            }
+            const int t0 = mt.tile * TILE_TOK;
+            const int nwords = (min(TILE_TOK, V - t0) + 31) >> 5;
+            const uint32_t* mw = reinterpret_cast<const uint32_t*>(ring.mask[stage]);
+            const unsigned char* tile = ring.logits[stage];
+#pragma unroll
+            for (int w = lane; w < TILE_TOK / 32; w += 32) {
+                uint32_t bits = (w < nwords) ? mw[w] : 0u;
+                while (bits) {
+                    const int b = __ffs(bits) - 1;
+                    bits &= bits - 1;
+                    const int e = w * 32 + b;
+                    online_update(m, s, idx, tile_elem<DT>(tile, e), t0 + e);
+                }
+            }
+            if (mt.flags & FLAG_LAST) {
+                float rm = m, rs = s;
+                int ri = idx;
+                warp_combine(rm, rs, ri);
+                if (P == 1) {
+                    finalize_row(a, mt.slot, mt.st, rm, rs, ri, lane);
+                } else {
+                    int t = 0;
+                    if (lane == 0) {
+                        a.partials[(long long)mt.slot * P + part] =
+                            make_int4(__float_as_int(rm), __float_as_int(rs), ri, 0);
+                        __threadfence();
+                        t = atomicAdd(a.tickets + mt.slot, 1);
+                    }
+                    t = __shfl_sync(FULL, t, 0);
+                    if (t == P - 1) {  // this warp completed the row: merge the P unit results
+                        if (lane == 0) a.tickets[mt.slot] = 0;
+                        __threadfence();
+                        float cm = -INFINITY, cs = 0.0f;
+                        int ci = 0x7FFFFFFF;
+                        for (int q = lane; q < P; q += 32) {
+                            const int4 v = __ldcg(a.partials + (long long)mt.slot * P + q);
+                            online_combine(cm, cs, ci, __int_as_float(v.x), __int_as_float(v.y), v.z);
+                        }
+                        warp_combine(cm, cs, ci);
+                        finalize_row(a, mt.slot, mt.st, cm, cs, ci, lane);
+                    }
+                }
+            }
+        }
+        ++consumed;
+        __syncwarp();
+        issue_one();
+    }
+
+    // ---------------- self-reset of the counters by the last warp of the grid
+    if (lane == 0) {
+        __threadfence();
+        const int d = atomicAdd(a.ctrs + 1, 1);
+        if (d == (int)total_warps - 1) {
+            a.ctrs[0] = 0;
+            a.ctrs[1] = 0;
+        }
+    }
+}
+
+}  // namespace cd

@@ -1,0 +1,453 @@
+"""Parity of the CUDA path (through the C ABI) with the CPU oracle, element by
+element on the same seeded inputs.
+
+Bar (BASELINE.json north_star): bit-exact token ids, next states, done flags
+and compacted row order; log-probs / lse within 1e-5 relative with fp32
+accumulation, read as abs(gpu - ref) <= 1e-5 * max(1, |ref|) (SURVEY 8(c) G9:
+-log(sum) is ill-conditioned relative to itself near 0; DESIGN.md derives the
+bound from the arithmetic).
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import workloads as wl
+from golden_util import read_decode
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def cd():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2606_31808_b200 as m
+
+    m.lib()
+    return m
+
+
+def dev_dfa(cd, aut):
+    return cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device="cuda:0")
+
+
+def close(gpu, ref, tol=TOL):
+    gpu = np.asarray(gpu, np.float64)
+    ref = np.asarray(ref, np.float64)
+    both_inf = np.isneginf(gpu) & np.isneginf(ref)
+    err = np.abs(np.where(both_inf, 0.0, gpu - ref))
+    bound = tol * np.maximum(1.0, np.abs(np.where(both_inf, 0.0, ref)))
+    return bool(np.all(err <= bound)), float(np.max(err / bound)) if err.size else 0.0
+
+
+def check_step(cd, oracle, aut, dfa, x_dev, states, row_map=None):
+    """One cd_step call against oracle.step on the same bytes."""
+    st_dev = torch.tensor(states, dtype=torch.int32, device="cuda:0")
+    rm_dev = None if row_map is None else torch.tensor(row_map, dtype=torch.int32, device="cuda:0")
+    tok, lp, lse, done = cd.step(dfa, x_dev, st_dev, row_map=rm_dev)
+    torch.cuda.synchronize()
+    o_tok, o_lp, o_lse, o_done, o_st = oracle.step(aut, x_dev.cpu(), states, row_map=row_map)
+    assert tok.cpu().numpy().tolist() == o_tok.tolist()
+    assert st_dev.cpu().numpy().tolist() == o_st.tolist()
+    assert done.cpu().numpy().tolist() == o_done.tolist()
+    ok, worst = close(lp.cpu().numpy(), o_lp)
+    assert ok, f"logprob off by {worst:.2f}x the bound"
+    ok, worst = close(lse.cpu().numpy(), o_lse)
+    assert ok, f"lse off by {worst:.2f}x the bound"
+    return tok, lp, lse, done
+
+
+def live_states(aut, n, stride=7):
+    live = [s for s in range(aut.S) if not aut.accepting[s]]
+    return [live[(stride * i) % len(live)] for i in range(n)]
+
+
+# ------------------------------------------------------------------ the step
+@pytest.mark.parametrize("dtype", [torch.float32, torch.bfloat16])
+@pytest.mark.parametrize(
+    "V,S,density,n",
+    [
+        (64, 5, 0.3, 9),          # one partial tile
+        (37, 4, 0.3, 11),         # row bytes not a multiple of 16: scalar tail path
+        (5001, 9, 0.03, 50),      # several tiles + 1-element tail after the bulk copy
+        (1024, 8, 0.05, 33),      # exactly one fp32 tile
+        (2048, 8, 0.05, 33),      # exactly one bf16 tile
+        (5000, 12, 0.02, 70),     # several tiles + ragged tail, V % 32 != 0
+        (40000, 16, 0.02, 301),   # many tiles, ragged
+        (262144, 6, 0.005, 24),   # full vocabulary, few rows (row split over many units)
+    ],
+)
+def test_step_matches_oracle_random_dfa(cd, oracle, dtype, V, S, density, n):
+    aut = wl.make_random_dfa(seed=V + S, V=V, S=S, density=density, accept_frac=0.25, device="cuda:0")
+    dfa = dev_dfa(cd, aut)
+    ld = (V + 7) // 8 * 8
+    x = wl.make_logits(V, 0, n, V, 2.0, dtype, device="cuda:0", ld=ld)
+    states = live_states(aut, n)
+    check_step(cd, oracle, aut, dfa, x, states)
+    # mixed with already-accepted slots (never advance) and a row_map permutation
+    acc = [s for s in range(S) if aut.accepting[s]]
+    if acc:
+        states2 = [acc[i % len(acc)] if i % 3 == 0 else s for i, s in enumerate(states)]
+        perm = np.random.default_rng(n).permutation(n).astype(np.int32)
+        check_step(cd, oracle, aut, dfa, x, states2, row_map=perm)
+    dfa.close()
+
+
+@pytest.mark.parametrize("dtype", [torch.float32, torch.bfloat16])
+def test_step_dense_masks(cd, oracle, dtype):
+    """All tokens allowed (reduces to textbook log-softmax/argmax) and 50 % density."""
+    for V, density in ((4096, 1.0), (10000, 1.0), (10000, 0.5)):
+        aut = wl.make_random_dfa(seed=17, V=V, S=3, density=density, accept_frac=0.0, device="cuda:0")
+        dfa = dev_dfa(cd, aut)
+        ld = (V + 7) // 8 * 8
+        x = wl.make_logits(3, 0, 40, V, 3.0, dtype, device="cuda:0", ld=ld)
+        states = [i % 3 for i in range(40)]
+        tok, lp, lse, _ = check_step(cd, oracle, aut, dfa, x, states)
+        if density == 1.0:  # independent library pin on the GPU result itself
+            xd = x[:, :V].double()
+            ref = torch.logsumexp(xd, dim=1)
+            assert torch.allclose(lse.double(), ref, rtol=0, atol=1e-5 * float(ref.abs().max().clamp(min=1)))
+            m = xd.max(dim=1).values
+            first = torch.stack([torch.nonzero(xd[i] == m[i])[0, 0] for i in range(40)])
+            assert tok.cpu().tolist() == first.cpu().tolist()
+        dfa.close()
+
+
+def _subset_aut(V, toks):
+    toks = sorted(toks)
+    return wl.Automaton(
+        V=V, S=2, start=0,
+        row_ptr=torch.tensor([0, len(toks), len(toks)], dtype=torch.int64),
+        tok=torch.tensor(toks, dtype=torch.int32),
+        next=torch.ones(len(toks), dtype=torch.int32),
+        accepting=torch.tensor([0, 1], dtype=torch.uint8),
+    )
+
+
+@pytest.mark.parametrize("dtype", [torch.float32, torch.bfloat16])
+def test_planted_ties_across_work_boundaries(cd, oracle, dtype):
+    """Equal maxima at lane / word / tile / unit / row boundaries: lowest id wins."""
+    V = 262144
+    tile = 1024 if dtype == torch.float32 else 2048
+    groups = [
+        [31, 32], [63, 64, 65], [tile - 1, tile], [2 * tile - 1, 2 * tile, 2 * tile + 1],
+        [16 * tile - 1, 16 * tile], [0, V - 1], [V // 2 - 1, V // 2, V - 1], [5, 100000, 200000, 262143],
+        [tile * 7 + 31, tile * 8 + 0, tile * 9 + 33],
+    ]
+    n = len(groups) * 2
+    g = torch.Generator(device="cuda:0").manual_seed(1)
+    x = (torch.randn(n, V, generator=g, device="cuda:0") * 2.0).clamp_(max=5.0)
+    for i, ids in enumerate(groups):
+        x[2 * i, ids] = 6.0
+        x[2 * i + 1, ids] = 6.0
+    x = x.to(dtype)
+    all_ones = _subset_aut(V, range(V))
+    dfa = dev_dfa(cd, all_ones)
+    tok, _, _, _ = check_step(cd, oracle, all_ones, dfa, x, [0] * n)
+    assert tok.cpu().tolist() == [ids[0] for ids in groups for _ in (0, 1)]
+    dfa.close()
+    # the same with a sparse allowed set that drops the lowest planted id of each group
+    allowed = set(range(0, V, 97))
+    for ids in groups:
+        allowed.update(ids[1:])
+        allowed.discard(ids[0])
+    sparse = _subset_aut(V, allowed)
+    dfa = dev_dfa(cd, sparse)
+    tok, _, _, _ = check_step(cd, oracle, sparse, dfa, x, [0] * n)
+    assert tok.cpu().tolist() == [ids[1] for ids in groups for _ in (0, 1)]
+    dfa.close()
+
+
+def test_closed_forms_on_gpu(cd, oracle):
+    V = 8192
+    aut = _subset_aut(V, [9, 4100])
+    dfa = dev_dfa(cd, aut)
+    pairs = [(0.5, -1.25), (-3.0, -3.0), (10.0, 9.0), (-20.0, 1.0), (100.0, 80.0), (0.0, 0.0)]
+    x = torch.full((len(pairs), V), 50.0, device="cuda:0")
+    for i, (a, b) in enumerate(pairs):
+        x[i, 9], x[i, 4100] = a, b
+    tok, lp, lse, done = check_step(cd, oracle, aut, dfa, x, [0] * len(pairs))
+    for i, (a, b) in enumerate(pairs):
+        assert int(tok[i]) == (9 if a >= b else 4100)
+        want = -math.log1p(math.exp(-abs(a - b)))
+        assert abs(float(lp[i]) - want) <= TOL
+    dfa.close()
+    one = _subset_aut(V, [4000])
+    dfa = dev_dfa(cd, one)
+    x = torch.randn(5, V, device="cuda:0")
+    tok, lp, lse, _ = check_step(cd, oracle, one, dfa, x, [0] * 5)
+    assert tok.cpu().tolist() == [4000] * 5 and lp.cpu().tolist() == [0.0] * 5
+    assert torch.equal(lse, x[:, 4000])
+    dfa.close()
+
+
+@pytest.mark.parametrize("dtype", [torch.float32, torch.bfloat16])
+def test_special_values(cd, oracle, dtype):
+    V = 4096
+    ids = [4, 800, 1500, 4095]
+    aut = _subset_aut(V, ids)
+    dfa = dev_dfa(cd, aut)
+    ninf, nan = -float("inf"), float("nan")
+    rows = [
+        [nan, 1.0, nan, 1.0],       # NaN read as -inf
+        [ninf, ninf, ninf, ninf],   # all -inf: lowest allowed id, logprob = lse = -inf
+        [nan, nan, nan, nan],       # all NaN: same
+        [ninf, 2.0, 2.0, ninf],
+        [-0.0, 0.0, -5.0, -5.0],    # signed zeros tie
+        [3e38, 3e38, -3e38, 0.0],
+    ]
+    x = torch.zeros((len(rows), V), device="cuda:0")
+    for i, r in enumerate(rows):
+        x[i, ids] = torch.tensor(r, device="cuda:0")
+    x = x.to(dtype)
+    tok, lp, lse, _ = check_step(cd, oracle, aut, dfa, x, [0] * len(rows))
+    assert tok.cpu().tolist()[:5] == [800, 4, 4, 800, 4]
+    assert float(lp[1]) == ninf and float(lse[1]) == ninf
+    # poisoned complement: disallowed logits must never matter
+    base = [t.clone() for t in cd.step(dfa, x, torch.zeros(len(rows), dtype=torch.int32, device="cuda:0"))]
+    for poison in (1e30, float("inf"), nan, ninf):
+        y = x.clone().float()
+        dis = torch.ones(V, dtype=torch.bool, device="cuda:0")
+        dis[ids] = False
+        y[:, dis] = poison
+        out = cd.step(dfa, y.to(dtype), torch.zeros(len(rows), dtype=torch.int32, device="cuda:0"))
+        for a, b in zip(base, out):
+            assert torch.equal(a.view(torch.uint8) if a.dtype != torch.uint8 else a,
+                               b.view(torch.uint8) if b.dtype != torch.uint8 else b)
+    # +inf: only the token is defined (lowest +inf id); parity of the values is unpinned (G6)
+    x2 = torch.zeros((1, V), device="cuda:0")
+    x2[0, 1500] = x2[0, 800] = float("inf")
+    tok2, _, _, _ = cd.step(dfa, x2.to(dtype), torch.zeros(1, dtype=torch.int32, device="cuda:0"))
+    assert int(tok2[0]) == 800
+    dfa.close()
+
+
+def test_step_n_zero_and_argument_errors(cd):
+    aut = _subset_aut(64, [1, 2])
+    dfa = dev_dfa(cd, aut)
+    x = torch.zeros((4, 64), device="cuda:0")
+    st = torch.zeros(0, dtype=torch.int32, device="cuda:0")
+    tok, lp, lse, done = cd.step(dfa, x, st)
+    assert tok.numel() == 0
+    with pytest.raises(cd.CdError) as e:  # ld < V
+        cd.step(dfa, torch.zeros((4, 32), device="cuda:0"), torch.zeros(4, dtype=torch.int32, device="cuda:0"))
+    assert e.value.code == 1
+    with pytest.raises(cd.CdError) as e:  # row stride not a multiple of 16 bytes
+        cd.step(dfa, torch.zeros((4, 66), device="cuda:0"), torch.zeros(4, dtype=torch.int32, device="cuda:0"))
+    assert e.value.code == 1
+    with pytest.raises(cd.CdError) as e:  # misaligned base
+        base = torch.zeros(4 * 64 + 4, device="cuda:0")
+        cd.step(dfa, base[1:1 + 4 * 64].view(4, 64), torch.zeros(4, dtype=torch.int32, device="cuda:0"))
+    assert e.value.code == 1
+    dfa.close()
+
+
+# ------------------------------------------------------------------ transition kernel
+def test_transition_kernel(cd, oracle):
+    aut = wl.make_random_dfa(seed=5, V=50000, S=40, density=0.02, accept_frac=0.2, device="cuda:0")
+    dfa = dev_dfa(cd, aut)
+    rng = np.random.default_rng(0)
+    n = 3000
+    states = rng.integers(0, aut.S, size=n).astype(np.int32)
+    tokens = np.empty(n, np.int32)
+    want_state = np.empty(n, np.int32)
+    rp, tk, nx = aut.row_ptr.numpy(), aut.tok.numpy(), aut.next.numpy()
+    for i, s in enumerate(states):
+        lo, hi = rp[s], rp[s + 1]
+        if i % 5 == 0 or hi == lo:  # token without a transition (or negative): state kept
+            tokens[i] = -1 if i % 10 == 0 else int(rng.integers(0, aut.V))
+            j = lo + np.searchsorted(tk[lo:hi], tokens[i])
+            want_state[i] = nx[j] if (tokens[i] >= 0 and j < hi and tk[j] == tokens[i]) else s
+        else:
+            j = int(rng.integers(lo, hi))
+            tokens[i], want_state[i] = tk[j], nx[j]
+    st = torch.tensor(states, device="cuda:0")
+    done = cd.transition(dfa, torch.tensor(tokens, device="cuda:0"), st)
+    assert st.cpu().numpy().tolist() == want_state.tolist()
+    assert done.cpu().numpy().tolist() == aut.accepting.numpy()[want_state].tolist()
+    dfa.close()
+
+
+# ------------------------------------------------------------------ compaction
+@pytest.mark.parametrize("n", [0, 1, 2, 31, 32, 33, 1000, 1023, 1024, 1025, 4096, 4097, 70000])
+@pytest.mark.parametrize("pattern", ["none", "all", "alt", "rand"])
+def test_compaction_bit_exact(cd, oracle, n, pattern):
+    rng = np.random.default_rng(n + 1)
+    done = {
+        "none": np.zeros(n, np.uint8),
+        "all": np.ones(n, np.uint8),
+        "alt": (np.arange(n) % 2).astype(np.uint8),
+        "rand": (rng.random(n) < 0.3).astype(np.uint8),
+    }[pattern]
+    ids = np.sort(rng.choice(10 * n + 1, size=n, replace=False)).astype(np.int32)
+    st = rng.integers(0, 5000, size=n).astype(np.int32)
+    d = torch.tensor(done, device="cuda:0")
+    ro, so, na = cd.compact(d, torch.tensor(ids, device="cuda:0"), torch.tensor(st, device="cuda:0"))
+    o_ro, o_so, k = oracle.compact(done, ids, st)
+    assert int(na) == k
+    assert ro[:k].cpu().numpy().tolist() == o_ro.tolist()
+    assert so[:k].cpu().numpy().tolist() == o_so.tolist()
+    ro2, _, na2 = cd.compact(d)  # implicit ids
+    assert int(na2) == k and ro2[:k].cpu().numpy().tolist() == [i for i in range(n) if not done[i]]
+
+
+# ------------------------------------------------------------------ the loop
+def check_loop(cd, oracle, aut, logits_dev, max_steps, ref=None, rows=None):
+    dfa = dev_dfa(cd, aut)
+    out = cd.decode_loop(dfa, logits_dev, max_steps=max_steps)
+    if ref is None:
+        ref = oracle.decode_loop(aut, [x.cpu() for x in logits_dev], max_steps=max_steps)
+    sel = slice(None) if rows is None else rows
+    for k in ("tokens", "len", "final_state", "done"):
+        assert np.array_equal(out[k].cpu().numpy()[sel], ref[k]), k
+    g, r = out["sum_logprob"].cpu().numpy().astype(np.float64)[sel], ref["sum_logprob"]
+    bound = TOL * (ref["len"] + np.abs(np.where(np.isinf(r), 0, r)))  # sum of per-step bounds
+    fin = np.isfinite(r)
+    assert np.array_equal(np.isfinite(g), fin)
+    assert np.all(np.abs(g[fin] - r[fin]) <= np.maximum(bound[fin], TOL)), float(np.max(np.abs(g[fin] - r[fin])))
+    dfa.close()
+    return out, ref
+
+
+def test_loop_c0_against_golden(cd, oracle):
+    """BASELINE.json configs[0] exactly as stated; expectation is the stored oracle result."""
+    cfg = wl.CONFIGS["c0"]
+    aut = wl.build_automaton(cfg)
+    logits = wl.build_step_logits(cfg, aut, device="cpu")  # the fixture was made from CPU-generated logits
+    gold = read_decode("c0_decode.txt")
+    out, _ = check_loop(cd, oracle, aut, [x.cuda() for x in logits], cfg.max_steps, ref=gold)
+    labels = {(17, 3), (42,)}
+    for r in range(cfg.B):
+        assert tuple(out["tokens"][r, : int(out["len"][r])].cpu().tolist()) in labels
+
+
+def test_loop_c3_small_against_golden(cd, oracle):
+    cfg = wl.scaled(wl.CONFIGS["c3"], V=4096, B=48, S=64, max_steps=10)
+    aut = wl.build_automaton(cfg)
+    logits = wl.build_step_logits(cfg, aut, device="cpu")
+    check_loop(cd, oracle, aut, [x.cuda() for x in logits], cfg.max_steps, ref=read_decode("c3_small_decode.txt"))
+
+
+def test_loop_accepting_start(cd, oracle):
+    aut = wl.Automaton(V=64, S=1, start=0, row_ptr=torch.tensor([0, 1]), tok=torch.tensor([1], dtype=torch.int32),
+                       next=torch.tensor([0], dtype=torch.int32), accepting=torch.tensor([1], dtype=torch.uint8))
+    check_loop(cd, oracle, aut, [torch.zeros(5, 64, device="cuda:0")] * 3, 3)
+
+
+@pytest.mark.parametrize("name", ["c1", "c2", "c3"])
+def test_loop_full_size_configs(cd, oracle, name):
+    """BASELINE.json configs[1..3] at full size, element by element (the oracle
+    only touches allowed logits, so it finishes in seconds even at V=262144)."""
+    cfg = wl.CONFIGS[name]
+    aut = wl.build_automaton(cfg, device="cuda:0")
+    assert oracle.validate(aut) == 0
+    logits = wl.build_step_logits(cfg, aut, device="cuda:0")
+    out, ref = check_loop(cd, oracle, aut, logits, cfg.max_steps)
+    if aut.labels is not None:  # tries: every decoded history is one of the labels
+        leaf = {tuple(l): aut.leaf_of_label[i] for i, l in enumerate(aut.labels)}
+        toks, ln, fs = out["tokens"].cpu().numpy(), out["len"].cpu().numpy(), out["final_state"].cpu().numpy()
+        for r in range(cfg.B):
+            h = tuple(toks[r, : ln[r]].tolist())
+            assert h in leaf and fs[r] == leaf[h]
+        assert bool(out["done"].all())
+    else:  # statistics sanity: survival ~ (1 - accept_frac)^k
+        acc = float(aut.accepting.float().mean())
+        hist = ref["n_active_hist"]
+        for k in range(0, cfg.max_steps, 4):
+            expect = cfg.B * (1 - acc) ** k
+            assert abs(hist[k] - expect) < 6 * math.sqrt(cfg.B) + 0.15 * expect
+
+
+def test_loop_c4_batch_sampled_rows(cd, oracle):
+    """BASELINE.json configs[4], one full batch (B=4096, S=4096, 16 steps, 32 GiB of
+    logits) in the launch configuration bench.py times.  The oracle checks a
+    sample of rows one by one (rows are independent: a row's result does not
+    depend on batch composition), plus size-independent
+    properties on every row."""
+    cfg = wl.CONFIGS["c4"]
+    free, _ = torch.cuda.mem_get_info()
+    if free < 40 * 2**30:
+        pytest.skip("needs ~34 GiB of device memory")
+    aut = wl.build_automaton(cfg, device="cuda:0")
+    logits = wl.build_step_logits(cfg, aut, device="cuda:0")
+    dfa = dev_dfa(cd, aut)
+    out = cd.decode_loop(dfa, logits, max_steps=cfg.max_steps)
+    toks, ln = out["tokens"].cpu().numpy(), out["len"].cpu().numpy()
+    fs, dn = out["final_state"].cpu().numpy(), out["done"].cpu().numpy()
+    slp = out["sum_logprob"].cpu().numpy().astype(np.float64)
+    # properties on every row: replay through the host CSR
+    rp, tk, nx, acc = aut.row_ptr.numpy(), aut.tok.numpy(), aut.next.numpy(), aut.accepting.numpy()
+    for r in range(cfg.B):
+        s = aut.start
+        for k in range(ln[r]):
+            assert not acc[s]
+            lo, hi = rp[s], rp[s + 1]
+            j = lo + np.searchsorted(tk[lo:hi], toks[r, k])
+            assert j < hi and tk[j] == toks[r, k]  # chosen token always allowed
+            s = nx[j]
+        assert fs[r] == s and dn[r] == acc[s]
+        assert (ln[r] == cfg.max_steps) or acc[s]
+        assert (toks[r, ln[r]:] == -1).all() and slp[r] <= 0
+    # sampled rows, one by one
+    rows = sorted(set(np.random.default_rng(4).choice(cfg.B, size=96, replace=False).tolist()) | {0, cfg.B - 1})
+    sub = [x[rows].cpu() for x in logits]
+    ref = oracle.decode_loop(aut, sub, max_steps=cfg.max_steps)
+    assert np.array_equal(toks[rows], ref["tokens"])
+    assert np.array_equal(ln[rows], ref["len"]) and np.array_equal(fs[rows], ref["final_state"])
+    assert np.array_equal(dn[rows], ref["done"])
+    bound = TOL * (ref["len"] + np.abs(ref["sum_logprob"]))
+    assert np.all(np.abs(slp[rows] - ref["sum_logprob"]) <= bound)
+    dfa.close()
+
+
+def test_host_buffer_loop_matches_device_loop(cd, oracle):
+    cfg = wl.scaled(wl.CONFIGS["c3"], V=30000, B=300, S=64, max_steps=8)
+    aut = wl.build_automaton(cfg, device="cuda:0")
+    logits = wl.build_step_logits(cfg, aut, device="cuda:0")
+    dfa = dev_dfa(cd, aut)
+    out = cd.decode_loop(dfa, logits, max_steps=cfg.max_steps)
+    host = [x.cpu().pin_memory() for x in logits]
+    out_h = cd.decode_loop_host(dfa, host, max_steps=cfg.max_steps)
+    for k in ("tokens", "len", "final_state", "done", "sum_logprob"):
+        assert torch.equal(out[k].cpu(), out_h[k]), k
+    dfa.close()
+
+
+def test_trie_sugar_equals_explicit_csr(cd, oracle):
+    cfg = wl.scaled(wl.CONFIGS["c2"], V=20000, B=200, K=30)
+    aut = wl.build_automaton(cfg)
+    logits = wl.build_step_logits(cfg, aut, device="cuda:0")
+    d1 = dev_dfa(cd, aut)
+    d2 = cd.compile_trie(cfg.V, aut.labels, device="cuda:0")
+    assert (d1.S, d1.nnz) == (d2.S, d2.nnz)
+    o1 = cd.decode_loop(d1, logits)
+    o2 = cd.decode_loop(d2, logits)
+    for k in o1:
+        assert torch.equal(o1[k], o2[k])
+    d1.close()
+    d2.close()
+
+
+def test_stepwise_api_reproduces_the_loop(cd, oracle):
+    cfg = wl.scaled(wl.CONFIGS["c3"], V=70000, B=700, S=128, max_steps=12)
+    aut = wl.build_automaton(cfg, device="cuda:0")
+    logits = wl.build_step_logits(cfg, aut, device="cuda:0")
+    dfa = dev_dfa(cd, aut)
+    out = cd.decode_loop(dfa, logits)
+    ids = torch.arange(cfg.B, dtype=torch.int32, device="cuda:0")
+    st = torch.full((cfg.B,), aut.start, dtype=torch.int32, device="cuda:0")
+    toks = torch.full((cfg.B, cfg.max_steps), -1, dtype=torch.int32, device="cuda:0")
+    n = cfg.B
+    for k in range(cfg.max_steps):
+        if n == 0:
+            break
+        tok, lp, lse, done = cd.step(dfa, logits[k], st, row_map=ids, n=n)
+        toks[ids[:n].long(), k] = tok
+        ids, st, na = cd.compact(done, ids, st, n=n)
+        n = int(na)
+    assert torch.equal(toks, out["tokens"])
+    dfa.close()
