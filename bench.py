@@ -1,0 +1,378 @@
+#!/usr/bin/env python
+"""bench.py -- constrained-step throughput on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config c4] [--impl reference]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input:
+cd_decode_loop on one batch of the workload (automaton store already
+compiled): per decoding step the fused mask + masked log-softmax + masked
+argmax + CSR transition kernel, then early-exit compaction, until max_steps.
+Default workload: one batch of BASELINE.json configs[4] (B=4096 rows,
+V=262144, bf16, random DFA S=4096 at 0.5 % density, <= 16 steps, 32 GiB of
+logits per batch) -- the largest single-GPU configuration.  `value` is table
+rows/s (rows decoded to completion or truncation per second, all GPUs).
+
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import torch  # noqa: E402
+
+import workloads as wl  # noqa: E402
+
+METRIC = "constrained-step rows/s and HBM GB/s (% of B200 peak) at V=262144"
+UNIT = "rows/s"
+NOMINAL_HBM_GBS = 8000.0
+FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel from the
+# `ncu --set full` capture summarised in profiles/ (None until a capture exists for this
+# workload); keyed by config name.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="c4", choices=["c1", "c2", "c3", "c4"])
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--batches", type=int, default=2, help="resident input batches rotated over the timed steps")
+    ap.add_argument("--cpu-sample-rows", type=int, default=512)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region."""
+
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.path = None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)],
+                stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+            time.sleep(0.35)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return None
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        try:
+            for line in open(self.path):
+                p = [x.strip() for x in line.split(",")]
+                if len(p) < 9:
+                    continue
+                try:
+                    sm.append(float(p[1]))
+                    mx.append(float(p[2]))
+                except ValueError:
+                    continue
+                for nm, v in zip(names, p[5:9]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            os.unlink(self.path)
+        except Exception:
+            return None
+        if not sm:
+            return None
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def build_inputs(cfg, device, n_batches, batch0):
+    aut = wl.build_automaton(cfg, device=device)
+    batches = [wl.build_step_logits(cfg, aut, device=device, batch=batch0 + b) for b in range(n_batches)]
+    return aut, batches
+
+
+def bytes_per_row_step(cfg):
+    sz = 2 if cfg.dtype == torch.bfloat16 else 4
+    return cfg.V * sz, cfg.V // 8
+
+
+def run_reference(args, rank):
+    """--impl reference: the CPU oracle, as it stands, timed on this box's host
+    cores on a bounded sample (the first --cpu-sample-rows rows of each batch)."""
+    if rank != 0:
+        return
+    import oracle
+
+    oracle.build()
+    cfg = wl.CONFIGS[args.config]
+    R = min(args.cpu_sample_rows, cfg.B)
+    dev = "cuda:0" if torch.cuda.is_available() else "cpu"
+    aut = wl.build_automaton(cfg, device=dev)
+    # the sample: rows [0, R) of every step buffer of batch 0 (generated on `dev`, bytes moved to the host)
+    # (make_logits draws rows in chunks of 512 from one generator stream, so the first chunks of a
+    # smaller batch are byte-identical to those of the full batch)
+    gen_rows = min(cfg.B, (R + 511) // 512 * 512)
+    logits = [x[:R].cpu().contiguous() for x in wl.build_step_logits(cfg, aut, device=dev, B=gen_rows)]
+    times, row_steps = [], 0
+    for i in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        res = oracle.decode_loop(aut, logits)
+        dt = time.perf_counter() - t0
+        if i >= args.warmup:
+            times.append(dt)
+            row_steps = int(res["n_active_hist"].sum())
+    total = sum(times)
+    value = R * args.steps / total
+    sample = f"rows [0,{R}) of one {cfg.name} batch (B={cfg.B}), all {cfg.max_steps} steps, {row_steps} row-steps per pass"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64 accumulate over " + str(cfg.dtype).replace("torch.", ""),
+        "data": "synthetic", "config": {"workload": cfg.desc, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "row_steps_per_s": row_steps * args.steps / total,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    import paper_2606_31808_b200 as cd
+
+    cd.lib()
+    torch.cuda.set_device(local_rank)
+    device = f"cuda:{local_rank}"
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+
+        dist = dist_mod
+        dist.init_process_group("nccl", device_id=torch.device(device))
+
+    cfg = wl.CONFIGS[args.config]
+    sz_logit, sz_mask = bytes_per_row_step(cfg)
+    # weak scaling: every rank decodes its own batches of the table (rows are
+    # independent, the automaton is replicated, no collective on the data path)
+    aut, batches = build_inputs(cfg, device, args.batches, batch0=rank * args.batches)
+    dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device=device)
+    dfa.reserve(cfg.B)
+    out = None
+    stream = torch.cuda.current_stream()
+
+    def one_step(i):
+        nonlocal out
+        out = cd.decode_loop(dfa, batches[i % len(batches)], max_steps=cfg.max_steps, out=out)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # row-steps of every resident batch (untimed): sum of generated lengths
+    rs_batch = []
+    for b in range(len(batches)):
+        one_step(b)
+        rs_batch.append(int(out["len"].sum()))
+    for i in range(args.warmup):
+        one_step(i)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    launches0 = cd.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for i in range(args.steps):
+        one_step(args.warmup + i)
+    e1.record(stream)
+    barrier()
+    launches = cd.launch_count() - launches0
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms], device=device)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t[0])
+    value = cfg.B * args.steps * world / (ms * 1e-3)
+
+    # ---------------- roofline of the dominant kernel (fused step), live, per launch:
+    # the same loop driven through cd_step / cd_compact with CUDA events around every
+    # cd_step launch on the launching stream.
+    peak, peak_src = measured_peak()
+    step_ms, step_bytes, step_rows = [], [], []
+    for rep in range(2):  # first repetition warms up the stepwise path
+        logits = batches[rep % len(batches)]
+        ids = torch.arange(cfg.B, dtype=torch.int32, device=device)
+        st = torch.full((cfg.B,), aut.start, dtype=torch.int32, device=device)
+        n = cfg.B
+        for k in range(cfg.max_steps):
+            if n == 0:
+                break
+            distinct = int(torch.unique(st[:n]).numel())
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            a.record(stream)
+            tok, lp, _, done = cd.step(dfa, logits[k], st, row_map=ids, n=n, want_lse=False)
+            b.record(stream)
+            torch.cuda.synchronize()
+            if rep == 1:
+                step_ms.append(a.elapsed_time(b))
+                step_bytes.append(n * sz_logit + distinct * sz_mask)
+                step_rows.append(n)
+            ids, st, na = cd.compact(done, ids, st, n=n)
+            n = int(na)
+    tot_bytes, tot_ms = sum(step_bytes), sum(step_ms)
+    achieved = tot_bytes / (tot_ms * 1e-3) / 1e9
+    best = max(bb / (mm * 1e-3) / 1e9 for bb, mm in zip(step_bytes, step_ms))
+    roofline = {
+        "bound": "hbm", "kernel": "cd::step_kernel (fused mask + masked logsumexp/argmax + CSR transition)",
+        "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+        "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+        "best_launch_gbs": best, "launches_timed": len(step_ms),
+        "bytes_per_launch_avg": tot_bytes / max(1, len(step_ms)), "us_per_launch_avg": 1e3 * tot_ms / max(1, len(step_ms)),
+        "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(cfg.name),
+        "step_kernel_share_of_loop": (tot_ms / (ms / args.steps)),
+    }
+    row_steps_timed = sum(rs_batch[(args.warmup + i) % len(batches)] for i in range(args.steps))
+    row_steps = row_steps_timed / args.steps
+
+    # ---------------- e2e: the same metric through the C ABI with HOST buffers
+    e2e = None
+    if not args.no_e2e:
+        try:
+            host = [torch.empty(x.shape, dtype=x.dtype, pin_memory=True) for x in batches[0]]
+            for h, x in zip(host, batches[0]):
+                h.copy_(x)
+            torch.cuda.synchronize()
+            out_h = None
+            k_e2e = max(1, min(args.steps, 5))
+            for i in range(1 + k_e2e):
+                if i == 1:
+                    barrier()
+                    t0 = time.perf_counter()
+                out_h = cd.decode_loop_host(dfa, host, max_steps=cfg.max_steps, out=out_h)
+            barrier()
+            dt = time.perf_counter() - t0
+            if dist is not None:
+                t = torch.tensor([dt], device=device)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                dt = float(t[0])
+            # the host loop copies step k+1 while step k runs and stops once nothing is active
+            steps_copied = min(cfg.max_steps, int(out_h["len"].max()) + 1)
+            h2d = steps_copied * cfg.B * cfg.V * (2 if cfg.dtype == torch.bfloat16 else 4)
+            d2h = cfg.B * (cfg.max_steps * 4 + 4 + 4 + 4 + 1) + 4 * steps_copied
+            e2e = {"value": cfg.B * k_e2e * world / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                   "d2h_bytes_per_step": d2h, "steps": k_e2e, "ms_per_step": 1e3 * dt / k_e2e,
+                   "h2d_gbs": h2d * k_e2e / dt / 1e9, "host_memory": "pinned"}
+            got0 = cd.decode_loop(dfa, batches[0], max_steps=cfg.max_steps)
+            assert torch.equal(out_h["tokens"], got0["tokens"].cpu()), "host-buffer loop disagrees with device loop"
+            del host
+        except Exception as ex:  # e.g. not enough pinned host memory on this box
+            e2e = {"value": None, "unit": UNIT, "error": str(ex)[:200]}
+
+    # ---------------- CPU oracle timed beside it (rank 0, bounded sample, a baseline not a target)
+    cpu = None
+    if rank == 0 and not args.no_cpu_baseline:
+        import oracle
+
+        oracle.build()
+        R = min(args.cpu_sample_rows, cfg.B)
+        sub = [x[:R].cpu().contiguous() for x in batches[0]]
+        t0 = time.perf_counter()
+        reps = 0
+        while True:
+            res = oracle.decode_loop(aut, sub)
+            reps += 1
+            if time.perf_counter() - t0 > 10.0 or reps >= 50:
+                break
+        dt = time.perf_counter() - t0
+        cpu = {"value": R * reps / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": f"rows [0,{R}) of one {cfg.name} batch, all {cfg.max_steps} steps, {reps} passes, "
+                         f"{int(res['n_active_hist'].sum())} row-steps per pass (D2H copy excluded)",
+               "row_steps_per_s": int(res["n_active_hist"].sum()) * reps / dt}
+        # parity spot check on the sample while we are here
+        import numpy as np
+
+        got = cd.decode_loop(dfa, batches[0], max_steps=cfg.max_steps)
+        assert np.array_equal(got["tokens"][:R].cpu().numpy(), res["tokens"]), "bench parity check failed"
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16" if cfg.dtype == torch.bfloat16 else "f32", "data": "synthetic",
+            "config": {
+                "workload": f"{cfg.name}: {cfg.desc}; one step = cd_decode_loop over one batch of B={cfg.B} rows",
+                "B": cfg.B, "V": cfg.V, "max_steps": cfg.max_steps, "S": aut.S, "nnz": aut.nnz,
+                "resident_batches": len(batches),
+                "l2": f"inputs larger than L2: {cfg.max_steps * cfg.B * sz_logit / 2**30:.1f} GiB of logits per step, "
+                      f"{len(batches)} batches rotated",
+                "parallelism": f"rows sharded over {world} GPU(s), automaton replicated, no collective",
+            },
+            "row_steps_per_step": row_steps,
+            "row_steps_per_s": row_steps_timed * world / (ms * 1e-3),
+            "loop_gbs_per_gpu": row_steps_timed * sz_logit / (ms * 1e-3) / 1e9,
+            "gpu_launches": launches,
+            "clocks": clocks,
+            "e2e": e2e,
+            "roofline": roofline,
+            "cpu_baseline": cpu,
+            "paper_context": "PAPER.md L17-18/L32: 390x lower cost, 3.8x lower latency than a proprietary API with a "
+                             "quantized model on one 16 GB GPU; no per-step number is published (BASELINE.md)",
+        }
+        print(json.dumps(line), flush=True)
+    dfa.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

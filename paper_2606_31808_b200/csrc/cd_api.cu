@@ -6,6 +6,7 @@
 #include <atomic>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -42,8 +43,21 @@ cd_status fail(cd_status st, const char* fmt, ...) {
         }                                                                                    \
     } while (0)
 
-constexpr int STEP_WARPS = 8;
-constexpr int STEP_STAGES = 4;
+// Launch shapes of the step kernel: warps per CTA (one CTA per SM), ring stages per warp, tile
+// bytes.  Variant 0 is the product default; the others exist for tuning runs
+// (environment variable CD_STEP_VARIANT, read once).
+struct StepCfg { int warps, stages, tile_bytes; };
+constexpr StepCfg STEP_CFGS[] = {{16, 3, 4096}, {8, 4, 4096}, {8, 3, 8192}, {12, 2, 8192}, {16, 2, 4096}, {12, 4, 4096}};
+constexpr int N_STEP_CFGS = sizeof(STEP_CFGS) / sizeof(STEP_CFGS[0]);
+
+int step_variant() {
+    static const int v = [] {
+        const char* e = std::getenv("CD_STEP_VARIANT");
+        const int x = e ? std::atoi(e) : 0;
+        return (x >= 0 && x < N_STEP_CFGS) ? x : 0;
+    }();
+    return v;
+}
 
 // Per (handle, stream) scratch.  Operations on one stream are ordered, so one area per stream
 // is race free; distinct streams get distinct areas.
@@ -116,11 +130,8 @@ struct DeviceGuard {
     }
 };
 
-template <int DT>
-constexpr int tile_tok() { return cd::TILE_BYTES / (DT == cd::DT_BF16 ? 2 : 4); }
-
 int tiles_per_row(int V, int dtype) {
-    const int tt = cd::TILE_BYTES / (dtype == CD_BF16 ? 2 : 4);
+    const int tt = STEP_CFGS[step_variant()].tile_bytes / (dtype == CD_BF16 ? 2 : 4);
     return (V + tt - 1) / tt;
 }
 
@@ -135,12 +146,12 @@ int step_grid(const cd_dfa* d, long long n_upper, int dtype) {
 // Upper bound of n' * P(n') over n' <= n for the largest grid (mirrors cd::tiles_per_unit):
 // unclamped tiles-per-unit gives n'P <= 4*warps + n'; clamped at TPU_MAX gives n' * ceil(T/16).
 long long step_units_cap(const cd_dfa* d, long long n) {
-    const int T = tiles_per_row(d->dev.V, CD_BF16) > tiles_per_row(d->dev.V, CD_F32)
-                      ? tiles_per_row(d->dev.V, CD_BF16)
-                      : tiles_per_row(d->dev.V, CD_F32);
-    const long long warps = (long long)d->num_sms * STEP_WARPS;
+    const StepCfg c = STEP_CFGS[step_variant()];
+    const int T = tiles_per_row(d->dev.V, CD_F32);  // fp32 rows have the most tiles
+    const int tpu_max = cd::TPU_MAX_BYTES / c.tile_bytes;
+    const long long warps = (long long)d->num_sms * c.warps;
     const long long a = warps * cd::UNITS_PER_WARP + n;
-    const long long b = n * ((T + cd::TPU_MAX - 1) / cd::TPU_MAX + 1);
+    const long long b = n * ((T + tpu_max - 1) / tpu_max + 1);
     // small grids (few rows) use fewer warps, hence fewer units: still below a
     return (a > b ? a : b) + 64;
 }
@@ -188,21 +199,34 @@ cd_status check_dtype(cd_dtype dt) {
     return CD_OK;
 }
 
-template <int DT>
+template <int DT, int VAR>
 cd_status launch_step_t(const cd::StepArgs& a, int grid, cudaStream_t stream) {
-    auto kern = cd::step_kernel<DT, STEP_WARPS, STEP_STAGES>;
-    const size_t smem = sizeof(cd::WarpRing<STEP_STAGES>) * STEP_WARPS;
-    static thread_local int configured_dev[2] = {-1, -1};
+    constexpr StepCfg C = STEP_CFGS[VAR];
+    auto kern = cd::step_kernel<DT, C.warps, C.stages, C.tile_bytes>;
+    const size_t smem = sizeof(cd::WarpRing<C.stages, C.tile_bytes>) * C.warps;
+    static thread_local int configured_dev = -1;
     int dev = 0;
     CU(cudaGetDevice(&dev));
-    if (configured_dev[DT] != dev) {
+    if (configured_dev != dev) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        configured_dev[DT] = dev;
+        configured_dev = dev;
     }
-    kern<<<grid, STEP_WARPS * 32, smem, stream>>>(a);
+    kern<<<grid, C.warps * 32, smem, stream>>>(a);
     CU(cudaGetLastError());
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return CD_OK;
+}
+
+template <int DT>
+cd_status launch_step_v(const cd::StepArgs& a, int grid, cudaStream_t stream) {
+    switch (step_variant()) {
+        case 1: return launch_step_t<DT, 1>(a, grid, stream);
+        case 2: return launch_step_t<DT, 2>(a, grid, stream);
+        case 3: return launch_step_t<DT, 3>(a, grid, stream);
+        case 4: return launch_step_t<DT, 4>(a, grid, stream);
+        case 5: return launch_step_t<DT, 5>(a, grid, stream);
+        default: return launch_step_t<DT, 0>(a, grid, stream);
+    }
 }
 
 // n_upper bounds the active count; n_dev (device int) overrides n inside the kernel.
@@ -225,8 +249,8 @@ cd_status launch_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype 
     a.tickets = s->tickets;
     a.ctrs = s->ctrs;
     const int grid = step_grid(d, n_upper, dtype);
-    return dtype == CD_BF16 ? launch_step_t<cd::DT_BF16>(a, grid, stream)
-                            : launch_step_t<cd::DT_F32>(a, grid, stream);
+    return dtype == CD_BF16 ? launch_step_v<cd::DT_BF16>(a, grid, stream)
+                            : launch_step_v<cd::DT_F32>(a, grid, stream);
 }
 
 cd_status check_logits_layout(const cd_dfa* d, const void* logits, cd_dtype dtype, long long ld) {

@@ -97,14 +97,24 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 // (m, s, idx): running masked maximum, sum of exp(x - m) over the allowed elements seen so
 // far, lowest token id attaining m.  Elements are presented in ascending token id per lane,
 // so "replace on strictly greater" keeps the lowest id (north_star: ties -> lowest token id).
+constexpr float LOG2E = 1.4426950408889634f;
+
+__device__ __forceinline__ float ex2_ftz(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// Branch-free.  x = -inf (a masked-out lane, or an allowed -inf / NaN logit) changes nothing.
+// One MUFU per element: either the old sum or the new term is scaled by e = exp(-|x - m|).
 __device__ __forceinline__ void online_update(float& m, float& s, int& idx, float x, int t) {
-    if (x > m) {
-        s = s * __expf(m - x) + 1.0f;  // m = -inf: exp(-inf) = 0
-        m = x;
-        idx = t;
-    } else if (x > -INFINITY) {  // x = -inf contributes exactly 0 (and m may still be -inf)
-        s += __expf(x - m);
-    }
+    const float lo = fminf(m, x), hi = fmaxf(m, x);
+    float e = ex2_ftz((lo - hi) * LOG2E);
+    e = (lo == -INFINITY) ? 0.0f : e;  // also covers m = x = -inf (lo - hi = NaN)
+    const bool gt = x > m;
+    s = gt ? fmaf(s, e, 1.0f) : s + e;
+    idx = gt ? t : idx;
+    m = hi;
 }
 
 // Merge two partial results; equal maxima keep the lower token id whatever the order.
@@ -112,7 +122,7 @@ __device__ __forceinline__ void online_combine(float& m, float& s, int& idx, flo
     const bool take2 = (m2 > m) || (m2 == m && i2 < idx);
     const float mw = take2 ? m2 : m, ml = take2 ? m : m2;
     const float sw = take2 ? s2 : s, sl = take2 ? s : s2;
-    const float f = (ml == -INFINITY) ? 0.0f : __expf(ml - mw);
+    const float f = (ml == -INFINITY) ? 0.0f : ex2_ftz((ml - mw) * LOG2E);
     s = fmaf(sl, f, sw);
     m = mw;
     idx = take2 ? i2 : idx;

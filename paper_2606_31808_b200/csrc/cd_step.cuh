@@ -23,9 +23,7 @@
 
 namespace cd {
 
-constexpr int TILE_BYTES = 4096;      // logits bytes per tile
-constexpr int MASK_SLOT_BYTES = 256;  // bf16: 2048 tokens -> 256 B of mask; fp32: 1024 -> 128 B
-constexpr int TPU_MAX = 16;           // at most 16 tiles (64 KiB) per unit
+constexpr int TPU_MAX_BYTES = 65536;  // at most 64 KiB of logits per unit
 constexpr int UNITS_PER_WARP = 4;     // aim for >= 4 units per warp when rows are few
 
 constexpr int FLAG_FIRST = 1;   // first tile of its unit: reset the lane accumulators
@@ -58,19 +56,19 @@ struct __align__(16) TileMeta {
     int st;     // automaton state of the slot
 };
 
-template <int STAGES>
+template <int STAGES, int TILE_BYTES>
 struct __align__(128) WarpRing {
     unsigned char logits[STAGES][TILE_BYTES];
-    unsigned char mask[STAGES][MASK_SLOT_BYTES];
+    unsigned char mask[STAGES][TILE_BYTES / 16];  // bf16: TILE_BYTES/2 tokens / 8; fp32 uses half
     TileMeta meta[STAGES];
     unsigned long long bar[STAGES];
 };
 
 // tiles per unit for n active rows (host mirrors this in cd_api.cu: step_units_cap)
-__host__ __device__ inline int tiles_per_unit(long long n, int tiles_per_row, long long total_warps) {
+__host__ __device__ inline int tiles_per_unit(long long n, int tiles_per_row, long long total_warps, int tpu_max) {
     long long t = (n * tiles_per_row + total_warps * UNITS_PER_WARP - 1) / (total_warps * UNITS_PER_WARP);
     if (t < 1) t = 1;
-    if (t > TPU_MAX) t = TPU_MAX;
+    if (t > tpu_max) t = tpu_max;
     return (int)t;
 }
 
@@ -117,14 +115,19 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, int slot, int st
     }
 }
 
-template <int DT, int WARPS, int STAGES>
+template <int DT, int WARPS, int STAGES, int TILE_BYTES>
 __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     constexpr int SZ = (DT == DT_BF16) ? 2 : 4;
     constexpr int TILE_TOK = TILE_BYTES / SZ;
+    constexpr int MASK_BYTES = TILE_TOK / 8;
+    constexpr int WPL = TILE_TOK / 1024;  // mask words per lane and tile
+    constexpr int TPU_MAX = TPU_MAX_BYTES / TILE_BYTES;
+    static_assert(WPL >= 1 && TILE_TOK % 1024 == 0, "tile must hold a multiple of 32 mask words");
+    using Ring = WarpRing<STAGES, TILE_BYTES>;
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    WarpRing<STAGES>& ring = reinterpret_cast<WarpRing<STAGES>*>(smem_raw)[warp];
+    Ring& ring = reinterpret_cast<Ring*>(smem_raw)[warp];
 
     if (lane == 0) {
 #pragma unroll
@@ -136,98 +139,110 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     const int n = a.n_dev ? __ldg(a.n_dev) : a.n;
     const int V = a.dfa.V;
     const int tiles_per_row = (V + TILE_TOK - 1) / TILE_TOK;
-    const long long total_warps = (long long)gridDim.x * WARPS;
-    const int tpu = tiles_per_unit(n, tiles_per_row, total_warps);
+    const int total_warps = gridDim.x * WARPS;
+    const int tpu = tiles_per_unit(n, tiles_per_row, total_warps, TPU_MAX);
     const int P = (tiles_per_row + tpu - 1) / tpu;  // units per row
     const int total_units = n * P;
+    const bool ragged_row = (V % TILE_TOK) != 0;
     const uint64_t pol_stream = l2_policy_evict_first();
 
     // ---------------- issue side (warp-uniform state)
     int next_u_l0 = 0;  // prefetched unit id, valid in lane 0
     if (lane == 0) next_u_l0 = atomicAdd(a.ctrs + 0, 1);
     bool exhausted = false;
-    int iss_tile = 0, iss_end = 0, iss_first = 0;
-    int iss_slot = 0, iss_part = 0, iss_st = 0;
-    const unsigned char* iss_row = nullptr;
-    const unsigned char* iss_mask = nullptr;
-    unsigned issued = 0, consumed = 0;
+    int iss_tile = 0, iss_end = 0;
+    int iss_slot = 0, iss_st = 0, iss_flags = 0;
+    const unsigned char* iss_src = nullptr;  // next logits tile of the current unit
+    const unsigned char* iss_msk = nullptr;  // next mask piece
+    int iss_stage = 0, in_flight = 0;
 
-    auto issue_one = [&]() -> bool {
+    auto issue_one = [&]() {
         if (iss_tile >= iss_end) {
-            if (exhausted) return false;
+            if (exhausted) return;
             const int u = __shfl_sync(FULL, next_u_l0, 0);
             if (u >= total_units) {
                 exhausted = true;
-                return false;
+                return;
             }
             if (lane == 0) next_u_l0 = atomicAdd(a.ctrs + 0, 1);
             iss_slot = u / P;
-            iss_part = u - iss_slot * P;
+            const int part = u - iss_slot * P;
             iss_st = a.state[iss_slot];  // updated only after every unit of the slot has arrived
             const bool bad = (iss_st < 0) || (iss_st >= a.dfa.S);
             const bool acc = !bad && (__ldg(a.dfa.accepting + iss_st) != 0);
             if (bad || acc) {
-                const int stage = issued % STAGES;
                 if (lane == 0) {
-                    ring.meta[stage] = TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (iss_part << 8), iss_st};
-                    mbar_arrive(smem_u32(&ring.bar[stage]));
+                    ring.meta[iss_stage] = TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (part << 8), iss_st};
+                    mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
-                ++issued;
+                iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
+                ++in_flight;
                 iss_tile = iss_end = 0;
-                return true;
+                return;
             }
             const long long r = a.row_map ? (long long)__ldg(a.row_map + iss_slot) : (long long)iss_slot;
-            iss_row = a.logits + r * a.ld_bytes;
-            iss_mask = reinterpret_cast<const unsigned char*>(a.dfa.mask + (long long)iss_st * a.dfa.Wpad);
-            iss_first = iss_part * tpu;
-            iss_tile = iss_first;
-            iss_end = min(iss_first + tpu, tiles_per_row);
+            iss_tile = part * tpu;
+            iss_end = min(iss_tile + tpu, tiles_per_row);
+            iss_src = a.logits + r * a.ld_bytes + (long long)iss_tile * TILE_BYTES;
+            iss_msk = reinterpret_cast<const unsigned char*>(a.dfa.mask + (long long)iss_st * a.dfa.Wpad) +
+                      (long long)iss_tile * MASK_BYTES;
+            iss_flags = (part << 8) | FLAG_FIRST;
         }
-        const int stage = issued % STAGES;
-        const int t0 = iss_tile * TILE_TOK;
-        const int ntok = min(TILE_TOK, V - t0);
-        const uint32_t bytes = (uint32_t)ntok * SZ;
-        const uint32_t bulk = bytes & ~15u;
-        const uint32_t mbytes = (uint32_t)(((ntok + 31) >> 5) * 4 + 15) & ~15u;
-        const unsigned char* src = iss_row + (long long)iss_tile * TILE_BYTES;
-        if (bulk < bytes) {  // < 16 trailing bytes (V*SZ not a multiple of 16): plain loads
+        const uint32_t bar = smem_u32(&ring.bar[iss_stage]);
+        const uint32_t dst = smem_u32(ring.logits[iss_stage]);
+        const uint32_t mdst = smem_u32(ring.mask[iss_stage]);
+        const int fl = iss_flags | ((iss_tile + 1 == iss_end) ? FLAG_LAST : 0);
+        if (ragged_row && iss_tile + 1 == tiles_per_row) {
+            // last tile of a row whose length is not a multiple of the tile: partial copies; the
+            // < 16 trailing logits bytes go through plain loads, unused mask words are zeroed.
+            const int ntok = V - iss_tile * TILE_TOK;
+            const uint32_t bytes = (uint32_t)ntok * SZ;
+            const uint32_t bulk = bytes & ~15u;
+            const uint32_t mbytes = (uint32_t)(((ntok + 31) >> 5) * 4 + 15) & ~15u;
             const int e = (int)(bulk / SZ) + lane;
             if (e < ntok) {
                 if (DT == DT_BF16)
-                    reinterpret_cast<uint16_t*>(ring.logits[stage])[e] = reinterpret_cast<const uint16_t*>(src)[e];
+                    reinterpret_cast<uint16_t*>(ring.logits[iss_stage])[e] = reinterpret_cast<const uint16_t*>(iss_src)[e];
                 else
-                    reinterpret_cast<float*>(ring.logits[stage])[e] = reinterpret_cast<const float*>(src)[e];
+                    reinterpret_cast<float*>(ring.logits[iss_stage])[e] = reinterpret_cast<const float*>(iss_src)[e];
             }
+            for (int w = (int)(mbytes / 4) + lane; w < MASK_BYTES / 4; w += 32)
+                reinterpret_cast<uint32_t*>(ring.mask[iss_stage])[w] = 0u;
+            __syncwarp();
+            if (lane == 0) {
+                ring.meta[iss_stage] = TileMeta{iss_slot, iss_tile, fl, iss_st};
+                mbar_arrive_expect_tx(bar, bulk + mbytes);
+                if (bulk) bulk_g2s_hint(dst, iss_src, bulk, bar, pol_stream);
+                bulk_g2s(mdst, iss_msk, mbytes, bar);
+            }
+        } else if (lane == 0) {
+            ring.meta[iss_stage] = TileMeta{iss_slot, iss_tile, fl, iss_st};
+            mbar_arrive_expect_tx(bar, TILE_BYTES + MASK_BYTES);
+            bulk_g2s_hint(dst, iss_src, TILE_BYTES, bar, pol_stream);
+            bulk_g2s(mdst, iss_msk, MASK_BYTES, bar);
         }
-        if (lane == 0) {
-            int fl = (iss_part << 8);
-            if (iss_tile == iss_first) fl |= FLAG_FIRST;
-            if (iss_tile + 1 == iss_end) fl |= FLAG_LAST;
-            ring.meta[stage] = TileMeta{iss_slot, iss_tile, fl, iss_st};
-            const uint32_t bar = smem_u32(&ring.bar[stage]);
-            mbar_arrive_expect_tx(bar, bulk + mbytes);
-            if (bulk) bulk_g2s_hint(smem_u32(ring.logits[stage]), src, bulk, bar, pol_stream);
-            bulk_g2s(smem_u32(ring.mask[stage]), iss_mask + (long long)iss_tile * (TILE_TOK / 8), mbytes, bar);
-        }
-        ++issued;
+        iss_flags &= ~FLAG_FIRST;
+        iss_src += TILE_BYTES;
+        iss_msk += MASK_BYTES;
         ++iss_tile;
-        return true;
+        ++in_flight;
+        iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
     };
 
 #pragma unroll 1
-    for (int k = 0; k < STAGES; ++k)
-        if (!issue_one()) break;
+    for (int k = 0; k < STAGES; ++k) issue_one();
 
     // ---------------- consume side
     float m = -INFINITY, s = 0.0f;
     int idx = 0x7FFFFFFF;
+    int cons_stage = 0;
+    uint32_t cons_phase = 0;
 
 #pragma unroll 1
-    while (consumed < issued) {
-        const int stage = consumed % STAGES;
-        mbar_wait(smem_u32(&ring.bar[stage]), (consumed / STAGES) & 1);
+    while (in_flight > 0) {
+        mbar_wait(smem_u32(&ring.bar[cons_stage]), cons_phase);
         __syncwarp();
-        const TileMeta mt = ring.meta[stage];
+        const TileMeta mt = ring.meta[cons_stage];
         const int part = mt.flags >> 8;
 
         if (mt.flags & (FLAG_ACCEPT | FLAG_BADSTATE)) {
@@ -246,17 +261,22 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 idx = 0x7FFFFFFF;
             }
             const int t0 = mt.tile * TILE_TOK;
-            const int nwords = (min(TILE_TOK, V - t0) + 31) >> 5;
-            const uint32_t* mw = reinterpret_cast<const uint32_t*>(ring.mask[stage]);
-            const unsigned char* tile = ring.logits[stage];
+            const uint32_t* mw = reinterpret_cast<const uint32_t*>(ring.mask[cons_stage]);
+            const unsigned char* tile = ring.logits[cons_stage];
+            uint32_t bits[WPL];
 #pragma unroll
-            for (int w = lane; w < TILE_TOK / 32; w += 32) {
-                uint32_t bits = (w < nwords) ? mw[w] : 0u;
-                while (bits) {
-                    const int b = __ffs(bits) - 1;
-                    bits &= bits - 1;
-                    const int e = w * 32 + b;
-                    online_update(m, s, idx, tile_elem<DT>(tile, e), t0 + e);
+            for (int j = 0; j < WPL; ++j) bits[j] = mw[j * 32 + lane];
+#pragma unroll
+            for (int j = 0; j < WPL; ++j) {
+                // warp-uniform trip count (max popcount over the lanes); idle lanes feed -inf
+                uint32_t b = bits[j];
+                const int e0 = (j * 32 + lane) * 32;
+                while (__any_sync(FULL, b != 0u)) {
+                    const bool v = b != 0u;
+                    const int e = e0 + (v ? (__ffs(b) - 1) : 0);
+                    b &= b - 1u;
+                    const float x = v ? tile_elem<DT>(tile, e) : -INFINITY;
+                    online_update(m, s, idx, x, t0 + e);
                 }
             }
             if (mt.flags & FLAG_LAST) {
@@ -289,7 +309,9 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 }
             }
         }
-        ++consumed;
+        --in_flight;
+        cons_stage = (cons_stage + 1 == STAGES) ? 0 : cons_stage + 1;
+        cons_phase ^= (cons_stage == 0) ? 1u : 0u;
         __syncwarp();
         issue_one();
     }
@@ -298,7 +320,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     if (lane == 0) {
         __threadfence();
         const int d = atomicAdd(a.ctrs + 1, 1);
-        if (d == (int)total_warps - 1) {
+        if (d == total_warps - 1) {
             a.ctrs[0] = 0;
             a.ctrs[1] = 0;
         }
