@@ -247,28 +247,53 @@ def main():
     # the same loop driven through cd_step / cd_compact with CUDA events around every
     # cd_step launch on the launching stream.
     peak, peak_src = measured_peak()
+    # Repetition 0 walks the loop with host reads of the active count (gives n_k and the number
+    # of distinct states per step); repetition 1 replays it with everything enqueued ahead of
+    # the GPU (a ~0.3 ms device-side sleep first, no host sync, preallocated outputs), so that
+    # the events bracket the kernel itself and not the host's launch gaps.
     step_ms, step_bytes, step_rows = [], [], []
-    for rep in range(2):  # first repetition warms up the stepwise path
-        logits = batches[rep % len(batches)]
-        ids = torch.arange(cfg.B, dtype=torch.int32, device=device)
-        st = torch.full((cfg.B,), aut.start, dtype=torch.int32, device=device)
+    logits = batches[0]
+    n_k, distinct_k = [], []
+    i32 = dict(dtype=torch.int32, device=device)
+    bufs = dict(tok=torch.empty(cfg.B, **i32), lp=torch.empty(cfg.B, dtype=torch.float32, device=device),
+                done=torch.empty(cfg.B, dtype=torch.uint8, device=device),
+                ids=[torch.empty(cfg.B, **i32) for _ in range(2)], st=[torch.empty(cfg.B, **i32) for _ in range(2)],
+                na=torch.empty(1, **i32))
+    for rep in range(2):
+        bufs["ids"][0].copy_(torch.arange(cfg.B, **i32))
+        bufs["st"][0].fill_(aut.start)
+        events = []
+        if rep == 1:
+            torch.cuda.synchronize()
+            torch.cuda._sleep(600000)
         n = cfg.B
         for k in range(cfg.max_steps):
-            if n == 0:
+            cur, nxt = k & 1, (k + 1) & 1
+            if rep == 0:
+                if n == 0:
+                    break
+                n_k.append(n)
+                distinct_k.append(int(torch.unique(bufs["st"][cur][:n]).numel()))
+            elif k >= len(n_k):
                 break
-            distinct = int(torch.unique(st[:n]).numel())
+            else:
+                n = n_k[k]
             a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            torch.cuda.synchronize()
             a.record(stream)
-            tok, lp, _, done = cd.step(dfa, logits[k], st, row_map=ids, n=n, want_lse=False)
+            cd.step(dfa, logits[k], bufs["st"][cur], row_map=bufs["ids"][cur], n=n, want_lse=False,
+                    out=(bufs["tok"], bufs["lp"], None, bufs["done"]))
             b.record(stream)
-            torch.cuda.synchronize()
-            if rep == 1:
+            events.append((a, b))
+            cd.compact(bufs["done"], bufs["ids"][cur], bufs["st"][cur], n=n,
+                       out=(bufs["ids"][nxt], bufs["st"][nxt], bufs["na"]))
+            if rep == 0:
+                n = int(bufs["na"])
+        torch.cuda.synchronize()
+        if rep == 1:
+            for k, (a, b) in enumerate(events):
                 step_ms.append(a.elapsed_time(b))
-                step_bytes.append(n * sz_logit + distinct * sz_mask)
-                step_rows.append(n)
-            ids, st, na = cd.compact(done, ids, st, n=n)
-            n = int(na)
+                step_bytes.append(n_k[k] * sz_logit + distinct_k[k] * sz_mask)
+                step_rows.append(n_k[k])
     tot_bytes, tot_ms = sum(step_bytes), sum(step_ms)
     achieved = tot_bytes / (tot_ms * 1e-3) / 1e9
     best = max(bb / (mm * 1e-3) / 1e9 for bb, mm in zip(step_bytes, step_ms))

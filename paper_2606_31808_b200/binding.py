@@ -166,9 +166,10 @@ def compile_trie(V: int, labels: Sequence[Sequence[int]], device="cuda") -> Dfa:
 
 
 def step(dfa: Dfa, logits: torch.Tensor, state: torch.Tensor, row_map: Optional[torch.Tensor] = None,
-         n: Optional[int] = None, want_lse: bool = True):
+         n: Optional[int] = None, want_lse: bool = True, out=None):
     """cd_step on torch's current stream.  state (int32, device) is updated in
-    place.  Returns (token i32[n], logprob f32[n], lse f32[n] or None, done u8[n])."""
+    place.  Returns (token i32[n], logprob f32[n], lse f32[n] or None, done u8[n]);
+    `out` may pass those four buffers in (each with at least n elements)."""
     dev = dfa.device
     if logits.dim() != 2 or not logits.is_cuda or logits.stride(1) != 1:
         raise TypeError("logits must be a 2-D CUDA tensor with unit inner stride")
@@ -176,10 +177,13 @@ def step(dfa: Dfa, logits: torch.Tensor, state: torch.Tensor, row_map: Optional[
     n = state.numel() if n is None else n
     if row_map is not None:
         _dev_tensor(row_map, torch.int32, "row_map", dev)
-    token = torch.empty(n, dtype=torch.int32, device=dev)
-    logprob = torch.empty(n, dtype=torch.float32, device=dev)
-    lse = torch.empty(n, dtype=torch.float32, device=dev) if want_lse else None
-    done = torch.empty(n, dtype=torch.uint8, device=dev)
+    if out is not None:
+        token, logprob, lse, done = out
+    else:
+        token = torch.empty(n, dtype=torch.int32, device=dev)
+        logprob = torch.empty(n, dtype=torch.float32, device=dev)
+        lse = torch.empty(n, dtype=torch.float32, device=dev) if want_lse else None
+        done = torch.empty(n, dtype=torch.uint8, device=dev)
     _check(lib().cd_step(dfa._h, _ptr(logits), C.c_int(_dt(logits)), C.c_int64(logits.stride(0)), _ptr(row_map),
                          _ptr(state), C.c_int32(n), _ptr(token), _ptr(logprob), _ptr(lse), _ptr(done),
                          _stream(dev)))
@@ -198,7 +202,7 @@ def transition(dfa: Dfa, token: torch.Tensor, state: torch.Tensor):
 
 
 def compact(done: torch.Tensor, row_ids: Optional[torch.Tensor] = None, state: Optional[torch.Tensor] = None,
-            n: Optional[int] = None):
+            n: Optional[int] = None, out=None):
     """cd_compact.  Returns (row_ids_out i32[n], state_out i32[n] or None,
     n_active device int32[1]); only the first n_active entries are meaningful."""
     dev = done.device
@@ -208,9 +212,12 @@ def compact(done: torch.Tensor, row_ids: Optional[torch.Tensor] = None, state: O
         _dev_tensor(row_ids, torch.int32, "row_ids", dev)
     if state is not None:
         _dev_tensor(state, torch.int32, "state", dev)
-    ro = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
-    so = torch.empty(max(n, 1), dtype=torch.int32, device=dev) if state is not None else None
-    na = torch.empty(1, dtype=torch.int32, device=dev)
+    if out is not None:
+        ro, so, na = out
+    else:
+        ro = torch.empty(max(n, 1), dtype=torch.int32, device=dev)
+        so = torch.empty(max(n, 1), dtype=torch.int32, device=dev) if state is not None else None
+        na = torch.empty(1, dtype=torch.int32, device=dev)
     with torch.cuda.device(dev):
         _check(lib().cd_compact(_ptr(done), _ptr(row_ids), _ptr(state), C.c_int32(n), _ptr(ro), _ptr(so), _ptr(na),
                                 _stream(dev)))

@@ -75,6 +75,14 @@ __device__ __forceinline__ uint64_t l2_policy_evict_last() {
     return p;
 }
 
+// Device-scope acquire-release add: earlier writes of this thread are visible to whoever
+// observes the new counter value; later reads of this thread see what earlier arrivers wrote.
+__device__ __forceinline__ int atom_add_acq_rel_gpu(int* p, int v) {
+    int old;
+    asm volatile("atom.add.acq_rel.gpu.global.s32 %0, [%1], %2;" : "=r"(old) : "l"(p), "r"(v) : "memory");
+    return old;
+}
+
 // 1-D bulk async copy global -> shared (TMA engine, SASS UBLKCP), completion on an mbarrier.
 // dst, src 16-byte aligned; bytes a positive multiple of 16.
 __device__ __forceinline__ void bulk_g2s_hint(uint32_t dst, const void* src, uint32_t bytes,

@@ -286,17 +286,17 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 if (P == 1) {
                     finalize_row(a, mt.slot, mt.st, rm, rs, ri, lane);
                 } else {
+                    // Publish from lane 1, not lane 0: lane 0 issues the bulk copies and a
+                    // release by that thread would wait for its copies still in flight.
                     int t = 0;
-                    if (lane == 0) {
+                    if (lane == 1) {
                         a.partials[(long long)mt.slot * P + part] =
                             make_int4(__float_as_int(rm), __float_as_int(rs), ri, 0);
-                        __threadfence();
-                        t = atomicAdd(a.tickets + mt.slot, 1);
+                        t = atom_add_acq_rel_gpu(a.tickets + mt.slot, 1);
                     }
-                    t = __shfl_sync(FULL, t, 0);
+                    t = __shfl_sync(FULL, t, 1);
                     if (t == P - 1) {  // this warp completed the row: merge the P unit results
-                        if (lane == 0) a.tickets[mt.slot] = 0;
-                        __threadfence();
+                        if (lane == 1) a.tickets[mt.slot] = 0;
                         float cm = -INFINITY, cs = 0.0f;
                         int ci = 0x7FFFFFFF;
                         for (int q = lane; q < P; q += 32) {
@@ -318,8 +318,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
 
     // ---------------- self-reset of the counters by the last warp of the grid
     if (lane == 0) {
-        __threadfence();
-        const int d = atomicAdd(a.ctrs + 1, 1);
+        const int d = atom_add_acq_rel_gpu(a.ctrs + 1, 1);
         if (d == total_warps - 1) {
             a.ctrs[0] = 0;
             a.ctrs[1] = 0;
