@@ -54,6 +54,7 @@ def parse_args():
     ap.add_argument("--cpu-sample-rows", type=int, default=512)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--verbose", action="store_true", help="per-launch table of the step kernel on stderr")
     return ap.parse_args()
 
 
@@ -294,6 +295,10 @@ def main():
                 step_ms.append(a.elapsed_time(b))
                 step_bytes.append(n_k[k] * sz_logit + distinct_k[k] * sz_mask)
                 step_rows.append(n_k[k])
+    if args.verbose and rank == 0:
+        for k, (mm, bb, rr) in enumerate(zip(step_ms, step_bytes, step_rows)):
+            print(f"  step {k:2d}: n={rr:5d} distinct_states={distinct_k[k]:5d} {1e3 * mm:8.1f} us "
+                  f"{bb / (mm * 1e-3) / 1e9:7.0f} GB/s", file=sys.stderr)
     tot_bytes, tot_ms = sum(step_bytes), sum(step_ms)
     achieved = tot_bytes / (tot_ms * 1e-3) / 1e9
     best = max(bb / (mm * 1e-3) / 1e9 for bb, mm in zip(step_bytes, step_ms))

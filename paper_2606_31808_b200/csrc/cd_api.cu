@@ -44,10 +44,11 @@ cd_status fail(cd_status st, const char* fmt, ...) {
     } while (0)
 
 // Launch shapes of the step kernel: warps per CTA (one CTA per SM), ring stages per warp, tile
-// bytes.  Variant 0 is the product default; the others exist for tuning runs
-// (environment variable CD_STEP_VARIANT, read once).
+// bytes.  Variant 0 (12 warps x 2 stages x 8 KiB = 192 KiB of logits in flight per SM) is the
+// product default: best or within noise of best on configs c1-c4 (profiles/r1_variant_sweep.md).
+// The others exist for tuning runs (environment variable CD_STEP_VARIANT, read once).
 struct StepCfg { int warps, stages, tile_bytes; };
-constexpr StepCfg STEP_CFGS[] = {{16, 3, 4096}, {8, 4, 4096}, {8, 3, 8192}, {12, 2, 8192}, {16, 2, 4096}, {12, 4, 4096}};
+constexpr StepCfg STEP_CFGS[] = {{12, 2, 8192}, {16, 3, 4096}, {8, 3, 8192}, {13, 2, 8192}, {6, 2, 16384}, {24, 2, 4096}};
 constexpr int N_STEP_CFGS = sizeof(STEP_CFGS) / sizeof(STEP_CFGS[0]);
 
 int step_variant() {
@@ -229,11 +230,37 @@ cd_status launch_step_v(const cd::StepArgs& a, int grid, cudaStream_t stream) {
     }
 }
 
+// Decode-loop extras of a step launch: per-row history + fused compaction (cd_step.cuh).
+struct LoopExtras {
+    int* tokens = nullptr;
+    int* len = nullptr;
+    int* final_state = nullptr;
+    float* sum_logprob = nullptr;
+    uint8_t* done = nullptr;
+    int step = 0, max_steps = 0;
+    int* row_ids_out = nullptr;
+    int* state_out = nullptr;
+    int* n_out = nullptr;
+};
+
 // n_upper bounds the active count; n_dev (device int) overrides n inside the kernel.
 cd_status launch_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype dtype, long long ld,
                       const int* row_map, int* state, int n_upper, const int* n_dev, int* token_out,
-                      float* logprob_out, float* lse_out, uint8_t* done_out, cudaStream_t stream) {
+                      float* logprob_out, float* lse_out, uint8_t* done_out, cudaStream_t stream,
+                      const LoopExtras* x = nullptr) {
     cd::StepArgs a{};
+    if (x) {
+        a.hist_tokens = x->tokens;
+        a.hist_len = x->len;
+        a.hist_final_state = x->final_state;
+        a.hist_sum_logprob = x->sum_logprob;
+        a.hist_done = x->done;
+        a.step = x->step;
+        a.max_steps = x->max_steps;
+        a.cmp_row_ids_out = x->row_ids_out;
+        a.cmp_state_out = x->state_out;
+        a.cmp_n_out = x->n_out;
+    }
     a.dfa = d->dev;
     a.logits = static_cast<const unsigned char*>(logits);
     a.ld_bytes = ld * (dtype == CD_BF16 ? 2 : 4);
@@ -359,16 +386,6 @@ cd_status compile_impl(int32_t V, int32_t S, int32_t start, const int64_t* row_p
     return CD_OK;
 }
 
-cd_status launch_compact(bool record, const cd::CompactArgs& a, cudaStream_t stream) {
-    if (record)
-        cd::compact_kernel<true><<<1, 1024, 0, stream>>>(a);
-    else
-        cd::compact_kernel<false><<<1, 1024, 0, stream>>>(a);
-    CU(cudaGetLastError());
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    return CD_OK;
-}
-
 cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, int* tokens_out, int* len_out,
                            int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream) {
     long long work = (long long)B * (max_steps > 0 ? max_steps : 1);
@@ -383,33 +400,25 @@ cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, in
     return CD_OK;
 }
 
-// One loop iteration k on `logits` ([B, ld], original row ids): step + record/compact.
+// One loop iteration k on `logits` ([B, ld], original row ids): ONE launch -- the step kernel
+// records the per-row history as rows finalise and its last CTA compacts the active list.
 cd_status enqueue_loop_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype dtype, long long ld, int B,
                             int k, int max_steps, int* tokens_out, int* len_out, int* final_state_out,
                             float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream) {
     const int cur = k & 1, nxt = cur ^ 1;
-    cd_status st = launch_step(d, s, logits, dtype, ld, s->row_ids[cur], s->state[cur], B, s->n_active + cur,
-                               s->token, s->logprob, nullptr, s->done, stream);
-    if (st != CD_OK) return st;
-    cd::CompactArgs c{};
-    c.done = s->done;
-    c.row_ids_in = s->row_ids[cur];
-    c.state_in = s->state[cur];
-    c.n = B;
-    c.n_dev = s->n_active + cur;
-    c.row_ids_out = s->row_ids[nxt];
-    c.state_out = s->state[nxt];
-    c.n_active_out = s->n_active + nxt;
-    c.token = s->token;
-    c.logprob = s->logprob;
-    c.step = k;
-    c.max_steps = max_steps;
-    c.tokens_out = tokens_out;
-    c.len_out = len_out;
-    c.final_state_out = final_state_out;
-    c.sum_logprob_out = sum_logprob_out;
-    c.done_row_out = done_out;
-    return launch_compact(true, c, stream);
+    LoopExtras x;
+    x.tokens = tokens_out;
+    x.len = len_out;
+    x.final_state = final_state_out;
+    x.sum_logprob = sum_logprob_out;
+    x.done = done_out;
+    x.step = k;
+    x.max_steps = max_steps;
+    x.row_ids_out = s->row_ids[nxt];
+    x.state_out = s->state[nxt];
+    x.n_out = s->n_active + nxt;
+    return launch_step(d, s, logits, dtype, ld, s->row_ids[cur], s->state[cur], B, s->n_active + cur, s->token,
+                       s->logprob, nullptr, s->done, stream, &x);
 }
 
 cd_status check_sticky_errors(Scratch* s, cudaStream_t stream) {
@@ -567,15 +576,11 @@ cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, const int32
     if (!n_active_out) return fail(CD_ERR_ARG, "n_active_out is NULL");
     if (n > 0 && (!done || !row_ids_out)) return fail(CD_ERR_ARG, "NULL pointer");
     if (n > 0 && state_in && !state_out) return fail(CD_ERR_ARG, "state_in given without state_out");
-    cd::CompactArgs c{};
-    c.done = done;
-    c.row_ids_in = row_ids_in;
-    c.state_in = state_in;
-    c.n = n;
-    c.row_ids_out = row_ids_out;
-    c.state_out = state_out;
-    c.n_active_out = n_active_out;
-    return launch_compact(false, c, static_cast<cudaStream_t>(cuda_stream));
+    cd::compact_kernel<<<1, 1024, 0, static_cast<cudaStream_t>(cuda_stream)>>>(done, row_ids_in, state_in, n, row_ids_out,
+                                                                              state_out, n_active_out);
+    CU(cudaGetLastError());
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return CD_OK;
 }
 
 cd_status cd_decode_loop(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,

@@ -46,78 +46,11 @@ __global__ void transition_kernel(DfaDev dfa, const int* __restrict__ token, int
     }
 }
 
-struct CompactArgs {
-    const uint8_t* done;
-    const int* row_ids_in;  // may be null -> i
-    const int* state_in;    // may be null
-    int n;
-    const int* n_dev;  // if non-null, n is read from the device
-    int* row_ids_out;
-    int* state_out;
-    int* n_active_out;
-    // RECORD only (decode loop): per-slot step results -> per-row history
-    const int* token;
-    const float* logprob;
-    int step, max_steps;
-    int* tokens_out;
-    int* len_out;
-    int* final_state_out;
-    float* sum_logprob_out;
-    uint8_t* done_row_out;
-};
-
-// a6: stable stream compaction by one CTA: warp ballot + lane prefix (popc of lower lanes),
-// warp totals scanned by warp 0, running base carried across 1024-slot chunks.  n <= 4096 in
-// every workload, i.e. at most four chunks.
-template <bool RECORD>
-__global__ void __launch_bounds__(1024, 1) compact_kernel(const CompactArgs a) {
-    __shared__ int warp_off[32];
-    __shared__ int chunk_total;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int n = a.n_dev ? *a.n_dev : a.n;
-    int base = 0;
-    for (int c0 = 0; c0 < n; c0 += 1024) {
-        const int i = c0 + tid;
-        const bool valid = i < n;
-        const uint8_t d = valid ? a.done[i] : 1;
-        const bool keep = valid && (d == 0);
-        int rid = 0, st = 0;
-        if (valid) {
-            rid = a.row_ids_in ? a.row_ids_in[i] : i;
-            if (a.state_in) st = a.state_in[i];
-        }
-        if (RECORD && valid) {
-            a.tokens_out[(long long)rid * a.max_steps + a.step] = a.token[i];
-            a.len_out[rid] = a.step + 1;
-            a.final_state_out[rid] = st;
-            a.sum_logprob_out[rid] += a.logprob[i];
-            a.done_row_out[rid] = d;
-        }
-        const unsigned bal = __ballot_sync(FULL, keep);
-        const int pre = __popc(bal & ((1u << lane) - 1u));
-        if (lane == 0) warp_off[warp] = __popc(bal);
-        __syncthreads();
-        if (warp == 0) {
-            const int v = warp_off[lane];
-            int inc = v;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int u = __shfl_up_sync(FULL, inc, o);
-                if (lane >= o) inc += u;
-            }
-            warp_off[lane] = inc - v;  // exclusive
-            if (lane == 31) chunk_total = inc;
-        }
-        __syncthreads();
-        if (keep) {
-            const int pos = base + warp_off[warp] + pre;
-            a.row_ids_out[pos] = rid;
-            if (a.state_in) a.state_out[pos] = st;
-        }
-        base += chunk_total;
-        __syncthreads();
-    }
-    if (tid == 0) *a.n_active_out = base;
+// a6 as a kernel of its own (cd_compact): one CTA of 1024 threads, see block_compact.
+__global__ void __launch_bounds__(1024, 1) compact_kernel(const uint8_t* done, const int* row_ids_in,
+                                                          const int* state_in, int n, int* row_ids_out,
+                                                          int* state_out, int* n_active_out) {
+    block_compact(done, row_ids_in, state_in, n, row_ids_out, state_out, n_active_out);
 }
 
 // a7 set-up: every row starts in the start state with an empty history.

@@ -169,4 +169,85 @@ __device__ __forceinline__ long long warp_csr_find(const int* __restrict__ tok, 
     return b ? lo + (__ffs(b) - 1) : -1;
 }
 
+// ---------------------------------------------------------------- stable compaction
+// Active-row compaction by one CTA: every thread takes 4 consecutive slots,
+// keep flags are counted per thread, prefix-summed over the warp with shuffles, over the warps
+// through shared memory, and the running base is carried across chunks of 4*blockDim slots.
+// Output order = input order (stable).  Inputs are read with ld.cg: in the fused path they were
+// written by other SMs during the same kernel.  blockDim.x must be a multiple of 32, <= 1024.
+__device__ __forceinline__ void block_compact(const uint8_t* __restrict__ done, const int* __restrict__ row_ids_in,
+                                              const int* __restrict__ state_in, int n, int* __restrict__ row_ids_out,
+                                              int* __restrict__ state_out, int* __restrict__ n_active_out) {
+    __shared__ int s_warp[32];
+    __shared__ int s_total;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+    // vector loads need 4-byte aligned flags and 16-byte aligned id / state lists
+    const bool vec_ok = ((reinterpret_cast<uintptr_t>(done) & 3) == 0) &&
+                        (!row_ids_in || (reinterpret_cast<uintptr_t>(row_ids_in) & 15) == 0) &&
+                        (!state_in || (reinterpret_cast<uintptr_t>(state_in) & 15) == 0);
+    int base = 0;
+    for (int c0 = 0; c0 < n; c0 += 4 * (int)blockDim.x) {
+        const int i0 = c0 + 4 * tid;
+        int rid[4], st[4];
+        bool keep[4];
+        if (vec_ok && i0 + 3 < n) {
+            const uint32_t d4 = __ldcg(reinterpret_cast<const uint32_t*>(done + i0));
+#pragma unroll
+            for (int q = 0; q < 4; ++q) keep[q] = ((d4 >> (8 * q)) & 0xFFu) == 0u;
+            if (row_ids_in) {
+                const int4 r4 = __ldcg(reinterpret_cast<const int4*>(row_ids_in + i0));
+                rid[0] = r4.x; rid[1] = r4.y; rid[2] = r4.z; rid[3] = r4.w;
+            } else {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) rid[q] = i0 + q;
+            }
+            if (state_in) {
+                const int4 s4 = __ldcg(reinterpret_cast<const int4*>(state_in + i0));
+                st[0] = s4.x; st[1] = s4.y; st[2] = s4.z; st[3] = s4.w;
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int i = i0 + q;
+                keep[q] = (i < n) && (__ldcg(done + i) == 0);
+                rid[q] = (i < n && row_ids_in) ? __ldcg(row_ids_in + i) : i;
+                st[q] = (i < n && state_in) ? __ldcg(state_in + i) : 0;
+            }
+        }
+        const int cnt = (int)keep[0] + (int)keep[1] + (int)keep[2] + (int)keep[3];
+        int inc = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int u = __shfl_up_sync(FULL, inc, o);
+            if (lane >= o) inc += u;
+        }
+        if (lane == 31) s_warp[warp] = inc;
+        __syncthreads();
+        if (warp == 0) {
+            const int v = (lane < nwarps) ? s_warp[lane] : 0;
+            int w = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int u = __shfl_up_sync(FULL, w, o);
+                if (lane >= o) w += u;
+            }
+            s_warp[lane] = w - v;  // exclusive offset of each warp
+            if (lane == 31) s_total = w;
+        }
+        __syncthreads();
+        int pos = base + s_warp[warp] + inc - cnt;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (keep[q]) {
+                row_ids_out[pos] = rid[q];
+                if (state_in) state_out[pos] = st[q];
+                ++pos;
+            }
+        }
+        base += s_total;
+        __syncthreads();
+    }
+    if (tid == 0) *n_active_out = base;
+}
+
 }  // namespace cd

@@ -46,7 +46,19 @@ struct StepArgs {
     // scratch (per handle+stream)
     int4* partials;  // [units] {m bits, s bits, idx, -}
     int* tickets;    // [rows], zero between launches
-    int* ctrs;       // [0] work counter, [1] finished warps, [2] sticky error count
+    int* ctrs;       // [0] work counter, [1] finished CTAs, [2] sticky error count
+    // decode loop only, all optional:
+    // per-row history, indexed by ORIGINAL row id (= row_map[slot]), written when the row's step is final
+    int* hist_tokens;  // [B, max_steps]
+    int* hist_len;
+    int* hist_final_state;
+    float* hist_sum_logprob;
+    uint8_t* hist_done;
+    int step, max_steps;
+    // fused early-exit compaction by the last CTA: (row_map, state) of not-done slots -> out lists
+    int* cmp_row_ids_out;
+    int* cmp_state_out;
+    int* cmp_n_out;
 };
 
 struct __align__(16) TileMeta {
@@ -107,11 +119,20 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, int slot, int st
         } else {
             atomicAdd(a.ctrs + 2, 1);
         }
+        const uint8_t dn = __ldg(a.dfa.accepting + ns) ? 1 : 0;
         a.state[slot] = ns;
         a.token_out[slot] = token;
         a.logprob_out[slot] = lp;
         if (a.lse_out) a.lse_out[slot] = lse;
-        a.done_out[slot] = __ldg(a.dfa.accepting + ns) ? 1 : 0;
+        a.done_out[slot] = dn;
+        if (a.hist_tokens) {  // decode loop: this slot's row, original id
+            const long long rid = a.row_map ? __ldg(a.row_map + slot) : slot;
+            a.hist_tokens[rid * a.max_steps + a.step] = token;
+            a.hist_len[rid] = a.step + 1;
+            a.hist_final_state[rid] = ns;
+            a.hist_sum_logprob[rid] += lp;
+            a.hist_done[rid] = dn;
+        }
     }
 }
 
@@ -316,14 +337,20 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
         issue_one();
     }
 
-    // ---------------- self-reset of the counters by the last warp of the grid
-    if (lane == 0) {
+    // ---------------- last CTA of the grid: reset the counters, then (decode loop) compact
+    __shared__ int s_is_last;
+    __syncthreads();
+    if (threadIdx.x == 0) {
         const int d = atom_add_acq_rel_gpu(a.ctrs + 1, 1);
-        if (d == total_warps - 1) {
+        s_is_last = (d == (int)gridDim.x - 1) ? 1 : 0;
+        if (s_is_last) {
             a.ctrs[0] = 0;
             a.ctrs[1] = 0;
         }
     }
+    __syncthreads();
+    if (s_is_last && a.cmp_row_ids_out)
+        block_compact(a.done_out, a.row_map, a.state, n, a.cmp_row_ids_out, a.cmp_state_out, a.cmp_n_out);
 }
 
 }  // namespace cd
