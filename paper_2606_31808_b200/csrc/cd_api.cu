@@ -65,9 +65,9 @@ int step_variant() {
 struct Scratch {
     int cap_rows = 0;
     long long cap_units = 0;
-    int4* partials = nullptr;
+    cd::PartialSlot* partials = nullptr;
     int* tickets = nullptr;
-    int* ctrs = nullptr;  // [0] work, [1] finished warps, [2] sticky errors, [3] spare
+    int* ctrs = nullptr;  // [0] work, [1] finished CTAs, [2] sticky errors, [3] launch generation
     // decode loop
     int* row_ids[2] = {nullptr, nullptr};
     int* state[2] = {nullptr, nullptr};
@@ -169,10 +169,12 @@ cd_status get_scratch(const cd_dfa* cd_, cudaStream_t stream, int rows, bool loo
         Scratch old = s;
         s.cap_rows = 0;
         const long long units = step_units_cap(d, rows);
-        CU(cudaMalloc(&s.partials, sizeof(int4) * units));
-        CU(cudaMalloc(&s.tickets, sizeof(int) * (size_t)rows));
+        CU(cudaMalloc(&s.partials, sizeof(cd::PartialSlot) * units));
         CU(cudaMalloc(&s.ctrs, sizeof(int) * 4));
+        CU(cudaMalloc(&s.tickets, sizeof(int) * (size_t)rows));
         CU(cudaMemset(s.tickets, 0, sizeof(int) * (size_t)rows));
+        CU(cudaMemset(s.partials, 0, sizeof(cd::PartialSlot) * units));  // generation tags start at 0 ...
+        sticky[3] = 1;                                                    // ... launches at 1
         CU(cudaMemcpy(s.ctrs, sticky, sizeof sticky, cudaMemcpyHostToDevice));
         for (int i = 0; i < 2; ++i) {
             CU(cudaMalloc(&s.row_ids[i], sizeof(int) * (size_t)rows));
@@ -360,7 +362,9 @@ cd_status compile_impl(int32_t V, int32_t S, int32_t start, const int64_t* row_p
             long long blocks = ((long long)S * 32 + threads - 1) / threads;
             if (blocks > 65535) blocks = 65535;
             cd::build_mask_kernel<<<(int)blocks, threads>>>(static_cast<const long long*>(d->d_row_ptr),
-                                                           static_cast<const int*>(d->d_tok), S, Wpad,
+                                                           static_cast<const int*>(d->d_tok),
+                                                           static_cast<int*>(d->d_next),
+                                                           static_cast<const uint8_t*>(d->d_acc), S, Wpad,
                                                            static_cast<uint32_t*>(d->d_mask));
             g_launches.fetch_add(1, std::memory_order_relaxed);
             e2 = cudaGetLastError();

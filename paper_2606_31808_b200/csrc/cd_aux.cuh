@@ -5,8 +5,10 @@
 
 namespace cd {
 
-// a0: CSR -> packed allowed-token bitmask.  One warp per state; mask is pre-zeroed.
+// a0: CSR -> packed allowed-token bitmask, and accepting[next] folded into bit 31 of next[]
+// (saves one dependent load per row in the step kernel).  One warp per state; mask pre-zeroed.
 __global__ void build_mask_kernel(const long long* __restrict__ row_ptr, const int* __restrict__ tok,
+                                  int* __restrict__ next, const uint8_t* __restrict__ accepting,
                                   int S, int Wpad, uint32_t* __restrict__ mask) {
     const int lane = threadIdx.x & 31;
     const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -17,6 +19,8 @@ __global__ void build_mask_kernel(const long long* __restrict__ row_ptr, const i
         for (long long j = lo + lane; j < hi; j += 32) {
             const int t = tok[j];
             atomicOr(row + (t >> 5), 1u << (t & 31));
+            const int ns = next[j];
+            next[j] = ns | (accepting[ns] ? (int)0x80000000 : 0);
         }
     }
 }
@@ -34,7 +38,7 @@ __global__ void transition_kernel(DfaDev dfa, const int* __restrict__ token, int
         if (st >= 0 && st < dfa.S) {
             if (t >= 0) {
                 const long long j = warp_csr_find(dfa.tok, dfa.row_ptr[st], dfa.row_ptr[st + 1], t, lane);
-                if (j >= 0) ns = dfa.next[j];
+                if (j >= 0) ns = dfa.next[j] & 0x7FFFFFFF;  // bit 31 carries accepting[next]
             }
             if (lane == 0) {
                 state[i] = ns;

@@ -19,7 +19,7 @@ struct DfaDev {
     const uint32_t* mask;      // [S][Wpad], LSB-first: token t <-> bit (t & 31) of word (t >> 5)
     const long long* row_ptr;  // [S + 1]
     const int* tok;            // [nnz] strictly increasing inside a state
-    const int* next;           // [nnz]
+    const int* next;           // [nnz] next state | (accepting[next state] << 31)
     const uint8_t* accepting;  // [S]
 };
 
@@ -147,19 +147,25 @@ __device__ __forceinline__ void warp_combine(float& m, float& s, int& idx) {
 }
 
 // ---------------------------------------------------------------- CSR transition lookup
-// Warp-cooperative 32-ary search of `token` in the sorted CSR row tok[lo, hi): every round the
-// 32 lanes probe 32 split points, so a 5,243-entry row (configs[3]) takes 2 rounds + 1 final
-// compare instead of 13 dependent probes.  Returns the position or -1.  All lanes return the
-// same value.
+// Warp-cooperative 128-ary search of `token` in the sorted CSR row tok[lo, hi): every round each
+// lane probes 4 of 128 split points (independent loads), so a row of <= 4096 entries needs one
+// round plus the final 32-wide compare, a 5,243-entry row (configs[3]) two: 2-3 dependent
+// memory latencies instead of 13 for a binary search.  Returns the position or -1; all lanes
+// return the same value.
 __device__ __forceinline__ long long warp_csr_find(const int* __restrict__ tok, long long lo,
                                                    long long hi, int token, int lane) {
     while (hi - lo > 32) {
-        const long long step = (hi - lo + 31) >> 5;
-        const long long q = lo + (long long)lane * step;
-        const bool le = (q < hi) && (__ldg(tok + q) <= token);
-        const unsigned b = __ballot_sync(FULL, le);
-        if (b == 0) return -1;  // token below the first entry
-        const int c = __popc(b);
+        const long long step = (hi - lo + 127) >> 7;
+        int v[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const long long q = lo + (long long)(lane * 4 + k) * step;
+            v[k] = (q < hi) ? __ldg(tok + q) : 0x7FFFFFFF;
+        }
+        int c = 0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) c += __popc(__ballot_sync(FULL, v[k] <= token));
+        if (c == 0) return -1;  // token below the first entry
         lo = lo + (long long)(c - 1) * step;
         hi = (lo + step < hi) ? lo + step : hi;
     }
@@ -167,6 +173,16 @@ __device__ __forceinline__ long long warp_csr_find(const int* __restrict__ tok, 
     const bool eq = (q < hi) && (__ldg(tok + q) == token);
     const unsigned b = __ballot_sync(FULL, eq);
     return b ? lo + (__ffs(b) - 1) : -1;
+}
+
+// Relaxed device-scope 64-bit accesses for the tagged partial-result slots (cd_step.cuh).
+__device__ __forceinline__ void st_relaxed_gpu_u64(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_relaxed_gpu_u64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
 }
 
 // ---------------------------------------------------------------- stable compaction

@@ -1,23 +1,33 @@
-// cd_step.cuh -- the fused constrained step (SURVEY 8(a) a1-a5; include/cd.h cd_step).
+// cd_step.cuh -- the fused constrained step (SURVEY 8(a) a1-a7; include/cd.h cd_step).
 //
 // Design (B200-first; the paper gives no kernel):
 //   * The step is one streaming pass over the logits, so it is HBM-bound: the job is to keep
 //     enough bytes in flight and to waste no issue slots.  Every WARP owns a private ring of
 //     STAGES shared-memory slots that it fills itself with 1-D bulk async copies (TMA engine,
-//     cp.async.bulk -> SASS UBLKCP) completing on per-slot mbarriers: a 4 KiB logits tile
-//     and the matching piece of the state's allowed-token bitmask land together.  No register
-//     staging, no block-wide barriers, WARPS*STAGES*4 KiB in flight per SM.
+//     cp.async.bulk -> SASS UBLKCP) completing on per-slot mbarriers: a logits tile and the
+//     matching piece of the state's allowed-token bitmask land together.  No register staging,
+//     no block-wide barriers in the streaming phase, WARPS*STAGES*TILE_BYTES in flight per SM.
 //   * Work unit = (active slot, part of the row).  Units are handed out by one global atomic
-//     counter (dynamic balance across the 148 SMs; the two dies do not run at the same speed),
+//     counter (dynamic balance across the 148 SMs; the two dies do not run at the same speed);
 //     the number of tiles per unit is derived on the device from the number of active rows, so
 //     the same launch shape serves a full batch and the few-rows tail of an early-exit loop
 //     without any host read of the active count.
-//   * Per tile a lane walks the set bits of its mask words and updates an online
-//     (max, sum-exp, argmax) triple; only allowed elements cost arithmetic.
-//   * Unit results of a row are merged by whichever warp finishes the row's last unit (ticket
-//     counter per slot); that warp also does the CSR transition (32-ary warp search), the
-//     accept test and the output writes, while the other warps keep streaming.
-//   * Tickets and the work counter are self-resetting, so a launch needs no memset.
+//   * Per tile a lane walks the set bits of its mask words (warp-uniform trip count, branch
+//     free body) and updates an online (max, sum-exp, argmax) triple; only allowed elements
+//     cost arithmetic.
+//   * Unit results of a row are merged without any fence: a unit stores its result into a slot
+//     of three 64-bit words, each carrying the launch generation in its upper half (8-byte
+//     stores are single-copy atomic, so a word is either stale or complete), then takes a
+//     RELAXED ticket.  The warp that draws the last ticket merges: it reads the other slots and
+//     re-reads any word whose tag is not current yet (the writers issued those stores before
+//     their tickets, so they are on their way; normally the first read succeeds).  A
+//     __threadfence here cost 3.8 us per unit (profiles/r1b): it waits for the bulk copies the
+//     same warp still has in flight.
+//   * That warp also does the CSR transition (128-ary warp search; row bounds were prefetched
+//     into the tile meta, accepting[next] rides in bit 31 of next[]), the output writes and, in
+//     the decode loop, the per-row history, while the other warps keep streaming.
+//   * The last CTA to finish resets the work counter, bumps the generation and, in the decode
+//     loop, performs the stable early-exit compaction: one launch per decoding step.
 #pragma once
 #include "cd_common.cuh"
 
@@ -30,6 +40,11 @@ constexpr int FLAG_FIRST = 1;   // first tile of its unit: reset the lane accumu
 constexpr int FLAG_LAST = 2;    // last tile of its unit: reduce and publish
 constexpr int FLAG_ACCEPT = 4;  // pseudo tile of a slot whose state already accepts (no copy)
 constexpr int FLAG_BADSTATE = 8;
+
+// Result of one unit, readable without a fence: {gen:32 | payload:32} x 3 (+ pad to 32 B).
+struct __align__(32) PartialSlot {
+    unsigned long long m, s, idx, pad;
+};
 
 struct StepArgs {
     DfaDev dfa;
@@ -44,9 +59,9 @@ struct StepArgs {
     float* lse_out;
     uint8_t* done_out;
     // scratch (per handle+stream)
-    int4* partials;  // [units] {m bits, s bits, idx, -}
-    int* tickets;    // [rows], zero between launches
-    int* ctrs;       // [0] work counter, [1] finished CTAs, [2] sticky error count
+    PartialSlot* partials;  // [units]
+    int* tickets;           // [rows] arrivals per slot, zero between launches
+    int* ctrs;              // [0] work counter, [1] finished CTAs, [2] sticky error count, [3] generation
     // decode loop only, all optional:
     // per-row history, indexed by ORIGINAL row id (= row_map[slot]), written when the row's step is final
     int* hist_tokens;  // [B, max_steps]
@@ -66,6 +81,9 @@ struct __align__(16) TileMeta {
     int tile;   // tile index inside the row
     int flags;  // FLAG_* | part << 8
     int st;     // automaton state of the slot
+    long long csr_lo;  // row_ptr[st]
+    int csr_len;       // row_ptr[st + 1] - row_ptr[st]
+    int pad;
 };
 
 template <int STAGES, int TILE_BYTES>
@@ -96,9 +114,9 @@ __device__ __forceinline__ float tile_elem(const unsigned char* tile, int e) {
 }
 
 // Row finished: (m, s, idx) is the merged result of all its units.  Warp-uniform.
-__device__ __forceinline__ void finalize_row(const StepArgs& a, int slot, int st, float m, float s,
-                                             int idx, int lane) {
-    const long long lo = __ldg(a.dfa.row_ptr + st), hi = __ldg(a.dfa.row_ptr + st + 1);
+__device__ __forceinline__ void finalize_row(const StepArgs& a, const TileMeta& mt, float m, float s, int idx,
+                                             int lane) {
+    const long long lo = mt.csr_lo, hi = mt.csr_lo + mt.csr_len;
     int token;
     float lp, lse;
     if (m == -INFINITY) {  // every allowed logit is -inf: lowest allowed id (G6)
@@ -113,13 +131,17 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, int slot, int st
     }
     const long long j = warp_csr_find(a.dfa.tok, lo, hi, token, lane);
     if (lane == 0) {
-        int ns = st;
+        const int slot = mt.slot;
+        int ns = mt.st;
+        uint8_t dn;
         if (j >= 0) {
-            ns = __ldg(a.dfa.next + j);
+            const int packed = __ldg(a.dfa.next + j);  // next state | accepting << 31
+            ns = packed & 0x7FFFFFFF;
+            dn = (packed < 0) ? 1 : 0;
         } else {
             atomicAdd(a.ctrs + 2, 1);
+            dn = 1;
         }
-        const uint8_t dn = __ldg(a.dfa.accepting + ns) ? 1 : 0;
         a.state[slot] = ns;
         a.token_out[slot] = token;
         a.logprob_out[slot] = lp;
@@ -157,7 +179,11 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     }
     __syncwarp();
 
-    const int n = a.n_dev ? __ldg(a.n_dev) : a.n;
+    // ---------------- issue side (warp-uniform state)
+    int next_u_l0 = 0;  // prefetched unit id, valid in lane 0
+    if (lane == 0) next_u_l0 = atomicAdd(a.ctrs + 0, 1);
+    const unsigned gen = (unsigned)__ldcg(a.ctrs + 3);  // launch generation (tag of the partial slots)
+    const int n = a.n_dev ? __ldcg(a.n_dev) : a.n;
     const int V = a.dfa.V;
     const int tiles_per_row = (V + TILE_TOK - 1) / TILE_TOK;
     const int total_warps = gridDim.x * WARPS;
@@ -167,12 +193,10 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     const bool ragged_row = (V % TILE_TOK) != 0;
     const uint64_t pol_stream = l2_policy_evict_first();
 
-    // ---------------- issue side (warp-uniform state)
-    int next_u_l0 = 0;  // prefetched unit id, valid in lane 0
-    if (lane == 0) next_u_l0 = atomicAdd(a.ctrs + 0, 1);
     bool exhausted = false;
     int iss_tile = 0, iss_end = 0;
-    int iss_slot = 0, iss_st = 0, iss_flags = 0;
+    int iss_slot = 0, iss_st = 0, iss_flags = 0, iss_len = 0;
+    long long iss_lo = 0;
     const unsigned char* iss_src = nullptr;  // next logits tile of the current unit
     const unsigned char* iss_msk = nullptr;  // next mask piece
     int iss_stage = 0, in_flight = 0;
@@ -188,12 +212,17 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
             if (lane == 0) next_u_l0 = atomicAdd(a.ctrs + 0, 1);
             iss_slot = u / P;
             const int part = u - iss_slot * P;
-            iss_st = a.state[iss_slot];  // updated only after every unit of the slot has arrived
+            iss_st = a.state[iss_slot];  // rewritten only after every unit of the slot has been merged
+            const long long r = a.row_map ? (long long)__ldg(a.row_map + iss_slot) : (long long)iss_slot;
             const bool bad = (iss_st < 0) || (iss_st >= a.dfa.S);
-            const bool acc = !bad && (__ldg(a.dfa.accepting + iss_st) != 0);
+            const int sts = bad ? 0 : iss_st;
+            const bool acc = !bad && (__ldg(a.dfa.accepting + sts) != 0);
+            iss_lo = __ldg(a.dfa.row_ptr + sts);
+            iss_len = (int)(__ldg(a.dfa.row_ptr + sts + 1) - iss_lo);
             if (bad || acc) {
                 if (lane == 0) {
-                    ring.meta[iss_stage] = TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (part << 8), iss_st};
+                    ring.meta[iss_stage] =
+                        TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (part << 8), iss_st, 0, 0, 0};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
                 iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
@@ -201,7 +230,6 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 iss_tile = iss_end = 0;
                 return;
             }
-            const long long r = a.row_map ? (long long)__ldg(a.row_map + iss_slot) : (long long)iss_slot;
             iss_tile = part * tpu;
             iss_end = min(iss_tile + tpu, tiles_per_row);
             iss_src = a.logits + r * a.ld_bytes + (long long)iss_tile * TILE_BYTES;
@@ -223,7 +251,8 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
             const int e = (int)(bulk / SZ) + lane;
             if (e < ntok) {
                 if (DT == DT_BF16)
-                    reinterpret_cast<uint16_t*>(ring.logits[iss_stage])[e] = reinterpret_cast<const uint16_t*>(iss_src)[e];
+                    reinterpret_cast<uint16_t*>(ring.logits[iss_stage])[e] =
+                        reinterpret_cast<const uint16_t*>(iss_src)[e];
                 else
                     reinterpret_cast<float*>(ring.logits[iss_stage])[e] = reinterpret_cast<const float*>(iss_src)[e];
             }
@@ -231,13 +260,13 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 reinterpret_cast<uint32_t*>(ring.mask[iss_stage])[w] = 0u;
             __syncwarp();
             if (lane == 0) {
-                ring.meta[iss_stage] = TileMeta{iss_slot, iss_tile, fl, iss_st};
+                ring.meta[iss_stage] = TileMeta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, 0};
                 mbar_arrive_expect_tx(bar, bulk + mbytes);
                 if (bulk) bulk_g2s_hint(dst, iss_src, bulk, bar, pol_stream);
                 bulk_g2s(mdst, iss_msk, mbytes, bar);
             }
         } else if (lane == 0) {
-            ring.meta[iss_stage] = TileMeta{iss_slot, iss_tile, fl, iss_st};
+            ring.meta[iss_stage] = TileMeta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, 0};
             mbar_arrive_expect_tx(bar, TILE_BYTES + MASK_BYTES);
             bulk_g2s_hint(dst, iss_src, TILE_BYTES, bar, pol_stream);
             bulk_g2s(mdst, iss_msk, MASK_BYTES, bar);
@@ -258,6 +287,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     int idx = 0x7FFFFFFF;
     int cons_stage = 0;
     uint32_t cons_phase = 0;
+    const unsigned long long tag = (unsigned long long)gen << 32;
 
 #pragma unroll 1
     while (in_flight > 0) {
@@ -305,27 +335,55 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 int ri = idx;
                 warp_combine(rm, rs, ri);
                 if (P == 1) {
-                    finalize_row(a, mt.slot, mt.st, rm, rs, ri, lane);
+                    finalize_row(a, mt, rm, rs, ri, lane);
                 } else {
-                    // Publish from lane 1, not lane 0: lane 0 issues the bulk copies and a
-                    // release by that thread would wait for its copies still in flight.
+                    // Publish from lane 1 (lane 0 is busy issuing copies): three self-validating
+                    // words, then a RELAXED ticket -- no fence anywhere.  The last arriver merges.
                     int t = 0;
                     if (lane == 1) {
-                        a.partials[(long long)mt.slot * P + part] =
-                            make_int4(__float_as_int(rm), __float_as_int(rs), ri, 0);
-                        t = atom_add_acq_rel_gpu(a.tickets + mt.slot, 1);
+                        PartialSlot* ps = a.partials + ((long long)mt.slot * P + part);
+                        st_relaxed_gpu_u64(&ps->m, tag | (unsigned)__float_as_int(rm));
+                        st_relaxed_gpu_u64(&ps->s, tag | (unsigned)__float_as_int(rs));
+                        st_relaxed_gpu_u64(&ps->idx, tag | (unsigned)ri);
+                        t = atomicAdd(a.tickets + mt.slot, 1);
                     }
                     t = __shfl_sync(FULL, t, 1);
-                    if (t == P - 1) {  // this warp completed the row: merge the P unit results
+                    if (t == P - 1) {
                         if (lane == 1) a.tickets[mt.slot] = 0;
-                        float cm = -INFINITY, cs = 0.0f;
-                        int ci = 0x7FFFFFFF;
-                        for (int q = lane; q < P; q += 32) {
-                            const int4 v = __ldcg(a.partials + (long long)mt.slot * P + q);
-                            online_combine(cm, cs, ci, __int_as_float(v.x), __int_as_float(v.y), v.z);
+                        // The other units' words were stored before their tickets, but nothing
+                        // orders them: poll until every tag is current (normally the first read).
+                        const PartialSlot* base = a.partials + (long long)mt.slot * P;
+                        // Merge in slot order whoever merges (bitwise reproducible): lane q%32 takes
+                        // slot q; the own result (identical in every lane after the butterfly) stands
+                        // in for slot `part`.
+                        const float om = rm, os = rs;
+                        const int oi = ri;
+                        rm = -INFINITY;
+                        rs = 0.0f;
+                        ri = 0x7FFFFFFF;
+                        for (int q0 = 0; q0 < P; q0 += 32) {
+                            const int q = q0 + lane;
+                            const bool want = (q < P) && (q != part);
+                            bool ok = !want;
+                            unsigned long long wm = 0, ws = 0, wi = 0;
+                            while (true) {
+                                if (!ok) {
+                                    wm = ld_relaxed_gpu_u64(&base[q].m);
+                                    ws = ld_relaxed_gpu_u64(&base[q].s);
+                                    wi = ld_relaxed_gpu_u64(&base[q].idx);
+                                    ok = ((wm >> 32) == gen) && ((ws >> 32) == gen) && ((wi >> 32) == gen);
+                                }
+                                if (__all_sync(FULL, ok)) break;
+                                __nanosleep(32);
+                            }
+                            if (want)
+                                online_combine(rm, rs, ri, __int_as_float((int)(unsigned)wm),
+                                               __int_as_float((int)(unsigned)ws), (int)(unsigned)wi);
+                            else if (q == part)
+                                online_combine(rm, rs, ri, om, os, oi);
                         }
-                        warp_combine(cm, cs, ci);
-                        finalize_row(a, mt.slot, mt.st, cm, cs, ci, lane);
+                        warp_combine(rm, rs, ri);
+                        finalize_row(a, mt, rm, rs, ri, lane);
                     }
                 }
             }
@@ -346,6 +404,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
         if (s_is_last) {
             a.ctrs[0] = 0;
             a.ctrs[1] = 0;
+            a.ctrs[3] = (int)(gen + 1u);
         }
     }
     __syncthreads();
