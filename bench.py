@@ -40,7 +40,10 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for this
 # workload); keyed by config name.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {
+    # profiles/r1c_step_kernel_c4.md, step 0 (n = 4096): 2,148,744,000 read + 4,729,344 written
+    "c4": 2148744000 + 4729344,
+}
 
 
 def parse_args():
@@ -361,7 +364,7 @@ def main():
         while True:
             res = oracle.decode_loop(aut, sub)
             reps += 1
-            if time.perf_counter() - t0 > 10.0 or reps >= 50:
+            if time.perf_counter() - t0 > 12.0 or reps >= 400:
                 break
         dt = time.perf_counter() - t0
         cpu = {"value": R * reps / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
