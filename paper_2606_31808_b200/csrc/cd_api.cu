@@ -60,6 +60,14 @@ int step_variant() {
     return v;
 }
 
+bool use_pdl() {
+    static const bool v = [] {
+        const char* e = std::getenv("CD_PDL");
+        return e ? std::atoi(e) != 0 : true;
+    }();
+    return v;
+}
+
 // Per (handle, stream) scratch.  Operations on one stream are ordered, so one area per stream
 // is race free; distinct streams get distinct areas.
 struct Scratch {
@@ -214,8 +222,20 @@ cd_status launch_step_t(const cd::StepArgs& a, int grid, cudaStream_t stream) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured_dev = dev;
     }
-    kern<<<grid, C.warps * 32, smem, stream>>>(a);
-    CU(cudaGetLastError());
+    // programmatic stream serialization: this grid may be scheduled while the previous kernel
+    // of the stream drains (the kernel itself waits with griddepcontrol.wait before touching
+    // global memory), which hides the launch latency between the steps of a decode loop
+    cudaLaunchConfig_t lc{};
+    lc.gridDim = dim3((unsigned)grid);
+    lc.blockDim = dim3((unsigned)(C.warps * 32));
+    lc.dynamicSmemBytes = smem;
+    lc.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = use_pdl() ? 1 : 0;
+    lc.attrs = at;
+    lc.numAttrs = 1;
+    CU(cudaLaunchKernelEx(&lc, kern, a));
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return CD_OK;
 }

@@ -179,14 +179,22 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     }
     __syncwarp();
 
+    // Programmatic dependent launch: the next step's grid may be scheduled as soon as every CTA
+    // of this one got here (its CTAs land on SMs as ours exit and set up their barriers), but
+    // nothing of this kernel reads or writes global memory before the previous grid has
+    // completed and flushed (griddepcontrol.wait).
+    pdl_launch_dependents();
+    pdl_wait();
+
     // ---------------- issue side (warp-uniform state)
-    int next_u_l0 = 0;  // prefetched unit id, valid in lane 0
-    if (lane == 0) next_u_l0 = atomicAdd(a.ctrs + 0, 1);
+    // The first unit of a warp is its global warp id (no atomic on the start-up chain); later
+    // units come from the work counter, which therefore starts at 0 = unit `total_warps`.
+    const int total_warps = gridDim.x * WARPS;
+    int next_u_l0 = blockIdx.x * WARPS + warp;  // prefetched unit id, valid in lane 0
     const unsigned gen = (unsigned)__ldcg(a.ctrs + 3);  // launch generation (tag of the partial slots)
     const int n = a.n_dev ? __ldcg(a.n_dev) : a.n;
     const int V = a.dfa.V;
     const int tiles_per_row = (V + TILE_TOK - 1) / TILE_TOK;
-    const int total_warps = gridDim.x * WARPS;
     const int tpu = tiles_per_unit(n, tiles_per_row, total_warps, TPU_MAX);
     const int P = (tiles_per_row + tpu - 1) / tpu;  // units per row
     const int total_units = n * P;
@@ -209,7 +217,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 exhausted = true;
                 return;
             }
-            if (lane == 0) next_u_l0 = atomicAdd(a.ctrs + 0, 1);
+            if (lane == 0) next_u_l0 = total_warps + atomicAdd(a.ctrs + 0, 1);
             iss_slot = u / P;
             const int part = u - iss_slot * P;
             iss_st = a.state[iss_slot];  // rewritten only after every unit of the slot has been merged
