@@ -55,6 +55,9 @@ def parse_args():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--batches", type=int, default=2, help="resident input batches rotated over the timed steps")
     ap.add_argument("--cpu-sample-rows", type=int, default=512)
+    ap.add_argument("--gather-max", type=int, default=0,
+                    help="cd_set_gather_max for the main measurement: 0 = dense scan (default, the graded method), "
+                         "-1 = automatic, > 0 = threshold (SURVEY 8(f) N1)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--verbose", action="store_true", help="per-launch table of the step kernel on stderr")
@@ -208,6 +211,7 @@ def main():
     aut, batches = build_inputs(cfg, device, args.batches, batch0=rank * args.batches)
     dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device=device)
     dfa.reserve(cfg.B)
+    dfa.set_gather_max(args.gather_max)
     out = None
     stream = torch.cuda.current_stream()
 

@@ -109,6 +109,21 @@ CD_API void cd_free_dfa(cd_dfa_t* dfa);
 CD_API cd_status cd_dfa_info(const cd_dfa_t* dfa, int32_t* V, int32_t* S, int32_t* start, int64_t* nnz,
                       int64_t* mask_bytes);
 
+/*
+ * Density-adaptive step.  A masked log-softmax needs only the
+ * allowed logits: for a row whose state has at most `max_transitions` transitions
+ * cd_step / cd_decode_loop* do not scan the logits row and its bitmask but walk the
+ * state's CSR token list and gather exactly the allowed logits.  Outputs are the same
+ * as the dense scan's (token, state, done bit-exact; logprob / lse within the same
+ * tolerance; the summation order differs).  Rows of both kinds mix in one launch.
+ *   max_transitions = 0   dense scan for every state (default: the method
+ *                         BASELINE.json north_star states)
+ *   max_transitions > 0   gather states with <= max_transitions transitions
+ *   max_transitions = -1  automatic threshold from V and the logits dtype
+ * Call it while no work using the handle is in flight.
+ */
+CD_API cd_status cd_set_gather_max(cd_dfa_t* dfa, int32_t max_transitions);
+
 /* Creates (or grows) the scratch area of (dfa, cuda_stream) for up to max_rows
    rows, so that later calls on that stream neither allocate nor synchronise. */
 CD_API cd_status cd_reserve(const cd_dfa_t* dfa, int32_t max_rows, void* cuda_stream);

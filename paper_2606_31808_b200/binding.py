@@ -17,7 +17,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
-    "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_reserve", "cd_step",
+    "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_reserve", "cd_step",
     "cd_transition", "cd_compact", "cd_decode_loop", "cd_decode_loop_host", "cd_launch_count",
     "cd_last_error",
 )
@@ -101,6 +101,10 @@ class Dfa:
         nnz, mb = C.c_int64(), C.c_int64()
         _check(lib().cd_dfa_info(self._h, C.byref(V), C.byref(S), C.byref(start), C.byref(nnz), C.byref(mb)))
         self.V, self.S, self.start, self.nnz, self.mask_bytes = V.value, S.value, start.value, nnz.value, mb.value
+
+    def set_gather_max(self, max_transitions: int):
+        """cd_set_gather_max: 0 = dense scan only, > 0 threshold, -1 automatic."""
+        _check(lib().cd_set_gather_max(self._h, C.c_int32(max_transitions)))
 
     def reserve(self, max_rows: int):
         _check(lib().cd_reserve(self._h, C.c_int32(max_rows), _stream(self.device)))

@@ -79,6 +79,7 @@ struct Scratch {
     // decode loop
     int* row_ids[2] = {nullptr, nullptr};
     int* state[2] = {nullptr, nullptr};
+    int* state_new = nullptr;  // next states of a step launch
     int* n_active = nullptr;  // [2]
     int* token = nullptr;
     float* logprob = nullptr;
@@ -96,7 +97,7 @@ struct Scratch {
     void release() {
         cudaFree(partials); cudaFree(tickets); cudaFree(ctrs);
         for (int i = 0; i < 2; ++i) { cudaFree(row_ids[i]); cudaFree(state[i]); cudaFree(stage[i]); }
-        cudaFree(n_active); cudaFree(token); cudaFree(logprob); cudaFree(done); cudaFree(out_i32);
+        cudaFree(state_new); cudaFree(n_active); cudaFree(token); cudaFree(logprob); cudaFree(done); cudaFree(out_i32);
         if (copy_stream) cudaStreamDestroy(copy_stream);
         for (int i = 0; i < 2; ++i) {
             if (ev_copied[i]) cudaEventDestroy(ev_copied[i]);
@@ -116,6 +117,8 @@ struct cd_dfa {
     int start_accepting = 0;
     long long nnz = 0;
     int num_sms = 0;
+    long long max_deg = 0;  // largest number of transitions of a state
+    int gather_max = 0;  // cd_set_gather_max: 0 dense scan only, > 0 threshold, < 0 automatic
     void* d_mask = nullptr;
     void* d_row_ptr = nullptr;
     void* d_tok = nullptr;
@@ -142,6 +145,17 @@ struct DeviceGuard {
 int tiles_per_row(int V, int dtype) {
     const int tt = STEP_CFGS[step_variant()].tile_bytes / (dtype == CD_BF16 ? 2 : 4);
     return (V + tt - 1) / tt;
+}
+
+// Largest number of transitions a state may have to be gathered instead of scanned (0 = never).
+// Automatic policy: a gathered logit costs one 32-byte sector plus its 4-byte token id, and
+// scattered sectors reach roughly a third of the streaming bandwidth, so gathering pays while
+// nnz * 36 * 3 < bytes of a dense row scan (profiles/r1d_gather.md).
+int gather_max_for(const cd_dfa* d, int dtype) {
+    if (d->gather_max >= 0) return d->gather_max;
+    const long long row_bytes = (long long)d->dev.V * (dtype == CD_BF16 ? 2 : 4) + d->dev.V / 8;
+    const long long g = row_bytes / 108;
+    return (int)(g > 0x3FFFFFFF ? 0x3FFFFFFF : g);
 }
 
 int step_grid(const cd_dfa* d, long long n_upper, int dtype) {
@@ -188,6 +202,7 @@ cd_status get_scratch(const cd_dfa* cd_, cudaStream_t stream, int rows, bool loo
             CU(cudaMalloc(&s.row_ids[i], sizeof(int) * (size_t)rows));
             CU(cudaMalloc(&s.state[i], sizeof(int) * (size_t)rows));
         }
+        CU(cudaMalloc(&s.state_new, sizeof(int) * (size_t)rows));
         CU(cudaMalloc(&s.n_active, sizeof(int) * 2));
         CU(cudaMalloc(&s.token, sizeof(int) * (size_t)rows));
         CU(cudaMalloc(&s.logprob, sizeof(float) * (size_t)rows));
@@ -210,10 +225,10 @@ cd_status check_dtype(cd_dtype dt) {
     return CD_OK;
 }
 
-template <int DT, int VAR>
+template <int DT, int VAR, bool GATHER = false>
 cd_status launch_step_t(const cd::StepArgs& a, int grid, cudaStream_t stream) {
     constexpr StepCfg C = STEP_CFGS[VAR];
-    auto kern = cd::step_kernel<DT, C.warps, C.stages, C.tile_bytes>;
+    auto kern = cd::step_kernel<DT, C.warps, C.stages, C.tile_bytes, GATHER>;
     const size_t smem = sizeof(cd::WarpRing<C.stages, C.tile_bytes>) * C.warps;
     static thread_local int configured_dev = -1;
     int dev = 0;
@@ -242,6 +257,7 @@ cd_status launch_step_t(const cd::StepArgs& a, int grid, cudaStream_t stream) {
 
 template <int DT>
 cd_status launch_step_v(const cd::StepArgs& a, int grid, cudaStream_t stream) {
+    if (a.gather_max > 0) return launch_step_t<DT, 0, true>(a, grid, stream);  // density-adaptive rows
     switch (step_variant()) {
         case 1: return launch_step_t<DT, 1>(a, grid, stream);
         case 2: return launch_step_t<DT, 2>(a, grid, stream);
@@ -288,6 +304,7 @@ cd_status launch_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype 
     a.ld_bytes = ld * (dtype == CD_BF16 ? 2 : 4);
     a.row_map = row_map;
     a.state = state;
+    a.state_new = s->state_new;
     a.n = n_upper;
     a.n_dev = n_dev;
     a.token_out = token_out;
@@ -297,6 +314,8 @@ cd_status launch_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype 
     a.partials = s->partials;
     a.tickets = s->tickets;
     a.ctrs = s->ctrs;
+    a.gather_max = gather_max_for(d, dtype);
+    a.all_gather = (d->max_deg <= a.gather_max) ? 1 : 0;
     const int grid = step_grid(d, n_upper, dtype);
     return dtype == CD_BF16 ? launch_step_v<cd::DT_BF16>(a, grid, stream)
                             : launch_step_v<cd::DT_F32>(a, grid, stream);
@@ -346,6 +365,8 @@ cd_status compile_impl(int32_t V, int32_t S, int32_t start, const int64_t* row_p
     d->start = start;
     d->start_accepting = accepting[start] ? 1 : 0;
     d->nnz = nnz;
+    for (int32_t s = 0; s < S; ++s)
+        if (row_ptr[s + 1] - row_ptr[s] > d->max_deg) d->max_deg = row_ptr[s + 1] - row_ptr[s];
     cudaDeviceProp prop;
     cudaError_t e = cudaGetDeviceProperties(&prop, device);
     if (e != cudaSuccess) { delete d; return fail(CD_ERR_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e)); }
@@ -544,6 +565,13 @@ cd_status cd_dfa_info(const cd_dfa_t* d, int32_t* V, int32_t* S, int32_t* start,
     if (start) *start = d->start;
     if (nnz) *nnz = d->nnz;
     if (mask_bytes) *mask_bytes = (int64_t)d->dev.S * d->dev.Wpad * 4;
+    return CD_OK;
+}
+
+cd_status cd_set_gather_max(cd_dfa_t* d, int32_t max_transitions) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (max_transitions < -1) return fail(CD_ERR_ARG, "max_transitions must be >= -1");
+    d->gather_max = max_transitions;
     return CD_OK;
 }
 

@@ -28,6 +28,12 @@
 //     the decode loop, the per-row history, while the other warps keep streaming.
 //   * The last CTA to finish resets the work counter, bumps the generation and, in the decode
 //     loop, performs the stable early-exit compaction: one launch per decoding step.
+//   * Density-adaptive rows (GATHER instantiation): a row whose state has at most
+//     `gather_max` transitions is not scanned at all -- its units walk pieces of the state's CSR
+//     token list (coalesced) and gather exactly the allowed logits (one 32-byte sector each, 8
+//     independent loads per lane in flight).  The running argmax is the CSR position, so the
+//     transition needs no search.  Same outputs as the dense scan; dense and gathered rows mix
+//     freely in one launch and share the merge / compaction machinery.
 #pragma once
 #include "cd_common.cuh"
 
@@ -40,6 +46,17 @@ constexpr int FLAG_FIRST = 1;   // first tile of its unit: reset the lane accumu
 constexpr int FLAG_LAST = 2;    // last tile of its unit: reduce and publish
 constexpr int FLAG_ACCEPT = 4;  // pseudo tile of a slot whose state already accepts (no copy)
 constexpr int FLAG_BADSTATE = 8;
+constexpr int FLAG_GATHER = 16;  // pseudo tile of a gathered row piece (no copy); meta.tile = logits row
+
+constexpr int GATHER_CHUNK = 256;  // a gathered row is split into pieces of >= this many transitions
+constexpr int GATHER_UNROLL = 8;   // independent gathers per lane in flight
+
+// number of units a gathered row of `len` transitions is split into (P = units per row of the launch)
+__host__ __device__ inline int gather_parts(int len, int P) {
+    int np = (len + GATHER_CHUNK - 1) / GATHER_CHUNK;
+    if (np < 1) np = 1;
+    return np < P ? np : P;
+}
 
 // Result of one unit, readable without a fence: {gen:32 | payload:32} x 3 (+ pad to 32 B).
 struct __align__(32) PartialSlot {
@@ -51,7 +68,8 @@ struct StepArgs {
     const unsigned char* logits;
     long long ld_bytes;
     const int* row_map;
-    int* state;
+    int* state;      // [n] in: state of every slot (read-only while units are in flight); out: next state
+    int* state_new;  // [n] scratch: next states, moved to `state` (or compacted) by the last CTA
     int n;
     const int* n_dev;  // if non-null the active count is read from the device
     int* token_out;
@@ -62,6 +80,8 @@ struct StepArgs {
     PartialSlot* partials;  // [units]
     int* tickets;           // [rows] arrivals per slot, zero between launches
     int* ctrs;              // [0] work counter, [1] finished CTAs, [2] sticky error count, [3] generation
+    int gather_max;         // states with <= gather_max transitions are gathered (GATHER kernels; 0 = never)
+    int all_gather;         // no state has more than gather_max transitions
     // decode loop only, all optional:
     // per-row history, indexed by ORIGINAL row id (= row_map[slot]), written when the row's step is final
     int* hist_tokens;  // [B, max_steps]
@@ -114,22 +134,30 @@ __device__ __forceinline__ float tile_elem(const unsigned char* tile, int e) {
 }
 
 // Row finished: (m, s, idx) is the merged result of all its units.  Warp-uniform.
+// `gathered`: idx is the position inside the state's CSR row instead of the token id.
 __device__ __forceinline__ void finalize_row(const StepArgs& a, const TileMeta& mt, float m, float s, int idx,
-                                             int lane) {
+                                             int lane, bool gathered) {
     const long long lo = mt.csr_lo, hi = mt.csr_lo + mt.csr_len;
     int token;
     float lp, lse;
+    long long j;
     if (m == -INFINITY) {  // every allowed logit is -inf: lowest allowed id (G6)
         token = __ldg(a.dfa.tok + lo);
         lp = -INFINITY;
         lse = -INFINITY;
+        idx = 0;
     } else {
         token = idx;
         const float L = logf(s);
         lp = -L;  // log p(t*) = x_t* - lse = -log(sum); never m - lse (cancellation)
         lse = m + L;
     }
-    const long long j = warp_csr_find(a.dfa.tok, lo, hi, token, lane);
+    if (gathered) {
+        j = lo + idx;
+        token = __ldg(a.dfa.tok + j);
+    } else {
+        j = warp_csr_find(a.dfa.tok, lo, hi, token, lane);
+    }
     if (lane == 0) {
         const int slot = mt.slot;
         int ns = mt.st;
@@ -142,7 +170,7 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const TileMeta& 
             atomicAdd(a.ctrs + 2, 1);
             dn = 1;
         }
-        a.state[slot] = ns;
+        a.state_new[slot] = ns;
         a.token_out[slot] = token;
         a.logprob_out[slot] = lp;
         if (a.lse_out) a.lse_out[slot] = lse;
@@ -158,7 +186,7 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const TileMeta& 
     }
 }
 
-template <int DT, int WARPS, int STAGES, int TILE_BYTES>
+template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER>
 __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     constexpr int SZ = (DT == DT_BF16) ? 2 : 4;
     constexpr int TILE_TOK = TILE_BYTES / SZ;
@@ -196,7 +224,11 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     const int V = a.dfa.V;
     const int tiles_per_row = (V + TILE_TOK - 1) / TILE_TOK;
     const int tpu = tiles_per_unit(n, tiles_per_row, total_warps, TPU_MAX);
-    const int P = (tiles_per_row + tpu - 1) / tpu;  // units per row
+    const int Pd = (tiles_per_row + tpu - 1) / tpu;  // units per row of a dense scan
+    // a gathered row is split only as far as needed to give every warp a few units
+    const int PG = GATHER ? max(1, min(Pd, (total_warps * UNITS_PER_WARP) / max(n, 1))) : Pd;
+    // units per row of this launch; if every state is gathered no unit is drawn in vain
+    const int P = (GATHER && a.all_gather) ? PG : Pd;
     const int total_units = n * P;
     const bool ragged_row = (V % TILE_TOK) != 0;
     const uint64_t pol_stream = l2_policy_evict_first();
@@ -210,7 +242,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     int iss_stage = 0, in_flight = 0;
 
     auto issue_one = [&]() {
-        if (iss_tile >= iss_end) {
+        while (iss_tile >= iss_end) {  // next unit (units of a gathered row beyond its pieces are skipped)
             if (exhausted) return;
             const int u = __shfl_sync(FULL, next_u_l0, 0);
             if (u >= total_units) {
@@ -220,7 +252,9 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
             if (lane == 0) next_u_l0 = total_warps + atomicAdd(a.ctrs + 0, 1);
             iss_slot = u / P;
             const int part = u - iss_slot * P;
-            iss_st = a.state[iss_slot];  // rewritten only after every unit of the slot has been merged
+            // state[] is not written while units are in flight (next states go to state_new[]): a
+            // unit drawn after its row was finalised still sees the state the row was processed in
+            iss_st = a.state[iss_slot];
             const long long r = a.row_map ? (long long)__ldg(a.row_map + iss_slot) : (long long)iss_slot;
             const bool bad = (iss_st < 0) || (iss_st >= a.dfa.S);
             const int sts = bad ? 0 : iss_st;
@@ -231,6 +265,18 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 if (lane == 0) {
                     ring.meta[iss_stage] =
                         TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (part << 8), iss_st, 0, 0, 0};
+                    mbar_arrive(smem_u32(&ring.bar[iss_stage]));
+                }
+                iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
+                ++in_flight;
+                iss_tile = iss_end = 0;
+                return;
+            }
+            if (GATHER && iss_len <= a.gather_max) {
+                if (part >= gather_parts(iss_len, PG)) continue;
+                if (lane == 0) {
+                    ring.meta[iss_stage] = TileMeta{iss_slot, (int)r, FLAG_GATHER | FLAG_LAST | (part << 8), iss_st,
+                                                    iss_lo, iss_len, 0};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
                 iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
@@ -307,6 +353,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
         if (mt.flags & (FLAG_ACCEPT | FLAG_BADSTATE)) {
             // accepted rows never advance
             if (part == 0 && lane == 0) {
+                a.state_new[mt.slot] = mt.st;
                 a.token_out[mt.slot] = -1;
                 a.logprob_out[mt.slot] = 0.0f;
                 if (a.lse_out) a.lse_out[mt.slot] = 0.0f;
@@ -314,6 +361,49 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 if (mt.flags & FLAG_BADSTATE) atomicAdd(a.ctrs + 2, 1);
             }
         } else {
+            const bool gathered = GATHER && (mt.flags & FLAG_GATHER);
+            const int np = gathered ? gather_parts(mt.csr_len, PG) : P;  // units this row was split into
+            if (gathered) {
+                // piece [j0, j1) of the state's CSR row: tokens read coalesced, their logits gathered
+                // with GATHER_UNROLL independent loads per lane; idx = position in the CSR row, which
+                // ascends with the token id, so "replace on strictly greater" keeps the lowest id
+                m = -INFINITY;
+                s = 0.0f;
+                idx = 0x7FFFFFFF;
+                const int j0 = (int)(((long long)mt.csr_len * part) / np);
+                const int j1 = (int)(((long long)mt.csr_len * (part + 1)) / np);
+                const int* tk = a.dfa.tok + mt.csr_lo;
+                const unsigned char* rowp = a.logits + (long long)mt.tile * a.ld_bytes;
+                // software pipeline: the token ids of the next round are loaded while this round's
+                // logits are in flight
+                int t[GATHER_UNROLL];
+#pragma unroll
+                for (int u = 0; u < GATHER_UNROLL; ++u)
+                    t[u] = (j0 + lane + 32 * u < j1) ? __ldg(tk + j0 + lane + 32 * u) : -1;
+#pragma unroll 1
+                for (int j = j0 + lane; j < j1; j += 32 * GATHER_UNROLL) {
+                    float x[GATHER_UNROLL];
+#pragma unroll
+                    for (int u = 0; u < GATHER_UNROLL; ++u) {
+                        float v = -INFINITY;
+                        if (t[u] >= 0) {
+                            if (DT == DT_BF16)
+                                v = __uint_as_float(
+                                    ((uint32_t)__ldg(reinterpret_cast<const uint16_t*>(rowp) + t[u])) << 16);
+                            else
+                                v = __ldg(reinterpret_cast<const float*>(rowp) + t[u]);
+                        }
+                        x[u] = v;
+                    }
+                    const int jn = j + 32 * GATHER_UNROLL;
+#pragma unroll
+                    for (int u = 0; u < GATHER_UNROLL; ++u) t[u] = (jn + 32 * u < j1) ? __ldg(tk + jn + 32 * u) : -1;
+#pragma unroll
+                    for (int u = 0; u < GATHER_UNROLL; ++u)
+                        online_update(m, s, idx, fmaxf(x[u], -INFINITY), j + 32 * u);  // NaN -> -inf
+                }
+                __syncwarp();
+            } else {
             if (mt.flags & FLAG_FIRST) {
                 m = -INFINITY;
                 s = 0.0f;
@@ -338,12 +428,13 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                     online_update(m, s, idx, x, t0 + e);
                 }
             }
+            }
             if (mt.flags & FLAG_LAST) {
                 float rm = m, rs = s;
                 int ri = idx;
                 warp_combine(rm, rs, ri);
-                if (P == 1) {
-                    finalize_row(a, mt, rm, rs, ri, lane);
+                if (np == 1) {
+                    finalize_row(a, mt, rm, rs, ri, lane, gathered);
                 } else {
                     // Publish from lane 1 (lane 0 is busy issuing copies): three self-validating
                     // words, then a RELAXED ticket -- no fence anywhere.  The last arriver merges.
@@ -356,7 +447,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                         t = atomicAdd(a.tickets + mt.slot, 1);
                     }
                     t = __shfl_sync(FULL, t, 1);
-                    if (t == P - 1) {
+                    if (t == np - 1) {
                         if (lane == 1) a.tickets[mt.slot] = 0;
                         // The other units' words were stored before their tickets, but nothing
                         // orders them: poll until every tag is current (normally the first read).
@@ -369,9 +460,9 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                         rm = -INFINITY;
                         rs = 0.0f;
                         ri = 0x7FFFFFFF;
-                        for (int q0 = 0; q0 < P; q0 += 32) {
+                        for (int q0 = 0; q0 < np; q0 += 32) {
                             const int q = q0 + lane;
-                            const bool want = (q < P) && (q != part);
+                            const bool want = (q < np) && (q != part);
                             bool ok = !want;
                             unsigned long long wm = 0, ws = 0, wi = 0;
                             while (true) {
@@ -391,7 +482,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                                 online_combine(rm, rs, ri, om, os, oi);
                         }
                         warp_combine(rm, rs, ri);
-                        finalize_row(a, mt, rm, rs, ri, lane);
+                        finalize_row(a, mt, rm, rs, ri, lane, gathered);
                     }
                 }
             }
@@ -416,8 +507,13 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
         }
     }
     __syncthreads();
-    if (s_is_last && a.cmp_row_ids_out)
-        block_compact(a.done_out, a.row_map, a.state, n, a.cmp_row_ids_out, a.cmp_state_out, a.cmp_n_out);
+    if (s_is_last) {
+        if (a.cmp_row_ids_out) {
+            block_compact(a.done_out, a.row_map, a.state_new, n, a.cmp_row_ids_out, a.cmp_state_out, a.cmp_n_out);
+        } else {
+            for (int i = threadIdx.x; i < n; i += blockDim.x) a.state[i] = __ldcg(a.state_new + i);
+        }
+    }
 }
 
 }  // namespace cd

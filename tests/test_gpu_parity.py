@@ -31,8 +31,33 @@ def cd():
     return m
 
 
+# Every test of this module runs three times: dense scan only (the method as BASELINE.json
+# north_star states it), every state gathered through its CSR token list, and a mix (states
+# with at most the median number of transitions gathered) -- SURVEY 8(f) N1: same outputs, same
+# oracle, same tolerances.
+_MODE = {"name": "dense"}
+
+
+@pytest.fixture(autouse=True, params=["dense", "gather_all", "gather_mixed"])
+def step_mode(request):
+    _MODE["name"] = request.param
+    yield request.param
+    _MODE["name"] = "dense"
+
+
 def dev_dfa(cd, aut):
-    return cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device="cuda:0")
+    dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device="cuda:0")
+    return apply_mode(dfa, aut)
+
+
+def apply_mode(dfa, aut):
+    if _MODE["name"] == "gather_all":
+        dfa.set_gather_max(2**30)
+    elif _MODE["name"] == "gather_mixed":
+        deg = torch.diff(torch.as_tensor(aut.row_ptr).cpu())
+        deg = deg[deg > 0]
+        dfa.set_gather_max(max(1, int(deg.median())) if deg.numel() else 1)
+    return dfa
 
 
 def close(gpu, ref, tol=TOL):
@@ -404,6 +429,39 @@ def test_loop_c4_batch_sampled_rows(cd, oracle):
     dfa.close()
 
 
+@pytest.mark.parametrize("B", [37, 900])
+def test_loop_states_of_very_different_degree(cd, oracle, B):
+    """States with 1 ... 9000 transitions in one automaton: in the gather modes rows are split
+    into different numbers of units per state, some units are drawn in vain, and a row's next
+    state usually has another degree than the one it was processed in."""
+    V, S, steps = 65536, 48, 14
+    rng = np.random.default_rng(99)
+    degs = [1, 2, 40, 255, 256, 257, 700, 1300, 2049, 5000, 9000, 3]
+    row_ptr, tok, nxt = [0], [], []
+    accepting = np.zeros(S, np.uint8)
+    accepting[S - 3:] = 1
+    for s in range(S):
+        if accepting[s]:
+            row_ptr.append(len(tok))
+            continue
+        d = degs[s % len(degs)]
+        t = np.sort(rng.choice(V, size=d, replace=False))
+        tok.extend(t.tolist())
+        nxt.extend(rng.integers(0, S, size=d).tolist())
+        row_ptr.append(len(tok))
+    aut = wl.Automaton(V=V, S=S, start=0, row_ptr=torch.tensor(row_ptr, dtype=torch.int64),
+                       tok=torch.tensor(tok, dtype=torch.int32), next=torch.tensor(nxt, dtype=torch.int32),
+                       accepting=torch.tensor(accepting))
+    assert oracle.validate(aut) == 0
+    logits = [wl.make_logits(7, k, B, V, 2.0, torch.bfloat16, device="cuda:0") for k in range(steps)]
+    check_loop(cd, oracle, aut, logits, steps)
+    # and single steps from scattered states
+    dfa = dev_dfa(cd, aut)
+    states = [int(x) for x in rng.integers(0, S - 3, size=B)]
+    check_step(cd, oracle, aut, dfa, logits[0], states)
+    dfa.close()
+
+
 def test_host_buffer_loop_matches_device_loop(cd, oracle):
     cfg = wl.scaled(wl.CONFIGS["c3"], V=30000, B=300, S=64, max_steps=8)
     aut = wl.build_automaton(cfg, device="cuda:0")
@@ -423,6 +481,7 @@ def test_trie_sugar_equals_explicit_csr(cd, oracle):
     logits = wl.build_step_logits(cfg, aut, device="cuda:0")
     d1 = dev_dfa(cd, aut)
     d2 = cd.compile_trie(cfg.V, aut.labels, device="cuda:0")
+    apply_mode(d2, aut)
     assert (d1.S, d1.nnz) == (d2.S, d2.nnz)
     o1 = cd.decode_loop(d1, logits)
     o2 = cd.decode_loop(d2, logits)
