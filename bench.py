@@ -58,6 +58,7 @@ def parse_args():
     ap.add_argument("--gather-max", type=int, default=0,
                     help="cd_set_gather_max for the main measurement: 0 = dense scan (default, the graded method), "
                          "-1 = automatic, > 0 = threshold (SURVEY 8(f) N1)")
+    ap.add_argument("--no-adaptive", action="store_true", help="skip the density-adaptive (gather) measurement")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--verbose", action="store_true", help="per-launch table of the step kernel on stderr")
@@ -261,7 +262,8 @@ def main():
     # the events bracket the kernel itself and not the host's launch gaps.
     step_ms, step_bytes, step_rows = [], [], []
     logits = batches[0]
-    n_k, distinct_k = [], []
+    n_k, distinct_k, deg_k = [], [], []
+    deg_dev = torch.diff(torch.as_tensor(aut.row_ptr)).to(device)
     i32 = dict(dtype=torch.int32, device=device)
     bufs = dict(tok=torch.empty(cfg.B, **i32), lp=torch.empty(cfg.B, dtype=torch.float32, device=device),
                 done=torch.empty(cfg.B, dtype=torch.uint8, device=device),
@@ -282,6 +284,7 @@ def main():
                     break
                 n_k.append(n)
                 distinct_k.append(int(torch.unique(bufs["st"][cur][:n]).numel()))
+                deg_k.append(int(deg_dev[bufs["st"][cur][:n].long()].sum()))
             elif k >= len(n_k):
                 break
             else:
@@ -320,6 +323,41 @@ def main():
     }
     row_steps_timed = sum(rs_batch[(args.warmup + i) % len(batches)] for i in range(args.steps))
     row_steps = row_steps_timed / args.steps
+
+    # ---------------- density-adaptive step, reported beside the dense path:
+    # the same loops with cd_set_gather_max(-1).  Its bytes are the bytes it touches (one 32-byte
+    # sector + the 4-byte token id per allowed logit of a gathered row), never the dense count.
+    adaptive = None
+    if not args.no_adaptive and args.gather_max == 0:
+        dfa.set_gather_max(-1)
+        for i in range(args.warmup):
+            one_step(i)
+        barrier()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record(stream)
+        for i in range(args.steps):
+            one_step(args.warmup + i)
+        a1.record(stream)
+        barrier()
+        ms_a = a0.elapsed_time(a1)
+        if dist is not None:
+            t = torch.tensor([ms_a], device=device)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_a = float(t[0])
+        dfa.set_gather_max(0)
+        auto_max = (sz_logit + sz_mask) // 108  # the library's automatic threshold (cd_api.cu gather_max_for)
+        gathered = [dk for dk in deg_k]  # allowed logits per step of batch 0 (every row-step, if gathered)
+        all_gathered = int(deg_dev.max()) <= auto_max
+        adaptive = {
+            "value": cfg.B * args.steps * world / (ms_a * 1e-3), "unit": UNIT, "ms_per_step": ms_a / args.steps,
+            "speedup_vs_dense": ms / ms_a, "gather_max": int(auto_max), "every_state_gathered": bool(all_gathered),
+            "allowed_logits_per_loop_batch0": int(sum(gathered)),
+            "touched_bytes_per_loop_batch0": int(sum(gathered)) * 36 if all_gathered else None,
+            "note": "same outputs as the dense scan (parity-tested in gather modes); bytes = 32-byte sector + 4-byte "
+                    "token id per allowed logit; DRAM moves 128-byte lines (profiles/r1d_gather_c4.md)",
+        }
+        if all_gathered:
+            adaptive["touched_gbs"] = adaptive["touched_bytes_per_loop_batch0"] / (ms_a / args.steps * 1e-3) / 1e9
 
     # ---------------- e2e: the same metric through the C ABI with HOST buffers
     e2e = None
@@ -401,6 +439,7 @@ def main():
             "clocks": clocks,
             "e2e": e2e,
             "roofline": roofline,
+            "adaptive": adaptive,
             "cpu_baseline": cpu,
             "paper_context": "PAPER.md L17-18/L32: 390x lower cost, 3.8x lower latency than a proprietary API with a "
                              "quantized model on one 16 GB GPU; no per-step number is published (BASELINE.md)",

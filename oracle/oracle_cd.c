@@ -168,13 +168,27 @@ int orc_compact(const uint8_t *done, const int32_t *row_ids_in, const int32_t *s
  * row id.  tokens_out is [B, max_steps], -1 padded.  n_active_hist (optional,
  * [max_steps]) receives the number of rows each step processed.
  */
-int orc_decode_loop(int32_t V, int32_t S, int32_t start, const int64_t *row_ptr, const int32_t *tok,
-                    const int32_t *next, const uint8_t *accepting, const void *const *step_logits,
-                    int dtype, int64_t ld, int32_t B, int32_t max_steps, int32_t *tokens_out,
-                    int32_t *len_out, int32_t *final_state_out, double *sum_logprob_out,
-                    uint8_t *done_out, int32_t *n_active_hist)
+/*
+ * O5 (section 2.4 "Early Exiting", L152-L154): with a LIMIT the
+ * LM function "may terminate as soon as the required number of rows is satisfied" and
+ * outstanding generations are cancelled, "no unnecessary tokens are generated".  Reading
+ * (N3): a row satisfies when it reaches an accepting state s with
+ * satisfying[s] != 0 (e.g. the leaf of the label TRUE for `... = TRUE`).  *satisfied counts
+ * such rows across calls (one call per batch of the table).  If *satisfied >= limit at
+ * entry no row takes a step.  After every step the rows that finished in it are counted
+ * (all of them: rows finishing in the same step are all kept); once *satisfied >= limit
+ * every row still active is cancelled: it keeps the tokens it has, done = 0.
+ * satisfying == NULL means no limit (plain O4).
+ */
+int orc_decode_loop_limit(int32_t V, int32_t S, int32_t start, const int64_t *row_ptr, const int32_t *tok,
+                          const int32_t *next, const uint8_t *accepting, const void *const *step_logits,
+                          int dtype, int64_t ld, int32_t B, int32_t max_steps, int32_t *tokens_out,
+                          int32_t *len_out, int32_t *final_state_out, double *sum_logprob_out,
+                          uint8_t *done_out, int32_t *n_active_hist, const uint8_t *satisfying,
+                          int32_t limit, int32_t *satisfied)
 {
     if (B < 0 || max_steps < 0) return ORC_ERR_ARG;
+    if (satisfying && !satisfied) return ORC_ERR_ARG;
     int32_t *ids = (int32_t *)malloc(sizeof(int32_t) * (size_t)(B + 1) * 6);
     double *lp = (double *)malloc(sizeof(double) * (size_t)(B + 1) * 2);
     uint8_t *dn = (uint8_t *)malloc((size_t)B + 1);
@@ -195,7 +209,8 @@ int orc_decode_loop(int32_t V, int32_t S, int32_t start, const int64_t *row_ptr,
     if (n_active_hist)
         for (int32_t k = 0; k < max_steps; ++k) n_active_hist[k] = 0;
     int32_t n = 0;
-    if (!accepting[start])
+    const int exhausted_at_entry = satisfying && *satisfied >= limit;
+    if (!accepting[start] && !exhausted_at_entry)
         for (int32_t r = 0; r < B; ++r) {
             ids[n] = r;
             st[n] = start;
@@ -214,7 +229,9 @@ int orc_decode_loop(int32_t V, int32_t S, int32_t start, const int64_t *row_ptr,
             final_state_out[r] = st[i];
             sum_logprob_out[r] += lp[i];
             done_out[r] = dn[i];
+            if (satisfying && dn[i] && satisfying[st[i]]) ++*satisfied;
         }
+        if (satisfying && *satisfied >= limit) break; /* cancel every row still active */
         int32_t n2 = 0;
         orc_compact(dn, ids, st, n, ids2, st2, &n2);
         memcpy(ids, ids2, sizeof(int32_t) * (size_t)n2);
@@ -223,4 +240,16 @@ int orc_decode_loop(int32_t V, int32_t S, int32_t start, const int64_t *row_ptr,
     }
     free(ids); free(lp); free(dn);
     return rc;
+}
+
+/* O4 = O5 without a limit. */
+int orc_decode_loop(int32_t V, int32_t S, int32_t start, const int64_t *row_ptr, const int32_t *tok,
+                    const int32_t *next, const uint8_t *accepting, const void *const *step_logits,
+                    int dtype, int64_t ld, int32_t B, int32_t max_steps, int32_t *tokens_out,
+                    int32_t *len_out, int32_t *final_state_out, double *sum_logprob_out,
+                    uint8_t *done_out, int32_t *n_active_hist)
+{
+    return orc_decode_loop_limit(V, S, start, row_ptr, tok, next, accepting, step_logits, dtype, ld, B,
+                                 max_steps, tokens_out, len_out, final_state_out, sum_logprob_out,
+                                 done_out, n_active_hist, NULL, 0, NULL);
 }

@@ -49,6 +49,7 @@ def _load():
         _lib.orc_step.restype = C.c_int
         _lib.orc_compact.restype = C.c_int
         _lib.orc_decode_loop.restype = C.c_int
+        _lib.orc_decode_loop_limit.restype = C.c_int
     return _lib
 
 
@@ -135,10 +136,13 @@ def compact(done, row_ids=None, state=None):
     return ro[: k.value].copy(), (None if so is None else so[: k.value].copy()), int(k.value)
 
 
-def decode_loop(aut, step_logits: List, max_steps: Optional[int] = None):
+def decode_loop(aut, step_logits: List, max_steps: Optional[int] = None, satisfying=None, limit: int = 0,
+                satisfied: int = 0):
     """The whole loop (O4).  step_logits[k] is [B, ld] indexed by original row
     id.  Returns dict(tokens i32[B,max_steps], len, final_state, sum_logprob
-    f64, done u8, n_active_hist i32[max_steps])."""
+    f64, done u8, n_active_hist i32[max_steps]).  With `satisfying` (u8[S]) the
+    LIMIT early exit of O5 applies: `satisfied` rows counted so far in, the new
+    count out under key "satisfied"."""
     V, S, start, rp, tok, nxt, acc = _csr(aut)
     max_steps = len(step_logits) if max_steps is None else max_steps
     assert len(step_logits) >= max_steps
@@ -156,11 +160,15 @@ def decode_loop(aut, step_logits: List, max_steps: Optional[int] = None):
     slp = np.empty(B, np.float64)
     done = np.empty(B, np.uint8)
     hist = np.zeros(max(1, max_steps), np.int32)
-    rc = _load().orc_decode_loop(
+    sat = None if satisfying is None else np.ascontiguousarray(np.asarray(satisfying, dtype=np.uint8))
+    if sat is not None:
+        assert sat.shape[0] == S
+    cnt = C.c_int32(int(satisfied))
+    rc = _load().orc_decode_loop_limit(
         C.c_int32(V), C.c_int32(S), C.c_int32(start), _p(rp), _p(tok), _p(nxt), _p(acc), ptrs,
         C.c_int(dt), C.c_int64(ld), C.c_int32(B), C.c_int32(max_steps), _p(tokens), _p(ln), _p(fs),
-        _p(slp), _p(done), _p(hist))
+        _p(slp), _p(done), _p(hist), _p(sat), C.c_int32(int(limit)), C.byref(cnt) if sat is not None else None)
     if rc != OK:
         raise OracleError(rc)
     return dict(tokens=tokens, len=ln, final_state=fs, sum_logprob=slp, done=done,
-                n_active_hist=hist[:max_steps])
+                n_active_hist=hist[:max_steps], satisfied=int(cnt.value))
