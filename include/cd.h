@@ -191,6 +191,34 @@ CD_API cd_status cd_decode_loop(const cd_dfa_t* dfa, const void* const* step_log
                          uint8_t* done_out, void* cuda_stream);
 
 /*
+ * LIMIT early exit (section 2.4 "Early Exiting",
+ * L152-L154: with a LIMIT the LM function "may terminate as soon as the required
+ * number of rows is satisfied ... a cancel event is issued and all outstanding
+ * generation requests are terminated").
+ * cd_set_satisfying marks the accepting states whose value satisfies the query's
+ * predicate (HOST u8[S], copied; e.g. the leaf of the label TRUE for `... = TRUE`;
+ * NULL clears).  Call it while no work using the handle is in flight.
+ * cd_decode_loop_limit is cd_decode_loop with a device counter *satisfied_inout
+ * (DEVICE int32, shared by the calls of one query, one call per batch of the
+ * table; the caller zeroes it first): every row that reaches an accepting state s
+ * with satisfying[s] != 0 adds 1.  If the counter is >= limit at entry no row
+ * takes a step (len 0, done 0).  After each decoding step, once the counter has
+ * reached limit, every row still active is cancelled: it keeps the tokens it has,
+ * done_out = 0, final_state_out = the state it stopped in.  Rows that finish in
+ * the same step are all kept, so the counter may end above limit (the caller
+ * keeps the first `limit` in row order).  The remaining step launches find an
+ * empty active list and do no work.
+ * Errors: as cd_decode_loop; CD_ERR_ARG if cd_set_satisfying was not called,
+ * satisfied_inout is NULL or limit < 0.
+ */
+CD_API cd_status cd_set_satisfying(cd_dfa_t* dfa, const uint8_t* satisfying /*[S] or NULL*/);
+CD_API cd_status cd_decode_loop_limit(const cd_dfa_t* dfa, const void* const* step_logits, cd_dtype dtype,
+                               int64_t ld_elems, int32_t B, int32_t max_steps, int32_t* tokens_out,
+                               int32_t* len_out, int32_t* final_state_out, float* sum_logprob_out,
+                               uint8_t* done_out, int32_t limit, int32_t* satisfied_inout,
+                               void* cuda_stream);
+
+/*
  * Same loop with HOST buffers end to end: step_logits_host[k] are HOST arrays
  * (pinned memory lets the copies overlap the kernels), the five outputs are
  * HOST arrays.  Host-to-device copies of step k+1 overlap the kernels of step

@@ -18,7 +18,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
     "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_reserve", "cd_step",
-    "cd_transition", "cd_compact", "cd_decode_loop", "cd_decode_loop_host", "cd_launch_count",
+    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_launch_count",
     "cd_last_error",
 )
 
@@ -105,6 +105,16 @@ class Dfa:
     def set_gather_max(self, max_transitions: int):
         """cd_set_gather_max: 0 = dense scan only, > 0 threshold, -1 automatic."""
         _check(lib().cd_set_gather_max(self._h, C.c_int32(max_transitions)))
+
+    def set_satisfying(self, satisfying):
+        """cd_set_satisfying: u8[S] host flags (None clears)."""
+        if satisfying is None:
+            _check(lib().cd_set_satisfying(self._h, C.c_void_p(None)))
+            return
+        t = _host(satisfying, torch.uint8)
+        if t.numel() != self.S:
+            raise ValueError("satisfying must have S entries")
+        _check(lib().cd_set_satisfying(self._h, _ptr(t)))
 
     def reserve(self, max_rows: int):
         _check(lib().cd_reserve(self._h, C.c_int32(max_rows), _stream(self.device)))
@@ -241,10 +251,12 @@ def _loop_outputs(B: int, max_steps: int, device, pin: bool = False):
     )
 
 
-def decode_loop(dfa: Dfa, step_logits: Sequence[torch.Tensor], max_steps: Optional[int] = None, out=None):
+def decode_loop(dfa: Dfa, step_logits: Sequence[torch.Tensor], max_steps: Optional[int] = None, out=None,
+                limit: Optional[int] = None, satisfied: Optional[torch.Tensor] = None):
     """cd_decode_loop: step_logits[k] are [B, ld] CUDA tensors indexed by original
     row id.  Returns dict(tokens, len, final_state, sum_logprob, done) of device
-    tensors.  Synchronises the current stream once."""
+    tensors.  Synchronises the current stream once.  With `limit` and the device
+    int32[1] counter `satisfied` it is cd_decode_loop_limit."""
     dev = dfa.device
     max_steps = len(step_logits) if max_steps is None else max_steps
     if max_steps > len(step_logits):
@@ -258,6 +270,13 @@ def decode_loop(dfa: Dfa, step_logits: Sequence[torch.Tensor], max_steps: Option
             raise TypeError("step_logits must share shape, stride and dtype")
     ptrs = (C.c_void_p * max_steps)(*[x.data_ptr() for x in step_logits[:max_steps]])
     out = _loop_outputs(B, max_steps, dev) if out is None else out
+    if limit is not None:
+        _dev_tensor(satisfied, torch.int32, "satisfied", dev)
+        _check(lib().cd_decode_loop_limit(dfa._h, ptrs, C.c_int(dt), C.c_int64(ld), C.c_int32(B), C.c_int32(max_steps),
+                                          _ptr(out["tokens"]), _ptr(out["len"]), _ptr(out["final_state"]),
+                                          _ptr(out["sum_logprob"]), _ptr(out["done"]), C.c_int32(limit),
+                                          _ptr(satisfied), _stream(dev)))
+        return out
     _check(lib().cd_decode_loop(dfa._h, ptrs, C.c_int(dt), C.c_int64(ld), C.c_int32(B), C.c_int32(max_steps),
                                 _ptr(out["tokens"]), _ptr(out["len"]), _ptr(out["final_state"]),
                                 _ptr(out["sum_logprob"]), _ptr(out["done"]), _stream(dev)))

@@ -124,6 +124,7 @@ struct cd_dfa {
     void* d_tok = nullptr;
     void* d_next = nullptr;
     void* d_acc = nullptr;
+    void* d_satisfying = nullptr;  // cd_set_satisfying
     std::mutex mu;
     std::map<cudaStream_t, Scratch> scratch;
 };
@@ -279,6 +280,9 @@ struct LoopExtras {
     int* row_ids_out = nullptr;
     int* state_out = nullptr;
     int* n_out = nullptr;
+    const uint8_t* satisfying = nullptr;
+    int* sat_ctr = nullptr;
+    int limit = 0;
 };
 
 // n_upper bounds the active count; n_dev (device int) overrides n inside the kernel.
@@ -298,6 +302,9 @@ cd_status launch_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype 
         a.cmp_row_ids_out = x->row_ids_out;
         a.cmp_state_out = x->state_out;
         a.cmp_n_out = x->n_out;
+        a.satisfying = x->satisfying;
+        a.sat_ctr = x->sat_ctr;
+        a.limit = x->limit;
     }
     a.dfa = d->dev;
     a.logits = static_cast<const unsigned char*>(logits);
@@ -431,15 +438,22 @@ cd_status compile_impl(int32_t V, int32_t S, int32_t start, const int64_t* row_p
     return CD_OK;
 }
 
+struct LimitArgs {
+    int* sat_ctr = nullptr;  // device counter; nullptr = no limit
+    int limit = 0;
+};
+
 cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, int* tokens_out, int* len_out,
-                           int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream) {
+                           int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream,
+                           const LimitArgs& lim = LimitArgs()) {
     long long work = (long long)B * (max_steps > 0 ? max_steps : 1);
     long long blocks = (work + 255) / 256;
     if (blocks < 1) blocks = 1;
     if (blocks > 4096) blocks = 4096;
     cd::loop_init_kernel<<<(int)blocks, 256, 0, stream>>>(B, max_steps, d->start, d->start_accepting, s->row_ids[0],
                                                           s->state[0], s->n_active, tokens_out, len_out,
-                                                          final_state_out, sum_logprob_out, done_out);
+                                                          final_state_out, sum_logprob_out, done_out, lim.sat_ctr,
+                                                          lim.limit);
     CU(cudaGetLastError());
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return CD_OK;
@@ -449,9 +463,15 @@ cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, in
 // records the per-row history as rows finalise and its last CTA compacts the active list.
 cd_status enqueue_loop_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype dtype, long long ld, int B,
                             int k, int max_steps, int* tokens_out, int* len_out, int* final_state_out,
-                            float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream) {
+                            float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream,
+                            const LimitArgs& lim = LimitArgs()) {
     const int cur = k & 1, nxt = cur ^ 1;
     LoopExtras x;
+    if (lim.sat_ctr) {
+        x.satisfying = static_cast<const uint8_t*>(d->d_satisfying);
+        x.sat_ctr = lim.sat_ctr;
+        x.limit = lim.limit;
+    }
     x.tokens = tokens_out;
     x.len = len_out;
     x.final_state = final_state_out;
@@ -555,6 +575,7 @@ void cd_free_dfa(cd_dfa_t* d) {
     DeviceGuard guard(d->device);
     for (auto& kv : d->scratch) kv.second.release();
     cudaFree(d->d_mask); cudaFree(d->d_row_ptr); cudaFree(d->d_tok); cudaFree(d->d_next); cudaFree(d->d_acc);
+    cudaFree(d->d_satisfying);
     delete d;
 }
 
@@ -635,9 +656,10 @@ cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, const int32
     return CD_OK;
 }
 
-cd_status cd_decode_loop(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
-                         int32_t B, int32_t max_steps, int32_t* tokens_out, int32_t* len_out,
-                         int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out, void* cuda_stream) {
+static cd_status decode_loop_impl(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
+                                  int32_t B, int32_t max_steps, int32_t* tokens_out, int32_t* len_out,
+                                  int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out,
+                                  const LimitArgs& lim, void* cuda_stream) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
     if (B < 0 || max_steps < 0) return fail(CD_ERR_ARG, "B / max_steps < 0");
     cd_status st = check_dtype(dtype);
@@ -656,15 +678,51 @@ cd_status cd_decode_loop(const cd_dfa_t* d, const void* const* step_logits, cd_d
     Scratch* s = nullptr;
     st = get_scratch(d, stream, B, true, &s);
     if (st != CD_OK) return st;
-    st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream);
+    st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream,
+                          lim);
     if (st != CD_OK) return st;
     if (!d->start_accepting)
         for (int k = 0; k < max_steps; ++k) {
             st = enqueue_loop_step(d, s, step_logits[k], dtype, ld_elems, B, k, max_steps, tokens_out, len_out,
-                                   final_state_out, sum_logprob_out, done_out, stream);
+                                   final_state_out, sum_logprob_out, done_out, stream, lim);
             if (st != CD_OK) return st;
         }
     return check_sticky_errors(s, stream);
+}
+
+cd_status cd_decode_loop(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
+                         int32_t B, int32_t max_steps, int32_t* tokens_out, int32_t* len_out,
+                         int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out, void* cuda_stream) {
+    return decode_loop_impl(d, step_logits, dtype, ld_elems, B, max_steps, tokens_out, len_out, final_state_out,
+                            sum_logprob_out, done_out, LimitArgs(), cuda_stream);
+}
+
+cd_status cd_set_satisfying(cd_dfa_t* d, const uint8_t* satisfying) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    DeviceGuard guard(d->device);
+    if (!satisfying) {
+        cudaFree(d->d_satisfying);
+        d->d_satisfying = nullptr;
+        return CD_OK;
+    }
+    if (!d->d_satisfying) CU(cudaMalloc(&d->d_satisfying, (size_t)d->dev.S));
+    CU(cudaMemcpy(d->d_satisfying, satisfying, (size_t)d->dev.S, cudaMemcpyHostToDevice));
+    return CD_OK;
+}
+
+cd_status cd_decode_loop_limit(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
+                               int32_t B, int32_t max_steps, int32_t* tokens_out, int32_t* len_out,
+                               int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out, int32_t limit,
+                               int32_t* satisfied_inout, void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (!d->d_satisfying) return fail(CD_ERR_ARG, "cd_set_satisfying has not been called on this automaton");
+    if (!satisfied_inout) return fail(CD_ERR_ARG, "satisfied_inout is NULL");
+    if (limit < 0) return fail(CD_ERR_ARG, "limit < 0");
+    LimitArgs lim;
+    lim.sat_ctr = satisfied_inout;
+    lim.limit = limit;
+    return decode_loop_impl(d, step_logits, dtype, ld_elems, B, max_steps, tokens_out, len_out, final_state_out,
+                            sum_logprob_out, done_out, lim, cuda_stream);
 }
 
 cd_status cd_decode_loop_host(const cd_dfa_t* d, const void* const* step_logits_host, cd_dtype dtype,

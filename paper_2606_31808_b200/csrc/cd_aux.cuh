@@ -60,7 +60,8 @@ __global__ void __launch_bounds__(1024, 1) compact_kernel(const uint8_t* done, c
 // a7 set-up: every row starts in the start state with an empty history.
 __global__ void loop_init_kernel(int B, int max_steps, int start, int start_accepting, int* row_ids,
                                  int* state, int* n_active, int* tokens_out, int* len_out,
-                                 int* final_state_out, float* sum_logprob_out, uint8_t* done_row_out) {
+                                 int* final_state_out, float* sum_logprob_out, uint8_t* done_row_out,
+                                 const int* sat_ctr, int limit) {
     const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long nth = (long long)gridDim.x * blockDim.x;
     for (long long j = tid; j < (long long)B * max_steps; j += nth) tokens_out[j] = -1;
@@ -72,7 +73,8 @@ __global__ void loop_init_kernel(int B, int max_steps, int start, int start_acce
         sum_logprob_out[r] = 0.0f;
         done_row_out[r] = start_accepting ? 1 : 0;
     }
-    if (tid == 0) *n_active = start_accepting ? 0 : B;
+    // LIMIT already satisfied by earlier batches: no row takes a step
+    if (tid == 0) *n_active = (start_accepting || (sat_ctr && *sat_ctr >= limit)) ? 0 : B;
 }
 
 }  // namespace cd

@@ -94,6 +94,12 @@ struct StepArgs {
     int* cmp_row_ids_out;
     int* cmp_state_out;
     int* cmp_n_out;
+    // LIMIT early exit (PAPER.md 2.4 "Early Exiting"), optional: rows that finish in a
+    // state with satisfying[s] != 0 are counted in *sat_ctr; once it reaches `limit` the last CTA
+    // empties the active list (every row still active is cancelled)
+    const uint8_t* satisfying;  // [S]
+    int* sat_ctr;
+    int limit;
 };
 
 struct __align__(16) TileMeta {
@@ -182,6 +188,7 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const TileMeta& 
             a.hist_final_state[rid] = ns;
             a.hist_sum_logprob[rid] += lp;
             a.hist_done[rid] = dn;
+            if (a.sat_ctr && dn && __ldg(a.satisfying + ns)) atomicAdd(a.sat_ctr, 1);
         }
     }
 }
@@ -510,6 +517,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     if (s_is_last) {
         if (a.cmp_row_ids_out) {
             block_compact(a.done_out, a.row_map, a.state_new, n, a.cmp_row_ids_out, a.cmp_state_out, a.cmp_n_out);
+            if (a.sat_ctr && threadIdx.x == 0 && __ldcg(a.sat_ctr) >= a.limit) *a.cmp_n_out = 0;
         } else {
             for (int i = threadIdx.x; i < n; i += blockDim.x) a.state[i] = __ldcg(a.state_new + i);
         }

@@ -462,6 +462,74 @@ def test_loop_states_of_very_different_degree(cd, oracle, B):
     dfa.close()
 
 
+# ------------------------------------------------------------------ LIMIT early exit
+def check_limit_loop(cd, oracle, aut, dfa, logits, max_steps, sat, limit, counter):
+    before = int(counter)
+    out = cd.decode_loop(dfa, logits, max_steps=max_steps, limit=limit, satisfied=counter)
+    ref = oracle.decode_loop(aut, [x.cpu() for x in logits], max_steps=max_steps, satisfying=sat, limit=limit,
+                             satisfied=before)
+    for k in ("tokens", "len", "final_state", "done"):
+        assert np.array_equal(out[k].cpu().numpy(), ref[k]), k
+    assert int(counter) == ref["satisfied"]
+    g, r = out["sum_logprob"].cpu().numpy().astype(np.float64), ref["sum_logprob"]
+    assert np.all(np.abs(g - r) <= np.maximum(TOL * (ref["len"] + np.abs(r)), TOL))
+    return out, ref
+
+
+@pytest.mark.parametrize("limit", [0, 1, 9, 60, 10**6])
+def test_limit_early_exit_random_dfa(cd, oracle, limit):
+    cfg = wl.scaled(wl.CONFIGS["c3"], V=40000, B=500, S=96, max_steps=12)
+    aut = wl.build_automaton(cfg, device="cuda:0")
+    logits = wl.build_step_logits(cfg, aut, device="cuda:0")
+    acc = aut.accepting.cpu().numpy()
+    sat = (acc * (np.arange(aut.S) % 2 == 0)).astype(np.uint8)
+    dfa = dev_dfa(cd, aut)
+    dfa.set_satisfying(sat)
+    counter = torch.zeros(1, dtype=torch.int32, device="cuda:0")
+    out, ref = check_limit_loop(cd, oracle, aut, dfa, logits, cfg.max_steps, sat, limit, counter)
+    if limit == 10**6:  # never reached: identical to the plain loop
+        plain = cd.decode_loop(dfa, logits, max_steps=cfg.max_steps)
+        for k in plain:
+            assert torch.equal(plain[k], out[k])
+    if limit == 0:
+        assert int(out["len"].max()) == 0 and int(counter) == 0
+    # a second batch of the same query continues from the counter (usually: nothing runs)
+    logits2 = wl.build_step_logits(cfg, aut, device="cuda:0", batch=1)
+    check_limit_loop(cd, oracle, aut, dfa, logits2, cfg.max_steps, sat, limit, counter)
+    dfa.close()
+
+
+def test_limit_early_exit_boolean_filter_c1(cd, oracle):
+    """`LLMMap(...) = TRUE ... LIMIT 10` on BASELINE.json configs[1] at full size."""
+    cfg = wl.CONFIGS["c1"]
+    aut = wl.build_automaton(cfg, device="cuda:0")
+    logits = wl.build_step_logits(cfg, aut, device="cuda:0")
+    sat = np.zeros(aut.S, np.uint8)
+    sat[int(aut.leaf_of_label[0])] = 1
+    dfa = dev_dfa(cd, aut)
+    dfa.set_satisfying(sat)
+    counter = torch.zeros(1, dtype=torch.int32, device="cuda:0")
+    check_limit_loop(cd, oracle, aut, dfa, logits, cfg.max_steps, sat, 10, counter)
+    dfa.close()
+
+
+def test_limit_argument_errors(cd):
+    aut = _subset_aut(64, [1, 2])
+    dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device="cuda:0")
+    x = [torch.zeros((4, 64), device="cuda:0")]
+    counter = torch.zeros(1, dtype=torch.int32, device="cuda:0")
+    with pytest.raises(cd.CdError) as e:  # cd_set_satisfying not called
+        cd.decode_loop(dfa, x, limit=1, satisfied=counter)
+    assert e.value.code == 1
+    dfa.set_satisfying([0, 1])
+    with pytest.raises(cd.CdError) as e:
+        cd.decode_loop(dfa, x, limit=-1, satisfied=counter)
+    assert e.value.code == 1
+    out = cd.decode_loop(dfa, x, limit=2, satisfied=counter)
+    assert int(counter) == 4 and bool(out["done"].all())  # rows finishing in the same step are all kept
+    dfa.close()
+
+
 def test_host_buffer_loop_matches_device_loop(cd, oracle):
     cfg = wl.scaled(wl.CONFIGS["c3"], V=30000, B=300, S=64, max_steps=8)
     aut = wl.build_automaton(cfg, device="cuda:0")
