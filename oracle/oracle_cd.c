@@ -253,3 +253,102 @@ int orc_decode_loop(int32_t V, int32_t S, int32_t start, const int64_t *row_ptr,
                                  max_steps, tokens_out, len_out, final_state_out, sum_logprob_out,
                                  done_out, n_active_hist, NULL, 0, NULL);
 }
+
+/*
+ * O6: the constrained step fused with the LM head.  The paper's point
+ * is that the constrained step should cost nothing next to the model forward (PAPER.md
+ * section 5: "adds little-to-no overhead"); the whole cost of the step is the
+ * logits tensor, so the step is defined directly on what produces it:
+ *
+ *     x_i[t] = sum_{h < H} hidden_i[h] * W[t][h]        (the LM head, no bias)
+ *
+ * with hidden [rows, ldh] and W [V, ldw] stored as bf16 (row t of W = output embedding
+ * of token t), followed by exactly O2 on x_i.  Reading (N2): the logit is the
+ * real-number dot product of the stored bf16 values -- it is never rounded to a storage
+ * type.  Here: every bf16 widened exactly to double, products and the sum in double,
+ * ascending h (H <= 2^20 terms of 16 significant bits each: the double sum is exact to
+ * ~1e-13 relative).  Only the allowed tokens' logits are formed (membership = the
+ * state's CSR row, as in O2).  NaN products are read as -inf (G6).
+ *
+ * Outputs as orc_step, plus gap_out[i] = m - (largest allowed logit at another token id),
+ * +inf if the state allows one token: a GPU path that accumulates in fp32 may pick a
+ * different token only when gap is below its rounding error (tests use it that way).
+ */
+static double bf16_to_double(uint16_t b)
+{
+    uint32_t bits = ((uint32_t)b) << 16;
+    float x;
+    memcpy(&x, &bits, 4);
+    return (double)x;
+}
+
+/* x = <hidden_row, W[t]> in double, ascending h. */
+double orc_head_logit(const uint16_t *hidden_row, const uint16_t *W, int64_t ldw, int32_t H, int32_t t)
+{
+    const uint16_t *w = W + (int64_t)t * ldw;
+    double acc = 0.0;
+    for (int32_t h = 0; h < H; ++h) acc += bf16_to_double(hidden_row[h]) * bf16_to_double(w[h]);
+    return acc;
+}
+
+int orc_head_step(int32_t V, int32_t S, const int64_t *row_ptr, const int32_t *tok, const int32_t *next,
+                  const uint8_t *accepting, const uint16_t *hidden, int64_t ldh, const uint16_t *W,
+                  int64_t ldw, int32_t H, const int32_t *row_map, int32_t *state, int32_t n,
+                  int32_t *token_out, double *logprob_out, double *lse_out, uint8_t *done_out,
+                  double *gap_out)
+{
+    if (n < 0 || H < 1 || ldh < H || ldw < H || V < 1) return ORC_ERR_ARG;
+    for (int32_t i = 0; i < n; ++i) {
+        const int32_t s = state[i];
+        if (s < 0 || s >= S) return ORC_ERR_ARG;
+        if (accepting[s]) { /* O2.1 */
+            token_out[i] = -1;
+            logprob_out[i] = 0.0;
+            lse_out[i] = 0.0;
+            done_out[i] = 1;
+            if (gap_out) gap_out[i] = INFINITY;
+            continue;
+        }
+        const int64_t r = row_map ? (int64_t)row_map[i] : (int64_t)i;
+        const uint16_t *hrow = hidden + r * ldh;
+        const int64_t lo = row_ptr[s], hi = row_ptr[s + 1];
+        double *x = (double *)malloc(sizeof(double) * (size_t)(hi - lo));
+        if (!x) return ORC_ERR_ARG;
+        for (int64_t j = lo; j < hi; ++j) {
+            double v = orc_head_logit(hrow, W, ldw, H, tok[j]);
+            if (v != v) v = -INFINITY;
+            x[j - lo] = v;
+        }
+        /* O2.3 on x: ascending id, replace on strictly greater */
+        double m = -INFINITY;
+        int64_t jstar = lo;
+        for (int64_t j = lo; j < hi; ++j)
+            if (x[j - lo] > m) {
+                m = x[j - lo];
+                jstar = j;
+            }
+        double second = -INFINITY;
+        for (int64_t j = lo; j < hi; ++j)
+            if (j != jstar && x[j - lo] > second) second = x[j - lo];
+        /* O2.4 */
+        double sum = 0.0;
+        for (int64_t j = lo; j < hi; ++j) {
+            if (x[j - lo] == -INFINITY) continue;
+            sum += exp(x[j - lo] - m);
+        }
+        if (m == -INFINITY) {
+            lse_out[i] = -INFINITY;
+            logprob_out[i] = -INFINITY;
+        } else {
+            lse_out[i] = m + log(sum);
+            logprob_out[i] = -log(sum);
+        }
+        if (gap_out) gap_out[i] = (hi - lo > 1) ? m - second : INFINITY;
+        free(x);
+        /* O2.5 */
+        token_out[i] = tok[jstar];
+        state[i] = next[jstar];
+        done_out[i] = accepting[next[jstar]] ? 1 : 0;
+    }
+    return ORC_OK;
+}

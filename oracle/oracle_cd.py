@@ -50,6 +50,8 @@ def _load():
         _lib.orc_compact.restype = C.c_int
         _lib.orc_decode_loop.restype = C.c_int
         _lib.orc_decode_loop_limit.restype = C.c_int
+        _lib.orc_head_step.restype = C.c_int
+        _lib.orc_head_logit.restype = C.c_double
     return _lib
 
 
@@ -172,3 +174,51 @@ def decode_loop(aut, step_logits: List, max_steps: Optional[int] = None, satisfy
         raise OracleError(rc)
     return dict(tokens=tokens, len=ln, final_state=fs, sum_logprob=slp, done=done,
                 n_active_hist=hist[:max_steps], satisfied=int(cnt.value))
+
+
+def _bf16_np(x) -> np.ndarray:
+    """[rows, ld] bf16 (torch tensor, or numpy uint16 holding the bits) -> contiguous uint16 array."""
+    if hasattr(x, "detach"):
+        import torch
+        x = x.detach().cpu().contiguous()
+        assert x.dtype == torch.bfloat16
+        return x.view(torch.int16).numpy().view(np.uint16)
+    x = np.ascontiguousarray(x)
+    assert x.dtype == np.uint16
+    return x
+
+
+def head_step(aut, hidden, W, H: int, state: Sequence[int], row_map: Optional[Sequence[int]] = None):
+    """One constrained step on x = hidden @ W[:, :H].T (O6).  hidden [rows, ldh] and
+    W [V, ldw] are bf16.  Returns (token, logprob f64, lse f64, done, new_state, gap f64)."""
+    V, S, start, rp, tok, nxt, acc = _csr(aut)
+    hd = _bf16_np(hidden)
+    w = _bf16_np(W)
+    assert hd.ndim == 2 and w.ndim == 2 and w.shape[0] == V
+    st = np.ascontiguousarray(np.asarray(state, dtype=np.int32)).copy()
+    n = st.shape[0]
+    rm = None if row_map is None else np.ascontiguousarray(np.asarray(row_map, dtype=np.int32))
+    if rm is not None:
+        assert rm.shape[0] == n and (n == 0 or (rm.min() >= 0 and rm.max() < hd.shape[0]))
+    else:
+        assert n <= hd.shape[0]
+    token = np.empty(n, np.int32)
+    lp = np.empty(n, np.float64)
+    lse = np.empty(n, np.float64)
+    done = np.empty(n, np.uint8)
+    gap = np.empty(n, np.float64)
+    rc = _load().orc_head_step(
+        C.c_int32(V), C.c_int32(S), _p(rp), _p(tok), _p(nxt), _p(acc), _p(hd), C.c_int64(hd.shape[1]),
+        _p(w), C.c_int64(w.shape[1]), C.c_int32(H), _p(rm), _p(st), C.c_int32(n), _p(token), _p(lp),
+        _p(lse), _p(done), _p(gap))
+    if rc != OK:
+        raise OracleError(rc)
+    return token, lp, lse, done, st, gap
+
+
+def head_logit(hidden, W, H: int, row: int, token: int) -> float:
+    """<hidden[row, :H], W[token, :H]> in double (O6)."""
+    hd = _bf16_np(hidden)
+    w = _bf16_np(W)
+    hrow = np.ascontiguousarray(hd[row])
+    return float(_load().orc_head_logit(_p(hrow), _p(w), C.c_int64(w.shape[1]), C.c_int32(H), C.c_int32(token)))

@@ -389,3 +389,55 @@ def shard_rows(B: int, world_size: int, rank: int) -> Tuple[int, int]:
     lo = rank * base + min(rank, rem)
     hi = lo + base + (1 if rank < rem else 0)
     return lo, hi
+
+
+# --------------------------------------------------------------------------
+# LM-head inputs: final hidden states and the output embedding
+# --------------------------------------------------------------------------
+def make_hidden(seed: int, step: int, B: int, H: int, device: str = "cpu", batch: int = 0,
+                exact: bool = False, ld: Optional[int] = None) -> torch.Tensor:
+    """Final hidden states [B, ld] bf16 (ld >= H, default H) of one decoding step.
+    exact=False: round_bf16(N(0,1)).  exact=True: multiples of 1/8 in [-1, 1]
+    from the integer hash, so that every partial sum of a dot product with a
+    make_head(exact=True) row is exactly representable in fp32 (the products are
+    multiples of 1/64 and |sum| < 2^17 for H <= 2^17): the logits then do not
+    depend on the order of accumulation."""
+    ld = H if ld is None else ld
+    assert ld >= H
+    dev = torch.device(device)
+    out = torch.zeros((B, ld), dtype=torch.bfloat16, device=dev)
+    if exact:
+        r = torch.arange(B, dtype=torch.int64, device=dev).unsqueeze(1)
+        h = torch.arange(H, dtype=torch.int64, device=dev).unsqueeze(0)
+        u = mix32_t(seed * 7919 + batch * 4099 + step, 11, r, h) % 17  # 0..16
+        out[:, :H] = ((u.to(torch.float32) - 8.0) / 8.0).to(torch.bfloat16)
+    else:
+        g = torch.Generator(device=dev)
+        g.manual_seed((seed * 1000003 + batch * 4099 + step + 0x5EED) & 0x7FFFFFFFFFFFFFFF)
+        out[:, :H] = torch.randn((B, H), generator=g, dtype=torch.float32, device=dev).to(torch.bfloat16)
+    return out
+
+
+def make_head(seed: int, V: int, H: int, std: float, device: str = "cpu", exact: bool = False,
+              ld: Optional[int] = None, rows_per_chunk: int = 16384) -> torch.Tensor:
+    """Output embedding W [V, ld] bf16 (row t = embedding of token t; ld >= H).
+    exact=False: round_bf16(N(0, std / sqrt(H))), so that logits of N(0,1) hidden
+    states are ~N(0, std) like the logits of BASELINE.json configs.
+    exact=True: multiples of 1/8 in [-1, 1] from the integer hash (see make_hidden)."""
+    ld = H if ld is None else ld
+    assert ld >= H
+    dev = torch.device(device)
+    out = torch.zeros((V, ld), dtype=torch.bfloat16, device=dev)
+    g = torch.Generator(device=dev)
+    g.manual_seed((seed * 1000003 + 0xEAD) & 0x7FFFFFFFFFFFFFFF)
+    h = torch.arange(H, dtype=torch.int64, device=dev).unsqueeze(0)
+    for t0 in range(0, V, rows_per_chunk):
+        t1 = min(V, t0 + rows_per_chunk)
+        if exact:
+            t = torch.arange(t0, t1, dtype=torch.int64, device=dev).unsqueeze(1)
+            u = mix32_t(seed, 12, t, h) % 17
+            out[t0:t1, :H] = ((u.to(torch.float32) - 8.0) / 8.0).to(torch.bfloat16)
+        else:
+            x = torch.randn((t1 - t0, H), generator=g, dtype=torch.float32, device=dev)
+            out[t0:t1, :H] = (x * (std / (H ** 0.5))).to(torch.bfloat16)
+    return out
