@@ -230,6 +230,37 @@ CD_API cd_status cd_decode_loop_host(const cd_dfa_t* dfa, const void* const* ste
                               int32_t* tokens_out, int32_t* len_out, int32_t* final_state_out,
                               float* sum_logprob_out, uint8_t* done_out, void* cuda_stream);
 
+/*
+ * The constrained step fused with the LM head.  The whole cost of the
+ * step is the logits tensor, and the paper's point is that constrained decoding should
+ * cost nothing next to the model forward (section 5), so the step is
+ * defined directly on what produces the logits:
+ *     x_i[t] = sum_{h < H} hidden_i[h] * W[t][h]          (LM head, no bias)
+ * followed by exactly the step of cd_step on x_i.  The logit is the dot product of the
+ * stored bf16 values accumulated in fp32 (tensor-core accumulation order); it is never
+ * rounded to a storage type and never written to HBM.  All pointers are DEVICE pointers.
+ *   hidden      [rows, ldh_elems] bf16, final hidden states; the row of active slot i is
+ *               hidden + row_map[i] * ldh_elems (row_map == NULL -> row i)
+ *   W           [V, ldw_elems] bf16, row t = output embedding of token t
+ *   H           hidden size, a positive multiple of 8; ldh_elems, ldw_elems >= H and
+ *               multiples of 8; both base pointers 16-byte aligned
+ *   state, n, token_out, logprob_out, lse_out (may be NULL), done_out: as cd_step
+ * Rows whose state has few transitions (boolean / option-set types) form only their
+ * allowed logits as gathered dot products; the others go through a dense tcgen05
+ * contraction whose epilogue applies each row's allowed-token bitmask
+ * (cd_set_head_gather_max: 0 = dense for every state, > 0 = gather states with at most
+ * that many transitions, -1 = automatic, the default).  Results agree with cd_step on
+ * exactly computed logits: token, state and done are identical whenever the best
+ * allowed logit leads the runner-up by more than the fp32 accumulation error (always,
+ * when the dot products are exact in fp32); logprob / lse within that error.
+ * Errors: CD_ERR_ARG (NULL pointer, bad H / stride / alignment), CD_ERR_CUDA, CD_ERR_OOM.
+ */
+CD_API cd_status cd_set_head_gather_max(cd_dfa_t* dfa, int32_t max_transitions);
+CD_API cd_status cd_head_step(const cd_dfa_t* dfa, const void* hidden, int64_t ldh_elems, const void* W,
+                       int64_t ldw_elems, int32_t H, const int32_t* row_map, int32_t* state, int32_t n,
+                       int32_t* token_out, float* logprob_out, float* lse_out, uint8_t* done_out,
+                       void* cuda_stream);
+
 /* Number of kernel launches this library has enqueued from the calling thread's
    process so far (monotone; used by bench.py to report gpu_launches). */
 CD_API int64_t cd_launch_count(void);

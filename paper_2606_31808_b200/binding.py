@@ -18,7 +18,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
     "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_reserve", "cd_step",
-    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_launch_count",
+    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_launch_count",
     "cd_last_error",
 )
 
@@ -105,6 +105,10 @@ class Dfa:
     def set_gather_max(self, max_transitions: int):
         """cd_set_gather_max: 0 = dense scan only, > 0 threshold, -1 automatic."""
         _check(lib().cd_set_gather_max(self._h, C.c_int32(max_transitions)))
+
+    def set_head_gather_max(self, max_transitions: int):
+        """cd_set_head_gather_max: 0 = dense contraction for every state, > 0 threshold, -1 automatic."""
+        _check(lib().cd_set_head_gather_max(self._h, C.c_int32(max_transitions)))
 
     def set_satisfying(self, satisfying):
         """cd_set_satisfying: u8[S] host flags (None clears)."""
@@ -201,6 +205,36 @@ def step(dfa: Dfa, logits: torch.Tensor, state: torch.Tensor, row_map: Optional[
     _check(lib().cd_step(dfa._h, _ptr(logits), C.c_int(_dt(logits)), C.c_int64(logits.stride(0)), _ptr(row_map),
                          _ptr(state), C.c_int32(n), _ptr(token), _ptr(logprob), _ptr(lse), _ptr(done),
                          _stream(dev)))
+    return token, logprob, lse, done
+
+
+def head_step(dfa: Dfa, hidden: torch.Tensor, W: torch.Tensor, state: torch.Tensor,
+              row_map: Optional[torch.Tensor] = None, n: Optional[int] = None, H: Optional[int] = None,
+              want_lse: bool = True, out=None):
+    """cd_head_step on torch's current stream: the constrained step on x = hidden[:, :H] @ W[:, :H].T
+    without materialising x.  hidden [rows, ldh] and W [V, ldw] are bf16 CUDA tensors with unit inner
+    stride; state (int32, device) is updated in place.  Returns (token, logprob, lse or None, done)."""
+    dev = dfa.device
+    for name, t in (("hidden", hidden), ("W", W)):
+        if t.dim() != 2 or not t.is_cuda or t.stride(1) != 1 or t.dtype != torch.bfloat16:
+            raise TypeError(f"{name} must be a 2-D bf16 CUDA tensor with unit inner stride")
+    H = hidden.shape[1] if H is None else H
+    if W.shape[0] != dfa.V or W.shape[1] < H or hidden.shape[1] < H:
+        raise ValueError("W must be [V, >= H] and hidden [rows, >= H]")
+    _dev_tensor(state, torch.int32, "state", dev)
+    n = state.numel() if n is None else n
+    if row_map is not None:
+        _dev_tensor(row_map, torch.int32, "row_map", dev)
+    if out is not None:
+        token, logprob, lse, done = out
+    else:
+        token = torch.empty(n, dtype=torch.int32, device=dev)
+        logprob = torch.empty(n, dtype=torch.float32, device=dev)
+        lse = torch.empty(n, dtype=torch.float32, device=dev) if want_lse else None
+        done = torch.empty(n, dtype=torch.uint8, device=dev)
+    _check(lib().cd_head_step(dfa._h, _ptr(hidden), C.c_int64(hidden.stride(0)), _ptr(W), C.c_int64(W.stride(0)),
+                              C.c_int32(H), _ptr(row_map), _ptr(state), C.c_int32(n), _ptr(token), _ptr(logprob),
+                              _ptr(lse), _ptr(done), _stream(dev)))
     return token, logprob, lse, done
 
 

@@ -18,6 +18,7 @@
 #include "cd_aux.cuh"
 #include "cd_common.cuh"
 #include "cd_step.cuh"
+#include "cd_head.cuh"
 
 namespace {
 
@@ -93,8 +94,18 @@ struct Scratch {
     cudaEvent_t ev_copied[2] = {nullptr, nullptr};
     cudaEvent_t ev_consumed[2] = {nullptr, nullptr};
     int* h_pinned = nullptr;  // [4] pinned host ints
+    // LM-head step (cd_head.cuh)
+    int head_rows = 0, head_H = 0;
+    uint8_t* h_flags = nullptr;   // [2 * rows]
+    int* h_lists = nullptr;       // [4 * rows] dense slot / dense state / gather slot / gather state
+    int* h_ctr = nullptr;         // [4]
+    uint16_t* h_A = nullptr;      // [rows_pad, ldA]
+    long long h_ldA = 0;
+    cd::HeadPartial* h_partials = nullptr;
+    CUtensorMap h_tmA{};
 
     void release() {
+        cudaFree(h_flags); cudaFree(h_lists); cudaFree(h_ctr); cudaFree(h_A); cudaFree(h_partials);
         cudaFree(partials); cudaFree(tickets); cudaFree(ctrs);
         for (int i = 0; i < 2; ++i) { cudaFree(row_ids[i]); cudaFree(state[i]); cudaFree(stage[i]); }
         cudaFree(state_new); cudaFree(n_active); cudaFree(token); cudaFree(logprob); cudaFree(done); cudaFree(out_i32);
@@ -125,6 +136,12 @@ struct cd_dfa {
     void* d_next = nullptr;
     void* d_acc = nullptr;
     void* d_satisfying = nullptr;  // cd_set_satisfying
+    long long min_deg_nonacc = 0;  // fewest transitions of a non-accepting state
+    int head_gather_max = -1;      // cd_set_head_gather_max: 0 never gather, > 0 threshold, < 0 automatic
+    const void* w_ptr = nullptr;   // cached tensor map of the output embedding (cd_head_step)
+    long long w_ld = 0;
+    int w_H = 0;
+    CUtensorMap w_tmap{};
     std::mutex mu;
     std::map<cudaStream_t, Scratch> scratch;
 };
@@ -214,6 +231,7 @@ cd_status get_scratch(const cd_dfa* cd_, cudaStream_t stream, int rows, bool loo
         old.stage[0] = old.stage[1] = nullptr; old.out_i32 = nullptr; old.copy_stream = nullptr;
         old.ev_copied[0] = old.ev_copied[1] = old.ev_consumed[0] = old.ev_consumed[1] = nullptr;
         old.h_pinned = nullptr;
+        old.h_flags = nullptr; old.h_lists = nullptr; old.h_ctr = nullptr; old.h_A = nullptr; old.h_partials = nullptr;
         old.release();
     }
     (void)loop_bufs;
@@ -372,8 +390,12 @@ cd_status compile_impl(int32_t V, int32_t S, int32_t start, const int64_t* row_p
     d->start = start;
     d->start_accepting = accepting[start] ? 1 : 0;
     d->nnz = nnz;
-    for (int32_t s = 0; s < S; ++s)
-        if (row_ptr[s + 1] - row_ptr[s] > d->max_deg) d->max_deg = row_ptr[s + 1] - row_ptr[s];
+    d->min_deg_nonacc = nnz + 1;
+    for (int32_t s = 0; s < S; ++s) {
+        const long long deg = row_ptr[s + 1] - row_ptr[s];
+        if (deg > d->max_deg) d->max_deg = deg;
+        if (!accepting[s] && deg < d->min_deg_nonacc) d->min_deg_nonacc = deg;
+    }
     cudaDeviceProp prop;
     cudaError_t e = cudaGetDeviceProperties(&prop, device);
     if (e != cudaSuccess) { delete d; return fail(CD_ERR_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e)); }
@@ -816,6 +838,181 @@ cd_status cd_decode_loop_host(const cd_dfa_t* d, const void* const* step_logits_
     CU(cudaMemcpyAsync(sum_logprob_out, d_slp, sizeof(float) * (size_t)B, cudaMemcpyDeviceToHost, stream));
     CU(cudaMemcpyAsync(done_out, d_done, (size_t)B, cudaMemcpyDeviceToHost, stream));
     return check_sticky_errors(s, stream);
+}
+
+}  // extern "C"
+
+// =============================================================================== LM-head step
+namespace {
+
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+EncodeTiledFn encode_tiled_fn() {
+    static EncodeTiledFn fn = [] {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+            q != cudaDriverEntryPointSuccess)
+            p = nullptr;
+        return reinterpret_cast<EncodeTiledFn>(p);
+    }();
+    return fn;
+}
+
+// bf16 [rows, ld] row-major, box = box_rows x 64 elements (128 bytes), 128-byte swizzle, OOB -> 0
+cd_status make_tmap_bf16(CUtensorMap* out, const void* base, long long rows, long long cols, long long ld,
+                         int box_rows) {
+    EncodeTiledFn fn = encode_tiled_fn();
+    if (!fn) return fail(CD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from this driver");
+    const cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
+    const cuuint32_t box[2] = {(cuuint32_t)cd::HD_BK, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = fn(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail(CD_ERR_CUDA, "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return CD_OK;
+}
+
+cd_status get_head_scratch(Scratch* s, int rows, int H, cudaStream_t stream) {
+    if (s->head_rows >= rows && s->head_H >= H) return CD_OK;
+    if (s->head_rows > 0) CU(cudaStreamSynchronize(stream));
+    cudaFree(s->h_flags); cudaFree(s->h_lists); cudaFree(s->h_ctr); cudaFree(s->h_A); cudaFree(s->h_partials);
+    s->h_flags = nullptr; s->h_lists = nullptr; s->h_ctr = nullptr; s->h_A = nullptr; s->h_partials = nullptr;
+    s->head_rows = 0;
+    if (rows < s->cap_rows) rows = s->cap_rows;
+    const long long rows_pad = ((long long)rows + cd::HD_BM - 1) / cd::HD_BM * cd::HD_BM;
+    const long long ldA = ((long long)H + 7) / 8 * 8;
+    CU(cudaMalloc(&s->h_flags, (size_t)rows * 2));
+    CU(cudaMalloc(&s->h_lists, sizeof(int) * (size_t)rows * 4));
+    CU(cudaMalloc(&s->h_ctr, sizeof(int) * 4));
+    CU(cudaMemset(s->h_ctr, 0, sizeof(int) * 4));
+    CU(cudaMalloc(&s->h_A, (size_t)rows_pad * (size_t)ldA * 2));
+    CU(cudaMemset(s->h_A, 0, (size_t)rows_pad * (size_t)ldA * 2));
+    CU(cudaMalloc(&s->h_partials, sizeof(cd::HeadPartial) * (size_t)cd::head_partials_cap(rows)));
+    s->h_ldA = ldA;
+    cd_status st = make_tmap_bf16(&s->h_tmA, s->h_A, rows_pad, H, ldA, cd::HD_BM);
+    if (st != CD_OK) return st;
+    s->head_rows = rows;
+    s->head_H = H;
+    return CD_OK;
+}
+
+// Largest number of transitions a state may have for its rows to be gathered by the LM-head
+// step.  A gathered logit reads one W row (2H bytes, mostly from L2) and costs 2H flops on the
+// CUDA cores; a dense row costs 2VH flops on the tensor cores.  Automatic policy: gather while
+// deg * 2H bytes at ~4 TB/s is below V * 2H flops at ~1.2 PFLOP/s, i.e. deg < V / 300.
+int head_gather_max_for(const cd_dfa* d) {
+    if (d->head_gather_max >= 0) return d->head_gather_max;
+    return d->dev.V / 300 > 1 ? d->dev.V / 300 : 1;
+}
+
+}  // namespace
+
+extern "C" {
+
+cd_status cd_set_head_gather_max(cd_dfa_t* d, int32_t max_transitions) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (max_transitions < -1) return fail(CD_ERR_ARG, "max_transitions must be >= -1");
+    d->head_gather_max = max_transitions;
+    return CD_OK;
+}
+
+cd_status cd_head_step(const cd_dfa_t* d, const void* hidden, int64_t ldh_elems, const void* W, int64_t ldw_elems,
+                       int32_t H, const int32_t* row_map, int32_t* state, int32_t n, int32_t* token_out,
+                       float* logprob_out, float* lse_out, uint8_t* done_out, void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (n < 0) return fail(CD_ERR_ARG, "n < 0");
+    if (H < 8 || (H % 8) != 0) return fail(CD_ERR_ARG, "H (%d) must be a positive multiple of 8", H);
+    if (n == 0) return CD_OK;
+    if (!hidden || !W || !state || !token_out || !logprob_out || !done_out) return fail(CD_ERR_ARG, "NULL pointer");
+    if (ldh_elems < H || ldw_elems < H) return fail(CD_ERR_ARG, "ldh_elems / ldw_elems < H");
+    if ((ldh_elems % 8) != 0 || (ldw_elems % 8) != 0) return fail(CD_ERR_ARG, "row strides must be multiples of 8 elements (16 bytes)");
+    if ((reinterpret_cast<uintptr_t>(hidden) & 15) != 0 || (reinterpret_cast<uintptr_t>(W) & 15) != 0)
+        return fail(CD_ERR_ARG, "hidden / W base is not 16-byte aligned");
+    DeviceGuard guard(d->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* s = nullptr;
+    cd_status st = get_scratch(d, stream, n, false, &s);
+    if (st != CD_OK) return st;
+    st = get_head_scratch(s, n, H, stream);
+    if (st != CD_OK) return st;
+    // tensor map of the output embedding (cached per handle: the weights rarely change)
+    cd_dfa* dm = const_cast<cd_dfa*>(d);
+    {
+        std::lock_guard<std::mutex> lk(dm->mu);
+        if (dm->w_ptr != W || dm->w_ld != ldw_elems || dm->w_H != H) {
+            st = make_tmap_bf16(&dm->w_tmap, W, d->dev.V, H, ldw_elems, cd::HD_BN);
+            if (st != CD_OK) return st;
+            dm->w_ptr = W; dm->w_ld = ldw_elems; dm->w_H = H;
+        }
+    }
+    cd::HeadArgs a{};
+    a.fin.dfa = d->dev;
+    a.fin.row_map = row_map;
+    a.fin.state = state;
+    a.fin.state_new = state;
+    a.fin.n = n;
+    a.fin.token_out = token_out;
+    a.fin.logprob_out = logprob_out;
+    a.fin.lse_out = lse_out;
+    a.fin.done_out = done_out;
+    a.fin.ctrs = s->ctrs;
+    a.hidden = static_cast<const uint16_t*>(hidden);
+    a.ldh = ldh_elems;
+    a.W = static_cast<const uint16_t*>(W);
+    a.ldw = ldw_elems;
+    a.H = H;
+    a.gather_max = head_gather_max_for(d);
+    a.not_dense = s->h_flags;
+    a.not_gather = s->h_flags + s->head_rows;
+    a.dense_slot = s->h_lists;
+    a.dense_state = s->h_lists + s->head_rows;
+    a.gather_slot = s->h_lists + 2 * (size_t)s->head_rows;
+    a.gather_state = s->h_lists + 3 * (size_t)s->head_rows;
+    a.hctr = s->h_ctr;
+    a.A = s->h_A;
+    a.ldA = s->h_ldA;
+    a.partials = s->h_partials;
+
+    cd::head_prepare_kernel<<<1, 1024, 0, stream>>>(a);
+    CU(cudaGetLastError());
+    const bool any_gather = a.gather_max > 0 && d->min_deg_nonacc <= a.gather_max;
+    const bool any_dense = d->max_deg > a.gather_max;
+    int launches = 1;
+    if (any_gather) {
+        const size_t smem = (size_t)H * 2;
+        static thread_local int cfg_dev = -1;
+        if (smem > 48 * 1024 && cfg_dev != d->device) {
+            CU(cudaFuncSetAttribute(cd::head_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            cfg_dev = d->device;
+        }
+        if (smem > 200 * 1024) return fail(CD_ERR_ARG, "H too large for the gather path");
+        cd::head_gather_kernel<<<n, cd::HG_WARPS * 32, smem, stream>>>(a);
+        CU(cudaGetLastError());
+        ++launches;
+    }
+    if (any_dense) {
+        const int rows_per_block = 8;
+        cd::head_pack_kernel<<<(n + rows_per_block - 1) / rows_per_block, rows_per_block * 32, 0, stream>>>(a);
+        CU(cudaGetLastError());
+        static thread_local int cfg_dev2 = -1;
+        if (cfg_dev2 != d->device) {
+            CU(cudaFuncSetAttribute(cd::head_dense_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, cd::HD_SMEM_BYTES));
+            cfg_dev2 = d->device;
+        }
+        cd::head_dense_kernel<<<d->num_sms, cd::HD_THREADS, cd::HD_SMEM_BYTES, stream>>>(s->h_tmA, d->w_tmap, a);
+        CU(cudaGetLastError());
+        cd::head_finish_kernel<<<(n + rows_per_block - 1) / rows_per_block, rows_per_block * 32, 0, stream>>>(a);
+        CU(cudaGetLastError());
+        launches += 3;
+    }
+    g_launches.fetch_add(launches, std::memory_order_relaxed);
+    return CD_OK;
 }
 
 }  // extern "C"

@@ -1,0 +1,473 @@
+// cd_head.cuh -- the constrained step fused with the LM head (include/cd.h
+// cd_head_step).  logits x_i[t] = <hidden_i, W[t]> are never written to HBM:
+//
+//   head_prepare_kernel  classifies the active slots by the density of their automaton state
+//                        (accepting / gathered / dense) and builds the two work lists;
+//   head_gather_kernel   low-density states (tries, option sets): one CTA per row forms exactly
+//                        the allowed logits as gathered dot products (W rows through the CSR
+//                        token list) and finishes the row (masked logsumexp/argmax, transition);
+//   head_pack_kernel     copies the hidden rows of the dense slots into a contiguous A operand;
+//   head_dense_kernel    the dense contraction on the 5th-gen tensor cores: persistent,
+//                        warp-specialised (TMA producer / tcgen05.mma issuer / 4 epilogue warps),
+//                        128x256 fp32 accumulators double-buffered in TMEM, operands staged by
+//                        TMA into 128B-swizzled shared memory.  The epilogue reads the
+//                        accumulator rows with tcgen05.ld and applies the allowed-token bitmask
+//                        of each row's own state to an online (max, sum-exp, argmax) -- one
+//                        partial result per (row, range of vocabulary tiles);
+//   head_finish_kernel   merges the partials of a dense row in a fixed order and does the CSR
+//                        transition + accept test.
+#pragma once
+#include <cuda.h>
+
+#include "cd_common.cuh"
+#include "cd_step.cuh"
+
+namespace cd {
+
+constexpr int HD_BM = 128;   // rows per tile (UMMA M)
+constexpr int HD_BN = 256;   // vocabulary entries per tile (UMMA N)
+constexpr int HD_BK = 64;    // K per pipeline stage: 64 bf16 = one 128-byte swizzle row
+constexpr int HD_UK = 16;    // K per tcgen05.mma (kind::f16)
+constexpr int HD_STAGES = 4;
+constexpr int HD_A_BYTES = HD_BM * HD_BK * 2;  // 16 KiB
+constexpr int HD_B_BYTES = HD_BN * HD_BK * 2;  // 32 KiB
+constexpr int HD_STAGE_BYTES = HD_A_BYTES + HD_B_BYTES;
+constexpr int HD_SMEM_BYTES = HD_STAGES * HD_STAGE_BYTES + 1024;  // + slack to align to 1024 B
+constexpr int HD_THREADS = 192;  // warp 0 TMA, warp 1 MMA + TMEM alloc, warps 2-5 epilogue
+constexpr int HD_TMEM_COLS = 512;
+constexpr int HD_UNITS_TARGET = 148 * 8;
+
+constexpr int HG_WARPS = 8;  // gather kernel: warps per CTA (one CTA per row)
+
+struct __align__(16) HeadPartial {
+    float m, s;
+    int idx, pad;
+};
+
+// Work decomposition of the dense contraction for n_dense rows: unit = (row tile, range of L
+// consecutive vocabulary tiles); a row has NU partial results.  Unit u -> row tile u % num_m,
+// range u / num_m, so that CTAs running at the same time share W tiles through L2.
+struct HeadSched {
+    int num_m, num_n, L, NU;
+};
+__host__ __device__ inline HeadSched head_sched(int n_dense, int V) {
+    HeadSched h;
+    h.num_m = (n_dense + HD_BM - 1) / HD_BM;
+    h.num_n = (V + HD_BN - 1) / HD_BN;
+    int nu0 = h.num_m > 0 ? (HD_UNITS_TARGET + h.num_m - 1) / h.num_m : 1;
+    if (nu0 > h.num_n) nu0 = h.num_n;
+    if (nu0 < 1) nu0 = 1;
+    h.L = (h.num_n + nu0 - 1) / nu0;
+    h.NU = (h.num_n + h.L - 1) / h.L;
+    return h;
+}
+// upper bound of rows_pad * NU over n_dense <= n (capacity of the partial buffer)
+__host__ inline long long head_partials_cap(int n) {
+    const long long num_m = (n + HD_BM - 1) / HD_BM;
+    return (long long)HD_BM * (HD_UNITS_TARGET + 2 * num_m + 2);
+}
+
+struct HeadArgs {
+    StepArgs fin;  // dfa, outputs, sticky counters, optional loop history (see finalize_row);
+                   // fin.state_new == fin.state: nothing reads state[] after head_prepare_kernel
+    const uint16_t* hidden;  // [rows, ldh] bf16
+    long long ldh;
+    const uint16_t* W;  // [V, ldw] bf16
+    long long ldw;
+    int H;
+    int gather_max;  // states with <= gather_max transitions are gathered
+    // scratch
+    uint8_t* not_dense;   // [n]
+    uint8_t* not_gather;  // [n]
+    int* dense_slot;      // [n] slot of dense row d
+    int* dense_state;     // [n]
+    int* gather_slot;     // [n]
+    int* gather_state;    // [n]
+    int* hctr;            // [0] n_dense, [1] n_gather
+    uint16_t* A;          // [rows_pad, ldA] packed hidden rows of the dense slots
+    long long ldA;
+    HeadPartial* partials;  // [rows_pad * NU]
+};
+
+// ---------------------------------------------------------------- sm_100a PTX: TMA, tcgen05
+__device__ __forceinline__ void tma_prefetch_desc(const void* tmap) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
+}
+
+// 2-D tiled TMA load global -> shared, completion (bytes) on an mbarrier.  c0 = inner coordinate.
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const void* tmap, int c0, int c1, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
+        "l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1), "r"(bar)
+        : "memory");
+}
+
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+
+// tcgen05.commit: the mbarrier gets one arrival when every tcgen05.mma issued so far by this
+// thread has completed (implies tcgen05.fence::before_thread_sync).
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+
+// D[tmem] (+)= A[smem] * B[smem]^T, bf16 x bf16 -> fp32, one thread issues for the CTA.
+__device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                            uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+// Shared-memory matrix descriptor of a K-major tile whose rows are 128 bytes (64 bf16) in the
+// 128-byte swizzle TMA writes: 8-row groups 1024 bytes apart (SBO), descriptor version 1
+// (Blackwell), layout type 2 = SWIZZLE_128B.  The tile base is 1024-byte aligned; a K step of
+// 16 elements inside the swizzle row advances the start address by 32 bytes.
+__device__ __forceinline__ uint64_t umma_desc_k_sw128(uint32_t smem_addr) {
+    return (uint64_t)((smem_addr >> 4) & 0x3FFFu) | (1ull << 16) | (64ull << 32) | (1ull << 46) | (2ull << 61);
+}
+
+// Instruction descriptor, kind::f16: D fp32 (bits 4-5 = 1), A and B bf16 (bits 7-9, 10-12 = 1),
+// both K-major (bits 15, 16 = 0), N >> 3 at bits 17-22, M >> 4 at bits 24-28.
+__host__ __device__ constexpr uint32_t umma_idesc_bf16(int M, int N) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+}
+
+// 32 consecutive fp32 columns of this thread's TMEM lane (lane = quadrant base + laneid).
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// ---------------------------------------------------------------- prepare: classify + lists
+// One CTA of 1024 threads.  A slot whose state already accepts (or is out of range) is finished
+// here; the others go to the gather list (state has <= gather_max
+// transitions) or to the dense list, both in slot order.
+__global__ void __launch_bounds__(1024, 1) head_prepare_kernel(const HeadArgs a) {
+    const StepArgs& f = a.fin;
+    const int n = f.n_dev ? __ldcg(f.n_dev) : f.n;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        const int st = f.state[i];
+        const bool bad = (st < 0) || (st >= f.dfa.S);
+        const bool acc = !bad && (__ldg(f.dfa.accepting + st) != 0);
+        uint8_t nd = 1, ng = 1;
+        if (bad || acc) {
+            f.token_out[i] = -1;
+            f.logprob_out[i] = 0.0f;
+            if (f.lse_out) f.lse_out[i] = 0.0f;
+            f.done_out[i] = 1;
+            if (bad) atomicAdd(f.ctrs + 2, 1);
+        } else {
+            const int deg = (int)(__ldg(f.dfa.row_ptr + st + 1) - __ldg(f.dfa.row_ptr + st));
+            if (deg <= a.gather_max) ng = 0; else nd = 0;
+        }
+        a.not_dense[i] = nd;
+        a.not_gather[i] = ng;
+    }
+    __syncthreads();
+    block_compact(a.not_dense, nullptr, f.state, n, a.dense_slot, a.dense_state, a.hctr + 0);
+    __syncthreads();
+    block_compact(a.not_gather, nullptr, f.state, n, a.gather_slot, a.gather_state, a.hctr + 1);
+}
+
+// ---------------------------------------------------------------- pack: dense rows -> A
+// One warp per dense row, 16-byte copies (H % 8 == 0, rows 16-byte aligned).
+__global__ void head_pack_kernel(const HeadArgs a) {
+    const int n_dense = __ldcg(a.hctr + 0);
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    const int nv = a.H >> 3;
+    for (int d = warp; d < n_dense; d += nwarps) {
+        const int slot = __ldcg(a.dense_slot + d);
+        const long long r = a.fin.row_map ? (long long)__ldg(a.fin.row_map + slot) : (long long)slot;
+        const uint4* src = reinterpret_cast<const uint4*>(a.hidden + r * a.ldh);
+        uint4* dst = reinterpret_cast<uint4*>(a.A + (long long)d * a.ldA);
+        for (int v = lane; v < nv; v += 32) dst[v] = __ldg(src + v);
+    }
+}
+
+// ---------------------------------------------------------------- gather: low-density states
+__device__ __forceinline__ float dot8(const uint4& w, const uint4& h, float acc) {
+    const uint32_t wu[4] = {w.x, w.y, w.z, w.w}, hu[4] = {h.x, h.y, h.z, h.w};
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        acc = fmaf(__uint_as_float(wu[q] << 16), __uint_as_float(hu[q] << 16), acc);
+        acc = fmaf(__uint_as_float(wu[q] & 0xFFFF0000u), __uint_as_float(hu[q] & 0xFFFF0000u), acc);
+    }
+    return acc;
+}
+
+// One CTA per gathered row: the hidden row is staged in shared memory, the warps split the
+// state's CSR token list into contiguous pieces, four dot products in flight per warp; the
+// running argmax is the CSR position (ascending token id), so the transition needs no search.
+__global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadArgs a) {
+    extern __shared__ __align__(16) unsigned char hg_smem[];
+    uint4* hid = reinterpret_cast<uint4*>(hg_smem);
+    __shared__ float s_m[HG_WARPS], s_s[HG_WARPS];
+    __shared__ int s_i[HG_WARPS];
+    const StepArgs& f = a.fin;
+    const int n_gather = __ldcg(a.hctr + 1);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int nv = a.H >> 3;
+    for (int g = blockIdx.x; g < n_gather; g += gridDim.x) {
+        const int slot = __ldcg(a.gather_slot + g);
+        const int st = __ldcg(a.gather_state + g);
+        const long long r = f.row_map ? (long long)__ldg(f.row_map + slot) : (long long)slot;
+        const uint4* src = reinterpret_cast<const uint4*>(a.hidden + r * a.ldh);
+        __syncthreads();  // previous row's readers are done with hid / s_*
+        for (int v = threadIdx.x; v < nv; v += blockDim.x) hid[v] = __ldg(src + v);
+        __syncthreads();
+        const long long lo = __ldg(f.dfa.row_ptr + st);
+        const int deg = (int)(__ldg(f.dfa.row_ptr + st + 1) - lo);
+        const int j0 = (int)(((long long)deg * warp) / HG_WARPS);
+        const int j1 = (int)(((long long)deg * (warp + 1)) / HG_WARPS);
+        float m = -INFINITY, s = 0.0f;
+        int idx = 0x7FFFFFFF;
+        for (int j = j0; j < j1; j += 4) {
+            const uint4* wp[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int jq = (j + q < j1) ? j + q : j1 - 1;
+                wp[q] = reinterpret_cast<const uint4*>(a.W + (long long)__ldg(f.dfa.tok + lo + jq) * a.ldw);
+            }
+            float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+            for (int v = lane; v < nv; v += 32) {
+                const uint4 h = hid[v];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) acc[q] = dot8(__ldg(wp[q] + v), h, acc[q]);
+            }
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q) acc[q] += __shfl_xor_sync(FULL, acc[q], o);
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                if (j + q < j1) online_update(m, s, idx, fmaxf(acc[q], -INFINITY), j + q);  // NaN -> -inf
+        }
+        if (lane == 0) {
+            s_m[warp] = m;
+            s_s[warp] = s;
+            s_i[warp] = idx;
+        }
+        __syncthreads();
+        if (warp == 0) {
+            float rm = (lane < HG_WARPS) ? s_m[lane] : -INFINITY;
+            float rs = (lane < HG_WARPS) ? s_s[lane] : 0.0f;
+            int ri = (lane < HG_WARPS) ? s_i[lane] : 0x7FFFFFFF;
+            warp_combine(rm, rs, ri);
+            const TileMeta mt{slot, 0, 0, st, lo, deg, 0};
+            finalize_row(f, mt, rm, rs, ri, lane, true);
+        }
+    }
+}
+
+// ---------------------------------------------------------------- dense: tcgen05 contraction
+// Persistent kernel, one CTA per SM.  Barriers:
+//   full[s]  / empty[s]   shared-memory stage s: TMA -> MMA / MMA (tcgen05.commit) -> TMA
+//   tfull[b] / tempty[b]  accumulator buffer b (256 TMEM columns): MMA -> epilogue / back
+// Every role walks the same sequence (units of this CTA -> vocabulary tiles -> K blocks), so
+// stage and phase counters stay in step without any other communication.
+__global__ void __launch_bounds__(HD_THREADS, 1)
+head_dense_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmW, const HeadArgs a) {
+    extern __shared__ __align__(1024) unsigned char hd_smem[];
+    __shared__ __align__(8) unsigned long long bar_full[HD_STAGES], bar_empty[HD_STAGES], bar_tfull[2], bar_tempty[2];
+    __shared__ uint32_t s_tmem;
+
+    const int n_dense = __ldcg(a.hctr + 0);
+    const HeadSched hs = head_sched(n_dense, a.fin.dfa.V);
+    if (hs.num_m == 0) return;  // uniform: nothing was allocated yet
+    const int total_units = hs.num_m * hs.NU;
+    const int num_k = (a.H + HD_BK - 1) / HD_BK;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t tiles = (smem_u32(hd_smem) + 1023u) & ~1023u;
+
+    if (warp == 0 && lane == 0) {
+        tma_prefetch_desc(&tmA);
+        tma_prefetch_desc(&tmW);
+#pragma unroll
+        for (int s = 0; s < HD_STAGES; ++s) {
+            mbar_init(smem_u32(&bar_full[s]), 1);
+            mbar_init(smem_u32(&bar_empty[s]), 1);
+        }
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(smem_u32(&bar_tfull[b]), 1);
+            mbar_init(smem_u32(&bar_tempty[b]), 4);  // one arrival per epilogue warp
+        }
+        fence_mbar_init();
+    }
+    if (warp == 1) tmem_alloc(smem_u32(&s_tmem), HD_TMEM_COLS);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = s_tmem;
+
+    if (warp == 0) {
+        // ===== TMA producer (one lane)
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int u = blockIdx.x; u < total_units; u += gridDim.x) {
+                const int m_tile = u % hs.num_m, n_unit = u / hs.num_m;
+                const int nt0 = n_unit * hs.L, nt1 = min(nt0 + hs.L, hs.num_n);
+                for (int nt = nt0; nt < nt1; ++nt) {
+                    for (int kb = 0; kb < num_k; ++kb) {
+                        mbar_wait(smem_u32(&bar_empty[stage]), phase ^ 1u);
+                        const uint32_t bar = smem_u32(&bar_full[stage]);
+                        const uint32_t sa = tiles + stage * HD_STAGE_BYTES;
+                        mbar_arrive_expect_tx(bar, HD_STAGE_BYTES);
+                        tma_load_2d(sa, &tmA, kb * HD_BK, m_tile * HD_BM, bar);
+                        tma_load_2d(sa + HD_A_BYTES, &tmW, kb * HD_BK, nt * HD_BN, bar);
+                        if (++stage == HD_STAGES) {
+                            stage = 0;
+                            phase ^= 1u;
+                        }
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (one lane)
+        if (lane == 0) {
+            constexpr uint32_t idesc = umma_idesc_bf16(HD_BM, HD_BN);
+            int stage = 0, ab = 0;
+            uint32_t phase = 0, aphase = 0;
+            for (int u = blockIdx.x; u < total_units; u += gridDim.x) {
+                const int n_unit = u / hs.num_m;
+                const int nt0 = n_unit * hs.L, nt1 = min(nt0 + hs.L, hs.num_n);
+                for (int nt = nt0; nt < nt1; ++nt) {
+                    mbar_wait(smem_u32(&bar_tempty[ab]), aphase ^ 1u);  // epilogue drained this buffer
+                    tc_fence_after();
+                    const uint32_t d_tmem = tmem + (uint32_t)ab * HD_BN;
+                    for (int kb = 0; kb < num_k; ++kb) {
+                        mbar_wait(smem_u32(&bar_full[stage]), phase);
+                        tc_fence_after();
+                        const uint32_t sa = tiles + stage * HD_STAGE_BYTES;
+                        const uint64_t da = umma_desc_k_sw128(sa), db = umma_desc_k_sw128(sa + HD_A_BYTES);
+#pragma unroll
+                        for (int k = 0; k < HD_BK / HD_UK; ++k)
+                            tc_mma_bf16(d_tmem, da + 2ull * k, db + 2ull * k, idesc, (kb | k) ? 1u : 0u);
+                        tc_commit(smem_u32(&bar_empty[stage]));  // stage free once these MMAs have read it
+                        if (++stage == HD_STAGES) {
+                            stage = 0;
+                            phase ^= 1u;
+                        }
+                    }
+                    tc_commit(smem_u32(&bar_tfull[ab]));  // accumulator complete
+                    ab ^= 1;
+                    if (ab == 0) aphase ^= 1u;
+                }
+            }
+        }
+    } else {
+        // ===== epilogue: thread <-> accumulator row (TMEM lane); a warp may only touch the lane
+        // quadrant warp_id % 4
+        const int quad = warp & 3;
+        const int row_in_tile = quad * 32 + lane;
+        const DfaDev& dfa = a.fin.dfa;
+        int ab = 0;
+        uint32_t aphase = 0;
+        for (int u = blockIdx.x; u < total_units; u += gridDim.x) {
+            const int m_tile = u % hs.num_m, n_unit = u / hs.num_m;
+            const int nt0 = n_unit * hs.L, nt1 = min(nt0 + hs.L, hs.num_n);
+            const int drow = m_tile * HD_BM + row_in_tile;
+            const bool valid = drow < n_dense;
+            const int st = valid ? __ldcg(a.dense_state + drow) : 0;
+            const uint32_t* mrow = dfa.mask + (long long)st * dfa.Wpad;
+            float m = -INFINITY, s = 0.0f;
+            int idx = 0x7FFFFFFF;
+            for (int nt = nt0; nt < nt1; ++nt) {
+                const int n0 = nt * HD_BN;
+                // the 8 mask words of this row for the tile's 256 tokens (two 16-byte loads)
+                uint32_t mw[8];
+                {
+                    const int w0 = n0 >> 5;
+                    uint4 lo4 = make_uint4(0, 0, 0, 0), hi4 = make_uint4(0, 0, 0, 0);
+                    if (valid && w0 + 3 < dfa.Wpad) lo4 = __ldg(reinterpret_cast<const uint4*>(mrow + w0));
+                    if (valid && w0 + 7 < dfa.Wpad) hi4 = __ldg(reinterpret_cast<const uint4*>(mrow + w0 + 4));
+                    mw[0] = lo4.x; mw[1] = lo4.y; mw[2] = lo4.z; mw[3] = lo4.w;
+                    mw[4] = hi4.x; mw[5] = hi4.y; mw[6] = hi4.z; mw[7] = hi4.w;
+                }
+                mbar_wait(smem_u32(&bar_tfull[ab]), aphase);
+                tc_fence_after();
+                const uint32_t tbase = tmem + ((uint32_t)(quad * 32) << 16) + (uint32_t)ab * HD_BN;
+#pragma unroll
+                for (int c = 0; c < HD_BN / 32; ++c) {
+                    const uint32_t bits = mw[c];
+                    if (__any_sync(FULL, bits != 0u)) {  // warp-uniform: skip columns nobody allows
+                        uint32_t v[32];
+                        tmem_ld32(tbase + c * 32, v);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int j = 0; j < 32; ++j)
+                            if ((bits >> j) & 1u)
+                                online_update(m, s, idx, fmaxf(__uint_as_float(v[j]), -INFINITY), n0 + c * 32 + j);
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(smem_u32(&bar_tempty[ab]));
+                ab ^= 1;
+                if (ab == 0) aphase ^= 1u;
+            }
+            if (valid) a.partials[(long long)drow * hs.NU + n_unit] = HeadPartial{m, s, idx, 0};
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    if (warp == 1) tmem_dealloc(tmem, HD_TMEM_COLS);
+}
+
+// ---------------------------------------------------------------- finish dense rows
+// One warp per dense row: partials merged in a fixed order (lane q % 32 takes ranges q, q + 32,
+// ... ascending, then the butterfly), then the CSR transition and the accept test.
+__global__ void head_finish_kernel(const HeadArgs a) {
+    const StepArgs& f = a.fin;
+    const int n_dense = __ldcg(a.hctr + 0);
+    const HeadSched hs = head_sched(n_dense, f.dfa.V);
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    for (int d = warp; d < n_dense; d += nwarps) {
+        const int slot = __ldcg(a.dense_slot + d);
+        const int st = __ldcg(a.dense_state + d);
+        float m = -INFINITY, s = 0.0f;
+        int idx = 0x7FFFFFFF;
+        for (int q = lane; q < hs.NU; q += 32) {
+            const int4 p = __ldcg(reinterpret_cast<const int4*>(a.partials + (long long)d * hs.NU + q));
+            online_combine(m, s, idx, __int_as_float(p.x), __int_as_float(p.y), p.z);
+        }
+        warp_combine(m, s, idx);
+        const long long lo = __ldg(f.dfa.row_ptr + st);
+        const int deg = (int)(__ldg(f.dfa.row_ptr + st + 1) - lo);
+        const TileMeta mt{slot, 0, 0, st, lo, deg, 0};
+        finalize_row(f, mt, m, s, idx, lane, false);
+    }
+}
+
+}  // namespace cd
