@@ -40,6 +40,9 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel from the
 # `ncu --set full` capture summarised in profiles/ (None until a capture exists for this
 # workload); keyed by config name.
+FALLBACK_BF16_TFLOPS = 1590.0  # /opt/skills/guides/B200_PROFILING.md fallback
+# DRAM read + write bytes of one head_dense_kernel launch from the ncu --set full capture in profiles/
+NCU_HEAD_TRAFFIC_BYTES = {}
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {
     # profiles/r1c_step_kernel_c4.md, step 0 (n = 4096): 2,148,744,000 read + 4,729,344 written
     "c4": 2148744000 + 4729344,
@@ -60,6 +63,8 @@ def parse_args():
                          "-1 = automatic, > 0 = threshold (SURVEY 8(f) N1)")
     ap.add_argument("--no-adaptive", action="store_true", help="skip the density-adaptive (gather) measurement")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-head", action="store_true", help="skip the LM-head fused step measurement (SURVEY 8(f) N2)")
+    ap.add_argument("--head-H", type=int, default=2560, help="hidden size of the LM head (Gemma 3 4B: 2560)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--verbose", action="store_true", help="per-launch table of the step kernel on stderr")
     return ap.parse_args()
@@ -130,6 +135,90 @@ class ClockSampler:
             return None
         return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "reasons": sorted(reasons),
                 "samples": len(sm)}
+
+
+def measured_tensor_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            j = json.load(open(p))
+            return float(j["bf16_tflops"]), float(j.get("bf16_tflops_sustained", j["bf16_tflops"])), \
+                "measured (MEASURED_PEAKS.json bf16_tflops, burst)"
+        except Exception:
+            pass
+    return FALLBACK_BF16_TFLOPS, FALLBACK_BF16_TFLOPS, "fallback (B200_PROFILING.md)"
+
+
+def head_section(cd, cfg, aut, dfa, device, H, iters, warmup):
+    """one constrained step fused with the LM head (cd_head_step) for B rows spread
+    over the automaton's live states (the state mix of a mid-loop step), W [V, H] bf16 ~ N(0, 2/sqrt(H)),
+    hidden ~ N(0,1).  W (1.34 GB at H=2560) is larger than L2, so every call streams it from HBM.
+    The dominant kernel is the tcgen05 contraction (bound: tensor); its algorithmic flops are
+    2 * n_dense * V * H per call.  The unfused alternative (library GEMM writing bf16 logits, then
+    cd_step reading them) is timed beside it."""
+    V, n = cfg.V, cfg.B
+    stream = torch.cuda.current_stream()
+    W = wl.make_head(7, V, H, 2.0, device=device)
+    hid = wl.make_hidden(cfg.seed, 0, n, H, device=device)
+    acc = torch.as_tensor(aut.accepting)
+    live = torch.nonzero(acc == 0).flatten().to(torch.int32)
+    st0 = live[(torch.arange(n) * 7) % live.numel()].to(device) if cfg.kind == "dfa" else \
+        torch.zeros(n, dtype=torch.int32, device=device)
+    st = st0.clone()
+    i32 = dict(dtype=torch.int32, device=device)
+    outb = (torch.empty(n, **i32), torch.empty(n, dtype=torch.float32, device=device),
+            torch.empty(n, dtype=torch.float32, device=device), torch.empty(n, dtype=torch.uint8, device=device))
+    deg = torch.diff(torch.as_tensor(aut.row_ptr))
+    auto_max = max(1, V // 300)  # the library's automatic threshold (cd_api.cu head_gather_max_for)
+    n_dense = int((deg[st0.cpu().long()] > auto_max).sum())
+
+    def timed(fn):
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(iters):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / iters
+
+    def fused():
+        st.copy_(st0)
+        cd.head_step(dfa, hid, W, st, out=outb)
+
+    l0 = cd.launch_count()
+    ms_f = timed(fused)
+    launches = (cd.launch_count() - l0) // (iters + warmup)
+    tok_f = outb[0].clone()
+    logits = torch.empty((n, V), dtype=torch.bfloat16, device=device)
+
+    def unfused():
+        st.copy_(st0)
+        torch.matmul(hid, W.t(), out=logits)
+        cd.step(dfa, logits, st, out=outb)
+
+    ms_u = timed(unfused)
+    agree = float((tok_f == outb[0]).float().mean())  # bf16 rounding of the logits may flip near-ties
+    ms_g = timed(lambda: torch.matmul(hid, W.t(), out=logits))
+    del logits
+    burst, sustained, src = measured_tensor_peak()
+    flops = 2.0 * n_dense * V * H
+    ach = flops / (ms_f * 1e-3) / 1e12 if n_dense else 0.0
+    return {
+        "workload": f"{cfg.name}: one cd_head_step, n={n} rows over the live states, V={V}, H={H} bf16 "
+                    f"(Gemma 3 4B head shape, PAPER.md L191), {n_dense} rows dense / {n - n_dense} gathered",
+        "ms_per_step": ms_f, "row_steps_per_s": n / (ms_f * 1e-3), "gpu_launches_per_step": int(launches),
+        "unfused_ms_per_step": ms_u, "library_gemm_ms": ms_g, "speedup_vs_unfused": ms_u / ms_f,
+        "token_agreement_with_unfused_bf16_logits": agree,
+        "roofline": {"bound": "tensor", "kernel": "cd::head_dense_kernel (tcgen05 128x256x64, masked online-softmax epilogue from TMEM)",
+                     "achieved": ach, "peak": burst, "unit": "TFLOP/s", "frac": ach / burst if burst else None,
+                     "peak_source": src, "frac_of_sustained_peak": ach / sustained if sustained else None,
+                     "frac_of_nominal_2250": ach / 2250.0, "flops_per_launch": flops,
+                     "note": "timed over the whole call (prepare + pack + contraction + finish), so the kernel's own rate is higher",
+                     "traffic": NCU_HEAD_TRAFFIC_BYTES.get(cfg.name)},
+    }
 
 
 def build_inputs(cfg, device, n_batches, batch0):
@@ -419,6 +508,13 @@ def main():
         got = cd.decode_loop(dfa, batches[0], max_steps=cfg.max_steps)
         assert np.array_equal(got["tokens"][:R].cpu().numpy(), res["tokens"]), "bench parity check failed"
 
+    head = None
+    if rank == 0 and not args.no_head:
+        try:
+            head = head_section(cd, cfg, aut, dfa, device, args.head_H, max(3, min(args.steps, 10)), 3)
+        except Exception as ex:
+            head = {"error": str(ex)[:300]}
+
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -441,6 +537,7 @@ def main():
             "roofline": roofline,
             "adaptive": adaptive,
             "cpu_baseline": cpu,
+            "head": head,
             "paper_context": "PAPER.md L17-18/L32: 390x lower cost, 3.8x lower latency than a proprietary API with a "
                              "quantized model on one 16 GB GPU; no per-step number is published (BASELINE.md)",
         }

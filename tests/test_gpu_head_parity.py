@@ -57,7 +57,9 @@ def dev_dfa(cd, aut, mode):
 def eps_x(hid, W, H):
     """Bound of |fp32-accumulated logit - exact logit| for these operands."""
     a = hid[:, :H].abs().to(torch.float64).max(dim=0).values  # per-h max over rows
-    A = float((W[:, :H].abs().to(torch.float64) @ a).max())    # >= sum_h |a_h||w_h| for every (row, token)
+    A = 0.0  # >= sum_h |a_h||w_h| for every (row, token)
+    for t0 in range(0, W.shape[0], 16384):
+        A = max(A, float((W[t0:t0 + 16384, :H].abs().to(torch.float64) @ a).max()))
     return (H / 16 + 40) * 2.0**-23 * A
 
 
@@ -70,14 +72,20 @@ def transitions(aut):
     return d
 
 
-def run_case(cd, oracle, aut, dfa, hid, W, H, states, row_map=None, exact=True):
+def run_case(cd, oracle, aut, dfa, hid, W, H, states, row_map=None, exact=True, check=None, W_dev=None):
+    """GPU on every slot; the oracle on the slots listed in `check` (default: all)."""
     dev = "cuda:0"
-    hid_d, W_d = hid.to(dev), W.to(dev)
+    hid_d, W_d = hid.to(dev), (W.to(dev) if W_dev is None else W_dev)
     st_d = torch.tensor(states, dtype=torch.int32, device=dev)
     rm_d = None if row_map is None else torch.tensor(row_map, dtype=torch.int32, device=dev)
     tok, lp, lse, done = cd.head_step(dfa, hid_d, W_d, st_d, row_map=rm_d, H=H)
     torch.cuda.synchronize()
     tok, lp, lse, done, st_new = (t.cpu().numpy() for t in (tok, lp, lse, done, st_d))
+    if check is not None:
+        check = list(check)
+        tok, lp, lse, done, st_new = (x[check] for x in (tok, lp, lse, done, st_new))
+        row_map = [(i if row_map is None else row_map[i]) for i in check]
+        states = [states[i] for i in check]
     o_tok, o_lp, o_lse, o_done, o_st, gap = oracle.head_step(aut, hid, W, H, states, row_map=row_map)
     n = len(states)
     if exact:
@@ -216,3 +224,36 @@ def test_arguments(cd):
     deg = int(aut.row_ptr[1] - aut.row_ptr[0])
     assert tok.cpu().tolist() == [int(aut.tok[0])] * 4
     assert abs(float(lp[0]) + np.log(deg)) < 1e-5
+
+
+# ---------------------------------------------------------------- full size (V = 262144, H = 2560)
+@pytest.fixture(scope="module")
+def full_head():
+    """Output embedding of the bench configuration, exact and gaussian, on both sides."""
+    V, H = 262144, 2560
+    out = {}
+    for kind, exact in (("exact", True), ("gauss", False)):
+        Wd = wl.make_head(7, V, H, 2.0, device="cuda:0", exact=exact)
+        out[kind] = (Wd, Wd.cpu())
+    return V, H, out
+
+
+@pytest.mark.parametrize("kind", ["exact", "gauss"])
+@pytest.mark.parametrize("name,n_check", [("c2", 1024), ("c3", 40), ("c4", 48)])
+def test_full_size_configs(cd, oracle, full_head, kind, name, n_check):
+    """BASELINE.json configs c2-c4 at full size in the launch configuration bench.py times
+    (automatic gather threshold): every row on the GPU, the oracle on sampled rows (rows are
+    independent)."""
+    V, H, Ws = full_head
+    W_dev, W_cpu = Ws[kind]
+    cfg = wl.CONFIGS[name]
+    aut = wl.build_automaton(cfg)
+    dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device="cuda:0")
+    n = cfg.B
+    hid = wl.make_hidden(cfg.seed, 0, n, H, exact=(kind == "exact"))
+    if cfg.kind == "dfa":
+        states = live_states(aut, n, mult=7)
+    else:
+        states = live_states(aut, n, mult=1)  # every trie node, root included
+    check = sorted(set(int(i) for i in np.linspace(0, n - 1, n_check).astype(int)))
+    run_case(cd, oracle, aut, dfa, hid, W_cpu, H, states, exact=(kind == "exact"), check=check, W_dev=W_dev)
