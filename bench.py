@@ -42,7 +42,10 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 # workload); keyed by config name.
 FALLBACK_BF16_TFLOPS = 1590.0  # /opt/skills/guides/B200_PROFILING.md fallback
 # DRAM read + write bytes of one head_dense_kernel launch from the ncu --set full capture in profiles/
-NCU_HEAD_TRAFFIC_BYTES = {}
+NCU_HEAD_TRAFFIC_BYTES = {
+    # profiles/r1e_head_dense_c4.md: 1,644,181,000 read + 6,551,040 written
+    "c4": 1644181000 + 6551040,
+}
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {
     # profiles/r1c_step_kernel_c4.md, step 0 (n = 4096): 2,148,744,000 read + 4,729,344 written
     "c4": 2148744000 + 4729344,
@@ -206,19 +209,30 @@ def head_section(cd, cfg, aut, dfa, device, H, iters, warmup):
     burst, sustained, src = measured_tensor_peak()
     flops = 2.0 * n_dense * V * H
     ach = flops / (ms_f * 1e-3) / 1e12 if n_dense else 0.0
-    return {
+    if n_dense == 0:
+        # every row gathered: the call reads deg W rows of 2H bytes per row (mostly from L2: rows in
+        # the same state share them) -- no dense contraction, no tensor roofline
+        gbytes = float(deg[st0.cpu().long()].sum()) * 2 * H
+        roof = {"bound": "hbm", "kernel": "cd::head_gather_kernel (gathered dot products through the CSR token list)",
+                "achieved": gbytes / (ms_f * 1e-3) / 1e9, "peak": measured_peak()[0], "unit": "GB/s",
+                "frac": gbytes / (ms_f * 1e-3) / 1e9 / measured_peak()[0], "traffic": None,
+                "note": "bytes = W rows touched (2H each), served by L2 when rows share a state; launch-latency bound at this size"}
+    else:
+        roof = None
+    head = {
         "workload": f"{cfg.name}: one cd_head_step, n={n} rows over the live states, V={V}, H={H} bf16 "
                     f"(Gemma 3 4B head shape, PAPER.md L191), {n_dense} rows dense / {n - n_dense} gathered",
         "ms_per_step": ms_f, "row_steps_per_s": n / (ms_f * 1e-3), "gpu_launches_per_step": int(launches),
         "unfused_ms_per_step": ms_u, "library_gemm_ms": ms_g, "speedup_vs_unfused": ms_u / ms_f,
         "token_agreement_with_unfused_bf16_logits": agree,
-        "roofline": {"bound": "tensor", "kernel": "cd::head_dense_kernel (tcgen05 128x256x64, masked online-softmax epilogue from TMEM)",
+        "roofline": roof or {"bound": "tensor", "kernel": "cd::head_dense_kernel (tcgen05 128x256x64, masked online-softmax epilogue from TMEM)",
                      "achieved": ach, "peak": burst, "unit": "TFLOP/s", "frac": ach / burst if burst else None,
                      "peak_source": src, "frac_of_sustained_peak": ach / sustained if sustained else None,
                      "frac_of_nominal_2250": ach / 2250.0, "flops_per_launch": flops,
                      "note": "timed over the whole call (prepare + pack + contraction + finish), so the kernel's own rate is higher",
                      "traffic": NCU_HEAD_TRAFFIC_BYTES.get(cfg.name)},
     }
+    return head
 
 
 def build_inputs(cfg, device, n_batches, batch0):
