@@ -261,6 +261,19 @@ CD_API cd_status cd_head_step(const cd_dfa_t* dfa, const void* hidden, int64_t l
                        int32_t* token_out, float* logprob_out, float* lse_out, uint8_t* done_out,
                        void* cuda_stream);
 
+/*
+ * The decode loop on top of cd_head_step (cd_decode_loop with the LM head fused in):
+ * step_hidden[k] (DEVICE pointers in a HOST array) are the final hidden states of
+ * decoding step k, [B, ldh_elems] bf16 indexed by ORIGINAL row id -- the output of the
+ * model forward, which is outside this library.  Outputs and semantics as
+ * cd_decode_loop; the active count stays on the device; the stream is synchronised once
+ * before returning.
+ */
+CD_API cd_status cd_head_decode_loop(const cd_dfa_t* dfa, const void* const* step_hidden, int64_t ldh_elems,
+                              const void* W, int64_t ldw_elems, int32_t H, int32_t B, int32_t max_steps,
+                              int32_t* tokens_out, int32_t* len_out, int32_t* final_state_out,
+                              float* sum_logprob_out, uint8_t* done_out, void* cuda_stream);
+
 /* Number of kernel launches this library has enqueued from the calling thread's
    process so far (monotone; used by bench.py to report gpu_launches). */
 CD_API int64_t cd_launch_count(void);

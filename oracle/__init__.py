@@ -8,6 +8,7 @@ from .oracle_cd import (  # noqa: F401
     build,
     compact,
     decode_loop,
+    head_decode_loop,
     head_logit,
     head_step,
     step,

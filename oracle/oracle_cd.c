@@ -352,3 +352,63 @@ int orc_head_step(int32_t V, int32_t S, const int64_t *row_ptr, const int32_t *t
     }
     return ORC_OK;
 }
+
+/*
+ * O7: the decode loop (O4) on top of the LM-head step (O6): step_hidden[k] is the [B, ldh]
+ * bf16 array of final hidden states of decoding step k, indexed by ORIGINAL row id (the
+ * model forward that produces it is outside the path).  Everything else as O4.
+ */
+int orc_head_decode_loop(int32_t V, int32_t S, int32_t start, const int64_t *row_ptr, const int32_t *tok,
+                         const int32_t *next, const uint8_t *accepting, const uint16_t *const *step_hidden,
+                         int64_t ldh, const uint16_t *W, int64_t ldw, int32_t H, int32_t B, int32_t max_steps,
+                         int32_t *tokens_out, int32_t *len_out, int32_t *final_state_out,
+                         double *sum_logprob_out, uint8_t *done_out, int32_t *n_active_hist)
+{
+    if (B < 0 || max_steps < 0) return ORC_ERR_ARG;
+    int32_t *ids = (int32_t *)malloc(sizeof(int32_t) * (size_t)(B + 1) * 5);
+    double *lp = (double *)malloc(sizeof(double) * (size_t)(B + 1) * 2);
+    uint8_t *dn = (uint8_t *)malloc((size_t)B + 1);
+    if (!ids || !lp || !dn) {
+        free(ids); free(lp); free(dn);
+        return ORC_ERR_ARG;
+    }
+    int32_t *st = ids + (B + 1), *ids2 = ids + 2 * (B + 1), *st2 = ids + 3 * (B + 1), *tk = ids + 4 * (B + 1);
+    double *lse = lp + (B + 1);
+    for (int32_t r = 0; r < B; ++r) {
+        for (int32_t k = 0; k < max_steps; ++k) tokens_out[(int64_t)r * max_steps + k] = -1;
+        len_out[r] = 0;
+        final_state_out[r] = start;
+        sum_logprob_out[r] = 0.0;
+        done_out[r] = accepting[start] ? 1 : 0;
+    }
+    int32_t n = 0;
+    if (!accepting[start])
+        for (int32_t r = 0; r < B; ++r) {
+            ids[n] = r;
+            st[n] = start;
+            ++n;
+        }
+    int rc = ORC_OK;
+    for (int32_t k = 0; k < max_steps; ++k) {
+        if (n_active_hist) n_active_hist[k] = n;
+        if (n == 0) continue;
+        rc = orc_head_step(V, S, row_ptr, tok, next, accepting, step_hidden[k], ldh, W, ldw, H, ids, st, n, tk, lp,
+                           lse, dn, NULL);
+        if (rc != ORC_OK) break;
+        for (int32_t i = 0; i < n; ++i) {
+            const int32_t r = ids[i];
+            tokens_out[(int64_t)r * max_steps + k] = tk[i];
+            len_out[r] = k + 1;
+            final_state_out[r] = st[i];
+            sum_logprob_out[r] += lp[i];
+            done_out[r] = dn[i];
+        }
+        int32_t n2 = 0;
+        orc_compact(dn, ids, st, n, ids2, st2, &n2);
+        memcpy(ids, ids2, sizeof(int32_t) * (size_t)n2);
+        memcpy(st, st2, sizeof(int32_t) * (size_t)n2);
+        n = n2;
+    }
+    free(ids); free(lp); free(dn);
+    return rc;
+}

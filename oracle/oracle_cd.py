@@ -51,6 +51,7 @@ def _load():
         _lib.orc_decode_loop.restype = C.c_int
         _lib.orc_decode_loop_limit.restype = C.c_int
         _lib.orc_head_step.restype = C.c_int
+        _lib.orc_head_decode_loop.restype = C.c_int
         _lib.orc_head_logit.restype = C.c_double
     return _lib
 
@@ -222,3 +223,28 @@ def head_logit(hidden, W, H: int, row: int, token: int) -> float:
     w = _bf16_np(W)
     hrow = np.ascontiguousarray(hd[row])
     return float(_load().orc_head_logit(_p(hrow), _p(w), C.c_int64(w.shape[1]), C.c_int32(H), C.c_int32(token)))
+
+
+def head_decode_loop(aut, step_hidden: List, W, H: int, max_steps: Optional[int] = None):
+    """The loop on the LM-head step (O7).  step_hidden[k] is [B, ldh] bf16 indexed by original row id."""
+    V, S, start, rp, tok, nxt, acc = _csr(aut)
+    max_steps = len(step_hidden) if max_steps is None else max_steps
+    assert 1 <= max_steps <= len(step_hidden)
+    arrs = [_bf16_np(x) for x in step_hidden[:max_steps]]
+    w = _bf16_np(W)
+    B, ldh = arrs[0].shape
+    assert all(a.shape == (B, ldh) for a in arrs) and w.shape[0] == V
+    ptrs = (C.c_void_p * max_steps)(*[a.ctypes.data for a in arrs])
+    tokens = np.empty((B, max_steps), np.int32)
+    ln = np.empty(B, np.int32)
+    fs = np.empty(B, np.int32)
+    slp = np.empty(B, np.float64)
+    done = np.empty(B, np.uint8)
+    hist = np.zeros(max_steps, np.int32)
+    rc = _load().orc_head_decode_loop(
+        C.c_int32(V), C.c_int32(S), C.c_int32(start), _p(rp), _p(tok), _p(nxt), _p(acc), ptrs, C.c_int64(ldh),
+        _p(w), C.c_int64(w.shape[1]), C.c_int32(H), C.c_int32(B), C.c_int32(max_steps), _p(tokens), _p(ln), _p(fs),
+        _p(slp), _p(done), _p(hist))
+    if rc != OK:
+        raise OracleError(rc)
+    return dict(tokens=tokens, len=ln, final_state=fs, sum_logprob=slp, done=done, n_active_hist=hist)

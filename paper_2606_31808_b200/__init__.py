@@ -16,6 +16,7 @@ from .binding import (  # noqa: F401
     compile_trie,
     decode_loop,
     decode_loop_host,
+    head_decode_loop,
     head_step,
     launch_count,
     lib,

@@ -18,7 +18,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
     "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_reserve", "cd_step",
-    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_launch_count",
+    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_launch_count",
     "cd_last_error",
 )
 
@@ -314,6 +314,35 @@ def decode_loop(dfa: Dfa, step_logits: Sequence[torch.Tensor], max_steps: Option
     _check(lib().cd_decode_loop(dfa._h, ptrs, C.c_int(dt), C.c_int64(ld), C.c_int32(B), C.c_int32(max_steps),
                                 _ptr(out["tokens"]), _ptr(out["len"]), _ptr(out["final_state"]),
                                 _ptr(out["sum_logprob"]), _ptr(out["done"]), _stream(dev)))
+    return out
+
+
+def head_decode_loop(dfa: Dfa, step_hidden: Sequence[torch.Tensor], W: torch.Tensor, H: Optional[int] = None,
+                     max_steps: Optional[int] = None, out=None):
+    """cd_head_decode_loop: step_hidden[k] are [B, ldh] bf16 CUDA tensors (hidden states of step k,
+    indexed by original row id), W [V, ldw] bf16.  Returns dict(tokens, len, final_state, sum_logprob,
+    done) of device tensors."""
+    dev = dfa.device
+    max_steps = len(step_hidden) if max_steps is None else max_steps
+    if max_steps == 0 or max_steps > len(step_hidden):
+        raise ValueError("need 1 <= max_steps <= len(step_hidden)")
+    h0 = step_hidden[0]
+    B, ldh = h0.shape[0], h0.stride(0)
+    H = h0.shape[1] if H is None else H
+    for h in list(step_hidden[:max_steps]) + [W]:
+        if h.dim() != 2 or not h.is_cuda or h.stride(1) != 1 or h.dtype != torch.bfloat16:
+            raise TypeError("hidden states and W must be 2-D bf16 CUDA tensors with unit inner stride")
+    for h in step_hidden[:max_steps]:
+        if h.shape[0] != B or h.stride(0) != ldh:
+            raise TypeError("step_hidden must share shape and stride")
+    if W.shape[0] != dfa.V:
+        raise ValueError("W must have V rows")
+    ptrs = (C.c_void_p * max_steps)(*[h.data_ptr() for h in step_hidden[:max_steps]])
+    out = _loop_outputs(B, max_steps, dev) if out is None else out
+    _check(lib().cd_head_decode_loop(dfa._h, ptrs, C.c_int64(ldh), _ptr(W), C.c_int64(W.stride(0)), C.c_int32(H),
+                                     C.c_int32(B), C.c_int32(max_steps), _ptr(out["tokens"]), _ptr(out["len"]),
+                                     _ptr(out["final_state"]), _ptr(out["sum_logprob"]), _ptr(out["done"]),
+                                     _stream(dev)))
     return out
 
 

@@ -911,61 +911,63 @@ int head_gather_max_for(const cd_dfa* d) {
     return d->dev.V / 300 > 1 ? d->dev.V / 300 : 1;
 }
 
-}  // namespace
-
-extern "C" {
-
-cd_status cd_set_head_gather_max(cd_dfa_t* d, int32_t max_transitions) {
-    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
-    if (max_transitions < -1) return fail(CD_ERR_ARG, "max_transitions must be >= -1");
-    d->head_gather_max = max_transitions;
+cd_status check_head_layout(const void* hidden, long long ldh, const void* W, long long ldw, int H) {
+    if (H < 8 || (H % 8) != 0) return fail(CD_ERR_ARG, "H (%d) must be a positive multiple of 8", H);
+    if (!hidden || !W) return fail(CD_ERR_ARG, "hidden / W is NULL");
+    if (ldh < H || ldw < H) return fail(CD_ERR_ARG, "ldh_elems / ldw_elems < H");
+    if ((ldh % 8) != 0 || (ldw % 8) != 0) return fail(CD_ERR_ARG, "row strides must be multiples of 8 elements (16 bytes)");
+    if ((reinterpret_cast<uintptr_t>(hidden) & 15) != 0 || (reinterpret_cast<uintptr_t>(W) & 15) != 0)
+        return fail(CD_ERR_ARG, "hidden / W base is not 16-byte aligned");
+    if ((size_t)H * 2 > 200 * 1024) return fail(CD_ERR_ARG, "H too large (hidden row must fit in shared memory)");
     return CD_OK;
 }
 
-cd_status cd_head_step(const cd_dfa_t* d, const void* hidden, int64_t ldh_elems, const void* W, int64_t ldw_elems,
-                       int32_t H, const int32_t* row_map, int32_t* state, int32_t n, int32_t* token_out,
-                       float* logprob_out, float* lse_out, uint8_t* done_out, void* cuda_stream) {
-    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
-    if (n < 0) return fail(CD_ERR_ARG, "n < 0");
-    if (H < 8 || (H % 8) != 0) return fail(CD_ERR_ARG, "H (%d) must be a positive multiple of 8", H);
-    if (n == 0) return CD_OK;
-    if (!hidden || !W || !state || !token_out || !logprob_out || !done_out) return fail(CD_ERR_ARG, "NULL pointer");
-    if (ldh_elems < H || ldw_elems < H) return fail(CD_ERR_ARG, "ldh_elems / ldw_elems < H");
-    if ((ldh_elems % 8) != 0 || (ldw_elems % 8) != 0) return fail(CD_ERR_ARG, "row strides must be multiples of 8 elements (16 bytes)");
-    if ((reinterpret_cast<uintptr_t>(hidden) & 15) != 0 || (reinterpret_cast<uintptr_t>(W) & 15) != 0)
-        return fail(CD_ERR_ARG, "hidden / W base is not 16-byte aligned");
-    DeviceGuard guard(d->device);
-    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    Scratch* s = nullptr;
-    cd_status st = get_scratch(d, stream, n, false, &s);
-    if (st != CD_OK) return st;
-    st = get_head_scratch(s, n, H, stream);
-    if (st != CD_OK) return st;
-    // tensor map of the output embedding (cached per handle: the weights rarely change)
+// tensor map of the output embedding, cached per handle (the weights rarely change)
+cd_status head_weight_map(const cd_dfa* d, const void* W, long long ldw, int H) {
     cd_dfa* dm = const_cast<cd_dfa*>(d);
-    {
-        std::lock_guard<std::mutex> lk(dm->mu);
-        if (dm->w_ptr != W || dm->w_ld != ldw_elems || dm->w_H != H) {
-            st = make_tmap_bf16(&dm->w_tmap, W, d->dev.V, H, ldw_elems, cd::HD_BN);
-            if (st != CD_OK) return st;
-            dm->w_ptr = W; dm->w_ld = ldw_elems; dm->w_H = H;
-        }
+    std::lock_guard<std::mutex> lk(dm->mu);
+    if (dm->w_ptr != W || dm->w_ld != ldw || dm->w_H != H) {
+        cd_status st = make_tmap_bf16(&dm->w_tmap, W, d->dev.V, H, ldw, cd::HD_BN);
+        if (st != CD_OK) return st;
+        dm->w_ptr = W; dm->w_ld = ldw; dm->w_H = H;
     }
+    return CD_OK;
+}
+
+// The kernels of one LM-head step for up to n_upper active slots (n_dev overrides the count on
+// the device).  With loop extras the rows' history is recorded as they finalise and a last
+// one-CTA kernel compacts the active list.
+cd_status launch_head(const cd_dfa* d, Scratch* s, const void* hidden, long long ldh, const void* W, long long ldw, int H,
+                      const int* row_map, int* state, int n_upper, const int* n_dev, int* token_out, float* logprob_out,
+                      float* lse_out, uint8_t* done_out, cudaStream_t stream, const LoopExtras* x) {
     cd::HeadArgs a{};
+    if (x) {
+        a.fin.hist_tokens = x->tokens;
+        a.fin.hist_len = x->len;
+        a.fin.hist_final_state = x->final_state;
+        a.fin.hist_sum_logprob = x->sum_logprob;
+        a.fin.hist_done = x->done;
+        a.fin.step = x->step;
+        a.fin.max_steps = x->max_steps;
+        a.fin.cmp_row_ids_out = x->row_ids_out;
+        a.fin.cmp_state_out = x->state_out;
+        a.fin.cmp_n_out = x->n_out;
+    }
     a.fin.dfa = d->dev;
     a.fin.row_map = row_map;
     a.fin.state = state;
     a.fin.state_new = state;
-    a.fin.n = n;
+    a.fin.n = n_upper;
+    a.fin.n_dev = n_dev;
     a.fin.token_out = token_out;
     a.fin.logprob_out = logprob_out;
     a.fin.lse_out = lse_out;
     a.fin.done_out = done_out;
     a.fin.ctrs = s->ctrs;
     a.hidden = static_cast<const uint16_t*>(hidden);
-    a.ldh = ldh_elems;
+    a.ldh = ldh;
     a.W = static_cast<const uint16_t*>(W);
-    a.ldw = ldw_elems;
+    a.ldw = ldw;
     a.H = H;
     a.gather_max = head_gather_max_for(d);
     a.not_dense = s->h_flags;
@@ -979,6 +981,7 @@ cd_status cd_head_step(const cd_dfa_t* d, const void* hidden, int64_t ldh_elems,
     a.ldA = s->h_ldA;
     a.partials = s->h_partials;
 
+    const int n = n_upper;
     cd::head_prepare_kernel<<<1, 1024, 0, stream>>>(a);
     CU(cudaGetLastError());
     const bool any_gather = a.gather_max > 0 && d->min_deg_nonacc <= a.gather_max;
@@ -991,7 +994,6 @@ cd_status cd_head_step(const cd_dfa_t* d, const void* hidden, int64_t ldh_elems,
             CU(cudaFuncSetAttribute(cd::head_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
             cfg_dev = d->device;
         }
-        if (smem > 200 * 1024) return fail(CD_ERR_ARG, "H too large for the gather path");
         cd::head_gather_kernel<<<n, cd::HG_WARPS * 32, smem, stream>>>(a);
         CU(cudaGetLastError());
         ++launches;
@@ -1011,8 +1013,94 @@ cd_status cd_head_step(const cd_dfa_t* d, const void* hidden, int64_t ldh_elems,
         CU(cudaGetLastError());
         launches += 3;
     }
+    if (x) {
+        cd::head_loop_tail_kernel<<<1, 1024, 0, stream>>>(a);
+        CU(cudaGetLastError());
+        ++launches;
+    }
     g_launches.fetch_add(launches, std::memory_order_relaxed);
     return CD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+cd_status cd_set_head_gather_max(cd_dfa_t* d, int32_t max_transitions) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (max_transitions < -1) return fail(CD_ERR_ARG, "max_transitions must be >= -1");
+    d->head_gather_max = max_transitions;
+    return CD_OK;
+}
+
+cd_status cd_head_step(const cd_dfa_t* d, const void* hidden, int64_t ldh_elems, const void* W, int64_t ldw_elems,
+                       int32_t H, const int32_t* row_map, int32_t* state, int32_t n, int32_t* token_out,
+                       float* logprob_out, float* lse_out, uint8_t* done_out, void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (n < 0) return fail(CD_ERR_ARG, "n < 0");
+    cd_status st = check_head_layout(hidden, ldh_elems, W, ldw_elems, H);
+    if (st != CD_OK) return st;
+    if (n == 0) return CD_OK;
+    if (!state || !token_out || !logprob_out || !done_out) return fail(CD_ERR_ARG, "NULL pointer");
+    DeviceGuard guard(d->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* s = nullptr;
+    st = get_scratch(d, stream, n, false, &s);
+    if (st != CD_OK) return st;
+    st = get_head_scratch(s, n, H, stream);
+    if (st != CD_OK) return st;
+    st = head_weight_map(d, W, ldw_elems, H);
+    if (st != CD_OK) return st;
+    return launch_head(d, s, hidden, ldh_elems, W, ldw_elems, H, row_map, state, n, nullptr, token_out, logprob_out,
+                       lse_out, done_out, stream, nullptr);
+}
+
+cd_status cd_head_decode_loop(const cd_dfa_t* d, const void* const* step_hidden, int64_t ldh_elems, const void* W,
+                              int64_t ldw_elems, int32_t H, int32_t B, int32_t max_steps, int32_t* tokens_out,
+                              int32_t* len_out, int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out,
+                              void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (B < 0 || max_steps < 0) return fail(CD_ERR_ARG, "B / max_steps < 0");
+    if (B == 0) return CD_OK;
+    if (!len_out || !final_state_out || !sum_logprob_out || !done_out || (max_steps > 0 && !tokens_out))
+        return fail(CD_ERR_ARG, "NULL output pointer");
+    if (max_steps > 0 && !step_hidden) return fail(CD_ERR_ARG, "step_hidden is NULL");
+    cd_status st = CD_OK;
+    for (int k = 0; k < max_steps; ++k) {
+        st = check_head_layout(step_hidden[k], ldh_elems, W, ldw_elems, H);
+        if (st != CD_OK) return st;
+    }
+    DeviceGuard guard(d->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* s = nullptr;
+    st = get_scratch(d, stream, B, true, &s);
+    if (st != CD_OK) return st;
+    st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream);
+    if (st != CD_OK) return st;
+    if (!d->start_accepting && max_steps > 0) {
+        st = get_head_scratch(s, B, H, stream);
+        if (st != CD_OK) return st;
+        st = head_weight_map(d, W, ldw_elems, H);
+        if (st != CD_OK) return st;
+        for (int k = 0; k < max_steps; ++k) {
+            const int cur = k & 1, nxt = cur ^ 1;
+            LoopExtras x;
+            x.tokens = tokens_out;
+            x.len = len_out;
+            x.final_state = final_state_out;
+            x.sum_logprob = sum_logprob_out;
+            x.done = done_out;
+            x.step = k;
+            x.max_steps = max_steps;
+            x.row_ids_out = s->row_ids[nxt];
+            x.state_out = s->state[nxt];
+            x.n_out = s->n_active + nxt;
+            st = launch_head(d, s, step_hidden[k], ldh_elems, W, ldw_elems, H, s->row_ids[cur], s->state[cur], B,
+                             s->n_active + cur, s->token, s->logprob, nullptr, s->done, stream, &x);
+            if (st != CD_OK) return st;
+        }
+    }
+    return check_sticky_errors(s, stream);
 }
 
 }  // extern "C"

@@ -470,4 +470,12 @@ __global__ void head_finish_kernel(const HeadArgs a) {
     }
 }
 
+// ---------------------------------------------------------------- decode loop: compaction
+// Last kernel of a loop step: stable early-exit compaction of the active list.
+__global__ void __launch_bounds__(1024, 1) head_loop_tail_kernel(const HeadArgs a) {
+    const StepArgs& f = a.fin;
+    const int n = f.n_dev ? __ldcg(f.n_dev) : f.n;
+    block_compact(f.done_out, f.row_map, f.state, n, f.cmp_row_ids_out, f.cmp_state_out, f.cmp_n_out);
+}
+
 }  // namespace cd

@@ -257,3 +257,43 @@ def test_full_size_configs(cd, oracle, full_head, kind, name, n_check):
         states = live_states(aut, n, mult=1)  # every trie node, root included
     check = sorted(set(int(i) for i in np.linspace(0, n - 1, n_check).astype(int)))
     run_case(cd, oracle, aut, dfa, hid, W_cpu, H, states, exact=(kind == "exact"), check=check, W_dev=W_dev)
+
+
+# ---------------------------------------------------------------- decode loop on the head step
+@pytest.mark.parametrize("kind,V,H,B,steps", [("dfa", 3000, 128, 300, 8), ("trie", 2000, 192, 150, 5),
+                                              ("dfa", 700, 64, 1, 4)])
+def test_head_decode_loop_exact_inputs(cd, oracle, mode, kind, V, H, B, steps):
+    """cd_head_decode_loop against O7 on exact-arithmetic inputs: bit-exact histories, lengths,
+    final states and done flags; sum of log-probs within the sum of the per-step bounds."""
+    if kind == "dfa":
+        aut = wl.make_random_dfa(23, V, 20, 0.1, 0.15)
+    else:
+        aut = wl.make_trie(V, wl.draw_labels(23, V, 25, 1, 5))
+    dfa = dev_dfa(cd, aut, mode)
+    W = wl.make_head(23, V, H, 2.0, exact=True)
+    hs = [wl.make_hidden(23, k, B, H, exact=True) for k in range(steps)]
+    got = cd.head_decode_loop(dfa, [h.to("cuda:0") for h in hs], W.to("cuda:0"), H=H)
+    torch.cuda.synchronize()
+    want = oracle.head_decode_loop(aut, hs, W, H)
+    for k in ("tokens", "len", "final_state", "done"):
+        assert np.array_equal(got[k].cpu().numpy(), want[k]), k
+    slp = got["sum_logprob"].cpu().numpy().astype(np.float64)
+    bound = TOL * (want["len"] + np.abs(want["sum_logprob"]))
+    assert np.all(np.abs(slp - want["sum_logprob"]) <= bound + 1e-12)
+    assert want["len"].max() > 1 or B == 1
+
+
+def test_head_decode_loop_matches_logits_loop(cd, mode):
+    """Same loop through cd_decode_loop on fp32 logits formed by a library matmul (exact inputs):
+    the two entry points of the library agree bit for bit."""
+    V, H, B, steps = 4096, 256, 200, 6
+    aut = wl.make_random_dfa(29, V, 30, 0.05, 0.1)
+    dfa = dev_dfa(cd, aut, mode)
+    W = wl.make_head(29, V, H, 2.0, exact=True, device="cuda:0")
+    hs = [wl.make_hidden(29, k, B, H, exact=True, device="cuda:0") for k in range(steps)]
+    logits = [(h.float() @ W.float().t()).contiguous() for h in hs]  # exact in fp32
+    a = cd.head_decode_loop(dfa, hs, W, H=H)
+    b = cd.decode_loop(dfa, logits)
+    torch.cuda.synchronize()
+    for k in ("tokens", "len", "final_state", "done"):
+        assert torch.equal(a[k], b[k]), k

@@ -148,3 +148,28 @@ def test_poisoned_complement_and_nan(oracle):
         xs = x[r, rest]
         assert tk[r] == rest[int(np.argmax(xs))]
         assert abs(lse[r] - (xs.max() + math.log(np.exp(xs - xs.max()).sum()))) < 1e-12
+
+
+@pytest.mark.parametrize("kind", ["dfa", "trie"])
+def test_head_loop_reduces_to_loop_on_library_matmul(oracle, kind):
+    """O7 against the pinned O4 (oracle.decode_loop) fed with logits from a library matmul:
+    exact-arithmetic inputs make the fp32 logits equal to the real dot products."""
+    V, H, B, steps = 400, 96, 23, 6
+    if kind == "dfa":
+        aut = wl.make_random_dfa(21, V, 9, 0.2, 0.25)
+    else:
+        aut = wl.make_trie(V, wl.draw_labels(21, V, 12, 1, 4))
+    W = wl.make_head(21, V, H, 2.0, exact=True, ld=H + 8)
+    hs = [wl.make_hidden(21, k, B, H, exact=True) for k in range(steps)]
+    logits = []
+    for h in hs:
+        x = f64(h[:, :H]) @ f64(W[:, :H]).T
+        x32 = x.astype(np.float32)
+        assert np.array_equal(x32.astype(np.float64), x)
+        logits.append(x32)
+    want = oracle.decode_loop(aut, logits)
+    got = oracle.head_decode_loop(aut, hs, W, H)
+    for k in ("tokens", "len", "final_state", "done", "n_active_hist"):
+        assert np.array_equal(got[k], want[k]), k
+    assert np.allclose(got["sum_logprob"], want["sum_logprob"], rtol=0, atol=1e-11)
+    assert want["n_active_hist"][0] == B and want["len"].max() > 1  # the loop really iterates
