@@ -274,6 +274,44 @@ CD_API cd_status cd_head_decode_loop(const cd_dfa_t* dfa, const void* const* ste
                               int32_t* tokens_out, int32_t* len_out, int32_t* final_state_out,
                               float* sum_logprob_out, uint8_t* done_out, void* cuda_stream);
 
+/*
+ * Early deduplication (section 2.4 "Early Deduplication of
+ * Database Values", L156): "the input set is deduplicated via a SELECT DISTINCT clause,
+ * and the mapped outputs are then aligned to the original table via a LEFT JOIN", which
+ * cuts the number of generations by the duplication factor N / |dom|.
+ * cd_dedup: keys [N] (DEVICE int64: interned value ids or hashes of the, possibly
+ * multi-column, input values; every int64 value is a valid key).  Distinct values are
+ * listed in order of first occurrence:
+ *   distinct_rows_out [N]  DEVICE; entry p = row id of the first row carrying the p-th
+ *                          distinct value (ascending); the first *n_distinct_out are written
+ *   rep_out           [N]  DEVICE; rep[i] = p with keys[distinct_rows[p]] == keys[i]
+ *   n_distinct_out         DEVICE int32
+ * The caller decodes the rows distinct_rows[0 .. n_distinct) only (cd_decode_loop /
+ * cd_head_decode_loop on logits or hidden states of those rows) and broadcasts the results
+ * back with cd_join_results: out[i] = in[rep[i]] for the five loop outputs (tokens
+ * [., max_steps]); an output pointer may be NULL to skip it.  Asynchronous on cuda_stream;
+ * scratch is stream-ordered (cudaMallocAsync).  Errors: CD_ERR_ARG, CD_ERR_CUDA, CD_ERR_OOM.
+ */
+CD_API cd_status cd_dedup(const int64_t* keys, int32_t N, int32_t* rep_out, int32_t* distinct_rows_out,
+                   int32_t* n_distinct_out, void* cuda_stream);
+CD_API cd_status cd_join_results(const int32_t* rep, int32_t N, int32_t max_steps, const int32_t* tokens_d,
+                          const int32_t* len_d, const int32_t* final_state_d, const float* sum_logprob_d,
+                          const uint8_t* done_d, int32_t* tokens_out, int32_t* len_out,
+                          int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out,
+                          void* cuda_stream);
+
+/*
+ * Cascade filtering (section 2.4): with conjunctive LM
+ * predicates "subsequent functions only process rows of data which satisfied all preceding
+ * predicates".  Given the decode results of one predicate (final_state, done: DEVICE [N])
+ * and the satisfying set of cd_set_satisfying, writes the ids of the rows that finished in
+ * a satisfying state, order kept (row_ids_in [N] or NULL -> 0..N-1), to row_ids_out [N] and
+ * their number to *n_out (DEVICE int32): the active list of the next predicate's loop.
+ */
+CD_API cd_status cd_filter_rows(const cd_dfa_t* dfa, const int32_t* final_state, const uint8_t* done,
+                         const int32_t* row_ids_in, int32_t N, int32_t* row_ids_out, int32_t* n_out,
+                         void* cuda_stream);
+
 /* Number of kernel launches this library has enqueued from the calling thread's
    process so far (monotone; used by bench.py to report gpu_launches). */
 CD_API int64_t cd_launch_count(void);

@@ -8,6 +8,9 @@ from .oracle_cd import (  # noqa: F401
     build,
     compact,
     decode_loop,
+    dedup,
+    filter_rows,
+    join_results,
     head_decode_loop,
     head_logit,
     head_step,

@@ -412,3 +412,63 @@ int orc_head_decode_loop(int32_t V, int32_t S, int32_t start, const int64_t *row
     free(ids); free(lp); free(dn);
     return rc;
 }
+
+/*
+ * O8 (section 2.4 "Early Deduplication of Database Values", L156):
+ * "the input set is deduplicated via a SELECT DISTINCT clause, and the mapped outputs are
+ * then aligned to the original table via a LEFT JOIN".  Row values are 64-bit keys.
+ * Reading (the paper does not order the DISTINCT result): distinct values are listed in
+ * order of FIRST OCCURRENCE, which makes the result unique.  distinct_rows[p] = row id of
+ * the first row carrying the p-th distinct value; rep[i] = p such that
+ * keys[distinct_rows[p]] == keys[i].  Written as the definition: every row scans the list
+ * of distinct values found so far.
+ */
+int orc_dedup(const int64_t *keys, int32_t N, int32_t *rep_out, int32_t *distinct_rows_out, int32_t *n_distinct_out)
+{
+    if (N < 0) return ORC_ERR_ARG;
+    int32_t D = 0;
+    for (int32_t i = 0; i < N; ++i) {
+        int32_t p = 0;
+        while (p < D && keys[distinct_rows_out[p]] != keys[i]) ++p;
+        if (p == D) distinct_rows_out[D++] = i;
+        rep_out[i] = p;
+    }
+    *n_distinct_out = D;
+    return ORC_OK;
+}
+
+/* LEFT JOIN back: row i receives the outputs of distinct value rep[i]. */
+int orc_join_results(const int32_t *rep, int32_t N, int32_t max_steps, const int32_t *tokens_d, const int32_t *len_d,
+                     const int32_t *fs_d, const double *slp_d, const uint8_t *done_d, int32_t *tokens, int32_t *len,
+                     int32_t *fs, double *slp, uint8_t *done)
+{
+    if (N < 0 || max_steps < 0) return ORC_ERR_ARG;
+    for (int32_t i = 0; i < N; ++i) {
+        const int32_t r = rep[i];
+        for (int32_t k = 0; k < max_steps; ++k) tokens[(int64_t)i * max_steps + k] = tokens_d[(int64_t)r * max_steps + k];
+        len[i] = len_d[r];
+        fs[i] = fs_d[r];
+        slp[i] = slp_d[r];
+        done[i] = done_d[r];
+    }
+    return ORC_OK;
+}
+
+/*
+ * O9 (section 2.4 "Cascade Filtering", L150): "subsequent functions only process
+ * rows of data which satisfied all preceding predicates".  A row satisfies the predicate
+ * when it finished (done) in a state of the satisfying set; survivors keep their order.
+ * row_ids_in == NULL means 0..N-1.
+ */
+int orc_filter_rows(const int32_t *final_state, const uint8_t *done, const int32_t *row_ids_in, int32_t N,
+                    const uint8_t *satisfying, int32_t S, int32_t *row_ids_out, int32_t *n_out)
+{
+    if (N < 0) return ORC_ERR_ARG;
+    int32_t k = 0;
+    for (int32_t i = 0; i < N; ++i) {
+        const int32_t s = final_state[i];
+        if (done[i] && s >= 0 && s < S && satisfying[s]) row_ids_out[k++] = row_ids_in ? row_ids_in[i] : i;
+    }
+    *n_out = k;
+    return ORC_OK;
+}

@@ -52,6 +52,9 @@ def _load():
         _lib.orc_decode_loop_limit.restype = C.c_int
         _lib.orc_head_step.restype = C.c_int
         _lib.orc_head_decode_loop.restype = C.c_int
+        _lib.orc_dedup.restype = C.c_int
+        _lib.orc_join_results.restype = C.c_int
+        _lib.orc_filter_rows.restype = C.c_int
         _lib.orc_head_logit.restype = C.c_double
     return _lib
 
@@ -248,3 +251,51 @@ def head_decode_loop(aut, step_hidden: List, W, H: int, max_steps: Optional[int]
     if rc != OK:
         raise OracleError(rc)
     return dict(tokens=tokens, len=ln, final_state=fs, sum_logprob=slp, done=done, n_active_hist=hist)
+
+
+def dedup(keys):
+    """SELECT DISTINCT in first-occurrence order (O8).  Returns (rep i32[N], distinct_rows i32[D])."""
+    k = np.ascontiguousarray(np.asarray(keys, dtype=np.int64))
+    N = k.shape[0]
+    rep = np.empty(N, np.int32)
+    dr = np.empty(max(N, 1), np.int32)
+    D = C.c_int32(0)
+    rc = _load().orc_dedup(_p(k), C.c_int32(N), _p(rep), _p(dr), C.byref(D))
+    if rc != OK:
+        raise OracleError(rc)
+    return rep, dr[: D.value].copy()
+
+
+def join_results(rep, res: dict):
+    """LEFT JOIN of the distinct values' decode results back to the rows (O8)."""
+    r = np.ascontiguousarray(np.asarray(rep, dtype=np.int32))
+    N = r.shape[0]
+    tk = np.ascontiguousarray(res["tokens"], dtype=np.int32)
+    ms = tk.shape[1]
+    ln = np.ascontiguousarray(res["len"], dtype=np.int32)
+    fs = np.ascontiguousarray(res["final_state"], dtype=np.int32)
+    slp = np.ascontiguousarray(res["sum_logprob"], dtype=np.float64)
+    dn = np.ascontiguousarray(res["done"], dtype=np.uint8)
+    out = dict(tokens=np.empty((N, ms), np.int32), len=np.empty(N, np.int32), final_state=np.empty(N, np.int32),
+               sum_logprob=np.empty(N, np.float64), done=np.empty(N, np.uint8))
+    rc = _load().orc_join_results(_p(r), C.c_int32(N), C.c_int32(ms), _p(tk), _p(ln), _p(fs), _p(slp), _p(dn),
+                                  _p(out["tokens"]), _p(out["len"]), _p(out["final_state"]), _p(out["sum_logprob"]),
+                                  _p(out["done"]))
+    if rc != OK:
+        raise OracleError(rc)
+    return out
+
+
+def filter_rows(final_state, done, satisfying, row_ids=None):
+    """Cascade filter (O9): ids of the rows that finished in a satisfying state, order kept."""
+    fs = np.ascontiguousarray(np.asarray(final_state, dtype=np.int32))
+    dn = np.ascontiguousarray(np.asarray(done, dtype=np.uint8))
+    sat = np.ascontiguousarray(np.asarray(satisfying, dtype=np.uint8))
+    ri = None if row_ids is None else np.ascontiguousarray(np.asarray(row_ids, dtype=np.int32))
+    N = fs.shape[0]
+    out = np.empty(max(N, 1), np.int32)
+    k = C.c_int32(0)
+    rc = _load().orc_filter_rows(_p(fs), _p(dn), _p(ri), C.c_int32(N), _p(sat), C.c_int32(sat.shape[0]), _p(out), C.byref(k))
+    if rc != OK:
+        raise OracleError(rc)
+    return out[: k.value].copy()

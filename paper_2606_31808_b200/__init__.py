@@ -16,6 +16,9 @@ from .binding import (  # noqa: F401
     compile_trie,
     decode_loop,
     decode_loop_host,
+    dedup,
+    filter_rows,
+    join_results,
     head_decode_loop,
     head_step,
     launch_count,

@@ -18,7 +18,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
     "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_reserve", "cd_step",
-    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_launch_count",
+    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
     "cd_last_error",
 )
 
@@ -362,3 +362,51 @@ def decode_loop_host(dfa: Dfa, step_logits_host: Sequence[torch.Tensor], max_ste
                                      _ptr(out["tokens"]), _ptr(out["len"]), _ptr(out["final_state"]),
                                      _ptr(out["sum_logprob"]), _ptr(out["done"]), _stream(dev)))
     return out
+
+
+def dedup(keys: torch.Tensor, out=None):
+    """cd_dedup: keys int64[N] on the device -> (rep i32[N], distinct_rows i32[N], n_distinct i32[1]);
+    only the first n_distinct entries of distinct_rows are meaningful."""
+    if keys.dtype != torch.int64 or not keys.is_cuda or not keys.is_contiguous() or keys.dim() != 1:
+        raise TypeError("keys must be a contiguous 1-D int64 CUDA tensor")
+    dev = keys.device
+    N = keys.numel()
+    if out is not None:
+        rep, dr, nd = out
+    else:
+        rep = torch.empty(max(N, 1), dtype=torch.int32, device=dev)
+        dr = torch.empty(max(N, 1), dtype=torch.int32, device=dev)
+        nd = torch.empty(1, dtype=torch.int32, device=dev)
+    with torch.cuda.device(dev):
+        _check(lib().cd_dedup(_ptr(keys), C.c_int32(N), _ptr(rep), _ptr(dr), _ptr(nd), _stream(dev)))
+    return rep[:N], dr, nd
+
+
+def join_results(rep: torch.Tensor, res: dict, out=None):
+    """cd_join_results: broadcast the distinct values' loop outputs (dict of device tensors) to the rows."""
+    dev = rep.device
+    _dev_tensor(rep, torch.int32, "rep", dev)
+    N = rep.numel()
+    ms = res["tokens"].shape[1]
+    out = _loop_outputs(N, ms, dev) if out is None else out
+    with torch.cuda.device(dev):
+        _check(lib().cd_join_results(_ptr(rep), C.c_int32(N), C.c_int32(ms), _ptr(res["tokens"]), _ptr(res["len"]),
+                                     _ptr(res["final_state"]), _ptr(res["sum_logprob"]), _ptr(res["done"]),
+                                     _ptr(out["tokens"]), _ptr(out["len"]), _ptr(out["final_state"]),
+                                     _ptr(out["sum_logprob"]), _ptr(out["done"]), _stream(dev)))
+    return out
+
+
+def filter_rows(dfa: Dfa, final_state: torch.Tensor, done: torch.Tensor, row_ids: Optional[torch.Tensor] = None):
+    """cd_filter_rows: (row_ids_out i32[N], n_out i32[1]) of the rows that finished in a satisfying state."""
+    dev = dfa.device
+    _dev_tensor(final_state, torch.int32, "final_state", dev)
+    _dev_tensor(done, torch.uint8, "done", dev)
+    if row_ids is not None:
+        _dev_tensor(row_ids, torch.int32, "row_ids", dev)
+    N = final_state.numel()
+    ro = torch.empty(max(N, 1), dtype=torch.int32, device=dev)
+    no = torch.empty(1, dtype=torch.int32, device=dev)
+    _check(lib().cd_filter_rows(dfa._h, _ptr(final_state), _ptr(done), _ptr(row_ids), C.c_int32(N), _ptr(ro), _ptr(no),
+                                _stream(dev)))
+    return ro, no

@@ -19,6 +19,7 @@
 #include "cd_common.cuh"
 #include "cd_step.cuh"
 #include "cd_head.cuh"
+#include "cd_dedup.cuh"
 
 namespace {
 
@@ -1101,6 +1102,121 @@ cd_status cd_head_decode_loop(const cd_dfa_t* d, const void* const* step_hidden,
         }
     }
     return check_sticky_errors(s, stream);
+}
+
+}  // extern "C"
+
+// =============================================================================== dedup / join / cascade
+namespace {
+
+int grid_for(long long n, int threads) {
+    long long b = (n + threads - 1) / threads;
+    if (b < 1) b = 1;
+    if (b > 148 * 16) b = 148 * 16;
+    return (int)b;
+}
+
+cd_status device_of(const void* p, int* dev) {
+    cudaPointerAttributes at;
+    CU(cudaPointerGetAttributes(&at, p));
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
+        return fail(CD_ERR_ARG, "expected a DEVICE pointer");
+    *dev = at.device;
+    return CD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+cd_status cd_dedup(const int64_t* keys, int32_t N, int32_t* rep_out, int32_t* distinct_rows_out,
+                   int32_t* n_distinct_out, void* cuda_stream) {
+    if (N < 0) return fail(CD_ERR_ARG, "N < 0");
+    if (!n_distinct_out) return fail(CD_ERR_ARG, "n_distinct_out is NULL");
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    int dev = 0;
+    cd_status st = device_of(n_distinct_out, &dev);
+    if (st != CD_OK) return st;
+    DeviceGuard guard(dev);
+    if (N == 0) {
+        CU(cudaMemsetAsync(n_distinct_out, 0, sizeof(int), stream));
+        return CD_OK;
+    }
+    if (!keys || !rep_out || !distinct_rows_out) return fail(CD_ERR_ARG, "NULL pointer");
+    uint32_t cap = 1024;
+    while (cap < 2ull * (uint32_t)N) cap <<= 1;
+    // stream-ordered scratch: table keys [cap + 1], table min rows [cap + 1], first [N], rank [N], flags [N]
+    const size_t off_min = sizeof(unsigned long long) * ((size_t)cap + 1);
+    const size_t off_first = off_min + sizeof(int) * ((size_t)cap + 1 + 3) / 16 * 16 + 16;
+    const size_t off_rank = off_first + sizeof(int) * (size_t)N;
+    const size_t off_flag = off_rank + sizeof(int) * (size_t)N;
+    const size_t total = off_flag + (size_t)N + 16;
+    unsigned char* buf = nullptr;
+    CU(cudaMallocAsync(reinterpret_cast<void**>(&buf), total, stream));
+    unsigned long long* tkey = reinterpret_cast<unsigned long long*>(buf);
+    int* tmin = reinterpret_cast<int*>(buf + off_min);
+    int* first = reinterpret_cast<int*>(buf + off_first);
+    int* rank = reinterpret_cast<int*>(buf + off_rank);
+    uint8_t* flag = buf + off_flag;
+    // min rows start at 0x7F7F7F7F (>= any row id); free slots hold DEDUP_EMPTY
+    CU(cudaMemsetAsync(tmin, 0x7F, sizeof(int) * ((size_t)cap + 1), stream));
+    cd::dedup_clear_kernel<<<grid_for((long long)cap + 1, 256), 256, 0, stream>>>(tkey, (long long)cap + 1);
+    cd::dedup_insert_kernel<<<grid_for(N, 256), 256, 0, stream>>>(reinterpret_cast<const long long*>(keys), N, tkey, tmin, cap);
+    cd::dedup_first_kernel<<<grid_for(N, 256), 256, 0, stream>>>(reinterpret_cast<const long long*>(keys), N, tkey, tmin, cap,
+                                                               first, flag);
+    cd::dedup_rank_kernel<<<1, 1024, 0, stream>>>(flag, N, distinct_rows_out, rank, n_distinct_out);
+    cd::dedup_rep_kernel<<<grid_for(N, 256), 256, 0, stream>>>(first, rank, N, rep_out);
+    CU(cudaGetLastError());
+    g_launches.fetch_add(5, std::memory_order_relaxed);
+    CU(cudaFreeAsync(buf, stream));
+    return CD_OK;
+}
+
+cd_status cd_join_results(const int32_t* rep, int32_t N, int32_t max_steps, const int32_t* tokens_d, const int32_t* len_d,
+                          const int32_t* final_state_d, const float* sum_logprob_d, const uint8_t* done_d,
+                          int32_t* tokens_out, int32_t* len_out, int32_t* final_state_out, float* sum_logprob_out,
+                          uint8_t* done_out, void* cuda_stream) {
+    if (N < 0 || max_steps < 0) return fail(CD_ERR_ARG, "N / max_steps < 0");
+    if (N == 0) return CD_OK;
+    if (!rep) return fail(CD_ERR_ARG, "rep is NULL");
+    if ((tokens_out && !tokens_d) || (len_out && !len_d) || (final_state_out && !final_state_d) ||
+        (sum_logprob_out && !sum_logprob_d) || (done_out && !done_d))
+        return fail(CD_ERR_ARG, "an output is requested without its source");
+    int dev = 0;
+    cd_status st = device_of(rep, &dev);
+    if (st != CD_OK) return st;
+    DeviceGuard guard(dev);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    cd::join_kernel<<<grid_for((long long)N * (max_steps > 0 ? max_steps : 1), 256), 256, 0, stream>>>(
+        rep, N, max_steps, tokens_d, len_d, final_state_d, sum_logprob_d, done_d, max_steps > 0 ? tokens_out : nullptr,
+        len_out, final_state_out, sum_logprob_out, done_out);
+    CU(cudaGetLastError());
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return CD_OK;
+}
+
+cd_status cd_filter_rows(const cd_dfa_t* d, const int32_t* final_state, const uint8_t* done, const int32_t* row_ids_in,
+                         int32_t N, int32_t* row_ids_out, int32_t* n_out, void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (!d->d_satisfying) return fail(CD_ERR_ARG, "cd_set_satisfying has not been called on this automaton");
+    if (N < 0) return fail(CD_ERR_ARG, "N < 0");
+    if (!n_out) return fail(CD_ERR_ARG, "n_out is NULL");
+    DeviceGuard guard(d->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (N == 0) {
+        CU(cudaMemsetAsync(n_out, 0, sizeof(int), stream));
+        return CD_OK;
+    }
+    if (!final_state || !done || !row_ids_out) return fail(CD_ERR_ARG, "NULL pointer");
+    uint8_t* drop = nullptr;
+    CU(cudaMallocAsync(reinterpret_cast<void**>(&drop), (size_t)N + 16, stream));
+    cd::filter_flag_kernel<<<grid_for(N, 256), 256, 0, stream>>>(final_state, done, N,
+                                                               static_cast<const uint8_t*>(d->d_satisfying), d->dev.S, drop);
+    cd::compact_kernel<<<1, 1024, 0, stream>>>(drop, row_ids_in, nullptr, N, row_ids_out, nullptr, n_out);
+    CU(cudaGetLastError());
+    g_launches.fetch_add(2, std::memory_order_relaxed);
+    CU(cudaFreeAsync(drop, stream));
+    return CD_OK;
 }
 
 }  // extern "C"

@@ -1,0 +1,166 @@
+// cd_dedup.cuh -- early deduplication and cascade filtering as device primitives (
+// PAPER.md section 2.4 "Early Deduplication of Database Values", L156, and "Cascade Filtering",
+// L150).  Row values are 64-bit keys (interned value ids or hashes of the column values):
+//   dedup_insert_kernel   SELECT DISTINCT: open-addressing hash table, one 64-bit CAS to claim a
+//                         slot + atomicMin of the row id, so every distinct value knows its FIRST row
+//   dedup_first_kernel    every row looks its value up: first[i] = first row with the same value
+//   dedup_rank_kernel     one CTA: stable scan over the rows that are first occurrences ->
+//                         distinct_rows[] (ascending row id = first-occurrence order) and the rank
+//                         of each of them
+//   dedup_rep_kernel      rep[i] = rank[first[i]]   (the key of the LEFT JOIN back)
+//   join_kernel           LEFT JOIN: broadcast the distinct rows' decode results to all rows
+//   filter_kernel         cascade: rows that finished in a satisfying state, in row order
+#pragma once
+#include "cd_common.cuh"
+
+namespace cd {
+
+constexpr unsigned long long DEDUP_EMPTY = 0x8000000000000000ull;  // INT64_MIN marks a free slot
+
+__device__ __forceinline__ uint32_t dedup_hash(unsigned long long k, uint32_t mask) {
+    k ^= k >> 33;
+    k *= 0xff51afd7ed558ccdull;
+    k ^= k >> 33;
+    k *= 0xc4ceb9fe1a85ec53ull;
+    k ^= k >> 33;
+    return (uint32_t)k & mask;
+}
+
+__global__ void dedup_clear_kernel(unsigned long long* tkey, long long n) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        tkey[i] = DEDUP_EMPTY;
+}
+
+// table: cap slots of {key, min row}; cap is a power of two >= 2N; slot `cap` is reserved for the
+// key INT64_MIN itself.  Pre-set: keys = DEDUP_EMPTY, minrow = INT_MAX.
+__global__ void dedup_insert_kernel(const long long* __restrict__ keys, int N, unsigned long long* tkey,
+                                    int* tmin, uint32_t cap) {
+    const uint32_t mask = cap - 1u;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        const unsigned long long k = (unsigned long long)keys[i];
+        uint32_t slot;
+        if (k == DEDUP_EMPTY) {
+            slot = cap;
+        } else {
+            slot = dedup_hash(k, mask);
+            while (true) {
+                const unsigned long long cur = atomicCAS(tkey + slot, DEDUP_EMPTY, k);
+                if (cur == DEDUP_EMPTY || cur == k) break;
+                slot = (slot + 1u) & mask;
+            }
+        }
+        atomicMin(tmin + slot, (int)i);
+    }
+}
+
+__global__ void dedup_first_kernel(const long long* __restrict__ keys, int N, const unsigned long long* __restrict__ tkey,
+                                   const int* __restrict__ tmin, uint32_t cap, int* __restrict__ first,
+                                   uint8_t* __restrict__ not_first) {
+    const uint32_t mask = cap - 1u;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        const unsigned long long k = (unsigned long long)keys[i];
+        uint32_t slot;
+        if (k == DEDUP_EMPTY) {
+            slot = cap;
+        } else {
+            slot = dedup_hash(k, mask);
+            while (tkey[slot] != k) slot = (slot + 1u) & mask;
+        }
+        const int f = tmin[slot];
+        first[i] = f;
+        not_first[i] = (f == (int)i) ? 0 : 1;
+    }
+}
+
+// One CTA of 1024 threads: stable scan of the first-occurrence flags.  distinct_rows[p] = row id of
+// the p-th distinct value; rank[that row] = p.
+__global__ void __launch_bounds__(1024, 1) dedup_rank_kernel(const uint8_t* __restrict__ not_first, int N,
+                                                             int* __restrict__ distinct_rows, int* __restrict__ rank,
+                                                             int* __restrict__ n_distinct) {
+    __shared__ int s_warp[32];
+    __shared__ int s_total;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    int base = 0;
+    for (int c0 = 0; c0 < N; c0 += 4 * 1024) {
+        const int i0 = c0 + 4 * tid;
+        bool keep[4];
+        if (i0 + 3 < N) {
+            const uint32_t d4 = *reinterpret_cast<const uint32_t*>(not_first + i0);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) keep[q] = ((d4 >> (8 * q)) & 0xFFu) == 0u;
+        } else {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) keep[q] = (i0 + q < N) && (not_first[i0 + q] == 0);
+        }
+        const int cnt = (int)keep[0] + (int)keep[1] + (int)keep[2] + (int)keep[3];
+        int inc = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int u = __shfl_up_sync(FULL, inc, o);
+            if (lane >= o) inc += u;
+        }
+        if (lane == 31) s_warp[warp] = inc;
+        __syncthreads();
+        if (warp == 0) {
+            const int v = s_warp[lane];
+            int w = v;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int u = __shfl_up_sync(FULL, w, o);
+                if (lane >= o) w += u;
+            }
+            s_warp[lane] = w - v;
+            if (lane == 31) s_total = w;
+        }
+        __syncthreads();
+        int pos = base + s_warp[warp] + inc - cnt;
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            if (keep[q]) {
+                distinct_rows[pos] = i0 + q;
+                rank[i0 + q] = pos;
+                ++pos;
+            }
+        base += s_total;
+        __syncthreads();
+    }
+    if (tid == 0) *n_distinct = base;
+}
+
+__global__ void dedup_rep_kernel(const int* __restrict__ first, const int* __restrict__ rank, int N, int* __restrict__ rep) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x)
+        rep[i] = rank[first[i]];
+}
+
+// LEFT JOIN back: row i receives the decode results of distinct value rep[i].
+__global__ void join_kernel(const int* __restrict__ rep, int N, int max_steps, const int* __restrict__ tokens_d,
+                            const int* __restrict__ len_d, const int* __restrict__ fs_d, const float* __restrict__ slp_d,
+                            const uint8_t* __restrict__ done_d, int* __restrict__ tokens, int* __restrict__ len,
+                            int* __restrict__ fs, float* __restrict__ slp, uint8_t* __restrict__ done) {
+    const long long nth = (long long)gridDim.x * blockDim.x;
+    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    for (long long i = tid; i < N; i += nth) {
+        const int r = rep[i];
+        if (len) len[i] = len_d[r];
+        if (fs) fs[i] = fs_d[r];
+        if (slp) slp[i] = slp_d[r];
+        if (done) done[i] = done_d[r];
+    }
+    if (tokens)
+        for (long long j = tid; j < (long long)N * max_steps; j += nth) {
+            const long long i = j / max_steps;
+            tokens[j] = tokens_d[(long long)rep[i] * max_steps + (j - i * max_steps)];
+        }
+}
+
+// Cascade filtering: flag = 1 for rows that are NOT passed on to the next LM
+// predicate (did not finish, or finished in a state outside the satisfying set).
+__global__ void filter_flag_kernel(const int* __restrict__ final_state, const uint8_t* __restrict__ done, int N,
+                                   const uint8_t* __restrict__ satisfying, int S, uint8_t* __restrict__ drop) {
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (long long)gridDim.x * blockDim.x) {
+        const int s = final_state[i];
+        drop[i] = (done[i] && s >= 0 && s < S && satisfying[s]) ? 0 : 1;
+    }
+}
+
+}  // namespace cd

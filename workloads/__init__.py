@@ -441,3 +441,26 @@ def make_head(seed: int, V: int, H: int, std: float, device: str = "cpu", exact:
             x = torch.randn((t1 - t0, H), generator=g, dtype=torch.float32, device=dev)
             out[t0:t1, :H] = (x * (std / (H ** 0.5))).to(torch.bfloat16)
     return out
+
+
+# --------------------------------------------------------------------------
+# row keys for early deduplication
+# --------------------------------------------------------------------------
+def make_keys(seed: int, N: int, n_values: int, device: str = "cpu", skew: bool = False) -> torch.Tensor:
+    """int64 [N] value keys of a table column with at most n_values distinct values (duplication
+    factor rho ~ N / n_values: N = 10^6 rows, |dom| << N).  Row i carries value
+    v_i = hash(seed, i) mod n_values (skew=True: the hash is squared down so that low value ids are
+    frequent, a long-tailed column); the key is a 64-bit scramble of v_i, so keys are spread over
+    the whole int64 range like hashes of strings."""
+    dev = torch.device(device)
+    i = torch.arange(N, dtype=torch.int64, device=dev)
+    z = torch.zeros_like(i)
+    u = mix32_t(seed, 21, i, z)
+    if skew:
+        u2 = mix32_t(seed, 22, i, z)
+        v = ((u % n_values) * (u2 % n_values)) // max(1, n_values)
+    else:
+        v = u % n_values
+    hi = mix32_t(seed, 23, v, z)
+    lo = mix32_t(seed, 24, v, z)
+    return ((hi - (1 << 31)) << 32) | lo
