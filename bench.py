@@ -507,6 +507,29 @@ def main():
         if all_gathered:
             adaptive["touched_gbs"] = adaptive["touched_bytes_per_loop_batch0"] / (ms_a / args.steps * 1e-3) / 1e9
 
+    # ---------------- sampled decoding: the same loops with cd_set_sampling(T = 1)
+    sampling = None
+    if not args.no_adaptive:
+        dfa.set_sampling(1.0, seed=2026)
+        for i in range(args.warmup):
+            one_step(i)
+        barrier()
+        s0, s1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record(stream)
+        for i in range(args.steps):
+            one_step(args.warmup + i)
+        s1.record(stream)
+        barrier()
+        ms_s = s0.elapsed_time(s1)
+        rs_s = int(out["len"].sum())
+        dfa.set_sampling(0.0)
+        sampling = {"value": cfg.B * args.steps * world / (ms_s * 1e-3), "unit": UNIT, "ms_per_step": ms_s / args.steps,
+                    "slowdown_vs_greedy": ms_s / ms, "temperature": 1.0,
+                    "row_steps_last_batch": rs_s,
+                    "note": "Gumbel-max over the allowed set, counter-based noise per (row, step, token): one hash + two "
+                            "fp32 logarithms per ALLOWED element; sampled rows take other paths through the automaton, so "
+                            "row-steps per loop differ from the greedy run"}
+
     # ---------------- e2e: the same metric through the C ABI with HOST buffers
     e2e = None
     if not args.no_e2e:
@@ -602,6 +625,7 @@ def main():
             "e2e": e2e,
             "roofline": roofline,
             "adaptive": adaptive,
+            "sampling": sampling,
             "cpu_baseline": cpu,
             "head": head,
             "dedup": dedup,

@@ -124,6 +124,25 @@ CD_API cd_status cd_dfa_info(const cd_dfa_t* dfa, int32_t* V, int32_t* S, int32_
  */
 CD_API cd_status cd_set_gather_max(cd_dfa_t* dfa, int32_t max_transitions);
 
+/*
+ * Sampling instead of greedy decoding (the paper leaves the decoding rule
+ * open -- only a hidden "temperature" of a comparison system is mentioned).
+ * With temperature T > 0 cd_step / cd_decode_loop* draw the token of every row from the
+ * masked softmax at temperature T by the Gumbel-max rule
+ *     y_t = fl32(x_t * fl32(1 / T)),   t* = argmax_{t in A} fl32(y_t + g(row, step, t))
+ * (ties -> lowest id), where g is Gumbel(0,1) noise from a counter-based generator keyed
+ * by (seed, ORIGINAL row id = row_map[i] or i, step_base + decoding step, token): results
+ * do not depend on batch composition, compaction or launch shape, and a rerun with the
+ * same seed reproduces them bit for bit.  The generator and the fp32 operation sequence
+ * of g are part of the definition (restated in oracle/oracle_cd.c O10).  Outputs:
+ * logprob_out = log of the sampled token's probability under the masked softmax of y,
+ * lse_out = masked logsumexp of y.  T = 0 (default) restores greedy decoding.  For
+ * cd_step the decoding step is step_base; cd_decode_loop* use step_base + k.
+ * Not available on the LM-head path (cd_head_* return CD_ERR_ARG while T > 0).
+ * Call it while no work using the handle is in flight.
+ */
+CD_API cd_status cd_set_sampling(cd_dfa_t* dfa, float temperature, uint64_t seed, int32_t step_base);
+
 /* Creates (or grows) the scratch area of (dfa, cuda_stream) for up to max_rows
    rows, so that later calls on that stream neither allocate nor synchronise. */
 CD_API cd_status cd_reserve(const cd_dfa_t* dfa, int32_t max_rows, void* cuda_stream);

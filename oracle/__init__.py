@@ -9,6 +9,10 @@ from .oracle_cd import (  # noqa: F401
     compact,
     decode_loop,
     dedup,
+    det_logf,
+    gumbel,
+    sample_decode_loop,
+    sample_step,
     filter_rows,
     join_results,
     head_decode_loop,

@@ -472,3 +472,175 @@ int orc_filter_rows(const int32_t *final_state, const uint8_t *done, const int32
     *n_out = k;
     return ORC_OK;
 }
+
+/*
+ * O10: sampling instead of greedy decoding.  The paper leaves the
+ * decoding rule open (only a hidden "temperature" of a comparison system is mentioned,
+ * PAPER.md L226).  Reading (N5): with temperature T > 0 the token of a row is
+ * drawn from the masked softmax of y_t = fl32(x_t * fl32(1/T)) by the Gumbel-max rule
+ *     t* = argmax_{t in A} fl32(y_t + g(row, step, t)),   ties -> lowest id,
+ * g = -ln(-ln u), u = (2 b + 1) / 2^24, b = top 23 bits of a counter hash of
+ * (seed, ORIGINAL row id, step, token).  Because fp32 decides an integer here, the
+ * generator and the fp32 operation sequence of g are part of the definition; this file
+ * restates them in plain C (every operation a single IEEE-754 fp32 operation: compile
+ * with -ffp-contract=off) -- it shares no code with the CUDA path.
+ * Outputs: logprob = log softmax(y)[t*] = (y_t* - m) - log(sum), lse = m + log(sum), with
+ * sum = sum_{t in A} exp(y_t - m) accumulated in double as in O2.
+ */
+static uint32_t orc_fmix32(uint32_t h)
+{
+    h ^= h >> 16;
+    h *= 0x85EBCA6Bu;
+    h ^= h >> 13;
+    h *= 0xC2B2AE35u;
+    h ^= h >> 16;
+    return h;
+}
+
+static uint32_t orc_row_key(uint32_t seed_lo, uint32_t seed_hi, uint32_t row, uint32_t step)
+{
+    uint32_t h = orc_fmix32(seed_lo ^ (row * 0x9E3779B1u));
+    return orc_fmix32(h ^ (step * 0x85EBCA77u) ^ seed_hi);
+}
+
+/* ln x for positive normal fp32 from +, *, /, fma: x = m 2^e, m in [sqrt(1/2), sqrt 2),
+   ln m = 2 atanh(s), s = (m - 1)/(m + 1), odd series up to s^9. */
+float orc_det_logf(float x)
+{
+    int32_t ix;
+    memcpy(&ix, &x, 4);
+    const int32_t e = (ix - 0x3F3504F3) >> 23;
+    const int32_t im = ix - (int32_t)((uint32_t)e << 23);
+    float m;
+    memcpy(&m, &im, 4);
+    const float f = m + -1.0f;
+    const float sden = 2.0f + f;
+    const float sq = f / sden;
+    const float z = sq * sq;
+    float p = fmaf(z, 0.111111111f, 0.142857143f);
+    p = fmaf(z, p, 0.2f);
+    p = fmaf(z, p, 0.333333333f);
+    p = fmaf(z, p, 1.0f);
+    const float two_s = 2.0f * sq;
+    const float r = two_s * p;
+    return fmaf((float)e, 0.693147181f, r);
+}
+
+float orc_gumbel(uint32_t seed_lo, uint32_t seed_hi, uint32_t row, uint32_t step, uint32_t tok)
+{
+    const uint32_t rk = orc_row_key(seed_lo, seed_hi, row, step);
+    const uint32_t h = orc_fmix32(orc_fmix32(rk ^ (tok * 0xC2B2AE3Du)) + 0x27D4EB2Fu);
+    const float u = (float)(2u * (h >> 9) + 1u) * 5.9604644775390625e-8f;
+    const float l1 = -orc_det_logf(u);
+    return -orc_det_logf(l1);
+}
+
+int orc_sample_step(int32_t V, int32_t S, const int64_t *row_ptr, const int32_t *tok, const int32_t *next,
+                    const uint8_t *accepting, const void *logits, int dtype, int64_t ld, const int32_t *row_map,
+                    int32_t *state, int32_t n, float temperature, uint64_t seed, int32_t step,
+                    int32_t *token_out, double *logprob_out, double *lse_out, uint8_t *done_out)
+{
+    if (n < 0 || ld < V || (dtype != ORC_F32 && dtype != ORC_BF16) || !(temperature > 0.0f)) return ORC_ERR_ARG;
+    const int64_t esz = dtype == ORC_BF16 ? 2 : 4;
+    const float inv_tau = 1.0f / temperature;
+    const uint32_t seed_lo = (uint32_t)(seed & 0xFFFFFFFFu), seed_hi = (uint32_t)(seed >> 32);
+    for (int32_t i = 0; i < n; ++i) {
+        const int32_t s = state[i];
+        if (s < 0 || s >= S) return ORC_ERR_ARG;
+        if (accepting[s]) {
+            token_out[i] = -1;
+            logprob_out[i] = 0.0;
+            lse_out[i] = 0.0;
+            done_out[i] = 1;
+            continue;
+        }
+        const int64_t r = row_map ? (int64_t)row_map[i] : (int64_t)i;
+        const char *row = (const char *)logits + r * ld * esz;
+        const int64_t lo = row_ptr[s], hi = row_ptr[s + 1];
+        float m = -INFINITY, kbest = -INFINITY, ybest = -INFINITY;
+        int64_t jstar = lo;
+        for (int64_t j = lo; j < hi; ++j) {
+            const float x = widen(row, dtype, tok[j]); /* NaN -> -inf */
+            const float y = x * inv_tau;
+            if (y > m) m = y;
+            const float g = orc_gumbel(seed_lo, seed_hi, (uint32_t)r, (uint32_t)step, (uint32_t)tok[j]);
+            const float key = y + g;
+            if (key > kbest) { /* ascending id, strictly greater: ties -> lowest id */
+                kbest = key;
+                ybest = y;
+                jstar = j;
+            }
+        }
+        double sum = 0.0;
+        for (int64_t j = lo; j < hi; ++j) {
+            const float y = widen(row, dtype, tok[j]) * inv_tau;
+            if (y == -INFINITY) continue;
+            sum += exp((double)y - (double)m);
+        }
+        if (m == -INFINITY) { /* every allowed logit -inf: lowest allowed id (G6) */
+            jstar = lo;
+            lse_out[i] = -INFINITY;
+            logprob_out[i] = -INFINITY;
+        } else {
+            lse_out[i] = (double)m + log(sum);
+            logprob_out[i] = ((double)ybest - (double)m) - log(sum);
+        }
+        token_out[i] = tok[jstar];
+        state[i] = next[jstar];
+        done_out[i] = accepting[next[jstar]] ? 1 : 0;
+    }
+    return ORC_OK;
+}
+
+/* O4 with O10 as the step: decoding step k uses RNG step step_base + k. */
+int orc_sample_decode_loop(int32_t V, int32_t S, int32_t start, const int64_t *row_ptr, const int32_t *tok,
+                           const int32_t *next, const uint8_t *accepting, const void *const *step_logits, int dtype,
+                           int64_t ld, int32_t B, int32_t max_steps, float temperature, uint64_t seed,
+                           int32_t step_base, int32_t *tokens_out, int32_t *len_out, int32_t *final_state_out,
+                           double *sum_logprob_out, uint8_t *done_out)
+{
+    if (B < 0 || max_steps < 0) return ORC_ERR_ARG;
+    int32_t *ids = (int32_t *)malloc(sizeof(int32_t) * (size_t)(B + 1) * 5);
+    double *lp = (double *)malloc(sizeof(double) * (size_t)(B + 1) * 2);
+    uint8_t *dn = (uint8_t *)malloc((size_t)B + 1);
+    if (!ids || !lp || !dn) {
+        free(ids); free(lp); free(dn);
+        return ORC_ERR_ARG;
+    }
+    int32_t *st = ids + (B + 1), *ids2 = ids + 2 * (B + 1), *st2 = ids + 3 * (B + 1), *tk = ids + 4 * (B + 1);
+    double *lse = lp + (B + 1);
+    int32_t n = 0;
+    for (int32_t r = 0; r < B; ++r) {
+        for (int32_t k = 0; k < max_steps; ++k) tokens_out[(int64_t)r * max_steps + k] = -1;
+        len_out[r] = 0;
+        final_state_out[r] = start;
+        sum_logprob_out[r] = 0.0;
+        done_out[r] = accepting[start] ? 1 : 0;
+        if (!accepting[start]) {
+            ids[n] = r;
+            st[n] = start;
+            ++n;
+        }
+    }
+    int rc = ORC_OK;
+    for (int32_t k = 0; k < max_steps && n > 0; ++k) {
+        rc = orc_sample_step(V, S, row_ptr, tok, next, accepting, step_logits[k], dtype, ld, ids, st, n, temperature,
+                             seed, step_base + k, tk, lp, lse, dn);
+        if (rc != ORC_OK) break;
+        for (int32_t i = 0; i < n; ++i) {
+            const int32_t r = ids[i];
+            tokens_out[(int64_t)r * max_steps + k] = tk[i];
+            len_out[r] = k + 1;
+            final_state_out[r] = st[i];
+            sum_logprob_out[r] += lp[i];
+            done_out[r] = dn[i];
+        }
+        int32_t n2 = 0;
+        orc_compact(dn, ids, st, n, ids2, st2, &n2);
+        memcpy(ids, ids2, sizeof(int32_t) * (size_t)n2);
+        memcpy(st, st2, sizeof(int32_t) * (size_t)n2);
+        n = n2;
+    }
+    free(ids); free(lp); free(dn);
+    return rc;
+}

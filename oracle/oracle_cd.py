@@ -35,7 +35,7 @@ def build(force: bool = False) -> str:
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
         tmp = _SO + f".tmp{os.getpid()}"
         subprocess.check_call(
-            ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"]
+            ["gcc", "-O2", "-ffp-contract=off", "-std=c11", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"]
         )
         os.replace(tmp, _SO)
     return _SO
@@ -53,6 +53,12 @@ def _load():
         _lib.orc_head_step.restype = C.c_int
         _lib.orc_head_decode_loop.restype = C.c_int
         _lib.orc_dedup.restype = C.c_int
+        _lib.orc_sample_step.restype = C.c_int
+        _lib.orc_sample_decode_loop.restype = C.c_int
+        _lib.orc_det_logf.restype = C.c_float
+        _lib.orc_det_logf.argtypes = [C.c_float]
+        _lib.orc_gumbel.restype = C.c_float
+        _lib.orc_gumbel.argtypes = [C.c_uint32] * 5
         _lib.orc_join_results.restype = C.c_int
         _lib.orc_filter_rows.restype = C.c_int
         _lib.orc_head_logit.restype = C.c_double
@@ -299,3 +305,58 @@ def filter_rows(final_state, done, satisfying, row_ids=None):
     if rc != OK:
         raise OracleError(rc)
     return out[: k.value].copy()
+
+
+def det_logf(x: float) -> float:
+    """The fp32 logarithm of the sampling definition (O10)."""
+    return float(_load().orc_det_logf(C.c_float(x)))
+
+
+def gumbel(seed: int, row: int, step: int, tok: int) -> float:
+    """Gumbel noise of (seed, row, step, token) (O10)."""
+    return float(_load().orc_gumbel(seed & 0xFFFFFFFF, (seed >> 32) & 0xFFFFFFFF, row, step, tok))
+
+
+def sample_step(aut, logits, state: Sequence[int], temperature: float, seed: int, step: int = 0,
+                row_map: Optional[Sequence[int]] = None):
+    """One sampled step (O10).  Returns (token, logprob f64, lse f64, done, new_state)."""
+    V, S, start, rp, tok, nxt, acc = _csr(aut)
+    x, dt = _logits_np(logits)
+    ld = x.shape[1]
+    st = np.ascontiguousarray(np.asarray(state, dtype=np.int32)).copy()
+    n = st.shape[0]
+    rm = None if row_map is None else np.ascontiguousarray(np.asarray(row_map, dtype=np.int32))
+    token = np.empty(n, np.int32)
+    lp = np.empty(n, np.float64)
+    lse = np.empty(n, np.float64)
+    done = np.empty(n, np.uint8)
+    rc = _load().orc_sample_step(
+        C.c_int32(V), C.c_int32(S), _p(rp), _p(tok), _p(nxt), _p(acc), _p(x), C.c_int(dt), C.c_int64(ld), _p(rm),
+        _p(st), C.c_int32(n), C.c_float(temperature), C.c_uint64(seed), C.c_int32(step), _p(token), _p(lp), _p(lse),
+        _p(done))
+    if rc != OK:
+        raise OracleError(rc)
+    return token, lp, lse, done, st
+
+
+def sample_decode_loop(aut, step_logits: List, temperature: float, seed: int, step_base: int = 0,
+                       max_steps: Optional[int] = None):
+    """The loop with sampled steps (O4 on O10)."""
+    V, S, start, rp, tok, nxt, acc = _csr(aut)
+    max_steps = len(step_logits) if max_steps is None else max_steps
+    arrs = [_logits_np(x) for x in step_logits[:max_steps]]
+    B, ld = arrs[0][0].shape
+    dt = arrs[0][1]
+    ptrs = (C.c_void_p * max_steps)(*[a.ctypes.data for a, _ in arrs])
+    tokens = np.empty((B, max_steps), np.int32)
+    ln = np.empty(B, np.int32)
+    fs = np.empty(B, np.int32)
+    slp = np.empty(B, np.float64)
+    done = np.empty(B, np.uint8)
+    rc = _load().orc_sample_decode_loop(
+        C.c_int32(V), C.c_int32(S), C.c_int32(start), _p(rp), _p(tok), _p(nxt), _p(acc), ptrs, C.c_int(dt),
+        C.c_int64(ld), C.c_int32(B), C.c_int32(max_steps), C.c_float(temperature), C.c_uint64(seed),
+        C.c_int32(step_base), _p(tokens), _p(ln), _p(fs), _p(slp), _p(done))
+    if rc != OK:
+        raise OracleError(rc)
+    return dict(tokens=tokens, len=ln, final_state=fs, sum_logprob=slp, done=done)

@@ -17,7 +17,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
-    "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_reserve", "cd_step",
+    "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_set_sampling", "cd_reserve", "cd_step",
     "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
     "cd_last_error",
 )
@@ -105,6 +105,10 @@ class Dfa:
     def set_gather_max(self, max_transitions: int):
         """cd_set_gather_max: 0 = dense scan only, > 0 threshold, -1 automatic."""
         _check(lib().cd_set_gather_max(self._h, C.c_int32(max_transitions)))
+
+    def set_sampling(self, temperature: float, seed: int = 0, step_base: int = 0):
+        """cd_set_sampling: temperature 0 = greedy; > 0 = seeded Gumbel-max sampling."""
+        _check(lib().cd_set_sampling(self._h, C.c_float(temperature), C.c_uint64(seed), C.c_int32(step_base)))
 
     def set_head_gather_max(self, max_transitions: int):
         """cd_set_head_gather_max: 0 = dense contraction for every state, > 0 threshold, -1 automatic."""

@@ -137,6 +137,9 @@ struct cd_dfa {
     void* d_next = nullptr;
     void* d_acc = nullptr;
     void* d_satisfying = nullptr;  // cd_set_satisfying
+    float inv_tau = 0.0f;          // cd_set_sampling: 0 = greedy, else 1 / temperature
+    unsigned long long seed = 0;
+    int rng_step_base = 0;
     long long min_deg_nonacc = 0;  // fewest transitions of a non-accepting state
     int head_gather_max = -1;      // cd_set_head_gather_max: 0 never gather, > 0 threshold, < 0 automatic
     const void* w_ptr = nullptr;   // cached tensor map of the output embedding (cd_head_step)
@@ -245,10 +248,10 @@ cd_status check_dtype(cd_dtype dt) {
     return CD_OK;
 }
 
-template <int DT, int VAR, bool GATHER = false>
+template <int DT, int VAR, bool GATHER = false, bool SAMPLE = false>
 cd_status launch_step_t(const cd::StepArgs& a, int grid, cudaStream_t stream) {
     constexpr StepCfg C = STEP_CFGS[VAR];
-    auto kern = cd::step_kernel<DT, C.warps, C.stages, C.tile_bytes, GATHER>;
+    auto kern = cd::step_kernel<DT, C.warps, C.stages, C.tile_bytes, GATHER, SAMPLE>;
     const size_t smem = sizeof(cd::WarpRing<C.stages, C.tile_bytes>) * C.warps;
     static thread_local int configured_dev = -1;
     int dev = 0;
@@ -277,6 +280,9 @@ cd_status launch_step_t(const cd::StepArgs& a, int grid, cudaStream_t stream) {
 
 template <int DT>
 cd_status launch_step_v(const cd::StepArgs& a, int grid, cudaStream_t stream) {
+    if (a.inv_tau > 0.0f)  // sampling
+        return a.gather_max > 0 ? launch_step_t<DT, 0, true, true>(a, grid, stream)
+                                : launch_step_t<DT, 0, false, true>(a, grid, stream);
     if (a.gather_max > 0) return launch_step_t<DT, 0, true>(a, grid, stream);  // density-adaptive rows
     switch (step_variant()) {
         case 1: return launch_step_t<DT, 1>(a, grid, stream);
@@ -342,6 +348,10 @@ cd_status launch_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype 
     a.ctrs = s->ctrs;
     a.gather_max = gather_max_for(d, dtype);
     a.all_gather = (d->max_deg <= a.gather_max) ? 1 : 0;
+    a.inv_tau = d->inv_tau;
+    a.seed_lo = (uint32_t)(d->seed & 0xFFFFFFFFull);
+    a.seed_hi = (uint32_t)(d->seed >> 32);
+    a.rng_step_base = d->rng_step_base;
     const int grid = step_grid(d, n_upper, dtype);
     return dtype == CD_BF16 ? launch_step_v<cd::DT_BF16>(a, grid, stream)
                             : launch_step_v<cd::DT_F32>(a, grid, stream);
@@ -1027,6 +1037,16 @@ cd_status launch_head(const cd_dfa* d, Scratch* s, const void* hidden, long long
 
 extern "C" {
 
+cd_status cd_set_sampling(cd_dfa_t* d, float temperature, uint64_t seed, int32_t step_base) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (!(temperature >= 0.0f) || temperature > 3.0e38f) return fail(CD_ERR_ARG, "temperature must be finite and >= 0");
+    if (step_base < 0) return fail(CD_ERR_ARG, "step_base < 0");
+    d->inv_tau = temperature > 0.0f ? 1.0f / temperature : 0.0f;  // IEEE fp32 division, as the oracle's
+    d->seed = seed;
+    d->rng_step_base = step_base;
+    return CD_OK;
+}
+
 cd_status cd_set_head_gather_max(cd_dfa_t* d, int32_t max_transitions) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
     if (max_transitions < -1) return fail(CD_ERR_ARG, "max_transitions must be >= -1");
@@ -1039,6 +1059,7 @@ cd_status cd_head_step(const cd_dfa_t* d, const void* hidden, int64_t ldh_elems,
                        float* logprob_out, float* lse_out, uint8_t* done_out, void* cuda_stream) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
     if (n < 0) return fail(CD_ERR_ARG, "n < 0");
+    if (d->inv_tau > 0.0f) return fail(CD_ERR_ARG, "sampling (cd_set_sampling) is not available on the LM-head path");
     cd_status st = check_head_layout(hidden, ldh_elems, W, ldw_elems, H);
     if (st != CD_OK) return st;
     if (n == 0) return CD_OK;
@@ -1066,6 +1087,7 @@ cd_status cd_head_decode_loop(const cd_dfa_t* d, const void* const* step_hidden,
     if (!len_out || !final_state_out || !sum_logprob_out || !done_out || (max_steps > 0 && !tokens_out))
         return fail(CD_ERR_ARG, "NULL output pointer");
     if (max_steps > 0 && !step_hidden) return fail(CD_ERR_ARG, "step_hidden is NULL");
+    if (d->inv_tau > 0.0f) return fail(CD_ERR_ARG, "sampling (cd_set_sampling) is not available on the LM-head path");
     cd_status st = CD_OK;
     for (int k = 0; k < max_steps; ++k) {
         st = check_head_layout(step_hidden[k], ldh_elems, W, ldw_elems, H);

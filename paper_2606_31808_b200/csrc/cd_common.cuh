@@ -154,6 +154,76 @@ __device__ __forceinline__ void warp_combine(float& m, float& s, int& idx) {
     }
 }
 
+// ---------------------------------------------------------------- sampling
+// Gumbel-max over the allowed set with a counter-based generator: the noise of (row, step, token)
+// is a pure function of the seed, so results do not depend on launch shape, compaction or the
+// order rows are processed in.  Every operation below is an IEEE-754 correctly rounded fp32
+// operation (explicit _rn intrinsics: never contracted or reordered) or integer arithmetic, so the
+// CPU oracle, which restates the same definition in C, decides the argmax on identical bits.
+__device__ __forceinline__ uint32_t fmix32(uint32_t h) {
+    h ^= h >> 16;
+    h *= 0x85EBCA6Bu;
+    h ^= h >> 13;
+    h *= 0xC2B2AE35u;
+    h ^= h >> 16;
+    return h;
+}
+
+// per (row, step) part of the counter hash
+__device__ __forceinline__ uint32_t rng_row_key(uint32_t seed_lo, uint32_t seed_hi, uint32_t row, uint32_t step) {
+    uint32_t h = fmix32(seed_lo ^ (row * 0x9E3779B1u));
+    return fmix32(h ^ (step * 0x85EBCA77u) ^ seed_hi);
+}
+
+// natural logarithm of a positive normal fp32 from +, *, /, fma only:
+// x = m * 2^e with m in [sqrt(1/2), sqrt(2)); ln m = 2 atanh(s), s = (m - 1) / (m + 1), odd series to s^9
+__device__ __forceinline__ float det_logf(float x) {
+    const int ix = __float_as_int(x);
+    const int e = (ix - 0x3F3504F3) >> 23;
+    const float m = __int_as_float(ix - (e << 23));
+    const float f = __fadd_rn(m, -1.0f);
+    const float sden = __fadd_rn(2.0f, f);
+    const float sq = __fdiv_rn(f, sden);
+    const float z = __fmul_rn(sq, sq);
+    float p = __fmaf_rn(z, 0.111111111f, 0.142857143f);
+    p = __fmaf_rn(z, p, 0.2f);
+    p = __fmaf_rn(z, p, 0.333333333f);
+    p = __fmaf_rn(z, p, 1.0f);
+    const float r = __fmul_rn(__fmul_rn(2.0f, sq), p);
+    return __fmaf_rn((float)e, 0.693147181f, r);
+}
+
+// Gumbel(0,1) noise of token `tok`: u = (2b + 1) / 2^24 with b = top 23 hash bits (exact in fp32,
+// inside (0,1)), g = -ln(-ln u)
+__device__ __forceinline__ float gumbel_noise(uint32_t row_key, uint32_t tok) {
+    const uint32_t h = fmix32(fmix32(row_key ^ (tok * 0xC2B2AE3Du)) + 0x27D4EB2Fu);
+    const float u = __fmul_rn((float)(2u * (h >> 9) + 1u), 5.9604644775390625e-8f);  // * 2^-24, exact
+    const float l1 = -det_logf(u);  // in [2^-24.x, 16.7]
+    return -det_logf(l1);
+}
+
+// Online update of the sampling state: (m, s) over y = x * inv_tau as in online_update, plus the
+// running best perturbed key and its token (ascending ids per lane: strictly greater replaces).
+__device__ __forceinline__ void online_update_sample(float& m, float& s, float& kb, int& kidx, float x, int t, int pos,
+                                                     float inv_tau, uint32_t row_key) {
+    const float y = fmaxf(__fmul_rn(x, inv_tau), -INFINITY);
+    const float lo = fminf(m, y), hi = fmaxf(m, y);
+    float e = ex2_ftz((lo - hi) * LOG2E);
+    e = (lo == -INFINITY) ? 0.0f : e;
+    s = (y > m) ? fmaf(s, e, 1.0f) : s + e;
+    m = hi;
+    const float key = __fadd_rn(y, gumbel_noise(row_key, (uint32_t)t));
+    const bool gt = key > kb;
+    kb = gt ? key : kb;
+    kidx = gt ? pos : kidx;
+}
+
+__device__ __forceinline__ void sample_combine(float& kb, int& kidx, float k2, int i2) {
+    const bool take2 = (k2 > kb) || (k2 == kb && i2 < kidx);
+    kb = take2 ? k2 : kb;
+    kidx = take2 ? i2 : kidx;
+}
+
 // ---------------------------------------------------------------- CSR transition lookup
 // Warp-cooperative 128-ary search of `token` in the sorted CSR row tok[lo, hi): every round each
 // lane probes 4 of 128 split points (independent loads), so a row of <= 4096 entries needs one

@@ -100,6 +100,11 @@ struct StepArgs {
     const uint8_t* satisfying;  // [S]
     int* sat_ctr;
     int limit;
+    // sampling (SAMPLE instantiation): Gumbel-max at temperature 1 / inv_tau with the
+    // counter-based noise of (seed, original row id, rng_step_base + step, token)
+    float inv_tau;
+    uint32_t seed_lo, seed_hi;
+    int rng_step_base;
 };
 
 struct __align__(16) TileMeta {
@@ -141,8 +146,9 @@ __device__ __forceinline__ float tile_elem(const unsigned char* tile, int e) {
 
 // Row finished: (m, s, idx) is the merged result of all its units.  Warp-uniform.
 // `gathered`: idx is the position inside the state's CSR row instead of the token id.
+// `sampled`: idx is the sampled token (position), ytok its tempered logit: logprob = (ytok - m) - log(sum).
 __device__ __forceinline__ void finalize_row(const StepArgs& a, const TileMeta& mt, float m, float s, int idx,
-                                             int lane, bool gathered) {
+                                             int lane, bool gathered, bool sampled = false, float ytok = 0.0f) {
     const long long lo = mt.csr_lo, hi = mt.csr_lo + mt.csr_len;
     int token;
     float lp, lse;
@@ -155,7 +161,7 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const TileMeta& 
     } else {
         token = idx;
         const float L = logf(s);
-        lp = -L;  // log p(t*) = x_t* - lse = -log(sum); never m - lse (cancellation)
+        lp = sampled ? (ytok - m) - L : -L;  // greedy: log p(t*) = -log(sum); never m - lse (cancellation)
         lse = m + L;
     }
     if (gathered) {
@@ -193,7 +199,25 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const TileMeta& 
     }
 }
 
-template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER>
+template <bool SAMPLE>
+__device__ __forceinline__ void warp_combine_s(float& m, float& s, int& idx, float& kb) {
+    if constexpr (!SAMPLE) {
+        warp_combine(m, s, idx);
+    } else {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const float m2 = __shfl_xor_sync(FULL, m, o);
+            const float s2 = __shfl_xor_sync(FULL, s, o);
+            const int i2 = __shfl_xor_sync(FULL, idx, o);
+            const float k2 = __shfl_xor_sync(FULL, kb, o);
+            int dummy = 0;
+            online_combine(m, s, dummy, m2, s2, 0);
+            sample_combine(kb, idx, k2, i2);
+        }
+    }
+}
+
+template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER, bool SAMPLE = false>
 __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     constexpr int SZ = (DT == DT_BF16) ? 2 : 4;
     constexpr int TILE_TOK = TILE_BYTES / SZ;
@@ -242,7 +266,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
 
     bool exhausted = false;
     int iss_tile = 0, iss_end = 0;
-    int iss_slot = 0, iss_st = 0, iss_flags = 0, iss_len = 0;
+    int iss_slot = 0, iss_st = 0, iss_flags = 0, iss_len = 0, iss_row = 0;
     long long iss_lo = 0;
     const unsigned char* iss_src = nullptr;  // next logits tile of the current unit
     const unsigned char* iss_msk = nullptr;  // next mask piece
@@ -263,6 +287,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
             // unit drawn after its row was finalised still sees the state the row was processed in
             iss_st = a.state[iss_slot];
             const long long r = a.row_map ? (long long)__ldg(a.row_map + iss_slot) : (long long)iss_slot;
+            iss_row = (int)r;
             const bool bad = (iss_st < 0) || (iss_st >= a.dfa.S);
             const int sts = bad ? 0 : iss_st;
             const bool acc = !bad && (__ldg(a.dfa.accepting + sts) != 0);
@@ -321,13 +346,13 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 reinterpret_cast<uint32_t*>(ring.mask[iss_stage])[w] = 0u;
             __syncwarp();
             if (lane == 0) {
-                ring.meta[iss_stage] = TileMeta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, 0};
+                ring.meta[iss_stage] = TileMeta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, iss_row};
                 mbar_arrive_expect_tx(bar, bulk + mbytes);
                 if (bulk) bulk_g2s_hint(dst, iss_src, bulk, bar, pol_stream);
                 bulk_g2s(mdst, iss_msk, mbytes, bar);
             }
         } else if (lane == 0) {
-            ring.meta[iss_stage] = TileMeta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, 0};
+            ring.meta[iss_stage] = TileMeta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, iss_row};
             mbar_arrive_expect_tx(bar, TILE_BYTES + MASK_BYTES);
             bulk_g2s_hint(dst, iss_src, TILE_BYTES, bar, pol_stream);
             bulk_g2s(mdst, iss_msk, MASK_BYTES, bar);
@@ -344,8 +369,9 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     for (int k = 0; k < STAGES; ++k) issue_one();
 
     // ---------------- consume side
-    float m = -INFINITY, s = 0.0f;
+    float m = -INFINITY, s = 0.0f, kb = -INFINITY;  // kb: best perturbed key (SAMPLE); idx then is its token
     int idx = 0x7FFFFFFF;
+    const int rng_step = a.rng_step_base + a.step;
     int cons_stage = 0;
     uint32_t cons_phase = 0;
     const unsigned long long tag = (unsigned long long)gen << 32;
@@ -376,7 +402,9 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 // ascends with the token id, so "replace on strictly greater" keeps the lowest id
                 m = -INFINITY;
                 s = 0.0f;
+                kb = -INFINITY;
                 idx = 0x7FFFFFFF;
+                const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, (uint32_t)mt.tile, (uint32_t)rng_step) : 0u;
                 const int j0 = (int)(((long long)mt.csr_len * part) / np);
                 const int j1 = (int)(((long long)mt.csr_len * (part + 1)) / np);
                 const int* tk = a.dfa.tok + mt.csr_lo;
@@ -403,19 +431,28 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                         x[u] = v;
                     }
                     const int jn = j + 32 * GATHER_UNROLL;
+                    int tc[GATHER_UNROLL];
+#pragma unroll
+                    for (int u = 0; u < GATHER_UNROLL; ++u) tc[u] = t[u];
 #pragma unroll
                     for (int u = 0; u < GATHER_UNROLL; ++u) t[u] = (jn + 32 * u < j1) ? __ldg(tk + jn + 32 * u) : -1;
 #pragma unroll
-                    for (int u = 0; u < GATHER_UNROLL; ++u)
-                        online_update(m, s, idx, fmaxf(x[u], -INFINITY), j + 32 * u);  // NaN -> -inf
+                    for (int u = 0; u < GATHER_UNROLL; ++u) {
+                        if (SAMPLE)
+                            online_update_sample(m, s, kb, idx, fmaxf(x[u], -INFINITY), tc[u], j + 32 * u, a.inv_tau, row_key);
+                        else
+                            online_update(m, s, idx, fmaxf(x[u], -INFINITY), j + 32 * u);  // NaN -> -inf
+                    }
                 }
                 __syncwarp();
             } else {
             if (mt.flags & FLAG_FIRST) {
                 m = -INFINITY;
                 s = 0.0f;
+                kb = -INFINITY;
                 idx = 0x7FFFFFFF;
             }
+            const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, (uint32_t)mt.pad, (uint32_t)rng_step) : 0u;
             const int t0 = mt.tile * TILE_TOK;
             const uint32_t* mw = reinterpret_cast<const uint32_t*>(ring.mask[cons_stage]);
             const unsigned char* tile = ring.logits[cons_stage];
@@ -432,16 +469,30 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                     const int e = e0 + (v ? (__ffs(b) - 1) : 0);
                     b &= b - 1u;
                     const float x = v ? tile_elem<DT>(tile, e) : -INFINITY;
-                    online_update(m, s, idx, x, t0 + e);
+                    if (SAMPLE)
+                        online_update_sample(m, s, kb, idx, x, t0 + e, t0 + e, a.inv_tau, row_key);
+                    else
+                        online_update(m, s, idx, x, t0 + e);
                 }
             }
             }
             if (mt.flags & FLAG_LAST) {
-                float rm = m, rs = s;
+                float rm = m, rs = s, rk = kb;
                 int ri = idx;
-                warp_combine(rm, rs, ri);
+                warp_combine_s<SAMPLE>(rm, rs, ri, rk);
+                // SAMPLE: the tempered logit of the sampled token is re-read from the logits row
+                auto sampled_y = [&](int pos) -> float {
+                    if (!SAMPLE || rm == -INFINITY) return 0.0f;
+                    const int tokid = gathered ? __ldg(a.dfa.tok + mt.csr_lo + pos) : pos;
+                    const long long rr = gathered ? (long long)mt.tile : (long long)mt.pad;
+                    const unsigned char* rowp = a.logits + rr * a.ld_bytes;
+                    const float xv = (DT == DT_BF16)
+                                         ? __uint_as_float(((uint32_t)__ldg(reinterpret_cast<const uint16_t*>(rowp) + tokid)) << 16)
+                                         : __ldg(reinterpret_cast<const float*>(rowp) + tokid);
+                    return __fmul_rn(xv, a.inv_tau);
+                };
                 if (np == 1) {
-                    finalize_row(a, mt, rm, rs, ri, lane, gathered);
+                    finalize_row(a, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
                 } else {
                     // Publish from lane 1 (lane 0 is busy issuing copies): three self-validating
                     // words, then a RELAXED ticket -- no fence anywhere.  The last arriver merges.
@@ -451,6 +502,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                         st_relaxed_gpu_u64(&ps->m, tag | (unsigned)__float_as_int(rm));
                         st_relaxed_gpu_u64(&ps->s, tag | (unsigned)__float_as_int(rs));
                         st_relaxed_gpu_u64(&ps->idx, tag | (unsigned)ri);
+                        if (SAMPLE) st_relaxed_gpu_u64(&ps->pad, tag | (unsigned)__float_as_int(rk));
                         t = atomicAdd(a.tickets + mt.slot, 1);
                     }
                     t = __shfl_sync(FULL, t, 1);
@@ -462,34 +514,49 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                         // Merge in slot order whoever merges (bitwise reproducible): lane q%32 takes
                         // slot q; the own result (identical in every lane after the butterfly) stands
                         // in for slot `part`.
-                        const float om = rm, os = rs;
+                        const float om = rm, os = rs, ok_ = rk;
                         const int oi = ri;
                         rm = -INFINITY;
                         rs = 0.0f;
+                        rk = -INFINITY;
                         ri = 0x7FFFFFFF;
                         for (int q0 = 0; q0 < np; q0 += 32) {
                             const int q = q0 + lane;
                             const bool want = (q < np) && (q != part);
                             bool ok = !want;
-                            unsigned long long wm = 0, ws = 0, wi = 0;
+                            unsigned long long wm = 0, ws = 0, wi = 0, wk = 0;
                             while (true) {
                                 if (!ok) {
                                     wm = ld_relaxed_gpu_u64(&base[q].m);
                                     ws = ld_relaxed_gpu_u64(&base[q].s);
                                     wi = ld_relaxed_gpu_u64(&base[q].idx);
                                     ok = ((wm >> 32) == gen) && ((ws >> 32) == gen) && ((wi >> 32) == gen);
+                                    if (SAMPLE) {
+                                        wk = ld_relaxed_gpu_u64(&base[q].pad);
+                                        ok = ok && ((wk >> 32) == gen);
+                                    }
                                 }
                                 if (__all_sync(FULL, ok)) break;
                                 __nanosleep(32);
                             }
-                            if (want)
+                            if (SAMPLE) {
+                                int dummy = 0;
+                                if (want) {
+                                    online_combine(rm, rs, dummy, __int_as_float((int)(unsigned)wm),
+                                                   __int_as_float((int)(unsigned)ws), 0);
+                                    sample_combine(rk, ri, __int_as_float((int)(unsigned)wk), (int)(unsigned)wi);
+                                } else if (q == part) {
+                                    online_combine(rm, rs, dummy, om, os, 0);
+                                    sample_combine(rk, ri, ok_, oi);
+                                }
+                            } else if (want)
                                 online_combine(rm, rs, ri, __int_as_float((int)(unsigned)wm),
                                                __int_as_float((int)(unsigned)ws), (int)(unsigned)wi);
                             else if (q == part)
                                 online_combine(rm, rs, ri, om, os, oi);
                         }
-                        warp_combine(rm, rs, ri);
-                        finalize_row(a, mt, rm, rs, ri, lane, gathered);
+                        warp_combine_s<SAMPLE>(rm, rs, ri, rk);
+                        finalize_row(a, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
                     }
                 }
             }

@@ -1,0 +1,155 @@
+"""Parity of the sampled step (cd_set_sampling, through the C ABI) with the
+oracle's O10.  The Gumbel-max decision is taken in fp32 on identical bits on both sides
+(counter-based generator and fp32 operation sequence are part of the definition), so token,
+state, done and histories are compared bit-exactly; logprob / lse within 1e-5*max(1,|ref|)."""
+import numpy as np
+import pytest
+import torch
+
+import workloads as wl
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-5
+
+
+@pytest.fixture(scope="module")
+def cd():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_2606_31808_b200 as m
+
+    m.lib()
+    return m
+
+
+@pytest.fixture(params=["dense", "gather_all", "gather_mixed"])
+def mode(request):
+    return request.param
+
+
+def dev_dfa(cd, aut, mode):
+    dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device="cuda:0")
+    if mode == "gather_all":
+        dfa.set_gather_max(2**30)
+    elif mode == "gather_mixed":
+        deg = torch.diff(torch.as_tensor(aut.row_ptr).cpu())
+        deg = deg[deg > 0]
+        dfa.set_gather_max(max(1, int(deg.median())))
+    return dfa
+
+
+def close(gpu, ref):
+    gpu = np.asarray(gpu, np.float64)
+    both_inf = np.isneginf(gpu) & np.isneginf(ref)
+    err = np.abs(np.where(both_inf, 0.0, gpu - ref))
+    return bool(np.all(err <= TOL * np.maximum(1.0, np.abs(np.where(both_inf, 0.0, ref)))))
+
+
+def live_states(aut, n, mult=3):
+    acc = np.asarray(aut.accepting)
+    live = [s for s in range(aut.S) if not acc[s]]
+    return [live[(i * mult) % len(live)] for i in range(n)]
+
+
+@pytest.mark.parametrize("V,S,n,density,dtype,T", [
+    (1000, 7, 37, 0.3, torch.float32, 1.0),
+    (40000, 12, 70, 0.05, torch.bfloat16, 0.7),    # several tiles and units per row
+    (262144, 16, 9, 0.02, torch.bfloat16, 1.3),    # full vocabulary, few rows: many units per row (merge path)
+    (5000, 5, 300, 1.0, torch.bfloat16, 2.0),      # everything allowed: ties in y, noise decides
+    (776, 4, 5, 0.5, torch.float32, 0.25),
+])
+def test_sampled_step_matches_oracle(cd, oracle, mode, V, S, n, density, dtype, T):
+    aut = wl.make_random_dfa(51, V, S, density, 0.2)
+    dfa = dev_dfa(cd, aut, mode)
+    dfa.set_sampling(T, seed=0x1234567890ABCDEF, step_base=4)
+    x = wl.make_logits(51, 0, n + 10, V, 2.0, dtype)
+    states = live_states(aut, n)
+    row_map = [(i * 7 + 3) % (n + 10) for i in range(n)]
+    st_d = torch.tensor(states, dtype=torch.int32, device="cuda:0")
+    rm_d = torch.tensor(row_map, dtype=torch.int32, device="cuda:0")
+    tok, lp, lse, done = cd.step(dfa, x.to("cuda:0"), st_d, row_map=rm_d)
+    torch.cuda.synchronize()
+    o_tok, o_lp, o_lse, o_done, o_st = oracle.sample_step(aut, x, states, T, seed=0x1234567890ABCDEF, step=4,
+                                                          row_map=row_map)
+    assert tok.cpu().numpy().tolist() == o_tok.tolist()
+    assert st_d.cpu().numpy().tolist() == o_st.tolist()
+    assert done.cpu().numpy().tolist() == o_done.tolist()
+    assert close(lp.cpu().numpy(), o_lp) and close(lse.cpu().numpy(), o_lse)
+    # greedy is restored by temperature 0
+    dfa.set_sampling(0.0)
+    st_d = torch.tensor(states, dtype=torch.int32, device="cuda:0")
+    tok, _, _, _ = cd.step(dfa, x.to("cuda:0"), st_d, row_map=rm_d)
+    g_tok = oracle.step(aut, x, states, row_map=row_map)[0]
+    assert tok.cpu().numpy().tolist() == g_tok.tolist()
+
+
+def test_sampled_step_special_values(cd, oracle, mode):
+    V, S, n = 600, 4, 20
+    aut = wl.make_random_dfa(53, V, S, 0.3, 0.25)
+    dfa = dev_dfa(cd, aut, mode)
+    dfa.set_sampling(1.0, seed=7)
+    x = wl.make_logits(53, 0, n, V, 2.0, torch.float32)
+    lo, hi = int(aut.row_ptr[0]), int(aut.row_ptr[1])
+    allowed0 = [int(t) for t in aut.tok[lo:hi]]
+    x[0, allowed0] = float("-inf")      # every allowed logit -inf: lowest allowed id, logprob -inf
+    x[1, allowed0[:3]] = float("nan")   # NaN read as -inf
+    x[2, :] = 1e30                      # huge everywhere
+    x[3, [t for t in range(V) if t not in set(allowed0)]] = float("nan")  # poisoned complement
+    states = [0] * n
+    st_d = torch.tensor(states, dtype=torch.int32, device="cuda:0")
+    tok, lp, lse, done = cd.step(dfa, x.to("cuda:0"), st_d)
+    torch.cuda.synchronize()
+    o_tok, o_lp, o_lse, o_done, o_st = oracle.sample_step(aut, x, states, 1.0, seed=7)
+    assert tok.cpu().numpy().tolist() == o_tok.tolist() and st_d.cpu().numpy().tolist() == o_st.tolist()
+    assert close(lp.cpu().numpy(), o_lp) and close(lse.cpu().numpy(), o_lse)
+    assert tok[0] == allowed0[0] and np.isneginf(float(lp[0]))
+
+
+@pytest.mark.parametrize("kind,V,B,steps,dtype", [("dfa", 3000, 300, 8, torch.bfloat16), ("trie", 2000, 150, 5, torch.float32)])
+def test_sampled_decode_loop_matches_oracle(cd, oracle, mode, kind, V, B, steps, dtype):
+    if kind == "dfa":
+        aut = wl.make_random_dfa(57, V, 20, 0.1, 0.15)
+    else:
+        aut = wl.make_trie(V, wl.draw_labels(57, V, 25, 1, 5))
+    dfa = dev_dfa(cd, aut, mode)
+    dfa.set_sampling(0.9, seed=99, step_base=2)
+    logits = [wl.make_logits(57, k, B, V, 2.0, dtype) for k in range(steps)]
+    got = cd.decode_loop(dfa, [x.to("cuda:0") for x in logits])
+    torch.cuda.synchronize()
+    want = oracle.sample_decode_loop(aut, logits, 0.9, seed=99, step_base=2)
+    for k in ("tokens", "len", "final_state", "done"):
+        assert np.array_equal(got[k].cpu().numpy(), want[k]), k
+    slp = got["sum_logprob"].cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(slp - want["sum_logprob"]) <= TOL * (want["len"] + np.abs(want["sum_logprob"])) + 1e-12)
+    # same seed reproduces bit for bit; another seed does not
+    again = cd.decode_loop(dfa, [x.to("cuda:0") for x in logits])
+    assert torch.equal(again["tokens"], got["tokens"]) and torch.equal(again["sum_logprob"], got["sum_logprob"])
+    dfa.set_sampling(0.9, seed=100, step_base=2)
+    other = cd.decode_loop(dfa, [x.to("cuda:0") for x in logits])
+    assert not torch.equal(other["tokens"], got["tokens"])
+
+
+def test_sampled_full_size_c4_batch(cd, oracle):
+    """One c4 step at full size (n = 4096, V = 262144, the launch configuration bench.py times) with
+    sampling on: every row on the GPU, the oracle on 64 sampled rows (rows are independent)."""
+    cfg = wl.CONFIGS["c4"]
+    aut = wl.build_automaton(cfg)
+    dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device="cuda:0")
+    dfa.set_sampling(1.0, seed=2026, step_base=0)
+    x = wl.make_logits(cfg.seed, 0, cfg.B, cfg.V, cfg.std, cfg.dtype, device="cuda:0")
+    states = live_states(aut, cfg.B, mult=7)
+    st_d = torch.tensor(states, dtype=torch.int32, device="cuda:0")
+    tok, lp, lse, done = cd.step(dfa, x, st_d)
+    torch.cuda.synchronize()
+    check = sorted(set(int(i) for i in np.linspace(0, cfg.B - 1, 64).astype(int)))
+    # the noise is keyed by the ORIGINAL row id = logits row, so the host copy keeps the row positions:
+    # an uninitialised [B, V] host array in which only the checked rows are filled (and read)
+    host = torch.empty((cfg.B, cfg.V), dtype=cfg.dtype)
+    for i in check:
+        host[i] = x[i].cpu()
+    o_tok, o_lp, o_lse, o_done, o_st = oracle.sample_step(aut, host, [states[i] for i in check], 1.0, seed=2026,
+                                                          step=0, row_map=check)
+    assert tok.cpu().numpy()[check].tolist() == o_tok.tolist()
+    assert st_d.cpu().numpy()[check].tolist() == o_st.tolist()
+    assert done.cpu().numpy()[check].tolist() == o_done.tolist()
+    assert close(lp.cpu().numpy()[check], o_lp) and close(lse.cpu().numpy()[check], o_lse)
