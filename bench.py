@@ -207,6 +207,37 @@ def head_section(cd, cfg, aut, dfa, device, H, iters, warmup):
     agree = float((tok_f == outb[0]).float().mean())  # bf16 rounding of the logits may flip near-ties
     ms_g = timed(lambda: torch.matmul(hid, W.t(), out=logits))
     del logits
+    # the whole decode loop on the head path: table rows/s (the bench's metric), device-resident hidden
+    # states and end to end from pinned host hidden states (H2D of every step's [B, H] inside the timed
+    # region, results read back to the host)
+    dfa.set_sampling(0.0)
+    hs_dev = [wl.make_hidden(cfg.seed, k, n, H, device=device) for k in range(cfg.max_steps)]
+    lout = None
+
+    def loop_dev():
+        nonlocal lout
+        lout = cd.head_decode_loop(dfa, hs_dev, W, H=H, out=lout)
+
+    ms_loop = timed(loop_dev)
+    row_steps_loop = int(lout["len"].sum())
+    hs_host = [h.cpu().pin_memory() for h in hs_dev]
+    hout = None
+    cd.head_decode_loop_host(dfa, hs_host, W, H=H)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    k_e2e = 3
+    for _ in range(k_e2e):
+        hout = cd.head_decode_loop_host(dfa, hs_host, W, H=H, out=hout)
+    torch.cuda.synchronize()
+    dt_e2e = (time.perf_counter() - t0) / k_e2e
+    assert torch.equal(hout["tokens"], lout["tokens"].cpu()), "host-buffer head loop disagrees with the device loop"
+    loop = {"value": n / (ms_loop * 1e-3), "unit": UNIT, "ms_per_step": ms_loop, "row_steps_per_loop": row_steps_loop,
+            "e2e": {"value": n / dt_e2e, "unit": UNIT, "ms_per_step": 1e3 * dt_e2e,
+                    "h2d_bytes_per_step": cfg.max_steps * n * H * 2,
+                    "d2h_bytes_per_step": n * (cfg.max_steps * 4 + 13), "host_memory": "pinned"},
+            "note": "one step = cd_head_decode_loop over one batch of B rows (all max_steps steps); the model forward that "
+                    "produces the hidden states is outside the path"}
+    del hs_dev, hs_host
     burst, sustained, src = measured_tensor_peak()
     flops = 2.0 * n_dense * V * H
     ach = flops / (ms_f * 1e-3) / 1e12 if n_dense else 0.0
@@ -224,6 +255,7 @@ def head_section(cd, cfg, aut, dfa, device, H, iters, warmup):
         "workload": f"{cfg.name}: one cd_head_step, n={n} rows over the live states, V={V}, H={H} bf16 "
                     f"(Gemma 3 4B head shape, PAPER.md L191), {n_dense} rows dense / {n - n_dense} gathered",
         "ms_per_step": ms_f, "row_steps_per_s": n / (ms_f * 1e-3), "gpu_launches_per_step": int(launches),
+        "decode_loop": loop,
         "unfused_ms_per_step": ms_u, "library_gemm_ms": ms_g, "speedup_vs_unfused": ms_u / ms_f,
         "token_agreement_with_unfused_bf16_logits": agree,
         "roofline": roof or {"bound": "tensor", "kernel": "cd::head_dense_kernel (tcgen05 128x256x64, masked online-softmax epilogue from TMEM)",

@@ -331,6 +331,18 @@ CD_API cd_status cd_filter_rows(const cd_dfa_t* dfa, const int32_t* final_state,
                          const int32_t* row_ids_in, int32_t N, int32_t* row_ids_out, int32_t* n_out,
                          void* cuda_stream);
 
+/*
+ * cd_head_decode_loop with HOST buffers end to end: step_hidden_host[k] are HOST arrays
+ * [B, ldh_elems] bf16 (pinned memory lets the copies overlap the kernels), W stays a DEVICE
+ * pointer (the weights live on the GPU), the five outputs are HOST arrays.  What crosses
+ * PCIe per step is B * ldh_elems * 2 bytes of hidden states instead of B * V logits.
+ */
+CD_API cd_status cd_head_decode_loop_host(const cd_dfa_t* dfa, const void* const* step_hidden_host,
+                                   int64_t ldh_elems, const void* W, int64_t ldw_elems, int32_t H, int32_t B,
+                                   int32_t max_steps, int32_t* tokens_out, int32_t* len_out,
+                                   int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out,
+                                   void* cuda_stream);
+
 /* Number of kernel launches this library has enqueued from the calling thread's
    process so far (monotone; used by bench.py to report gpu_launches). */
 CD_API int64_t cd_launch_count(void);

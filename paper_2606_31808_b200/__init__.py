@@ -20,6 +20,7 @@ from .binding import (  # noqa: F401
     filter_rows,
     join_results,
     head_decode_loop,
+    head_decode_loop_host,
     head_step,
     launch_count,
     lib,

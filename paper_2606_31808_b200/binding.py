@@ -18,7 +18,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
     "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_set_sampling", "cd_reserve", "cd_step",
-    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
+    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
     "cd_last_error",
 )
 
@@ -318,6 +318,29 @@ def decode_loop(dfa: Dfa, step_logits: Sequence[torch.Tensor], max_steps: Option
     _check(lib().cd_decode_loop(dfa._h, ptrs, C.c_int(dt), C.c_int64(ld), C.c_int32(B), C.c_int32(max_steps),
                                 _ptr(out["tokens"]), _ptr(out["len"]), _ptr(out["final_state"]),
                                 _ptr(out["sum_logprob"]), _ptr(out["done"]), _stream(dev)))
+    return out
+
+
+def head_decode_loop_host(dfa: Dfa, step_hidden_host: Sequence[torch.Tensor], W: torch.Tensor,
+                          H: Optional[int] = None, max_steps: Optional[int] = None, out=None):
+    """cd_head_decode_loop_host: HOST hidden states in (pinned memory overlaps the copies), device W,
+    HOST outputs; the host<->device copies happen inside the call."""
+    dev = dfa.device
+    max_steps = len(step_hidden_host) if max_steps is None else max_steps
+    h0 = step_hidden_host[0]
+    B, ldh = h0.shape[0], h0.stride(0)
+    H = h0.shape[1] if H is None else H
+    for h in step_hidden_host[:max_steps]:
+        if h.is_cuda or h.dim() != 2 or h.stride(1) != 1 or h.dtype != torch.bfloat16 or h.shape[0] != B or h.stride(0) != ldh:
+            raise TypeError("step_hidden_host must be host bf16 tensors sharing shape and stride")
+    if not W.is_cuda or W.dtype != torch.bfloat16 or W.stride(1) != 1 or W.shape[0] != dfa.V:
+        raise TypeError("W must be a [V, ld] bf16 CUDA tensor")
+    ptrs = (C.c_void_p * max_steps)(*[h.data_ptr() for h in step_hidden_host[:max_steps]])
+    out = _loop_outputs(B, max_steps, dev, pin=True) if out is None else out
+    _check(lib().cd_head_decode_loop_host(dfa._h, ptrs, C.c_int64(ldh), _ptr(W), C.c_int64(W.stride(0)), C.c_int32(H),
+                                          C.c_int32(B), C.c_int32(max_steps), _ptr(out["tokens"]), _ptr(out["len"]),
+                                          _ptr(out["final_state"]), _ptr(out["sum_logprob"]), _ptr(out["done"]),
+                                          _stream(dev)))
     return out
 
 

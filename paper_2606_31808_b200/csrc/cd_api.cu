@@ -1077,10 +1077,12 @@ cd_status cd_head_step(const cd_dfa_t* d, const void* hidden, int64_t ldh_elems,
                        lse_out, done_out, stream, nullptr);
 }
 
-cd_status cd_head_decode_loop(const cd_dfa_t* d, const void* const* step_hidden, int64_t ldh_elems, const void* W,
-                              int64_t ldw_elems, int32_t H, int32_t B, int32_t max_steps, int32_t* tokens_out,
-                              int32_t* len_out, int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out,
-                              void* cuda_stream) {
+// Shared by cd_head_decode_loop (DEVICE hidden states) and cd_head_decode_loop_host (HOST hidden
+// states and outputs: the H2D copy of step k+1 overlaps the kernels of step k).
+static cd_status head_loop_impl(const cd_dfa_t* d, const void* const* step_hidden, bool host, int64_t ldh_elems,
+                                const void* W, int64_t ldw_elems, int32_t H, int32_t B, int32_t max_steps,
+                                int32_t* tokens_out, int32_t* len_out, int32_t* final_state_out,
+                                float* sum_logprob_out, uint8_t* done_out, void* cuda_stream) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
     if (B < 0 || max_steps < 0) return fail(CD_ERR_ARG, "B / max_steps < 0");
     if (B == 0) return CD_OK;
@@ -1090,40 +1092,122 @@ cd_status cd_head_decode_loop(const cd_dfa_t* d, const void* const* step_hidden,
     if (d->inv_tau > 0.0f) return fail(CD_ERR_ARG, "sampling (cd_set_sampling) is not available on the LM-head path");
     cd_status st = CD_OK;
     for (int k = 0; k < max_steps; ++k) {
-        st = check_head_layout(step_hidden[k], ldh_elems, W, ldw_elems, H);
+        // host rows need no 16-byte alignment of their own: they are copied into aligned staging
+        st = check_head_layout(host ? W : step_hidden[k], ldh_elems, W, ldw_elems, H);
         if (st != CD_OK) return st;
+        if (!step_hidden[k]) return fail(CD_ERR_ARG, "step_hidden[%d] is NULL", k);
     }
     DeviceGuard guard(d->device);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     Scratch* s = nullptr;
     st = get_scratch(d, stream, B, true, &s);
     if (st != CD_OK) return st;
-    st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream);
+    int* d_tokens = tokens_out;
+    int* d_len = len_out;
+    int* d_fs = final_state_out;
+    float* d_slp = sum_logprob_out;
+    uint8_t* d_done = done_out;
+    const size_t step_bytes = (size_t)B * (size_t)ldh_elems * 2;
+    const size_t n_tok = (size_t)B * (size_t)(max_steps > 0 ? max_steps : 1);
+    if (host) {
+        if (s->stage_bytes < step_bytes) {
+            CU(cudaStreamSynchronize(stream));
+            for (int i = 0; i < 2; ++i) { cudaFree(s->stage[i]); s->stage[i] = nullptr; }
+            s->stage_bytes = 0;
+            for (int i = 0; i < 2; ++i) CU(cudaMalloc(&s->stage[i], step_bytes));
+            s->stage_bytes = step_bytes;
+        }
+        const size_t out_bytes = sizeof(int) * (n_tok + 3 * (size_t)B) + (size_t)B + 64;
+        if (s->out_bytes < out_bytes) {
+            CU(cudaStreamSynchronize(stream));
+            cudaFree(s->out_i32); s->out_i32 = nullptr; s->out_bytes = 0;
+            CU(cudaMalloc(&s->out_i32, out_bytes));
+            s->out_bytes = out_bytes;
+        }
+        if (!s->copy_stream) {
+            CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+            for (int i = 0; i < 2; ++i) {
+                CU(cudaEventCreateWithFlags(&s->ev_copied[i], cudaEventDisableTiming));
+                CU(cudaEventCreateWithFlags(&s->ev_consumed[i], cudaEventDisableTiming));
+            }
+            CU(cudaMallocHost(&s->h_pinned, sizeof(int) * 4));
+        }
+        d_tokens = s->out_i32;
+        d_len = d_tokens + n_tok;
+        d_fs = d_len + B;
+        d_slp = reinterpret_cast<float*>(d_fs + B);
+        d_done = reinterpret_cast<uint8_t*>(d_slp + B);
+    }
+    st = launch_loop_init(d, s, B, max_steps, d_tokens, d_len, d_fs, d_slp, d_done, stream);
     if (st != CD_OK) return st;
     if (!d->start_accepting && max_steps > 0) {
         st = get_head_scratch(s, B, H, stream);
         if (st != CD_OK) return st;
         st = head_weight_map(d, W, ldw_elems, H);
         if (st != CD_OK) return st;
+        if (host) {
+            CU(cudaEventRecord(s->ev_consumed[0], stream));
+            CU(cudaEventRecord(s->ev_consumed[1], stream));
+            CU(cudaStreamWaitEvent(s->copy_stream, s->ev_consumed[0], 0));
+            CU(cudaMemcpyAsync(s->stage[0], step_hidden[0], step_bytes, cudaMemcpyHostToDevice, s->copy_stream));
+            CU(cudaEventRecord(s->ev_copied[0], s->copy_stream));
+        }
         for (int k = 0; k < max_steps; ++k) {
             const int cur = k & 1, nxt = cur ^ 1;
+            const void* hid = step_hidden[k];
+            if (host) {
+                if (k + 1 < max_steps) {
+                    CU(cudaStreamWaitEvent(s->copy_stream, s->ev_consumed[nxt], 0));
+                    CU(cudaMemcpyAsync(s->stage[nxt], step_hidden[k + 1], step_bytes, cudaMemcpyHostToDevice,
+                                       s->copy_stream));
+                    CU(cudaEventRecord(s->ev_copied[nxt], s->copy_stream));
+                }
+                CU(cudaStreamWaitEvent(stream, s->ev_copied[cur], 0));
+                hid = s->stage[cur];
+            }
             LoopExtras x;
-            x.tokens = tokens_out;
-            x.len = len_out;
-            x.final_state = final_state_out;
-            x.sum_logprob = sum_logprob_out;
-            x.done = done_out;
+            x.tokens = d_tokens;
+            x.len = d_len;
+            x.final_state = d_fs;
+            x.sum_logprob = d_slp;
+            x.done = d_done;
             x.step = k;
             x.max_steps = max_steps;
             x.row_ids_out = s->row_ids[nxt];
             x.state_out = s->state[nxt];
             x.n_out = s->n_active + nxt;
-            st = launch_head(d, s, step_hidden[k], ldh_elems, W, ldw_elems, H, s->row_ids[cur], s->state[cur], B,
+            st = launch_head(d, s, hid, ldh_elems, W, ldw_elems, H, s->row_ids[cur], s->state[cur], B,
                              s->n_active + cur, s->token, s->logprob, nullptr, s->done, stream, &x);
             if (st != CD_OK) return st;
+            if (host) CU(cudaEventRecord(s->ev_consumed[cur], stream));
         }
+        if (host) CU(cudaStreamSynchronize(s->copy_stream));
+    }
+    if (host) {
+        if (max_steps > 0)
+            CU(cudaMemcpyAsync(tokens_out, d_tokens, sizeof(int) * (size_t)B * max_steps, cudaMemcpyDeviceToHost, stream));
+        CU(cudaMemcpyAsync(len_out, d_len, sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, stream));
+        CU(cudaMemcpyAsync(final_state_out, d_fs, sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, stream));
+        CU(cudaMemcpyAsync(sum_logprob_out, d_slp, sizeof(float) * (size_t)B, cudaMemcpyDeviceToHost, stream));
+        CU(cudaMemcpyAsync(done_out, d_done, (size_t)B, cudaMemcpyDeviceToHost, stream));
     }
     return check_sticky_errors(s, stream);
+}
+
+cd_status cd_head_decode_loop(const cd_dfa_t* d, const void* const* step_hidden, int64_t ldh_elems, const void* W,
+                              int64_t ldw_elems, int32_t H, int32_t B, int32_t max_steps, int32_t* tokens_out,
+                              int32_t* len_out, int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out,
+                              void* cuda_stream) {
+    return head_loop_impl(d, step_hidden, false, ldh_elems, W, ldw_elems, H, B, max_steps, tokens_out, len_out,
+                          final_state_out, sum_logprob_out, done_out, cuda_stream);
+}
+
+cd_status cd_head_decode_loop_host(const cd_dfa_t* d, const void* const* step_hidden_host, int64_t ldh_elems,
+                                   const void* W, int64_t ldw_elems, int32_t H, int32_t B, int32_t max_steps,
+                                   int32_t* tokens_out, int32_t* len_out, int32_t* final_state_out,
+                                   float* sum_logprob_out, uint8_t* done_out, void* cuda_stream) {
+    return head_loop_impl(d, step_hidden_host, true, ldh_elems, W, ldw_elems, H, B, max_steps, tokens_out, len_out,
+                          final_state_out, sum_logprob_out, done_out, cuda_stream);
 }
 
 }  // extern "C"

@@ -297,3 +297,19 @@ def test_head_decode_loop_matches_logits_loop(cd, mode):
     torch.cuda.synchronize()
     for k in ("tokens", "len", "final_state", "done"):
         assert torch.equal(a[k], b[k]), k
+
+
+def test_head_decode_loop_host_equals_device_loop(cd, mode):
+    """cd_head_decode_loop_host (pinned host hidden states in, host outputs) against the device-buffer loop."""
+    V, H, B, steps = 4096, 256, 200, 6
+    aut = wl.make_random_dfa(29, V, 30, 0.05, 0.1)
+    dfa = dev_dfa(cd, aut, mode)
+    W = wl.make_head(29, V, H, 2.0, device="cuda:0")
+    hs = [wl.make_hidden(29, k, B, H) for k in range(steps)]
+    pinned = [h.pin_memory() for h in hs]
+    a = cd.head_decode_loop_host(dfa, pinned, W, H=H)
+    b = cd.head_decode_loop(dfa, [h.to("cuda:0") for h in hs], W, H=H)
+    torch.cuda.synchronize()
+    for k in ("tokens", "len", "final_state", "done", "sum_logprob"):
+        assert torch.equal(a[k], b[k].cpu()), k
+    assert not a["tokens"].is_cuda and int(a["len"].max()) > 1
