@@ -583,9 +583,9 @@ def main():
                 t = torch.tensor([dt], device=device)
                 dist.all_reduce(t, op=dist.ReduceOp.MAX)
                 dt = float(t[0])
-            # the host loop copies step k+1 while step k runs and stops once nothing is active
-            steps_copied = min(cfg.max_steps, int(out_h["len"].max()) + 1)
-            h2d = steps_copied * cfg.B * cfg.V * (2 if cfg.dtype == torch.bfloat16 else 4)
+            # the host loop copies only the rows still active at each step: one logits row per row-step
+            steps_copied = int(out_h["len"].max())
+            h2d = int(out_h["len"].sum()) * cfg.V * (2 if cfg.dtype == torch.bfloat16 else 4)
             d2h = cfg.B * (cfg.max_steps * 4 + 4 + 4 + 4 + 1) + 4 * steps_copied
             e2e = {"value": cfg.B * k_e2e * world / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
                    "d2h_bytes_per_step": d2h, "steps": k_e2e, "ms_per_step": 1e3 * dt / k_e2e,

@@ -239,10 +239,12 @@ CD_API cd_status cd_decode_loop_limit(const cd_dfa_t* dfa, const void* const* st
 
 /*
  * Same loop with HOST buffers end to end: step_logits_host[k] are HOST arrays
- * (pinned memory lets the copies overlap the kernels), the five outputs are
- * HOST arrays.  Host-to-device copies of step k+1 overlap the kernels of step
- * k through device staging buffers kept in the (handle, stream) scratch area;
- * copying stops as soon as no row is active.
+ * (pinned memory gives full PCIe rate), the five outputs are HOST arrays.  Early
+ * exit reaches the PCIe link: before step k the host reads the compacted active
+ * list and copies only the rows still active (runs of consecutive rows as one
+ * copy) into a compact device staging buffer kept in the (handle, stream) scratch
+ * area, so a loop moves (row-steps * ld_elems * sizeof) bytes instead of
+ * (steps * B * ld_elems * sizeof); copying stops as soon as no row is active.
  */
 CD_API cd_status cd_decode_loop_host(const cd_dfa_t* dfa, const void* const* step_logits_host,
                               cd_dtype dtype, int64_t ld_elems, int32_t B, int32_t max_steps,

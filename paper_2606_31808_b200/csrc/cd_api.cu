@@ -95,6 +95,8 @@ struct Scratch {
     cudaEvent_t ev_copied[2] = {nullptr, nullptr};
     cudaEvent_t ev_consumed[2] = {nullptr, nullptr};
     int* h_pinned = nullptr;  // [4] pinned host ints
+    int* h_ids = nullptr;     // [h_ids_cap] pinned host copy of the active row ids (host-buffer loop)
+    int h_ids_cap = 0;
     // LM-head step (cd_head.cuh)
     int head_rows = 0, head_H = 0;
     uint8_t* h_flags = nullptr;   // [2 * rows]
@@ -116,6 +118,7 @@ struct Scratch {
             if (ev_consumed[i]) cudaEventDestroy(ev_consumed[i]);
         }
         if (h_pinned) cudaFreeHost(h_pinned);
+        if (h_ids) cudaFreeHost(h_ids);
         *this = Scratch();
     }
 };
@@ -235,6 +238,7 @@ cd_status get_scratch(const cd_dfa* cd_, cudaStream_t stream, int rows, bool loo
         old.stage[0] = old.stage[1] = nullptr; old.out_i32 = nullptr; old.copy_stream = nullptr;
         old.ev_copied[0] = old.ev_copied[1] = old.ev_consumed[0] = old.ev_consumed[1] = nullptr;
         old.h_pinned = nullptr;
+        old.h_ids = nullptr;
         old.h_flags = nullptr; old.h_lists = nullptr; old.h_ctr = nullptr; old.h_A = nullptr; old.h_partials = nullptr;
         old.release();
     }
@@ -308,6 +312,7 @@ struct LoopExtras {
     const uint8_t* satisfying = nullptr;
     int* sat_ctr = nullptr;
     int limit = 0;
+    int logits_by_slot = 0;
 };
 
 // n_upper bounds the active count; n_dev (device int) overrides n inside the kernel.
@@ -330,6 +335,7 @@ cd_status launch_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype 
         a.satisfying = x->satisfying;
         a.sat_ctr = x->sat_ctr;
         a.limit = x->limit;
+        a.logits_by_slot = x->logits_by_slot;
     }
     a.dfa = d->dev;
     a.logits = static_cast<const unsigned char*>(logits);
@@ -497,9 +503,10 @@ cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, in
 cd_status enqueue_loop_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype dtype, long long ld, int B,
                             int k, int max_steps, int* tokens_out, int* len_out, int* final_state_out,
                             float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream,
-                            const LimitArgs& lim = LimitArgs()) {
+                            const LimitArgs& lim = LimitArgs(), int logits_by_slot = 0) {
     const int cur = k & 1, nxt = cur ^ 1;
     LoopExtras x;
+    x.logits_by_slot = logits_by_slot;
     if (lim.sat_ctr) {
         x.satisfying = static_cast<const uint8_t*>(d->d_satisfying);
         x.sat_ctr = lim.sat_ctr;
@@ -816,29 +823,43 @@ cd_status cd_decode_loop_host(const cd_dfa_t* d, const void* const* step_logits_
     st = launch_loop_init(d, s, B, max_steps, d_tokens, d_len, d_fs, d_slp, d_done, stream);
     if (st != CD_OK) return st;
     if (!d->start_accepting && max_steps > 0) {
-        // copy of step k+1 (copy stream) overlaps the kernels of step k (compute stream)
-        CU(cudaEventRecord(s->ev_consumed[0], stream));  // staging free from here on
-        CU(cudaEventRecord(s->ev_consumed[1], stream));
-        CU(cudaStreamWaitEvent(s->copy_stream, s->ev_consumed[0], 0));
-        CU(cudaMemcpyAsync(s->stage[0], step_logits_host[0], step_bytes, cudaMemcpyHostToDevice, s->copy_stream));
-        CU(cudaEventRecord(s->ev_copied[0], s->copy_stream));
+        // Early exit reaches the PCIe link too: only the rows still active are copied.  After step
+        // k - 1 the host reads the compacted active list (n and the original row ids), copies those
+        // rows of step k's logits into a compact staging buffer (runs of consecutive ids as one copy)
+        // and launches the step with logits row = slot.  Kernel time is ~1 % of the copy time, so
+        // nothing is lost by not overlapping the two.
+        if (s->h_ids_cap < B) {
+            if (s->h_ids) cudaFreeHost(s->h_ids);
+            s->h_ids = nullptr;
+            s->h_ids_cap = 0;
+            CU(cudaMallocHost(&s->h_ids, sizeof(int) * (size_t)B));
+            s->h_ids_cap = B;
+        }
+        const size_t row_bytes = (size_t)ld_elems * (size_t)sz;
+        int n_h = B;
+        for (int i = 0; i < B; ++i) s->h_ids[i] = i;
         for (int k = 0; k < max_steps; ++k) {
             const int cur = k & 1, nxt = cur ^ 1;
-            if (k + 1 < max_steps) {
-                CU(cudaStreamWaitEvent(s->copy_stream, s->ev_consumed[nxt], 0));
-                CU(cudaMemcpyAsync(s->stage[nxt], step_logits_host[k + 1], step_bytes, cudaMemcpyHostToDevice,
-                                   s->copy_stream));
-                CU(cudaEventRecord(s->ev_copied[nxt], s->copy_stream));
+            if (k > 0) {
+                CU(cudaMemcpyAsync(s->h_pinned, s->n_active + cur, sizeof(int), cudaMemcpyDeviceToHost, stream));
+                CU(cudaMemcpyAsync(s->h_ids, s->row_ids[cur], sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, stream));
+                CU(cudaStreamSynchronize(stream));
+                n_h = s->h_pinned[0];
             }
-            CU(cudaStreamWaitEvent(stream, s->ev_copied[cur], 0));
-            st = enqueue_loop_step(d, s, s->stage[cur], dtype, ld_elems, B, k, max_steps, d_tokens, d_len, d_fs, d_slp,
-                                   d_done, stream);
+            if (n_h <= 0) break;
+            const unsigned char* src = static_cast<const unsigned char*>(step_logits_host[k]);
+            unsigned char* dst = static_cast<unsigned char*>(s->stage[0]);
+            for (int i = 0; i < n_h;) {
+                int e = i + 1;
+                while (e < n_h && s->h_ids[e] == s->h_ids[e - 1] + 1) ++e;
+                CU(cudaMemcpyAsync(dst + (size_t)i * row_bytes, src + (size_t)s->h_ids[i] * row_bytes,
+                                   (size_t)(e - i) * row_bytes, cudaMemcpyHostToDevice, stream));
+                i = e;
+            }
+            st = enqueue_loop_step(d, s, s->stage[0], dtype, ld_elems, B, k, max_steps, d_tokens, d_len, d_fs, d_slp,
+                                   d_done, stream, LimitArgs(), 1);
             if (st != CD_OK) return st;
-            CU(cudaEventRecord(s->ev_consumed[cur], stream));
-            // early exit of the host loop: stop copying once nothing is active
-            CU(cudaMemcpyAsync(s->h_pinned, s->n_active + nxt, sizeof(int), cudaMemcpyDeviceToHost, stream));
-            CU(cudaStreamSynchronize(stream));
-            if (s->h_pinned[0] == 0) break;
+            (void)nxt;
         }
         CU(cudaStreamSynchronize(s->copy_stream));
     }

@@ -105,6 +105,9 @@ struct StepArgs {
     float inv_tau;
     uint32_t seed_lo, seed_hi;
     int rng_step_base;
+    // host-buffer loop: the logits buffer holds the ACTIVE rows only, row = slot (row_map still names
+    // the original row for the history and the sampling noise)
+    int logits_by_slot;
 };
 
 struct __align__(16) TileMeta {
@@ -287,7 +290,8 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
             // unit drawn after its row was finalised still sees the state the row was processed in
             iss_st = a.state[iss_slot];
             const long long r = a.row_map ? (long long)__ldg(a.row_map + iss_slot) : (long long)iss_slot;
-            iss_row = (int)r;
+            const long long rl = a.logits_by_slot ? (long long)iss_slot : r;  // row of the logits buffer
+            iss_row = (int)rl;
             const bool bad = (iss_st < 0) || (iss_st >= a.dfa.S);
             const int sts = bad ? 0 : iss_st;
             const bool acc = !bad && (__ldg(a.dfa.accepting + sts) != 0);
@@ -307,7 +311,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
             if (GATHER && iss_len <= a.gather_max) {
                 if (part >= gather_parts(iss_len, PG)) continue;
                 if (lane == 0) {
-                    ring.meta[iss_stage] = TileMeta{iss_slot, (int)r, FLAG_GATHER | FLAG_LAST | (part << 8), iss_st,
+                    ring.meta[iss_stage] = TileMeta{iss_slot, (int)rl, FLAG_GATHER | FLAG_LAST | (part << 8), iss_st,
                                                     iss_lo, iss_len, 0};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
@@ -318,7 +322,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
             }
             iss_tile = part * tpu;
             iss_end = min(iss_tile + tpu, tiles_per_row);
-            iss_src = a.logits + r * a.ld_bytes + (long long)iss_tile * TILE_BYTES;
+            iss_src = a.logits + rl * a.ld_bytes + (long long)iss_tile * TILE_BYTES;
             iss_msk = reinterpret_cast<const unsigned char*>(a.dfa.mask + (long long)iss_st * a.dfa.Wpad) +
                       (long long)iss_tile * MASK_BYTES;
             iss_flags = (part << 8) | FLAG_FIRST;
@@ -404,7 +408,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 s = 0.0f;
                 kb = -INFINITY;
                 idx = 0x7FFFFFFF;
-                const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, (uint32_t)mt.tile, (uint32_t)rng_step) : 0u;
+                const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, (uint32_t)(a.row_map ? __ldg(a.row_map + mt.slot) : mt.slot), (uint32_t)rng_step) : 0u;
                 const int j0 = (int)(((long long)mt.csr_len * part) / np);
                 const int j1 = (int)(((long long)mt.csr_len * (part + 1)) / np);
                 const int* tk = a.dfa.tok + mt.csr_lo;
@@ -452,7 +456,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 kb = -INFINITY;
                 idx = 0x7FFFFFFF;
             }
-            const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, (uint32_t)mt.pad, (uint32_t)rng_step) : 0u;
+            const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, (uint32_t)(a.row_map ? __ldg(a.row_map + mt.slot) : mt.slot), (uint32_t)rng_step) : 0u;
             const int t0 = mt.tile * TILE_TOK;
             const uint32_t* mw = reinterpret_cast<const uint32_t*>(ring.mask[cons_stage]);
             const unsigned char* tile = ring.logits[cons_stage];
