@@ -198,8 +198,9 @@ long long step_units_cap(const cd_dfa* d, long long n) {
     const int T = tiles_per_row(d->dev.V, CD_F32);  // fp32 rows have the most tiles
     const int tpu_max = cd::TPU_MAX_BYTES / c.tile_bytes;
     const long long warps = (long long)d->num_sms * c.warps;
-    const long long a = warps * cd::UNITS_PER_WARP + n;
-    const long long b = n * ((T + tpu_max - 1) / tpu_max + 1);
+    const long long a = warps * 32 + n;  // up to 32 units per warp (CD_UPW)
+    const long long b = n * (long long)(T + 1);  // any tiles-per-unit clamp >= 1 (CD_TPU_MAX)
+    (void)tpu_max;
     // small grids (few rows) use fewer warps, hence fewer units: still below a
     return (a > b ? a : b) + 64;
 }
@@ -354,6 +355,10 @@ cd_status launch_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype 
     a.ctrs = s->ctrs;
     a.gather_max = gather_max_for(d, dtype);
     a.all_gather = (d->max_deg <= a.gather_max) ? 1 : 0;
+    static const int env_upw = [] { const char* e = std::getenv("CD_UPW"); const int v = e ? std::atoi(e) : 0; return (v >= 1 && v <= 32) ? v : cd::UNITS_PER_WARP; }();
+    static const int env_tpu = [] { const char* e = std::getenv("CD_TPU_MAX"); const int v = e ? std::atoi(e) : 0; return v >= 1 ? v : (1 << 20); }();
+    a.upw = env_upw;
+    a.tpu_max = env_tpu;
     a.inv_tau = d->inv_tau;
     a.seed_lo = (uint32_t)(d->seed & 0xFFFFFFFFull);
     a.seed_hi = (uint32_t)(d->seed >> 32);

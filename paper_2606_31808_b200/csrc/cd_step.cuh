@@ -108,6 +108,7 @@ struct StepArgs {
     // host-buffer loop: the logits buffer holds the ACTIVE rows only, row = slot (row_map still names
     // the original row for the history and the sampling noise)
     int logits_by_slot;
+    int upw, tpu_max;  // unit sizing (tuning knobs CD_UPW / CD_TPU_MAX): target units per warp, most tiles per unit
 };
 
 struct __align__(16) TileMeta {
@@ -129,8 +130,9 @@ struct __align__(128) WarpRing {
 };
 
 // tiles per unit for n active rows (host mirrors this in cd_api.cu: step_units_cap)
-__host__ __device__ inline int tiles_per_unit(long long n, int tiles_per_row, long long total_warps, int tpu_max) {
-    long long t = (n * tiles_per_row + total_warps * UNITS_PER_WARP - 1) / (total_warps * UNITS_PER_WARP);
+__host__ __device__ inline int tiles_per_unit(long long n, int tiles_per_row, long long total_warps, int tpu_max,
+                                              int upw = UNITS_PER_WARP) {
+    long long t = (n * tiles_per_row + total_warps * upw - 1) / (total_warps * upw);
     if (t < 1) t = 1;
     if (t > tpu_max) t = tpu_max;
     return (int)t;
@@ -257,7 +259,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     const int n = a.n_dev ? __ldcg(a.n_dev) : a.n;
     const int V = a.dfa.V;
     const int tiles_per_row = (V + TILE_TOK - 1) / TILE_TOK;
-    const int tpu = tiles_per_unit(n, tiles_per_row, total_warps, TPU_MAX);
+    const int tpu = tiles_per_unit(n, tiles_per_row, total_warps, min(TPU_MAX, a.tpu_max), a.upw);
     const int Pd = (tiles_per_row + tpu - 1) / tpu;  // units per row of a dense scan
     // a gathered row is split only as far as needed to give every warp a few units
     const int PG = GATHER ? max(1, min(Pd, (total_warps * UNITS_PER_WARP) / max(n, 1))) : Pd;
