@@ -489,6 +489,11 @@ def main():
         for k, (mm, bb, rr) in enumerate(zip(step_ms, step_bytes, step_rows)):
             print(f"  step {k:2d}: n={rr:5d} distinct_states={distinct_k[k]:5d} {1e3 * mm:8.1f} us "
                   f"{bb / (mm * 1e-3) / 1e9:7.0f} GB/s", file=sys.stderr)
+    # pure-read ceiling of the kernel's own copy machinery on this GPU, measured live on one step's logits
+    try:
+        read_probe = cd.probe_read(logits[0], iters=10)
+    except Exception:
+        read_probe = None
     tot_bytes, tot_ms = sum(step_bytes), sum(step_ms)
     achieved = tot_bytes / (tot_ms * 1e-3) / 1e9
     best = max(bb / (mm * 1e-3) / 1e9 for bb, mm in zip(step_bytes, step_ms))
@@ -497,6 +502,7 @@ def main():
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
         "best_launch_gbs": best, "launches_timed": len(step_ms),
+        "read_probe_gbs": read_probe, "frac_of_read_probe": (achieved / read_probe) if read_probe else None,
         "bytes_per_launch_avg": tot_bytes / max(1, len(step_ms)), "us_per_launch_avg": 1e3 * tot_ms / max(1, len(step_ms)),
         "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(cfg.name),
         "step_kernel_share_of_loop": (tot_ms / (ms / args.steps)),

@@ -345,6 +345,17 @@ CD_API cd_status cd_head_decode_loop_host(const cd_dfa_t* dfa, const void* const
                                    int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out,
                                    void* cuda_stream);
 
+/*
+ * Measurement aid for the roofline: streams `bytes` (>= 8192, rounded down to
+ * 8 KiB tiles) of the DEVICE buffer `buf` (16-byte aligned) through the copy machinery of the
+ * step kernel -- per-warp rings of 1-D bulk async copies, 12 warps x 2 stages x 8 KiB per SM --
+ * with no arithmetic, `iters` times after 2 warm-up launches, and writes the average duration
+ * of one pass in milliseconds to *ms_out (HOST float).  bytes / time is what a pure-read
+ * kernel of this shape reaches on this GPU; bench.py reports it beside the measured copy
+ * peak.  Synchronises the stream.
+ */
+CD_API cd_status cd_probe_read(const void* buf, int64_t bytes, int32_t iters, float* ms_out, void* cuda_stream);
+
 /* Number of kernel launches this library has enqueued from the calling thread's
    process so far (monotone; used by bench.py to report gpu_launches). */
 CD_API int64_t cd_launch_count(void);

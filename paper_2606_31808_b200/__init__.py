@@ -23,6 +23,7 @@ from .binding import (  # noqa: F401
     head_decode_loop_host,
     head_step,
     launch_count,
+    probe_read,
     lib,
     lib_path,
     step,

@@ -18,7 +18,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
     "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_set_sampling", "cd_reserve", "cd_step",
-    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
+    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_probe_read", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
     "cd_last_error",
 )
 
@@ -437,3 +437,14 @@ def filter_rows(dfa: Dfa, final_state: torch.Tensor, done: torch.Tensor, row_ids
     _check(lib().cd_filter_rows(dfa._h, _ptr(final_state), _ptr(done), _ptr(row_ids), C.c_int32(N), _ptr(ro), _ptr(no),
                                 _stream(dev)))
     return ro, no
+
+
+def probe_read(buf: torch.Tensor, iters: int = 10) -> float:
+    """cd_probe_read: GB/s of a pure-read pass over `buf` with the step kernel's copy machinery."""
+    if not buf.is_cuda or not buf.is_contiguous():
+        raise TypeError("buf must be a contiguous CUDA tensor")
+    nbytes = buf.numel() * buf.element_size()
+    ms = C.c_float(0.0)
+    with torch.cuda.device(buf.device):
+        _check(lib().cd_probe_read(_ptr(buf), C.c_int64(nbytes), C.c_int32(iters), C.byref(ms), _stream(buf.device)))
+    return (nbytes // 8192 * 8192) / (ms.value * 1e-3) / 1e9

@@ -1261,6 +1261,39 @@ cd_status device_of(const void* p, int* dev) {
 
 extern "C" {
 
+cd_status cd_probe_read(const void* buf, int64_t bytes, int32_t iters, float* ms_out, void* cuda_stream) {
+    if (!buf || bytes < 8192 || iters < 1 || !ms_out) return fail(CD_ERR_ARG, "bad argument");
+    if ((reinterpret_cast<uintptr_t>(buf) & 15) != 0) return fail(CD_ERR_ARG, "buffer is not 16-byte aligned");
+    int dev = 0;
+    cd_status st = device_of(buf, &dev);
+    if (st != CD_OK) return st;
+    DeviceGuard guard(dev);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    constexpr int W = 12, S = 2, T = 8192;
+    auto kern = cd::read_probe_kernel<W, S, T>;
+    const size_t smem = (size_t)W * S * T;
+    CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    cudaDeviceProp prop;
+    CU(cudaGetDeviceProperties(&prop, dev));
+    const unsigned long long ntiles = (unsigned long long)bytes / T;
+    cudaEvent_t e0, e1;
+    CU(cudaEventCreate(&e0));
+    CU(cudaEventCreate(&e1));
+    for (int i = 0; i < 2; ++i) kern<<<prop.multiProcessorCount, W * 32, smem, stream>>>(static_cast<const unsigned char*>(buf), ntiles, nullptr);
+    CU(cudaEventRecord(e0, stream));
+    for (int i = 0; i < iters; ++i) kern<<<prop.multiProcessorCount, W * 32, smem, stream>>>(static_cast<const unsigned char*>(buf), ntiles, nullptr);
+    CU(cudaEventRecord(e1, stream));
+    CU(cudaEventSynchronize(e1));
+    CU(cudaGetLastError());
+    float ms = 0.0f;
+    CU(cudaEventElapsedTime(&ms, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    g_launches.fetch_add(iters + 2, std::memory_order_relaxed);
+    *ms_out = ms / iters;
+    return CD_OK;
+}
+
 cd_status cd_dedup(const int64_t* keys, int32_t N, int32_t* rep_out, int32_t* distinct_rows_out,
                    int32_t* n_distinct_out, void* cuda_stream) {
     if (N < 0) return fail(CD_ERR_ARG, "N < 0");

@@ -77,4 +77,49 @@ __global__ void loop_init_kernel(int B, int max_steps, int start, int start_acce
     if (tid == 0) *n_active = (start_accepting || (sat_ctr && *sat_ctr >= limit)) ? 0 : B;
 }
 
+// Measurement aid (cd_probe_read): the copy machinery of the step kernel -- per-warp rings of 1-D bulk
+// async copies on mbarriers, 12 warps x 2 stages x 8 KiB per SM -- streaming a buffer with NO arithmetic
+// (one word per tile is read so the copy is not dead).  What it reaches is the ceiling of a pure-read
+// kernel of this shape on this GPU.
+template <int WARPS, int STAGES, int TILE>
+__global__ void __launch_bounds__(WARPS * 32, 1) read_probe_kernel(const unsigned char* __restrict__ p,
+                                                                   unsigned long long ntiles, unsigned* sink) {
+    extern __shared__ __align__(128) unsigned char probe_smem[];
+    __shared__ __align__(8) unsigned long long bars[WARPS * STAGES];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    unsigned char* ring = probe_smem + (size_t)warp * STAGES * TILE;
+    unsigned long long* bar = bars + warp * STAGES;
+    if (lane == 0) {
+        for (int s = 0; s < STAGES; ++s) mbar_init(smem_u32(&bar[s]), 1);
+        fence_mbar_init();
+    }
+    __syncwarp();
+    const unsigned long long tw = (unsigned long long)gridDim.x * WARPS;
+    unsigned long long next = (unsigned long long)blockIdx.x * WARPS + warp;
+    int in_flight = 0, st_i = 0, st_c = 0;
+    uint32_t phase = 0;
+    unsigned acc = 0;
+    auto issue = [&]() {
+        if (next >= ntiles) return;
+        if (lane == 0) {
+            mbar_arrive_expect_tx(smem_u32(&bar[st_i]), TILE);
+            bulk_g2s(smem_u32(ring + st_i * TILE), p + next * TILE, TILE, smem_u32(&bar[st_i]));
+        }
+        next += tw;
+        ++in_flight;
+        st_i = (st_i + 1 == STAGES) ? 0 : st_i + 1;
+    };
+    for (int s = 0; s < STAGES; ++s) issue();
+    while (in_flight > 0) {
+        mbar_wait(smem_u32(&bar[st_c]), phase);
+        acc ^= reinterpret_cast<const unsigned*>(ring + st_c * TILE)[lane];
+        --in_flight;
+        st_c = (st_c + 1 == STAGES) ? 0 : st_c + 1;
+        phase ^= (st_c == 0) ? 1u : 0u;
+        __syncwarp();
+        issue();
+    }
+    if (acc == 0x9E3779B9u && sink) *sink = acc;  // practically never: keeps the loads alive
+}
+
 }  // namespace cd
