@@ -356,6 +356,33 @@ CD_API cd_status cd_head_decode_loop_host(const cd_dfa_t* dfa, const void* const
  */
 CD_API cd_status cd_probe_read(const void* buf, int64_t bytes, int32_t iters, float* ms_out, void* cuda_stream);
 
+/*
+ * Callback forms of the loops ("how a real LM forward would plug in").  Before
+ * decoding step k the library calls, on the calling host thread,
+ *     next_logits(user, k, d_row_ids, d_n_active, n_upper, &logits, &ld_elems, &by_slot)
+ * with DEVICE pointers to the current active list (original row ids of the active slots,
+ * ascending; *d_n_active of them, at most n_upper = B) -- valid for work enqueued on
+ * cuda_stream.  The callback enqueues whatever produces step k's logits (the model forward
+ * over the active rows) on the same stream, without synchronising, and returns the DEVICE
+ * buffer: *by_slot != 0 means row i of the buffer belongs to active slot i (a compact batch,
+ * what a forward over the active rows yields), 0 means rows are indexed by original row id.
+ * A non-zero return value aborts the loop with CD_ERR_ARG.  The buffer must stay valid
+ * until the loop returns.  Everything else as cd_decode_loop / cd_head_decode_loop (for the
+ * head form the callback returns hidden states [., ldh_elems] bf16).
+ */
+typedef int (*cd_next_logits_fn)(void* user, int32_t step, const int32_t* d_row_ids, const int32_t* d_n_active,
+                                 int32_t n_upper, const void** logits_out, int64_t* ld_elems_out,
+                                 int32_t* by_slot_out);
+typedef cd_next_logits_fn cd_next_hidden_fn;
+CD_API cd_status cd_decode_loop_cb(const cd_dfa_t* dfa, cd_next_logits_fn next_logits, void* user, cd_dtype dtype,
+                            int32_t B, int32_t max_steps, int32_t* tokens_out, int32_t* len_out,
+                            int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out,
+                            void* cuda_stream);
+CD_API cd_status cd_head_decode_loop_cb(const cd_dfa_t* dfa, cd_next_hidden_fn next_hidden, void* user, const void* W,
+                                 int64_t ldw_elems, int32_t H, int32_t B, int32_t max_steps,
+                                 int32_t* tokens_out, int32_t* len_out, int32_t* final_state_out,
+                                 float* sum_logprob_out, uint8_t* done_out, void* cuda_stream);
+
 /* Number of kernel launches this library has enqueued from the calling thread's
    process so far (monotone; used by bench.py to report gpu_launches). */
 CD_API int64_t cd_launch_count(void);

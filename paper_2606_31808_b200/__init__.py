@@ -15,6 +15,8 @@ from .binding import (  # noqa: F401
     compile_dfa,
     compile_trie,
     decode_loop,
+    decode_loop_cb,
+    head_decode_loop_cb,
     decode_loop_host,
     dedup,
     filter_rows,

@@ -18,7 +18,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
     "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_set_sampling", "cd_reserve", "cd_step",
-    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_probe_read", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
+    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_probe_read", "cd_decode_loop_cb", "cd_head_decode_loop_cb", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
     "cd_last_error",
 )
 
@@ -448,3 +448,64 @@ def probe_read(buf: torch.Tensor, iters: int = 10) -> float:
     with torch.cuda.device(buf.device):
         _check(lib().cd_probe_read(_ptr(buf), C.c_int64(nbytes), C.c_int32(iters), C.byref(ms), _stream(buf.device)))
     return (nbytes // 8192 * 8192) / (ms.value * 1e-3) / 1e9
+
+
+_NEXT_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_void_p),
+                       C.POINTER(C.c_int64), C.POINTER(C.c_int32))
+
+
+def _wrap_next(fn, dev, B, keep):
+    """fn(step, row_ids i32[B] device view, n_active i32[1] device view) -> (tensor [rows, ld], by_slot)."""
+    def thunk(user, step, d_ids, d_n, n_upper, out_ptr, out_ld, out_by_slot):
+        try:
+            ids = _view_i32(d_ids, n_upper, dev)
+            n = _view_i32(d_n, 1, dev)
+            t, by_slot = fn(int(step), ids, n)
+            if t.dim() != 2 or not t.is_cuda or t.stride(1) != 1:
+                return 2
+            keep.append(t)  # the buffer must outlive the loop
+            out_ptr[0] = t.data_ptr()
+            out_ld[0] = t.stride(0)
+            out_by_slot[0] = 1 if by_slot else 0
+            return 0
+        except Exception:  # never raise through the C ABI
+            import traceback
+            traceback.print_exc()
+            return 1
+    return _NEXT_FN(thunk)
+
+
+def _view_i32(ptr: int, n: int, dev) -> torch.Tensor:
+    """Zero-copy int32 view of device memory owned by the library (valid during the callback's loop)."""
+    class _Holder:
+        pass
+    h = _Holder()
+    h.__cuda_array_interface__ = {"shape": (n,), "typestr": "<i4", "data": (int(ptr), False), "version": 3}
+    return torch.as_tensor(h, device=dev)
+
+
+def decode_loop_cb(dfa: Dfa, next_logits, dtype: torch.dtype, B: int, max_steps: int, out=None):
+    """cd_decode_loop_cb: next_logits(step, row_ids, n_active) -> (logits tensor, by_slot) is called before
+    every step and must only enqueue work on torch's current stream."""
+    dev = dfa.device
+    keep: List[torch.Tensor] = []
+    cb = _wrap_next(next_logits, dev, B, keep)
+    out = _loop_outputs(B, max_steps, dev) if out is None else out
+    dt = BF16 if dtype == torch.bfloat16 else F32
+    _check(lib().cd_decode_loop_cb(dfa._h, cb, C.c_void_p(None), C.c_int(dt), C.c_int32(B), C.c_int32(max_steps),
+                                   _ptr(out["tokens"]), _ptr(out["len"]), _ptr(out["final_state"]),
+                                   _ptr(out["sum_logprob"]), _ptr(out["done"]), _stream(dev)))
+    return out
+
+
+def head_decode_loop_cb(dfa: Dfa, next_hidden, W: torch.Tensor, H: int, B: int, max_steps: int, out=None):
+    """cd_head_decode_loop_cb: next_hidden(step, row_ids, n_active) -> (hidden bf16 tensor, by_slot)."""
+    dev = dfa.device
+    keep: List[torch.Tensor] = []
+    cb = _wrap_next(next_hidden, dev, B, keep)
+    out = _loop_outputs(B, max_steps, dev) if out is None else out
+    _check(lib().cd_head_decode_loop_cb(dfa._h, cb, C.c_void_p(None), _ptr(W), C.c_int64(W.stride(0)), C.c_int32(H),
+                                        C.c_int32(B), C.c_int32(max_steps), _ptr(out["tokens"]), _ptr(out["len"]),
+                                        _ptr(out["final_state"]), _ptr(out["sum_logprob"]), _ptr(out["done"]),
+                                        _stream(dev)))
+    return out

@@ -989,6 +989,7 @@ cd_status launch_head(const cd_dfa* d, Scratch* s, const void* hidden, long long
         a.fin.cmp_row_ids_out = x->row_ids_out;
         a.fin.cmp_state_out = x->state_out;
         a.fin.cmp_n_out = x->n_out;
+        a.fin.logits_by_slot = x->logits_by_slot;  // here: hidden rows indexed by slot
     }
     a.fin.dfa = d->dev;
     a.fin.row_map = row_map;
@@ -1382,6 +1383,100 @@ cd_status cd_filter_rows(const cd_dfa_t* d, const int32_t* final_state, const ui
     g_launches.fetch_add(2, std::memory_order_relaxed);
     CU(cudaFreeAsync(drop, stream));
     return CD_OK;
+}
+
+}  // extern "C"
+
+// =============================================================================== callback loops
+extern "C" {
+
+cd_status cd_decode_loop_cb(const cd_dfa_t* d, cd_next_logits_fn next_logits, void* user, cd_dtype dtype, int32_t B,
+                            int32_t max_steps, int32_t* tokens_out, int32_t* len_out, int32_t* final_state_out,
+                            float* sum_logprob_out, uint8_t* done_out, void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (!next_logits) return fail(CD_ERR_ARG, "next_logits is NULL");
+    if (B < 0 || max_steps < 0) return fail(CD_ERR_ARG, "B / max_steps < 0");
+    cd_status st = check_dtype(dtype);
+    if (st != CD_OK) return st;
+    if (B == 0) return CD_OK;
+    if (!len_out || !final_state_out || !sum_logprob_out || !done_out || (max_steps > 0 && !tokens_out))
+        return fail(CD_ERR_ARG, "NULL output pointer");
+    DeviceGuard guard(d->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* s = nullptr;
+    st = get_scratch(d, stream, B, true, &s);
+    if (st != CD_OK) return st;
+    st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream);
+    if (st != CD_OK) return st;
+    if (!d->start_accepting)
+        for (int k = 0; k < max_steps; ++k) {
+            const int cur = k & 1;
+            const void* logits = nullptr;
+            int64_t ld = 0;
+            int32_t by_slot = 0;
+            const int rc = next_logits(user, k, s->row_ids[cur], s->n_active + cur, B, &logits, &ld, &by_slot);
+            if (rc != 0) return fail(CD_ERR_ARG, "next_logits returned %d at step %d", rc, k);
+            st = check_logits_layout(d, logits, dtype, ld);
+            if (st != CD_OK) return st;
+            st = enqueue_loop_step(d, s, logits, dtype, ld, B, k, max_steps, tokens_out, len_out, final_state_out,
+                                   sum_logprob_out, done_out, stream, LimitArgs(), by_slot ? 1 : 0);
+            if (st != CD_OK) return st;
+        }
+    return check_sticky_errors(s, stream);
+}
+
+cd_status cd_head_decode_loop_cb(const cd_dfa_t* d, cd_next_hidden_fn next_hidden, void* user, const void* W,
+                                 int64_t ldw_elems, int32_t H, int32_t B, int32_t max_steps, int32_t* tokens_out,
+                                 int32_t* len_out, int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out,
+                                 void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (!next_hidden) return fail(CD_ERR_ARG, "next_hidden is NULL");
+    if (B < 0 || max_steps < 0) return fail(CD_ERR_ARG, "B / max_steps < 0");
+    if (B == 0) return CD_OK;
+    if (!len_out || !final_state_out || !sum_logprob_out || !done_out || (max_steps > 0 && !tokens_out))
+        return fail(CD_ERR_ARG, "NULL output pointer");
+    if (d->inv_tau > 0.0f) return fail(CD_ERR_ARG, "sampling (cd_set_sampling) is not available on the LM-head path");
+    DeviceGuard guard(d->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    Scratch* s = nullptr;
+    cd_status st = get_scratch(d, stream, B, true, &s);
+    if (st != CD_OK) return st;
+    st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream);
+    if (st != CD_OK) return st;
+    if (!d->start_accepting && max_steps > 0) {
+        st = get_head_scratch(s, B, H, stream);
+        if (st != CD_OK) return st;
+        for (int k = 0; k < max_steps; ++k) {
+            const int cur = k & 1, nxt = cur ^ 1;
+            const void* hidden = nullptr;
+            int64_t ldh = 0;
+            int32_t by_slot = 0;
+            const int rc = next_hidden(user, k, s->row_ids[cur], s->n_active + cur, B, &hidden, &ldh, &by_slot);
+            if (rc != 0) return fail(CD_ERR_ARG, "next_hidden returned %d at step %d", rc, k);
+            st = check_head_layout(hidden, ldh, W, ldw_elems, H);
+            if (st != CD_OK) return st;
+            if (k == 0) {
+                st = head_weight_map(d, W, ldw_elems, H);
+                if (st != CD_OK) return st;
+            }
+            LoopExtras x;
+            x.tokens = tokens_out;
+            x.len = len_out;
+            x.final_state = final_state_out;
+            x.sum_logprob = sum_logprob_out;
+            x.done = done_out;
+            x.step = k;
+            x.max_steps = max_steps;
+            x.row_ids_out = s->row_ids[nxt];
+            x.state_out = s->state[nxt];
+            x.n_out = s->n_active + nxt;
+            x.logits_by_slot = by_slot ? 1 : 0;
+            st = launch_head(d, s, hidden, ldh, W, ldw_elems, H, s->row_ids[cur], s->state[cur], B, s->n_active + cur,
+                             s->token, s->logprob, nullptr, s->done, stream, &x);
+            if (st != CD_OK) return st;
+        }
+    }
+    return check_sticky_errors(s, stream);
 }
 
 }  // extern "C"

@@ -202,7 +202,7 @@ __global__ void head_pack_kernel(const HeadArgs a) {
     const int nv = a.H >> 3;
     for (int d = warp; d < n_dense; d += nwarps) {
         const int slot = __ldcg(a.dense_slot + d);
-        const long long r = a.fin.row_map ? (long long)__ldg(a.fin.row_map + slot) : (long long)slot;
+        const long long r = (a.fin.row_map && !a.fin.logits_by_slot) ? (long long)__ldg(a.fin.row_map + slot) : (long long)slot;
         const uint4* src = reinterpret_cast<const uint4*>(a.hidden + r * a.ldh);
         uint4* dst = reinterpret_cast<uint4*>(a.A + (long long)d * a.ldA);
         for (int v = lane; v < nv; v += 32) dst[v] = __ldg(src + v);
@@ -235,7 +235,7 @@ __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadAr
     for (int g = blockIdx.x; g < n_gather; g += gridDim.x) {
         const int slot = __ldcg(a.gather_slot + g);
         const int st = __ldcg(a.gather_state + g);
-        const long long r = f.row_map ? (long long)__ldg(f.row_map + slot) : (long long)slot;
+        const long long r = (f.row_map && !f.logits_by_slot) ? (long long)__ldg(f.row_map + slot) : (long long)slot;
         const uint4* src = reinterpret_cast<const uint4*>(a.hidden + r * a.ldh);
         __syncthreads();  // previous row's readers are done with hid / s_*
         for (int v = threadIdx.x; v < nv; v += blockDim.x) hid[v] = __ldg(src + v);
