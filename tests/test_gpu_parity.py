@@ -578,3 +578,69 @@ def test_stepwise_api_reproduces_the_loop(cd, oracle):
         n = int(na)
     assert torch.equal(toks, out["tokens"])
     dfa.close()
+
+
+def test_two_streams_share_one_handle(cd, oracle):
+    """include/cd.h: a handle may be used from several streams at once (scratch is kept per
+    (handle, stream)).  Two loops on two streams, interleaved launches, different inputs."""
+    cfg = wl.scaled(wl.CONFIGS["c3"], V=20000, B=200, S=40, max_steps=6)
+    aut = wl.build_automaton(cfg)
+    dfa = dev_dfa(cd, aut)
+    la = wl.build_step_logits(cfg, aut, device="cuda:0", batch=0)
+    lb = wl.build_step_logits(cfg, aut, device="cuda:0", batch=1)
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    outs = {}
+    for rep in range(3):
+        with torch.cuda.stream(s1):
+            outs["a"] = cd.decode_loop(dfa, la)
+        with torch.cuda.stream(s2):
+            outs["b"] = cd.decode_loop(dfa, lb)
+    torch.cuda.synchronize()
+    for key, logits in (("a", la), ("b", lb)):
+        want = oracle.decode_loop(aut, [x.cpu() for x in logits])
+        for k in ("tokens", "len", "final_state", "done"):
+            assert np.array_equal(outs[key][k].cpu().numpy(), want[k]), (key, k)
+
+
+def test_step_and_compact_in_a_cuda_graph(cd, oracle):
+    """cd_step / cd_compact neither allocate nor synchronise after cd_reserve, so a decoding step
+    can be captured in a CUDA graph and replayed on new inputs written into the same buffers."""
+    cfg = wl.scaled(wl.CONFIGS["c3"], V=20000, B=96, S=40, max_steps=1)
+    aut = wl.build_automaton(cfg)
+    dfa = dev_dfa(cd, aut)
+    n = cfg.B
+    x = torch.empty((n, cfg.V), dtype=torch.bfloat16, device="cuda:0")
+    st = torch.empty(n, dtype=torch.int32, device="cuda:0")
+    outb = (torch.empty(n, dtype=torch.int32, device="cuda:0"), torch.empty(n, dtype=torch.float32, device="cuda:0"),
+            torch.empty(n, dtype=torch.float32, device="cuda:0"), torch.empty(n, dtype=torch.uint8, device="cuda:0"))
+    cmp_out = (torch.empty(n, dtype=torch.int32, device="cuda:0"), torch.empty(n, dtype=torch.int32, device="cuda:0"),
+               torch.empty(1, dtype=torch.int32, device="cuda:0"))
+    acc = np.asarray(aut.accepting)
+    live = [s for s in range(aut.S) if not acc[s]]
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        dfa.reserve(n)
+        st.fill_(live[0])
+        x.zero_()
+        cd.step(dfa, x, st, out=outb)  # warm-up on the capture stream: scratch + kernel attributes
+        cd.compact(outb[3], None, st, out=cmp_out)
+        side.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=side):
+            cd.step(dfa, x, st, out=outb)
+            cd.compact(outb[3], None, st, out=cmp_out)
+    torch.cuda.synchronize()
+    for rep in range(3):
+        logits = wl.make_logits(100 + rep, 0, n, cfg.V, 3.0, torch.bfloat16)
+        states = [live[(i + rep) % len(live)] for i in range(n)]
+        x.copy_(logits)
+        st.copy_(torch.tensor(states, dtype=torch.int32))
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        o_tok, o_lp, o_lse, o_done, o_st = oracle.step(aut, logits, states)
+        assert outb[0].cpu().numpy().tolist() == o_tok.tolist()
+        assert st.cpu().numpy().tolist() == o_st.tolist()
+        o_ro, o_so, k = oracle.compact(o_done, None, o_st)
+        assert int(cmp_out[2]) == k and cmp_out[0][:k].cpu().numpy().tolist() == o_ro.tolist()
