@@ -238,6 +238,15 @@ CD_API cd_status cd_decode_loop_limit(const cd_dfa_t* dfa, const void* const* st
                                void* cuda_stream);
 
 /*
+ * LIMIT early exit for every loop entry point: after cd_set_limit(dfa, limit, satisfied)
+ * (satisfied: DEVICE int32 owned by the caller, shared by the calls of one query; needs
+ * cd_set_satisfying) cd_decode_loop, cd_decode_loop_host, cd_decode_loop_cb and the
+ * cd_head_decode_loop* family all behave as cd_decode_loop_limit does.  satisfied == NULL
+ * clears it.  Call it while no work using the handle is in flight.
+ */
+CD_API cd_status cd_set_limit(cd_dfa_t* dfa, int32_t limit, int32_t* satisfied_inout);
+
+/*
  * Same loop with HOST buffers end to end: step_logits_host[k] are HOST arrays
  * (pinned memory gives full PCIe rate), the five outputs are HOST arrays.  Early
  * exit reaches the PCIe link: before step k the host reads the compacted active

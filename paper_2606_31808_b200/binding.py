@@ -18,7 +18,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
     "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_set_sampling", "cd_reserve", "cd_step",
-    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_probe_read", "cd_decode_loop_cb", "cd_head_decode_loop_cb", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
+    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_set_limit", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_probe_read", "cd_decode_loop_cb", "cd_head_decode_loop_cb", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
     "cd_last_error",
 )
 
@@ -123,6 +123,13 @@ class Dfa:
         if t.numel() != self.S:
             raise ValueError("satisfying must have S entries")
         _check(lib().cd_set_satisfying(self._h, _ptr(t)))
+
+    def set_limit(self, limit: int, satisfied: Optional[torch.Tensor]):
+        """cd_set_limit: LIMIT early exit for every loop; satisfied = device int32[1] counter (None clears)."""
+        if satisfied is not None:
+            _dev_tensor(satisfied, torch.int32, "satisfied", self.device)
+        self._limit_ctr = satisfied  # keep the counter alive
+        _check(lib().cd_set_limit(self._h, C.c_int32(limit), _ptr(satisfied)))
 
     def reserve(self, max_rows: int):
         _check(lib().cd_reserve(self._h, C.c_int32(max_rows), _stream(self.device)))

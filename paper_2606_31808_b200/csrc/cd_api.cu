@@ -140,6 +140,8 @@ struct cd_dfa {
     void* d_next = nullptr;
     void* d_acc = nullptr;
     void* d_satisfying = nullptr;  // cd_set_satisfying
+    int limit = 0;                 // cd_set_limit: LIMIT early exit applied by every loop entry point
+    int* limit_ctr = nullptr;      //   device counter of satisfied rows (caller-owned); nullptr = no limit
     float inv_tau = 0.0f;          // cd_set_sampling: 0 = greedy, else 1 / temperature
     unsigned long long seed = 0;
     int rng_step_base = 0;
@@ -487,6 +489,17 @@ struct LimitArgs {
     int limit = 0;
 };
 
+// the LIMIT a loop runs under: the explicit one (cd_decode_loop_limit), else the handle's (cd_set_limit)
+LimitArgs resolve_limit(const cd_dfa* d, const LimitArgs& explicit_lim = LimitArgs()) {
+    if (explicit_lim.sat_ctr) return explicit_lim;
+    LimitArgs l;
+    if (d->limit_ctr && d->d_satisfying) {
+        l.sat_ctr = d->limit_ctr;
+        l.limit = d->limit;
+    }
+    return l;
+}
+
 cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, int* tokens_out, int* len_out,
                            int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream,
                            const LimitArgs& lim = LimitArgs()) {
@@ -704,9 +717,10 @@ cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, const int32
 static cd_status decode_loop_impl(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
                                   int32_t B, int32_t max_steps, int32_t* tokens_out, int32_t* len_out,
                                   int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out,
-                                  const LimitArgs& lim, void* cuda_stream) {
+                                  const LimitArgs& lim_in, void* cuda_stream) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
     if (B < 0 || max_steps < 0) return fail(CD_ERR_ARG, "B / max_steps < 0");
+    const LimitArgs lim = resolve_limit(d, lim_in);
     cd_status st = check_dtype(dtype);
     if (st != CD_OK) return st;
     if (B == 0) return CD_OK;
@@ -825,7 +839,8 @@ cd_status cd_decode_loop_host(const cd_dfa_t* d, const void* const* step_logits_
     float* d_slp = reinterpret_cast<float*>(d_fs + B);
     uint8_t* d_done = reinterpret_cast<uint8_t*>(d_slp + B);
 
-    st = launch_loop_init(d, s, B, max_steps, d_tokens, d_len, d_fs, d_slp, d_done, stream);
+    const LimitArgs lim = resolve_limit(d);
+    st = launch_loop_init(d, s, B, max_steps, d_tokens, d_len, d_fs, d_slp, d_done, stream, lim);
     if (st != CD_OK) return st;
     if (!d->start_accepting && max_steps > 0) {
         // Early exit reaches the PCIe link too: only the rows still active are copied.  After step
@@ -845,7 +860,7 @@ cd_status cd_decode_loop_host(const cd_dfa_t* d, const void* const* step_logits_
         for (int i = 0; i < B; ++i) s->h_ids[i] = i;
         for (int k = 0; k < max_steps; ++k) {
             const int cur = k & 1, nxt = cur ^ 1;
-            if (k > 0) {
+            if (k > 0 || lim.sat_ctr) {  // (with a LIMIT the list may be empty from the start)
                 CU(cudaMemcpyAsync(s->h_pinned, s->n_active + cur, sizeof(int), cudaMemcpyDeviceToHost, stream));
                 CU(cudaMemcpyAsync(s->h_ids, s->row_ids[cur], sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, stream));
                 CU(cudaStreamSynchronize(stream));
@@ -862,7 +877,7 @@ cd_status cd_decode_loop_host(const cd_dfa_t* d, const void* const* step_logits_
                 i = e;
             }
             st = enqueue_loop_step(d, s, s->stage[0], dtype, ld_elems, B, k, max_steps, d_tokens, d_len, d_fs, d_slp,
-                                   d_done, stream, LimitArgs(), 1);
+                                   d_done, stream, lim, 1);
             if (st != CD_OK) return st;
             (void)nxt;
         }
@@ -990,6 +1005,9 @@ cd_status launch_head(const cd_dfa* d, Scratch* s, const void* hidden, long long
         a.fin.cmp_state_out = x->state_out;
         a.fin.cmp_n_out = x->n_out;
         a.fin.logits_by_slot = x->logits_by_slot;  // here: hidden rows indexed by slot
+        a.fin.satisfying = x->satisfying;
+        a.fin.sat_ctr = x->sat_ctr;
+        a.fin.limit = x->limit;
     }
     a.fin.dfa = d->dev;
     a.fin.row_map = row_map;
@@ -1063,6 +1081,20 @@ cd_status launch_head(const cd_dfa* d, Scratch* s, const void* hidden, long long
 }  // namespace
 
 extern "C" {
+
+cd_status cd_set_limit(cd_dfa_t* d, int32_t limit, int32_t* satisfied_inout) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (!satisfied_inout) {  // clear
+        d->limit_ctr = nullptr;
+        d->limit = 0;
+        return CD_OK;
+    }
+    if (limit < 0) return fail(CD_ERR_ARG, "limit < 0");
+    if (!d->d_satisfying) return fail(CD_ERR_ARG, "cd_set_satisfying has not been called on this automaton");
+    d->limit_ctr = satisfied_inout;
+    d->limit = limit;
+    return CD_OK;
+}
 
 cd_status cd_set_sampling(cd_dfa_t* d, float temperature, uint64_t seed, int32_t step_base) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
@@ -1165,7 +1197,8 @@ static cd_status head_loop_impl(const cd_dfa_t* d, const void* const* step_hidde
         d_slp = reinterpret_cast<float*>(d_fs + B);
         d_done = reinterpret_cast<uint8_t*>(d_slp + B);
     }
-    st = launch_loop_init(d, s, B, max_steps, d_tokens, d_len, d_fs, d_slp, d_done, stream);
+    const LimitArgs lim = resolve_limit(d);
+    st = launch_loop_init(d, s, B, max_steps, d_tokens, d_len, d_fs, d_slp, d_done, stream, lim);
     if (st != CD_OK) return st;
     if (!d->start_accepting && max_steps > 0) {
         st = get_head_scratch(s, B, H, stream);
@@ -1203,6 +1236,11 @@ static cd_status head_loop_impl(const cd_dfa_t* d, const void* const* step_hidde
             x.row_ids_out = s->row_ids[nxt];
             x.state_out = s->state[nxt];
             x.n_out = s->n_active + nxt;
+            if (lim.sat_ctr) {
+                x.satisfying = static_cast<const uint8_t*>(d->d_satisfying);
+                x.sat_ctr = lim.sat_ctr;
+                x.limit = lim.limit;
+            }
             st = launch_head(d, s, hid, ldh_elems, W, ldw_elems, H, s->row_ids[cur], s->state[cur], B,
                              s->n_active + cur, s->token, s->logprob, nullptr, s->done, stream, &x);
             if (st != CD_OK) return st;
@@ -1406,7 +1444,9 @@ cd_status cd_decode_loop_cb(const cd_dfa_t* d, cd_next_logits_fn next_logits, vo
     Scratch* s = nullptr;
     st = get_scratch(d, stream, B, true, &s);
     if (st != CD_OK) return st;
-    st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream);
+    const LimitArgs lim = resolve_limit(d);
+    st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream,
+                          lim);
     if (st != CD_OK) return st;
     if (!d->start_accepting)
         for (int k = 0; k < max_steps; ++k) {
@@ -1419,7 +1459,7 @@ cd_status cd_decode_loop_cb(const cd_dfa_t* d, cd_next_logits_fn next_logits, vo
             st = check_logits_layout(d, logits, dtype, ld);
             if (st != CD_OK) return st;
             st = enqueue_loop_step(d, s, logits, dtype, ld, B, k, max_steps, tokens_out, len_out, final_state_out,
-                                   sum_logprob_out, done_out, stream, LimitArgs(), by_slot ? 1 : 0);
+                                   sum_logprob_out, done_out, stream, lim, by_slot ? 1 : 0);
             if (st != CD_OK) return st;
         }
     return check_sticky_errors(s, stream);
@@ -1441,7 +1481,9 @@ cd_status cd_head_decode_loop_cb(const cd_dfa_t* d, cd_next_hidden_fn next_hidde
     Scratch* s = nullptr;
     cd_status st = get_scratch(d, stream, B, true, &s);
     if (st != CD_OK) return st;
-    st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream);
+    const LimitArgs lim = resolve_limit(d);
+    st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream,
+                          lim);
     if (st != CD_OK) return st;
     if (!d->start_accepting && max_steps > 0) {
         st = get_head_scratch(s, B, H, stream);
@@ -1471,6 +1513,11 @@ cd_status cd_head_decode_loop_cb(const cd_dfa_t* d, cd_next_hidden_fn next_hidde
             x.state_out = s->state[nxt];
             x.n_out = s->n_active + nxt;
             x.logits_by_slot = by_slot ? 1 : 0;
+            if (lim.sat_ctr) {
+                x.satisfying = static_cast<const uint8_t*>(d->d_satisfying);
+                x.sat_ctr = lim.sat_ctr;
+                x.limit = lim.limit;
+            }
             st = launch_head(d, s, hidden, ldh, W, ldw_elems, H, s->row_ids[cur], s->state[cur], B, s->n_active + cur,
                              s->token, s->logprob, nullptr, s->done, stream, &x);
             if (st != CD_OK) return st;

@@ -476,6 +476,8 @@ __global__ void __launch_bounds__(1024, 1) head_loop_tail_kernel(const HeadArgs 
     const StepArgs& f = a.fin;
     const int n = f.n_dev ? __ldcg(f.n_dev) : f.n;
     block_compact(f.done_out, f.row_map, f.state, n, f.cmp_row_ids_out, f.cmp_state_out, f.cmp_n_out);
+    // LIMIT early exit: enough rows satisfied -> every row still active is cancelled
+    if (f.sat_ctr && threadIdx.x == 0 && __ldcg(f.sat_ctr) >= f.limit) *f.cmp_n_out = 0;
 }
 
 }  // namespace cd

@@ -82,3 +82,58 @@ def test_callback_failure_is_reported(cd):
 
     with pytest.raises(cd.CdError):
         cd.decode_loop_cb(dfa, bad, torch.float32, 8, 3)
+
+
+def test_handle_level_limit_applies_to_every_loop(cd, oracle):
+    """cd_set_limit (LIMIT early exit) on the device loop, the host-buffer loop, the
+    callback loop and the LM-head loops, against the oracle's limited loop (O5).  Exact-arithmetic head
+    inputs make the fp32 logits of a library matmul equal to the head's dot products."""
+    V, H, B, steps = 2048, 128, 240, 8
+    aut = wl.make_random_dfa(67, V, 16, 0.1, 0.3)
+    acc = np.asarray(aut.accepting)
+    sat = ((np.arange(aut.S) % 2 == 0) & (acc != 0)).astype(np.uint8)
+    if sat.sum() == 0:
+        sat = acc.astype(np.uint8)
+    W = wl.make_head(67, V, H, 2.0, exact=True)
+    hs = [wl.make_hidden(67, k, B, H, exact=True) for k in range(steps)]
+    logits = [(h.double() @ W.double().t()).float().contiguous() for h in hs]  # exact in fp32
+    full = oracle.decode_loop(aut, logits)
+    n_sat = int(sum(1 for r in range(B) if full["done"][r] and sat[full["final_state"][r]]))
+    assert n_sat >= 4
+    limit = max(2, n_sat // 3)
+    want = oracle.decode_loop(aut, logits, satisfying=sat, limit=limit, satisfied=0)
+    assert (want["len"] < full["len"]).any()  # the limit really cancels rows
+
+    dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device="cuda:0")
+    dfa.set_satisfying(sat)
+    ctr = torch.zeros(1, dtype=torch.int32, device="cuda:0")
+    dfa.set_limit(limit, ctr)
+    ldev = [x.to("cuda:0") for x in logits]
+    hdev = [h.to("cuda:0") for h in hs]
+    Wd = W.to("cuda:0")
+
+    def check(got, name):
+        torch.cuda.synchronize()
+        for k in ("tokens", "len", "final_state", "done"):
+            assert np.array_equal(got[k].cpu().numpy(), want[k]), (name, k)
+        assert int(ctr) == want["satisfied"], name
+        ctr.zero_()
+
+    check(cd.decode_loop(dfa, ldev), "device loop")
+    check(cd.decode_loop_host(dfa, [x.pin_memory() for x in logits]), "host loop")
+    check(cd.decode_loop_cb(dfa, lambda k, ids, n: (ldev[k], False), torch.float32, B, steps), "callback loop")
+    for gmax in (0, 2**30):
+        dfa.set_head_gather_max(gmax)
+        check(cd.head_decode_loop(dfa, hdev, Wd, H=H), f"head loop gmax={gmax}")
+    check(cd.head_decode_loop_host(dfa, [h.pin_memory() for h in hs], Wd, H=H), "head host loop")
+    check(cd.head_decode_loop_cb(dfa, lambda k, ids, n: (hdev[k], False), Wd, H, B, steps), "head callback loop")
+    # a second batch of the same query starts with the counter already at the limit: nothing runs
+    ctr.fill_(limit)
+    got = cd.head_decode_loop(dfa, hdev, Wd, H=H)
+    torch.cuda.synchronize()
+    assert int(got["len"].max()) == 0 and int(got["done"].max()) == 0
+    # cleared: the unlimited result again
+    dfa.set_limit(0, None)
+    got = cd.decode_loop(dfa, ldev)
+    torch.cuda.synchronize()
+    assert np.array_equal(got["tokens"].cpu().numpy(), full["tokens"])
