@@ -138,7 +138,8 @@ CD_API cd_status cd_set_gather_max(cd_dfa_t* dfa, int32_t max_transitions);
  * logprob_out = log of the sampled token's probability under the masked softmax of y,
  * lse_out = masked logsumexp of y.  T = 0 (default) restores greedy decoding.  For
  * cd_step the decoding step is step_base; cd_decode_loop* use step_base + k.
- * Not available on the LM-head path (cd_head_* return CD_ERR_ARG while T > 0).
+ * On the LM-head path (cd_head_*) the same rule applies to the fp32-accumulated logits
+ * (bit-identical to the logits path whenever the dot products are exact in fp32).
  * Call it while no work using the handle is in flight.
  */
 CD_API cd_status cd_set_sampling(cd_dfa_t* dfa, float temperature, uint64_t seed, int32_t step_base);

@@ -1020,6 +1020,11 @@ cd_status launch_head(const cd_dfa* d, Scratch* s, const void* hidden, long long
     a.fin.lse_out = lse_out;
     a.fin.done_out = done_out;
     a.fin.ctrs = s->ctrs;
+    a.fin.inv_tau = d->inv_tau;
+    a.fin.seed_lo = (uint32_t)(d->seed & 0xFFFFFFFFull);
+    a.fin.seed_hi = (uint32_t)(d->seed >> 32);
+    a.fin.rng_step_base = d->rng_step_base;
+    const bool sample = d->inv_tau > 0.0f;
     a.hidden = static_cast<const uint16_t*>(hidden);
     a.ldh = ldh;
     a.W = static_cast<const uint16_t*>(W);
@@ -1047,10 +1052,12 @@ cd_status launch_head(const cd_dfa* d, Scratch* s, const void* hidden, long long
         const size_t smem = (size_t)H * 2;
         static thread_local int cfg_dev = -1;
         if (smem > 48 * 1024 && cfg_dev != d->device) {
-            CU(cudaFuncSetAttribute(cd::head_gather_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            CU(cudaFuncSetAttribute(cd::head_gather_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            CU(cudaFuncSetAttribute(cd::head_gather_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
             cfg_dev = d->device;
         }
-        cd::head_gather_kernel<<<n, cd::HG_WARPS * 32, smem, stream>>>(a);
+        if (sample) cd::head_gather_kernel<true><<<n, cd::HG_WARPS * 32, smem, stream>>>(a);
+        else cd::head_gather_kernel<false><<<n, cd::HG_WARPS * 32, smem, stream>>>(a);
         CU(cudaGetLastError());
         ++launches;
     }
@@ -1060,12 +1067,20 @@ cd_status launch_head(const cd_dfa* d, Scratch* s, const void* hidden, long long
         CU(cudaGetLastError());
         static thread_local int cfg_dev2 = -1;
         if (cfg_dev2 != d->device) {
-            CU(cudaFuncSetAttribute(cd::head_dense_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, cd::HD_SMEM_BYTES));
+            CU(cudaFuncSetAttribute(cd::head_dense_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, cd::HD_SMEM_BYTES));
+            CU(cudaFuncSetAttribute(cd::head_dense_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, cd::HD_SMEM_BYTES));
             cfg_dev2 = d->device;
         }
-        cd::head_dense_kernel<<<d->num_sms, cd::HD_THREADS, cd::HD_SMEM_BYTES, stream>>>(s->h_tmA, d->w_tmap, a);
-        CU(cudaGetLastError());
-        cd::head_finish_kernel<<<(n + rows_per_block - 1) / rows_per_block, rows_per_block * 32, 0, stream>>>(a);
+        const int fin_blocks = (n + rows_per_block - 1) / rows_per_block;
+        if (sample) {
+            cd::head_dense_kernel<true><<<d->num_sms, cd::HD_THREADS, cd::HD_SMEM_BYTES, stream>>>(s->h_tmA, d->w_tmap, a);
+            CU(cudaGetLastError());
+            cd::head_finish_kernel<true><<<fin_blocks, rows_per_block * 32, 0, stream>>>(a);
+        } else {
+            cd::head_dense_kernel<false><<<d->num_sms, cd::HD_THREADS, cd::HD_SMEM_BYTES, stream>>>(s->h_tmA, d->w_tmap, a);
+            CU(cudaGetLastError());
+            cd::head_finish_kernel<false><<<fin_blocks, rows_per_block * 32, 0, stream>>>(a);
+        }
         CU(cudaGetLastError());
         launches += 3;
     }
@@ -1118,7 +1133,6 @@ cd_status cd_head_step(const cd_dfa_t* d, const void* hidden, int64_t ldh_elems,
                        float* logprob_out, float* lse_out, uint8_t* done_out, void* cuda_stream) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
     if (n < 0) return fail(CD_ERR_ARG, "n < 0");
-    if (d->inv_tau > 0.0f) return fail(CD_ERR_ARG, "sampling (cd_set_sampling) is not available on the LM-head path");
     cd_status st = check_head_layout(hidden, ldh_elems, W, ldw_elems, H);
     if (st != CD_OK) return st;
     if (n == 0) return CD_OK;
@@ -1148,7 +1162,6 @@ static cd_status head_loop_impl(const cd_dfa_t* d, const void* const* step_hidde
     if (!len_out || !final_state_out || !sum_logprob_out || !done_out || (max_steps > 0 && !tokens_out))
         return fail(CD_ERR_ARG, "NULL output pointer");
     if (max_steps > 0 && !step_hidden) return fail(CD_ERR_ARG, "step_hidden is NULL");
-    if (d->inv_tau > 0.0f) return fail(CD_ERR_ARG, "sampling (cd_set_sampling) is not available on the LM-head path");
     cd_status st = CD_OK;
     for (int k = 0; k < max_steps; ++k) {
         // host rows need no 16-byte alignment of their own: they are copied into aligned staging
@@ -1475,7 +1488,6 @@ cd_status cd_head_decode_loop_cb(const cd_dfa_t* d, cd_next_hidden_fn next_hidde
     if (B == 0) return CD_OK;
     if (!len_out || !final_state_out || !sum_logprob_out || !done_out || (max_steps > 0 && !tokens_out))
         return fail(CD_ERR_ARG, "NULL output pointer");
-    if (d->inv_tau > 0.0f) return fail(CD_ERR_ARG, "sampling (cd_set_sampling) is not available on the LM-head path");
     DeviceGuard guard(d->device);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     Scratch* s = nullptr;

@@ -39,10 +39,53 @@ constexpr int HD_UNITS_TARGET = 148 * 8;
 
 constexpr int HG_WARPS = 8;  // gather kernel: warps per CTA (one CTA per row)
 
-struct __align__(16) HeadPartial {
+struct __align__(32) HeadPartial {
     float m, s;
-    int idx, pad;
+    int idx;        // greedy: argmax token; sampling: sampled token
+    float kb, yb;   // sampling: best perturbed key and the tempered logit of its token
+    int pad[3];
 };
+
+// Sampling on the head path: as online_update_sample, and the tempered logit of the running winner is
+// kept (the accumulator is gone once the tile is drained, so it cannot be re-read at finalisation).
+__device__ __forceinline__ void head_update_sample(float& m, float& s, float& kb, int& kidx, float& yb, float x, int t,
+                                                   int pos, float inv_tau, uint32_t row_key) {
+    const float y = fmaxf(__fmul_rn(x, inv_tau), -INFINITY);
+    const float lo = fminf(m, y), hi = fmaxf(m, y);
+    float e = ex2_ftz((lo - hi) * LOG2E);
+    e = (lo == -INFINITY) ? 0.0f : e;
+    s = (y > m) ? fmaf(s, e, 1.0f) : s + e;
+    m = hi;
+    const float key = __fadd_rn(y, gumbel_noise(row_key, (uint32_t)t));
+    const bool gt = key > kb;
+    kb = gt ? key : kb;
+    kidx = gt ? pos : kidx;
+    yb = gt ? y : yb;
+}
+
+__device__ __forceinline__ void head_sample_combine(float& kb, int& kidx, float& yb, float k2, int i2, float y2) {
+    const bool take2 = (k2 > kb) || (k2 == kb && i2 < kidx);
+    kb = take2 ? k2 : kb;
+    kidx = take2 ? i2 : kidx;
+    yb = take2 ? y2 : yb;
+}
+
+template <bool SAMPLE>
+__device__ __forceinline__ void head_warp_combine(float& m, float& s, int& idx, float& kb, float& yb) {
+    if constexpr (!SAMPLE) {
+        warp_combine(m, s, idx);
+    } else {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const float m2 = __shfl_xor_sync(FULL, m, o), s2 = __shfl_xor_sync(FULL, s, o);
+            const int i2 = __shfl_xor_sync(FULL, idx, o);
+            const float k2 = __shfl_xor_sync(FULL, kb, o), y2 = __shfl_xor_sync(FULL, yb, o);
+            int dummy = 0;
+            online_combine(m, s, dummy, m2, s2, 0);
+            head_sample_combine(kb, idx, yb, k2, i2, y2);
+        }
+    }
+}
 
 // Work decomposition of the dense contraction for n_dense rows: unit = (row tile, range of L
 // consecutive vocabulary tiles); a row has NU partial results.  Unit u -> row tile u % num_m,
@@ -223,10 +266,11 @@ __device__ __forceinline__ float dot8(const uint4& w, const uint4& h, float acc)
 // One CTA per gathered row: the hidden row is staged in shared memory, the warps split the
 // state's CSR token list into contiguous pieces, four dot products in flight per warp; the
 // running argmax is the CSR position (ascending token id), so the transition needs no search.
+template <bool SAMPLE>
 __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadArgs a) {
     extern __shared__ __align__(16) unsigned char hg_smem[];
     uint4* hid = reinterpret_cast<uint4*>(hg_smem);
-    __shared__ float s_m[HG_WARPS], s_s[HG_WARPS];
+    __shared__ float s_m[HG_WARPS], s_s[HG_WARPS], s_k[HG_WARPS], s_y[HG_WARPS];
     __shared__ int s_i[HG_WARPS];
     const StepArgs& f = a.fin;
     const int n_gather = __ldcg(a.hctr + 1);
@@ -244,14 +288,20 @@ __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadAr
         const int deg = (int)(__ldg(f.dfa.row_ptr + st + 1) - lo);
         const int j0 = (int)(((long long)deg * warp) / HG_WARPS);
         const int j1 = (int)(((long long)deg * (warp + 1)) / HG_WARPS);
-        float m = -INFINITY, s = 0.0f;
+        float m = -INFINITY, s = 0.0f, kb = -INFINITY, yb = -INFINITY;
         int idx = 0x7FFFFFFF;
+        const uint32_t row_key =
+            SAMPLE ? rng_row_key(f.seed_lo, f.seed_hi, (uint32_t)(f.row_map ? __ldg(f.row_map + slot) : slot),
+                                 (uint32_t)(f.rng_step_base + f.step))
+                   : 0u;
         for (int j = j0; j < j1; j += 4) {
             const uint4* wp[4];
+            int tq[4];
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int jq = (j + q < j1) ? j + q : j1 - 1;
-                wp[q] = reinterpret_cast<const uint4*>(a.W + (long long)__ldg(f.dfa.tok + lo + jq) * a.ldw);
+                tq[q] = __ldg(f.dfa.tok + lo + jq);
+                wp[q] = reinterpret_cast<const uint4*>(a.W + (long long)tq[q] * a.ldw);
             }
             float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
             for (int v = lane; v < nv; v += 32) {
@@ -266,21 +316,30 @@ __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadAr
             }
 #pragma unroll
             for (int q = 0; q < 4; ++q)
-                if (j + q < j1) online_update(m, s, idx, fmaxf(acc[q], -INFINITY), j + q);  // NaN -> -inf
+                if (j + q < j1) {
+                    if (SAMPLE)
+                        head_update_sample(m, s, kb, idx, yb, fmaxf(acc[q], -INFINITY), tq[q], j + q, f.inv_tau, row_key);
+                    else
+                        online_update(m, s, idx, fmaxf(acc[q], -INFINITY), j + q);  // NaN -> -inf
+                }
         }
         if (lane == 0) {
             s_m[warp] = m;
             s_s[warp] = s;
             s_i[warp] = idx;
+            s_k[warp] = kb;
+            s_y[warp] = yb;
         }
         __syncthreads();
         if (warp == 0) {
             float rm = (lane < HG_WARPS) ? s_m[lane] : -INFINITY;
             float rs = (lane < HG_WARPS) ? s_s[lane] : 0.0f;
             int ri = (lane < HG_WARPS) ? s_i[lane] : 0x7FFFFFFF;
-            warp_combine(rm, rs, ri);
+            float rk = (lane < HG_WARPS) ? s_k[lane] : -INFINITY;
+            float ry = (lane < HG_WARPS) ? s_y[lane] : -INFINITY;
+            head_warp_combine<SAMPLE>(rm, rs, ri, rk, ry);
             const TileMeta mt{slot, 0, 0, st, lo, deg, 0};
-            finalize_row(f, mt, rm, rs, ri, lane, true);
+            finalize_row(f, mt, rm, rs, ri, lane, true, SAMPLE, ry);
         }
     }
 }
@@ -291,6 +350,7 @@ __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadAr
 //   tfull[b] / tempty[b]  accumulator buffer b (256 TMEM columns): MMA -> epilogue / back
 // Every role walks the same sequence (units of this CTA -> vocabulary tiles -> K blocks), so
 // stage and phase counters stay in step without any other communication.
+template <bool SAMPLE>
 __global__ void __launch_bounds__(HD_THREADS, 1)
 head_dense_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmW, const HeadArgs a) {
     extern __shared__ __align__(1024) unsigned char hd_smem[];
@@ -398,8 +458,15 @@ head_dense_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
             const bool valid = drow < n_dense;
             const int st = valid ? __ldcg(a.dense_state + drow) : 0;
             const uint32_t* mrow = dfa.mask + (long long)st * dfa.Wpad;
-            float m = -INFINITY, s = 0.0f;
+            float m = -INFINITY, s = 0.0f, kb = -INFINITY, yb = -INFINITY;
             int idx = 0x7FFFFFFF;
+            uint32_t row_key = 0u;
+            if (SAMPLE && valid) {
+                const int slot = __ldcg(a.dense_slot + drow);
+                row_key = rng_row_key(a.fin.seed_lo, a.fin.seed_hi,
+                                      (uint32_t)(a.fin.row_map ? __ldg(a.fin.row_map + slot) : slot),
+                                      (uint32_t)(a.fin.rng_step_base + a.fin.step));
+            }
             for (int nt = nt0; nt < nt1; ++nt) {
                 const int n0 = nt * HD_BN;
                 // the 8 mask words of this row for the tile's 256 tokens (two 16-byte loads)
@@ -424,8 +491,13 @@ head_dense_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                         tmem_ld_wait();
 #pragma unroll
                         for (int j = 0; j < 32; ++j)
-                            if ((bits >> j) & 1u)
-                                online_update(m, s, idx, fmaxf(__uint_as_float(v[j]), -INFINITY), n0 + c * 32 + j);
+                            if ((bits >> j) & 1u) {
+                                if (SAMPLE)
+                                    head_update_sample(m, s, kb, idx, yb, fmaxf(__uint_as_float(v[j]), -INFINITY),
+                                                       n0 + c * 32 + j, n0 + c * 32 + j, a.fin.inv_tau, row_key);
+                                else
+                                    online_update(m, s, idx, fmaxf(__uint_as_float(v[j]), -INFINITY), n0 + c * 32 + j);
+                            }
                     }
                 }
                 tc_fence_before();
@@ -434,7 +506,7 @@ head_dense_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
                 ab ^= 1;
                 if (ab == 0) aphase ^= 1u;
             }
-            if (valid) a.partials[(long long)drow * hs.NU + n_unit] = HeadPartial{m, s, idx, 0};
+            if (valid) a.partials[(long long)drow * hs.NU + n_unit] = HeadPartial{m, s, idx, kb, yb, {0, 0, 0}};
         }
     }
     tc_fence_before();
@@ -446,6 +518,7 @@ head_dense_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
 // ---------------------------------------------------------------- finish dense rows
 // One warp per dense row: partials merged in a fixed order (lane q % 32 takes ranges q, q + 32,
 // ... ascending, then the butterfly), then the CSR transition and the accept test.
+template <bool SAMPLE>
 __global__ void head_finish_kernel(const HeadArgs a) {
     const StepArgs& f = a.fin;
     const int n_dense = __ldcg(a.hctr + 0);
@@ -456,17 +529,25 @@ __global__ void head_finish_kernel(const HeadArgs a) {
     for (int d = warp; d < n_dense; d += nwarps) {
         const int slot = __ldcg(a.dense_slot + d);
         const int st = __ldcg(a.dense_state + d);
-        float m = -INFINITY, s = 0.0f;
+        float m = -INFINITY, s = 0.0f, kb = -INFINITY, yb = -INFINITY;
         int idx = 0x7FFFFFFF;
         for (int q = lane; q < hs.NU; q += 32) {
-            const int4 p = __ldcg(reinterpret_cast<const int4*>(a.partials + (long long)d * hs.NU + q));
-            online_combine(m, s, idx, __int_as_float(p.x), __int_as_float(p.y), p.z);
+            const int4* pp = reinterpret_cast<const int4*>(a.partials + (long long)d * hs.NU + q);
+            const int4 p = __ldcg(pp);
+            if (SAMPLE) {
+                const int4 p2 = __ldcg(pp + 1);
+                int dummy = 0;
+                online_combine(m, s, dummy, __int_as_float(p.x), __int_as_float(p.y), 0);
+                head_sample_combine(kb, idx, yb, __int_as_float(p.w), p.z, __int_as_float(p2.x));
+            } else {
+                online_combine(m, s, idx, __int_as_float(p.x), __int_as_float(p.y), p.z);
+            }
         }
-        warp_combine(m, s, idx);
+        head_warp_combine<SAMPLE>(m, s, idx, kb, yb);
         const long long lo = __ldg(f.dfa.row_ptr + st);
         const int deg = (int)(__ldg(f.dfa.row_ptr + st + 1) - lo);
         const TileMeta mt{slot, 0, 0, st, lo, deg, 0};
-        finalize_row(f, mt, m, s, idx, lane, false);
+        finalize_row(f, mt, m, s, idx, lane, false, SAMPLE, yb);
     }
 }
 

@@ -313,3 +313,45 @@ def test_head_decode_loop_host_equals_device_loop(cd, mode):
     for k in ("tokens", "len", "final_state", "done", "sum_logprob"):
         assert torch.equal(a[k], b[k].cpu()), k
     assert not a["tokens"].is_cuda and int(a["len"].max()) > 1
+
+
+# ---------------------------------------------------------------- sampling on the head path (N5 x N2)
+@pytest.mark.parametrize("V,H,S,n,density,T", [(3000, 128, 12, 150, 0.1, 1.0), (5000, 256, 8, 300, 1.0, 0.6),
+                                               (1000, 200, 7, 37, 0.3, 2.0)])
+def test_head_sampled_step_matches_oracle_on_exact_logits(cd, oracle, mode, V, H, S, n, density, T):
+    """cd_set_sampling on cd_head_step against O10 applied to fp32 logits from a library matmul
+    (exact-arithmetic inputs: the head's fp32 dot products equal them bit for bit)."""
+    aut = wl.make_random_dfa(71, V, S, density, 0.2)
+    dfa = dev_dfa(cd, aut, mode)
+    dfa.set_sampling(T, seed=0xABCDEF0123, step_base=3)
+    hid = wl.make_hidden(71, 0, n + 9, H, exact=True)
+    W = wl.make_head(71, V, H, 2.0, exact=True)
+    x32 = (hid.double() @ W.double().t()).float().contiguous()
+    states = live_states(aut, n)
+    row_map = [(i * 5 + 2) % (n + 9) for i in range(n)]
+    st_d = torch.tensor(states, dtype=torch.int32, device="cuda:0")
+    rm_d = torch.tensor(row_map, dtype=torch.int32, device="cuda:0")
+    tok, lp, lse, done = cd.head_step(dfa, hid.to("cuda:0"), W.to("cuda:0"), st_d, row_map=rm_d, H=H)
+    torch.cuda.synchronize()
+    o_tok, o_lp, o_lse, o_done, o_st = oracle.sample_step(aut, x32, states, T, seed=0xABCDEF0123, step=3, row_map=row_map)
+    assert tok.cpu().numpy().tolist() == o_tok.tolist()
+    assert st_d.cpu().numpy().tolist() == o_st.tolist() and done.cpu().numpy().tolist() == o_done.tolist()
+    for g, r in ((lp, o_lp), (lse, o_lse)):
+        assert np.all(np.abs(g.cpu().numpy().astype(np.float64) - r) <= TOL * np.maximum(1.0, np.abs(r)))
+
+
+def test_head_sampled_loop_matches_logits_loop(cd, oracle, mode):
+    V, H, B, steps = 4096, 256, 200, 6
+    aut = wl.make_random_dfa(73, V, 30, 0.05, 0.1)
+    dfa = dev_dfa(cd, aut, mode)
+    dfa.set_sampling(0.8, seed=17, step_base=1)
+    W = wl.make_head(73, V, H, 2.0, exact=True)
+    hs = [wl.make_hidden(73, k, B, H, exact=True) for k in range(steps)]
+    logits = [(h.double() @ W.double().t()).float().contiguous() for h in hs]
+    got = cd.head_decode_loop(dfa, [h.to("cuda:0") for h in hs], W.to("cuda:0"), H=H)
+    torch.cuda.synchronize()
+    want = oracle.sample_decode_loop(aut, logits, 0.8, seed=17, step_base=1)
+    for k in ("tokens", "len", "final_state", "done"):
+        assert np.array_equal(got[k].cpu().numpy(), want[k]), k
+    slp = got["sum_logprob"].cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(slp - want["sum_logprob"]) <= TOL * (want["len"] + np.abs(want["sum_logprob"])) + 1e-12)
