@@ -1300,6 +1300,21 @@ int grid_for(long long n, int threads) {
     return (int)b;
 }
 
+// Stream-ordered scratch (cudaMallocAsync) must not be handed back to the OS at every synchronisation:
+// keep the default pool's memory (once per device).
+void keep_pool_memory(int dev) {
+    static std::mutex mu;
+    static std::map<int, bool> done;
+    std::lock_guard<std::mutex> lk(mu);
+    if (done[dev]) return;
+    cudaMemPool_t pool = nullptr;
+    if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess && pool) {
+        unsigned long long thr = ~0ull;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+    }
+    done[dev] = true;
+}
+
 cd_status device_of(const void* p, int* dev) {
     cudaPointerAttributes at;
     CU(cudaPointerGetAttributes(&at, p));
@@ -1355,6 +1370,7 @@ cd_status cd_dedup(const int64_t* keys, int32_t N, int32_t* rep_out, int32_t* di
     cd_status st = device_of(n_distinct_out, &dev);
     if (st != CD_OK) return st;
     DeviceGuard guard(dev);
+    keep_pool_memory(dev);
     if (N == 0) {
         CU(cudaMemsetAsync(n_distinct_out, 0, sizeof(int), stream));
         return CD_OK;
@@ -1425,6 +1441,7 @@ cd_status cd_filter_rows(const cd_dfa_t* d, const int32_t* final_state, const ui
         return CD_OK;
     }
     if (!final_state || !done || !row_ids_out) return fail(CD_ERR_ARG, "NULL pointer");
+    keep_pool_memory(d->device);
     uint8_t* drop = nullptr;
     CU(cudaMallocAsync(reinterpret_cast<void**>(&drop), (size_t)N + 16, stream));
     cd::filter_flag_kernel<<<grid_for(N, 256), 256, 0, stream>>>(final_state, done, N,
