@@ -646,7 +646,8 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "bf16" if cfg.dtype == torch.bfloat16 else "f32", "data": "synthetic",
+            "vs_baseline": None, "dtype": "f32", "logits_dtype": "bf16" if cfg.dtype == torch.bfloat16 else "f32",
+            "data": "synthetic",
             "config": {
                 "workload": f"{cfg.name}: {cfg.desc}; one step = cd_decode_loop over one batch of B={cfg.B} rows",
                 "B": cfg.B, "V": cfg.V, "max_steps": cfg.max_steps, "S": aut.S, "nnz": aut.nnz,

@@ -975,7 +975,7 @@ cd_status check_head_layout(const void* hidden, long long ldh, const void* W, lo
 }
 
 // tensor map of the output embedding, cached per handle (the weights rarely change)
-cd_status head_weight_map(const cd_dfa* d, const void* W, long long ldw, int H) {
+cd_status head_weight_map(const cd_dfa* d, const void* W, long long ldw, int H, CUtensorMap* out) {
     cd_dfa* dm = const_cast<cd_dfa*>(d);
     std::lock_guard<std::mutex> lk(dm->mu);
     if (dm->w_ptr != W || dm->w_ld != ldw || dm->w_H != H) {
@@ -983,6 +983,7 @@ cd_status head_weight_map(const cd_dfa* d, const void* W, long long ldw, int H) 
         if (st != CD_OK) return st;
         dm->w_ptr = W; dm->w_ld = ldw; dm->w_H = H;
     }
+    *out = dm->w_tmap;  // copied under the lock: concurrent callers may use different weights
     return CD_OK;
 }
 
@@ -1043,6 +1044,11 @@ cd_status launch_head(const cd_dfa* d, Scratch* s, const void* hidden, long long
     a.partials = s->h_partials;
 
     const int n = n_upper;
+    CUtensorMap tmW;
+    {
+        const cd_status stw = head_weight_map(d, W, ldw, H, &tmW);
+        if (stw != CD_OK) return stw;
+    }
     cd::head_prepare_kernel<<<1, 1024, 0, stream>>>(a);
     CU(cudaGetLastError());
     const bool any_gather = a.gather_max > 0 && d->min_deg_nonacc <= a.gather_max;
@@ -1073,11 +1079,11 @@ cd_status launch_head(const cd_dfa* d, Scratch* s, const void* hidden, long long
         }
         const int fin_blocks = (n + rows_per_block - 1) / rows_per_block;
         if (sample) {
-            cd::head_dense_kernel<true><<<d->num_sms, cd::HD_THREADS, cd::HD_SMEM_BYTES, stream>>>(s->h_tmA, d->w_tmap, a);
+            cd::head_dense_kernel<true><<<d->num_sms, cd::HD_THREADS, cd::HD_SMEM_BYTES, stream>>>(s->h_tmA, tmW, a);
             CU(cudaGetLastError());
             cd::head_finish_kernel<true><<<fin_blocks, rows_per_block * 32, 0, stream>>>(a);
         } else {
-            cd::head_dense_kernel<false><<<d->num_sms, cd::HD_THREADS, cd::HD_SMEM_BYTES, stream>>>(s->h_tmA, d->w_tmap, a);
+            cd::head_dense_kernel<false><<<d->num_sms, cd::HD_THREADS, cd::HD_SMEM_BYTES, stream>>>(s->h_tmA, tmW, a);
             CU(cudaGetLastError());
             cd::head_finish_kernel<false><<<fin_blocks, rows_per_block * 32, 0, stream>>>(a);
         }
@@ -1143,8 +1149,6 @@ cd_status cd_head_step(const cd_dfa_t* d, const void* hidden, int64_t ldh_elems,
     st = get_scratch(d, stream, n, false, &s);
     if (st != CD_OK) return st;
     st = get_head_scratch(s, n, H, stream);
-    if (st != CD_OK) return st;
-    st = head_weight_map(d, W, ldw_elems, H);
     if (st != CD_OK) return st;
     return launch_head(d, s, hidden, ldh_elems, W, ldw_elems, H, row_map, state, n, nullptr, token_out, logprob_out,
                        lse_out, done_out, stream, nullptr);
@@ -1215,8 +1219,6 @@ static cd_status head_loop_impl(const cd_dfa_t* d, const void* const* step_hidde
     if (st != CD_OK) return st;
     if (!d->start_accepting && max_steps > 0) {
         st = get_head_scratch(s, B, H, stream);
-        if (st != CD_OK) return st;
-        st = head_weight_map(d, W, ldw_elems, H);
         if (st != CD_OK) return st;
         if (host) {
             CU(cudaEventRecord(s->ev_consumed[0], stream));
@@ -1526,10 +1528,6 @@ cd_status cd_head_decode_loop_cb(const cd_dfa_t* d, cd_next_hidden_fn next_hidde
             if (rc != 0) return fail(CD_ERR_ARG, "next_hidden returned %d at step %d", rc, k);
             st = check_head_layout(hidden, ldh, W, ldw_elems, H);
             if (st != CD_OK) return st;
-            if (k == 0) {
-                st = head_weight_map(d, W, ldw_elems, H);
-                if (st != CD_OK) return st;
-            }
             LoopExtras x;
             x.tokens = tokens_out;
             x.len = len_out;

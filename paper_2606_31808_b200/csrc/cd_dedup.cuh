@@ -146,11 +146,14 @@ __global__ void join_kernel(const int* __restrict__ rep, int N, int max_steps, c
         if (slp) slp[i] = slp_d[r];
         if (done) done[i] = done_d[r];
     }
-    if (tokens)
-        for (long long j = tid; j < (long long)N * max_steps; j += nth) {
-            const long long i = j / max_steps;
-            tokens[j] = tokens_d[(long long)rep[i] * max_steps + (j - i * max_steps)];
+    if (tokens) {
+        // one warp per row: coalesced over the steps, no division per element
+        const int lane = threadIdx.x & 31;
+        for (long long i = tid >> 5; i < N; i += nth >> 5) {
+            const long long src = (long long)rep[i] * max_steps, dst = i * max_steps;
+            for (int k = lane; k < max_steps; k += 32) tokens[dst + k] = tokens_d[src + k];
         }
+    }
 }
 
 // Cascade filtering: flag = 1 for rows that are NOT passed on to the next LM
