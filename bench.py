@@ -354,7 +354,7 @@ def run_reference(args, rank):
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64 accumulate over " + str(cfg.dtype).replace("torch.", ""),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "logits_dtype": str(cfg.dtype).replace("torch.", ""),
         "data": "synthetic", "config": {"workload": cfg.desc, "sample": sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
