@@ -355,3 +355,18 @@ def test_head_sampled_loop_matches_logits_loop(cd, oracle, mode):
         assert np.array_equal(got[k].cpu().numpy(), want[k]), k
     slp = got["sum_logprob"].cpu().numpy().astype(np.float64)
     assert np.all(np.abs(slp - want["sum_logprob"]) <= TOL * (want["len"] + np.abs(want["sum_logprob"])) + 1e-12)
+
+
+def test_head_loop_many_rows(cd, oracle, mode):
+    """B = 6,000 rows (47 row tiles, more than one chunk of the one-CTA list building) on the head path."""
+    V, H, B, steps = 1536, 64, 6000, 4
+    aut = wl.make_random_dfa(79, V, 16, 0.08, 0.2)
+    dfa = dev_dfa(cd, aut, mode)
+    W = wl.make_head(79, V, H, 2.0, exact=True)
+    hs = [wl.make_hidden(79, k, B, H, exact=True) for k in range(steps)]
+    got = cd.head_decode_loop(dfa, [h.to("cuda:0") for h in hs], W.to("cuda:0"), H=H)
+    torch.cuda.synchronize()
+    want = oracle.head_decode_loop(aut, hs, W, H)
+    for k in ("tokens", "len", "final_state", "done"):
+        assert np.array_equal(got[k].cpu().numpy(), want[k]), k
+    assert want["n_active_hist"][1] > 4096

@@ -644,3 +644,20 @@ def test_step_and_compact_in_a_cuda_graph(cd, oracle):
         assert st.cpu().numpy().tolist() == o_st.tolist()
         o_ro, o_so, k = oracle.compact(o_done, None, o_st)
         assert int(cmp_out[2]) == k and cmp_out[0][:k].cpu().numpy().tolist() == o_ro.tolist()
+
+
+def test_loop_many_rows_small_vocab(cd, oracle):
+    """B = 10,000 rows (more than one chunk of the one-CTA compaction, more rows than the c4 batch)
+    at a small vocabulary: the fused loop end to end against the oracle."""
+    cfg = wl.scaled(wl.CONFIGS["c3"], V=2048, B=10000, S=24, max_steps=6, density=0.05)
+    aut = wl.build_automaton(cfg)
+    dfa = dev_dfa(cd, aut)
+    logits = wl.build_step_logits(cfg, aut, device="cuda:0")
+    got = cd.decode_loop(dfa, logits)
+    torch.cuda.synchronize()
+    want = oracle.decode_loop(aut, [x.cpu() for x in logits])
+    for k in ("tokens", "len", "final_state", "done"):
+        assert np.array_equal(got[k].cpu().numpy(), want[k]), k
+    ok, worst = close(got["sum_logprob"].cpu().numpy(), want["sum_logprob"], tol=TOL * cfg.max_steps)
+    assert ok, worst
+    assert want["n_active_hist"][1] > 4096  # the second step still compacts more than one chunk
