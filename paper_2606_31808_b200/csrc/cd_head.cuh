@@ -304,7 +304,20 @@ __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadAr
                 wp[q] = reinterpret_cast<const uint4*>(a.W + (long long)tq[q] * a.ldw);
             }
             float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-            for (int v = lane; v < nv; v += 32) {
+            // two chunks of the four W rows per round: 8 independent 16-byte loads in flight per lane
+            int v = lane;
+            for (; v + 32 < nv; v += 64) {
+                uint4 w0[4], w1[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    w0[q] = __ldg(wp[q] + v);
+                    w1[q] = __ldg(wp[q] + v + 32);
+                }
+                const uint4 h0 = hid[v], h1 = hid[v + 32];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) acc[q] = dot8(w1[q], h1, dot8(w0[q], h0, acc[q]));
+            }
+            for (; v < nv; v += 32) {
                 const uint4 h = hid[v];
 #pragma unroll
                 for (int q = 0; q < 4; ++q) acc[q] = dot8(__ldg(wp[q] + v), h, acc[q]);
