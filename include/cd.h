@@ -101,6 +101,33 @@ CD_API cd_status cd_compile_dfa(int32_t V, int32_t S, int32_t start, const int64
 CD_API cd_status cd_compile_trie(int32_t V, int32_t K, const int64_t* label_ptr /*[K+1]*/,
                           const int32_t* label_tok, int device, cd_dfa_t** out);
 
+/*
+ * Sugar for collection types with a quantifier (section 2.3: "If the
+ * return_type is a collection, the quantifier argument can be used to apply a regular
+ * expression-style modifier to restrict the number of generated items (e.g. {3} for
+ * exactly three, {1,5} for between one and five)"): the token-level automaton of
+ *     open  item (sep item)^(c-1)  close        for min_items <= c <= max_items
+ * (c = 0: open close), every item one of the K labels of cd_compile_trie's form; open, sep,
+ * close are token-id sequences (HOST pointers; open may be empty, sep may be empty when
+ * max_items == 1, close must not be).  One accepting state, reached by the last token of
+ * close.  Deterministic by construction or rejected (CD_ERR_AUTOMATON): labels non-empty,
+ * distinct and prefix-free, sep[0] != close[0], and close[0] does not start a label when
+ * min_items == 0.  State 0 is the start state.
+ * cd_build_list is pure host code (no device needed): it writes the number of states and
+ * transitions to *S_out / *nnz_out and, where the array pointers are not NULL, the CSR
+ * (row_ptr [S+1], tok / next [nnz], accepting [S]; size them from a first call with NULL
+ * arrays).  cd_compile_list builds the same automaton and compiles it (as cd_compile_dfa).
+ */
+CD_API cd_status cd_build_list(int32_t V, int32_t K, const int64_t* label_ptr, const int32_t* label_tok,
+                        const int32_t* open, int32_t n_open, const int32_t* sep, int32_t n_sep,
+                        const int32_t* close, int32_t n_close, int32_t min_items, int32_t max_items,
+                        int32_t* S_out, int64_t* nnz_out, int64_t* row_ptr_out, int32_t* tok_out,
+                        int32_t* next_out, uint8_t* accepting_out);
+CD_API cd_status cd_compile_list(int32_t V, int32_t K, const int64_t* label_ptr, const int32_t* label_tok,
+                          const int32_t* open, int32_t n_open, const int32_t* sep, int32_t n_sep,
+                          const int32_t* close, int32_t n_close, int32_t min_items, int32_t max_items,
+                          int device, cd_dfa_t** out);
+
 /* Releases the device image and every per-stream scratch area.  NULL is a no-op.
    The caller makes sure no work using the handle is still in flight. */
 CD_API void cd_free_dfa(cd_dfa_t* dfa);

@@ -12,7 +12,9 @@ from .binding import (  # noqa: F401
     CdError,
     Dfa,
     compact,
+    build_list,
     compile_dfa,
+    compile_list,
     compile_trie,
     decode_loop,
     decode_loop_cb,

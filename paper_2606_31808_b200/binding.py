@@ -17,7 +17,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
-    "cd_compile_dfa", "cd_compile_trie", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_set_sampling", "cd_reserve", "cd_step",
+    "cd_compile_dfa", "cd_compile_trie", "cd_build_list", "cd_compile_list", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_set_sampling", "cd_reserve", "cd_step",
     "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_set_limit", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_probe_read", "cd_decode_loop_cb", "cd_head_decode_loop_cb", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
     "cd_last_error",
 )
@@ -516,3 +516,45 @@ def head_decode_loop_cb(dfa: Dfa, next_hidden, W: torch.Tensor, H: int, B: int, 
                                         _ptr(out["final_state"]), _ptr(out["sum_logprob"]), _ptr(out["done"]),
                                         _stream(dev)))
     return out
+
+
+def _list_args(V, labels, open_, sep, close, min_items, max_items):
+    ptr, flat = [0], []
+    for lab in labels:
+        flat.extend(int(t) for t in lab)
+        ptr.append(len(flat))
+    lp = torch.tensor(ptr, dtype=torch.int64)
+    lt = torch.tensor(flat if flat else [0], dtype=torch.int32)
+    ts = [torch.tensor(list(x) if len(x) else [0], dtype=torch.int32) for x in (open_, sep, close)]
+    args = [C.c_int32(V), C.c_int32(len(labels)), _ptr(lp), _ptr(lt), _ptr(ts[0]), C.c_int32(len(open_)), _ptr(ts[1]),
+            C.c_int32(len(sep)), _ptr(ts[2]), C.c_int32(len(close)), C.c_int32(min_items), C.c_int32(max_items)]
+    return args, (lp, lt, ts)
+
+
+def build_list(V: int, labels: Sequence[Sequence[int]], open_: Sequence[int], sep: Sequence[int],
+               close: Sequence[int], min_items: int, max_items: int):
+    """cd_build_list (host only, no device needed): the CSR of the quantified-list automaton as
+    (S, row_ptr i64[S+1], tok i32[nnz], next i32[nnz], accepting u8[S])."""
+    args, keep = _list_args(V, labels, open_, sep, close, min_items, max_items)
+    S, nnz = C.c_int32(0), C.c_int64(0)
+    null = C.c_void_p(None)
+    _check(lib().cd_build_list(*args, C.byref(S), C.byref(nnz), null, null, null, null))
+    rp = torch.empty(S.value + 1, dtype=torch.int64)
+    tk = torch.empty(max(nnz.value, 1), dtype=torch.int32)
+    nx = torch.empty(max(nnz.value, 1), dtype=torch.int32)
+    ac = torch.empty(S.value, dtype=torch.uint8)
+    _check(lib().cd_build_list(*args, C.byref(S), C.byref(nnz), _ptr(rp), _ptr(tk), _ptr(nx), _ptr(ac)))
+    return S.value, rp, tk[: nnz.value], nx[: nnz.value], ac
+
+
+def compile_list(V: int, labels: Sequence[Sequence[int]], open_: Sequence[int], sep: Sequence[int],
+                 close: Sequence[int], min_items: int, max_items: int, device="cuda") -> Dfa:
+    """cd_compile_list: collection type with a quantifier ({min_items, max_items} items of an option set)."""
+    args, keep = _list_args(V, labels, open_, sep, close, min_items, max_items)
+    dev_index, dev = 0, None
+    if torch.cuda.is_available():
+        dev = _device_index(device)
+        dev_index = dev.index
+    out = C.c_void_p()
+    _check(lib().cd_compile_list(*args, C.c_int(dev_index), C.byref(out)))
+    return Dfa(out.value, dev)

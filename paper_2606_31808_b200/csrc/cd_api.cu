@@ -20,6 +20,7 @@
 #include "cd_step.cuh"
 #include "cd_head.cuh"
 #include "cd_dedup.cuh"
+#include "cd_types.hpp"
 
 namespace {
 
@@ -1551,6 +1552,55 @@ cd_status cd_head_decode_loop_cb(const cd_dfa_t* d, cd_next_hidden_fn next_hidde
         }
     }
     return check_sticky_errors(s, stream);
+}
+
+}  // extern "C"
+
+// =============================================================================== typed-output sugar
+extern "C" {
+
+cd_status cd_build_list(int32_t V, int32_t K, const int64_t* label_ptr, const int32_t* label_tok, const int32_t* open,
+                        int32_t n_open, const int32_t* sep, int32_t n_sep, const int32_t* close, int32_t n_close,
+                        int32_t min_items, int32_t max_items, int32_t* S_out, int64_t* nnz_out, int64_t* row_ptr_out,
+                        int32_t* tok_out, int32_t* next_out, uint8_t* accepting_out) {
+    try {
+        if (!label_ptr || !S_out || !nnz_out) return fail(CD_ERR_ARG, "NULL argument");
+        if (K >= 1 && label_ptr[K] > 0 && !label_tok) return fail(CD_ERR_ARG, "label_tok is NULL");
+        if ((n_open > 0 && !open) || (n_sep > 0 && !sep) || (n_close > 0 && !close)) return fail(CD_ERR_ARG, "NULL token list");
+        cdt::HostCsr c;
+        const std::string err = cdt::build_list(V, K, label_ptr, label_tok, open, n_open, sep, n_sep, close, n_close,
+                                                min_items, max_items, &c);
+        if (!err.empty()) return fail(CD_ERR_AUTOMATON, "%s", err.c_str());
+        *S_out = c.S;
+        *nnz_out = (int64_t)c.tok.size();
+        if (row_ptr_out) std::memcpy(row_ptr_out, c.row_ptr.data(), sizeof(int64_t) * c.row_ptr.size());
+        if (tok_out && !c.tok.empty()) std::memcpy(tok_out, c.tok.data(), sizeof(int32_t) * c.tok.size());
+        if (next_out && !c.next.empty()) std::memcpy(next_out, c.next.data(), sizeof(int32_t) * c.next.size());
+        if (accepting_out) std::memcpy(accepting_out, c.accepting.data(), c.accepting.size());
+        return CD_OK;
+    } catch (const std::bad_alloc&) {
+        return fail(CD_ERR_OOM, "host allocation failed");
+    } catch (...) {
+        return fail(CD_ERR_INTERNAL, "unexpected exception");
+    }
+}
+
+cd_status cd_compile_list(int32_t V, int32_t K, const int64_t* label_ptr, const int32_t* label_tok, const int32_t* open,
+                          int32_t n_open, const int32_t* sep, int32_t n_sep, const int32_t* close, int32_t n_close,
+                          int32_t min_items, int32_t max_items, int device, cd_dfa_t** out) {
+    try {
+        if (!label_ptr || !out) return fail(CD_ERR_ARG, "NULL argument");
+        if ((n_open > 0 && !open) || (n_sep > 0 && !sep) || (n_close > 0 && !close)) return fail(CD_ERR_ARG, "NULL token list");
+        cdt::HostCsr c;
+        const std::string err = cdt::build_list(V, K, label_ptr, label_tok, open, n_open, sep, n_sep, close, n_close,
+                                                min_items, max_items, &c);
+        if (!err.empty()) return fail(CD_ERR_AUTOMATON, "%s", err.c_str());
+        return compile_impl(V, c.S, 0, c.row_ptr.data(), c.tok.data(), c.next.data(), c.accepting.data(), device, out);
+    } catch (const std::bad_alloc&) {
+        return fail(CD_ERR_OOM, "host allocation failed");
+    } catch (...) {
+        return fail(CD_ERR_INTERNAL, "unexpected exception");
+    }
 }
 
 }  // extern "C"
