@@ -531,7 +531,7 @@ def main():
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             ms_a = float(t[0])
         dfa.set_gather_max(0)
-        auto_max = (sz_logit + sz_mask) // 108  # the library's automatic threshold (cd_api.cu gather_max_for)
+        auto_max = (sz_logit + sz_mask) // 232  # the library's automatic threshold (cd_api.cu gather_max_for)
         gathered = [dk for dk in deg_k]  # allowed logits per step of batch 0 (every row-step, if gathered)
         all_gathered = int(deg_dev.max()) <= auto_max
         adaptive = {

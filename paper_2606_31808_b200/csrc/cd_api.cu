@@ -176,13 +176,14 @@ int tiles_per_row(int V, int dtype) {
 }
 
 // Largest number of transitions a state may have to be gathered instead of scanned (0 = never).
-// Automatic policy: a gathered logit costs one 32-byte sector plus its 4-byte token id, and
-// scattered sectors reach roughly a third of the streaming bandwidth, so gathering pays while
-// nnz * 36 * 3 < bytes of a dense row scan (profiles/r1d_gather.md).
+// Automatic policy from the measured rates (profiles/r1d_gather_c4.md): the gather is transaction bound
+// at ~31 G allowed logits/s (one scattered 2-byte logit per 64-byte DRAM granule), the dense scan streams
+// a row at ~6.8 TB/s, so gathering pays while nnz / 31e9 < row_bytes / 6.8e12, i.e. nnz < row_bytes / 220;
+// 232 leaves a margin so that states near the break-even stay on the dense path.
 int gather_max_for(const cd_dfa* d, int dtype) {
     if (d->gather_max >= 0) return d->gather_max;
     const long long row_bytes = (long long)d->dev.V * (dtype == CD_BF16 ? 2 : 4) + d->dev.V / 8;
-    const long long g = row_bytes / 108;
+    const long long g = row_bytes / 232;
     return (int)(g > 0x3FFFFFFF ? 0x3FFFFFFF : g);
 }
 
