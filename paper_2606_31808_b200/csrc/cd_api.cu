@@ -200,11 +200,14 @@ int step_grid(const cd_dfa* d, long long n_upper, int dtype) {
 long long step_units_cap(const cd_dfa* d, long long n) {
     const StepCfg c = STEP_CFGS[step_variant()];
     const int T = tiles_per_row(d->dev.V, CD_F32);  // fp32 rows have the most tiles
-    const int tpu_max = cd::TPU_MAX_BYTES / c.tile_bytes;
+    int tpu_max = cd::TPU_MAX_BYTES / c.tile_bytes;
+    if (const char* e = std::getenv("CD_TPU_MAX")) {  // tuning knob: fewer tiles per unit -> more units per row
+        const int v = std::atoi(e);
+        if (v >= 1 && v < tpu_max) tpu_max = v;
+    }
     const long long warps = (long long)d->num_sms * c.warps;
-    const long long a = warps * 32 + n;  // up to 32 units per warp (CD_UPW)
-    const long long b = n * (long long)(T + 1);  // any tiles-per-unit clamp >= 1 (CD_TPU_MAX)
-    (void)tpu_max;
+    const long long a = warps * 32 + n;  // up to 32 units per warp (tuning knob CD_UPW)
+    const long long b = n * (long long)((T + tpu_max - 1) / tpu_max + 1);
     // small grids (few rows) use fewer warps, hence fewer units: still below a
     return (a > b ? a : b) + 64;
 }
