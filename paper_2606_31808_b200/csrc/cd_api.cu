@@ -63,6 +63,15 @@ int step_variant() {
     return v;
 }
 
+int host_gather_mult() {  // CTAs per SM of the zero-copy row gather (tuning knob CD_HOST_GATHER_CTAS)
+    static const int v = [] {
+        const char* e = std::getenv("CD_HOST_GATHER_CTAS");
+        const int x = e ? std::atoi(e) : 4;  // flat from 2 to 32 (51 GB/s on PCIe Gen5 x16)
+        return (x >= 1 && x <= 64) ? x : 4;
+    }();
+    return v;
+}
+
 bool use_pdl() {
     static const bool v = [] {
         const char* e = std::getenv("CD_PDL");
@@ -848,6 +857,40 @@ cd_status cd_decode_loop_host(const cd_dfa_t* d, const void* const* step_logits_
     st = launch_loop_init(d, s, B, max_steps, d_tokens, d_len, d_fs, d_slp, d_done, stream, lim);
     if (st != CD_OK) return st;
     if (!d->start_accepting && max_steps > 0) {
+        // Pinned, device-mapped host buffers (what cudaHostAlloc / torch pin_memory give under unified
+        // addressing): the SMs pull the active rows over PCIe themselves, nothing is read back per step.
+        bool mapped = true;
+        std::vector<const unsigned char*> dev_view((size_t)max_steps, nullptr);
+        {
+            static const bool allow = [] { const char* e = std::getenv("CD_HOST_ZEROCOPY"); return e ? std::atoi(e) != 0 : true; }();
+            mapped = allow && ((ld_elems * sz) % 16 == 0);
+            for (int k = 0; k < max_steps && mapped; ++k) {
+                cudaPointerAttributes at;
+                if (cudaPointerGetAttributes(&at, step_logits_host[k]) != cudaSuccess) {
+                    cudaGetLastError();
+                    mapped = false;
+                } else if (at.type != cudaMemoryTypeHost || !at.devicePointer ||
+                           (reinterpret_cast<uintptr_t>(at.devicePointer) & 15) != 0) {
+                    mapped = false;
+                } else {
+                    dev_view[(size_t)k] = static_cast<const unsigned char*>(at.devicePointer);
+                }
+            }
+        }
+        if (mapped) {
+            const unsigned long long row_bytes = (unsigned long long)ld_elems * (unsigned long long)sz;
+            for (int k = 0; k < max_steps; ++k) {
+                const int cur = k & 1;
+                cd::host_gather_rows_kernel<<<d->num_sms * host_gather_mult(), 256, 0, stream>>>(dev_view[(size_t)k], row_bytes, s->row_ids[cur],
+                                                                                 s->n_active + cur,
+                                                                                 static_cast<unsigned char*>(s->stage[0]));
+                CU(cudaGetLastError());
+                g_launches.fetch_add(1, std::memory_order_relaxed);
+                st = enqueue_loop_step(d, s, s->stage[0], dtype, ld_elems, B, k, max_steps, d_tokens, d_len, d_fs, d_slp,
+                                       d_done, stream, lim, 1);
+                if (st != CD_OK) return st;
+            }
+        } else {
         // Early exit reaches the PCIe link too: only the rows still active are copied.  After step
         // k - 1 the host reads the compacted active list (n and the original row ids), copies those
         // rows of step k's logits into a compact staging buffer (runs of consecutive ids as one copy)
@@ -885,6 +928,7 @@ cd_status cd_decode_loop_host(const cd_dfa_t* d, const void* const* step_logits_
                                    d_done, stream, lim, 1);
             if (st != CD_OK) return st;
             (void)nxt;
+        }
         }
         CU(cudaStreamSynchronize(s->copy_stream));
     }

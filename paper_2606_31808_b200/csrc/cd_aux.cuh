@@ -77,6 +77,39 @@ __global__ void loop_init_kernel(int B, int max_steps, int start, int start_acce
     if (tid == 0) *n_active = (start_accepting || (sat_ctr && *sat_ctr >= limit)) ? 0 : B;
 }
 
+// Host-buffer loop (cd_decode_loop_host) when the caller's logits are in pinned, device-mapped host
+// memory: the rows still active are pulled over PCIe by the SMs themselves, straight from the host
+// buffer into the compact staging buffer (row = slot) -- no host read of the active list, no
+// per-row copy calls.  16-byte loads, 4 independent ones per thread in flight.
+__global__ void host_gather_rows_kernel(const unsigned char* __restrict__ src, unsigned long long row_bytes,
+                                        const int* __restrict__ row_ids, const int* __restrict__ n_dev,
+                                        unsigned char* __restrict__ dst) {
+    const int n = __ldcg(n_dev);
+    const unsigned long long vec_per_row = row_bytes >> 4;
+    const unsigned long long total = (unsigned long long)n * vec_per_row;
+    const unsigned long long nth = (unsigned long long)gridDim.x * blockDim.x;
+    unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + 3 * nth < total; i += 4 * nth) {
+        uint4 v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const unsigned long long j = i + q * nth;
+            const unsigned long long slot = j / vec_per_row, off = j - slot * vec_per_row;
+            v[q] = *reinterpret_cast<const uint4*>(src + (unsigned long long)__ldg(row_ids + slot) * row_bytes + (off << 4));
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const unsigned long long j = i + q * nth;
+            reinterpret_cast<uint4*>(dst)[j] = v[q];
+        }
+    }
+    for (; i < total; i += nth) {
+        const unsigned long long slot = i / vec_per_row, off = i - slot * vec_per_row;
+        reinterpret_cast<uint4*>(dst)[i] =
+            *reinterpret_cast<const uint4*>(src + (unsigned long long)__ldg(row_ids + slot) * row_bytes + (off << 4));
+    }
+}
+
 // Measurement aid (cd_probe_read): the copy machinery of the step kernel -- per-warp rings of 1-D bulk
 // async copies on mbarriers, 12 warps x 2 stages x 8 KiB per SM -- streaming a buffer with NO arithmetic
 // (one word per tile is read so the copy is not dead).  What it reaches is the ceiling of a pure-read
