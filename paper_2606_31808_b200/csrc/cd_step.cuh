@@ -48,6 +48,8 @@ constexpr int FLAG_ACCEPT = 4;  // pseudo tile of a slot whose state already acc
 constexpr int FLAG_BADSTATE = 8;
 constexpr int FLAG_GATHER = 16;  // pseudo tile of a gathered row piece (no copy); meta.tile = logits row
 
+constexpr int SAMPLE_LIST_CAP = 128;  // tiles with at most this many allowed elements are compacted (SAMPLE)
+
 constexpr int GATHER_CHUNK = 256;  // a gathered row is split into pieces of >= this many transitions
 constexpr int GATHER_UNROLL = 8;   // independent gathers per lane in flight
 
@@ -127,6 +129,7 @@ struct __align__(128) WarpRing {
     unsigned char mask[STAGES][TILE_BYTES / 16];  // bf16: TILE_BYTES/2 tokens / 8; fp32 uses half
     TileMeta meta[STAGES];
     unsigned long long bar[STAGES];
+    unsigned short list[SAMPLE_LIST_CAP];  // SAMPLE: positions of a tile's allowed elements, compacted
 };
 
 // tiles per unit for n active rows (host mirrors this in cd_api.cu: step_units_cap)
@@ -465,6 +468,47 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
             uint32_t bits[WPL];
 #pragma unroll
             for (int j = 0; j < WPL; ++j) bits[j] = mw[j * 32 + lane];
+            // SAMPLE, sparse tile: the noise costs ~60 instructions per evaluation, so the allowed
+            // positions are first compacted across the warp (exclusive scan of the per-lane popcounts
+            // in (word, lane) = ascending token order, positions written to a small shared list) and
+            // each lane then evaluates exactly the elements of rank lane, lane + 32, ... (ascending per
+            // lane, so "replace on strictly greater" still keeps the lowest id).
+            bool compacted = false;
+            if constexpr (SAMPLE) {
+                int cnt[WPL], offs[WPL], total = 0;
+#pragma unroll
+                for (int j = 0; j < WPL; ++j) {
+                    cnt[j] = __popc(bits[j]);
+                    int inc = cnt[j];
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int up = __shfl_up_sync(FULL, inc, o);
+                        if (lane >= o) inc += up;
+                    }
+                    offs[j] = total + inc - cnt[j];
+                    total += __shfl_sync(FULL, inc, 31);
+                }
+                if (total <= SAMPLE_LIST_CAP) {
+                    compacted = true;
+#pragma unroll
+                    for (int j = 0; j < WPL; ++j) {
+                        uint32_t b = bits[j];
+                        int o = offs[j];
+                        const int e0 = (j * 32 + lane) * 32;
+                        while (b != 0u) {
+                            ring.list[o++] = (unsigned short)(e0 + __ffs(b) - 1);
+                            b &= b - 1u;
+                        }
+                    }
+                    __syncwarp();
+                    for (int r = lane; r < total; r += 32) {
+                        const int e = ring.list[r];
+                        online_update_sample(m, s, kb, idx, tile_elem<DT>(tile, e), t0 + e, t0 + e, a.inv_tau, row_key);
+                    }
+                    __syncwarp();
+                }
+            }
+            if (!compacted) {
 #pragma unroll
             for (int j = 0; j < WPL; ++j) {
                 // warp-uniform trip count (max popcount over the lanes); idle lanes feed -inf
@@ -480,6 +524,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                     else
                         online_update(m, s, idx, x, t0 + e);
                 }
+            }
             }
             }
             if (mt.flags & FLAG_LAST) {
