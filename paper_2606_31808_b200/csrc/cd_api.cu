@@ -980,7 +980,7 @@ cd_status make_tmap_bf16(CUtensorMap* out, const void* base, long long rows, lon
 }
 
 cd_status get_head_scratch(Scratch* s, int rows, int H, cudaStream_t stream) {
-    if (s->head_rows >= rows && s->head_H >= H) return CD_OK;
+    if (s->head_rows >= rows && s->head_H == H) return CD_OK;  // the A tensor map is built for exactly H columns
     if (s->head_rows > 0) CU(cudaStreamSynchronize(stream));
     cudaFree(s->h_flags); cudaFree(s->h_lists); cudaFree(s->h_ctr); cudaFree(s->h_A); cudaFree(s->h_partials);
     s->h_flags = nullptr; s->h_lists = nullptr; s->h_ctr = nullptr; s->h_A = nullptr; s->h_partials = nullptr;

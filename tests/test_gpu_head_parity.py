@@ -370,3 +370,16 @@ def test_head_loop_many_rows(cd, oracle, mode):
     for k in ("tokens", "len", "final_state", "done"):
         assert np.array_equal(got[k].cpu().numpy(), want[k]), k
     assert want["n_active_hist"][1] > 4096
+
+
+def test_head_step_changing_hidden_size_on_one_handle(cd, oracle):
+    """One handle / stream used with H = 200, then H = 72, then H = 200 again (K tails in both): the packed
+    A operand and its tensor map must follow H."""
+    V, S, n = 900, 6, 70
+    aut = wl.make_random_dfa(83, V, S, 0.3, 0.2)
+    dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device="cuda:0")
+    dfa.set_head_gather_max(0)
+    for H in (200, 72, 200, 8):
+        hid = wl.make_hidden(83 + H, 0, n, H, exact=True)
+        W = wl.make_head(83 + H, V, H, 2.0, exact=True)
+        run_case(cd, oracle, aut, dfa, hid, W, H, live_states(aut, n))
