@@ -348,7 +348,8 @@ CD_API cd_status cd_head_decode_loop(const cd_dfa_t* dfa, const void* const* ste
  * cd_head_decode_loop on logits or hidden states of those rows) and broadcasts the results
  * back with cd_join_results: out[i] = in[rep[i]] for the five loop outputs (tokens
  * [., max_steps]); an output pointer may be NULL to skip it.  Asynchronous on cuda_stream;
- * scratch is stream-ordered (cudaMallocAsync).  Errors: CD_ERR_ARG, CD_ERR_CUDA, CD_ERR_OOM.
+ * scratch is stream-ordered (cudaMallocAsync).  N <= 2^30 per call.  Errors: CD_ERR_ARG, CD_ERR_CUDA,
+ * CD_ERR_OOM.
  */
 CD_API cd_status cd_dedup(const int64_t* keys, int32_t N, int32_t* rep_out, int32_t* distinct_rows_out,
                    int32_t* n_distinct_out, void* cuda_stream);

@@ -1427,6 +1427,7 @@ cd_status cd_dedup(const int64_t* keys, int32_t N, int32_t* rep_out, int32_t* di
         return CD_OK;
     }
     if (!keys || !rep_out || !distinct_rows_out) return fail(CD_ERR_ARG, "NULL pointer");
+    if (N > (1 << 30)) return fail(CD_ERR_ARG, "N (%d) exceeds 2^30 rows per call", N);  // table of 2N..4N 32-bit slots
     uint32_t cap = 1024;
     while (cap < 2ull * (uint32_t)N) cap <<= 1;
     // stream-ordered scratch: table keys [cap + 1], table min rows [cap + 1], first [N], rank [N], flags [N]
