@@ -224,6 +224,8 @@ long long step_units_cap(const cd_dfa* d, long long n) {
 cd_status get_scratch(const cd_dfa* cd_, cudaStream_t stream, int rows, bool loop_bufs, Scratch** out) {
     cd_dfa* d = const_cast<cd_dfa*>(cd_);
     std::lock_guard<std::mutex> lk(d->mu);
+    if ((long long)rows * (tiles_per_row(d->dev.V, CD_F32) + 1) >= 0x7FFFFFFFLL)
+        return fail(CD_ERR_ARG, "rows (%d) * tiles per row overflows the unit index", rows);
     Scratch& s = d->scratch[stream];
     if (rows < 1) rows = 1;
     if (s.cap_rows < rows) {
