@@ -5,6 +5,7 @@ Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
 """
 from .oracle_cd import (  # noqa: F401
     OracleError,
+    asan_runtime,
     build,
     compact,
     decode_loop,
@@ -21,3 +22,4 @@ from .oracle_cd import (  # noqa: F401
     step,
     validate,
 )
+from .oracle_types import TypeAutomaton, language_dfa, list_language, trie_eos  # noqa: F401

@@ -17,6 +17,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "oracle_cd.c")
 _SO = os.path.join(_HERE, "liboracle_cd.so")
+_SO_SAN = os.path.join(_HERE, "liboracle_cd_san.so")
 _lib = None
 
 F32, BF16 = 0, 1
@@ -29,22 +30,32 @@ class OracleError(RuntimeError):
         self.code = code
 
 
-def build(force: bool = False) -> str:
+def build(force: bool = False, sanitize: bool = False) -> str:
     """gcc -O2 the oracle into oracle/liboracle_cd.so (no -ffast-math: the
-    summation order and exp/log are the definition)."""
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        tmp = _SO + f".tmp{os.getpid()}"
+    summation order and exp/log are the definition).  sanitize=True builds
+    oracle/liboracle_cd_san.so with AddressSanitizer + UndefinedBehaviorSanitizer
+    (loaded by a process started with LD_PRELOAD=libasan and
+    ORACLE_CD_SANITIZE=1, see tests/test_oracle_sanitized.py)."""
+    so = _SO_SAN if sanitize else _SO
+    if force or not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
+        tmp = so + f".tmp{os.getpid()}"
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer"] if sanitize else ["-O2"]
         subprocess.check_call(
-            ["gcc", "-O2", "-ffp-contract=off", "-std=c11", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"]
+            ["gcc"] + flags + ["-ffp-contract=off", "-std=c11", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC, "-lm"]
         )
-        os.replace(tmp, _SO)
-    return _SO
+        os.replace(tmp, so)
+    return so
+
+
+def asan_runtime() -> str:
+    """Path of gcc's libasan.so (to LD_PRELOAD into the python process that loads the sanitized oracle)."""
+    return subprocess.check_output(["gcc", "-print-file-name=libasan.so"], text=True).strip()
 
 
 def _load():
     global _lib
     if _lib is None:
-        _lib = C.CDLL(build())
+        _lib = C.CDLL(build(sanitize=os.environ.get("ORACLE_CD_SANITIZE") == "1"))
         _lib.orc_validate.restype = C.c_int
         _lib.orc_step.restype = C.c_int
         _lib.orc_compact.restype = C.c_int
