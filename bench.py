@@ -37,19 +37,24 @@ METRIC = "constrained-step rows/s and HBM GB/s (% of B200 peak) at V=262144"
 UNIT = "rows/s"
 NOMINAL_HBM_GBS = 8000.0
 FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the step kernel from the
-# `ncu --set full` capture summarised in profiles/ (None until a capture exists for this
-# workload); keyed by config name.
 FALLBACK_BF16_TFLOPS = 1590.0  # /opt/skills/guides/B200_PROFILING.md fallback
-# DRAM read + write bytes of one head_dense_kernel launch from the ncu --set full capture in profiles/
-NCU_HEAD_TRAFFIC_BYTES = {
-    # profiles/r1e_head_dense_c4.md: 1,644,181,000 read + 6,551,040 written
-    "c4": 1644181000 + 6551040,
-}
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {
-    # profiles/r1c_step_kernel_c4.md, step 0 (n = 4096): 2,148,744,000 read + 4,729,344 written
-    "c4": 2148744000 + 4729344,
-}
+READ_RATE_GBS = 7200.0  # the kernel's own pure-read probe on this pool (cd_probe_read): used for the fixed-cost estimate only
+
+
+def ncu_traffic(kernel: str, config: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of `kernel` on `config` from the committed
+    `ncu --set full` captures, listed in profiles/ncu_traffic.csv (kernel,config,dram_read_bytes,
+    dram_write_bytes,profile,note).  Not measured in this run (never profile a timed run): the JSON names
+    the capture it comes from; None if no capture of that kernel / config is committed."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.csv")
+    try:
+        for line in open(path):
+            p = [x.strip() for x in line.split(",")]
+            if len(p) >= 5 and p[0] == kernel and p[1] == config:
+                return {"bytes": int(p[2]) + int(p[3]), "profile": p[4]}
+    except Exception:
+        pass
+    return None
 
 
 def parse_args():
@@ -71,6 +76,12 @@ def parse_args():
     ap.add_argument("--head-H", type=int, default=2560, help="hidden size of the LM head (Gemma 3 4B: 2560)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--verbose", action="store_true", help="per-launch table of the step kernel on stderr")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="weak: every rank decodes its own batches (default); strong: ONE batch of B rows is "
+                         "sharded B/N rows per rank (SURVEY 8(e): contiguous row ranges, no collective)")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the c1-c3 block (per_config)")
+    ap.add_argument("--loop-mode", default="auto", choices=["auto", "per_step"],
+                    help="auto: cd_decode_loop as ONE persistent kernel (default); per_step: one launch per decoding step")
     return ap.parse_args()
 
 
@@ -263,7 +274,8 @@ def head_section(cd, cfg, aut, dfa, device, H, iters, warmup):
                      "peak_source": src, "frac_of_sustained_peak": ach / sustained if sustained else None,
                      "frac_of_nominal_2250": ach / 2250.0, "flops_per_launch": flops,
                      "note": "timed over the whole call (prepare + pack + contraction + finish), so the kernel's own rate is higher",
-                     "traffic": NCU_HEAD_TRAFFIC_BYTES.get(cfg.name)},
+                     "traffic": (ncu_traffic("cd::head_dense_kernel", cfg.name) or {}).get("bytes"),
+                     "traffic_source": (ncu_traffic("cd::head_dense_kernel", cfg.name) or {}).get("profile")},
     }
     return head
 
@@ -312,15 +324,166 @@ def dedup_section(cd, device, iters, warmup):
                     "negligible next to the decode loop they remove (256 batches x ~4 ms)"}
 
 
-def build_inputs(cfg, device, n_batches, batch0):
+def build_inputs(cfg, device, n_batches, batch0, rows=None):
     aut = wl.build_automaton(cfg, device=device)
-    batches = [wl.build_step_logits(cfg, aut, device=device, batch=batch0 + b) for b in range(n_batches)]
+    batches = [wl.build_step_logits(cfg, aut, device=device, batch=batch0 + b, rows=rows) for b in range(n_batches)]
     return aut, batches
 
 
 def bytes_per_row_step(cfg):
     sz = 2 if cfg.dtype == torch.bfloat16 else 4
     return cfg.V * sz, cfg.V // 8
+
+
+def replay_stepwise(cd, cfg, aut, dfa, logits, device, timed):
+    """One decode loop of `logits` driven through the stepwise API (cd_step + cd_compact) with the active
+    count read back after every step: gives, per decoding step, the active rows n_k, the number of
+    distinct automaton states among them (each costs one 32 KiB mask row from HBM) and the
+    sum of their out-degrees.  timed=True replays it once more with everything enqueued ahead of the GPU
+    (a device-side sleep first, no host sync, preallocated outputs) and a CUDA event pair around every
+    cd_step launch, so that the events bracket the kernel itself and not the host's launch gaps."""
+    stream = torch.cuda.current_stream()
+    B = logits[0].shape[0]
+    i32 = dict(dtype=torch.int32, device=device)
+    deg_dev = torch.diff(torch.as_tensor(aut.row_ptr)).to(device)
+    bufs = dict(tok=torch.empty(B, **i32), lp=torch.empty(B, dtype=torch.float32, device=device),
+                done=torch.empty(B, dtype=torch.uint8, device=device),
+                ids=[torch.empty(B, **i32) for _ in range(2)], st=[torch.empty(B, **i32) for _ in range(2)],
+                na=torch.empty(1, **i32))
+    n_k, distinct_k, deg_k, step_ms = [], [], [], []
+    for rep in range(2 if timed else 1):
+        bufs["ids"][0].copy_(torch.arange(B, **i32))
+        bufs["st"][0].fill_(aut.start)
+        events = []
+        if rep == 1:
+            torch.cuda.synchronize()
+            torch.cuda._sleep(600000)
+        n = B
+        for k in range(cfg.max_steps):
+            cur, nxt = k & 1, (k + 1) & 1
+            if rep == 0:
+                if n == 0:
+                    break
+                n_k.append(n)
+                distinct_k.append(int(torch.unique(bufs["st"][cur][:n]).numel()))
+                deg_k.append(int(deg_dev[bufs["st"][cur][:n].long()].sum()))
+            elif k >= len(n_k):
+                break
+            else:
+                n = n_k[k]
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            cd.step(dfa, logits[k], bufs["st"][cur], row_map=bufs["ids"][cur], n=n, want_lse=False,
+                    out=(bufs["tok"], bufs["lp"], None, bufs["done"]))
+            b.record(stream)
+            events.append((a, b))
+            cd.compact(bufs["done"], bufs["ids"][cur], bufs["st"][cur], n=n,
+                       out=(bufs["ids"][nxt], bufs["st"][nxt], bufs["na"]))
+            if rep == 0:
+                n = int(bufs["na"])
+        torch.cuda.synchronize()
+        if rep == 1:
+            step_ms = [a.elapsed_time(b) for a, b in events]
+    return n_k, distinct_k, deg_k, step_ms
+
+
+def measure_loop(cd, cfg, aut, dfa, batches, device, steps, warmup, peak, verbose=False, label=""):
+    """The decode loop of one configuration: K timed cd_decode_loop calls over the rotated resident
+    batches (CUDA events on the launching stream), then the per-step picture of the persistent kernel
+    from its own device-side trace (cd_loop_trace: active rows and nanoseconds per decoding step) with
+    the algorithmic bytes of every step (n_k logits rows + one mask row per distinct state)."""
+    stream = torch.cuda.current_stream()
+    sz_logit, sz_mask = bytes_per_row_step(cfg)
+    out = None
+    per_batch = []
+    for b, logits in enumerate(batches):  # untimed: per-step n_k / distinct states / bytes of every resident batch
+        n_k, distinct_k, deg_k, _ = replay_stepwise(cd, cfg, aut, dfa, logits, device, timed=False)
+        per_batch.append(dict(n=n_k, distinct=distinct_k, deg=deg_k,
+                              bytes=[n * sz_logit + d * sz_mask for n, d in zip(n_k, distinct_k)]))
+    for i in range(warmup):
+        out = cd.decode_loop(dfa, batches[i % len(batches)], max_steps=cfg.max_steps, out=out)
+    torch.cuda.synchronize()
+    l0 = cd.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(steps):
+        out = cd.decode_loop(dfa, batches[(warmup + i) % len(batches)], max_steps=cfg.max_steps, out=out)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    launches = cd.launch_count() - l0
+    ms = e0.elapsed_time(e1) / steps
+    timed = [(warmup + i) % len(batches) for i in range(steps)]
+    loop_bytes = sum(sum(per_batch[b]["bytes"]) for b in timed) / steps
+    row_steps = sum(sum(per_batch[b]["n"]) for b in timed) / steps
+    # the last timed loop, step by step, from the kernel's own trace
+    last = per_batch[timed[-1]]
+    tr_n, tr_ns = dfa.loop_trace()
+    res = {
+        "B": cfg.B, "max_steps": cfg.max_steps, "resident_batches": len(batches), "loops_timed": steps,
+        "rows_per_s": cfg.B / (ms * 1e-3), "ms_per_loop": ms, "row_steps_per_loop": row_steps,
+        "gpu_launches_per_loop": launches / steps,
+        "loop_gbs": loop_bytes / (ms * 1e-3) / 1e9,
+        "frac_of_measured_peak": loop_bytes / (ms * 1e-3) / 1e9 / peak,
+        "frac_of_nominal_8TBs": loop_bytes / (ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+        "bytes_per_loop": loop_bytes,
+        "n_per_step": last["n"],
+    }
+    if tr_n and tr_n == last["n"]:
+        us = [t / 1e3 for t in tr_ns]
+        gbs = [b / (t * 1e-9) / 1e9 for b, t in zip(last["bytes"], tr_ns)]
+        fixed = [u - b / (READ_RATE_GBS * 1e3) for u, b in zip(us, last["bytes"])]
+        kern_us = sum(us)
+        k0 = max(range(len(us)), key=lambda k: last["bytes"][k])
+        res.update({
+            "kernel": "cd::loop_kernel (one cooperative launch per loop)",
+            "kernel_us_per_loop": kern_us,
+            "kernel_gbs": sum(last["bytes"]) / (kern_us * 1e-6) / 1e9,
+            "kernel_frac_of_measured_peak": sum(last["bytes"]) / (kern_us * 1e-6) / 1e9 / peak,
+            "kernel_frac_of_nominal_8TBs": sum(last["bytes"]) / (kern_us * 1e-6) / 1e9 / NOMINAL_HBM_GBS,
+            "largest_step": {"n": last["n"][k0], "us": us[k0], "gbs": gbs[k0], "frac_of_measured_peak": gbs[k0] / peak,
+                             "frac_of_nominal_8TBs": gbs[k0] / NOMINAL_HBM_GBS},
+            "us_per_step": [round(u, 2) for u in us],
+            "gbs_per_step": [round(g, 0) for g in gbs],
+            "fixed_us_per_step_avg": sum(fixed) / len(fixed),
+            "fixed_cost_note": f"step time minus its bytes at the kernel's pure-read rate ({READ_RATE_GBS:.0f} GB/s)",
+        })
+        if verbose:
+            for k, (n, u, g, f) in enumerate(zip(last["n"], us, gbs, fixed)):
+                print(f"  {label} step {k:2d}: n={n:5d} distinct={last['distinct'][k]:5d} {u:8.1f} us {g:7.0f} GB/s "
+                      f"fixed {f:5.1f} us", file=sys.stderr)
+    else:
+        res["kernel"] = "cd::step_kernel (one launch per decoding step)"
+    return res, per_batch, out
+
+
+def per_config_section(cd, device, peak, verbose):
+    """BASELINE.json configs c1-c3 beside the c4 headline (north_star: "on all five configs", ">= 70 % ... at
+    V = 262144, B >= 1024" covers c2): the same event protocol; 4 resident batches for c1 / c2 and 2 for c3 (a
+    loop streams 0.27 / 1.9 / 2.7 GB of distinct logits, all larger than the 126 MB L2, and consecutive loops
+    use different batches)."""
+    out = {}
+    for name, nb, k in (("c1", 4, 40), ("c2", 4, 20), ("c3", 2, 10)):
+        cfg = wl.CONFIGS[name]
+        aut, batches = build_inputs(cfg, device, nb, 0)
+        dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device=device)
+        dfa.reserve(cfg.B)
+        res, _, _ = measure_loop(cd, cfg, aut, dfa, batches, device, k, 5, peak, verbose=verbose, label=name)
+        # the same loops as one launch per decoding step (the round-1 path; still what the callback / host forms use)
+        dfa.set_loop_mode(cd.LOOP_PER_STEP)
+        ps, _, _ = measure_loop(cd, cfg, aut, dfa, batches, device, k, 5, peak)
+        res["per_step_launches"] = {"rows_per_s": ps["rows_per_s"], "ms_per_loop": ps["ms_per_loop"], "loop_gbs": ps["loop_gbs"],
+                                    "frac_of_measured_peak": ps["frac_of_measured_peak"]}
+        dfa.set_loop_mode(cd.LOOP_AUTO)
+        # density-adaptive (tries never need the scan)
+        dfa.set_gather_max(-1)
+        ga, _, _ = measure_loop(cd, cfg, aut, dfa, batches, device, k, 5, peak)
+        res["adaptive_rows_per_s"] = ga["rows_per_s"]
+        dfa.close()
+        del batches
+        torch.cuda.empty_cache()
+        res["workload"] = cfg.desc
+        out[name] = res
+    return out
 
 
 def run_reference(args, rank):
@@ -387,14 +550,34 @@ def main():
 
     cfg = wl.CONFIGS[args.config]
     sz_logit, sz_mask = bytes_per_row_step(cfg)
-    # weak scaling: every rank decodes its own batches of the table (rows are
-    # independent, the automaton is replicated, no collective on the data path)
-    aut, batches = build_inputs(cfg, device, args.batches, batch0=rank * args.batches)
+    peak, peak_src = measured_peak()
+    stream = torch.cuda.current_stream()
+
+    # ---------------- c1-c3 beside the headline (rank 0; untimed for the others, who wait at the barrier)
+    per_config = None
+    if rank == 0 and not args.no_per_config and args.config == "c4" and args.gather_max == 0 and args.loop_mode == "auto":
+        try:
+            per_config = per_config_section(cd, device, peak, args.verbose)
+        except Exception as ex:
+            per_config = {"error": str(ex)[:300]}
+
+    # weak scaling (default): every rank decodes its own batches of the table; strong scaling: ONE batch,
+    # rank r takes the contiguous rows [r*B/N, (r+1)*B/N) (rows are independent, the automaton
+    # is replicated, the concatenation of the ranks' results in rank order is the batch's -- no collective
+    # on the data path)
+    if args.scaling == "strong":
+        lo, hi = wl.shard_rows(cfg.B, world, rank)
+        aut, batches = build_inputs(cfg, device, args.batches, batch0=0, rows=(lo, hi))
+        cfg = wl.scaled(cfg, B=hi - lo)
+        rows_per_step_all_ranks = wl.CONFIGS[args.config].B
+    else:
+        aut, batches = build_inputs(cfg, device, args.batches, batch0=rank * args.batches)
+        rows_per_step_all_ranks = cfg.B * world
     dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device=device)
     dfa.reserve(cfg.B)
     dfa.set_gather_max(args.gather_max)
+    dfa.set_loop_mode(cd.LOOP_AUTO if args.loop_mode == "auto" else cd.LOOP_PER_STEP)
     out = None
-    stream = torch.cuda.current_stream()
 
     def one_step(i):
         nonlocal out
@@ -405,11 +588,18 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    # row-steps of every resident batch (untimed): sum of generated lengths
-    rs_batch = []
-    for b in range(len(batches)):
-        one_step(b)
-        rs_batch.append(int(out["len"].sum()))
+    # per-step active rows / distinct states / algorithmic bytes of every resident batch (untimed, through
+    # the stepwise API); the event-timed replay of batch 0 gives the per-launch numbers of cd::step_kernel
+    per_batch = []
+    step_ms = []
+    for b, logits in enumerate(batches):
+        n_k, distinct_k, deg_k, t_k = replay_stepwise(cd, cfg, aut, dfa, logits, device, timed=(b == 0))
+        per_batch.append(dict(n=n_k, distinct=distinct_k, deg=deg_k,
+                              bytes=[n * sz_logit + d * sz_mask for n, d in zip(n_k, distinct_k)]))
+        if b == 0:
+            step_ms = t_k
+    deg_k = per_batch[0]["deg"]
+    deg_dev = torch.diff(torch.as_tensor(aut.row_ptr)).to(device)
     for i in range(args.warmup):
         one_step(i)
     barrier()
@@ -426,89 +616,84 @@ def main():
     launches = cd.launch_count() - launches0
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1)
+    tr_n, tr_ns = dfa.loop_trace()  # the last timed loop, step by step, from the persistent kernel's own trace
     if dist is not None:
         t = torch.tensor([ms], device=device)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t[0])
-    value = cfg.B * args.steps * world / (ms * 1e-3)
+    value = rows_per_step_all_ranks * args.steps / (ms * 1e-3)
+    timed = [(args.warmup + i) % len(batches) for i in range(args.steps)]
+    row_steps_timed = sum(sum(per_batch[b]["n"]) for b in timed)
+    row_steps = row_steps_timed / args.steps
+    bytes_timed = sum(sum(per_batch[b]["bytes"]) for b in timed)
 
-    # ---------------- roofline of the dominant kernel (fused step), live, per launch:
-    # the same loop driven through cd_step / cd_compact with CUDA events around every
-    # cd_step launch on the launching stream.
-    peak, peak_src = measured_peak()
-    # Repetition 0 walks the loop with host reads of the active count (gives n_k and the number
-    # of distinct states per step); repetition 1 replays it with everything enqueued ahead of
-    # the GPU (a ~0.3 ms device-side sleep first, no host sync, preallocated outputs), so that
-    # the events bracket the kernel itself and not the host's launch gaps.
-    step_ms, step_bytes, step_rows = [], [], []
-    logits = batches[0]
-    n_k, distinct_k, deg_k = [], [], []
-    deg_dev = torch.diff(torch.as_tensor(aut.row_ptr)).to(device)
-    i32 = dict(dtype=torch.int32, device=device)
-    bufs = dict(tok=torch.empty(cfg.B, **i32), lp=torch.empty(cfg.B, dtype=torch.float32, device=device),
-                done=torch.empty(cfg.B, dtype=torch.uint8, device=device),
-                ids=[torch.empty(cfg.B, **i32) for _ in range(2)], st=[torch.empty(cfg.B, **i32) for _ in range(2)],
-                na=torch.empty(1, **i32))
-    for rep in range(2):
-        bufs["ids"][0].copy_(torch.arange(cfg.B, **i32))
-        bufs["st"][0].fill_(aut.start)
-        events = []
-        if rep == 1:
-            torch.cuda.synchronize()
-            torch.cuda._sleep(600000)
-        n = cfg.B
-        for k in range(cfg.max_steps):
-            cur, nxt = k & 1, (k + 1) & 1
-            if rep == 0:
-                if n == 0:
-                    break
-                n_k.append(n)
-                distinct_k.append(int(torch.unique(bufs["st"][cur][:n]).numel()))
-                deg_k.append(int(deg_dev[bufs["st"][cur][:n].long()].sum()))
-            elif k >= len(n_k):
-                break
-            else:
-                n = n_k[k]
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            cd.step(dfa, logits[k], bufs["st"][cur], row_map=bufs["ids"][cur], n=n, want_lse=False,
-                    out=(bufs["tok"], bufs["lp"], None, bufs["done"]))
-            b.record(stream)
-            events.append((a, b))
-            cd.compact(bufs["done"], bufs["ids"][cur], bufs["st"][cur], n=n,
-                       out=(bufs["ids"][nxt], bufs["st"][nxt], bufs["na"]))
-            if rep == 0:
-                n = int(bufs["na"])
-        torch.cuda.synchronize()
-        if rep == 1:
-            for k, (a, b) in enumerate(events):
-                step_ms.append(a.elapsed_time(b))
-                step_bytes.append(n_k[k] * sz_logit + distinct_k[k] * sz_mask)
-                step_rows.append(n_k[k])
-    if args.verbose and rank == 0:
-        for k, (mm, bb, rr) in enumerate(zip(step_ms, step_bytes, step_rows)):
-            print(f"  step {k:2d}: n={rr:5d} distinct_states={distinct_k[k]:5d} {1e3 * mm:8.1f} us "
-                  f"{bb / (mm * 1e-3) / 1e9:7.0f} GB/s", file=sys.stderr)
-    # pure-read ceiling of the kernel's own copy machinery on this GPU, measured live on one step's logits
+    # ---------------- roofline of the dominant kernel, live.
+    # The whole loop is ONE launch of cd::loop_kernel, so "per launch" = per loop: algorithmic bytes of the
+    # loop (every step's active rows x 512 KiB of logits + one 32 KiB mask row per distinct state) over the
+    # CUDA-event duration of the timed region / K.  That duration also contains the loop's set-up kernel
+    # and the host's hand-over between loops, so it is a lower bound of the kernel's own rate; the kernel's
+    # device-side trace (cd_loop_trace) gives the per-step times of the last loop beside it.
     try:
-        read_probe = cd.probe_read(logits[0], iters=10)
+        read_probe = cd.probe_read(batches[0][0], iters=10)
     except Exception:
         read_probe = None
-    tot_bytes, tot_ms = sum(step_bytes), sum(step_ms)
-    achieved = tot_bytes / (tot_ms * 1e-3) / 1e9
-    best = max(bb / (mm * 1e-3) / 1e9 for bb, mm in zip(step_bytes, step_ms))
+    achieved = bytes_timed / (ms * 1e-3) / 1e9
+    persistent = bool(tr_n) and tr_n == per_batch[timed[-1]]["n"]
+    kname = "cd::loop_kernel" if persistent else "cd::step_kernel"
+    tinfo = ncu_traffic(kname, cfg.name)
     roofline = {
-        "bound": "hbm", "kernel": "cd::step_kernel (fused mask + masked logsumexp/argmax + CSR transition)",
+        "bound": "hbm",
+        "kernel": ("cd::loop_kernel (persistent: the whole decode loop in one cooperative launch; per step: fused mask + "
+                   "masked logsumexp/argmax + transition, grid barrier)") if persistent else
+                  "cd::step_kernel (fused mask + masked logsumexp/argmax + CSR transition), one launch per decoding step",
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
-        "best_launch_gbs": best, "launches_timed": len(step_ms),
+        "launches_timed": args.steps if persistent else int(row_steps and sum(len(per_batch[b]["n"]) for b in timed)),
+        "bytes_per_launch_avg": bytes_timed / args.steps if persistent else bytes_timed / max(1, sum(len(per_batch[b]["n"]) for b in timed)),
+        "us_per_launch_avg": 1e3 * ms / args.steps if persistent else 1e3 * ms / max(1, sum(len(per_batch[b]["n"]) for b in timed)),
+        "duration_note": "CUDA events around the K timed cd_decode_loop calls / K (includes the set-up kernel and the host hand-over)",
         "read_probe_gbs": read_probe, "frac_of_read_probe": (achieved / read_probe) if read_probe else None,
-        "bytes_per_launch_avg": tot_bytes / max(1, len(step_ms)), "us_per_launch_avg": 1e3 * tot_ms / max(1, len(step_ms)),
-        "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(cfg.name),
-        "step_kernel_share_of_loop": (tot_ms / (ms / args.steps)),
+        "traffic": tinfo["bytes"] if tinfo else None,
+        "traffic_source": (f"committed ncu --set full capture {tinfo['profile']} (one launch; not measured in this run)"
+                           if tinfo else None),
     }
-    row_steps_timed = sum(rs_batch[(args.warmup + i) % len(batches)] for i in range(args.steps))
-    row_steps = row_steps_timed / args.steps
+    if persistent:
+        last = per_batch[timed[-1]]
+        us = [t / 1e3 for t in tr_ns]
+        kern_us = sum(us)
+        gbs = [b / (t * 1e-9) / 1e9 for b, t in zip(last["bytes"], tr_ns)]
+        roofline["device_trace"] = {
+            "kernel_us_last_loop": kern_us, "kernel_gbs_last_loop": sum(last["bytes"]) / (kern_us * 1e-6) / 1e9,
+            "kernel_frac_of_measured_peak": sum(last["bytes"]) / (kern_us * 1e-6) / 1e9 / peak,
+            "kernel_share_of_loop_time": kern_us / (1e3 * ms / args.steps),
+            "n_per_step": last["n"], "us_per_step": [round(u, 1) for u in us], "gbs_per_step": [round(g) for g in gbs],
+            "best_step_gbs": max(gbs),
+            "fixed_us_per_step_avg": sum(u - b / (READ_RATE_GBS * 1e3) for u, b in zip(us, last["bytes"])) / len(us),
+        }
+        if args.verbose and rank == 0:
+            for k, (n, u, g) in enumerate(zip(last["n"], us, gbs)):
+                print(f"  loop_kernel step {k:2d}: n={n:5d} distinct_states={last['distinct'][k]:5d} {u:8.1f} us {g:7.0f} GB/s",
+                      file=sys.stderr)
+    # cd::step_kernel (what cd_step launches: the stepwise API, the callback / host-buffer loops), per launch,
+    # from the event-timed replay of batch 0
+    if step_ms:
+        sb = per_batch[0]["bytes"]
+        tot_b, tot_ms = sum(sb), sum(step_ms)
+        sk = ncu_traffic("cd::step_kernel", cfg.name)
+        roofline["step_kernel"] = {
+            "kernel": "cd::step_kernel (one launch per decoding step: cd_step)",
+            "achieved": tot_b / (tot_ms * 1e-3) / 1e9, "frac": tot_b / (tot_ms * 1e-3) / 1e9 / peak,
+            "frac_of_nominal_8TBs": tot_b / (tot_ms * 1e-3) / 1e9 / NOMINAL_HBM_GBS,
+            "best_launch_gbs": max(bb / (mm * 1e-3) / 1e9 for bb, mm in zip(sb, step_ms)),
+            "launches_timed": len(step_ms), "bytes_per_launch_avg": tot_b / len(step_ms),
+            "us_per_launch_avg": 1e3 * tot_ms / len(step_ms),
+            "traffic": sk["bytes"] if sk else None,
+            "traffic_source": f"committed ncu --set full capture {sk['profile']} (the n = {per_batch[0]['n'][0]} launch)" if sk else None,
+        }
+        if args.verbose and rank == 0:
+            for k, (mm, bb) in enumerate(zip(step_ms, sb)):
+                print(f"  step_kernel step {k:2d}: n={per_batch[0]['n'][k]:5d} {1e3 * mm:8.1f} us {bb / (mm * 1e-3) / 1e9:7.0f} GB/s",
+                      file=sys.stderr)
 
     # ---------------- density-adaptive step, reported beside the dense path:
     # the same loops with cd_set_gather_max(-1).  Its bytes are the bytes it touches (one 32-byte
@@ -535,7 +720,7 @@ def main():
         gathered = [dk for dk in deg_k]  # allowed logits per step of batch 0 (every row-step, if gathered)
         all_gathered = int(deg_dev.max()) <= auto_max
         adaptive = {
-            "value": cfg.B * args.steps * world / (ms_a * 1e-3), "unit": UNIT, "ms_per_step": ms_a / args.steps,
+            "value": rows_per_step_all_ranks * args.steps / (ms_a * 1e-3), "unit": UNIT, "ms_per_step": ms_a / args.steps,
             "speedup_vs_dense": ms / ms_a, "gather_max": int(auto_max), "every_state_gathered": bool(all_gathered),
             "allowed_logits_per_loop_batch0": int(sum(gathered)),
             "touched_bytes_per_loop_batch0": int(sum(gathered)) * 36 if all_gathered else None,
@@ -561,7 +746,7 @@ def main():
         ms_s = s0.elapsed_time(s1)
         rs_s = int(out["len"].sum())
         dfa.set_sampling(0.0)
-        sampling = {"value": cfg.B * args.steps * world / (ms_s * 1e-3), "unit": UNIT, "ms_per_step": ms_s / args.steps,
+        sampling = {"value": rows_per_step_all_ranks * args.steps / (ms_s * 1e-3), "unit": UNIT, "ms_per_step": ms_s / args.steps,
                     "slowdown_vs_greedy": ms_s / ms, "temperature": 1.0,
                     "row_steps_last_batch": rs_s,
                     "note": "Gumbel-max over the allowed set, counter-based noise per (row, step, token): one hash + two "
@@ -593,7 +778,7 @@ def main():
             steps_copied = int(out_h["len"].max())
             h2d = int(out_h["len"].sum()) * cfg.V * (2 if cfg.dtype == torch.bfloat16 else 4)
             d2h = cfg.B * (cfg.max_steps * 4 + 4 + 4 + 4 + 1) + 4 * steps_copied
-            e2e = {"value": cfg.B * k_e2e * world / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
+            e2e = {"value": rows_per_step_all_ranks * k_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": h2d,
                    "d2h_bytes_per_step": d2h, "steps": k_e2e, "ms_per_step": 1e3 * dt / k_e2e,
                    "h2d_gbs": h2d * k_e2e / dt / 1e9, "host_memory": "pinned"}
             got0 = cd.decode_loop(dfa, batches[0], max_steps=cfg.max_steps)
@@ -645,7 +830,7 @@ def main():
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": args.scaling,
             "vs_baseline": None, "dtype": "f32", "logits_dtype": "bf16" if cfg.dtype == torch.bfloat16 else "f32",
             "data": "synthetic",
             "config": {
@@ -654,15 +839,19 @@ def main():
                 "resident_batches": len(batches),
                 "l2": f"inputs larger than L2: {cfg.max_steps * cfg.B * sz_logit / 2**30:.1f} GiB of logits per step, "
                       f"{len(batches)} batches rotated",
-                "parallelism": f"rows sharded over {world} GPU(s), automaton replicated, no collective",
+                "parallelism": (f"one batch of {rows_per_step_all_ranks} rows sharded over {world} GPU(s) ({cfg.B} rows each)"
+                                if args.scaling == "strong" else f"every one of {world} GPU(s) decodes its own batches") +
+                               ", automaton replicated, no collective",
+                "loop_mode": args.loop_mode,
             },
             "row_steps_per_step": row_steps,
-            "row_steps_per_s": row_steps_timed * world / (ms * 1e-3),
+            "row_steps_per_s": row_steps_timed * world / (ms * 1e-3),  # rank 0's count x ranks
             "loop_gbs_per_gpu": row_steps_timed * sz_logit / (ms * 1e-3) / 1e9,
             "gpu_launches": launches,
             "clocks": clocks,
             "e2e": e2e,
             "roofline": roofline,
+            "per_config": per_config,
             "adaptive": adaptive,
             "sampling": sampling,
             "cpu_baseline": cpu,

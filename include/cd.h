@@ -33,11 +33,18 @@
  *     (a cudaStream_t passed as void*; NULL = legacy default stream) and do
  *     not synchronise with the host; cd_decode_loop* synchronise the stream
  *     once before returning;
- *   - a handle is immutable after cd_compile_*.  It may be used from several
- *     streams and host threads at once: scratch memory is kept per
- *     (handle, stream) and created on the first call that uses that stream
- *     (that first call allocates and therefore synchronises; cd_reserve does
- *     it ahead of time, e.g. before CUDA-graph capture);
+ *   - the automaton of a handle is immutable after cd_compile_*.  A handle may
+ *     be used from several streams and host threads at once: scratch memory is
+ *     kept per (handle, stream) and created on the first call that uses that
+ *     stream (that first call allocates and therefore synchronises; cd_reserve
+ *     does it ahead of time, e.g. before CUDA-graph capture).  The cd_set_*
+ *     calls change the handle's SETTINGS (gather thresholds, sampling, LIMIT,
+ *     loop mode): every entry point takes a snapshot of the settings when it
+ *     starts, under the handle's lock, so a setter may run at any time and
+ *     applies to the calls that start after it returns.  Settings are per
+ *     handle: two streams that need different settings use two handles (or
+ *     order their calls).  cd_set_satisfying overwrites the device copy of the
+ *     set in place: do not call it while a loop that uses a LIMIT is running;
  *   - logits rows start 16-byte aligned: the base pointer is 16-byte aligned
  *     and ld_elems * sizeof(element) is a multiple of 16; ld_elems >= V.
  *   - there is no CPU fallback: without a CUDA device every call fails with
@@ -67,8 +74,12 @@ typedef enum {
     CD_ERR_DEAD_STATE = 3, /* a non-accepting state has no transition: argmax over the empty set  */
     CD_ERR_CUDA = 4,       /* a CUDA runtime call failed (message in cd_last_error)               */
     CD_ERR_OOM = 5,        /* host or device allocation failed                                    */
-    CD_ERR_INTERNAL = 6    /* a device-side consistency check failed (state out of range, chosen
-                              token missing from the CSR); only cd_decode_loop* can report it     */
+    CD_ERR_INTERNAL = 6    /* a device-side consistency check failed during THIS loop (state out of
+                              range, chosen token missing from the CSR) or the persistent loop
+                              kernel gave up at a grid barrier; only cd_decode_loop* report it: the
+                              affected rows come back with done = 0 in the state they had.  cd_step
+                              is asynchronous and reports a slot whose state is outside [0, S)
+                              through its outputs only: token -1, logprob 0, done 1, state kept   */
 } cd_status;
 
 typedef enum { CD_F32 = 0, CD_BF16 = 1 } cd_dtype;
@@ -94,12 +105,30 @@ CD_API cd_status cd_compile_dfa(int32_t V, int32_t S, int32_t start, const int64
  * Sugar for boolean / option-set types (PAPER.md L61 `options`, L110-L133):
  * builds the trie automaton of K labels given as token-id sequences
  * label_tok[label_ptr[k] .. label_ptr[k+1]) (HOST pointers) and compiles it.
- * State 0 is the root, states are numbered in insertion order, one accepting
- * leaf per label.  Labels must be non-empty, distinct and prefix-free
- * (SURVEY 8(c) G5), else CD_ERR_AUTOMATON.
+ *   eos < 0   a row is finished the first time its state accepts: one
+ *             accepting leaf per label, so the final state names the label.  Labels must
+ *             be non-empty, distinct and prefix-free (G5: a label extending another would
+ *             be unreachable), else CD_ERR_AUTOMATON.
+ *   eos >= 0  the EOS / longest-match variant (G4, G5; the paper leaves the
+ *             stopping rule to the engine): the language is
+ *             { label + [eos] }.  Every state reached by a whole label ("may stop") gets an
+ *             eos edge to ONE accepting sink and only the sink accepts, so a label may be a
+ *             token-prefix of another ("New York" / "New York City"): in the shorter label's
+ *             end state the model either emits eos or goes on.  The decoded row is
+ *             label + [eos]; the label is read from the token history.  Labels must be
+ *             non-empty, distinct and must not contain eos; eos < V.
+ * State numbering (both): 0 = root, trie nodes in insertion order (labels in the given
+ * order, token by token), the sink (eos >= 0) last.
+ * cd_build_trie is pure host code (no device needed): it writes the number of states and
+ * transitions to *S_out / *nnz_out and, where the array pointers are not NULL, the CSR
+ * (row_ptr [S+1], tok / next [nnz], accepting [S]; size them from a first call with NULL
+ * arrays).  cd_compile_trie builds the same automaton and compiles it (as cd_compile_dfa).
  */
+CD_API cd_status cd_build_trie(int32_t V, int32_t K, const int64_t* label_ptr /*[K+1]*/, const int32_t* label_tok,
+                        int32_t eos, int32_t* S_out, int64_t* nnz_out, int64_t* row_ptr_out, int32_t* tok_out,
+                        int32_t* next_out, uint8_t* accepting_out);
 CD_API cd_status cd_compile_trie(int32_t V, int32_t K, const int64_t* label_ptr /*[K+1]*/,
-                          const int32_t* label_tok, int device, cd_dfa_t** out);
+                          const int32_t* label_tok, int32_t eos, int device, cd_dfa_t** out);
 
 /*
  * Sugar for collection types with a quantifier (section 2.3: "If the
@@ -113,6 +142,11 @@ CD_API cd_status cd_compile_trie(int32_t V, int32_t K, const int64_t* label_ptr 
  * close.  Deterministic by construction or rejected (CD_ERR_AUTOMATON): labels non-empty,
  * distinct and prefix-free, sep[0] != close[0], and close[0] does not start a label when
  * min_items == 0.  State 0 is the start state.
+ * eos >= 0 (the EOS / longest-match variant, see cd_compile_trie): the list is followed by
+ * eos -- the accepting state is reached by eos after the last token of close -- and a label
+ * may be a token-prefix of another label: an item ends when sep or close follows, so in the
+ * shorter label's end state sep[0] / close[0] must not continue a longer label (else
+ * CD_ERR_AUTOMATON); eos occurs in no label and in none of open / sep / close.
  * cd_build_list is pure host code (no device needed): it writes the number of states and
  * transitions to *S_out / *nnz_out and, where the array pointers are not NULL, the CSR
  * (row_ptr [S+1], tok / next [nnz], accepting [S]; size them from a first call with NULL
@@ -121,12 +155,12 @@ CD_API cd_status cd_compile_trie(int32_t V, int32_t K, const int64_t* label_ptr 
 CD_API cd_status cd_build_list(int32_t V, int32_t K, const int64_t* label_ptr, const int32_t* label_tok,
                         const int32_t* open, int32_t n_open, const int32_t* sep, int32_t n_sep,
                         const int32_t* close, int32_t n_close, int32_t min_items, int32_t max_items,
-                        int32_t* S_out, int64_t* nnz_out, int64_t* row_ptr_out, int32_t* tok_out,
+                        int32_t eos, int32_t* S_out, int64_t* nnz_out, int64_t* row_ptr_out, int32_t* tok_out,
                         int32_t* next_out, uint8_t* accepting_out);
 CD_API cd_status cd_compile_list(int32_t V, int32_t K, const int64_t* label_ptr, const int32_t* label_tok,
                           const int32_t* open, int32_t n_open, const int32_t* sep, int32_t n_sep,
                           const int32_t* close, int32_t n_close, int32_t min_items, int32_t max_items,
-                          int device, cd_dfa_t** out);
+                          int32_t eos, int device, cd_dfa_t** out);
 
 /* Releases the device image and every per-stream scratch area.  NULL is a no-op.
    The caller makes sure no work using the handle is still in flight. */
@@ -147,7 +181,6 @@ CD_API cd_status cd_dfa_info(const cd_dfa_t* dfa, int32_t* V, int32_t* S, int32_
  *                         BASELINE.json north_star states)
  *   max_transitions > 0   gather states with <= max_transitions transitions
  *   max_transitions = -1  automatic threshold from V and the logits dtype
- * Call it while no work using the handle is in flight.
  */
 CD_API cd_status cd_set_gather_max(cd_dfa_t* dfa, int32_t max_transitions);
 
@@ -167,7 +200,6 @@ CD_API cd_status cd_set_gather_max(cd_dfa_t* dfa, int32_t max_transitions);
  * cd_step the decoding step is step_base; cd_decode_loop* use step_base + k.
  * On the LM-head path (cd_head_*) the same rule applies to the fp32-accumulated logits
  * (bit-identical to the logits path whenever the dot products are exact in fp32).
- * Call it while no work using the handle is in flight.
  */
 CD_API cd_status cd_set_sampling(cd_dfa_t* dfa, float temperature, uint64_t seed, int32_t step_base);
 
@@ -187,7 +219,9 @@ CD_API cd_status cd_reserve(const cd_dfa_t* dfa, int32_t max_rows, void* cuda_st
  *   lse_out     [n] masked logsumexp (may be NULL)
  *   done_out    [n] 1 iff the new state is accepting
  * A slot whose state is already accepting does not advance: state unchanged,
- * token -1, logprob 0, lse 0, done 1.  If every allowed logit is -inf (or NaN)
+ * token -1, logprob 0, lse 0, done 1; a slot whose state is outside [0, S) is
+ * reported the same way (nothing else can be said about it without a host
+ * synchronisation).  If every allowed logit is -inf (or NaN)
  * the lowest allowed id is chosen and logprob = lse = -inf.  With an allowed
  * +inf logit the lowest such id is chosen; logprob / lse are unspecified.
  * n == 0 is valid and launches nothing.
@@ -213,6 +247,9 @@ CD_API cd_status cd_transition(const cd_dfa_t* dfa, const int32_t* token, int32_
  *   state_in    [n] or NULL (then state_out is not written)
  *   row_ids_out [n], state_out [n]: first n_active entries are written
  *   n_active_out device int32
+ * Up to 4096 slots one CTA does it (no allocation: the call can be captured in a CUDA
+ * graph); longer lists take a single-pass scan over ceil(n / 4096) CTAs with decoupled
+ * look-back, whose few bytes of chunk state are stream-ordered scratch (cudaMallocAsync).
  */
 CD_API cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, const int32_t* state_in,
                      int32_t n, int32_t* row_ids_out, int32_t* state_out, int32_t* n_active_out,
@@ -231,7 +268,29 @@ CD_API cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, cons
  *   sum_logprob_out [B] sum of the chosen tokens' log-probs (fp32)
  *   done_out        [B] 1 iff the row reached an accepting state (0 = truncated)
  * If the start state is accepting every row is done with len 0.
+ *
+ * How it runs (cd_set_loop_mode):
+ *   CD_LOOP_AUTO (default)  ONE cooperative kernel launch for the whole loop when the
+ *       device supports it and B <= 32768: the CTAs stay resident, meet at a grid barrier
+ *       after every decoding step and read step_logits[k] themselves; the active set is a
+ *       bitmap over original row ids (slot i of a step = its i-th set bit, i.e. the stable
+ *       order of cd_compact) -- no launch, no counter reset and no compaction pass between
+ *       steps.  cd_decode_loop and cd_decode_loop_limit take this path; otherwise, and for
+ *       the host-buffer and callback forms (whose step inputs appear between steps), the
+ *       loop is one cd_step-like launch per decoding step with the compaction fused into
+ *       the step kernel's last CTA.
+ *   CD_LOOP_PER_STEP        always one launch per decoding step.
+ * Both give the same results bit for bit (token, state, done, len) and the same fp32
+ * sums.  cd_loop_trace returns, for the last loop that ran in the persistent kernel on
+ * (dfa, cuda_stream), the number of decoding steps it ran (*steps_out), and for the first
+ * min(cap, 256) of them the active rows and the duration in nanoseconds measured on the
+ * device (HOST arrays; *steps_out = 0 if that loop took the per-step path).  It
+ * synchronises the stream.
  */
+typedef enum { CD_LOOP_AUTO = 0, CD_LOOP_PER_STEP = 1 } cd_loop_mode;
+CD_API cd_status cd_set_loop_mode(cd_dfa_t* dfa, int32_t mode);
+CD_API cd_status cd_loop_trace(const cd_dfa_t* dfa, void* cuda_stream, int32_t cap, int64_t* t_ns_out,
+                        int32_t* n_active_out, int32_t* steps_out);
 CD_API cd_status cd_decode_loop(const cd_dfa_t* dfa, const void* const* step_logits, cd_dtype dtype,
                          int64_t ld_elems, int32_t B, int32_t max_steps, int32_t* tokens_out,
                          int32_t* len_out, int32_t* final_state_out, float* sum_logprob_out,
@@ -244,7 +303,7 @@ CD_API cd_status cd_decode_loop(const cd_dfa_t* dfa, const void* const* step_log
  * generation requests are terminated").
  * cd_set_satisfying marks the accepting states whose value satisfies the query's
  * predicate (HOST u8[S], copied; e.g. the leaf of the label TRUE for `... = TRUE`;
- * NULL clears).  Call it while no work using the handle is in flight.
+ * NULL clears).
  * cd_decode_loop_limit is cd_decode_loop with a device counter *satisfied_inout
  * (DEVICE int32, shared by the calls of one query, one call per batch of the
  * table; the caller zeroes it first): every row that reaches an accepting state s
@@ -270,7 +329,7 @@ CD_API cd_status cd_decode_loop_limit(const cd_dfa_t* dfa, const void* const* st
  * (satisfied: DEVICE int32 owned by the caller, shared by the calls of one query; needs
  * cd_set_satisfying) cd_decode_loop, cd_decode_loop_host, cd_decode_loop_cb and the
  * cd_head_decode_loop* family all behave as cd_decode_loop_limit does.  satisfied == NULL
- * clears it.  Call it while no work using the handle is in flight.
+ * clears it.
  */
 CD_API cd_status cd_set_limit(cd_dfa_t* dfa, int32_t limit, int32_t* satisfied_inout);
 

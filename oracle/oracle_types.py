@@ -17,7 +17,7 @@ The automaton of a finite language is its prefix tree -- that is all this file b
 nothing with paper_2606_31808_b200/ (whose builder is csrc/cd_types.hpp) and must never be imported
 from it.  Pure-python loops: option sets are small.
 
-State numbering (the convention include/cd.h documents for cd_compile_trie with eos >= 0, so that
+State numbering (the convention the product's C-ABI header documents for its option-set sugar with eos >= 0, so that
 final states compare bit for bit): state 0 is the empty prefix; the other proper prefixes of L are
 numbered in order of first appearance when the strings are inserted in the given order, token by
 token; the single accepting sink is numbered last (S - 1).

@@ -9,6 +9,9 @@ raise.
 from .binding import (  # noqa: F401
     BF16,
     F32,
+    LOOP_AUTO,
+    LOOP_PER_STEP,
+    build_trie,
     CdError,
     Dfa,
     compact,

@@ -12,12 +12,13 @@ _SO = os.path.join(HERE, "libcd.so")
 _lib = None
 
 F32, BF16 = 0, 1
+LOOP_AUTO, LOOP_PER_STEP = 0, 1
 STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_STATE",
           4: "CD_ERR_CUDA", 5: "CD_ERR_OOM", 6: "CD_ERR_INTERNAL"}
 
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
-    "cd_compile_dfa", "cd_compile_trie", "cd_build_list", "cd_compile_list", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_set_sampling", "cd_reserve", "cd_step",
+    "cd_compile_dfa", "cd_build_trie", "cd_compile_trie", "cd_build_list", "cd_set_loop_mode", "cd_loop_trace", "cd_compile_list", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_set_sampling", "cd_reserve", "cd_step",
     "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_set_limit", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_probe_read", "cd_decode_loop_cb", "cd_head_decode_loop_cb", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
     "cd_last_error",
 )
@@ -114,6 +115,20 @@ class Dfa:
         """cd_set_head_gather_max: 0 = dense contraction for every state, > 0 threshold, -1 automatic."""
         _check(lib().cd_set_head_gather_max(self._h, C.c_int32(max_transitions)))
 
+    def set_loop_mode(self, mode: int):
+        """cd_set_loop_mode: LOOP_AUTO (one persistent kernel per decode loop when possible) or LOOP_PER_STEP."""
+        _check(lib().cd_set_loop_mode(self._h, C.c_int32(mode)))
+
+    def loop_trace(self, cap: int = 256):
+        """cd_loop_trace: (active rows, nanoseconds) per decoding step of the last persistent loop on the
+        current stream, as two python lists (empty if that loop ran as per-step launches)."""
+        t = (C.c_int64 * max(cap, 1))()
+        n = (C.c_int32 * max(cap, 1))()
+        steps = C.c_int32(0)
+        _check(lib().cd_loop_trace(self._h, _stream(self.device), C.c_int32(cap), t, n, C.byref(steps)))
+        k = min(steps.value, cap)
+        return [int(n[i]) for i in range(k)], [int(t[i]) for i in range(k)]
+
     def set_satisfying(self, satisfying):
         """cd_set_satisfying: u8[S] host flags (None clears)."""
         if satisfying is None:
@@ -173,23 +188,43 @@ def compile_dfa(V: int, S: int, start: int, row_ptr, tok, next, accepting, devic
     return Dfa(out.value, dev)
 
 
-def compile_trie(V: int, labels: Sequence[Sequence[int]], device="cuda") -> Dfa:
-    """cd_compile_trie: option-set / boolean types as a trie over token-id labels."""
-    L = lib()
+def _label_args(labels):
     ptr = [0]
     flat: List[int] = []
     for lab in labels:
         flat.extend(int(t) for t in lab)
         ptr.append(len(flat))
-    lp = torch.tensor(ptr, dtype=torch.int64)
-    lt = torch.tensor(flat, dtype=torch.int32)
+    return torch.tensor(ptr, dtype=torch.int64), torch.tensor(flat if flat else [0], dtype=torch.int32)
+
+
+def build_trie(V: int, labels: Sequence[Sequence[int]], eos: int = -1):
+    """cd_build_trie (host only, no device needed): the CSR of the option-set automaton as
+    (S, row_ptr i64[S+1], tok i32[nnz], next i32[nnz], accepting u8[S]); eos >= 0 = the EOS / longest-match variant."""
+    lp, lt = _label_args(labels)
+    head = [C.c_int32(V), C.c_int32(len(labels)), _ptr(lp), _ptr(lt), C.c_int32(eos)]
+    S, nnz = C.c_int32(0), C.c_int64(0)
+    null = C.c_void_p(None)
+    _check(lib().cd_build_trie(*head, C.byref(S), C.byref(nnz), null, null, null, null))
+    rp = torch.empty(S.value + 1, dtype=torch.int64)
+    tk = torch.empty(max(nnz.value, 1), dtype=torch.int32)
+    nx = torch.empty(max(nnz.value, 1), dtype=torch.int32)
+    ac = torch.empty(S.value, dtype=torch.uint8)
+    _check(lib().cd_build_trie(*head, C.byref(S), C.byref(nnz), _ptr(rp), _ptr(tk), _ptr(nx), _ptr(ac)))
+    return S.value, rp, tk[: nnz.value], nx[: nnz.value], ac
+
+
+def compile_trie(V: int, labels: Sequence[Sequence[int]], device="cuda", eos: int = -1) -> Dfa:
+    """cd_compile_trie: option-set / boolean types as a trie over token-id labels (eos >= 0: labels may be
+    prefixes of one another, every row ends with eos in the one accepting sink)."""
+    L = lib()
+    lp, lt = _label_args(labels)
     dev_index = 0
     dev = None
     if torch.cuda.is_available():
         dev = _device_index(device)
         dev_index = dev.index
     out = C.c_void_p()
-    _check(L.cd_compile_trie(C.c_int32(V), C.c_int32(len(labels)), _ptr(lp), _ptr(lt), C.c_int(dev_index),
+    _check(L.cd_compile_trie(C.c_int32(V), C.c_int32(len(labels)), _ptr(lp), _ptr(lt), C.c_int32(eos), C.c_int(dev_index),
                              C.byref(out)))
     return Dfa(out.value, dev)
 
@@ -518,7 +553,7 @@ def head_decode_loop_cb(dfa: Dfa, next_hidden, W: torch.Tensor, H: int, B: int, 
     return out
 
 
-def _list_args(V, labels, open_, sep, close, min_items, max_items):
+def _list_args(V, labels, open_, sep, close, min_items, max_items, eos=-1):
     ptr, flat = [0], []
     for lab in labels:
         flat.extend(int(t) for t in lab)
@@ -527,15 +562,16 @@ def _list_args(V, labels, open_, sep, close, min_items, max_items):
     lt = torch.tensor(flat if flat else [0], dtype=torch.int32)
     ts = [torch.tensor(list(x) if len(x) else [0], dtype=torch.int32) for x in (open_, sep, close)]
     args = [C.c_int32(V), C.c_int32(len(labels)), _ptr(lp), _ptr(lt), _ptr(ts[0]), C.c_int32(len(open_)), _ptr(ts[1]),
-            C.c_int32(len(sep)), _ptr(ts[2]), C.c_int32(len(close)), C.c_int32(min_items), C.c_int32(max_items)]
+            C.c_int32(len(sep)), _ptr(ts[2]), C.c_int32(len(close)), C.c_int32(min_items), C.c_int32(max_items),
+            C.c_int32(eos)]
     return args, (lp, lt, ts)
 
 
 def build_list(V: int, labels: Sequence[Sequence[int]], open_: Sequence[int], sep: Sequence[int],
-               close: Sequence[int], min_items: int, max_items: int):
+               close: Sequence[int], min_items: int, max_items: int, eos: int = -1):
     """cd_build_list (host only, no device needed): the CSR of the quantified-list automaton as
     (S, row_ptr i64[S+1], tok i32[nnz], next i32[nnz], accepting u8[S])."""
-    args, keep = _list_args(V, labels, open_, sep, close, min_items, max_items)
+    args, keep = _list_args(V, labels, open_, sep, close, min_items, max_items, eos)
     S, nnz = C.c_int32(0), C.c_int64(0)
     null = C.c_void_p(None)
     _check(lib().cd_build_list(*args, C.byref(S), C.byref(nnz), null, null, null, null))
@@ -548,9 +584,9 @@ def build_list(V: int, labels: Sequence[Sequence[int]], open_: Sequence[int], se
 
 
 def compile_list(V: int, labels: Sequence[Sequence[int]], open_: Sequence[int], sep: Sequence[int],
-                 close: Sequence[int], min_items: int, max_items: int, device="cuda") -> Dfa:
+                 close: Sequence[int], min_items: int, max_items: int, device="cuda", eos: int = -1) -> Dfa:
     """cd_compile_list: collection type with a quantifier ({min_items, max_items} items of an option set)."""
-    args, keep = _list_args(V, labels, open_, sep, close, min_items, max_items)
+    args, keep = _list_args(V, labels, open_, sep, close, min_items, max_items, eos)
     dev_index, dev = 0, None
     if torch.cuda.is_available():
         dev = _device_index(device)

@@ -1,6 +1,9 @@
 """In-tree build of the C-ABI library (libcd.so) for sm_100a with nvcc.
 
-    python -m paper_2606_31808_b200.build [--force] [--verbose]
+    python -m paper_2606_31808_b200.build [--force] [--verbose] [--nvtx] [--tuning]
+
+--nvtx / --tuning build a second library (libcd_nvtx.so / libcd_tuning.so) beside the product one:
+NVTX ranges per loop and decoding step, and the environment knobs used by the launch-shape sweeps.
 
 The .so is git-ignored but travels to the GPU box with the gpurun snapshot.
 nvcc cross-compiles without a GPU.
@@ -42,17 +45,22 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in DEPS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not needs_build():
+def build(force: bool = False, verbose: bool = False, defines=(), out: str = SO) -> str:
+    """defines: extra -D flags.  CD_NVTX = NVTX ranges around every loop and decoding step (SURVEY section 5);
+    CD_TUNING = the environment knobs of the launch-shape sweeps (never set for the product .so).  A build
+    with defines should go to another `out` path."""
+    if not force and out == SO and not needs_build():
         return SO
-    tmp = SO + f".tmp{os.getpid()}"
-    cmd = [nvcc_path()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
+    tmp = out + f".tmp{os.getpid()}"
+    cmd = [nvcc_path()] + NVCC_FLAGS + [f"-D{d}" for d in defines] + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + SOURCES
     if verbose:
         print(" ".join(cmd), file=sys.stderr)
     subprocess.check_call(cmd)
-    os.replace(tmp, SO)
-    return SO
+    os.replace(tmp, out)
+    return out
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    defs = [d for f, d in (("--nvtx", "CD_NVTX"), ("--tuning", "CD_TUNING")) if f in sys.argv]
+    target = SO if not defs else os.path.join(HERE, "libcd_" + "_".join(d[3:].lower() for d in defs) + ".so")
+    print(build(force="--force" in sys.argv or bool(defs), verbose="--verbose" in sys.argv, defines=defs, out=target))

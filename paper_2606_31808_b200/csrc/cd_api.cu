@@ -1,6 +1,6 @@
 // cd_api.cu -- the C ABI of include/cd.h: validation, automaton store, scratch management and
 // kernel launches.  No torch types, no CPU fallback: every step of the path runs in the
-// kernels of cd_step.cuh / cd_aux.cuh.
+// kernels of cd_step.cuh / cd_aux.cuh / cd_head.cuh / cd_dedup.cuh.
 #include <cuda_runtime.h>
 
 #include <atomic>
@@ -21,6 +21,17 @@
 #include "cd_head.cuh"
 #include "cd_dedup.cuh"
 #include "cd_types.hpp"
+
+// NVTX ranges around every loop and every decoding step's enqueue: compiled in
+// with -DCD_NVTX (python -m paper_2606_31808_b200.build --nvtx); header-only, nothing to link.
+#ifdef CD_NVTX
+#include <nvtx3/nvToolsExt.h>
+#define CD_RANGE_PUSH(name) nvtxRangePushA(name)
+#define CD_RANGE_POP() nvtxRangePop()
+#else
+#define CD_RANGE_PUSH(name) ((void)0)
+#define CD_RANGE_POP() ((void)0)
+#endif
 
 namespace {
 
@@ -46,65 +57,85 @@ cd_status fail(cd_status st, const char* fmt, ...) {
         }                                                                                    \
     } while (0)
 
-// Launch shapes of the step kernel: warps per CTA (one CTA per SM), ring stages per warp, tile
-// bytes.  Variant 0 (12 warps x 2 stages x 8 KiB = 192 KiB of logits in flight per SM) is the
-// product default: best or within noise of best on configs c1-c4 (profiles/r1_variant_sweep.md).
-// The others exist for tuning runs (environment variable CD_STEP_VARIANT, read once).
-struct StepCfg { int warps, stages, tile_bytes; };
-constexpr StepCfg STEP_CFGS[] = {{12, 2, 8192}, {16, 3, 4096}, {8, 3, 8192}, {13, 2, 8192}, {6, 2, 16384}, {24, 2, 4096}};
-constexpr int N_STEP_CFGS = sizeof(STEP_CFGS) / sizeof(STEP_CFGS[0]);
+struct RangeGuard {  // NVTX range for the scope (a no-op unless built with -DCD_NVTX)
+    explicit RangeGuard(const char* name) { CD_RANGE_PUSH(name); (void)name; }
+    ~RangeGuard() { CD_RANGE_POP(); }
+};
 
-int step_variant() {
-    static const int v = [] {
-        const char* e = std::getenv("CD_STEP_VARIANT");
-        const int x = e ? std::atoi(e) : 0;
-        return (x >= 0 && x < N_STEP_CFGS) ? x : 0;
-    }();
-    return v;
-}
+// Launch shape of the step / loop kernels: 12 warps per CTA (one CTA per SM), 2 ring stages per warp,
+// 8 KiB tiles = 192 KiB of logits in flight per SM.  Best or within noise of best on configs c1-c4 among
+// the shapes swept in round 1 (profiles/r1_variant_sweep.md).
+constexpr int STEP_WARPS = 12, STEP_STAGES = 2, STEP_TILE = 8192;
+using StepRing = cd::WarpRing<STEP_STAGES, STEP_TILE>;
 
-int host_gather_mult() {  // CTAs per SM of the zero-copy row gather (tuning knob CD_HOST_GATHER_CTAS)
-    static const int v = [] {
-        const char* e = std::getenv("CD_HOST_GATHER_CTAS");
-        const int x = e ? std::atoi(e) : 4;  // flat from 2 to 32 (51 GB/s on PCIe Gen5 x16)
-        return (x >= 1 && x <= 64) ? x : 4;
-    }();
-    return v;
+// Tuning knobs exist only in builds made with -DCD_TUNING (python -m paper_2606_31808_b200.build --tuning);
+// the product reads no environment variable.
+#ifdef CD_TUNING
+int tune_int(const char* name, int def, int lo, int hi) {
+    const char* e = std::getenv(name);
+    if (!e) return def;
+    const int v = std::atoi(e);
+    return (v >= lo && v <= hi) ? v : def;
 }
+#else
+constexpr int tune_int(const char*, int def, int, int) { return def; }
+#endif
 
-bool use_pdl() {
-    static const bool v = [] {
-        const char* e = std::getenv("CD_PDL");
-        return e ? std::atoi(e) != 0 : true;
-    }();
-    return v;
-}
+int units_per_warp() { static const int v = tune_int("CD_UPW", cd::UNITS_PER_WARP, 1, 32); return v; }
+int tpu_max_tiles() { static const int v = tune_int("CD_TPU_MAX", cd::TPU_MAX_BYTES / STEP_TILE, 1, cd::TPU_MAX_BYTES / STEP_TILE); return v; }
+bool use_pdl() { static const int v = tune_int("CD_PDL", 1, 0, 1); return v != 0; }
+int host_gather_mult() { static const int v = tune_int("CD_HOST_GATHER_CTAS", 4, 1, 64); return v; }  // flat from 2 to 32 (51 GB/s on PCIe Gen5 x16)
 
 // Per (handle, stream) scratch.  Operations on one stream are ordered, so one area per stream
 // is race free; distinct streams get distinct areas.
-struct Scratch {
+struct StepBufs {  // sized by rows; replaced as a whole when the area grows
     int cap_rows = 0;
     long long cap_units = 0;
     cd::PartialSlot* partials = nullptr;
-    int* tickets = nullptr;
-    int* ctrs = nullptr;  // [0] work, [1] finished CTAs, [2] sticky errors, [3] launch generation
-    // decode loop
+    int* tickets = nullptr;  // [rows] zero between launches
+    int* ctrs = nullptr;  // [0] work, [1] finished CTAs, [2] errors of the running loop, [3] launch generation
+    // per-step decode loops
     int* row_ids[2] = {nullptr, nullptr};
     int* state[2] = {nullptr, nullptr};
     int* state_new = nullptr;  // next states of a step launch
-    int* n_active = nullptr;  // [2]
+    int* n_active = nullptr;   // [2]
     int* token = nullptr;
     float* logprob = nullptr;
     uint8_t* done = nullptr;
-    // host-buffer loop
+    // persistent loop
+    uint32_t* alive[3] = {nullptr, nullptr, nullptr};  // [ceil(rows / 32)] each
+    int* state2[2] = {nullptr, nullptr};                // [rows] each
+    int* bar = nullptr;                                 // [4]
+    unsigned long long* trace_t = nullptr;              // [LOOP_TRACE_STEPS + 1]
+    int* trace_n = nullptr;                             // [LOOP_TRACE_STEPS + 1]
+    unsigned long long* phase = nullptr;                // tuning builds: [LOOP_TRACE_STEPS][8]
+
+    void release() {
+        cudaFree(partials); cudaFree(tickets); cudaFree(ctrs);
+        for (int i = 0; i < 2; ++i) { cudaFree(row_ids[i]); cudaFree(state[i]); cudaFree(state2[i]); }
+        for (int i = 0; i < 3; ++i) cudaFree(alive[i]);
+        cudaFree(state_new); cudaFree(n_active); cudaFree(token); cudaFree(logprob); cudaFree(done);
+        cudaFree(bar); cudaFree(trace_t); cudaFree(trace_n); cudaFree(phase);
+        *this = StepBufs();
+    }
+};
+
+struct Scratch {
+    StepBufs b;
+    // persistent loop: per-step work counters and the device copy of the step pointers
+    int loop_steps_cap = 0;
+    int* loop_work = nullptr;
+    const void** loop_ptrs = nullptr;
+    bool trace_valid = false;  // the last loop on this stream ran in loop_kernel
+    // host-buffer loops
     void* stage[2] = {nullptr, nullptr};
-    size_t stage_bytes = 0;
+    size_t stage_bytes[2] = {0, 0};
     int* out_i32 = nullptr;  // device copies of the host outputs
     size_t out_bytes = 0;
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_copied[2] = {nullptr, nullptr};
     cudaEvent_t ev_consumed[2] = {nullptr, nullptr};
-    int* h_pinned = nullptr;  // [4] pinned host ints
+    int* h_pinned = nullptr;  // [8] pinned host ints
     int* h_ids = nullptr;     // [h_ids_cap] pinned host copy of the active row ids (host-buffer loop)
     int h_ids_cap = 0;
     // LM-head step (cd_head.cuh)
@@ -117,11 +148,18 @@ struct Scratch {
     cd::HeadPartial* h_partials = nullptr;
     CUtensorMap h_tmA{};
 
-    void release() {
+    void release_head() {
         cudaFree(h_flags); cudaFree(h_lists); cudaFree(h_ctr); cudaFree(h_A); cudaFree(h_partials);
-        cudaFree(partials); cudaFree(tickets); cudaFree(ctrs);
-        for (int i = 0; i < 2; ++i) { cudaFree(row_ids[i]); cudaFree(state[i]); cudaFree(stage[i]); }
-        cudaFree(state_new); cudaFree(n_active); cudaFree(token); cudaFree(logprob); cudaFree(done); cudaFree(out_i32);
+        h_flags = nullptr; h_lists = nullptr; h_ctr = nullptr; h_A = nullptr; h_partials = nullptr;
+        head_rows = 0;
+        head_H = 0;
+    }
+    void release() {
+        b.release();
+        release_head();
+        cudaFree(loop_work); cudaFree(loop_ptrs);
+        for (int i = 0; i < 2; ++i) cudaFree(stage[i]);
+        cudaFree(out_i32);
         if (copy_stream) cudaStreamDestroy(copy_stream);
         for (int i = 0; i < 2; ++i) {
             if (ev_copied[i]) cudaEventDestroy(ev_copied[i]);
@@ -133,6 +171,21 @@ struct Scratch {
     }
 };
 
+// What the cd_set_* calls configure.  Every entry point takes a copy under the handle's mutex when it
+// starts and works from that copy, so a setter never races with a call in progress: it applies to the
+// calls that start after it returns.
+struct Settings {
+    int gather_max = 0;        // cd_set_gather_max: 0 dense scan only, > 0 threshold, < 0 automatic
+    int head_gather_max = -1;  // cd_set_head_gather_max: 0 never gather, > 0 threshold, < 0 automatic
+    float inv_tau = 0.0f;      // cd_set_sampling: 0 = greedy, else 1 / temperature
+    unsigned long long seed = 0;
+    int rng_step_base = 0;
+    int limit = 0;             // cd_set_limit: LIMIT early exit applied by every loop entry point
+    int* limit_ctr = nullptr;  //   device counter of satisfied rows (caller-owned); nullptr = no limit
+    bool has_satisfying = false;  // cd_set_satisfying was called with a set
+    int loop_mode = CD_LOOP_AUTO;  // cd_set_loop_mode
+};
+
 }  // namespace
 
 struct cd_dfa {
@@ -142,30 +195,32 @@ struct cd_dfa {
     int start_accepting = 0;
     long long nnz = 0;
     int num_sms = 0;
+    int coop_launch = 0;    // the device supports cooperative launches
     long long max_deg = 0;  // largest number of transitions of a state
-    int gather_max = 0;  // cd_set_gather_max: 0 dense scan only, > 0 threshold, < 0 automatic
+    long long min_deg_nonacc = 0;  // fewest transitions of a non-accepting state
     void* d_mask = nullptr;
     void* d_row_ptr = nullptr;
     void* d_tok = nullptr;
     void* d_next = nullptr;
     void* d_acc = nullptr;
-    void* d_satisfying = nullptr;  // cd_set_satisfying
-    int limit = 0;                 // cd_set_limit: LIMIT early exit applied by every loop entry point
-    int* limit_ctr = nullptr;      //   device counter of satisfied rows (caller-owned); nullptr = no limit
-    float inv_tau = 0.0f;          // cd_set_sampling: 0 = greedy, else 1 / temperature
-    unsigned long long seed = 0;
-    int rng_step_base = 0;
-    long long min_deg_nonacc = 0;  // fewest transitions of a non-accepting state
-    int head_gather_max = -1;      // cd_set_head_gather_max: 0 never gather, > 0 threshold, < 0 automatic
+    void* d_rank = nullptr;
+    void* d_satisfying = nullptr;  // [S], allocated with the handle, never freed before cd_free_dfa
     const void* w_ptr = nullptr;   // cached tensor map of the output embedding (cd_head_step)
     long long w_ld = 0;
     int w_H = 0;
     CUtensorMap w_tmap{};
-    std::mutex mu;
+    std::mutex mu;  // guards cfg, the weight map cache and the scratch map
+    Settings cfg;
     std::map<cudaStream_t, Scratch> scratch;
 };
 
 namespace {
+
+Settings settings_of(const cd_dfa* d) {
+    cd_dfa* dm = const_cast<cd_dfa*>(d);
+    std::lock_guard<std::mutex> lk(dm->mu);
+    return dm->cfg;
+}
 
 struct DeviceGuard {
     int prev = -1;
@@ -180,7 +235,7 @@ struct DeviceGuard {
 };
 
 int tiles_per_row(int V, int dtype) {
-    const int tt = STEP_CFGS[step_variant()].tile_bytes / (dtype == CD_BF16 ? 2 : 4);
+    const int tt = STEP_TILE / (dtype == CD_BF16 ? 2 : 4);
     return (V + tt - 1) / tt;
 }
 
@@ -189,8 +244,8 @@ int tiles_per_row(int V, int dtype) {
 // at ~31 G allowed logits/s (one scattered 2-byte logit per 64-byte DRAM granule), the dense scan streams
 // a row at ~6.8 TB/s, so gathering pays while nnz / 31e9 < row_bytes / 6.8e12, i.e. nnz < row_bytes / 220;
 // 232 leaves a margin so that states near the break-even stay on the dense path.
-int gather_max_for(const cd_dfa* d, int dtype) {
-    if (d->gather_max >= 0) return d->gather_max;
+int gather_max_for(const cd_dfa* d, const Settings& cfg, int dtype) {
+    if (cfg.gather_max >= 0) return cfg.gather_max;
     const long long row_bytes = (long long)d->dev.V * (dtype == CD_BF16 ? 2 : 4) + d->dev.V / 8;
     const long long g = row_bytes / 232;
     return (int)(g > 0x3FFFFFFF ? 0x3FFFFFFF : g);
@@ -205,64 +260,123 @@ int step_grid(const cd_dfa* d, long long n_upper, int dtype) {
 }
 
 // Upper bound of n' * P(n') over n' <= n for the largest grid (mirrors cd::tiles_per_unit):
-// unclamped tiles-per-unit gives n'P <= 4*warps + n'; clamped at TPU_MAX gives n' * ceil(T/16).
+// unclamped tiles-per-unit gives n'P <= upw*warps + n'; clamped at the most tiles per unit gives n' * ceil(T/tpu_max).
 long long step_units_cap(const cd_dfa* d, long long n) {
-    const StepCfg c = STEP_CFGS[step_variant()];
     const int T = tiles_per_row(d->dev.V, CD_F32);  // fp32 rows have the most tiles
-    int tpu_max = cd::TPU_MAX_BYTES / c.tile_bytes;
-    if (const char* e = std::getenv("CD_TPU_MAX")) {  // tuning knob: fewer tiles per unit -> more units per row
-        const int v = std::atoi(e);
-        if (v >= 1 && v < tpu_max) tpu_max = v;
-    }
-    const long long warps = (long long)d->num_sms * c.warps;
-    const long long a = warps * 32 + n;  // up to 32 units per warp (tuning knob CD_UPW)
+    const int tpu_max = tpu_max_tiles();
+    const long long warps = (long long)d->num_sms * STEP_WARPS;
+    const long long a = warps * 32 + n;  // up to 32 units per warp
     const long long b = n * (long long)((T + tpu_max - 1) / tpu_max + 1);
     // small grids (few rows) use fewer warps, hence fewer units: still below a
     return (a > b ? a : b) + 64;
 }
 
-cd_status get_scratch(const cd_dfa* cd_, cudaStream_t stream, int rows, bool loop_bufs, Scratch** out) {
+template <typename T>
+cudaError_t dev_alloc(T** p, size_t count) {
+    return cudaMalloc(reinterpret_cast<void**>(p), sizeof(T) * (count ? count : 1));
+}
+
+// Allocates a complete set of step buffers for `rows` rows; on failure nothing is kept.
+cd_status alloc_step_bufs(const cd_dfa* d, int rows, StepBufs* out) {
+    StepBufs n;
+    const long long units = step_units_cap(d, rows);
+    const size_t nwords = ((size_t)rows + 31) / 32;
+    cudaError_t e = cudaSuccess;
+    auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+    A(dev_alloc(&n.partials, (size_t)units));
+    A(dev_alloc(&n.ctrs, 4));
+    A(dev_alloc(&n.tickets, (size_t)rows));
+    for (int i = 0; i < 2; ++i) {
+        A(dev_alloc(&n.row_ids[i], (size_t)rows));
+        A(dev_alloc(&n.state[i], (size_t)rows));
+        A(dev_alloc(&n.state2[i], (size_t)rows));
+    }
+    for (int i = 0; i < 3; ++i) A(dev_alloc(&n.alive[i], nwords));
+    A(dev_alloc(&n.state_new, (size_t)rows));
+    A(dev_alloc(&n.n_active, 2));
+    A(dev_alloc(&n.token, (size_t)rows));
+    A(dev_alloc(&n.logprob, (size_t)rows));
+    A(dev_alloc(&n.done, (size_t)rows));
+    A(dev_alloc(&n.bar, 4));
+    A(dev_alloc(&n.trace_t, (size_t)cd::LOOP_TRACE_STEPS + 1));
+    A(dev_alloc(&n.trace_n, (size_t)cd::LOOP_TRACE_STEPS + 1));
+#ifdef CD_TUNING
+    A(dev_alloc(&n.phase, (size_t)cd::LOOP_TRACE_STEPS * 8));
+#endif
+    if (e == cudaSuccess) e = cudaMemset(n.partials, 0, sizeof(cd::PartialSlot) * (size_t)units);  // generation tags start at 0 ...
+    if (e == cudaSuccess) {
+        const int init[4] = {0, 0, 0, 1};  // ... launches at 1
+        e = cudaMemcpy(n.ctrs, init, sizeof init, cudaMemcpyHostToDevice);
+    }
+    if (e == cudaSuccess) e = cudaMemset(n.tickets, 0, sizeof(int) * (size_t)rows);
+    if (e == cudaSuccess) e = cudaMemset(n.trace_n, 0, sizeof(int) * ((size_t)cd::LOOP_TRACE_STEPS + 1));
+    if (e != cudaSuccess) {
+        n.release();
+        return fail(e == cudaErrorMemoryAllocation ? CD_ERR_OOM : CD_ERR_CUDA, "scratch for %d rows: %s", rows,
+                    cudaGetErrorString(e));
+    }
+    n.cap_units = units;
+    n.cap_rows = rows;
+    *out = n;
+    return CD_OK;
+}
+
+cd_status get_scratch(const cd_dfa* cd_, cudaStream_t stream, int rows, Scratch** out) {
     cd_dfa* d = const_cast<cd_dfa*>(cd_);
     std::lock_guard<std::mutex> lk(d->mu);
     if ((long long)rows * (tiles_per_row(d->dev.V, CD_F32) + 1) >= 0x7FFFFFFFLL)
         return fail(CD_ERR_ARG, "rows (%d) * tiles per row overflows the unit index", rows);
     Scratch& s = d->scratch[stream];
     if (rows < 1) rows = 1;
-    if (s.cap_rows < rows) {
-        // growing: wait for the work that still uses the old buffers
-        if (s.cap_rows > 0) CU(cudaStreamSynchronize(stream));
-        int sticky[4] = {0, 0, 0, 0};
-        Scratch old = s;
-        s.cap_rows = 0;
-        const long long units = step_units_cap(d, rows);
-        CU(cudaMalloc(&s.partials, sizeof(cd::PartialSlot) * units));
-        CU(cudaMalloc(&s.ctrs, sizeof(int) * 4));
-        CU(cudaMalloc(&s.tickets, sizeof(int) * (size_t)rows));
-        CU(cudaMemset(s.tickets, 0, sizeof(int) * (size_t)rows));
-        CU(cudaMemset(s.partials, 0, sizeof(cd::PartialSlot) * units));  // generation tags start at 0 ...
-        sticky[3] = 1;                                                    // ... launches at 1
-        CU(cudaMemcpy(s.ctrs, sticky, sizeof sticky, cudaMemcpyHostToDevice));
-        for (int i = 0; i < 2; ++i) {
-            CU(cudaMalloc(&s.row_ids[i], sizeof(int) * (size_t)rows));
-            CU(cudaMalloc(&s.state[i], sizeof(int) * (size_t)rows));
+    if (s.b.cap_rows < rows) {
+        // growing: the new set is complete before the old one is touched; then wait for the work that
+        // still uses the old buffers and drop them
+        StepBufs fresh;
+        const cd_status st = alloc_step_bufs(d, rows, &fresh);
+        if (st != CD_OK) return st;
+        if (s.b.cap_rows > 0) {
+            const cudaError_t e = cudaStreamSynchronize(stream);
+            if (e != cudaSuccess) {
+                fresh.release();
+                return fail(CD_ERR_CUDA, "cudaStreamSynchronize: %s", cudaGetErrorString(e));
+            }
         }
-        CU(cudaMalloc(&s.state_new, sizeof(int) * (size_t)rows));
-        CU(cudaMalloc(&s.n_active, sizeof(int) * 2));
-        CU(cudaMalloc(&s.token, sizeof(int) * (size_t)rows));
-        CU(cudaMalloc(&s.logprob, sizeof(float) * (size_t)rows));
-        CU(cudaMalloc(&s.done, (size_t)rows));
-        s.cap_units = units;
-        s.cap_rows = rows;
-        // keep the host-loop resources, drop the old step buffers
-        old.stage[0] = old.stage[1] = nullptr; old.out_i32 = nullptr; old.copy_stream = nullptr;
-        old.ev_copied[0] = old.ev_copied[1] = old.ev_consumed[0] = old.ev_consumed[1] = nullptr;
-        old.h_pinned = nullptr;
-        old.h_ids = nullptr;
-        old.h_flags = nullptr; old.h_lists = nullptr; old.h_ctr = nullptr; old.h_A = nullptr; old.h_partials = nullptr;
-        old.release();
+        s.b.release();
+        s.b = fresh;
+        s.trace_valid = false;
     }
-    (void)loop_bufs;
     *out = &s;
+    return CD_OK;
+}
+
+// grows a device buffer of the scratch area (contents are not kept); on failure the old buffer stays
+cd_status grow_buffer(void** buf, size_t* have, size_t want, cudaStream_t stream) {
+    if (*have >= want) return CD_OK;
+    void* fresh = nullptr;
+    CU(cudaMalloc(&fresh, want));
+    const cudaError_t e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) {
+        cudaFree(fresh);
+        return fail(CD_ERR_CUDA, "cudaStreamSynchronize: %s", cudaGetErrorString(e));
+    }
+    cudaFree(*buf);
+    *buf = fresh;
+    *have = want;
+    return CD_OK;
+}
+
+// staging + device copies of the outputs + copy stream / events of the host-buffer loops
+cd_status get_host_loop_scratch(Scratch* s, size_t stage0_bytes, size_t stage1_bytes, size_t out_bytes, cudaStream_t stream) {
+    cd_status st = grow_buffer(&s->stage[0], &s->stage_bytes[0], stage0_bytes, stream);
+    if (st == CD_OK && stage1_bytes) st = grow_buffer(&s->stage[1], &s->stage_bytes[1], stage1_bytes, stream);
+    if (st == CD_OK) st = grow_buffer(reinterpret_cast<void**>(&s->out_i32), &s->out_bytes, out_bytes, stream);
+    if (st != CD_OK) return st;
+    if (!s->copy_stream) CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+        if (!s->ev_copied[i]) CU(cudaEventCreateWithFlags(&s->ev_copied[i], cudaEventDisableTiming));
+        if (!s->ev_consumed[i]) CU(cudaEventCreateWithFlags(&s->ev_consumed[i], cudaEventDisableTiming));
+    }
+    if (!s->h_pinned) CU(cudaMallocHost(&s->h_pinned, sizeof(int) * 8));
     return CD_OK;
 }
 
@@ -271,11 +385,10 @@ cd_status check_dtype(cd_dtype dt) {
     return CD_OK;
 }
 
-template <int DT, int VAR, bool GATHER = false, bool SAMPLE = false>
+template <int DT, bool GATHER = false, bool SAMPLE = false>
 cd_status launch_step_t(const cd::StepArgs& a, int grid, cudaStream_t stream) {
-    constexpr StepCfg C = STEP_CFGS[VAR];
-    auto kern = cd::step_kernel<DT, C.warps, C.stages, C.tile_bytes, GATHER, SAMPLE>;
-    const size_t smem = sizeof(cd::WarpRing<C.stages, C.tile_bytes>) * C.warps;
+    auto kern = cd::step_kernel<DT, STEP_WARPS, STEP_STAGES, STEP_TILE, GATHER, SAMPLE>;
+    const size_t smem = sizeof(StepRing) * STEP_WARPS;
     static thread_local int configured_dev = -1;
     int dev = 0;
     CU(cudaGetDevice(&dev));
@@ -285,10 +398,10 @@ cd_status launch_step_t(const cd::StepArgs& a, int grid, cudaStream_t stream) {
     }
     // programmatic stream serialization: this grid may be scheduled while the previous kernel
     // of the stream drains (the kernel itself waits with griddepcontrol.wait before touching
-    // global memory), which hides the launch latency between the steps of a decode loop
+    // global memory), which hides the launch latency between the steps of a per-step decode loop
     cudaLaunchConfig_t lc{};
     lc.gridDim = dim3((unsigned)grid);
-    lc.blockDim = dim3((unsigned)(C.warps * 32));
+    lc.blockDim = dim3((unsigned)(STEP_WARPS * 32));
     lc.dynamicSmemBytes = smem;
     lc.stream = stream;
     cudaLaunchAttribute at[1];
@@ -304,17 +417,57 @@ cd_status launch_step_t(const cd::StepArgs& a, int grid, cudaStream_t stream) {
 template <int DT>
 cd_status launch_step_v(const cd::StepArgs& a, int grid, cudaStream_t stream) {
     if (a.inv_tau > 0.0f)  // sampling
-        return a.gather_max > 0 ? launch_step_t<DT, 0, true, true>(a, grid, stream)
-                                : launch_step_t<DT, 0, false, true>(a, grid, stream);
-    if (a.gather_max > 0) return launch_step_t<DT, 0, true>(a, grid, stream);  // density-adaptive rows
-    switch (step_variant()) {
-        case 1: return launch_step_t<DT, 1>(a, grid, stream);
-        case 2: return launch_step_t<DT, 2>(a, grid, stream);
-        case 3: return launch_step_t<DT, 3>(a, grid, stream);
-        case 4: return launch_step_t<DT, 4>(a, grid, stream);
-        case 5: return launch_step_t<DT, 5>(a, grid, stream);
-        default: return launch_step_t<DT, 0>(a, grid, stream);
+        return a.gather_max > 0 ? launch_step_t<DT, true, true>(a, grid, stream)
+                                : launch_step_t<DT, false, true>(a, grid, stream);
+    if (a.gather_max > 0) return launch_step_t<DT, true>(a, grid, stream);  // density-adaptive rows
+    return launch_step_t<DT>(a, grid, stream);
+}
+
+// Persistent loop: one cooperative launch (every CTA resident; they meet at a grid barrier after each
+// decoding step).  *fits = false if the device cannot hold the grid (then the caller uses per-step launches).
+template <int DT, bool GATHER = false, bool SAMPLE = false>
+cd_status launch_loop_t(const cd::StepArgs& a, const cd::LoopArgs& L, int grid, cudaStream_t stream, bool* fits) {
+    auto kern = cd::loop_kernel<DT, STEP_WARPS, STEP_STAGES, STEP_TILE, GATHER, SAMPLE>;
+    const size_t nwords = ((size_t)L.B + 31) / 32;
+    const size_t smem = sizeof(StepRing) * STEP_WARPS + ((2 * nwords + 1) * 4 + 15) / 16 * 16;
+    static thread_local int configured_dev = -1;
+    static thread_local int max_smem = 0;
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    if (configured_dev != dev) {
+        CU(cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
+        const size_t top = sizeof(StepRing) * STEP_WARPS + ((2 * ((size_t)cd::LOOP_MAX_ROWS / 32) + 1) * 4 + 15) / 16 * 16;
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(top < (size_t)max_smem ? top : (size_t)max_smem)));
+        configured_dev = dev;
     }
+    int per_sm = 0;
+    if (smem <= (size_t)max_smem) CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, STEP_WARPS * 32, smem));
+    int sms = 0;
+    CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    *fits = per_sm >= 1 && (long long)per_sm * sms >= grid;
+    if (!*fits) return CD_OK;
+    cudaLaunchConfig_t lc{};
+    lc.gridDim = dim3((unsigned)grid);
+    lc.blockDim = dim3((unsigned)(STEP_WARPS * 32));
+    lc.dynamicSmemBytes = smem;
+    lc.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeCooperative;
+    at[0].val.cooperative = 1;
+    lc.attrs = at;
+    lc.numAttrs = 1;
+    CU(cudaLaunchKernelEx(&lc, kern, a, L));
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return CD_OK;
+}
+
+template <int DT>
+cd_status launch_loop_v(const cd::StepArgs& a, const cd::LoopArgs& L, int grid, cudaStream_t stream, bool* fits) {
+    if (a.inv_tau > 0.0f)
+        return a.gather_max > 0 ? launch_loop_t<DT, true, true>(a, L, grid, stream, fits)
+                                : launch_loop_t<DT, false, true>(a, L, grid, stream, fits);
+    if (a.gather_max > 0) return launch_loop_t<DT, true>(a, L, grid, stream, fits);
+    return launch_loop_t<DT>(a, L, grid, stream, fits);
 }
 
 // Decode-loop extras of a step launch: per-row history + fused compaction (cd_step.cuh).
@@ -334,11 +487,9 @@ struct LoopExtras {
     int logits_by_slot = 0;
 };
 
-// n_upper bounds the active count; n_dev (device int) overrides n inside the kernel.
-cd_status launch_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype dtype, long long ld,
-                      const int* row_map, int* state, int n_upper, const int* n_dev, int* token_out,
-                      float* logprob_out, float* lse_out, uint8_t* done_out, cudaStream_t stream,
-                      const LoopExtras* x = nullptr) {
+// the arguments every step launch shares (one cd_step, one step of a per-step loop, or the persistent loop)
+cd::StepArgs make_step_args(const cd_dfa* d, const Settings& cfg, Scratch* s, cd_dtype dtype, long long ld,
+                            const LoopExtras* x) {
     cd::StepArgs a{};
     if (x) {
         a.hist_tokens = x->tokens;
@@ -357,30 +508,37 @@ cd_status launch_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype 
         a.logits_by_slot = x->logits_by_slot;
     }
     a.dfa = d->dev;
-    a.logits = static_cast<const unsigned char*>(logits);
     a.ld_bytes = ld * (dtype == CD_BF16 ? 2 : 4);
+    a.state_new = s->b.state_new;
+    a.partials = s->b.partials;
+    a.tickets = s->b.tickets;
+    a.ctrs = s->b.ctrs;
+    a.gather_max = gather_max_for(d, cfg, dtype);
+    a.all_gather = (d->max_deg <= a.gather_max) ? 1 : 0;
+    a.upw = units_per_warp();
+    a.tpu_max = tpu_max_tiles();
+    a.inv_tau = cfg.inv_tau;
+    a.seed_lo = (uint32_t)(cfg.seed & 0xFFFFFFFFull);
+    a.seed_hi = (uint32_t)(cfg.seed >> 32);
+    a.rng_step_base = cfg.rng_step_base;
+    return a;
+}
+
+// n_upper bounds the active count; n_dev (device int) overrides n inside the kernel.
+cd_status launch_step(const cd_dfa* d, const Settings& cfg, Scratch* s, const void* logits, cd_dtype dtype, long long ld,
+                      const int* row_map, int* state, int n_upper, const int* n_dev, int* token_out,
+                      float* logprob_out, float* lse_out, uint8_t* done_out, cudaStream_t stream,
+                      const LoopExtras* x = nullptr) {
+    cd::StepArgs a = make_step_args(d, cfg, s, dtype, ld, x);
+    a.logits = static_cast<const unsigned char*>(logits);
     a.row_map = row_map;
     a.state = state;
-    a.state_new = s->state_new;
     a.n = n_upper;
     a.n_dev = n_dev;
     a.token_out = token_out;
     a.logprob_out = logprob_out;
     a.lse_out = lse_out;
     a.done_out = done_out;
-    a.partials = s->partials;
-    a.tickets = s->tickets;
-    a.ctrs = s->ctrs;
-    a.gather_max = gather_max_for(d, dtype);
-    a.all_gather = (d->max_deg <= a.gather_max) ? 1 : 0;
-    static const int env_upw = [] { const char* e = std::getenv("CD_UPW"); const int v = e ? std::atoi(e) : 0; return (v >= 1 && v <= 32) ? v : cd::UNITS_PER_WARP; }();
-    static const int env_tpu = [] { const char* e = std::getenv("CD_TPU_MAX"); const int v = e ? std::atoi(e) : 0; return v >= 1 ? v : (1 << 20); }();
-    a.upw = env_upw;
-    a.tpu_max = env_tpu;
-    a.inv_tau = d->inv_tau;
-    a.seed_lo = (uint32_t)(d->seed & 0xFFFFFFFFull);
-    a.seed_hi = (uint32_t)(d->seed >> 32);
-    a.rng_step_base = d->rng_step_base;
     const int grid = step_grid(d, n_upper, dtype);
     return dtype == CD_BF16 ? launch_step_v<cd::DT_BF16>(a, grid, stream)
                             : launch_step_v<cd::DT_F32>(a, grid, stream);
@@ -440,8 +598,10 @@ cd_status compile_impl(int32_t V, int32_t S, int32_t start, const int64_t* row_p
     cudaError_t e = cudaGetDeviceProperties(&prop, device);
     if (e != cudaSuccess) { delete d; return fail(CD_ERR_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e)); }
     d->num_sms = prop.multiProcessorCount;
+    d->coop_launch = prop.cooperativeLaunch;
     const int W = (V + 31) / 32;
     const int Wpad = (W + 3) & ~3;
+    const int nblk = (V + 1023) / 1024;
     const size_t mask_bytes = (size_t)S * Wpad * 4;
     cd_status st = CD_OK;
     auto alloc = [&](void** p, size_t bytes) {
@@ -455,6 +615,8 @@ cd_status compile_impl(int32_t V, int32_t S, int32_t start, const int64_t* row_p
     alloc(&d->d_tok, sizeof(int) * (size_t)nnz);
     alloc(&d->d_next, sizeof(int) * (size_t)nnz);
     alloc(&d->d_acc, (size_t)S);
+    alloc(&d->d_rank, sizeof(int) * (size_t)S * nblk);
+    alloc(&d->d_satisfying, (size_t)S);
     auto copy = [&](void* dst, const void* src, size_t bytes) {
         if (st != CD_OK || bytes == 0) return;
         cudaError_t e2 = cudaMemcpy(dst, src, bytes, cudaMemcpyHostToDevice);
@@ -467,10 +629,11 @@ cd_status compile_impl(int32_t V, int32_t S, int32_t start, const int64_t* row_p
     copy(d->d_acc, accepting, (size_t)S);
     if (st == CD_OK) {
         cudaError_t e2 = cudaMemset(d->d_mask, 0, mask_bytes);
+        if (e2 == cudaSuccess) e2 = cudaMemset(d->d_satisfying, 0, (size_t)S);
+        const int threads = 256;
+        long long blocks = ((long long)S * 32 + threads - 1) / threads;
+        if (blocks > 65535) blocks = 65535;
         if (e2 == cudaSuccess && nnz > 0) {
-            const int threads = 256;
-            long long blocks = ((long long)S * 32 + threads - 1) / threads;
-            if (blocks > 65535) blocks = 65535;
             cd::build_mask_kernel<<<(int)blocks, threads>>>(static_cast<const long long*>(d->d_row_ptr),
                                                            static_cast<const int*>(d->d_tok),
                                                            static_cast<int*>(d->d_next),
@@ -478,12 +641,19 @@ cd_status compile_impl(int32_t V, int32_t S, int32_t start, const int64_t* row_p
                                                            static_cast<uint32_t*>(d->d_mask));
             g_launches.fetch_add(1, std::memory_order_relaxed);
             e2 = cudaGetLastError();
-            if (e2 == cudaSuccess) e2 = cudaDeviceSynchronize();
         }
+        if (e2 == cudaSuccess) {
+            cd::build_rank_kernel<<<(int)blocks, threads>>>(static_cast<const uint32_t*>(d->d_mask), S, Wpad, nblk,
+                                                           static_cast<int*>(d->d_rank));
+            g_launches.fetch_add(1, std::memory_order_relaxed);
+            e2 = cudaGetLastError();
+        }
+        if (e2 == cudaSuccess) e2 = cudaDeviceSynchronize();
         if (e2 != cudaSuccess) st = fail(CD_ERR_CUDA, "mask build: %s", cudaGetErrorString(e2));
     }
     if (st != CD_OK) {
         cudaFree(d->d_mask); cudaFree(d->d_row_ptr); cudaFree(d->d_tok); cudaFree(d->d_next); cudaFree(d->d_acc);
+        cudaFree(d->d_rank); cudaFree(d->d_satisfying);
         delete d;
         return st;
     }
@@ -496,7 +666,24 @@ cd_status compile_impl(int32_t V, int32_t S, int32_t start, const int64_t* row_p
     d->dev.tok = static_cast<const int*>(d->d_tok);
     d->dev.next = static_cast<const int*>(d->d_next);
     d->dev.accepting = static_cast<const uint8_t*>(d->d_acc);
+    d->dev.rank1k = static_cast<const int*>(d->d_rank);
+    d->dev.nblk = nblk;
     *out = d;
+    return CD_OK;
+}
+
+cd_status compile_csr(int32_t V, const cdt::HostCsr& c, int device, cd_dfa_t** out) {
+    return compile_impl(V, c.S, 0, c.row_ptr.data(), c.tok.data(), c.next.data(), c.accepting.data(), device, out);
+}
+
+cd_status copy_csr_out(const cdt::HostCsr& c, int32_t* S_out, int64_t* nnz_out, int64_t* row_ptr_out, int32_t* tok_out,
+                       int32_t* next_out, uint8_t* accepting_out) {
+    *S_out = c.S;
+    *nnz_out = (int64_t)c.tok.size();
+    if (row_ptr_out) std::memcpy(row_ptr_out, c.row_ptr.data(), sizeof(int64_t) * c.row_ptr.size());
+    if (tok_out && !c.tok.empty()) std::memcpy(tok_out, c.tok.data(), sizeof(int32_t) * c.tok.size());
+    if (next_out && !c.next.empty()) std::memcpy(next_out, c.next.data(), sizeof(int32_t) * c.next.size());
+    if (accepting_out) std::memcpy(accepting_out, c.accepting.data(), c.accepting.size());
     return CD_OK;
 }
 
@@ -506,38 +693,61 @@ struct LimitArgs {
 };
 
 // the LIMIT a loop runs under: the explicit one (cd_decode_loop_limit), else the handle's (cd_set_limit)
-LimitArgs resolve_limit(const cd_dfa* d, const LimitArgs& explicit_lim = LimitArgs()) {
+LimitArgs resolve_limit(const Settings& cfg, const LimitArgs& explicit_lim = LimitArgs()) {
     if (explicit_lim.sat_ctr) return explicit_lim;
     LimitArgs l;
-    if (d->limit_ctr && d->d_satisfying) {
-        l.sat_ctr = d->limit_ctr;
-        l.limit = d->limit;
+    if (cfg.limit_ctr && cfg.has_satisfying) {
+        l.sat_ctr = cfg.limit_ctr;
+        l.limit = cfg.limit;
     }
     return l;
 }
 
+// persist: also initialise the bitmaps / states / counters of loop_kernel
 cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, int* tokens_out, int* len_out,
                            int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream,
-                           const LimitArgs& lim = LimitArgs()) {
+                           const LimitArgs& lim = LimitArgs(), bool persist = false) {
     long long work = (long long)B * (max_steps > 0 ? max_steps : 1);
     long long blocks = (work + 255) / 256;
     if (blocks < 1) blocks = 1;
     if (blocks > 4096) blocks = 4096;
-    cd::loop_init_kernel<<<(int)blocks, 256, 0, stream>>>(B, max_steps, d->start, d->start_accepting, s->row_ids[0],
-                                                          s->state[0], s->n_active, tokens_out, len_out,
-                                                          final_state_out, sum_logprob_out, done_out, lim.sat_ctr,
-                                                          lim.limit);
+    cd::LoopInitArgs a{};
+    a.B = B;
+    a.max_steps = max_steps;
+    a.start = d->start;
+    a.start_accepting = d->start_accepting;
+    a.tokens_out = tokens_out;
+    a.len_out = len_out;
+    a.final_state_out = final_state_out;
+    a.sum_logprob_out = sum_logprob_out;
+    a.done_row_out = done_out;
+    a.sat_ctr = lim.sat_ctr;
+    a.limit = lim.limit;
+    a.ctrs = s->b.ctrs;
+    if (persist) {
+        for (int i = 0; i < 3; ++i) a.alive[i] = s->b.alive[i];
+        for (int i = 0; i < 2; ++i) a.state2[i] = s->b.state2[i];
+        a.work = s->loop_work;
+        a.bar = s->b.bar;
+    } else {
+        a.row_ids = s->b.row_ids[0];
+        a.state = s->b.state[0];
+        a.n_active = s->b.n_active;
+    }
+    cd::loop_init_kernel<<<(int)blocks, 256, 0, stream>>>(a);
     CU(cudaGetLastError());
     g_launches.fetch_add(1, std::memory_order_relaxed);
+    s->trace_valid = false;
     return CD_OK;
 }
 
-// One loop iteration k on `logits` ([B, ld], original row ids): ONE launch -- the step kernel
-// records the per-row history as rows finalise and its last CTA compacts the active list.
-cd_status enqueue_loop_step(const cd_dfa* d, Scratch* s, const void* logits, cd_dtype dtype, long long ld, int B,
-                            int k, int max_steps, int* tokens_out, int* len_out, int* final_state_out,
-                            float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream,
+// One iteration k of a per-step loop on `logits` ([B, ld], original row ids): ONE launch -- the step
+// kernel records the per-row history as rows finalise and its last CTA compacts the active list.
+cd_status enqueue_loop_step(const cd_dfa* d, const Settings& cfg, Scratch* s, const void* logits, cd_dtype dtype,
+                            long long ld, int B, int k, int max_steps, int* tokens_out, int* len_out,
+                            int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream,
                             const LimitArgs& lim = LimitArgs(), int logits_by_slot = 0) {
+    RangeGuard range("cd decoding step");
     const int cur = k & 1, nxt = cur ^ 1;
     LoopExtras x;
     x.logits_by_slot = logits_by_slot;
@@ -553,23 +763,160 @@ cd_status enqueue_loop_step(const cd_dfa* d, Scratch* s, const void* logits, cd_
     x.done = done_out;
     x.step = k;
     x.max_steps = max_steps;
-    x.row_ids_out = s->row_ids[nxt];
-    x.state_out = s->state[nxt];
-    x.n_out = s->n_active + nxt;
-    return launch_step(d, s, logits, dtype, ld, s->row_ids[cur], s->state[cur], B, s->n_active + cur, s->token,
-                       s->logprob, nullptr, s->done, stream, &x);
+    x.row_ids_out = s->b.row_ids[nxt];
+    x.state_out = s->b.state[nxt];
+    x.n_out = s->b.n_active + nxt;
+    return launch_step(d, cfg, s, logits, dtype, ld, s->b.row_ids[cur], s->b.state[cur], B, s->b.n_active + cur,
+                       s->b.token, s->b.logprob, nullptr, s->b.done, stream, &x);
 }
 
-cd_status check_sticky_errors(Scratch* s, cudaStream_t stream) {
-    int h[4] = {0, 0, 0, 0};
-    CU(cudaMemcpyAsync(h, s->ctrs, sizeof h, cudaMemcpyDeviceToHost, stream));
-    CU(cudaStreamSynchronize(stream));
-    if (h[2] != 0) {
-        int zero = 0;
-        cudaMemcpyAsync(s->ctrs + 2, &zero, sizeof zero, cudaMemcpyHostToDevice, stream);
-        cudaStreamSynchronize(stream);
-        return fail(CD_ERR_INTERNAL, "%d device-side consistency failures (state out of range or token missing from CSR)", h[2]);
+// The whole loop in ONE cooperative launch (cd_step.cuh loop_kernel).  *launched = false when this loop
+// cannot take that path (too many rows for the bitmap snapshot, no cooperative launch, CTAs do not fit):
+// the caller then enqueues per-step launches.
+cd_status enqueue_persistent_loop(const cd_dfa* d, const Settings& cfg, Scratch* s, const void* const* step_logits,
+                                  cd_dtype dtype, long long ld, int B, int max_steps, int* tokens_out, int* len_out,
+                                  int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream,
+                                  const LimitArgs& lim, bool* launched) {
+    RangeGuard range("cd decode loop (persistent kernel)");
+    *launched = false;
+    LoopExtras x;
+    if (lim.sat_ctr) {
+        x.satisfying = static_cast<const uint8_t*>(d->d_satisfying);
+        x.sat_ctr = lim.sat_ctr;
+        x.limit = lim.limit;
     }
+    x.tokens = tokens_out;
+    x.len = len_out;
+    x.final_state = final_state_out;
+    x.sum_logprob = sum_logprob_out;
+    x.done = done_out;
+    x.max_steps = max_steps;
+    cd::StepArgs a = make_step_args(d, cfg, s, dtype, ld, &x);
+    a.n = B;
+    cd::LoopArgs L{};
+    if (max_steps <= cd::LOOP_PARAM_STEPS) {
+        for (int k = 0; k < max_steps; ++k) L.step_ptrs[k] = step_logits[k];
+    } else {
+        CU(cudaMemcpyAsync(s->loop_ptrs, step_logits, sizeof(void*) * (size_t)max_steps, cudaMemcpyHostToDevice, stream));
+        L.step_ptrs_dev = s->loop_ptrs;
+    }
+    L.B = B;
+    for (int i = 0; i < 3; ++i) L.alive[i] = s->b.alive[i];
+    for (int i = 0; i < 2; ++i) L.state2[i] = s->b.state2[i];
+    L.work = s->loop_work;
+    L.bar = s->b.bar;
+    L.trace_t = s->b.trace_t;
+    L.trace_n = s->b.trace_n;
+#ifdef CD_TUNING
+    L.phase = s->b.phase;
+    CU(cudaMemsetAsync(s->b.phase, 0, sizeof(unsigned long long) * (size_t)cd::LOOP_TRACE_STEPS * 8, stream));
+#endif
+    const int grid = step_grid(d, B, dtype);
+    const cd_status st = dtype == CD_BF16 ? launch_loop_v<cd::DT_BF16>(a, L, grid, stream, launched)
+                                          : launch_loop_v<cd::DT_F32>(a, L, grid, stream, launched);
+    if (st == CD_OK && *launched) s->trace_valid = true;
+    return st;
+}
+
+std::mutex& coop_mutex(int dev) {
+    static std::mutex mu[64];
+    return mu[dev & 63];
+}
+
+// can this loop run in loop_kernel at all?  (the launch itself still checks that the CTAs fit)
+bool persistent_loop_possible(const cd_dfa* d, const Settings& cfg, int B, int max_steps) {
+    return cfg.loop_mode != CD_LOOP_PER_STEP && d->coop_launch && B <= cd::LOOP_MAX_ROWS && max_steps > 0 &&
+           !d->start_accepting;
+}
+
+// per-step work counters / device step pointers of the persistent loop
+cd_status get_loop_scratch(Scratch* s, int max_steps, cudaStream_t stream) {
+    if (s->loop_steps_cap >= max_steps) return CD_OK;
+    int* work = nullptr;
+    const void** ptrs = nullptr;
+    const int cap = max_steps < 64 ? 64 : max_steps;
+    CU(dev_alloc(&work, (size_t)cap));
+    if (dev_alloc(&ptrs, (size_t)cap) != cudaSuccess) {
+        cudaFree(work);
+        return fail(CD_ERR_OOM, "loop scratch for %d steps", max_steps);
+    }
+    if (s->loop_steps_cap > 0) cudaStreamSynchronize(stream);
+    cudaFree(s->loop_work);
+    cudaFree(s->loop_ptrs);
+    s->loop_work = work;
+    s->loop_ptrs = ptrs;
+    s->loop_steps_cap = cap;
+    return CD_OK;
+}
+
+// Stream-ordered scratch (cudaMallocAsync) must not be handed back to the OS at every synchronisation:
+// keep the default pool's memory (once per device).
+void keep_pool_memory(int dev) {
+    static std::mutex mu;
+    static std::map<int, bool> done;
+    std::lock_guard<std::mutex> lk(mu);
+    if (done[dev]) return;
+    cudaMemPool_t pool = nullptr;
+    if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess && pool) {
+        unsigned long long thr = ~0ull;
+        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+    }
+    done[dev] = true;
+}
+
+cd_status device_of(const void* p, int* dev) {
+    cudaPointerAttributes at;
+    CU(cudaPointerGetAttributes(&at, p));
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
+        return fail(CD_ERR_ARG, "expected a DEVICE pointer");
+    *dev = at.device;
+    return CD_OK;
+}
+
+// Stable compaction of n slots (a6): one CTA up to one chunk (no allocation: capturable in a CUDA graph),
+// above that the single-pass look-back kernel over ceil(n / 4096) CTAs with stream-ordered scratch for the
+// chunk states.  rank_out: see compact_lookback_kernel.
+cd_status launch_compact(const uint8_t* done, const int* row_ids_in, const int* state_in, int n, int* row_ids_out,
+                         int* state_out, int* n_out, int* rank_out, cudaStream_t stream) {
+    if (n <= cd::SCAN_CHUNK && !rank_out) {
+        cd::compact_kernel<<<1, 1024, 0, stream>>>(done, row_ids_in, state_in, n, row_ids_out, state_out, n_out);
+        CU(cudaGetLastError());
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        return CD_OK;
+    }
+    int dev = 0;
+    cd_status st = device_of(n_out, &dev);
+    if (st != CD_OK) return st;
+    DeviceGuard guard(dev);
+    keep_pool_memory(dev);
+    const int chunks = n > 0 ? (n + cd::SCAN_CHUNK - 1) / cd::SCAN_CHUNK : 1;
+    const size_t bytes = sizeof(unsigned long long) * ((size_t)chunks + 1);
+    unsigned long long* tile = nullptr;
+    CU(cudaMallocAsync(reinterpret_cast<void**>(&tile), bytes, stream));
+    cudaError_t e = cudaMemsetAsync(tile, 0, bytes, stream);
+    if (e == cudaSuccess) {
+        cd::compact_lookback_kernel<<<chunks, 1024, 0, stream>>>(done, row_ids_in, state_in, n, row_ids_out, state_out,
+                                                                n_out, rank_out, tile, reinterpret_cast<int*>(tile + chunks));
+        e = cudaGetLastError();
+    }
+    cudaFreeAsync(tile, stream);  // on every path
+    if (e != cudaSuccess) return fail(CD_ERR_CUDA, "compaction launch: %s", cudaGetErrorString(e));
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return CD_OK;
+}
+
+// End of every loop: one read of the error counter (and of the persistent loop's abort flag) and the one
+// stream synchronisation the loops promise.
+cd_status finish_loop(Scratch* s, cudaStream_t stream, bool persistent) {
+    int h[4] = {0, 0, 0, 0};
+    int hb[4] = {0, 0, 0, 0};
+    CU(cudaMemcpyAsync(h, s->b.ctrs, sizeof h, cudaMemcpyDeviceToHost, stream));
+    if (persistent) CU(cudaMemcpyAsync(hb, s->b.bar, sizeof hb, cudaMemcpyDeviceToHost, stream));
+    CU(cudaStreamSynchronize(stream));
+    if (hb[2] != 0)
+        return fail(CD_ERR_INTERNAL, "the persistent loop kernel timed out at a grid barrier (device shared with a kernel that never ends?)");
+    if (h[2] != 0)
+        return fail(CD_ERR_INTERNAL, "%d device-side consistency failures (state out of range or token missing from the CSR)", h[2]);
     return CD_OK;
 }
 
@@ -593,50 +940,34 @@ cd_status cd_compile_dfa(int32_t V, int32_t S, int32_t start, const int64_t* row
     }
 }
 
-cd_status cd_compile_trie(int32_t V, int32_t K, const int64_t* label_ptr, const int32_t* label_tok, int device,
-                          cd_dfa_t** out) {
+cd_status cd_build_trie(int32_t V, int32_t K, const int64_t* label_ptr, const int32_t* label_tok, int32_t eos,
+                        int32_t* S_out, int64_t* nnz_out, int64_t* row_ptr_out, int32_t* tok_out, int32_t* next_out,
+                        uint8_t* accepting_out) {
+    try {
+        if (!label_ptr || !S_out || !nnz_out) return fail(CD_ERR_ARG, "NULL argument");
+        if (V < 1 || K < 1) return fail(CD_ERR_ARG, "V and K must be >= 1");
+        if (label_ptr[K] > 0 && !label_tok) return fail(CD_ERR_ARG, "label_tok is NULL");
+        cdt::HostCsr c;
+        const std::string err = cdt::build_trie(V, K, label_ptr, label_tok, eos, &c);
+        if (!err.empty()) return fail(CD_ERR_AUTOMATON, "%s", err.c_str());
+        return copy_csr_out(c, S_out, nnz_out, row_ptr_out, tok_out, next_out, accepting_out);
+    } catch (const std::bad_alloc&) {
+        return fail(CD_ERR_OOM, "host allocation failed");
+    } catch (...) {
+        return fail(CD_ERR_INTERNAL, "unexpected exception");
+    }
+}
+
+cd_status cd_compile_trie(int32_t V, int32_t K, const int64_t* label_ptr, const int32_t* label_tok, int32_t eos,
+                          int device, cd_dfa_t** out) {
     try {
         if (!out || !label_ptr) return fail(CD_ERR_ARG, "NULL argument");
         if (V < 1 || K < 1) return fail(CD_ERR_ARG, "V and K must be >= 1");
-        if (label_ptr[0] != 0) return fail(CD_ERR_AUTOMATON, "label_ptr[0] must be 0");
         if (label_ptr[K] > 0 && !label_tok) return fail(CD_ERR_ARG, "label_tok is NULL");
-        // trie in insertion order; children kept sorted per node
-        std::vector<std::map<int, int>> child(1);
-        std::vector<uint8_t> leaf(1, 0);
-        for (int k = 0; k < K; ++k) {
-            const long long lo = label_ptr[k], hi = label_ptr[k + 1];
-            if (hi <= lo) return fail(CD_ERR_AUTOMATON, "label %d is empty", k);
-            int node = 0;
-            for (long long j = lo; j < hi; ++j) {
-                const int t = label_tok[j];
-                if (t < 0 || t >= V) return fail(CD_ERR_AUTOMATON, "label %d: token %d outside [0,%d)", k, t, V);
-                if (leaf[node]) return fail(CD_ERR_AUTOMATON, "label %d extends another label (not prefix-free)", k);
-                auto it = child[node].find(t);
-                if (it == child[node].end()) {
-                    const int nn = (int)child.size();
-                    child[node][t] = nn;
-                    child.emplace_back();
-                    leaf.push_back(0);
-                    node = nn;
-                } else {
-                    node = it->second;
-                }
-            }
-            if (leaf[node] || !child[node].empty())
-                return fail(CD_ERR_AUTOMATON, "label %d duplicates or is a prefix of another label", k);
-            leaf[node] = 1;
-        }
-        const int S = (int)child.size();
-        std::vector<int64_t> rp(S + 1, 0);
-        std::vector<int32_t> tk, nx;
-        for (int s = 0; s < S; ++s) {
-            for (auto& kv : child[s]) {
-                tk.push_back(kv.first);
-                nx.push_back(kv.second);
-            }
-            rp[s + 1] = (int64_t)tk.size();
-        }
-        return compile_impl(V, S, 0, rp.data(), tk.data(), nx.data(), leaf.data(), device, out);
+        cdt::HostCsr c;
+        const std::string err = cdt::build_trie(V, K, label_ptr, label_tok, eos, &c);
+        if (!err.empty()) return fail(CD_ERR_AUTOMATON, "%s", err.c_str());
+        return compile_csr(V, c, device, out);
     } catch (const std::bad_alloc&) {
         return fail(CD_ERR_OOM, "host allocation failed");
     } catch (...) {
@@ -649,7 +980,7 @@ void cd_free_dfa(cd_dfa_t* d) {
     DeviceGuard guard(d->device);
     for (auto& kv : d->scratch) kv.second.release();
     cudaFree(d->d_mask); cudaFree(d->d_row_ptr); cudaFree(d->d_tok); cudaFree(d->d_next); cudaFree(d->d_acc);
-    cudaFree(d->d_satisfying);
+    cudaFree(d->d_rank); cudaFree(d->d_satisfying);
     delete d;
 }
 
@@ -666,7 +997,16 @@ cd_status cd_dfa_info(const cd_dfa_t* d, int32_t* V, int32_t* S, int32_t* start,
 cd_status cd_set_gather_max(cd_dfa_t* d, int32_t max_transitions) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
     if (max_transitions < -1) return fail(CD_ERR_ARG, "max_transitions must be >= -1");
-    d->gather_max = max_transitions;
+    std::lock_guard<std::mutex> lk(d->mu);
+    d->cfg.gather_max = max_transitions;
+    return CD_OK;
+}
+
+cd_status cd_set_loop_mode(cd_dfa_t* d, int32_t mode) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (mode != CD_LOOP_AUTO && mode != CD_LOOP_PER_STEP) return fail(CD_ERR_ARG, "mode must be CD_LOOP_AUTO or CD_LOOP_PER_STEP");
+    std::lock_guard<std::mutex> lk(d->mu);
+    d->cfg.loop_mode = mode;
     return CD_OK;
 }
 
@@ -675,7 +1015,7 @@ cd_status cd_reserve(const cd_dfa_t* d, int32_t max_rows, void* cuda_stream) {
     if (max_rows < 0) return fail(CD_ERR_ARG, "max_rows < 0");
     DeviceGuard guard(d->device);
     Scratch* s = nullptr;
-    return get_scratch(d, static_cast<cudaStream_t>(cuda_stream), max_rows, true, &s);
+    return get_scratch(d, static_cast<cudaStream_t>(cuda_stream), max_rows, &s);
 }
 
 cd_status cd_step(const cd_dfa_t* d, const void* logits, cd_dtype dtype, int64_t ld_elems, const int32_t* row_map,
@@ -693,10 +1033,11 @@ cd_status cd_step(const cd_dfa_t* d, const void* logits, cd_dtype dtype, int64_t
         return fail(CD_ERR_ARG, "n * tiles_per_row overflows the unit index");
     DeviceGuard guard(d->device);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const Settings cfg = settings_of(d);
     Scratch* s = nullptr;
-    st = get_scratch(d, stream, n, false, &s);
+    st = get_scratch(d, stream, n, &s);
     if (st != CD_OK) return st;
-    return launch_step(d, s, logits, dtype, ld_elems, row_map, state, n, nullptr, token_out, logprob_out, lse_out,
+    return launch_step(d, cfg, s, logits, dtype, ld_elems, row_map, state, n, nullptr, token_out, logprob_out, lse_out,
                        done_out, stream);
 }
 
@@ -723,11 +1064,8 @@ cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, const int32
     if (!n_active_out) return fail(CD_ERR_ARG, "n_active_out is NULL");
     if (n > 0 && (!done || !row_ids_out)) return fail(CD_ERR_ARG, "NULL pointer");
     if (n > 0 && state_in && !state_out) return fail(CD_ERR_ARG, "state_in given without state_out");
-    cd::compact_kernel<<<1, 1024, 0, static_cast<cudaStream_t>(cuda_stream)>>>(done, row_ids_in, state_in, n, row_ids_out,
-                                                                              state_out, n_active_out);
-    CU(cudaGetLastError());
-    g_launches.fetch_add(1, std::memory_order_relaxed);
-    return CD_OK;
+    return launch_compact(done, row_ids_in, state_in, n, row_ids_out, state_out, n_active_out, nullptr,
+                          static_cast<cudaStream_t>(cuda_stream));
 }
 
 static cd_status decode_loop_impl(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
@@ -736,7 +1074,8 @@ static cd_status decode_loop_impl(const cd_dfa_t* d, const void* const* step_log
                                   const LimitArgs& lim_in, void* cuda_stream) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
     if (B < 0 || max_steps < 0) return fail(CD_ERR_ARG, "B / max_steps < 0");
-    const LimitArgs lim = resolve_limit(d, lim_in);
+    const Settings cfg = settings_of(d);
+    const LimitArgs lim = resolve_limit(cfg, lim_in);
     cd_status st = check_dtype(dtype);
     if (st != CD_OK) return st;
     if (B == 0) return CD_OK;
@@ -748,21 +1087,43 @@ static cd_status decode_loop_impl(const cd_dfa_t* d, const void* const* step_log
             st = check_logits_layout(d, step_logits[k], dtype, ld_elems);
             if (st != CD_OK) return st;
         }
+    RangeGuard range("cd_decode_loop");
     DeviceGuard guard(d->device);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     Scratch* s = nullptr;
-    st = get_scratch(d, stream, B, true, &s);
+    st = get_scratch(d, stream, B, &s);
     if (st != CD_OK) return st;
-    st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream,
-                          lim);
-    if (st != CD_OK) return st;
-    if (!d->start_accepting)
-        for (int k = 0; k < max_steps; ++k) {
-            st = enqueue_loop_step(d, s, step_logits[k], dtype, ld_elems, B, k, max_steps, tokens_out, len_out,
-                                   final_state_out, sum_logprob_out, done_out, stream, lim);
-            if (st != CD_OK) return st;
-        }
-    return check_sticky_errors(s, stream);
+    bool persist = persistent_loop_possible(d, cfg, B, max_steps);
+    // Two persistent loops must never share the SMs: each waits at its grid barrier for CTAs that the
+    // other one keeps from being scheduled.  Within this process they are serialised per device (the loop
+    // synchronises its stream before returning anyway).
+    std::unique_lock<std::mutex> coop_lock;
+    if (persist) coop_lock = std::unique_lock<std::mutex>(coop_mutex(d->device));
+    if (persist) {
+        st = get_loop_scratch(s, max_steps, stream);
+        if (st != CD_OK) return st;
+        // both forms of the set-up are cheap; the persistent one is tried first and tells whether its CTAs fit
+        st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out,
+                              stream, lim, true);
+        if (st != CD_OK) return st;
+        bool launched = false;
+        st = enqueue_persistent_loop(d, cfg, s, step_logits, dtype, ld_elems, B, max_steps, tokens_out, len_out,
+                                     final_state_out, sum_logprob_out, done_out, stream, lim, &launched);
+        if (st != CD_OK) return st;
+        persist = launched;
+    }
+    if (!persist) {
+        st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out,
+                              stream, lim);
+        if (st != CD_OK) return st;
+        if (!d->start_accepting)
+            for (int k = 0; k < max_steps; ++k) {
+                st = enqueue_loop_step(d, cfg, s, step_logits[k], dtype, ld_elems, B, k, max_steps, tokens_out, len_out,
+                                       final_state_out, sum_logprob_out, done_out, stream, lim);
+                if (st != CD_OK) return st;
+            }
+    }
+    return finish_loop(s, stream, persist);
 }
 
 cd_status cd_decode_loop(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
@@ -772,16 +1133,69 @@ cd_status cd_decode_loop(const cd_dfa_t* d, const void* const* step_logits, cd_d
                             sum_logprob_out, done_out, LimitArgs(), cuda_stream);
 }
 
+cd_status cd_loop_trace(const cd_dfa_t* d, void* cuda_stream, int32_t cap, int64_t* t_ns_out, int32_t* n_active_out,
+                        int32_t* steps_out) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    if (cap < 0 || !steps_out || (cap > 0 && (!t_ns_out || !n_active_out))) return fail(CD_ERR_ARG, "bad argument");
+    DeviceGuard guard(d->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    cd_dfa* dm = const_cast<cd_dfa*>(d);
+    const unsigned long long* tt = nullptr;
+    const int* tn = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(dm->mu);
+        auto it = dm->scratch.find(stream);
+        if (it != dm->scratch.end() && it->second.trace_valid) {
+            tt = it->second.b.trace_t;
+            tn = it->second.b.trace_n;
+        }
+    }
+    *steps_out = 0;
+    if (!tt) return CD_OK;  // the last loop on this stream did not run in the persistent kernel
+    std::vector<unsigned long long> ht((size_t)cd::LOOP_TRACE_STEPS + 1);
+    std::vector<int> hn((size_t)cd::LOOP_TRACE_STEPS + 1);
+    CU(cudaMemcpyAsync(ht.data(), tt, sizeof(unsigned long long) * ht.size(), cudaMemcpyDeviceToHost, stream));
+    CU(cudaMemcpyAsync(hn.data(), tn, sizeof(int) * hn.size(), cudaMemcpyDeviceToHost, stream));
+    CU(cudaStreamSynchronize(stream));
+    int steps = hn[cd::LOOP_TRACE_STEPS];
+    if (steps > cd::LOOP_TRACE_STEPS) steps = cd::LOOP_TRACE_STEPS;
+    *steps_out = steps;
+    for (int k = 0; k < steps && k < cap; ++k) {
+        n_active_out[k] = hn[(size_t)k];
+        t_ns_out[k] = (int64_t)(ht[(size_t)k + 1] - ht[(size_t)k]);
+    }
+    return CD_OK;
+}
+
+#ifdef CD_TUNING
+// tuning builds only (not declared in cd.h): the raw phase timestamps of the last persistent loop
+__attribute__((visibility("default"))) cd_status cd_loop_phase_trace(const cd_dfa_t* d, void* cuda_stream, uint64_t* out /*[256][8]*/,
+                                                                      uint64_t* t_out /*[257]*/) {
+    DeviceGuard guard(d->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    cd_dfa* dm = const_cast<cd_dfa*>(d);
+    Scratch* s = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(dm->mu);
+        s = &dm->scratch[stream];
+    }
+    CU(cudaMemcpyAsync(out, s->b.phase, sizeof(uint64_t) * (size_t)cd::LOOP_TRACE_STEPS * 8, cudaMemcpyDeviceToHost, stream));
+    CU(cudaMemcpyAsync(t_out, s->b.trace_t, sizeof(uint64_t) * ((size_t)cd::LOOP_TRACE_STEPS + 1), cudaMemcpyDeviceToHost, stream));
+    CU(cudaStreamSynchronize(stream));
+    return CD_OK;
+}
+#endif
+
 cd_status cd_set_satisfying(cd_dfa_t* d, const uint8_t* satisfying) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
     DeviceGuard guard(d->device);
+    std::lock_guard<std::mutex> lk(d->mu);
     if (!satisfying) {
-        cudaFree(d->d_satisfying);
-        d->d_satisfying = nullptr;
+        d->cfg.has_satisfying = false;  // the device array stays allocated: a loop in flight may still read it
         return CD_OK;
     }
-    if (!d->d_satisfying) CU(cudaMalloc(&d->d_satisfying, (size_t)d->dev.S));
     CU(cudaMemcpy(d->d_satisfying, satisfying, (size_t)d->dev.S, cudaMemcpyHostToDevice));
+    d->cfg.has_satisfying = true;
     return CD_OK;
 }
 
@@ -790,7 +1204,7 @@ cd_status cd_decode_loop_limit(const cd_dfa_t* d, const void* const* step_logits
                                int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out, int32_t limit,
                                int32_t* satisfied_inout, void* cuda_stream) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
-    if (!d->d_satisfying) return fail(CD_ERR_ARG, "cd_set_satisfying has not been called on this automaton");
+    if (!settings_of(d).has_satisfying) return fail(CD_ERR_ARG, "cd_set_satisfying has not been called on this automaton");
     if (!satisfied_inout) return fail(CD_ERR_ARG, "satisfied_inout is NULL");
     if (limit < 0) return fail(CD_ERR_ARG, "limit < 0");
     LimitArgs lim;
@@ -818,121 +1232,98 @@ cd_status cd_decode_loop_host(const cd_dfa_t* d, const void* const* step_logits_
     for (int k = 0; k < max_steps; ++k)
         if (!step_logits_host[k]) return fail(CD_ERR_ARG, "step_logits_host[%d] is NULL", k);
 
+    RangeGuard range("cd_decode_loop_host");
     DeviceGuard guard(d->device);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const Settings cfg = settings_of(d);
     Scratch* s = nullptr;
-    st = get_scratch(d, stream, B, true, &s);
+    st = get_scratch(d, stream, B, &s);
     if (st != CD_OK) return st;
 
-    // staging + device copies of the outputs, kept in the scratch area
+    // one staging buffer (the active rows of one step, compact) + device copies of the outputs
     const size_t step_bytes = (size_t)B * (size_t)ld_elems * (size_t)sz;
-    if (s->stage_bytes < step_bytes) {
-        CU(cudaStreamSynchronize(stream));
-        for (int i = 0; i < 2; ++i) { cudaFree(s->stage[i]); s->stage[i] = nullptr; }
-        s->stage_bytes = 0;
-        for (int i = 0; i < 2; ++i) CU(cudaMalloc(&s->stage[i], step_bytes));
-        s->stage_bytes = step_bytes;
-    }
     const size_t n_tok = (size_t)B * (size_t)(max_steps > 0 ? max_steps : 1);
     const size_t out_bytes = sizeof(int) * (n_tok + 3 * (size_t)B) + (size_t)B + 64;
-    if (s->out_bytes < out_bytes) {
-        CU(cudaStreamSynchronize(stream));
-        cudaFree(s->out_i32); s->out_i32 = nullptr; s->out_bytes = 0;
-        CU(cudaMalloc(&s->out_i32, out_bytes));
-        s->out_bytes = out_bytes;
-    }
-    if (!s->copy_stream) {
-        CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
-        for (int i = 0; i < 2; ++i) {
-            CU(cudaEventCreateWithFlags(&s->ev_copied[i], cudaEventDisableTiming));
-            CU(cudaEventCreateWithFlags(&s->ev_consumed[i], cudaEventDisableTiming));
-        }
-        CU(cudaMallocHost(&s->h_pinned, sizeof(int) * 4));
-    }
+    st = get_host_loop_scratch(s, step_bytes, 0, out_bytes, stream);
+    if (st != CD_OK) return st;
     int* d_tokens = s->out_i32;
     int* d_len = d_tokens + n_tok;
     int* d_fs = d_len + B;
     float* d_slp = reinterpret_cast<float*>(d_fs + B);
     uint8_t* d_done = reinterpret_cast<uint8_t*>(d_slp + B);
 
-    const LimitArgs lim = resolve_limit(d);
+    const LimitArgs lim = resolve_limit(cfg);
     st = launch_loop_init(d, s, B, max_steps, d_tokens, d_len, d_fs, d_slp, d_done, stream, lim);
     if (st != CD_OK) return st;
     if (!d->start_accepting && max_steps > 0) {
         // Pinned, device-mapped host buffers (what cudaHostAlloc / torch pin_memory give under unified
         // addressing): the SMs pull the active rows over PCIe themselves, nothing is read back per step.
-        bool mapped = true;
+        bool mapped = tune_int("CD_HOST_ZEROCOPY", 1, 0, 1) != 0;
         std::vector<const unsigned char*> dev_view((size_t)max_steps, nullptr);
-        {
-            static const bool allow = [] { const char* e = std::getenv("CD_HOST_ZEROCOPY"); return e ? std::atoi(e) != 0 : true; }();
-            mapped = allow && ((ld_elems * sz) % 16 == 0);
-            for (int k = 0; k < max_steps && mapped; ++k) {
-                cudaPointerAttributes at;
-                if (cudaPointerGetAttributes(&at, step_logits_host[k]) != cudaSuccess) {
-                    cudaGetLastError();
-                    mapped = false;
-                } else if (at.type != cudaMemoryTypeHost || !at.devicePointer ||
-                           (reinterpret_cast<uintptr_t>(at.devicePointer) & 15) != 0) {
-                    mapped = false;
-                } else {
-                    dev_view[(size_t)k] = static_cast<const unsigned char*>(at.devicePointer);
-                }
+        for (int k = 0; k < max_steps && mapped; ++k) {
+            cudaPointerAttributes at;
+            if (cudaPointerGetAttributes(&at, step_logits_host[k]) != cudaSuccess) {
+                cudaGetLastError();
+                mapped = false;
+            } else if (at.type != cudaMemoryTypeHost || !at.devicePointer ||
+                       (reinterpret_cast<uintptr_t>(at.devicePointer) & 15) != 0) {
+                mapped = false;
+            } else {
+                dev_view[(size_t)k] = static_cast<const unsigned char*>(at.devicePointer);
             }
         }
         if (mapped) {
             const unsigned long long row_bytes = (unsigned long long)ld_elems * (unsigned long long)sz;
             for (int k = 0; k < max_steps; ++k) {
                 const int cur = k & 1;
-                cd::host_gather_rows_kernel<<<d->num_sms * host_gather_mult(), 256, 0, stream>>>(dev_view[(size_t)k], row_bytes, s->row_ids[cur],
-                                                                                 s->n_active + cur,
-                                                                                 static_cast<unsigned char*>(s->stage[0]));
+                cd::host_gather_rows_kernel<<<d->num_sms * host_gather_mult(), 256, 0, stream>>>(
+                    dev_view[(size_t)k], row_bytes, s->b.row_ids[cur], s->b.n_active + cur,
+                    static_cast<unsigned char*>(s->stage[0]));
                 CU(cudaGetLastError());
                 g_launches.fetch_add(1, std::memory_order_relaxed);
-                st = enqueue_loop_step(d, s, s->stage[0], dtype, ld_elems, B, k, max_steps, d_tokens, d_len, d_fs, d_slp,
-                                       d_done, stream, lim, 1);
+                st = enqueue_loop_step(d, cfg, s, s->stage[0], dtype, ld_elems, B, k, max_steps, d_tokens, d_len, d_fs,
+                                       d_slp, d_done, stream, lim, 1);
                 if (st != CD_OK) return st;
             }
         } else {
-        // Early exit reaches the PCIe link too: only the rows still active are copied.  After step
-        // k - 1 the host reads the compacted active list (n and the original row ids), copies those
-        // rows of step k's logits into a compact staging buffer (runs of consecutive ids as one copy)
-        // and launches the step with logits row = slot.  Kernel time is ~1 % of the copy time, so
-        // nothing is lost by not overlapping the two.
-        if (s->h_ids_cap < B) {
-            if (s->h_ids) cudaFreeHost(s->h_ids);
-            s->h_ids = nullptr;
-            s->h_ids_cap = 0;
-            CU(cudaMallocHost(&s->h_ids, sizeof(int) * (size_t)B));
-            s->h_ids_cap = B;
-        }
-        const size_t row_bytes = (size_t)ld_elems * (size_t)sz;
-        int n_h = B;
-        for (int i = 0; i < B; ++i) s->h_ids[i] = i;
-        for (int k = 0; k < max_steps; ++k) {
-            const int cur = k & 1, nxt = cur ^ 1;
-            if (k > 0 || lim.sat_ctr) {  // (with a LIMIT the list may be empty from the start)
-                CU(cudaMemcpyAsync(s->h_pinned, s->n_active + cur, sizeof(int), cudaMemcpyDeviceToHost, stream));
-                CU(cudaMemcpyAsync(s->h_ids, s->row_ids[cur], sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, stream));
-                CU(cudaStreamSynchronize(stream));
-                n_h = s->h_pinned[0];
+            // Early exit reaches the PCIe link too: only the rows still active are copied.  After step
+            // k - 1 the host reads the compacted active list (n and the original row ids), copies those
+            // rows of step k's logits into the compact staging buffer (runs of consecutive ids as one copy)
+            // and launches the step with logits row = slot.  Kernel time is ~1 % of the copy time, so
+            // nothing is lost by not overlapping the two.
+            if (s->h_ids_cap < B) {
+                if (s->h_ids) cudaFreeHost(s->h_ids);
+                s->h_ids = nullptr;
+                s->h_ids_cap = 0;
+                CU(cudaMallocHost(&s->h_ids, sizeof(int) * (size_t)B));
+                s->h_ids_cap = B;
             }
-            if (n_h <= 0) break;
-            const unsigned char* src = static_cast<const unsigned char*>(step_logits_host[k]);
-            unsigned char* dst = static_cast<unsigned char*>(s->stage[0]);
-            for (int i = 0; i < n_h;) {
-                int e = i + 1;
-                while (e < n_h && s->h_ids[e] == s->h_ids[e - 1] + 1) ++e;
-                CU(cudaMemcpyAsync(dst + (size_t)i * row_bytes, src + (size_t)s->h_ids[i] * row_bytes,
-                                   (size_t)(e - i) * row_bytes, cudaMemcpyHostToDevice, stream));
-                i = e;
+            const size_t row_bytes = (size_t)ld_elems * (size_t)sz;
+            int n_h = B;
+            for (int i = 0; i < B; ++i) s->h_ids[i] = i;
+            for (int k = 0; k < max_steps; ++k) {
+                const int cur = k & 1;
+                if (k > 0 || lim.sat_ctr) {  // (with a LIMIT the list may be empty from the start)
+                    CU(cudaMemcpyAsync(s->h_pinned, s->b.n_active + cur, sizeof(int), cudaMemcpyDeviceToHost, stream));
+                    CU(cudaMemcpyAsync(s->h_ids, s->b.row_ids[cur], sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, stream));
+                    CU(cudaStreamSynchronize(stream));
+                    n_h = s->h_pinned[0];
+                }
+                if (n_h <= 0) break;
+                const unsigned char* src = static_cast<const unsigned char*>(step_logits_host[k]);
+                unsigned char* dst = static_cast<unsigned char*>(s->stage[0]);
+                for (int i = 0; i < n_h;) {
+                    int e = i + 1;
+                    while (e < n_h && s->h_ids[e] == s->h_ids[e - 1] + 1) ++e;
+                    CU(cudaMemcpyAsync(dst + (size_t)i * row_bytes, src + (size_t)s->h_ids[i] * row_bytes,
+                                       (size_t)(e - i) * row_bytes, cudaMemcpyHostToDevice, stream));
+                    i = e;
+                }
+                st = enqueue_loop_step(d, cfg, s, s->stage[0], dtype, ld_elems, B, k, max_steps, d_tokens, d_len, d_fs,
+                                       d_slp, d_done, stream, lim, 1);
+                if (st != CD_OK) return st;
             }
-            st = enqueue_loop_step(d, s, s->stage[0], dtype, ld_elems, B, k, max_steps, d_tokens, d_len, d_fs, d_slp,
-                                   d_done, stream, lim, 1);
-            if (st != CD_OK) return st;
-            (void)nxt;
         }
-        }
-        CU(cudaStreamSynchronize(s->copy_stream));
     }
     if (max_steps > 0)
         CU(cudaMemcpyAsync(tokens_out, d_tokens, sizeof(int) * (size_t)B * max_steps, cudaMemcpyDeviceToHost, stream));
@@ -940,7 +1331,7 @@ cd_status cd_decode_loop_host(const cd_dfa_t* d, const void* const* step_logits_
     CU(cudaMemcpyAsync(final_state_out, d_fs, sizeof(int) * (size_t)B, cudaMemcpyDeviceToHost, stream));
     CU(cudaMemcpyAsync(sum_logprob_out, d_slp, sizeof(float) * (size_t)B, cudaMemcpyDeviceToHost, stream));
     CU(cudaMemcpyAsync(done_out, d_done, (size_t)B, cudaMemcpyDeviceToHost, stream));
-    return check_sticky_errors(s, stream);
+    return finish_loop(s, stream, false);
 }
 
 }  // extern "C"
@@ -984,22 +1375,28 @@ cd_status make_tmap_bf16(CUtensorMap* out, const void* base, long long rows, lon
 cd_status get_head_scratch(Scratch* s, int rows, int H, cudaStream_t stream) {
     if (s->head_rows >= rows && s->head_H == H) return CD_OK;  // the A tensor map is built for exactly H columns
     if (s->head_rows > 0) CU(cudaStreamSynchronize(stream));
-    cudaFree(s->h_flags); cudaFree(s->h_lists); cudaFree(s->h_ctr); cudaFree(s->h_A); cudaFree(s->h_partials);
-    s->h_flags = nullptr; s->h_lists = nullptr; s->h_ctr = nullptr; s->h_A = nullptr; s->h_partials = nullptr;
-    s->head_rows = 0;
-    if (rows < s->cap_rows) rows = s->cap_rows;
+    s->release_head();
+    if (rows < s->b.cap_rows) rows = s->b.cap_rows;
     const long long rows_pad = ((long long)rows + cd::HD_BM - 1) / cd::HD_BM * cd::HD_BM;
     const long long ldA = ((long long)H + 7) / 8 * 8;
-    CU(cudaMalloc(&s->h_flags, (size_t)rows * 2));
-    CU(cudaMalloc(&s->h_lists, sizeof(int) * (size_t)rows * 4));
-    CU(cudaMalloc(&s->h_ctr, sizeof(int) * 4));
-    CU(cudaMemset(s->h_ctr, 0, sizeof(int) * 4));
-    CU(cudaMalloc(&s->h_A, (size_t)rows_pad * (size_t)ldA * 2));
-    CU(cudaMemset(s->h_A, 0, (size_t)rows_pad * (size_t)ldA * 2));
-    CU(cudaMalloc(&s->h_partials, sizeof(cd::HeadPartial) * (size_t)cd::head_partials_cap(rows)));
+    cudaError_t e = cudaSuccess;
+    auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
+    A(cudaMalloc(&s->h_flags, (size_t)rows * 2));
+    A(cudaMalloc(&s->h_lists, sizeof(int) * (size_t)rows * 4));
+    A(cudaMalloc(&s->h_ctr, sizeof(int) * 4));
+    A(cudaMalloc(&s->h_A, (size_t)rows_pad * (size_t)ldA * 2));
+    A(cudaMalloc(&s->h_partials, sizeof(cd::HeadPartial) * (size_t)cd::head_partials_cap(rows)));
+    if (e == cudaSuccess) e = cudaMemset(s->h_ctr, 0, sizeof(int) * 4);
+    if (e == cudaSuccess) e = cudaMemset(s->h_A, 0, (size_t)rows_pad * (size_t)ldA * 2);
+    cd_status st = CD_OK;
+    if (e != cudaSuccess)
+        st = fail(e == cudaErrorMemoryAllocation ? CD_ERR_OOM : CD_ERR_CUDA, "LM-head scratch: %s", cudaGetErrorString(e));
     s->h_ldA = ldA;
-    cd_status st = make_tmap_bf16(&s->h_tmA, s->h_A, rows_pad, H, ldA, cd::HD_BM);
-    if (st != CD_OK) return st;
+    if (st == CD_OK) st = make_tmap_bf16(&s->h_tmA, s->h_A, rows_pad, H, ldA, cd::HD_BM);
+    if (st != CD_OK) {
+        s->release_head();  // nothing half-built is kept
+        return st;
+    }
     s->head_rows = rows;
     s->head_H = H;
     return CD_OK;
@@ -1009,8 +1406,8 @@ cd_status get_head_scratch(Scratch* s, int rows, int H, cudaStream_t stream) {
 // step.  A gathered logit reads one W row (2H bytes, mostly from L2) and costs 2H flops on the
 // CUDA cores; a dense row costs 2VH flops on the tensor cores.  Automatic policy: gather while
 // deg * 2H bytes at ~4 TB/s is below V * 2H flops at ~1.2 PFLOP/s, i.e. deg < V / 300.
-int head_gather_max_for(const cd_dfa* d) {
-    if (d->head_gather_max >= 0) return d->head_gather_max;
+int head_gather_max_for(const cd_dfa* d, const Settings& cfg) {
+    if (cfg.head_gather_max >= 0) return cfg.head_gather_max;
     return d->dev.V / 300 > 1 ? d->dev.V / 300 : 1;
 }
 
@@ -1041,7 +1438,7 @@ cd_status head_weight_map(const cd_dfa* d, const void* W, long long ldw, int H, 
 // The kernels of one LM-head step for up to n_upper active slots (n_dev overrides the count on
 // the device).  With loop extras the rows' history is recorded as they finalise and a last
 // one-CTA kernel compacts the active list.
-cd_status launch_head(const cd_dfa* d, Scratch* s, const void* hidden, long long ldh, const void* W, long long ldw, int H,
+cd_status launch_head(const cd_dfa* d, const Settings& cfg, Scratch* s, const void* hidden, long long ldh, const void* W, long long ldw, int H,
                       const int* row_map, int* state, int n_upper, const int* n_dev, int* token_out, float* logprob_out,
                       float* lse_out, uint8_t* done_out, cudaStream_t stream, const LoopExtras* x) {
     cd::HeadArgs a{};
@@ -1071,18 +1468,18 @@ cd_status launch_head(const cd_dfa* d, Scratch* s, const void* hidden, long long
     a.fin.logprob_out = logprob_out;
     a.fin.lse_out = lse_out;
     a.fin.done_out = done_out;
-    a.fin.ctrs = s->ctrs;
-    a.fin.inv_tau = d->inv_tau;
-    a.fin.seed_lo = (uint32_t)(d->seed & 0xFFFFFFFFull);
-    a.fin.seed_hi = (uint32_t)(d->seed >> 32);
-    a.fin.rng_step_base = d->rng_step_base;
-    const bool sample = d->inv_tau > 0.0f;
+    a.fin.ctrs = s->b.ctrs;
+    a.fin.inv_tau = cfg.inv_tau;
+    a.fin.seed_lo = (uint32_t)(cfg.seed & 0xFFFFFFFFull);
+    a.fin.seed_hi = (uint32_t)(cfg.seed >> 32);
+    a.fin.rng_step_base = cfg.rng_step_base;
+    const bool sample = cfg.inv_tau > 0.0f;
     a.hidden = static_cast<const uint16_t*>(hidden);
     a.ldh = ldh;
     a.W = static_cast<const uint16_t*>(W);
     a.ldw = ldw;
     a.H = H;
-    a.gather_max = head_gather_max_for(d);
+    a.gather_max = head_gather_max_for(d, cfg);
     a.not_dense = s->h_flags;
     a.not_gather = s->h_flags + s->head_rows;
     a.dense_slot = s->h_lists;
@@ -1156,15 +1553,16 @@ extern "C" {
 
 cd_status cd_set_limit(cd_dfa_t* d, int32_t limit, int32_t* satisfied_inout) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    std::lock_guard<std::mutex> lk(d->mu);
     if (!satisfied_inout) {  // clear
-        d->limit_ctr = nullptr;
-        d->limit = 0;
+        d->cfg.limit_ctr = nullptr;
+        d->cfg.limit = 0;
         return CD_OK;
     }
     if (limit < 0) return fail(CD_ERR_ARG, "limit < 0");
-    if (!d->d_satisfying) return fail(CD_ERR_ARG, "cd_set_satisfying has not been called on this automaton");
-    d->limit_ctr = satisfied_inout;
-    d->limit = limit;
+    if (!d->cfg.has_satisfying) return fail(CD_ERR_ARG, "cd_set_satisfying has not been called on this automaton");
+    d->cfg.limit_ctr = satisfied_inout;
+    d->cfg.limit = limit;
     return CD_OK;
 }
 
@@ -1172,16 +1570,18 @@ cd_status cd_set_sampling(cd_dfa_t* d, float temperature, uint64_t seed, int32_t
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
     if (!(temperature >= 0.0f) || temperature > 3.0e38f) return fail(CD_ERR_ARG, "temperature must be finite and >= 0");
     if (step_base < 0) return fail(CD_ERR_ARG, "step_base < 0");
-    d->inv_tau = temperature > 0.0f ? 1.0f / temperature : 0.0f;  // IEEE fp32 division, as the oracle's
-    d->seed = seed;
-    d->rng_step_base = step_base;
+    std::lock_guard<std::mutex> lk(d->mu);
+    d->cfg.inv_tau = temperature > 0.0f ? 1.0f / temperature : 0.0f;  // IEEE fp32 division, as the oracle's
+    d->cfg.seed = seed;
+    d->cfg.rng_step_base = step_base;
     return CD_OK;
 }
 
 cd_status cd_set_head_gather_max(cd_dfa_t* d, int32_t max_transitions) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
     if (max_transitions < -1) return fail(CD_ERR_ARG, "max_transitions must be >= -1");
-    d->head_gather_max = max_transitions;
+    std::lock_guard<std::mutex> lk(d->mu);
+    d->cfg.head_gather_max = max_transitions;
     return CD_OK;
 }
 
@@ -1196,12 +1596,13 @@ cd_status cd_head_step(const cd_dfa_t* d, const void* hidden, int64_t ldh_elems,
     if (!state || !token_out || !logprob_out || !done_out) return fail(CD_ERR_ARG, "NULL pointer");
     DeviceGuard guard(d->device);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const Settings cfg = settings_of(d);
     Scratch* s = nullptr;
-    st = get_scratch(d, stream, n, false, &s);
+    st = get_scratch(d, stream, n, &s);
     if (st != CD_OK) return st;
     st = get_head_scratch(s, n, H, stream);
     if (st != CD_OK) return st;
-    return launch_head(d, s, hidden, ldh_elems, W, ldw_elems, H, row_map, state, n, nullptr, token_out, logprob_out,
+    return launch_head(d, cfg, s, hidden, ldh_elems, W, ldw_elems, H, row_map, state, n, nullptr, token_out, logprob_out,
                        lse_out, done_out, stream, nullptr);
 }
 
@@ -1224,10 +1625,12 @@ static cd_status head_loop_impl(const cd_dfa_t* d, const void* const* step_hidde
         if (st != CD_OK) return st;
         if (!step_hidden[k]) return fail(CD_ERR_ARG, "step_hidden[%d] is NULL", k);
     }
+    RangeGuard range("cd_head_decode_loop");
     DeviceGuard guard(d->device);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const Settings cfg = settings_of(d);
     Scratch* s = nullptr;
-    st = get_scratch(d, stream, B, true, &s);
+    st = get_scratch(d, stream, B, &s);
     if (st != CD_OK) return st;
     int* d_tokens = tokens_out;
     int* d_len = len_out;
@@ -1237,35 +1640,17 @@ static cd_status head_loop_impl(const cd_dfa_t* d, const void* const* step_hidde
     const size_t step_bytes = (size_t)B * (size_t)ldh_elems * 2;
     const size_t n_tok = (size_t)B * (size_t)(max_steps > 0 ? max_steps : 1);
     if (host) {
-        if (s->stage_bytes < step_bytes) {
-            CU(cudaStreamSynchronize(stream));
-            for (int i = 0; i < 2; ++i) { cudaFree(s->stage[i]); s->stage[i] = nullptr; }
-            s->stage_bytes = 0;
-            for (int i = 0; i < 2; ++i) CU(cudaMalloc(&s->stage[i], step_bytes));
-            s->stage_bytes = step_bytes;
-        }
+        // two staging buffers: the H2D copy of step k + 1 overlaps the kernels of step k
         const size_t out_bytes = sizeof(int) * (n_tok + 3 * (size_t)B) + (size_t)B + 64;
-        if (s->out_bytes < out_bytes) {
-            CU(cudaStreamSynchronize(stream));
-            cudaFree(s->out_i32); s->out_i32 = nullptr; s->out_bytes = 0;
-            CU(cudaMalloc(&s->out_i32, out_bytes));
-            s->out_bytes = out_bytes;
-        }
-        if (!s->copy_stream) {
-            CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
-            for (int i = 0; i < 2; ++i) {
-                CU(cudaEventCreateWithFlags(&s->ev_copied[i], cudaEventDisableTiming));
-                CU(cudaEventCreateWithFlags(&s->ev_consumed[i], cudaEventDisableTiming));
-            }
-            CU(cudaMallocHost(&s->h_pinned, sizeof(int) * 4));
-        }
+        st = get_host_loop_scratch(s, step_bytes, step_bytes, out_bytes, stream);
+        if (st != CD_OK) return st;
         d_tokens = s->out_i32;
         d_len = d_tokens + n_tok;
         d_fs = d_len + B;
         d_slp = reinterpret_cast<float*>(d_fs + B);
         d_done = reinterpret_cast<uint8_t*>(d_slp + B);
     }
-    const LimitArgs lim = resolve_limit(d);
+    const LimitArgs lim = resolve_limit(cfg);
     st = launch_loop_init(d, s, B, max_steps, d_tokens, d_len, d_fs, d_slp, d_done, stream, lim);
     if (st != CD_OK) return st;
     if (!d->start_accepting && max_steps > 0) {
@@ -1299,16 +1684,17 @@ static cd_status head_loop_impl(const cd_dfa_t* d, const void* const* step_hidde
             x.done = d_done;
             x.step = k;
             x.max_steps = max_steps;
-            x.row_ids_out = s->row_ids[nxt];
-            x.state_out = s->state[nxt];
-            x.n_out = s->n_active + nxt;
+            x.row_ids_out = s->b.row_ids[nxt];
+            x.state_out = s->b.state[nxt];
+            x.n_out = s->b.n_active + nxt;
             if (lim.sat_ctr) {
                 x.satisfying = static_cast<const uint8_t*>(d->d_satisfying);
                 x.sat_ctr = lim.sat_ctr;
                 x.limit = lim.limit;
             }
-            st = launch_head(d, s, hid, ldh_elems, W, ldw_elems, H, s->row_ids[cur], s->state[cur], B,
-                             s->n_active + cur, s->token, s->logprob, nullptr, s->done, stream, &x);
+            RangeGuard step_range("cd decoding step (LM head)");
+            st = launch_head(d, cfg, s, hid, ldh_elems, W, ldw_elems, H, s->b.row_ids[cur], s->b.state[cur], B,
+                             s->b.n_active + cur, s->b.token, s->b.logprob, nullptr, s->b.done, stream, &x);
             if (st != CD_OK) return st;
             if (host) CU(cudaEventRecord(s->ev_consumed[cur], stream));
         }
@@ -1322,7 +1708,7 @@ static cd_status head_loop_impl(const cd_dfa_t* d, const void* const* step_hidde
         CU(cudaMemcpyAsync(sum_logprob_out, d_slp, sizeof(float) * (size_t)B, cudaMemcpyDeviceToHost, stream));
         CU(cudaMemcpyAsync(done_out, d_done, (size_t)B, cudaMemcpyDeviceToHost, stream));
     }
-    return check_sticky_errors(s, stream);
+    return finish_loop(s, stream, false);
 }
 
 cd_status cd_head_decode_loop(const cd_dfa_t* d, const void* const* step_hidden, int64_t ldh_elems, const void* W,
@@ -1351,30 +1737,6 @@ int grid_for(long long n, int threads) {
     if (b < 1) b = 1;
     if (b > 148 * 16) b = 148 * 16;
     return (int)b;
-}
-
-// Stream-ordered scratch (cudaMallocAsync) must not be handed back to the OS at every synchronisation:
-// keep the default pool's memory (once per device).
-void keep_pool_memory(int dev) {
-    static std::mutex mu;
-    static std::map<int, bool> done;
-    std::lock_guard<std::mutex> lk(mu);
-    if (done[dev]) return;
-    cudaMemPool_t pool = nullptr;
-    if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess && pool) {
-        unsigned long long thr = ~0ull;
-        cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
-    }
-    done[dev] = true;
-}
-
-cd_status device_of(const void* p, int* dev) {
-    cudaPointerAttributes at;
-    CU(cudaPointerGetAttributes(&at, p));
-    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
-        return fail(CD_ERR_ARG, "expected a DEVICE pointer");
-    *dev = at.device;
-    return CD_OK;
 }
 
 }  // namespace
@@ -1446,17 +1808,26 @@ cd_status cd_dedup(const int64_t* keys, int32_t N, int32_t* rep_out, int32_t* di
     int* rank = reinterpret_cast<int*>(buf + off_rank);
     uint8_t* flag = buf + off_flag;
     // min rows start at 0x7F7F7F7F (>= any row id); free slots hold DEDUP_EMPTY
-    CU(cudaMemsetAsync(tmin, 0x7F, sizeof(int) * ((size_t)cap + 1), stream));
-    cd::dedup_clear_kernel<<<grid_for((long long)cap + 1, 256), 256, 0, stream>>>(tkey, (long long)cap + 1);
-    cd::dedup_insert_kernel<<<grid_for(N, 256), 256, 0, stream>>>(reinterpret_cast<const long long*>(keys), N, tkey, tmin, cap);
-    cd::dedup_first_kernel<<<grid_for(N, 256), 256, 0, stream>>>(reinterpret_cast<const long long*>(keys), N, tkey, tmin, cap,
-                                                               first, flag);
-    cd::dedup_rank_kernel<<<1, 1024, 0, stream>>>(flag, N, distinct_rows_out, rank, n_distinct_out);
-    cd::dedup_rep_kernel<<<grid_for(N, 256), 256, 0, stream>>>(first, rank, N, rep_out);
-    CU(cudaGetLastError());
-    g_launches.fetch_add(5, std::memory_order_relaxed);
-    CU(cudaFreeAsync(buf, stream));
-    return CD_OK;
+    cudaError_t e = cudaMemsetAsync(tmin, 0x7F, sizeof(int) * ((size_t)cap + 1), stream);
+    if (e == cudaSuccess) {
+        cd::dedup_clear_kernel<<<grid_for((long long)cap + 1, 256), 256, 0, stream>>>(tkey, (long long)cap + 1);
+        cd::dedup_insert_kernel<<<grid_for(N, 256), 256, 0, stream>>>(reinterpret_cast<const long long*>(keys), N, tkey, tmin, cap);
+        cd::dedup_first_kernel<<<grid_for(N, 256), 256, 0, stream>>>(reinterpret_cast<const long long*>(keys), N, tkey, tmin,
+                                                                   cap, first, flag);
+        e = cudaGetLastError();
+    }
+    // stable ranking of the first occurrences: the compaction of a6 over the "not first" flags (ids = row numbers),
+    // with the output position of every kept row recorded
+    st = (e == cudaSuccess) ? launch_compact(flag, nullptr, nullptr, N, distinct_rows_out, nullptr, n_distinct_out, rank, stream)
+                            : fail(CD_ERR_CUDA, "dedup launch: %s", cudaGetErrorString(e));
+    if (st == CD_OK) {
+        cd::dedup_rep_kernel<<<grid_for(N, 256), 256, 0, stream>>>(first, rank, N, rep_out);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) st = fail(CD_ERR_CUDA, "dedup launch: %s", cudaGetErrorString(e));
+    }
+    cudaFreeAsync(buf, stream);  // on every path
+    if (st == CD_OK) g_launches.fetch_add(4, std::memory_order_relaxed);
+    return st;
 }
 
 cd_status cd_join_results(const int32_t* rep, int32_t N, int32_t max_steps, const int32_t* tokens_d, const int32_t* len_d,
@@ -1485,7 +1856,7 @@ cd_status cd_join_results(const int32_t* rep, int32_t N, int32_t max_steps, cons
 cd_status cd_filter_rows(const cd_dfa_t* d, const int32_t* final_state, const uint8_t* done, const int32_t* row_ids_in,
                          int32_t N, int32_t* row_ids_out, int32_t* n_out, void* cuda_stream) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
-    if (!d->d_satisfying) return fail(CD_ERR_ARG, "cd_set_satisfying has not been called on this automaton");
+    if (!settings_of(d).has_satisfying) return fail(CD_ERR_ARG, "cd_set_satisfying has not been called on this automaton");
     if (N < 0) return fail(CD_ERR_ARG, "N < 0");
     if (!n_out) return fail(CD_ERR_ARG, "n_out is NULL");
     DeviceGuard guard(d->device);
@@ -1500,11 +1871,12 @@ cd_status cd_filter_rows(const cd_dfa_t* d, const int32_t* final_state, const ui
     CU(cudaMallocAsync(reinterpret_cast<void**>(&drop), (size_t)N + 16, stream));
     cd::filter_flag_kernel<<<grid_for(N, 256), 256, 0, stream>>>(final_state, done, N,
                                                                static_cast<const uint8_t*>(d->d_satisfying), d->dev.S, drop);
-    cd::compact_kernel<<<1, 1024, 0, stream>>>(drop, row_ids_in, nullptr, N, row_ids_out, nullptr, n_out);
-    CU(cudaGetLastError());
-    g_launches.fetch_add(2, std::memory_order_relaxed);
-    CU(cudaFreeAsync(drop, stream));
-    return CD_OK;
+    const cudaError_t e = cudaGetLastError();
+    const cd_status st = (e == cudaSuccess) ? launch_compact(drop, row_ids_in, nullptr, N, row_ids_out, nullptr, n_out, nullptr, stream)
+                                            : fail(CD_ERR_CUDA, "filter launch: %s", cudaGetErrorString(e));
+    cudaFreeAsync(drop, stream);  // on every path
+    if (st == CD_OK) g_launches.fetch_add(1, std::memory_order_relaxed);
+    return st;
 }
 
 }  // extern "C"
@@ -1525,10 +1897,12 @@ cd_status cd_decode_loop_cb(const cd_dfa_t* d, cd_next_logits_fn next_logits, vo
         return fail(CD_ERR_ARG, "NULL output pointer");
     DeviceGuard guard(d->device);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    RangeGuard range("cd_decode_loop_cb");
+    const Settings cfg = settings_of(d);
     Scratch* s = nullptr;
-    st = get_scratch(d, stream, B, true, &s);
+    st = get_scratch(d, stream, B, &s);
     if (st != CD_OK) return st;
-    const LimitArgs lim = resolve_limit(d);
+    const LimitArgs lim = resolve_limit(cfg);
     st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream,
                           lim);
     if (st != CD_OK) return st;
@@ -1538,15 +1912,15 @@ cd_status cd_decode_loop_cb(const cd_dfa_t* d, cd_next_logits_fn next_logits, vo
             const void* logits = nullptr;
             int64_t ld = 0;
             int32_t by_slot = 0;
-            const int rc = next_logits(user, k, s->row_ids[cur], s->n_active + cur, B, &logits, &ld, &by_slot);
+            const int rc = next_logits(user, k, s->b.row_ids[cur], s->b.n_active + cur, B, &logits, &ld, &by_slot);
             if (rc != 0) return fail(CD_ERR_ARG, "next_logits returned %d at step %d", rc, k);
             st = check_logits_layout(d, logits, dtype, ld);
             if (st != CD_OK) return st;
-            st = enqueue_loop_step(d, s, logits, dtype, ld, B, k, max_steps, tokens_out, len_out, final_state_out,
+            st = enqueue_loop_step(d, cfg, s, logits, dtype, ld, B, k, max_steps, tokens_out, len_out, final_state_out,
                                    sum_logprob_out, done_out, stream, lim, by_slot ? 1 : 0);
             if (st != CD_OK) return st;
         }
-    return check_sticky_errors(s, stream);
+    return finish_loop(s, stream, false);
 }
 
 cd_status cd_head_decode_loop_cb(const cd_dfa_t* d, cd_next_hidden_fn next_hidden, void* user, const void* W,
@@ -1561,10 +1935,12 @@ cd_status cd_head_decode_loop_cb(const cd_dfa_t* d, cd_next_hidden_fn next_hidde
         return fail(CD_ERR_ARG, "NULL output pointer");
     DeviceGuard guard(d->device);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    RangeGuard range("cd_head_decode_loop_cb");
+    const Settings cfg = settings_of(d);
     Scratch* s = nullptr;
-    cd_status st = get_scratch(d, stream, B, true, &s);
+    cd_status st = get_scratch(d, stream, B, &s);
     if (st != CD_OK) return st;
-    const LimitArgs lim = resolve_limit(d);
+    const LimitArgs lim = resolve_limit(cfg);
     st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out, stream,
                           lim);
     if (st != CD_OK) return st;
@@ -1576,7 +1952,7 @@ cd_status cd_head_decode_loop_cb(const cd_dfa_t* d, cd_next_hidden_fn next_hidde
             const void* hidden = nullptr;
             int64_t ldh = 0;
             int32_t by_slot = 0;
-            const int rc = next_hidden(user, k, s->row_ids[cur], s->n_active + cur, B, &hidden, &ldh, &by_slot);
+            const int rc = next_hidden(user, k, s->b.row_ids[cur], s->b.n_active + cur, B, &hidden, &ldh, &by_slot);
             if (rc != 0) return fail(CD_ERR_ARG, "next_hidden returned %d at step %d", rc, k);
             st = check_head_layout(hidden, ldh, W, ldw_elems, H);
             if (st != CD_OK) return st;
@@ -1588,21 +1964,22 @@ cd_status cd_head_decode_loop_cb(const cd_dfa_t* d, cd_next_hidden_fn next_hidde
             x.done = done_out;
             x.step = k;
             x.max_steps = max_steps;
-            x.row_ids_out = s->row_ids[nxt];
-            x.state_out = s->state[nxt];
-            x.n_out = s->n_active + nxt;
+            x.row_ids_out = s->b.row_ids[nxt];
+            x.state_out = s->b.state[nxt];
+            x.n_out = s->b.n_active + nxt;
             x.logits_by_slot = by_slot ? 1 : 0;
             if (lim.sat_ctr) {
                 x.satisfying = static_cast<const uint8_t*>(d->d_satisfying);
                 x.sat_ctr = lim.sat_ctr;
                 x.limit = lim.limit;
             }
-            st = launch_head(d, s, hidden, ldh, W, ldw_elems, H, s->row_ids[cur], s->state[cur], B, s->n_active + cur,
-                             s->token, s->logprob, nullptr, s->done, stream, &x);
+            RangeGuard step_range("cd decoding step (LM head)");
+            st = launch_head(d, cfg, s, hidden, ldh, W, ldw_elems, H, s->b.row_ids[cur], s->b.state[cur], B,
+                             s->b.n_active + cur, s->b.token, s->b.logprob, nullptr, s->b.done, stream, &x);
             if (st != CD_OK) return st;
         }
     }
-    return check_sticky_errors(s, stream);
+    return finish_loop(s, stream, false);
 }
 
 }  // extern "C"
@@ -1612,23 +1989,17 @@ extern "C" {
 
 cd_status cd_build_list(int32_t V, int32_t K, const int64_t* label_ptr, const int32_t* label_tok, const int32_t* open,
                         int32_t n_open, const int32_t* sep, int32_t n_sep, const int32_t* close, int32_t n_close,
-                        int32_t min_items, int32_t max_items, int32_t* S_out, int64_t* nnz_out, int64_t* row_ptr_out,
-                        int32_t* tok_out, int32_t* next_out, uint8_t* accepting_out) {
+                        int32_t min_items, int32_t max_items, int32_t eos, int32_t* S_out, int64_t* nnz_out,
+                        int64_t* row_ptr_out, int32_t* tok_out, int32_t* next_out, uint8_t* accepting_out) {
     try {
         if (!label_ptr || !S_out || !nnz_out) return fail(CD_ERR_ARG, "NULL argument");
         if (K >= 1 && label_ptr[K] > 0 && !label_tok) return fail(CD_ERR_ARG, "label_tok is NULL");
         if ((n_open > 0 && !open) || (n_sep > 0 && !sep) || (n_close > 0 && !close)) return fail(CD_ERR_ARG, "NULL token list");
         cdt::HostCsr c;
         const std::string err = cdt::build_list(V, K, label_ptr, label_tok, open, n_open, sep, n_sep, close, n_close,
-                                                min_items, max_items, &c);
+                                                min_items, max_items, eos, &c);
         if (!err.empty()) return fail(CD_ERR_AUTOMATON, "%s", err.c_str());
-        *S_out = c.S;
-        *nnz_out = (int64_t)c.tok.size();
-        if (row_ptr_out) std::memcpy(row_ptr_out, c.row_ptr.data(), sizeof(int64_t) * c.row_ptr.size());
-        if (tok_out && !c.tok.empty()) std::memcpy(tok_out, c.tok.data(), sizeof(int32_t) * c.tok.size());
-        if (next_out && !c.next.empty()) std::memcpy(next_out, c.next.data(), sizeof(int32_t) * c.next.size());
-        if (accepting_out) std::memcpy(accepting_out, c.accepting.data(), c.accepting.size());
-        return CD_OK;
+        return copy_csr_out(c, S_out, nnz_out, row_ptr_out, tok_out, next_out, accepting_out);
     } catch (const std::bad_alloc&) {
         return fail(CD_ERR_OOM, "host allocation failed");
     } catch (...) {
@@ -1638,15 +2009,15 @@ cd_status cd_build_list(int32_t V, int32_t K, const int64_t* label_ptr, const in
 
 cd_status cd_compile_list(int32_t V, int32_t K, const int64_t* label_ptr, const int32_t* label_tok, const int32_t* open,
                           int32_t n_open, const int32_t* sep, int32_t n_sep, const int32_t* close, int32_t n_close,
-                          int32_t min_items, int32_t max_items, int device, cd_dfa_t** out) {
+                          int32_t min_items, int32_t max_items, int32_t eos, int device, cd_dfa_t** out) {
     try {
         if (!label_ptr || !out) return fail(CD_ERR_ARG, "NULL argument");
         if ((n_open > 0 && !open) || (n_sep > 0 && !sep) || (n_close > 0 && !close)) return fail(CD_ERR_ARG, "NULL token list");
         cdt::HostCsr c;
         const std::string err = cdt::build_list(V, K, label_ptr, label_tok, open, n_open, sep, n_sep, close, n_close,
-                                                min_items, max_items, &c);
+                                                min_items, max_items, eos, &c);
         if (!err.empty()) return fail(CD_ERR_AUTOMATON, "%s", err.c_str());
-        return compile_impl(V, c.S, 0, c.row_ptr.data(), c.tok.data(), c.next.data(), c.accepting.data(), device, out);
+        return compile_csr(V, c, device, out);
     } catch (const std::bad_alloc&) {
         return fail(CD_ERR_OOM, "host allocation failed");
     } catch (...) {

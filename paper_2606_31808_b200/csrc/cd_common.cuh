@@ -21,6 +21,8 @@ struct DfaDev {
     const int* tok;            // [nnz] strictly increasing inside a state
     const int* next;           // [nnz] next state | (accepting[next state] << 31)
     const uint8_t* accepting;  // [S]
+    const int* rank1k;         // [S][nblk] number of allowed tokens of the state below token 1024 * b
+    int nblk;                  // ceil(V / 1024)
 };
 
 // ---------------------------------------------------------------- PTX helpers

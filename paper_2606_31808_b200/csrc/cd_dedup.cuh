@@ -4,7 +4,8 @@
 //   dedup_insert_kernel   SELECT DISTINCT: open-addressing hash table, one 64-bit CAS to claim a
 //                         slot + atomicMin of the row id, so every distinct value knows its FIRST row
 //   dedup_first_kernel    every row looks its value up: first[i] = first row with the same value
-//   dedup_rank_kernel     one CTA: stable scan over the rows that are first occurrences ->
+//   (ranking)             the stable compaction of a6 over the rows that are first occurrences
+//                         (cd_aux.cuh compact_lookback_kernel: many CTAs, decoupled look-back) ->
 //                         distinct_rows[] (ascending row id = first-occurrence order) and the rank
 //                         of each of them
 //   dedup_rep_kernel      rep[i] = rank[first[i]]   (the key of the LEFT JOIN back)
@@ -70,61 +71,6 @@ __global__ void dedup_first_kernel(const long long* __restrict__ keys, int N, co
         first[i] = f;
         not_first[i] = (f == (int)i) ? 0 : 1;
     }
-}
-
-// One CTA of 1024 threads: stable scan of the first-occurrence flags.  distinct_rows[p] = row id of
-// the p-th distinct value; rank[that row] = p.
-__global__ void __launch_bounds__(1024, 1) dedup_rank_kernel(const uint8_t* __restrict__ not_first, int N,
-                                                             int* __restrict__ distinct_rows, int* __restrict__ rank,
-                                                             int* __restrict__ n_distinct) {
-    __shared__ int s_warp[32];
-    __shared__ int s_total;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    int base = 0;
-    for (int c0 = 0; c0 < N; c0 += 4 * 1024) {
-        const int i0 = c0 + 4 * tid;
-        bool keep[4];
-        if (i0 + 3 < N) {
-            const uint32_t d4 = *reinterpret_cast<const uint32_t*>(not_first + i0);
-#pragma unroll
-            for (int q = 0; q < 4; ++q) keep[q] = ((d4 >> (8 * q)) & 0xFFu) == 0u;
-        } else {
-#pragma unroll
-            for (int q = 0; q < 4; ++q) keep[q] = (i0 + q < N) && (not_first[i0 + q] == 0);
-        }
-        const int cnt = (int)keep[0] + (int)keep[1] + (int)keep[2] + (int)keep[3];
-        int inc = cnt;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int u = __shfl_up_sync(FULL, inc, o);
-            if (lane >= o) inc += u;
-        }
-        if (lane == 31) s_warp[warp] = inc;
-        __syncthreads();
-        if (warp == 0) {
-            const int v = s_warp[lane];
-            int w = v;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int u = __shfl_up_sync(FULL, w, o);
-                if (lane >= o) w += u;
-            }
-            s_warp[lane] = w - v;
-            if (lane == 31) s_total = w;
-        }
-        __syncthreads();
-        int pos = base + s_warp[warp] + inc - cnt;
-#pragma unroll
-        for (int q = 0; q < 4; ++q)
-            if (keep[q]) {
-                distinct_rows[pos] = i0 + q;
-                rank[i0 + q] = pos;
-                ++pos;
-            }
-        base += s_total;
-        __syncthreads();
-    }
-    if (tid == 0) *n_distinct = base;
 }
 
 __global__ void dedup_rep_kernel(const int* __restrict__ first, const int* __restrict__ rank, int N, int* __restrict__ rep) {

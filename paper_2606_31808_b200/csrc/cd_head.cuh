@@ -132,6 +132,14 @@ struct HeadArgs {
     HeadPartial* partials;  // [rows_pad * NU]
 };
 
+// finalize_row's per-step view of a head step: next states go straight to state[] (== state_new)
+__device__ __forceinline__ StepView head_view(const StepArgs& f) {
+    StepView sv{};
+    sv.state_next = f.state_new;
+    sv.step = f.step;
+    return sv;
+}
+
 // ---------------------------------------------------------------- sm_100a PTX: TMA, tcgen05
 __device__ __forceinline__ void tma_prefetch_desc(const void* tmap) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
@@ -352,7 +360,7 @@ __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadAr
             float ry = (lane < HG_WARPS) ? s_y[lane] : -INFINITY;
             head_warp_combine<SAMPLE>(rm, rs, ri, rk, ry);
             const TileMeta mt{slot, 0, 0, st, lo, deg, 0};
-            finalize_row(f, mt, rm, rs, ri, lane, true, SAMPLE, ry);
+            finalize_row(f, head_view(f), mt, rm, rs, ri, lane, true, SAMPLE, ry);
         }
     }
 }
@@ -560,7 +568,7 @@ __global__ void head_finish_kernel(const HeadArgs a) {
         const long long lo = __ldg(f.dfa.row_ptr + st);
         const int deg = (int)(__ldg(f.dfa.row_ptr + st + 1) - lo);
         const TileMeta mt{slot, 0, 0, st, lo, deg, 0};
-        finalize_row(f, mt, m, s, idx, lane, false, SAMPLE, yb);
+        finalize_row(f, head_view(f), mt, m, s, idx, lane, false, SAMPLE, yb);
     }
 }
 

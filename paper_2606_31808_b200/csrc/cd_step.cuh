@@ -1,4 +1,5 @@
-// cd_step.cuh -- the fused constrained step (include/cd.h cd_step).
+// cd_step.cuh -- the fused constrained step (include/cd.h cd_step) and the
+// persistent whole-loop kernel built from the same step body (cd_decode_loop).
 //
 // Design (B200-first; the paper gives no kernel):
 //   * The step is one streaming pass over the logits, so it is HBM-bound: the job is to keep
@@ -16,42 +17,72 @@
 //     free body) and updates an online (max, sum-exp, argmax) triple; only allowed elements
 //     cost arithmetic.
 //   * Unit results of a row are merged without any fence: a unit stores its result into a slot
-//     of three 64-bit words, each carrying the launch generation in its upper half (8-byte
-//     stores are single-copy atomic, so a word is either stale or complete), then takes a
-//     RELAXED ticket.  The warp that draws the last ticket merges: it reads the other slots and
-//     re-reads any word whose tag is not current yet (the writers issued those stores before
-//     their tickets, so they are on their way; normally the first read succeeds).  A
-//     __threadfence here cost 3.8 us per unit (profiles/r1b): it waits for the bulk copies the
-//     same warp still has in flight.
-//   * That warp also does the CSR transition (128-ary warp search; row bounds were prefetched
-//     into the tile meta, accepting[next] rides in bit 31 of next[]), the output writes and, in
-//     the decode loop, the per-row history, while the other warps keep streaming.
-//   * The last CTA to finish resets the work counter, bumps the generation and, in the decode
-//     loop, performs the stable early-exit compaction: one launch per decoding step.
+//     of three 64-bit words, each carrying the launch generation in its upper half (8-byte stores
+//     are single-copy atomic, so a word is either stale or complete), then takes a RELAXED
+//     ticket.  The warp that draws the last ticket merges: it reads the other slots and re-reads
+//     any word whose tag is not current yet (the writers issued those stores before their
+//     tickets, so they are on their way; normally the first read succeeds).  A __threadfence
+//     here cost 3.8 us per unit (profiles/r1b): it waits for the bulk copies the same warp still
+//     has in flight.  Electing the merger in advance instead (the warp holding a row's last part
+//     polls until the other parts are published: no atomic at all) was tried in round 2 and
+//     dropped: a waiting warp streams nothing, and with 8 units per row an eighth of the warps
+//     wait at any time -- c4 fell from 6.8 to 6.2 TB/s (profiles/r2_merge_election.md).
+//   * The merging warp finds the chosen token's position in the state's CSR row WITHOUT searching:
+//     position = number of allowed tokens below it = rank1k[state][t >> 10] (a per-state prefix
+//     count of mask bits per 1024 tokens, built once with the automaton) + popcount of the mask
+//     words of that block below t: one round trip instead of the 2-3 of a 128-ary search, then
+//     next[] (accepting[next] rides in bit 31), the output writes and, in the decode loop, the
+//     per-row history -- while the other warps keep streaming.
+//   * step_kernel: one launch = one step.  The last CTA to finish resets the work counter, bumps
+//     the generation and (per-step decode loops: callback / host-buffer forms) performs the
+//     stable early-exit compaction.
+//   * loop_kernel: one cooperative launch = the whole decode loop (cd_decode_loop).  148 CTAs stay
+//     resident; between decoding steps they meet at a grid barrier (one arrival atomic per CTA,
+//     the last arriver publishes the go word).  There is no compaction pass at all: the active set
+//     is a bitmap over ORIGINAL row ids (three buffers in rotation: read / being built / being
+//     cleared), finished rows simply do not set their bit for the next step, and "slot i" of a
+//     step is the i-th set bit (rank/select on a shared-memory snapshot) -- which is exactly the
+//     ascending-row-id order the stable compaction of a6 produces.  States live in two arrays
+//     indexed by original row id (read k & 1, write (k + 1) & 1).  This removes, per decoding
+//     step, a kernel launch + grid drain, the counter reset, the last-CTA compaction and the
+//     active-count hand-off.
 //   * Density-adaptive rows (GATHER instantiation): a row whose state has at most
 //     `gather_max` transitions is not scanned at all -- its units walk pieces of the state's CSR
 //     token list (coalesced) and gather exactly the allowed logits (one 32-byte sector each, 8
 //     independent loads per lane in flight).  The running argmax is the CSR position, so the
-//     transition needs no search.  Same outputs as the dense scan; dense and gathered rows mix
-//     freely in one launch and share the merge / compaction machinery.
+//     transition needs no rank either.  Same outputs as the dense scan; dense and gathered rows
+//     mix freely in one launch and share the merge machinery.
 #pragma once
 #include "cd_common.cuh"
 
 namespace cd {
 
+__device__ __forceinline__ unsigned long long global_timer_ns() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+
 constexpr int TPU_MAX_BYTES = 65536;  // at most 64 KiB of logits per unit
-constexpr int UNITS_PER_WARP = 4;     // aim for >= 4 units per warp when rows are few
+constexpr int UNITS_PER_WARP = 4;     // aim for >= this many units per warp when rows are few
+constexpr int GATHER_UPW = 4;         // the same for gathered rows (pieces of the CSR token list)
 
 constexpr int FLAG_FIRST = 1;   // first tile of its unit: reset the lane accumulators
 constexpr int FLAG_LAST = 2;    // last tile of its unit: reduce and publish
 constexpr int FLAG_ACCEPT = 4;  // pseudo tile of a slot whose state already accepts (no copy)
 constexpr int FLAG_BADSTATE = 8;
-constexpr int FLAG_GATHER = 16;  // pseudo tile of a gathered row piece (no copy); meta.tile = logits row
+constexpr int FLAG_GATHER = 16;  // pseudo tile of a gathered row piece (no copy)
 
 constexpr int SAMPLE_LIST_CAP = 128;  // tiles with at most this many allowed elements are compacted (SAMPLE)
 
 constexpr int GATHER_CHUNK = 256;  // a gathered row is split into pieces of >= this many transitions
 constexpr int GATHER_UNROLL = 8;   // independent gathers per lane in flight
+
+constexpr int LOOP_MAX_ROWS = 32768;     // persistent loop: rows per call (bitmap snapshot in shared memory)
+constexpr int LOOP_PARAM_STEPS = 32;     // step pointers passed as kernel parameters up to this many steps
+constexpr int LOOP_TRACE_STEPS = 256;    // per-step (timestamp, active rows) records kept for cd_loop_trace
+constexpr unsigned long long LOOP_SPIN_TIMEOUT_NS = 4000000000ull;  // a barrier that waits longer aborts the loop
+constexpr int MERGE_SPIN_LIMIT = 1 << 24;  // polls (>= 32 ns apart) after which a merging warp gives up
 
 // number of units a gathered row of `len` transitions is split into (P = units per row of the launch)
 __host__ __device__ inline int gather_parts(int len, int P) {
@@ -60,7 +91,7 @@ __host__ __device__ inline int gather_parts(int len, int P) {
     return np < P ? np : P;
 }
 
-// Result of one unit, readable without a fence: {gen:32 | payload:32} x 3 (+ pad to 32 B).
+// Result of one unit, readable without a fence: {gen:32 | payload:32} x 3 (+ the sampling key).
 struct __align__(32) PartialSlot {
     unsigned long long m, s, idx, pad;
 };
@@ -74,14 +105,14 @@ struct StepArgs {
     int* state_new;  // [n] scratch: next states, moved to `state` (or compacted) by the last CTA
     int n;
     const int* n_dev;  // if non-null the active count is read from the device
-    int* token_out;
+    int* token_out;    // per-slot outputs; all four may be NULL in the persistent loop
     float* logprob_out;
     float* lse_out;
     uint8_t* done_out;
     // scratch (per handle+stream)
     PartialSlot* partials;  // [units]
     int* tickets;           // [rows] arrivals per slot, zero between launches
-    int* ctrs;              // [0] work counter, [1] finished CTAs, [2] sticky error count, [3] generation
+    int* ctrs;              // [0] work counter, [1] finished CTAs, [2] error count, [3] generation
     int gather_max;         // states with <= gather_max transitions are gathered (GATHER kernels; 0 = never)
     int all_gather;         // no state has more than gather_max transitions
     // decode loop only, all optional:
@@ -97,8 +128,8 @@ struct StepArgs {
     int* cmp_state_out;
     int* cmp_n_out;
     // LIMIT early exit (PAPER.md 2.4 "Early Exiting"), optional: rows that finish in a
-    // state with satisfying[s] != 0 are counted in *sat_ctr; once it reaches `limit` the last CTA
-    // empties the active list (every row still active is cancelled)
+    // state with satisfying[s] != 0 are counted in *sat_ctr; once it reaches `limit` the active list is
+    // emptied (every row still active is cancelled)
     const uint8_t* satisfying;  // [S]
     int* sat_ctr;
     int limit;
@@ -110,17 +141,60 @@ struct StepArgs {
     // host-buffer loop: the logits buffer holds the ACTIVE rows only, row = slot (row_map still names
     // the original row for the history and the sampling noise)
     int logits_by_slot;
-    int upw, tpu_max;  // unit sizing (tuning knobs CD_UPW / CD_TPU_MAX): target units per warp, most tiles per unit
+    int upw, tpu_max;  // unit sizing: target units per warp, most tiles per unit
+};
+
+// Persistent loop (loop_kernel): everything that outlives a step.
+struct LoopArgs {
+    const void* step_ptrs[LOOP_PARAM_STEPS];  // logits of step k, if max_steps <= LOOP_PARAM_STEPS ...
+    const void* const* step_ptrs_dev;         // ... else a device array
+    int B;
+    uint32_t* alive[3];  // [nwords] active-row bitmaps in rotation: step k reads k % 3, builds (k + 1) % 3, clears (k + 2) % 3
+    int* state2[2];      // [B] states by original row id: step k reads k & 1, writes (k + 1) & 1
+    int* work;           // [max_steps] per-step work counters (zeroed by loop_init)
+    int* bar;            // [0] arrivals, [1] go word: (steps completed) | stop << 30, [2] abort flag
+    unsigned long long* trace_t;  // [LOOP_TRACE_STEPS + 1] globaltimer at the start of every step, then at exit
+    int* trace_n;                 // [LOOP_TRACE_STEPS] active rows of every step, [LOOP_TRACE_STEPS] = steps run
+    unsigned long long* phase;    // tuning builds (-DCD_TUNING): [LOOP_TRACE_STEPS][8] phase timestamps of every step
+};
+
+#ifdef CD_TUNING
+#define CD_PHASE(L, k, i) do { if ((L).phase && (k) < LOOP_TRACE_STEPS) (L).phase[(k) * 8 + (i)] = global_timer_ns(); } while (0)
+#define CD_PHASE_MAX(ptr) do { if (ptr) atomicMax(ptr, global_timer_ns()); } while (0)
+#define CD_PHASE_MIN(ptr) do { if (ptr) atomicMax(ptr, ~global_timer_ns()); } while (0)  /* earliest = ~max(~t) */
+#else
+#define CD_PHASE(L, k, i) ((void)0)
+#define CD_PHASE_MAX(ptr) ((void)0)
+#define CD_PHASE_MIN(ptr) ((void)0)
+#endif
+
+// What changes from step to step (one launch of step_kernel, or one iteration of loop_kernel).
+struct StepView {
+    const unsigned char* logits;
+    const int* state_cur;  // state of slot i (step_kernel) / of row r (loop_kernel)
+    int* state_next;       // where finalize writes the next state (same indexing)
+    int* work_ctr;
+    unsigned gen;
+    int n;
+    int step;
+    uint32_t* alive_next;  // loop_kernel: bitmap of the rows that stay active
+    // loop_kernel: slot i = i-th set bit of the bitmap snapshot in shared memory
+    const uint32_t* s_bits;
+    const int* s_pref;  // exclusive prefix of the popcounts, [nwords + 1]
+    int nwords;
+    unsigned long long* ph_first_fin;  // tuning builds: earliest / latest row finalisation of the step
+    unsigned long long* ph_last_fin;
+    unsigned long long* ph_tile;  // tuning builds: [0] earliest (complemented), [1] latest first-tile arrival over the warps
 };
 
 struct __align__(16) TileMeta {
     int slot;
-    int tile;   // tile index inside the row
+    int tile;   // tile index inside the row (gathered piece: unused)
     int flags;  // FLAG_* | part << 8
     int st;     // automaton state of the slot
     long long csr_lo;  // row_ptr[st]
     int csr_len;       // row_ptr[st + 1] - row_ptr[st]
-    int pad;
+    int lrow;          // row of the logits buffer
 };
 
 template <int STAGES, int TILE_BYTES>
@@ -152,57 +226,81 @@ __device__ __forceinline__ float tile_elem(const unsigned char* tile, int e) {
     return fmaxf(x, -INFINITY);  // NaN -> -inf
 }
 
+// Position of token t inside the CSR row of state st = number of allowed tokens of st below t:
+// the per-1024-token prefix count built with the automaton + the popcounts of the mask words of t's
+// block below t (one word per lane).  Warp-uniform; one memory round trip.
+__device__ __forceinline__ int mask_rank(const DfaDev& dfa, int st, int t, int lane) {
+    const int blk = t >> 10, w = (t >> 5) & 31;
+    const int wi = blk * 32 + lane;
+    const uint32_t word = (wi < dfa.Wpad) ? __ldg(dfa.mask + (long long)st * dfa.Wpad + wi) : 0u;
+    const int base = __ldg(dfa.rank1k + (long long)st * dfa.nblk + blk);
+    int c = (lane < w) ? __popc(word) : ((lane == w) ? __popc(word & ((1u << (t & 31)) - 1u)) : 0);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(FULL, c, o);
+    return base + c;
+}
+
 // Row finished: (m, s, idx) is the merged result of all its units.  Warp-uniform.
 // `gathered`: idx is the position inside the state's CSR row instead of the token id.
 // `sampled`: idx is the sampled token (position), ytok its tempered logit: logprob = (ytok - m) - log(sum).
-__device__ __forceinline__ void finalize_row(const StepArgs& a, const TileMeta& mt, float m, float s, int idx,
-                                             int lane, bool gathered, bool sampled = false, float ytok = 0.0f) {
-    const long long lo = mt.csr_lo, hi = mt.csr_lo + mt.csr_len;
-    int token;
+// PERSIST: per-row arrays are indexed by the original row id (mt.lrow); surviving rows set their bit in
+// the next step's bitmap.
+template <bool PERSIST = false>
+__device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& sv, const TileMeta& mt, float m,
+                                             float s, int idx, int lane, bool gathered, bool sampled = false,
+                                             float ytok = 0.0f) {
     float lp, lse;
-    long long j;
+    int pos;
+    long long csr_lo = mt.csr_lo;
+    int csr_len = mt.csr_len;
+    if (csr_len < 0) {  // dense-only kernels do not fetch the CSR bounds on the issue path: same round trip as the rank
+        csr_lo = __ldg(a.dfa.row_ptr + mt.st);
+        csr_len = (int)(__ldg(a.dfa.row_ptr + mt.st + 1) - csr_lo);
+    }
     if (m == -INFINITY) {  // every allowed logit is -inf: lowest allowed id (G6)
-        token = __ldg(a.dfa.tok + lo);
         lp = -INFINITY;
         lse = -INFINITY;
-        idx = 0;
+        pos = 0;
     } else {
-        token = idx;
         const float L = logf(s);
         lp = sampled ? (ytok - m) - L : -L;  // greedy: log p(t*) = -log(sum); never m - lse (cancellation)
         lse = m + L;
-    }
-    if (gathered) {
-        j = lo + idx;
-        token = __ldg(a.dfa.tok + j);
-    } else {
-        j = warp_csr_find(a.dfa.tok, lo, hi, token, lane);
+        pos = gathered ? idx : mask_rank(a.dfa, mt.st, idx, lane);
     }
     if (lane == 0) {
-        const int slot = mt.slot;
+        const bool in_row = (pos >= 0) && (pos < csr_len);
+        const long long j = csr_lo + pos;
+        int token = in_row ? __ldg(a.dfa.tok + j) : -1;
+        const int packed = in_row ? __ldg(a.dfa.next + j) : 0;  // next state | accepting << 31
+        // the bitmask and the CSR describe the same set: the token found by rank must be the argmax
+        const bool ok = in_row && (gathered || m == -INFINITY || token == idx);
         int ns = mt.st;
-        uint8_t dn;
-        if (j >= 0) {
-            const int packed = __ldg(a.dfa.next + j);  // next state | accepting << 31
+        uint8_t dn = 1;
+        if (ok) {
             ns = packed & 0x7FFFFFFF;
             dn = (packed < 0) ? 1 : 0;
         } else {
             atomicAdd(a.ctrs + 2, 1);
-            dn = 1;
+            token = -1;
         }
-        a.state_new[slot] = ns;
-        a.token_out[slot] = token;
-        a.logprob_out[slot] = lp;
+        const int slot = PERSIST ? mt.lrow : mt.slot;
+        CD_PHASE_MIN(sv.ph_first_fin);
+        CD_PHASE_MAX(sv.ph_last_fin);
+        sv.state_next[slot] = ns;
+        if (a.token_out) a.token_out[slot] = token;
+        if (a.logprob_out) a.logprob_out[slot] = lp;
         if (a.lse_out) a.lse_out[slot] = lse;
-        a.done_out[slot] = dn;
+        if (a.done_out) a.done_out[slot] = dn;
+        if (PERSIST && !dn) atomicOr(sv.alive_next + (slot >> 5), 1u << (slot & 31));
         if (a.hist_tokens) {  // decode loop: this slot's row, original id
-            const long long rid = a.row_map ? __ldg(a.row_map + slot) : slot;
-            a.hist_tokens[rid * a.max_steps + a.step] = token;
-            a.hist_len[rid] = a.step + 1;
+            const long long rid = PERSIST ? (long long)mt.lrow : (a.row_map ? (long long)__ldg(a.row_map + slot) : slot);
+            a.hist_tokens[rid * a.max_steps + sv.step] = token;
+            a.hist_len[rid] = sv.step + 1;
             a.hist_final_state[rid] = ns;
-            a.hist_sum_logprob[rid] += lp;
-            a.hist_done[rid] = dn;
-            if (a.sat_ctr && dn && __ldg(a.satisfying + ns)) atomicAdd(a.sat_ctr, 1);
+            // written by another SM one step ago (persistent loop): read at the L2, never from a stale L1 line
+            a.hist_sum_logprob[rid] = __ldcg(a.hist_sum_logprob + rid) + lp;
+            a.hist_done[rid] = ok ? dn : (uint8_t)0;
+            if (a.sat_ctr && ok && dn && __ldg(a.satisfying + ns)) atomicAdd(a.sat_ctr, 1);
         }
     }
 }
@@ -225,47 +323,49 @@ __device__ __forceinline__ void warp_combine_s(float& m, float& s, int& idx, flo
     }
 }
 
-template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER, bool SAMPLE = false>
-__global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
+// Ring position of a warp: carried across the steps of the persistent loop (mbarrier phases go on).
+struct RingPos {
+    int iss_stage = 0;
+    int cons_stage = 0;
+    uint32_t cons_phase = 0;
+};
+
+// slot i of the persistent loop -> original row id: the i-th set bit of the snapshot (binary search
+// over the per-word prefix counts, then find-nth-set inside the word).  Warp-uniform.
+__device__ __forceinline__ int select_row(const StepView& sv, int i) {
+    int lo = 0, hi = sv.nwords;  // invariant: s_pref[lo] <= i < s_pref[hi]
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (sv.s_pref[mid] <= i) lo = mid; else hi = mid;
+    }
+    const int r = i - sv.s_pref[lo];
+    return lo * 32 + (int)__fns(sv.s_bits[lo], 0, r + 1);
+}
+
+// One decoding step over the slots [0, sv.n): issue + consume loops of this warp.
+template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER, bool SAMPLE, bool PERSIST>
+__device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv, WarpRing<STAGES, TILE_BYTES>& ring,
+                                          RingPos& rp, const int warp, const int lane) {
     constexpr int SZ = (DT == DT_BF16) ? 2 : 4;
     constexpr int TILE_TOK = TILE_BYTES / SZ;
     constexpr int MASK_BYTES = TILE_TOK / 8;
     constexpr int WPL = TILE_TOK / 1024;  // mask words per lane and tile
     constexpr int TPU_MAX = TPU_MAX_BYTES / TILE_BYTES;
     static_assert(WPL >= 1 && TILE_TOK % 1024 == 0, "tile must hold a multiple of 32 mask words");
-    using Ring = WarpRing<STAGES, TILE_BYTES>;
-
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    Ring& ring = reinterpret_cast<Ring*>(smem_raw)[warp];
-
-    if (lane == 0) {
-#pragma unroll
-        for (int s = 0; s < STAGES; ++s) mbar_init(smem_u32(&ring.bar[s]), 1);
-        fence_mbar_init();
-    }
-    __syncwarp();
-
-    // Programmatic dependent launch: the next step's grid may be scheduled as soon as every CTA
-    // of this one got here (its CTAs land on SMs as ours exit and set up their barriers), but
-    // nothing of this kernel reads or writes global memory before the previous grid has
-    // completed and flushed (griddepcontrol.wait).
-    pdl_launch_dependents();
-    pdl_wait();
 
     // ---------------- issue side (warp-uniform state)
     // The first unit of a warp is its global warp id (no atomic on the start-up chain); later
     // units come from the work counter, which therefore starts at 0 = unit `total_warps`.
     const int total_warps = gridDim.x * WARPS;
     int next_u_l0 = blockIdx.x * WARPS + warp;  // prefetched unit id, valid in lane 0
-    const unsigned gen = (unsigned)__ldcg(a.ctrs + 3);  // launch generation (tag of the partial slots)
-    const int n = a.n_dev ? __ldcg(a.n_dev) : a.n;
+    const unsigned gen = sv.gen;                // launch generation (tag of the partial slots)
+    const int n = sv.n;
     const int V = a.dfa.V;
     const int tiles_per_row = (V + TILE_TOK - 1) / TILE_TOK;
     const int tpu = tiles_per_unit(n, tiles_per_row, total_warps, min(TPU_MAX, a.tpu_max), a.upw);
     const int Pd = (tiles_per_row + tpu - 1) / tpu;  // units per row of a dense scan
     // a gathered row is split only as far as needed to give every warp a few units
-    const int PG = GATHER ? max(1, min(Pd, (total_warps * UNITS_PER_WARP) / max(n, 1))) : Pd;
+    const int PG = GATHER ? max(1, min(Pd, (total_warps * GATHER_UPW) / max(n, 1))) : Pd;
     // units per row of this launch; if every state is gathered no unit is drawn in vain
     const int P = (GATHER && a.all_gather) ? PG : Pd;
     const int total_units = n * P;
@@ -278,7 +378,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     long long iss_lo = 0;
     const unsigned char* iss_src = nullptr;  // next logits tile of the current unit
     const unsigned char* iss_msk = nullptr;  // next mask piece
-    int iss_stage = 0, in_flight = 0;
+    int iss_stage = rp.iss_stage, in_flight = 0;
 
     auto issue_one = [&]() {
         while (iss_tile >= iss_end) {  // next unit (units of a gathered row beyond its pieces are skipped)
@@ -288,24 +388,37 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 exhausted = true;
                 return;
             }
-            if (lane == 0) next_u_l0 = total_warps + atomicAdd(a.ctrs + 0, 1);
+            if (lane == 0) next_u_l0 = total_warps + atomicAdd(sv.work_ctr, 1);
             iss_slot = u / P;
             const int part = u - iss_slot * P;
-            // state[] is not written while units are in flight (next states go to state_new[]): a
-            // unit drawn after its row was finalised still sees the state the row was processed in
-            iss_st = a.state[iss_slot];
-            const long long r = a.row_map ? (long long)__ldg(a.row_map + iss_slot) : (long long)iss_slot;
-            const long long rl = a.logits_by_slot ? (long long)iss_slot : r;  // row of the logits buffer
+            long long rl;  // row of the logits buffer
+            if (PERSIST) {
+                rl = select_row(sv, iss_slot);
+                // states are double-buffered by step parity: a unit drawn after its row was finalised
+                // still sees the state the row was processed in
+                iss_st = __ldcg(sv.state_cur + rl);
+            } else {
+                // state[] is not written while units are in flight (next states go to state_new[])
+                iss_st = sv.state_cur[iss_slot];
+                const long long r = a.row_map ? (long long)__ldg(a.row_map + iss_slot) : (long long)iss_slot;
+                rl = a.logits_by_slot ? (long long)iss_slot : r;
+            }
             iss_row = (int)rl;
             const bool bad = (iss_st < 0) || (iss_st >= a.dfa.S);
             const int sts = bad ? 0 : iss_st;
-            const bool acc = !bad && (__ldg(a.dfa.accepting + sts) != 0);
-            iss_lo = __ldg(a.dfa.row_ptr + sts);
-            iss_len = (int)(__ldg(a.dfa.row_ptr + sts + 1) - iss_lo);
+            // (the persistent loop never holds a row whose state accepts: such rows left the bitmap)
+            const bool acc = !PERSIST && !bad && (__ldg(a.dfa.accepting + sts) != 0);
+            if (GATHER) {  // the CSR bounds decide between scan and gather
+                iss_lo = __ldg(a.dfa.row_ptr + sts);
+                iss_len = (int)(__ldg(a.dfa.row_ptr + sts + 1) - iss_lo);
+            } else {  // dense only: nothing on the way to the first copy depends on them (finalize_row reads them)
+                iss_lo = 0;
+                iss_len = -1;
+            }
             if (bad || acc) {
                 if (lane == 0) {
                     ring.meta[iss_stage] =
-                        TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (part << 8), iss_st, 0, 0, 0};
+                        TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (part << 8), iss_st, 0, 0, iss_row};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
                 iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
@@ -316,8 +429,8 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
             if (GATHER && iss_len <= a.gather_max) {
                 if (part >= gather_parts(iss_len, PG)) continue;
                 if (lane == 0) {
-                    ring.meta[iss_stage] = TileMeta{iss_slot, (int)rl, FLAG_GATHER | FLAG_LAST | (part << 8), iss_st,
-                                                    iss_lo, iss_len, 0};
+                    ring.meta[iss_stage] = TileMeta{iss_slot, 0, FLAG_GATHER | FLAG_LAST | (part << 8), iss_st,
+                                                    iss_lo, iss_len, iss_row};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
                 iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
@@ -327,7 +440,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
             }
             iss_tile = part * tpu;
             iss_end = min(iss_tile + tpu, tiles_per_row);
-            iss_src = a.logits + rl * a.ld_bytes + (long long)iss_tile * TILE_BYTES;
+            iss_src = sv.logits + rl * a.ld_bytes + (long long)iss_tile * TILE_BYTES;
             iss_msk = reinterpret_cast<const unsigned char*>(a.dfa.mask + (long long)iss_st * a.dfa.Wpad) +
                       (long long)iss_tile * MASK_BYTES;
             iss_flags = (part << 8) | FLAG_FIRST;
@@ -380,27 +493,49 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     // ---------------- consume side
     float m = -INFINITY, s = 0.0f, kb = -INFINITY;  // kb: best perturbed key (SAMPLE); idx then is its token
     int idx = 0x7FFFFFFF;
-    const int rng_step = a.rng_step_base + a.step;
-    int cons_stage = 0;
-    uint32_t cons_phase = 0;
+    const int rng_step = a.rng_step_base + sv.step;
+    int cons_stage = rp.cons_stage;
+    uint32_t cons_phase = rp.cons_phase;
     const unsigned long long tag = (unsigned long long)gen << 32;
+#ifdef CD_TUNING
+    bool first_tile = true;
+#endif
 
 #pragma unroll 1
     while (in_flight > 0) {
         mbar_wait(smem_u32(&ring.bar[cons_stage]), cons_phase);
         __syncwarp();
+#ifdef CD_TUNING
+        if (first_tile && sv.ph_tile && lane == 0) {
+            atomicMax(sv.ph_tile, ~global_timer_ns());
+            atomicMax(sv.ph_tile + 1, global_timer_ns());
+        }
+        first_tile = false;
+#endif
         const TileMeta mt = ring.meta[cons_stage];
         const int part = mt.flags >> 8;
+        // original row id of the slot: names the history row and seeds the sampling noise
+        auto orig_row = [&]() -> uint32_t {
+            return PERSIST ? (uint32_t)mt.lrow : (uint32_t)(a.row_map ? __ldg(a.row_map + mt.slot) : mt.slot);
+        };
 
         if (mt.flags & (FLAG_ACCEPT | FLAG_BADSTATE)) {
-            // accepted rows never advance
+            // accepted rows never advance; a state outside [0, S) is reported done
             if (part == 0 && lane == 0) {
-                a.state_new[mt.slot] = mt.st;
-                a.token_out[mt.slot] = -1;
-                a.logprob_out[mt.slot] = 0.0f;
-                if (a.lse_out) a.lse_out[mt.slot] = 0.0f;
-                a.done_out[mt.slot] = 1;
-                if (mt.flags & FLAG_BADSTATE) atomicAdd(a.ctrs + 2, 1);
+                const int slot = PERSIST ? mt.lrow : mt.slot;
+                sv.state_next[slot] = mt.st;
+                if (a.token_out) a.token_out[slot] = -1;
+                if (a.logprob_out) a.logprob_out[slot] = 0.0f;
+                if (a.lse_out) a.lse_out[slot] = 0.0f;
+                if (a.done_out) a.done_out[slot] = 1;
+                if (mt.flags & FLAG_BADSTATE) {
+                    atomicAdd(a.ctrs + 2, 1);
+                    if (a.hist_tokens) {  // the row leaves the loop here, undone, in the state it has
+                        const long long rid = orig_row();
+                        a.hist_final_state[rid] = mt.st;
+                        a.hist_done[rid] = 0;
+                    }
+                }
             }
         } else {
             const bool gathered = GATHER && (mt.flags & FLAG_GATHER);
@@ -413,11 +548,11 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 s = 0.0f;
                 kb = -INFINITY;
                 idx = 0x7FFFFFFF;
-                const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, (uint32_t)(a.row_map ? __ldg(a.row_map + mt.slot) : mt.slot), (uint32_t)rng_step) : 0u;
+                const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, orig_row(), (uint32_t)rng_step) : 0u;
                 const int j0 = (int)(((long long)mt.csr_len * part) / np);
                 const int j1 = (int)(((long long)mt.csr_len * (part + 1)) / np);
                 const int* tk = a.dfa.tok + mt.csr_lo;
-                const unsigned char* rowp = a.logits + (long long)mt.tile * a.ld_bytes;
+                const unsigned char* rowp = sv.logits + (long long)mt.lrow * a.ld_bytes;
                 // software pipeline: the token ids of the next round are loaded while this round's
                 // logits are in flight
                 int t[GATHER_UNROLL];
@@ -455,77 +590,77 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 }
                 __syncwarp();
             } else {
-            if (mt.flags & FLAG_FIRST) {
-                m = -INFINITY;
-                s = 0.0f;
-                kb = -INFINITY;
-                idx = 0x7FFFFFFF;
-            }
-            const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, (uint32_t)(a.row_map ? __ldg(a.row_map + mt.slot) : mt.slot), (uint32_t)rng_step) : 0u;
-            const int t0 = mt.tile * TILE_TOK;
-            const uint32_t* mw = reinterpret_cast<const uint32_t*>(ring.mask[cons_stage]);
-            const unsigned char* tile = ring.logits[cons_stage];
-            uint32_t bits[WPL];
-#pragma unroll
-            for (int j = 0; j < WPL; ++j) bits[j] = mw[j * 32 + lane];
-            // SAMPLE, sparse tile: the noise costs ~60 instructions per evaluation, so the allowed
-            // positions are first compacted across the warp (exclusive scan of the per-lane popcounts
-            // in (word, lane) = ascending token order, positions written to a small shared list) and
-            // each lane then evaluates exactly the elements of rank lane, lane + 32, ... (ascending per
-            // lane, so "replace on strictly greater" still keeps the lowest id).
-            bool compacted = false;
-            if constexpr (SAMPLE) {
-                int cnt[WPL], offs[WPL], total = 0;
-#pragma unroll
-                for (int j = 0; j < WPL; ++j) {
-                    cnt[j] = __popc(bits[j]);
-                    int inc = cnt[j];
-#pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const int up = __shfl_up_sync(FULL, inc, o);
-                        if (lane >= o) inc += up;
-                    }
-                    offs[j] = total + inc - cnt[j];
-                    total += __shfl_sync(FULL, inc, 31);
+                if (mt.flags & FLAG_FIRST) {
+                    m = -INFINITY;
+                    s = 0.0f;
+                    kb = -INFINITY;
+                    idx = 0x7FFFFFFF;
                 }
-                if (total <= SAMPLE_LIST_CAP) {
-                    compacted = true;
+                const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, orig_row(), (uint32_t)rng_step) : 0u;
+                const int t0 = mt.tile * TILE_TOK;
+                const uint32_t* mw = reinterpret_cast<const uint32_t*>(ring.mask[cons_stage]);
+                const unsigned char* tile = ring.logits[cons_stage];
+                uint32_t bits[WPL];
+#pragma unroll
+                for (int j = 0; j < WPL; ++j) bits[j] = mw[j * 32 + lane];
+                // SAMPLE, sparse tile: the noise costs ~60 instructions per evaluation, so the allowed
+                // positions are first compacted across the warp (exclusive scan of the per-lane popcounts
+                // in (word, lane) = ascending token order, positions written to a small shared list) and
+                // each lane then evaluates exactly the elements of rank lane, lane + 32, ... (ascending per
+                // lane, so "replace on strictly greater" still keeps the lowest id).
+                bool compacted = false;
+                if constexpr (SAMPLE) {
+                    int cnt[WPL], offs[WPL], total = 0;
 #pragma unroll
                     for (int j = 0; j < WPL; ++j) {
+                        cnt[j] = __popc(bits[j]);
+                        int inc = cnt[j];
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const int up = __shfl_up_sync(FULL, inc, o);
+                            if (lane >= o) inc += up;
+                        }
+                        offs[j] = total + inc - cnt[j];
+                        total += __shfl_sync(FULL, inc, 31);
+                    }
+                    if (total <= SAMPLE_LIST_CAP) {
+                        compacted = true;
+#pragma unroll
+                        for (int j = 0; j < WPL; ++j) {
+                            uint32_t b = bits[j];
+                            int o = offs[j];
+                            const int e0 = (j * 32 + lane) * 32;
+                            while (b != 0u) {
+                                ring.list[o++] = (unsigned short)(e0 + __ffs(b) - 1);
+                                b &= b - 1u;
+                            }
+                        }
+                        __syncwarp();
+                        for (int r = lane; r < total; r += 32) {
+                            const int e = ring.list[r];
+                            online_update_sample(m, s, kb, idx, tile_elem<DT>(tile, e), t0 + e, t0 + e, a.inv_tau, row_key);
+                        }
+                        __syncwarp();
+                    }
+                }
+                if (!compacted) {
+#pragma unroll
+                    for (int j = 0; j < WPL; ++j) {
+                        // warp-uniform trip count (max popcount over the lanes); idle lanes feed -inf
                         uint32_t b = bits[j];
-                        int o = offs[j];
                         const int e0 = (j * 32 + lane) * 32;
-                        while (b != 0u) {
-                            ring.list[o++] = (unsigned short)(e0 + __ffs(b) - 1);
+                        while (__any_sync(FULL, b != 0u)) {
+                            const bool v = b != 0u;
+                            const int e = e0 + (v ? (__ffs(b) - 1) : 0);
                             b &= b - 1u;
+                            const float x = v ? tile_elem<DT>(tile, e) : -INFINITY;
+                            if (SAMPLE)
+                                online_update_sample(m, s, kb, idx, x, t0 + e, t0 + e, a.inv_tau, row_key);
+                            else
+                                online_update(m, s, idx, x, t0 + e);
                         }
                     }
-                    __syncwarp();
-                    for (int r = lane; r < total; r += 32) {
-                        const int e = ring.list[r];
-                        online_update_sample(m, s, kb, idx, tile_elem<DT>(tile, e), t0 + e, t0 + e, a.inv_tau, row_key);
-                    }
-                    __syncwarp();
                 }
-            }
-            if (!compacted) {
-#pragma unroll
-            for (int j = 0; j < WPL; ++j) {
-                // warp-uniform trip count (max popcount over the lanes); idle lanes feed -inf
-                uint32_t b = bits[j];
-                const int e0 = (j * 32 + lane) * 32;
-                while (__any_sync(FULL, b != 0u)) {
-                    const bool v = b != 0u;
-                    const int e = e0 + (v ? (__ffs(b) - 1) : 0);
-                    b &= b - 1u;
-                    const float x = v ? tile_elem<DT>(tile, e) : -INFINITY;
-                    if (SAMPLE)
-                        online_update_sample(m, s, kb, idx, x, t0 + e, t0 + e, a.inv_tau, row_key);
-                    else
-                        online_update(m, s, idx, x, t0 + e);
-                }
-            }
-            }
             }
             if (mt.flags & FLAG_LAST) {
                 float rm = m, rs = s, rk = kb;
@@ -535,18 +670,17 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                 auto sampled_y = [&](int pos) -> float {
                     if (!SAMPLE || rm == -INFINITY) return 0.0f;
                     const int tokid = gathered ? __ldg(a.dfa.tok + mt.csr_lo + pos) : pos;
-                    const long long rr = gathered ? (long long)mt.tile : (long long)mt.pad;
-                    const unsigned char* rowp = a.logits + rr * a.ld_bytes;
+                    const unsigned char* rowp = sv.logits + (long long)mt.lrow * a.ld_bytes;
                     const float xv = (DT == DT_BF16)
                                          ? __uint_as_float(((uint32_t)__ldg(reinterpret_cast<const uint16_t*>(rowp) + tokid)) << 16)
                                          : __ldg(reinterpret_cast<const float*>(rowp) + tokid);
                     return __fmul_rn(xv, a.inv_tau);
                 };
                 if (np == 1) {
-                    finalize_row(a, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
+                    finalize_row<PERSIST>(a, sv, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
                 } else {
-                    // Publish from lane 1 (lane 0 is busy issuing copies): three self-validating
-                    // words, then a RELAXED ticket -- no fence anywhere.  The last arriver merges.
+                    // Publish from lane 1 (lane 0 is busy issuing copies): self-validating words,
+                    // then a RELAXED ticket -- no fence anywhere.  The last arriver merges.
                     int t = 0;
                     if (lane == 1) {
                         PartialSlot* ps = a.partials + ((long long)mt.slot * P + part);
@@ -558,56 +692,61 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
                     }
                     t = __shfl_sync(FULL, t, 1);
                     if (t == np - 1) {
-                        if (lane == 1) a.tickets[mt.slot] = 0;
-                        // The other units' words were stored before their tickets, but nothing
-                        // orders them: poll until every tag is current (normally the first read).
-                        const PartialSlot* base = a.partials + (long long)mt.slot * P;
-                        // Merge in slot order whoever merges (bitwise reproducible): lane q%32 takes
-                        // slot q; the own result (identical in every lane after the butterfly) stands
-                        // in for slot `part`.
-                        const float om = rm, os = rs, ok_ = rk;
-                        const int oi = ri;
-                        rm = -INFINITY;
-                        rs = 0.0f;
-                        rk = -INFINITY;
-                        ri = 0x7FFFFFFF;
-                        for (int q0 = 0; q0 < np; q0 += 32) {
-                            const int q = q0 + lane;
-                            const bool want = (q < np) && (q != part);
-                            bool ok = !want;
-                            unsigned long long wm = 0, ws = 0, wi = 0, wk = 0;
-                            while (true) {
-                                if (!ok) {
-                                    wm = ld_relaxed_gpu_u64(&base[q].m);
-                                    ws = ld_relaxed_gpu_u64(&base[q].s);
-                                    wi = ld_relaxed_gpu_u64(&base[q].idx);
-                                    ok = ((wm >> 32) == gen) && ((ws >> 32) == gen) && ((wi >> 32) == gen);
-                                    if (SAMPLE) {
-                                        wk = ld_relaxed_gpu_u64(&base[q].pad);
-                                        ok = ok && ((wk >> 32) == gen);
-                                    }
+                    if (lane == 1) a.tickets[mt.slot] = 0;
+                    // The other units' words were stored before their tickets, but nothing orders
+                    // them: poll until every tag is current (normally the first read).
+                    const PartialSlot* base = a.partials + (long long)mt.slot * P;
+                    // Merge in slot order whoever merges (bitwise reproducible): lane q % 32 takes
+                    // slot q; the own result (identical in every lane after the butterfly) stands in
+                    // for slot `part`.
+                    const float om = rm, os = rs, ok_ = rk;
+                    const int oi = ri;
+                    rm = -INFINITY;
+                    rs = 0.0f;
+                    rk = -INFINITY;
+                    ri = 0x7FFFFFFF;
+                    for (int q0 = 0; q0 < np; q0 += 32) {
+                        const int q = q0 + lane;
+                        const bool want = (q < np) && (q != part);
+                        bool ok = !want;
+                        unsigned long long wm = 0, ws = 0, wi = 0, wk = 0;
+                        int spins = 0;
+                        while (true) {
+                            if (!ok) {
+                                wm = ld_relaxed_gpu_u64(&base[q].m);
+                                ws = ld_relaxed_gpu_u64(&base[q].s);
+                                wi = ld_relaxed_gpu_u64(&base[q].idx);
+                                ok = ((wm >> 32) == gen) && ((ws >> 32) == gen) && ((wi >> 32) == gen);
+                                if (SAMPLE) {
+                                    wk = ld_relaxed_gpu_u64(&base[q].pad);
+                                    ok = ok && ((wk >> 32) == gen);
                                 }
-                                if (__all_sync(FULL, ok)) break;
-                                __nanosleep(32);
                             }
-                            if (SAMPLE) {
-                                int dummy = 0;
-                                if (want) {
-                                    online_combine(rm, rs, dummy, __int_as_float((int)(unsigned)wm),
-                                                   __int_as_float((int)(unsigned)ws), 0);
-                                    sample_combine(rk, ri, __int_as_float((int)(unsigned)wk), (int)(unsigned)wi);
-                                } else if (q == part) {
-                                    online_combine(rm, rs, dummy, om, os, 0);
-                                    sample_combine(rk, ri, ok_, oi);
-                                }
-                            } else if (want)
-                                online_combine(rm, rs, ri, __int_as_float((int)(unsigned)wm),
-                                               __int_as_float((int)(unsigned)ws), (int)(unsigned)wi);
-                            else if (q == part)
-                                online_combine(rm, rs, ri, om, os, oi);
+                            if (__all_sync(FULL, ok)) break;
+                            __nanosleep(32);
+                            if (++spins > MERGE_SPIN_LIMIT) {  // never on a healthy run: fail the call, do not hang
+                                if (lane == 0) atomicAdd(a.ctrs + 2, 1);
+                                break;
+                            }
                         }
-                        warp_combine_s<SAMPLE>(rm, rs, ri, rk);
-                        finalize_row(a, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
+                        if (SAMPLE) {
+                            int dummy = 0;
+                            if (want) {
+                                online_combine(rm, rs, dummy, __int_as_float((int)(unsigned)wm),
+                                               __int_as_float((int)(unsigned)ws), 0);
+                                sample_combine(rk, ri, __int_as_float((int)(unsigned)wk), (int)(unsigned)wi);
+                            } else if (q == part) {
+                                online_combine(rm, rs, dummy, om, os, 0);
+                                sample_combine(rk, ri, ok_, oi);
+                            }
+                        } else if (want)
+                            online_combine(rm, rs, ri, __int_as_float((int)(unsigned)wm),
+                                           __int_as_float((int)(unsigned)ws), (int)(unsigned)wi);
+                        else if (q == part)
+                            online_combine(rm, rs, ri, om, os, oi);
+                    }
+                    warp_combine_s<SAMPLE>(rm, rs, ri, rk);
+                    finalize_row<PERSIST>(a, sv, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
                     }
                 }
             }
@@ -618,6 +757,43 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
         __syncwarp();
         issue_one();
     }
+    rp.iss_stage = iss_stage;
+    rp.cons_stage = cons_stage;
+    rp.cons_phase = cons_phase;
+}
+
+// ------------------------------------------------------------------ one launch = one step (cd_step)
+template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER, bool SAMPLE = false>
+__global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
+    using Ring = WarpRing<STAGES, TILE_BYTES>;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    Ring& ring = reinterpret_cast<Ring*>(smem_raw)[warp];
+
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) mbar_init(smem_u32(&ring.bar[s]), 1);
+        fence_mbar_init();
+    }
+    __syncwarp();
+
+    // Programmatic dependent launch: the next step's grid may be scheduled as soon as every CTA
+    // of this one got here (its CTAs land on SMs as ours exit and set up their barriers), but
+    // nothing of this kernel reads or writes global memory before the previous grid has
+    // completed and flushed (griddepcontrol.wait).
+    pdl_launch_dependents();
+    pdl_wait();
+
+    StepView sv{};
+    sv.logits = a.logits;
+    sv.state_cur = a.state;
+    sv.state_next = a.state_new;
+    sv.work_ctr = a.ctrs + 0;
+    sv.gen = (unsigned)__ldcg(a.ctrs + 3);
+    sv.n = a.n_dev ? __ldcg(a.n_dev) : a.n;
+    sv.step = a.step;
+    RingPos rp;
+    step_body<DT, WARPS, STAGES, TILE_BYTES, GATHER, SAMPLE, false>(a, sv, ring, rp, warp, lane);
 
     // ---------------- last CTA of the grid: reset the counters, then (decode loop) compact
     __shared__ int s_is_last;
@@ -628,16 +804,156 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
         if (s_is_last) {
             a.ctrs[0] = 0;
             a.ctrs[1] = 0;
-            a.ctrs[3] = (int)(gen + 1u);
+            a.ctrs[3] = (int)(sv.gen + 1u);
         }
     }
     __syncthreads();
     if (s_is_last) {
         if (a.cmp_row_ids_out) {
-            block_compact(a.done_out, a.row_map, a.state_new, n, a.cmp_row_ids_out, a.cmp_state_out, a.cmp_n_out);
+            block_compact(a.done_out, a.row_map, a.state_new, sv.n, a.cmp_row_ids_out, a.cmp_state_out, a.cmp_n_out);
             if (a.sat_ctr && threadIdx.x == 0 && __ldcg(a.sat_ctr) >= a.limit) *a.cmp_n_out = 0;
         } else {
-            for (int i = threadIdx.x; i < n; i += blockDim.x) a.state[i] = __ldcg(a.state_new + i);
+            for (int i = threadIdx.x; i < sv.n; i += blockDim.x) a.state[i] = __ldcg(a.state_new + i);
+        }
+    }
+}
+
+// ------------------------------------------------------------------ one launch = the whole loop
+__device__ __forceinline__ int ld_acquire_gpu_s32(const int* p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_gpu_s32(int* p, int v) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// Grid barrier after decoding step k (k1 = k + 1 barriers completed once everybody is through).  The
+// last arriver has observed every finalisation of the step (acq_rel arrival chain), so it decides the
+// LIMIT stop there, once, for the whole grid, and publishes it with the go word.  Returns the go word's
+// flags: bit 0 = stop (LIMIT reached or abort).
+__device__ __forceinline__ int loop_barrier(const LoopArgs& L, int k1, const int* sat_ctr, int limit) {
+    __shared__ int s_go;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int old = atom_add_acq_rel_gpu(L.bar + 0, 1);
+        if (old == k1 * (int)gridDim.x - 1) {
+            const int stop = (sat_ctr && __ldcg(sat_ctr) >= limit) ? 1 : 0;
+            st_release_gpu_s32(L.bar + 1, k1 | (stop << 30));
+        }
+        int v;
+        const unsigned long long t0 = global_timer_ns();
+        while (((v = ld_acquire_gpu_s32(L.bar + 1)) & 0x3FFFFFFF) < k1) {
+            if (ld_acquire_gpu_s32(L.bar + 2) != 0) { v = k1 | (1 << 30); break; }
+            if (global_timer_ns() - t0 > LOOP_SPIN_TIMEOUT_NS) {  // never on a healthy device: fail, do not hang
+                atomicExch(L.bar + 2, 1);
+                v = k1 | (1 << 30);
+                break;
+            }
+        }
+        s_go = v;
+    }
+    __syncthreads();
+    return (s_go >> 30) & 1;
+}
+
+template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER, bool SAMPLE = false>
+__global__ void __launch_bounds__(WARPS * 32, 1) loop_kernel(const StepArgs a, const LoopArgs L) {
+    using Ring = WarpRing<STAGES, TILE_BYTES>;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    Ring& ring = reinterpret_cast<Ring*>(smem_raw)[warp];
+    const int nwords = (L.B + 31) >> 5;
+    uint32_t* s_bits = reinterpret_cast<uint32_t*>(smem_raw + sizeof(Ring) * WARPS);
+    int* s_pref = reinterpret_cast<int*>(s_bits + nwords);  // [nwords + 1]
+
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) mbar_init(smem_u32(&ring.bar[s]), 1);
+        fence_mbar_init();
+    }
+    __syncwarp();
+
+    const unsigned gen0 = (unsigned)__ldcg(a.ctrs + 3);
+    RingPos rp;
+    int k = 0;
+#pragma unroll 1
+    for (; k < a.max_steps; ++k) {
+        // ---- snapshot of the active-row bitmap -> shared memory, per-word prefix counts, n
+        const uint32_t* cur = L.alive[k % 3];
+        for (int w = threadIdx.x; w < nwords; w += WARPS * 32) s_bits[w] = __ldcg(cur + w);
+        __syncthreads();
+        if (warp == 0) {
+            int carry = 0;
+            for (int w0 = 0; w0 < nwords; w0 += 32) {
+                const int w = w0 + lane;
+                const int c = (w < nwords) ? __popc(s_bits[w]) : 0;
+                int inc = c;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int up = __shfl_up_sync(FULL, inc, o);
+                    if (lane >= o) inc += up;
+                }
+                if (w < nwords) s_pref[w] = carry + inc - c;
+                carry += __shfl_sync(FULL, inc, 31);
+            }
+            if (lane == 0) s_pref[nwords] = carry;
+        }
+        __syncthreads();
+        const int n = s_pref[nwords];
+        if (blockIdx.x == 0 && threadIdx.x == 0 && k < LOOP_TRACE_STEPS) {
+            L.trace_t[k] = global_timer_ns();
+            L.trace_n[k] = n;
+        }
+        if (blockIdx.x == 0 && threadIdx.x == 0) CD_PHASE(L, k, 0);  // snapshot done
+        if (n == 0) break;  // every CTA reads the same bitmap: uniform across the grid
+        // the bitmap read two steps from now was last read one step ago: clear it (nobody touches it
+        // before the next barrier)
+        if (blockIdx.x == 0) {
+            uint32_t* clr = L.alive[(k + 2) % 3];
+            for (int w = threadIdx.x; w < nwords; w += WARPS * 32) clr[w] = 0u;
+        }
+
+        StepView sv{};
+        sv.logits = static_cast<const unsigned char*>(L.step_ptrs_dev ? L.step_ptrs_dev[k] : L.step_ptrs[k]);
+        sv.state_cur = L.state2[k & 1];
+        sv.state_next = L.state2[(k + 1) & 1];
+        sv.work_ctr = L.work + k;
+        sv.gen = gen0 + (unsigned)k;
+        sv.n = n;
+        sv.step = k;
+        sv.alive_next = L.alive[(k + 1) % 3];
+        sv.s_bits = s_bits;
+        sv.s_pref = s_pref;
+        sv.nwords = nwords;
+#ifdef CD_TUNING
+        if (L.phase && k < LOOP_TRACE_STEPS) {
+            sv.ph_first_fin = L.phase + k * 8 + 2;
+            sv.ph_last_fin = L.phase + k * 8 + 3;
+            sv.ph_tile = L.phase + k * 8 + 5;
+        }
+#endif
+        step_body<DT, WARPS, STAGES, TILE_BYTES, GATHER, SAMPLE, true>(a, sv, ring, rp, warp, lane);
+        if (blockIdx.x == 0 && threadIdx.x == 0) CD_PHASE(L, k, 1);  // CTA 0 / warp 0 ran out of work
+#ifdef CD_TUNING
+        __syncthreads();
+        if (threadIdx.x == 0 && L.phase && k < LOOP_TRACE_STEPS) atomicMax(L.phase + k * 8 + 4, global_timer_ns());  // last CTA at the barrier
+#endif
+
+        if (loop_barrier(L, k + 1, a.sat_ctr, a.limit)) {
+            ++k;
+            break;
+        }
+    }
+    // ---------------- last CTA to leave: generation for the next launch, trace end
+    if (threadIdx.x == 0) {
+        const int d = atom_add_acq_rel_gpu(a.ctrs + 1, 1);
+        if (d == (int)gridDim.x - 1) {
+            a.ctrs[1] = 0;
+            a.ctrs[3] = (int)(gen0 + (unsigned)a.max_steps + 1u);
+            const int kk = k < LOOP_TRACE_STEPS ? k : LOOP_TRACE_STEPS;
+            L.trace_t[kk] = global_timer_ns();
+            L.trace_n[LOOP_TRACE_STEPS] = k;
         }
     }
 }

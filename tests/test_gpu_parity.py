@@ -8,6 +8,7 @@ accumulation, read as abs(gpu - ref) <= 1e-5 * max(1, |ref|) (SURVEY 8(c) G9:
 bound from the arithmetic).
 """
 import math
+import threading
 
 import numpy as np
 import pytest
@@ -322,10 +323,27 @@ def test_compaction_bit_exact(cd, oracle, n, pattern):
 
 # ------------------------------------------------------------------ the loop
 def check_loop(cd, oracle, aut, logits_dev, max_steps, ref=None, rows=None):
+    """cd_decode_loop against O4, in both loop modes: the persistent kernel (one cooperative launch for
+    the whole loop, bitmap-select instead of compaction) and one launch per decoding step.  The two must
+    agree bit for bit, fp32 sums included (same unit split, same merge order)."""
     dfa = dev_dfa(cd, aut)
+    dfa.set_loop_mode(cd.LOOP_PER_STEP)
+    per_step = cd.decode_loop(dfa, logits_dev, max_steps=max_steps)
+    assert dfa.loop_trace() == ([], [])
+    dfa.set_loop_mode(cd.LOOP_AUTO)
     out = cd.decode_loop(dfa, logits_dev, max_steps=max_steps)
+    for k in per_step:
+        assert torch.equal(per_step[k].view(torch.uint8) if per_step[k].dtype == torch.float32 else per_step[k],
+                           out[k].view(torch.uint8) if out[k].dtype == torch.float32 else out[k]), ("loop modes differ", k)
     if ref is None:
         ref = oracle.decode_loop(aut, [x.cpu() for x in logits_dev], max_steps=max_steps)
+    B = logits_dev[0].shape[0]
+    if B <= 32768 and not bool(aut.accepting[aut.start]) and rows is None and "n_active_hist" in ref:
+        # the persistent kernel ran, and its per-step active counts are the oracle's
+        n_tr, t_tr = dfa.loop_trace()
+        hist = [int(v) for v in ref["n_active_hist"] if v > 0]
+        assert n_tr == hist, (n_tr, hist)
+        assert all(t > 0 for t in t_tr)
     sel = slice(None) if rows is None else rows
     for k in ("tokens", "len", "final_state", "done"):
         assert np.array_equal(out[k].cpu().numpy()[sel], ref[k]), k
@@ -387,45 +405,145 @@ def test_loop_full_size_configs(cd, oracle, name):
             assert abs(hist[k] - expect) < 6 * math.sqrt(cfg.B) + 0.15 * expect
 
 
-def test_loop_c4_batch_sampled_rows(cd, oracle):
-    """BASELINE.json configs[4], one full batch (B=4096, S=4096, 16 steps, 32 GiB of
-    logits) in the launch configuration bench.py times.  The oracle checks a
-    sample of rows one by one (rows are independent: a row's result does not
-    depend on batch composition), plus size-independent
-    properties on every row."""
+C4_BATCHES = (0, 127, 255)  # "batches 0, 127, 255; all steps"
+
+
+@pytest.mark.parametrize("batch", C4_BATCHES)
+def test_loop_c4_every_row_of_three_batches(cd, oracle, step_mode, batch):
+    """BASELINE.json configs[4]: full batches (B = 4096, S = 4096, 16 steps, 32 GiB of logits each) in
+    the launch configuration bench.py times, EVERY row compared with the oracle: tokens, len,
+    final_state and done bit for bit, sum_logprob within 1e-5 * (len + |sum|).  The oracle is fed row
+    chunks of 512 rows x 16 steps (4 GiB of host memory at a time; rows are independent, PAPER.md
+    L106).  The three gather modes and the two loop modes all run on the same logits against one
+    oracle pass, so the test body runs once (under the autouse mode "dense")."""
+    if step_mode != "dense":
+        pytest.skip("the three gather modes are run inside the dense instance, on one set of logits")
     cfg = wl.CONFIGS["c4"]
     free, _ = torch.cuda.mem_get_info()
     if free < 40 * 2**30:
         pytest.skip("needs ~34 GiB of device memory")
     aut = wl.build_automaton(cfg, device="cuda:0")
-    logits = wl.build_step_logits(cfg, aut, device="cuda:0")
+    logits = wl.build_step_logits(cfg, aut, device="cuda:0", batch=batch)
+    # the oracle, chunk by chunk
+    ref = dict(tokens=[], len=[], final_state=[], done=[], sum_logprob=[])
+    for r0 in range(0, cfg.B, 512):
+        sub = [x[r0:r0 + 512].cpu() for x in logits]
+        part = oracle.decode_loop(aut, sub, max_steps=cfg.max_steps)
+        for k in ref:
+            ref[k].append(part[k])
+        del sub
+    ref = {k: np.concatenate(v) for k, v in ref.items()}
+    assert int(ref["len"].sum()) > 8 * cfg.B  # ~11 row-steps per row
+    for mode in ("dense", "gather_all", "gather_mixed"):
+        _MODE["name"] = mode
+        dfa = dev_dfa(cd, aut)
+        for lm in (cd.LOOP_AUTO, cd.LOOP_PER_STEP):
+            dfa.set_loop_mode(lm)
+            out = cd.decode_loop(dfa, logits, max_steps=cfg.max_steps)
+            for k in ("tokens", "len", "final_state", "done"):
+                assert np.array_equal(out[k].cpu().numpy(), ref[k]), (mode, lm, k)
+            slp = out["sum_logprob"].cpu().numpy().astype(np.float64)
+            bound = TOL * (ref["len"] + np.abs(ref["sum_logprob"]))
+            assert np.all(np.abs(slp - ref["sum_logprob"]) <= bound), (mode, lm)
+        dfa.close()
+    _MODE["name"] = "dense"
+    # properties that hold at any size (a second, independent look at the same outputs)
+    toks, ln, fs, dn = ref["tokens"], ref["len"], ref["final_state"], ref["done"]
+    acc = aut.accepting.numpy()
+    assert np.array_equal(dn, acc[fs]) and bool(np.all((ln == cfg.max_steps) | (dn == 1)))
+    assert bool(np.all((toks >= 0) == (np.arange(cfg.max_steps)[None, :] < ln[:, None])))
+
+
+def test_step_and_loop_are_bitwise_reproducible(cd, oracle, step_mode):
+    """Stand-in for racecheck (compute-sanitizer is closed on this pool): the fence-free, ticket-free
+    merge of the unit results (cd_step.cuh: tagged 64-bit slots polled by the warp that holds a row's
+    last part) and the grid barrier / bitmap rotation of the persistent loop must give IDENTICAL BITS on
+    every run.  The same c4-shaped cd_step and cd_decode_loop are run 200 times at n in {8, 148, 1024,
+    4096}, on two streams at once (two grids sharing the SMs: the merge waits only for units that were
+    drawn earlier, so partial residency must not deadlock it), and compared with the first run."""
+    cfg = wl.CONFIGS["c4"]
+    free, _ = torch.cuda.mem_get_info()
+    if free < 12 * 2**30:
+        pytest.skip("needs ~10 GiB of device memory")
+    aut = wl.build_automaton(cfg, device="cuda:0")
     dfa = dev_dfa(cd, aut)
-    out = cd.decode_loop(dfa, logits, max_steps=cfg.max_steps)
-    toks, ln = out["tokens"].cpu().numpy(), out["len"].cpu().numpy()
-    fs, dn = out["final_state"].cpu().numpy(), out["done"].cpu().numpy()
-    slp = out["sum_logprob"].cpu().numpy().astype(np.float64)
-    # properties on every row: replay through the host CSR
-    rp, tk, nx, acc = aut.row_ptr.numpy(), aut.tok.numpy(), aut.next.numpy(), aut.accepting.numpy()
-    for r in range(cfg.B):
-        s = aut.start
-        for k in range(ln[r]):
-            assert not acc[s]
-            lo, hi = rp[s], rp[s + 1]
-            j = lo + np.searchsorted(tk[lo:hi], toks[r, k])
-            assert j < hi and tk[j] == toks[r, k]  # chosen token always allowed
-            s = nx[j]
-        assert fs[r] == s and dn[r] == acc[s]
-        assert (ln[r] == cfg.max_steps) or acc[s]
-        assert (toks[r, ln[r]:] == -1).all() and slp[r] <= 0
-    # sampled rows, one by one
-    rows = sorted(set(np.random.default_rng(4).choice(cfg.B, size=96, replace=False).tolist()) | {0, cfg.B - 1})
-    sub = [x[rows].cpu() for x in logits]
-    ref = oracle.decode_loop(aut, sub, max_steps=cfg.max_steps)
-    assert np.array_equal(toks[rows], ref["tokens"])
-    assert np.array_equal(ln[rows], ref["len"]) and np.array_equal(fs[rows], ref["final_state"])
-    assert np.array_equal(dn[rows], ref["done"])
-    bound = TOL * (ref["len"] + np.abs(ref["sum_logprob"]))
-    assert np.all(np.abs(slp[rows] - ref["sum_logprob"]) <= bound)
+    xs = [wl.make_logits(cfg.seed, k, cfg.B, cfg.V, cfg.std, cfg.dtype, device="cuda:0") for k in range(2)]
+    live = live_states(aut, cfg.B)
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    reps = 200
+    for n in (8, 148, 1024, 4096):
+        st0 = torch.tensor(live[:n], dtype=torch.int32, device="cuda:0")
+        steps = [xs[k & 1][:n] for k in range(cfg.max_steps)]
+        first_step, first_loop = None, None
+        torch.cuda.synchronize()
+        for rep in range(0, reps, 2):
+            got = []
+            for si, stream in enumerate(streams):
+                with torch.cuda.stream(stream):
+                    st = st0.clone()
+                    tok, lp, lse, done = cd.step(dfa, xs[0], st, n=n)
+                    got.append((tok, lp, lse, done, st))
+            # the loops synchronise their stream before returning: two host threads keep both streams busy
+            loops = [None, None]
+
+            def run_loop(si):
+                with torch.cuda.stream(streams[si]):
+                    loops[si] = cd.decode_loop(dfa, steps)
+
+            dfa.set_loop_mode(cd.LOOP_AUTO if (rep // 2) % 2 == 0 else cd.LOOP_PER_STEP)
+            threads = [threading.Thread(target=run_loop, args=(si,)) for si in range(2)]
+            for t in threads:
+                t.start()
+            for t in threads:
+                t.join()
+            torch.cuda.synchronize()
+            for g in got:
+                cur = [t.view(torch.uint8) if t.dtype == torch.float32 else t for t in g]
+                if first_step is None:
+                    first_step = [t.clone() for t in cur]
+                for a, b in zip(first_step, cur):
+                    assert torch.equal(a, b), ("cd_step not reproducible", n, rep)
+            for lo in loops:
+                cur = {k: (v.view(torch.uint8) if v.dtype == torch.float32 else v) for k, v in lo.items()}
+                if first_loop is None:
+                    first_loop = {k: v.clone() for k, v in cur.items()}
+                for k in cur:
+                    assert torch.equal(first_loop[k], cur[k]), ("cd_decode_loop not reproducible", n, rep, k)
+        # and the first run is right (8 and 148 rows: the oracle in full; larger n: the first 256 rows)
+        m = min(n, 256)
+        o_tok, o_lp, o_lse, o_done, o_st = oracle.step(aut, xs[0][:m].cpu(), live[:m])
+        assert first_step[0][:m].cpu().numpy().tolist() == o_tok.tolist()
+        assert first_step[4][:m].cpu().numpy().tolist() == o_st.tolist()
+        want = oracle.decode_loop(aut, [x[:m].cpu() for x in steps])
+        assert np.array_equal(first_loop["tokens"][:m].cpu().numpy(), want["tokens"])
+    dfa.set_loop_mode(cd.LOOP_AUTO)
+    dfa.close()
+
+
+def test_bad_state_is_reported_through_the_outputs_and_does_not_stick(cd, oracle):
+    """A slot whose state is outside [0, S): cd_step cannot fail asynchronously, it reports the slot as
+    done with token -1 and keeps the state; the error counter of the scratch area must not leak into the
+    NEXT loop on the stream, which is clean and must return CD_OK (round-1 advice)."""
+    cfg = wl.scaled(wl.CONFIGS["c3"], V=20000, B=64, S=32, max_steps=4)
+    aut = wl.build_automaton(cfg)
+    dfa = dev_dfa(cd, aut)
+    logits = wl.build_step_logits(cfg, aut, device="cuda:0")
+    live = live_states(aut, cfg.B)
+    states = list(live)
+    states[3], states[17], states[40] = aut.S, -1, aut.S + 1000
+    st = torch.tensor(states, dtype=torch.int32, device="cuda:0")
+    tok, lp, lse, done = cd.step(dfa, logits[0], st)
+    torch.cuda.synchronize()
+    good = [i for i in range(cfg.B) if i not in (3, 17, 40)]
+    o_tok, o_lp, o_lse, o_done, o_st = oracle.step(aut, logits[0].cpu(), [states[i] for i in good], row_map=good)
+    assert tok.cpu().numpy()[good].tolist() == o_tok.tolist() and st.cpu().numpy()[good].tolist() == o_st.tolist()
+    for i in (3, 17, 40):
+        assert int(tok[i]) == -1 and int(done[i]) == 1 and int(st[i]) == states[i] and float(lp[i]) == 0.0
+    for lm in (cd.LOOP_AUTO, cd.LOOP_PER_STEP):  # the following loops are clean: CD_OK, right results
+        dfa.set_loop_mode(lm)
+        out = cd.decode_loop(dfa, logits)
+        want = oracle.decode_loop(aut, [x.cpu() for x in logits])
+        assert np.array_equal(out["tokens"].cpu().numpy(), want["tokens"])
     dfa.close()
 
 

@@ -255,17 +255,23 @@ def make_logits(
     batch: int = 0,
     ld: Optional[int] = None,
     rows_per_chunk: int = 512,
+    rows: Optional[Tuple[int, int]] = None,
 ) -> torch.Tensor:
     """One step's logits [B, ld] (ld >= V, default V): round_to_dtype(N(0, std)
     [+ bias on bias_tokens, added before rounding]).  'N(0,2)' in BASELINE.json
     is read as standard deviation 2.  The generator is
-    re-seeded per (seed, batch, step) so any step can be produced on its own."""
+    re-seeded per (seed, batch, step) so any step can be produced on its own.
+    rows = (lo, hi): only rows [lo, hi) of the batch are kept ([hi - lo, ld]); every
+    chunk is still drawn, so the kept rows are byte-identical to those of the whole
+    batch (a rank's shard of a batch)."""
     ld = V if ld is None else ld
     assert ld >= V
+    lo, hi = (0, B) if rows is None else rows
+    assert 0 <= lo <= hi <= B
     dev = torch.device(device)
     g = torch.Generator(device=dev)
     g.manual_seed((seed * 1000003 + batch * 4099 + step) & 0x7FFFFFFFFFFFFFFF)
-    out = torch.empty((B, ld), dtype=dtype, device=dev)
+    out = torch.empty((hi - lo, ld), dtype=dtype, device=dev)
     if ld > V:
         out[:, V:] = 0
     bt = None
@@ -273,11 +279,16 @@ def make_logits(
         bt = torch.tensor(sorted(set(int(t) for t in bias_tokens)), dtype=torch.int64, device=dev)
     for r0 in range(0, B, rows_per_chunk):
         r1 = min(B, r0 + rows_per_chunk)
+        if r0 >= hi:
+            break
         x = torch.randn((r1 - r0, V), generator=g, dtype=torch.float32, device=dev)
-        x.mul_(std)
-        if bt is not None:
-            x[:, bt] += bias
-        out[r0:r1, :V] = x.to(dtype)
+        a, b = max(r0, lo), min(r1, hi)
+        if a < b:
+            x = x[a - r0:b - r0]
+            x.mul_(std)
+            if bt is not None:
+                x[:, bt] += bias
+            out[a - lo:b - lo, :V] = x.to(dtype)
         del x
     return out
 
@@ -368,15 +379,16 @@ def bias_tokens_of(cfg: Config, aut: Automaton) -> List[int]:
 
 def build_step_logits(
     cfg: Config, aut: Automaton, device: str = "cpu", batch: int = 0,
-    steps: Optional[int] = None, B: Optional[int] = None,
+    steps: Optional[int] = None, B: Optional[int] = None, rows: Optional[Tuple[int, int]] = None,
 ) -> List[torch.Tensor]:
-    """The list step_logits[k] ([B, V], indexed by ORIGINAL row id) of one batch."""
+    """The list step_logits[k] ([B, V], indexed by ORIGINAL row id) of one batch (rows = (lo, hi): that
+    shard of it, see make_logits)."""
     steps = cfg.max_steps if steps is None else steps
     B = cfg.B if B is None else B
     bt = bias_tokens_of(cfg, aut)
     return [
         make_logits(cfg.seed, k, B, cfg.V, cfg.std, cfg.dtype, device=device,
-                    bias_tokens=bt, bias=cfg.bias, batch=batch)
+                    bias_tokens=bt, bias=cfg.bias, batch=batch, rows=rows)
         for k in range(steps)
     ]
 
