@@ -80,8 +80,9 @@ def parse_args():
                     help="weak: every rank decodes its own batches (default); strong: ONE batch of B rows is "
                          "sharded B/N rows per rank (SURVEY 8(e): contiguous row ranges, no collective)")
     ap.add_argument("--no-per-config", action="store_true", help="skip the c1-c3 block (per_config)")
-    ap.add_argument("--loop-mode", default="auto", choices=["auto", "per_step"],
-                    help="auto: cd_decode_loop as ONE persistent kernel (default); per_step: one launch per decoding step")
+    ap.add_argument("--loop-mode", default="auto", choices=["auto", "barrier", "per_step"],
+                    help="auto: cd_decode_loop as ONE persistent kernel, row groups advancing independently (default); "
+                         "barrier: the lock-step persistent kernel; per_step: one launch per decoding step")
     return ap.parse_args()
 
 
@@ -435,7 +436,7 @@ def measure_loop(cd, cfg, aut, dfa, batches, device, steps, warmup, peak, verbos
         kern_us = sum(us)
         k0 = max(range(len(us)), key=lambda k: last["bytes"][k])
         res.update({
-            "kernel": "cd::loop_kernel (one cooperative launch per loop)",
+            "kernel": "cd::flow_kernel (one launch per loop; row groups advance independently, no grid barrier)",
             "kernel_us_per_loop": kern_us,
             "kernel_gbs": sum(last["bytes"]) / (kern_us * 1e-6) / 1e9,
             "kernel_frac_of_measured_peak": sum(last["bytes"]) / (kern_us * 1e-6) / 1e9 / peak,
@@ -445,7 +446,9 @@ def measure_loop(cd, cfg, aut, dfa, batches, device, steps, warmup, peak, verbos
             "us_per_step": [round(u, 2) for u in us],
             "gbs_per_step": [round(g, 0) for g in gbs],
             "fixed_us_per_step_avg": sum(fixed) / len(fixed),
-            "fixed_cost_note": f"step time minus its bytes at the kernel's pure-read rate ({READ_RATE_GBS:.0f} GB/s)",
+            "fixed_cost_note": f"step time minus its bytes at the kernel's pure-read rate ({READ_RATE_GBS:.0f} GB/s); with row "
+                               "groups a step lasts from the publication of its last group to that of the next step's, so "
+                               "the first step carries the pipeline fill and single steps can come out below their byte time",
         })
         if verbose:
             for k, (n, u, g, f) in enumerate(zip(last["n"], us, gbs, fixed)):
@@ -468,11 +471,17 @@ def per_config_section(cd, device, peak, verbose):
         dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device=device)
         dfa.reserve(cfg.B)
         res, _, _ = measure_loop(cd, cfg, aut, dfa, batches, device, k, 5, peak, verbose=verbose, label=name)
-        # the same loops as one launch per decoding step (the round-1 path; still what the callback / host forms use)
+        # the same loops as one launch per decoding step (the round-1 structure; still what the callback / host
+        # forms use) and in the lock-step persistent kernel (grid barrier per step; what a LIMIT loop runs in)
         dfa.set_loop_mode(cd.LOOP_PER_STEP)
         ps, _, _ = measure_loop(cd, cfg, aut, dfa, batches, device, k, 5, peak)
         res["per_step_launches"] = {"rows_per_s": ps["rows_per_s"], "ms_per_loop": ps["ms_per_loop"], "loop_gbs": ps["loop_gbs"],
                                     "frac_of_measured_peak": ps["frac_of_measured_peak"]}
+        dfa.set_loop_mode(cd.LOOP_BARRIER)
+        lb, _, _ = measure_loop(cd, cfg, aut, dfa, batches, device, k, 5, peak)
+        res["lock_step_kernel"] = {"rows_per_s": lb["rows_per_s"], "ms_per_loop": lb["ms_per_loop"],
+                                   "kernel_us_per_loop": lb.get("kernel_us_per_loop"), "kernel_gbs": lb.get("kernel_gbs"),
+                                   "us_per_step": lb.get("us_per_step"), "fixed_us_per_step_avg": lb.get("fixed_us_per_step_avg")}
         dfa.set_loop_mode(cd.LOOP_AUTO)
         # density-adaptive (tries never need the scan)
         dfa.set_gather_max(-1)
@@ -576,7 +585,7 @@ def main():
     dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device=device)
     dfa.reserve(cfg.B)
     dfa.set_gather_max(args.gather_max)
-    dfa.set_loop_mode(cd.LOOP_AUTO if args.loop_mode == "auto" else cd.LOOP_PER_STEP)
+    dfa.set_loop_mode({"auto": cd.LOOP_AUTO, "barrier": cd.LOOP_BARRIER, "per_step": cd.LOOP_PER_STEP}[args.loop_mode])
     out = None
 
     def one_step(i):
@@ -639,12 +648,13 @@ def main():
         read_probe = None
     achieved = bytes_timed / (ms * 1e-3) / 1e9
     persistent = bool(tr_n) and tr_n == per_batch[timed[-1]]["n"]
-    kname = "cd::loop_kernel" if persistent else "cd::step_kernel"
+    kname = ("cd::flow_kernel" if args.loop_mode == "auto" else "cd::loop_kernel") if persistent else "cd::step_kernel"
     tinfo = ncu_traffic(kname, cfg.name)
     roofline = {
         "bound": "hbm",
-        "kernel": ("cd::loop_kernel (persistent: the whole decode loop in one cooperative launch; per step: fused mask + "
-                   "masked logsumexp/argmax + transition, grid barrier)") if persistent else
+        "kernel": (kname + " (persistent: the whole decode loop in one launch; per row and step: fused mask read + masked "
+                   "logsumexp/argmax + transition; " + ("row groups advance independently, no barrier)" if args.loop_mode == "auto"
+                                                        else "grid barrier between steps)")) if persistent else
                   "cd::step_kernel (fused mask + masked logsumexp/argmax + CSR transition), one launch per decoding step",
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
         "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,

@@ -270,24 +270,34 @@ CD_API cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, cons
  * If the start state is accepting every row is done with len 0.
  *
  * How it runs (cd_set_loop_mode):
- *   CD_LOOP_AUTO (default)  ONE cooperative kernel launch for the whole loop when the
- *       device supports it and B <= 32768: the CTAs stay resident, meet at a grid barrier
- *       after every decoding step and read step_logits[k] themselves; the active set is a
- *       bitmap over original row ids (slot i of a step = its i-th set bit, i.e. the stable
- *       order of cd_compact) -- no launch, no counter reset and no compaction pass between
- *       steps.  cd_decode_loop and cd_decode_loop_limit take this path; otherwise, and for
- *       the host-buffer and callback forms (whose step inputs appear between steps), the
- *       loop is one cd_step-like launch per decoding step with the compaction fused into
- *       the step kernel's last CTA.
+ *   CD_LOOP_AUTO (default)  ONE kernel launch for the whole loop when the device supports it and
+ *       B <= 32768; the CTAs stay resident and read step_logits[k] themselves.
+ *       - cd_decode_loop: the rows are split into (up to 4) groups of consecutive row ids and every
+ *         group is a decode loop of its own: the warp that finalises the last row of a group's step
+ *         builds the group's next active list (ascending row id, i.e. the stable order of
+ *         cd_compact) and publishes the step; every warp draws work from whichever group has a
+ *         published step with units left, oldest step first.  While one group is between two steps
+ *         the others keep the memory system busy: no launch, no counter reset, no compaction pass
+ *         and no grid-wide barrier between steps.
+ *       - cd_decode_loop_limit (and cd_set_limit): a LIMIT is defined step by step over ALL rows, so
+ *         the steps run in lock-step: one cooperative launch, a grid barrier after every step, the
+ *         active set a bitmap over original row ids (slot i of a step = its i-th set bit).
+ *       Otherwise, and for the host-buffer and callback forms (whose step inputs appear between
+ *       steps), the loop is one cd_step-like launch per decoding step with the compaction fused
+ *       into the step kernel's last CTA.
+ *   CD_LOOP_BARRIER         the lock-step persistent kernel also without a LIMIT.
  *   CD_LOOP_PER_STEP        always one launch per decoding step.
- * Both give the same results bit for bit (token, state, done, len) and the same fp32
- * sums.  cd_loop_trace returns, for the last loop that ran in the persistent kernel on
- * (dfa, cuda_stream), the number of decoding steps it ran (*steps_out), and for the first
- * min(cap, 256) of them the active rows and the duration in nanoseconds measured on the
- * device (HOST arrays; *steps_out = 0 if that loop took the per-step path).  It
- * synchronises the stream.
+ * All three give the same tokens, lengths, states and done flags bit for bit; sum_logprob_out is
+ * bit-identical between CD_LOOP_BARRIER and CD_LOOP_PER_STEP and within the stated tolerance for
+ * CD_LOOP_AUTO (rows are split into work units per group, which changes the fp32 summation
+ * order); each mode by itself is bitwise reproducible from run to run.
+ * cd_loop_trace returns, for the last loop that ran in a persistent kernel on (dfa, cuda_stream),
+ * the number of decoding steps it ran (*steps_out), and for the first min(cap, 256) of them the
+ * active rows and the duration in nanoseconds measured on the device (HOST arrays; with row groups
+ * step k lasts from the moment its last group was published to the moment step k + 1's was;
+ * *steps_out = 0 if that loop took the per-step path).  It synchronises the stream.
  */
-typedef enum { CD_LOOP_AUTO = 0, CD_LOOP_PER_STEP = 1 } cd_loop_mode;
+typedef enum { CD_LOOP_AUTO = 0, CD_LOOP_PER_STEP = 1, CD_LOOP_BARRIER = 2 } cd_loop_mode;
 CD_API cd_status cd_set_loop_mode(cd_dfa_t* dfa, int32_t mode);
 CD_API cd_status cd_loop_trace(const cd_dfa_t* dfa, void* cuda_stream, int32_t cap, int64_t* t_ns_out,
                         int32_t* n_active_out, int32_t* steps_out);

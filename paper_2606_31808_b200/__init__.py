@@ -10,6 +10,7 @@ from .binding import (  # noqa: F401
     BF16,
     F32,
     LOOP_AUTO,
+    LOOP_BARRIER,
     LOOP_PER_STEP,
     build_trie,
     CdError,

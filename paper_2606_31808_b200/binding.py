@@ -12,7 +12,7 @@ _SO = os.path.join(HERE, "libcd.so")
 _lib = None
 
 F32, BF16 = 0, 1
-LOOP_AUTO, LOOP_PER_STEP = 0, 1
+LOOP_AUTO, LOOP_PER_STEP, LOOP_BARRIER = 0, 1, 2
 STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_STATE",
           4: "CD_ERR_CUDA", 5: "CD_ERR_OOM", 6: "CD_ERR_INTERNAL"}
 
@@ -116,7 +116,9 @@ class Dfa:
         _check(lib().cd_set_head_gather_max(self._h, C.c_int32(max_transitions)))
 
     def set_loop_mode(self, mode: int):
-        """cd_set_loop_mode: LOOP_AUTO (one persistent kernel per decode loop when possible) or LOOP_PER_STEP."""
+        """cd_set_loop_mode: LOOP_AUTO (one persistent kernel per decode loop when possible: row groups that advance
+        independently, or the lock-step kernel when a LIMIT is set), LOOP_BARRIER (the lock-step persistent kernel)
+        or LOOP_PER_STEP (one launch per decoding step)."""
         _check(lib().cd_set_loop_mode(self._h, C.c_int32(mode)))
 
     def loop_trace(self, cap: int = 256):

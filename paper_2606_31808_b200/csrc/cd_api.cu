@@ -84,6 +84,8 @@ constexpr int tune_int(const char*, int def, int, int) { return def; }
 int units_per_warp() { static const int v = tune_int("CD_UPW", cd::UNITS_PER_WARP, 1, 32); return v; }
 int tpu_max_tiles() { static const int v = tune_int("CD_TPU_MAX", cd::TPU_MAX_BYTES / STEP_TILE, 1, cd::TPU_MAX_BYTES / STEP_TILE); return v; }
 bool use_pdl() { static const int v = tune_int("CD_PDL", 1, 0, 1); return v != 0; }
+int flow_idle_ns() { static const int v = tune_int("CD_IDLE_NS", 32, 0, 100000); return v; }  // 32 / 128 / 512 ns: 648 / 660 / 675 us per c3 loop
+int flow_groups_target() { static const int v = tune_int("CD_GROUPS", 4, 1, cd::FLOW_MAX_GROUPS); return v; }
 int host_gather_mult() { static const int v = tune_int("CD_HOST_GATHER_CTAS", 4, 1, 64); return v; }  // flat from 2 to 32 (51 GB/s on PCIe Gen5 x16)
 
 // Per (handle, stream) scratch.  Operations on one stream are ordered, so one area per stream
@@ -109,6 +111,13 @@ struct StepBufs {  // sized by rows; replaced as a whole when the area grows
     unsigned long long* trace_t = nullptr;              // [LOOP_TRACE_STEPS + 1]
     int* trace_n = nullptr;                             // [LOOP_TRACE_STEPS + 1]
     unsigned long long* phase = nullptr;                // tuning builds: [LOOP_TRACE_STEPS][8]
+    // flow_kernel (row groups advancing independently)
+    unsigned long long* f_desc = nullptr;                // [FLOW_MAX_GROUPS]
+    unsigned long long* f_list[2] = {nullptr, nullptr};  // [rows + pad]
+    unsigned int* f_listf[2] = {nullptr, nullptr};
+    unsigned long long* f_res = nullptr;
+    unsigned long long* f_resf = nullptr;
+    int* f_fin = nullptr;                                // [FLOW_MAX_GROUPS]
 
     void release() {
         cudaFree(partials); cudaFree(tickets); cudaFree(ctrs);
@@ -116,6 +125,8 @@ struct StepBufs {  // sized by rows; replaced as a whole when the area grows
         for (int i = 0; i < 3; ++i) cudaFree(alive[i]);
         cudaFree(state_new); cudaFree(n_active); cudaFree(token); cudaFree(logprob); cudaFree(done);
         cudaFree(bar); cudaFree(trace_t); cudaFree(trace_n); cudaFree(phase);
+        cudaFree(f_desc); cudaFree(f_res); cudaFree(f_resf); cudaFree(f_fin);
+        for (int i = 0; i < 2; ++i) { cudaFree(f_list[i]); cudaFree(f_listf[i]); }
         *this = StepBufs();
     }
 };
@@ -183,7 +194,7 @@ struct Settings {
     int limit = 0;             // cd_set_limit: LIMIT early exit applied by every loop entry point
     int* limit_ctr = nullptr;  //   device counter of satisfied rows (caller-owned); nullptr = no limit
     bool has_satisfying = false;  // cd_set_satisfying was called with a set
-    int loop_mode = CD_LOOP_AUTO;  // cd_set_loop_mode
+    int loop_mode = CD_LOOP_AUTO;  // cd_set_loop_mode: AUTO / PER_STEP / BARRIER
 };
 
 }  // namespace
@@ -271,6 +282,15 @@ long long step_units_cap(const cd_dfa* d, long long n) {
     return (a > b ? a : b) + 64;
 }
 
+// flow_kernel: B rows as G groups of Bg consecutive rows (Bg a multiple of 32)
+void flow_plan(int B, int* G, int* Bg) {
+    const int gt = flow_groups_target();
+    int bg = ((B + gt - 1) / gt + 31) / 32 * 32;
+    if (bg < 32) bg = 32;
+    *Bg = bg;
+    *G = (B + bg - 1) / bg;
+}
+
 template <typename T>
 cudaError_t dev_alloc(T** p, size_t count) {
     return cudaMalloc(reinterpret_cast<void**>(p), sizeof(T) * (count ? count : 1));
@@ -279,8 +299,15 @@ cudaError_t dev_alloc(T** p, size_t count) {
 // Allocates a complete set of step buffers for `rows` rows; on failure nothing is kept.
 cd_status alloc_step_bufs(const cd_dfa* d, int rows, StepBufs* out) {
     StepBufs n;
-    const long long units = step_units_cap(d, rows);
+    long long units = step_units_cap(d, rows);
+    {   // flow_kernel: every group has a region of its own in the partial buffer
+        int G = 1, Bg = rows;
+        flow_plan(rows, &G, &Bg);
+        const long long fu = (long long)G * step_units_cap(d, Bg);
+        if (fu > units) units = fu;
+    }
     const size_t nwords = ((size_t)rows + 31) / 32;
+    const size_t frows = (size_t)rows + 32 * cd::FLOW_MAX_GROUPS;
     cudaError_t e = cudaSuccess;
     auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
     A(dev_alloc(&n.partials, (size_t)units));
@@ -300,6 +327,16 @@ cd_status alloc_step_bufs(const cd_dfa* d, int rows, StepBufs* out) {
     A(dev_alloc(&n.bar, 4));
     A(dev_alloc(&n.trace_t, (size_t)cd::LOOP_TRACE_STEPS + 1));
     A(dev_alloc(&n.trace_n, (size_t)cd::LOOP_TRACE_STEPS + 1));
+    A(dev_alloc(&n.f_desc, (size_t)cd::FLOW_MAX_GROUPS));
+    A(dev_alloc(&n.f_fin, (size_t)cd::FLOW_MAX_GROUPS));
+    A(dev_alloc(&n.f_res, frows));
+    A(dev_alloc(&n.f_resf, frows));
+    for (int i = 0; i < 2; ++i) {
+        A(dev_alloc(&n.f_list[i], frows));
+        A(dev_alloc(&n.f_listf[i], frows));
+    }
+    if (e == cudaSuccess) e = cudaMemset(n.f_res, 0, sizeof(unsigned long long) * frows);   // tags start at 0
+    if (e == cudaSuccess) e = cudaMemset(n.f_resf, 0, sizeof(unsigned long long) * frows);
 #ifdef CD_TUNING
     A(dev_alloc(&n.phase, (size_t)cd::LOOP_TRACE_STEPS * 8));
 #endif
@@ -328,6 +365,9 @@ cd_status get_scratch(const cd_dfa* cd_, cudaStream_t stream, int rows, Scratch*
         return fail(CD_ERR_ARG, "rows (%d) * tiles per row overflows the unit index", rows);
     Scratch& s = d->scratch[stream];
     if (rows < 1) rows = 1;
+    // (the group plan of flow_kernel depends on the row count of the CALL, the partial buffer is sized for the
+    // capacity: a smaller call never needs more units per group than the capacity's plan provides -- see
+    // alloc_step_bufs; calls are checked against cap_units when they are launched)
     if (s.b.cap_rows < rows) {
         // growing: the new set is complete before the old one is touched; then wait for the work that
         // still uses the old buffers and drop them
@@ -470,6 +510,34 @@ cd_status launch_loop_v(const cd::StepArgs& a, const cd::LoopArgs& L, int grid, 
     return launch_loop_t<DT>(a, L, grid, stream, fits);
 }
 
+// Persistent loop without a barrier (flow_kernel): a plain launch -- no warp of it ever waits for a warp that
+// is not running, so it needs no co-residency guarantee.
+template <int DT, bool GATHER = false, bool SAMPLE = false>
+cd_status launch_flow_t(const cd::StepArgs& a, const cd::FlowArgs& F, int grid, cudaStream_t stream) {
+    auto kern = cd::flow_kernel<DT, STEP_WARPS, STEP_STAGES, STEP_TILE, GATHER, SAMPLE>;
+    const size_t smem = sizeof(StepRing) * STEP_WARPS;
+    static thread_local int configured_dev = -1;
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    if (configured_dev != dev) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        configured_dev = dev;
+    }
+    kern<<<grid, STEP_WARPS * 32, smem, stream>>>(a, F);
+    CU(cudaGetLastError());
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return CD_OK;
+}
+
+template <int DT>
+cd_status launch_flow_v(const cd::StepArgs& a, const cd::FlowArgs& F, int grid, cudaStream_t stream) {
+    if (a.inv_tau > 0.0f)
+        return a.gather_max > 0 ? launch_flow_t<DT, true, true>(a, F, grid, stream)
+                                : launch_flow_t<DT, false, true>(a, F, grid, stream);
+    if (a.gather_max > 0) return launch_flow_t<DT, true>(a, F, grid, stream);
+    return launch_flow_t<DT>(a, F, grid, stream);
+}
+
 // Decode-loop extras of a step launch: per-row history + fused compaction (cd_step.cuh).
 struct LoopExtras {
     int* tokens = nullptr;
@@ -517,6 +585,7 @@ cd::StepArgs make_step_args(const cd_dfa* d, const Settings& cfg, Scratch* s, cd
     a.all_gather = (d->max_deg <= a.gather_max) ? 1 : 0;
     a.upw = units_per_warp();
     a.tpu_max = tpu_max_tiles();
+    a.idle_ns = flow_idle_ns();
     a.inv_tau = cfg.inv_tau;
     a.seed_lo = (uint32_t)(cfg.seed & 0xFFFFFFFFull);
     a.seed_hi = (uint32_t)(cfg.seed >> 32);
@@ -706,7 +775,8 @@ LimitArgs resolve_limit(const Settings& cfg, const LimitArgs& explicit_lim = Lim
 // persist: also initialise the bitmaps / states / counters of loop_kernel
 cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, int* tokens_out, int* len_out,
                            int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream,
-                           const LimitArgs& lim = LimitArgs(), bool persist = false) {
+                           const LimitArgs& lim = LimitArgs(), int persist = 0 /*0 per step, 1 loop_kernel, 2 flow_kernel*/,
+                           int grid = 0, int dtype = CD_BF16) {
     long long work = (long long)B * (max_steps > 0 ? max_steps : 1);
     long long blocks = (work + 255) / 256;
     if (blocks < 1) blocks = 1;
@@ -724,11 +794,28 @@ cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, in
     a.sat_ctr = lim.sat_ctr;
     a.limit = lim.limit;
     a.ctrs = s->b.ctrs;
-    if (persist) {
+    if (persist == 1) {
         for (int i = 0; i < 3; ++i) a.alive[i] = s->b.alive[i];
         for (int i = 0; i < 2; ++i) a.state2[i] = s->b.state2[i];
         a.work = s->loop_work;
         a.bar = s->b.bar;
+    } else if (persist == 2) {
+        flow_plan(B, &a.G, &a.Bg);
+        a.work = s->loop_work;
+        a.work_len = a.G * max_steps;
+        a.desc = s->b.f_desc;
+        a.list0 = s->b.f_list[0];
+        a.listf0 = s->b.f_listf[0];
+        a.fin = s->b.f_fin;
+        a.trace_t = s->b.trace_t;
+        a.trace_n = s->b.trace_n;
+        a.trace_len = cd::LOOP_TRACE_STEPS + 1;
+        const int T = tiles_per_row(d->dev.V, dtype);
+        for (int g = 0; g < a.G; ++g) {
+            const int ng = (g + 1) * a.Bg <= B ? a.Bg : B - g * a.Bg;
+            // unit size as if all G groups had this many rows: the groups share the warps
+            a.tpu0[g] = cd::tiles_per_unit((long long)ng * a.G, T, (long long)grid * STEP_WARPS, tpu_max_tiles(), units_per_warp());
+        }
     } else {
         a.row_ids = s->b.row_ids[0];
         a.state = s->b.state[0];
@@ -818,6 +905,49 @@ cd_status enqueue_persistent_loop(const cd_dfa* d, const Settings& cfg, Scratch*
     return st;
 }
 
+// The whole loop in ONE launch of flow_kernel (no LIMIT: a LIMIT is defined step by step over all rows, which
+// needs the lock-step of loop_kernel).
+cd_status enqueue_flow_loop(const cd_dfa* d, const Settings& cfg, Scratch* s, const void* const* step_logits,
+                            cd_dtype dtype, long long ld, int B, int max_steps, int* tokens_out, int* len_out,
+                            int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream, int grid) {
+    RangeGuard range("cd decode loop (persistent kernel, row groups)");
+    LoopExtras x;
+    x.tokens = tokens_out;
+    x.len = len_out;
+    x.final_state = final_state_out;
+    x.sum_logprob = sum_logprob_out;
+    x.done = done_out;
+    x.max_steps = max_steps;
+    cd::StepArgs a = make_step_args(d, cfg, s, dtype, ld, &x);
+    a.n = B;
+    cd::FlowArgs F{};
+    if (max_steps <= cd::LOOP_PARAM_STEPS) {
+        for (int k = 0; k < max_steps; ++k) F.step_ptrs[k] = step_logits[k];
+    } else {
+        CU(cudaMemcpyAsync(s->loop_ptrs, step_logits, sizeof(void*) * (size_t)max_steps, cudaMemcpyHostToDevice, stream));
+        F.step_ptrs_dev = s->loop_ptrs;
+    }
+    F.B = B;
+    flow_plan(B, &F.G, &F.Bg);
+    F.desc = s->b.f_desc;
+    for (int i = 0; i < 2; ++i) {
+        F.list[i] = s->b.f_list[i];
+        F.listf[i] = s->b.f_listf[i];
+    }
+    F.res = s->b.f_res;
+    F.resf = s->b.f_resf;
+    F.fin = s->b.f_fin;
+    F.work = s->loop_work;
+    F.pcap = step_units_cap(d, F.Bg);
+    F.trace_t = s->b.trace_t;
+    F.trace_n = s->b.trace_n;
+    if ((long long)F.G * F.pcap > s->b.cap_units) return fail(CD_ERR_INTERNAL, "partial buffer too small for %d groups", F.G);
+    const cd_status st = dtype == CD_BF16 ? launch_flow_v<cd::DT_BF16>(a, F, grid, stream)
+                                          : launch_flow_v<cd::DT_F32>(a, F, grid, stream);
+    if (st == CD_OK) s->trace_valid = true;
+    return st;
+}
+
 std::mutex& coop_mutex(int dev) {
     static std::mutex mu[64];
     return mu[dev & 63];
@@ -826,7 +956,7 @@ std::mutex& coop_mutex(int dev) {
 // can this loop run in loop_kernel at all?  (the launch itself still checks that the CTAs fit)
 bool persistent_loop_possible(const cd_dfa* d, const Settings& cfg, int B, int max_steps) {
     return cfg.loop_mode != CD_LOOP_PER_STEP && d->coop_launch && B <= cd::LOOP_MAX_ROWS && max_steps > 0 &&
-           !d->start_accepting;
+           max_steps < (1 << 24) && !d->start_accepting;
 }
 
 // per-step work counters / device step pointers of the persistent loop
@@ -1004,7 +1134,8 @@ cd_status cd_set_gather_max(cd_dfa_t* d, int32_t max_transitions) {
 
 cd_status cd_set_loop_mode(cd_dfa_t* d, int32_t mode) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
-    if (mode != CD_LOOP_AUTO && mode != CD_LOOP_PER_STEP) return fail(CD_ERR_ARG, "mode must be CD_LOOP_AUTO or CD_LOOP_PER_STEP");
+    if (mode != CD_LOOP_AUTO && mode != CD_LOOP_PER_STEP && mode != CD_LOOP_BARRIER)
+        return fail(CD_ERR_ARG, "mode must be CD_LOOP_AUTO, CD_LOOP_PER_STEP or CD_LOOP_BARRIER");
     std::lock_guard<std::mutex> lk(d->mu);
     d->cfg.loop_mode = mode;
     return CD_OK;
@@ -1094,17 +1225,30 @@ static cd_status decode_loop_impl(const cd_dfa_t* d, const void* const* step_log
     st = get_scratch(d, stream, B, &s);
     if (st != CD_OK) return st;
     bool persist = persistent_loop_possible(d, cfg, B, max_steps);
-    // Two persistent loops must never share the SMs: each waits at its grid barrier for CTAs that the
-    // other one keeps from being scheduled.  Within this process they are serialised per device (the loop
+    // no LIMIT: the barrier-free kernel (row groups advance independently); with a LIMIT, or on request, the
+    // lock-step kernel (a LIMIT is defined step by step over ALL rows)
+    const bool flow = persist && !lim.sat_ctr && cfg.loop_mode != CD_LOOP_BARRIER;
+    // Two lock-step loops must never share the SMs: each waits at its grid barrier for CTAs that the other
+    // one keeps from being scheduled.  Within this process they are serialised per device (the loop
     // synchronises its stream before returning anyway).
     std::unique_lock<std::mutex> coop_lock;
-    if (persist) coop_lock = std::unique_lock<std::mutex>(coop_mutex(d->device));
+    if (persist && !flow) coop_lock = std::unique_lock<std::mutex>(coop_mutex(d->device));
     if (persist) {
-        st = get_loop_scratch(s, max_steps, stream);
+        st = get_loop_scratch(s, flow ? max_steps * cd::FLOW_MAX_GROUPS : max_steps, stream);
         if (st != CD_OK) return st;
+    }
+    if (flow) {
+        const int grid = step_grid(d, B, dtype);
+        st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out,
+                              stream, lim, 2, grid, dtype);
+        if (st != CD_OK) return st;
+        st = enqueue_flow_loop(d, cfg, s, step_logits, dtype, ld_elems, B, max_steps, tokens_out, len_out,
+                               final_state_out, sum_logprob_out, done_out, stream, grid);
+        if (st != CD_OK) return st;
+    } else if (persist) {
         // both forms of the set-up are cheap; the persistent one is tried first and tells whether its CTAs fit
         st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out,
-                              stream, lim, true);
+                              stream, lim, 1);
         if (st != CD_OK) return st;
         bool launched = false;
         st = enqueue_persistent_loop(d, cfg, s, step_logits, dtype, ld_elems, B, max_steps, tokens_out, len_out,
@@ -1123,7 +1267,7 @@ static cd_status decode_loop_impl(const cd_dfa_t* d, const void* const* step_log
                 if (st != CD_OK) return st;
             }
     }
-    return finish_loop(s, stream, persist);
+    return finish_loop(s, stream, persist && !flow);
 }
 
 cd_status cd_decode_loop(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
@@ -1160,6 +1304,9 @@ cd_status cd_loop_trace(const cd_dfa_t* d, void* cuda_stream, int32_t cap, int64
     int steps = hn[cd::LOOP_TRACE_STEPS];
     if (steps > cd::LOOP_TRACE_STEPS) steps = cd::LOOP_TRACE_STEPS;
     *steps_out = steps;
+    // (row groups: a group that finishes early stops contributing to later entries -- keep the times monotone)
+    for (int k = 1; k <= steps; ++k)
+        if (ht[(size_t)k] < ht[(size_t)k - 1]) ht[(size_t)k] = ht[(size_t)k - 1];
     for (int k = 0; k < steps && k < cap; ++k) {
         n_active_out[k] = hn[(size_t)k];
         t_ns_out[k] = (int64_t)(ht[(size_t)k + 1] - ht[(size_t)k]);

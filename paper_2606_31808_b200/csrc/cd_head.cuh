@@ -360,7 +360,7 @@ __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadAr
             float ry = (lane < HG_WARPS) ? s_y[lane] : -INFINITY;
             head_warp_combine<SAMPLE>(rm, rs, ri, rk, ry);
             const TileMeta mt{slot, 0, 0, st, lo, deg, 0};
-            finalize_row(f, head_view(f), mt, rm, rs, ri, lane, true, SAMPLE, ry);
+            finalize_row(f, head_view(f), nullptr, mt, rm, rs, ri, lane, true, SAMPLE, ry);
         }
     }
 }
@@ -568,7 +568,7 @@ __global__ void head_finish_kernel(const HeadArgs a) {
         const long long lo = __ldg(f.dfa.row_ptr + st);
         const int deg = (int)(__ldg(f.dfa.row_ptr + st + 1) - lo);
         const TileMeta mt{slot, 0, 0, st, lo, deg, 0};
-        finalize_row(f, head_view(f), mt, m, s, idx, lane, false, SAMPLE, yb);
+        finalize_row(f, head_view(f), nullptr, mt, m, s, idx, lane, false, SAMPLE, yb);
     }
 }
 

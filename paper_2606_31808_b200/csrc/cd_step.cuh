@@ -82,6 +82,7 @@ constexpr int LOOP_MAX_ROWS = 32768;     // persistent loop: rows per call (bitm
 constexpr int LOOP_PARAM_STEPS = 32;     // step pointers passed as kernel parameters up to this many steps
 constexpr int LOOP_TRACE_STEPS = 256;    // per-step (timestamp, active rows) records kept for cd_loop_trace
 constexpr unsigned long long LOOP_SPIN_TIMEOUT_NS = 4000000000ull;  // a barrier that waits longer aborts the loop
+constexpr int FLOW_IDLE_LIMIT = 1 << 23;   // idle polls (>= 128 ns apart: > 1 s) after which a worker of flow_kernel gives up
 constexpr int MERGE_SPIN_LIMIT = 1 << 24;  // polls (>= 32 ns apart) after which a merging warp gives up
 
 // number of units a gathered row of `len` transitions is split into (P = units per row of the launch)
@@ -142,6 +143,7 @@ struct StepArgs {
     // the original row for the history and the sampling noise)
     int logits_by_slot;
     int upw, tpu_max;  // unit sizing: target units per warp, most tiles per unit
+    int idle_ns;       // flow_kernel: sleep between two looks at the groups' descriptors when nothing is published
 };
 
 // Persistent loop (loop_kernel): everything that outlives a step.
@@ -195,7 +197,46 @@ struct __align__(16) TileMeta {
     long long csr_lo;  // row_ptr[st]
     int csr_len;       // row_ptr[st + 1] - row_ptr[st]
     int lrow;          // row of the logits buffer
+    // flow_kernel: the (group, step) this tile belongs to -- a warp's ring may hold tiles of several
+    int step, n, tpu, grp;
 };
+
+constexpr int MODE_STEP = 0;  // step_kernel: one launch = one step
+constexpr int MODE_LOOP = 1;  // loop_kernel: whole loop, grid barrier between steps (LIMIT loops)
+constexpr int MODE_FLOW = 2;  // flow_kernel: whole loop, row groups advance independently (no barrier)
+
+// flow_kernel (cd_decode_loop without a LIMIT): the rows are split into G groups of Bg consecutive
+// original row ids, and every group is a decode loop of its own whose steps are published one by one:
+//   desc[g]      {step:24 | n:24 | tpu:16} of the step whose units may be drawn now (DONE when the group is finished);
+//                written with release by the warp that finalised the LAST row of the previous step of the group,
+//                read with acquire by every warp before it draws a unit of that step
+//   list[k&1]    [G*Bg] {row | state << 32}: the active rows of step k of each group, ascending row id (the stable
+//                order of a6); listf[k&1] the running sum of log-probs of those rows (fp32 bits)
+//   res / resf   [G*Bg] results of the running step by slot: {tag | done << 31 | next state}, {tag | new sum bits};
+//                tag = launch generation + step, so a word is either stale or complete (as the partial slots)
+//   fin[g]       rows finalised in the running step (relaxed counter: whoever brings it to n publishes the next step)
+//   work         [G][max_steps] unit counters
+// Nothing in it waits for a warp that is not running: units are only ever drawn by running warps.
+struct FlowArgs {
+    const void* step_ptrs[LOOP_PARAM_STEPS];
+    const void* const* step_ptrs_dev;
+    int B, G, Bg;
+    unsigned long long* desc;
+    unsigned long long* list[2];
+    unsigned int* listf[2];
+    unsigned long long* res;
+    unsigned long long* resf;
+    int* fin;
+    int* work;
+    long long pcap;  // partial slots per group
+    unsigned long long* trace_t;  // [LOOP_TRACE_STEPS + 1] time at which the last group published step k; [steps] = exit
+    int* trace_n;                 // [LOOP_TRACE_STEPS] active rows of step k over all groups; [LOOP_TRACE_STEPS] = steps run
+};
+constexpr unsigned long long FLOW_DONE = ~0ull;
+constexpr int FLOW_MAX_GROUPS = 8;
+__host__ __device__ inline unsigned long long flow_pack(int step, int n, int tpu) {
+    return (unsigned long long)(unsigned)step | ((unsigned long long)(unsigned)n << 24) | ((unsigned long long)(unsigned)tpu << 48);
+}
 
 template <int STAGES, int TILE_BYTES>
 struct __align__(128) WarpRing {
@@ -204,6 +245,7 @@ struct __align__(128) WarpRing {
     TileMeta meta[STAGES];
     unsigned long long bar[STAGES];
     unsigned short list[SAMPLE_LIST_CAP];  // SAMPLE: positions of a tile's allowed elements, compacted
+    int want[FLOW_MAX_GROUPS];             // flow_kernel: first step of each group this warp has not seen exhausted
 };
 
 // tiles per unit for n active rows (host mirrors this in cd_api.cu: step_units_cap)
@@ -240,14 +282,77 @@ __device__ __forceinline__ int mask_rank(const DfaDev& dfa, int st, int t, int l
     return base + c;
 }
 
+// flow_kernel: every row of step `step` of group `grp` is final -- build the group's next step.  Warp-
+// cooperative.  The results of the step were stored by the rows' finalisers before their (relaxed) count,
+// so they are on their way: poll until every tag is current.  Survivors keep their order (ascending row
+// id: the stable compaction of a6).  The new step is published with a release store of its descriptor.
+template <int WARPS>
+__device__ __forceinline__ void flow_publish(const StepArgs& a, const FlowArgs& F, int grp, int step, int n, unsigned gen0,
+                                             int tiles_per_row, int tpu_max, int lane) {
+    const int kk = step + 1;
+    const unsigned long long tag = (unsigned long long)(gen0 + (unsigned)step) << 32;
+    const long long off = (long long)grp * F.Bg;
+    const unsigned long long* cur = F.list[step & 1] + off;
+    unsigned long long* nxt = F.list[kk & 1] + off;
+    unsigned int* nxtf = F.listf[kk & 1] + off;
+    int base = 0;
+    constexpr int U = 4;  // chunks of 32 slots in flight
+#pragma unroll 1
+    for (int i0 = 0; i0 < n; i0 += 32 * U) {
+        unsigned long long r[U], f[U], e[U];
+#pragma unroll
+        for (int q = 0; q < U; ++q) {
+            const int i = i0 + q * 32 + lane;
+            r[q] = f[q] = tag;
+            e[q] = 0;
+            if (i < n) {
+                e[q] = ld_relaxed_gpu_u64(cur + i);
+                int spins = 0;
+                do {
+                    r[q] = ld_relaxed_gpu_u64(F.res + off + i);
+                    f[q] = ld_relaxed_gpu_u64(F.resf + off + i);
+                } while (((r[q] ^ tag) >> 32 || (f[q] ^ tag) >> 32) && ++spins < MERGE_SPIN_LIMIT);
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < U; ++q) {
+            const int i = i0 + q * 32 + lane;
+            const bool keep = (i < n) && (((unsigned)r[q] >> 31) == 0u) && !((r[q] ^ tag) >> 32);
+            const unsigned b = __ballot_sync(FULL, keep);
+            if (keep) {
+                const int p = base + __popc(b & ((1u << lane) - 1u));
+                nxt[p] = (e[q] & 0xFFFFFFFFull) | ((unsigned long long)((unsigned)r[q] & 0x7FFFFFFFu) << 32);
+                nxtf[p] = (unsigned)f[q];
+            }
+            base += __popc(b);
+        }
+    }
+    __syncwarp();
+    if (lane == 0) {
+        const bool stop = (base == 0) || (kk >= a.max_steps);
+        F.fin[grp] = 0;
+        if (stop) atomicMax(F.trace_n + LOOP_TRACE_STEPS, kk);  // steps run = the most any group ran
+        if (kk <= LOOP_TRACE_STEPS) {
+            if (kk < LOOP_TRACE_STEPS) atomicAdd(F.trace_n + kk, base);
+            atomicMax(F.trace_t + kk, global_timer_ns());
+        }
+        const unsigned long long d =
+            stop ? FLOW_DONE
+                 // unit size as if all G groups had this many rows: the groups share the warps
+                 : flow_pack(kk, base, tiles_per_unit((long long)base * F.G, tiles_per_row, (long long)gridDim.x * WARPS, tpu_max, a.upw));
+        asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(F.desc + grp), "l"(d) : "memory");
+    }
+}
+
 // Row finished: (m, s, idx) is the merged result of all its units.  Warp-uniform.
 // `gathered`: idx is the position inside the state's CSR row instead of the token id.
 // `sampled`: idx is the sampled token (position), ytok its tempered logit: logprob = (ytok - m) - log(sum).
-// PERSIST: per-row arrays are indexed by the original row id (mt.lrow); surviving rows set their bit in
-// the next step's bitmap.
-template <bool PERSIST = false>
-__device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& sv, const TileMeta& mt, float m,
-                                             float s, int idx, int lane, bool gathered, bool sampled = false,
+// MODE_LOOP: per-row arrays are indexed by the original row id (mt.lrow); surviving rows set their bit in
+// the next step's bitmap.  MODE_FLOW: the result goes to the group's result slots; returns true (in every
+// lane) if this was the last row of the group's step (the caller then publishes the next step).
+template <int MODE = MODE_STEP>
+__device__ __forceinline__ bool finalize_row(const StepArgs& a, const StepView& sv, const FlowArgs* F, const TileMeta& mt,
+                                             float m, float s, int idx, int lane, bool gathered, bool sampled = false,
                                              float ytok = 0.0f) {
     float lp, lse;
     int pos;
@@ -257,6 +362,9 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& 
         csr_lo = __ldg(a.dfa.row_ptr + mt.st);
         csr_len = (int)(__ldg(a.dfa.row_ptr + mt.st + 1) - csr_lo);
     }
+    unsigned sum_prev_bits = 0;
+    if (MODE == MODE_FLOW && lane == 0)  // the row's running sum travels with its list entry (same round trip as the rank)
+        sum_prev_bits = __ldcg(F->listf[mt.step & 1] + (long long)mt.grp * F->Bg + mt.slot);
     if (m == -INFINITY) {  // every allowed logit is -inf: lowest allowed id (G6)
         lp = -INFINITY;
         lse = -INFINITY;
@@ -267,6 +375,7 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& 
         lse = m + L;
         pos = gathered ? idx : mask_rank(a.dfa, mt.st, idx, lane);
     }
+    int last = 0;
     if (lane == 0) {
         const bool in_row = (pos >= 0) && (pos < csr_len);
         const long long j = csr_lo + pos;
@@ -283,26 +392,41 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& 
             atomicAdd(a.ctrs + 2, 1);
             token = -1;
         }
-        const int slot = PERSIST ? mt.lrow : mt.slot;
+        const int step = (MODE == MODE_FLOW) ? mt.step : sv.step;
+        const int slot = (MODE == MODE_STEP) ? mt.slot : mt.lrow;
         CD_PHASE_MIN(sv.ph_first_fin);
         CD_PHASE_MAX(sv.ph_last_fin);
-        sv.state_next[slot] = ns;
-        if (a.token_out) a.token_out[slot] = token;
-        if (a.logprob_out) a.logprob_out[slot] = lp;
-        if (a.lse_out) a.lse_out[slot] = lse;
-        if (a.done_out) a.done_out[slot] = dn;
-        if (PERSIST && !dn) atomicOr(sv.alive_next + (slot >> 5), 1u << (slot & 31));
+        if (MODE != MODE_FLOW) {
+            sv.state_next[slot] = ns;
+            if (a.token_out) a.token_out[slot] = token;
+            if (a.logprob_out) a.logprob_out[slot] = lp;
+            if (a.lse_out) a.lse_out[slot] = lse;
+            if (a.done_out) a.done_out[slot] = dn;
+        }
+        if (MODE == MODE_LOOP && !dn) atomicOr(sv.alive_next + (slot >> 5), 1u << (slot & 31));
         if (a.hist_tokens) {  // decode loop: this slot's row, original id
-            const long long rid = PERSIST ? (long long)mt.lrow : (a.row_map ? (long long)__ldg(a.row_map + slot) : slot);
-            a.hist_tokens[rid * a.max_steps + sv.step] = token;
-            a.hist_len[rid] = sv.step + 1;
+            const long long rid = (MODE != MODE_STEP) ? (long long)mt.lrow : (a.row_map ? (long long)__ldg(a.row_map + slot) : slot);
+            a.hist_tokens[rid * a.max_steps + step] = token;
+            a.hist_len[rid] = step + 1;
             a.hist_final_state[rid] = ns;
-            // written by another SM one step ago (persistent loop): read at the L2, never from a stale L1 line
-            a.hist_sum_logprob[rid] = __ldcg(a.hist_sum_logprob + rid) + lp;
+            float sum;
+            if (MODE == MODE_FLOW) sum = (step == 0 ? 0.0f : __uint_as_float(sum_prev_bits)) + lp;
+            // (written by another SM one step ago in loop_kernel: read at the L2, never from a stale L1 line)
+            else sum = __ldcg(a.hist_sum_logprob + rid) + lp;
+            a.hist_sum_logprob[rid] = sum;
             a.hist_done[rid] = ok ? dn : (uint8_t)0;
-            if (a.sat_ctr && ok && dn && __ldg(a.satisfying + ns)) atomicAdd(a.sat_ctr, 1);
+            if (MODE != MODE_FLOW && a.sat_ctr && ok && dn && __ldg(a.satisfying + ns)) atomicAdd(a.sat_ctr, 1);
+            if (MODE == MODE_FLOW) {
+                const unsigned long long tag = (unsigned long long)(sv.gen + (unsigned)step) << 32;
+                const long long o = (long long)mt.grp * F->Bg + mt.slot;
+                st_relaxed_gpu_u64(F->res + o, tag | ((unsigned)ns & 0x7FFFFFFFu) | ((unsigned)dn << 31));
+                st_relaxed_gpu_u64(F->resf + o, tag | __float_as_uint(sum));
+                last = (atomicAdd(F->fin + mt.grp, 1) == mt.n - 1) ? 1 : 0;
+            }
         }
     }
+    if (MODE == MODE_FLOW) return __shfl_sync(FULL, last, 0) != 0;
+    return false;
 }
 
 template <bool SAMPLE>
@@ -330,8 +454,8 @@ struct RingPos {
     uint32_t cons_phase = 0;
 };
 
-// slot i of the persistent loop -> original row id: the i-th set bit of the snapshot (binary search
-// over the per-word prefix counts, then find-nth-set inside the word).  Warp-uniform.
+// slot i of loop_kernel -> original row id: the i-th set bit of the snapshot (binary search over the
+// per-word prefix counts, then find-nth-set inside the word).  Warp-uniform.
 __device__ __forceinline__ int select_row(const StepView& sv, int i) {
     int lo = 0, hi = sv.nwords;  // invariant: s_pref[lo] <= i < s_pref[hi]
     while (hi - lo > 1) {
@@ -342,10 +466,37 @@ __device__ __forceinline__ int select_row(const StepView& sv, int i) {
     return lo * 32 + (int)__fns(sv.s_bits[lo], 0, r + 1);
 }
 
-// One decoding step over the slots [0, sv.n): issue + consume loops of this warp.
-template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER, bool SAMPLE, bool PERSIST>
-__device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv, WarpRing<STAGES, TILE_BYTES>& ring,
-                                          RingPos& rp, const int warp, const int lane) {
+// The step a unit belongs to: how its rows are split and where its shared state lives.
+struct UnitCtx {
+    int n, tpu, Pd, PG, P, total_units, step, grp;
+    const unsigned char* logits;
+    int* work;
+    long long pbase;  // first partial slot
+    int tbase;        // first ticket
+};
+
+template <int WARPS, int TILE_TOK, int TPU_MAX, bool GATHER>
+__device__ __forceinline__ void unit_ctx_split(UnitCtx& c, const StepArgs& a, int n, int tpu) {
+    const int total_warps = gridDim.x * WARPS;
+    const int tiles_per_row = (a.dfa.V + TILE_TOK - 1) / TILE_TOK;
+    c.n = n;
+    c.tpu = tpu;
+    c.Pd = (tiles_per_row + tpu - 1) / tpu;  // units per row of a dense scan
+    // a gathered row is split only as far as needed to give every warp a few units
+    c.PG = GATHER ? max(1, min(c.Pd, (total_warps * GATHER_UPW) / max(n, 1))) : c.Pd;
+    // units per row of this step; if every state is gathered no unit is drawn in vain
+    c.P = (GATHER && a.all_gather) ? c.PG : c.Pd;
+    c.total_units = n * c.P;
+}
+
+// The streaming engine of a warp: issue + consume loops.
+//   MODE_STEP / MODE_LOOP: one decoding step over the slots [0, sv.n); returns when the step's units are
+//   exhausted and this warp's tiles are consumed.
+//   MODE_FLOW: the whole loop; the warp draws units from whichever group has a published step with units
+//   left (oldest step first) and returns when every group is finished.
+template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER, bool SAMPLE, int MODE>
+__device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv, const FlowArgs* F,
+                                          WarpRing<STAGES, TILE_BYTES>& ring, RingPos& rp, const int warp, const int lane) {
     constexpr int SZ = (DT == DT_BF16) ? 2 : 4;
     constexpr int TILE_TOK = TILE_BYTES / SZ;
     constexpr int MASK_BYTES = TILE_TOK / 8;
@@ -354,21 +505,31 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
     static_assert(WPL >= 1 && TILE_TOK % 1024 == 0, "tile must hold a multiple of 32 mask words");
 
     // ---------------- issue side (warp-uniform state)
-    // The first unit of a warp is its global warp id (no atomic on the start-up chain); later
-    // units come from the work counter, which therefore starts at 0 = unit `total_warps`.
+    // MODE_STEP / MODE_LOOP: the first unit of a warp is its global warp id (no atomic on the start-up
+    // chain); later units come from the work counter, which therefore starts at 0 = unit `total_warps`.
+    // MODE_FLOW: every unit is drawn from its step's counter.
     const int total_warps = gridDim.x * WARPS;
+    const int draw_base = (MODE == MODE_FLOW) ? 0 : total_warps;
     int next_u_l0 = blockIdx.x * WARPS + warp;  // prefetched unit id, valid in lane 0
-    const unsigned gen = sv.gen;                // launch generation (tag of the partial slots)
-    const int n = sv.n;
     const int V = a.dfa.V;
     const int tiles_per_row = (V + TILE_TOK - 1) / TILE_TOK;
-    const int tpu = tiles_per_unit(n, tiles_per_row, total_warps, min(TPU_MAX, a.tpu_max), a.upw);
-    const int Pd = (tiles_per_row + tpu - 1) / tpu;  // units per row of a dense scan
-    // a gathered row is split only as far as needed to give every warp a few units
-    const int PG = GATHER ? max(1, min(Pd, (total_warps * GATHER_UPW) / max(n, 1))) : Pd;
-    // units per row of this launch; if every state is gathered no unit is drawn in vain
-    const int P = (GATHER && a.all_gather) ? PG : Pd;
-    const int total_units = n * P;
+    const int tpu_max = min(TPU_MAX, a.tpu_max);
+    UnitCtx cur{};
+    bool have_step = false;   // MODE_FLOW: `cur` is a published step with units left (as far as this warp knows)
+    bool all_done = false;    // MODE_FLOW: every group is finished
+    if (MODE != MODE_FLOW) {
+        unit_ctx_split<WARPS, TILE_TOK, TPU_MAX, GATHER>(cur, a, sv.n, tiles_per_unit(sv.n, tiles_per_row, total_warps, tpu_max, a.upw));
+        cur.step = sv.step;
+        cur.grp = 0;
+        cur.logits = sv.logits;
+        cur.work = sv.work_ctr;
+        cur.pbase = 0;
+        cur.tbase = 0;
+        have_step = true;
+    } else {
+        if (lane < FLOW_MAX_GROUPS) ring.want[lane] = 0;
+        __syncwarp();
+    }
     const bool ragged_row = (V % TILE_TOK) != 0;
     const uint64_t pol_stream = l2_policy_evict_first();
 
@@ -380,19 +541,65 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
     const unsigned char* iss_msk = nullptr;  // next mask piece
     int iss_stage = rp.iss_stage, in_flight = 0;
 
-    auto issue_one = [&]() {
+    // MODE_FLOW: look at the groups' descriptors (one per lane, acquire) and take the oldest published step
+    // this warp has not seen exhausted; false if there is none right now
+    auto acquire_step = [&]() -> bool {
+        unsigned long long d = FLOW_DONE;
+        if (lane < F->G) asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(d) : "l"(F->desc + lane) : "memory");
+        const bool done_g = (lane >= F->G) || (d == FLOW_DONE);
+        const int st_g = (int)(d & 0xFFFFFFull);
+        const bool avail = !done_g && (st_g >= ring.want[lane & (FLOW_MAX_GROUPS - 1)]);
+        if (__all_sync(FULL, done_g)) {
+            all_done = true;
+            return false;
+        }
+        int key = avail ? (st_g * FLOW_MAX_GROUPS + lane) : 0x7FFFFFFF;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) key = min(key, __shfl_xor_sync(FULL, key, o));
+        if (key == 0x7FFFFFFF) return false;
+        const int g = key & (FLOW_MAX_GROUPS - 1);
+        d = __shfl_sync(FULL, d, g);
+        const int step = (int)(d & 0xFFFFFFull), n = (int)((d >> 24) & 0xFFFFFFull), tpu = (int)(d >> 48);
+        unit_ctx_split<WARPS, TILE_TOK, TPU_MAX, GATHER>(cur, a, n, tpu);
+        cur.step = step;
+        cur.grp = g;
+        cur.logits = static_cast<const unsigned char*>(F->step_ptrs_dev ? F->step_ptrs_dev[step] : F->step_ptrs[step]);
+        cur.work = F->work + (long long)g * a.max_steps + step;
+        cur.pbase = (long long)g * F->pcap;
+        cur.tbase = g * F->Bg;
+        if (lane == 0) next_u_l0 = atomicAdd(cur.work, 1);
+        have_step = true;
+        return true;
+    };
+
+    // issues one tile (or pseudo tile); false if there is nothing to issue right now
+    auto issue_one = [&]() -> bool {
         while (iss_tile >= iss_end) {  // next unit (units of a gathered row beyond its pieces are skipped)
-            if (exhausted) return;
-            const int u = __shfl_sync(FULL, next_u_l0, 0);
-            if (u >= total_units) {
-                exhausted = true;
-                return;
+            if (MODE == MODE_FLOW) {
+                if (!have_step && !acquire_step()) return false;
+            } else if (exhausted) {
+                return false;
             }
-            if (lane == 0) next_u_l0 = total_warps + atomicAdd(sv.work_ctr, 1);
-            iss_slot = u / P;
-            const int part = u - iss_slot * P;
+            const int u = __shfl_sync(FULL, next_u_l0, 0);
+            if (u >= cur.total_units) {
+                if (MODE == MODE_FLOW) {  // this step has no units left: never look at it again
+                    if (lane == 0) ring.want[cur.grp] = cur.step + 1;
+                    __syncwarp();
+                    have_step = false;
+                    continue;
+                }
+                exhausted = true;
+                return false;
+            }
+            if (lane == 0) next_u_l0 = draw_base + atomicAdd(cur.work, 1);
+            iss_slot = u / cur.P;
+            const int part = u - iss_slot * cur.P;
             long long rl;  // row of the logits buffer
-            if (PERSIST) {
+            if (MODE == MODE_FLOW) {
+                const unsigned long long e = ld_relaxed_gpu_u64(F->list[cur.step & 1] + (long long)cur.grp * F->Bg + iss_slot);
+                rl = (long long)(unsigned)e;
+                iss_st = (int)(e >> 32);
+            } else if (MODE == MODE_LOOP) {
                 rl = select_row(sv, iss_slot);
                 // states are double-buffered by step parity: a unit drawn after its row was finalised
                 // still sees the state the row was processed in
@@ -406,8 +613,8 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             iss_row = (int)rl;
             const bool bad = (iss_st < 0) || (iss_st >= a.dfa.S);
             const int sts = bad ? 0 : iss_st;
-            // (the persistent loop never holds a row whose state accepts: such rows left the bitmap)
-            const bool acc = !PERSIST && !bad && (__ldg(a.dfa.accepting + sts) != 0);
+            // (the persistent loops never hold a row whose state accepts: such rows left the active set)
+            const bool acc = (MODE == MODE_STEP) && !bad && (__ldg(a.dfa.accepting + sts) != 0);
             if (GATHER) {  // the CSR bounds decide between scan and gather
                 iss_lo = __ldg(a.dfa.row_ptr + sts);
                 iss_len = (int)(__ldg(a.dfa.row_ptr + sts + 1) - iss_lo);
@@ -417,30 +624,30 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             }
             if (bad || acc) {
                 if (lane == 0) {
-                    ring.meta[iss_stage] =
-                        TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (part << 8), iss_st, 0, 0, iss_row};
+                    ring.meta[iss_stage] = TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (part << 8), iss_st, 0, 0,
+                                                    iss_row, cur.step, cur.n, cur.tpu, cur.grp};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
                 iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
                 ++in_flight;
                 iss_tile = iss_end = 0;
-                return;
+                return true;
             }
             if (GATHER && iss_len <= a.gather_max) {
-                if (part >= gather_parts(iss_len, PG)) continue;
+                if (part >= gather_parts(iss_len, cur.PG)) continue;
                 if (lane == 0) {
-                    ring.meta[iss_stage] = TileMeta{iss_slot, 0, FLAG_GATHER | FLAG_LAST | (part << 8), iss_st,
-                                                    iss_lo, iss_len, iss_row};
+                    ring.meta[iss_stage] = TileMeta{iss_slot, 0, FLAG_GATHER | FLAG_LAST | (part << 8), iss_st, iss_lo, iss_len,
+                                                    iss_row, cur.step, cur.n, cur.tpu, cur.grp};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
                 iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
                 ++in_flight;
                 iss_tile = iss_end = 0;
-                return;
+                return true;
             }
-            iss_tile = part * tpu;
-            iss_end = min(iss_tile + tpu, tiles_per_row);
-            iss_src = sv.logits + rl * a.ld_bytes + (long long)iss_tile * TILE_BYTES;
+            iss_tile = part * cur.tpu;
+            iss_end = min(iss_tile + cur.tpu, tiles_per_row);
+            iss_src = cur.logits + rl * a.ld_bytes + (long long)iss_tile * TILE_BYTES;
             iss_msk = reinterpret_cast<const unsigned char*>(a.dfa.mask + (long long)iss_st * a.dfa.Wpad) +
                       (long long)iss_tile * MASK_BYTES;
             iss_flags = (part << 8) | FLAG_FIRST;
@@ -449,6 +656,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
         const uint32_t dst = smem_u32(ring.logits[iss_stage]);
         const uint32_t mdst = smem_u32(ring.mask[iss_stage]);
         const int fl = iss_flags | ((iss_tile + 1 == iss_end) ? FLAG_LAST : 0);
+        const TileMeta meta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, iss_row, cur.step, cur.n, cur.tpu, cur.grp};
         if (ragged_row && iss_tile + 1 == tiles_per_row) {
             // last tile of a row whose length is not a multiple of the tile: partial copies; the
             // < 16 trailing logits bytes go through plain loads, unused mask words are zeroed.
@@ -468,13 +676,13 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 reinterpret_cast<uint32_t*>(ring.mask[iss_stage])[w] = 0u;
             __syncwarp();
             if (lane == 0) {
-                ring.meta[iss_stage] = TileMeta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, iss_row};
+                ring.meta[iss_stage] = meta;
                 mbar_arrive_expect_tx(bar, bulk + mbytes);
                 if (bulk) bulk_g2s_hint(dst, iss_src, bulk, bar, pol_stream);
                 bulk_g2s(mdst, iss_msk, mbytes, bar);
             }
         } else if (lane == 0) {
-            ring.meta[iss_stage] = TileMeta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, iss_row};
+            ring.meta[iss_stage] = meta;
             mbar_arrive_expect_tx(bar, TILE_BYTES + MASK_BYTES);
             bulk_g2s_hint(dst, iss_src, TILE_BYTES, bar, pol_stream);
             bulk_g2s(mdst, iss_msk, MASK_BYTES, bar);
@@ -485,24 +693,33 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
         ++iss_tile;
         ++in_flight;
         iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
+        return true;
     };
-
-#pragma unroll 1
-    for (int k = 0; k < STAGES; ++k) issue_one();
 
     // ---------------- consume side
     float m = -INFINITY, s = 0.0f, kb = -INFINITY;  // kb: best perturbed key (SAMPLE); idx then is its token
     int idx = 0x7FFFFFFF;
-    const int rng_step = a.rng_step_base + sv.step;
     int cons_stage = rp.cons_stage;
     uint32_t cons_phase = rp.cons_phase;
-    const unsigned long long tag = (unsigned long long)gen << 32;
 #ifdef CD_TUNING
     bool first_tile = true;
 #endif
+    int idle_polls = 0;
 
 #pragma unroll 1
-    while (in_flight > 0) {
+    for (;;) {
+        while (in_flight < STAGES && issue_one()) {
+        }
+        if (in_flight == 0) {
+            if (MODE != MODE_FLOW || all_done) break;
+            __nanosleep(a.idle_ns);  // nothing published right now: some group is between two steps
+            if (++idle_polls > FLOW_IDLE_LIMIT) {  // never on a healthy run: fail the call, do not hang
+                if (lane == 0) atomicAdd(a.ctrs + 2, 1);
+                break;
+            }
+            continue;
+        }
+        idle_polls = 0;
         mbar_wait(smem_u32(&ring.bar[cons_stage]), cons_phase);
         __syncwarp();
 #ifdef CD_TUNING
@@ -514,32 +731,58 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
 #endif
         const TileMeta mt = ring.meta[cons_stage];
         const int part = mt.flags >> 8;
+        // the step this tile belongs to (MODE_FLOW: whatever the ring holds; else the step of this call)
+        UnitCtx cc = cur;
+        if (MODE == MODE_FLOW) {
+            unit_ctx_split<WARPS, TILE_TOK, TPU_MAX, GATHER>(cc, a, mt.n, mt.tpu);
+            cc.step = mt.step;
+            cc.grp = mt.grp;
+            cc.logits = static_cast<const unsigned char*>(F->step_ptrs_dev ? F->step_ptrs_dev[mt.step] : F->step_ptrs[mt.step]);
+            cc.pbase = (long long)mt.grp * F->pcap;
+            cc.tbase = mt.grp * F->Bg;
+        }
+        const unsigned gen = sv.gen + ((MODE == MODE_FLOW) ? (unsigned)cc.step : 0u);  // tag of the partial slots
+        const unsigned long long tag = (unsigned long long)gen << 32;
+        const int rng_step = a.rng_step_base + cc.step;
         // original row id of the slot: names the history row and seeds the sampling noise
         auto orig_row = [&]() -> uint32_t {
-            return PERSIST ? (uint32_t)mt.lrow : (uint32_t)(a.row_map ? __ldg(a.row_map + mt.slot) : mt.slot);
+            return (MODE != MODE_STEP) ? (uint32_t)mt.lrow : (uint32_t)(a.row_map ? __ldg(a.row_map + mt.slot) : mt.slot);
         };
+        bool publish = false;  // MODE_FLOW: this warp finalised the last row of (cc.grp, cc.step)
 
         if (mt.flags & (FLAG_ACCEPT | FLAG_BADSTATE)) {
             // accepted rows never advance; a state outside [0, S) is reported done
-            if (part == 0 && lane == 0) {
-                const int slot = PERSIST ? mt.lrow : mt.slot;
-                sv.state_next[slot] = mt.st;
-                if (a.token_out) a.token_out[slot] = -1;
-                if (a.logprob_out) a.logprob_out[slot] = 0.0f;
-                if (a.lse_out) a.lse_out[slot] = 0.0f;
-                if (a.done_out) a.done_out[slot] = 1;
-                if (mt.flags & FLAG_BADSTATE) {
-                    atomicAdd(a.ctrs + 2, 1);
-                    if (a.hist_tokens) {  // the row leaves the loop here, undone, in the state it has
-                        const long long rid = orig_row();
-                        a.hist_final_state[rid] = mt.st;
-                        a.hist_done[rid] = 0;
+            if (part == 0) {
+                int last = 0;
+                if (lane == 0) {
+                    const int slot = (MODE == MODE_STEP) ? mt.slot : mt.lrow;
+                    if (MODE != MODE_FLOW) {
+                        sv.state_next[slot] = mt.st;
+                        if (a.token_out) a.token_out[slot] = -1;
+                        if (a.logprob_out) a.logprob_out[slot] = 0.0f;
+                        if (a.lse_out) a.lse_out[slot] = 0.0f;
+                        if (a.done_out) a.done_out[slot] = 1;
+                    }
+                    if (mt.flags & FLAG_BADSTATE) {
+                        atomicAdd(a.ctrs + 2, 1);
+                        if (a.hist_tokens) {  // the row leaves the loop here, undone, in the state it has
+                            const long long rid = orig_row();
+                            a.hist_final_state[rid] = mt.st;
+                            a.hist_done[rid] = 0;
+                        }
+                    }
+                    if (MODE == MODE_FLOW) {  // the row leaves its group
+                        const long long o = (long long)mt.grp * F->Bg + mt.slot;
+                        st_relaxed_gpu_u64(F->res + o, tag | 0x80000000u);
+                        st_relaxed_gpu_u64(F->resf + o, tag);
+                        last = (atomicAdd(F->fin + mt.grp, 1) == mt.n - 1) ? 1 : 0;
                     }
                 }
+                if (MODE == MODE_FLOW) publish = __shfl_sync(FULL, last, 0) != 0;
             }
         } else {
             const bool gathered = GATHER && (mt.flags & FLAG_GATHER);
-            const int np = gathered ? gather_parts(mt.csr_len, PG) : P;  // units this row was split into
+            const int np = gathered ? gather_parts(mt.csr_len, cc.PG) : cc.P;  // units this row was split into
             if (gathered) {
                 // piece [j0, j1) of the state's CSR row: tokens read coalesced, their logits gathered
                 // with GATHER_UNROLL independent loads per lane; idx = position in the CSR row, which
@@ -552,7 +795,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 const int j0 = (int)(((long long)mt.csr_len * part) / np);
                 const int j1 = (int)(((long long)mt.csr_len * (part + 1)) / np);
                 const int* tk = a.dfa.tok + mt.csr_lo;
-                const unsigned char* rowp = sv.logits + (long long)mt.lrow * a.ld_bytes;
+                const unsigned char* rowp = cc.logits + (long long)mt.lrow * a.ld_bytes;
                 // software pipeline: the token ids of the next round are loaded while this round's
                 // logits are in flight
                 int t[GATHER_UNROLL];
@@ -670,92 +913,93 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 auto sampled_y = [&](int pos) -> float {
                     if (!SAMPLE || rm == -INFINITY) return 0.0f;
                     const int tokid = gathered ? __ldg(a.dfa.tok + mt.csr_lo + pos) : pos;
-                    const unsigned char* rowp = sv.logits + (long long)mt.lrow * a.ld_bytes;
+                    const unsigned char* rowp = cc.logits + (long long)mt.lrow * a.ld_bytes;
                     const float xv = (DT == DT_BF16)
                                          ? __uint_as_float(((uint32_t)__ldg(reinterpret_cast<const uint16_t*>(rowp) + tokid)) << 16)
                                          : __ldg(reinterpret_cast<const float*>(rowp) + tokid);
                     return __fmul_rn(xv, a.inv_tau);
                 };
                 if (np == 1) {
-                    finalize_row<PERSIST>(a, sv, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
+                    publish = finalize_row<MODE>(a, sv, F, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
                 } else {
                     // Publish from lane 1 (lane 0 is busy issuing copies): self-validating words,
                     // then a RELAXED ticket -- no fence anywhere.  The last arriver merges.
                     int t = 0;
                     if (lane == 1) {
-                        PartialSlot* ps = a.partials + ((long long)mt.slot * P + part);
+                        PartialSlot* ps = a.partials + (cc.pbase + (long long)mt.slot * cc.P + part);
                         st_relaxed_gpu_u64(&ps->m, tag | (unsigned)__float_as_int(rm));
                         st_relaxed_gpu_u64(&ps->s, tag | (unsigned)__float_as_int(rs));
                         st_relaxed_gpu_u64(&ps->idx, tag | (unsigned)ri);
                         if (SAMPLE) st_relaxed_gpu_u64(&ps->pad, tag | (unsigned)__float_as_int(rk));
-                        t = atomicAdd(a.tickets + mt.slot, 1);
+                        t = atomicAdd(a.tickets + cc.tbase + mt.slot, 1);
                     }
                     t = __shfl_sync(FULL, t, 1);
                     if (t == np - 1) {
-                    if (lane == 1) a.tickets[mt.slot] = 0;
-                    // The other units' words were stored before their tickets, but nothing orders
-                    // them: poll until every tag is current (normally the first read).
-                    const PartialSlot* base = a.partials + (long long)mt.slot * P;
-                    // Merge in slot order whoever merges (bitwise reproducible): lane q % 32 takes
-                    // slot q; the own result (identical in every lane after the butterfly) stands in
-                    // for slot `part`.
-                    const float om = rm, os = rs, ok_ = rk;
-                    const int oi = ri;
-                    rm = -INFINITY;
-                    rs = 0.0f;
-                    rk = -INFINITY;
-                    ri = 0x7FFFFFFF;
-                    for (int q0 = 0; q0 < np; q0 += 32) {
-                        const int q = q0 + lane;
-                        const bool want = (q < np) && (q != part);
-                        bool ok = !want;
-                        unsigned long long wm = 0, ws = 0, wi = 0, wk = 0;
-                        int spins = 0;
-                        while (true) {
-                            if (!ok) {
-                                wm = ld_relaxed_gpu_u64(&base[q].m);
-                                ws = ld_relaxed_gpu_u64(&base[q].s);
-                                wi = ld_relaxed_gpu_u64(&base[q].idx);
-                                ok = ((wm >> 32) == gen) && ((ws >> 32) == gen) && ((wi >> 32) == gen);
-                                if (SAMPLE) {
-                                    wk = ld_relaxed_gpu_u64(&base[q].pad);
-                                    ok = ok && ((wk >> 32) == gen);
+                        if (lane == 1) a.tickets[cc.tbase + mt.slot] = 0;
+                        // The other units' words were stored before their tickets, but nothing orders
+                        // them: poll until every tag is current (normally the first read).
+                        const PartialSlot* base = a.partials + (cc.pbase + (long long)mt.slot * cc.P);
+                        // Merge in slot order whoever merges (bitwise reproducible): lane q % 32 takes
+                        // slot q; the own result (identical in every lane after the butterfly) stands in
+                        // for slot `part`.
+                        const float om = rm, os = rs, ok_ = rk;
+                        const int oi = ri;
+                        rm = -INFINITY;
+                        rs = 0.0f;
+                        rk = -INFINITY;
+                        ri = 0x7FFFFFFF;
+                        for (int q0 = 0; q0 < np; q0 += 32) {
+                            const int q = q0 + lane;
+                            const bool want = (q < np) && (q != part);
+                            bool ok = !want;
+                            unsigned long long wm = 0, ws = 0, wi = 0, wk = 0;
+                            int spins = 0;
+                            while (true) {
+                                if (!ok) {
+                                    wm = ld_relaxed_gpu_u64(&base[q].m);
+                                    ws = ld_relaxed_gpu_u64(&base[q].s);
+                                    wi = ld_relaxed_gpu_u64(&base[q].idx);
+                                    ok = ((wm >> 32) == gen) && ((ws >> 32) == gen) && ((wi >> 32) == gen);
+                                    if (SAMPLE) {
+                                        wk = ld_relaxed_gpu_u64(&base[q].pad);
+                                        ok = ok && ((wk >> 32) == gen);
+                                    }
+                                }
+                                if (__all_sync(FULL, ok)) break;
+                                __nanosleep(32);
+                                if (++spins > MERGE_SPIN_LIMIT) {  // never on a healthy run: fail the call, do not hang
+                                    if (lane == 0) atomicAdd(a.ctrs + 2, 1);
+                                    break;
                                 }
                             }
-                            if (__all_sync(FULL, ok)) break;
-                            __nanosleep(32);
-                            if (++spins > MERGE_SPIN_LIMIT) {  // never on a healthy run: fail the call, do not hang
-                                if (lane == 0) atomicAdd(a.ctrs + 2, 1);
-                                break;
-                            }
+                            if (SAMPLE) {
+                                int dummy = 0;
+                                if (want) {
+                                    online_combine(rm, rs, dummy, __int_as_float((int)(unsigned)wm),
+                                                   __int_as_float((int)(unsigned)ws), 0);
+                                    sample_combine(rk, ri, __int_as_float((int)(unsigned)wk), (int)(unsigned)wi);
+                                } else if (q == part) {
+                                    online_combine(rm, rs, dummy, om, os, 0);
+                                    sample_combine(rk, ri, ok_, oi);
+                                }
+                            } else if (want)
+                                online_combine(rm, rs, ri, __int_as_float((int)(unsigned)wm),
+                                               __int_as_float((int)(unsigned)ws), (int)(unsigned)wi);
+                            else if (q == part)
+                                online_combine(rm, rs, ri, om, os, oi);
                         }
-                        if (SAMPLE) {
-                            int dummy = 0;
-                            if (want) {
-                                online_combine(rm, rs, dummy, __int_as_float((int)(unsigned)wm),
-                                               __int_as_float((int)(unsigned)ws), 0);
-                                sample_combine(rk, ri, __int_as_float((int)(unsigned)wk), (int)(unsigned)wi);
-                            } else if (q == part) {
-                                online_combine(rm, rs, dummy, om, os, 0);
-                                sample_combine(rk, ri, ok_, oi);
-                            }
-                        } else if (want)
-                            online_combine(rm, rs, ri, __int_as_float((int)(unsigned)wm),
-                                           __int_as_float((int)(unsigned)ws), (int)(unsigned)wi);
-                        else if (q == part)
-                            online_combine(rm, rs, ri, om, os, oi);
-                    }
-                    warp_combine_s<SAMPLE>(rm, rs, ri, rk);
-                    finalize_row<PERSIST>(a, sv, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
+                        warp_combine_s<SAMPLE>(rm, rs, ri, rk);
+                        publish = finalize_row<MODE>(a, sv, F, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
                     }
                 }
             }
         }
+        if (MODE == MODE_FLOW && publish)
+            flow_publish<WARPS>(a, *F, cc.grp, cc.step, cc.n, sv.gen, tiles_per_row, tpu_max, lane);
         --in_flight;
         cons_stage = (cons_stage + 1 == STAGES) ? 0 : cons_stage + 1;
         cons_phase ^= (cons_stage == 0) ? 1u : 0u;
         __syncwarp();
-        issue_one();
     }
     rp.iss_stage = iss_stage;
     rp.cons_stage = cons_stage;
@@ -793,7 +1037,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) step_kernel(const StepArgs a) {
     sv.n = a.n_dev ? __ldcg(a.n_dev) : a.n;
     sv.step = a.step;
     RingPos rp;
-    step_body<DT, WARPS, STAGES, TILE_BYTES, GATHER, SAMPLE, false>(a, sv, ring, rp, warp, lane);
+    step_body<DT, WARPS, STAGES, TILE_BYTES, GATHER, SAMPLE, MODE_STEP>(a, sv, nullptr, ring, rp, warp, lane);
 
     // ---------------- last CTA of the grid: reset the counters, then (decode loop) compact
     __shared__ int s_is_last;
@@ -933,7 +1177,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) loop_kernel(const StepArgs a, c
             sv.ph_tile = L.phase + k * 8 + 5;
         }
 #endif
-        step_body<DT, WARPS, STAGES, TILE_BYTES, GATHER, SAMPLE, true>(a, sv, ring, rp, warp, lane);
+        step_body<DT, WARPS, STAGES, TILE_BYTES, GATHER, SAMPLE, MODE_LOOP>(a, sv, nullptr, ring, rp, warp, lane);
         if (blockIdx.x == 0 && threadIdx.x == 0) CD_PHASE(L, k, 1);  // CTA 0 / warp 0 ran out of work
 #ifdef CD_TUNING
         __syncthreads();
@@ -954,6 +1198,42 @@ __global__ void __launch_bounds__(WARPS * 32, 1) loop_kernel(const StepArgs a, c
             const int kk = k < LOOP_TRACE_STEPS ? k : LOOP_TRACE_STEPS;
             L.trace_t[kk] = global_timer_ns();
             L.trace_n[LOOP_TRACE_STEPS] = k;
+        }
+    }
+}
+
+// ------------------------------------------------------------------ one launch = the whole loop, no barrier
+// cd_decode_loop without a LIMIT.  Every warp is an independent worker: it draws units from whichever row
+// group has a published step with units left (oldest step first, so the groups stay staggered: while one
+// group is between two steps -- last rows being merged, transition looked up, next step published -- the
+// others keep the memory system busy), and returns when every group is finished.  There is no block-wide
+// or grid-wide synchronisation after the ring set-up, and no warp ever waits for a warp that is not
+// running, so the launch needs no co-residency guarantee.
+template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER, bool SAMPLE = false>
+__global__ void __launch_bounds__(WARPS * 32, 1) flow_kernel(const StepArgs a, const FlowArgs F) {
+    using Ring = WarpRing<STAGES, TILE_BYTES>;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    Ring& ring = reinterpret_cast<Ring*>(smem_raw)[warp];
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) mbar_init(smem_u32(&ring.bar[s]), 1);
+        fence_mbar_init();
+    }
+    __syncwarp();
+    const unsigned gen0 = (unsigned)__ldcg(a.ctrs + 3);
+    if (blockIdx.x == 0 && threadIdx.x == 0) atomicMax(F.trace_t + 0, global_timer_ns());
+    StepView sv{};
+    sv.gen = gen0;
+    RingPos rp;
+    step_body<DT, WARPS, STAGES, TILE_BYTES, GATHER, SAMPLE, MODE_FLOW>(a, sv, &F, ring, rp, warp, lane);
+    // ---------------- last CTA to leave: generation for the next launch
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int d = atom_add_acq_rel_gpu(a.ctrs + 1, 1);
+        if (d == (int)gridDim.x - 1) {
+            a.ctrs[1] = 0;
+            a.ctrs[3] = (int)(gen0 + (unsigned)a.max_steps + 1u);
         }
     }
 }

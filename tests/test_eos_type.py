@@ -129,7 +129,7 @@ def _loop_equal(got, want, tol=1e-5, final_state=True):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("mode", ["auto", "per_step"])
+@pytest.mark.parametrize("mode", ["auto", "barrier", "per_step"])
 @pytest.mark.parametrize("gather", [0, 2**30])
 def test_decoding_option_sets_with_eos_greedy_and_sampled(cd, oracle, mode, gather):
     if not torch.cuda.is_available():
@@ -141,7 +141,7 @@ def test_decoding_option_sets_with_eos_greedy_and_sampled(cd, oracle, mode, gath
     dfa = cd.compile_trie(V, labels, device="cuda:0", eos=eos)
     assert (dfa.S, dfa.nnz) == (aut.S, aut.nnz)
     dfa.set_gather_max(gather)
-    dfa.set_loop_mode(cd.LOOP_AUTO if mode == "auto" else cd.LOOP_PER_STEP)
+    dfa.set_loop_mode({"auto": cd.LOOP_AUTO, "barrier": cd.LOOP_BARRIER, "per_step": cd.LOOP_PER_STEP}[mode])
     steps = max(len(l) for l in labels) + 1
     # bias eos a little so that rows stop at inner may-stop states as well as at the longest labels
     logits = [wl.make_logits(11, k, B, V, 2.0, torch.bfloat16, device="cuda:0", bias_tokens=[eos], bias=1.0)

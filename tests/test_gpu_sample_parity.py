@@ -154,7 +154,7 @@ def test_sampled_full_size_c4_batch(cd, oracle):
     steps = [xs[k & 1] for k in range(4)]
     hosts = [host, xs[1].cpu()]
     want = oracle.sample_decode_loop(aut, [hosts[k & 1] for k in range(4)], 1.0, seed=2026)
-    for lm in (cd.LOOP_AUTO, cd.LOOP_PER_STEP):
+    for lm in (cd.LOOP_AUTO, cd.LOOP_BARRIER, cd.LOOP_PER_STEP):
         dfa.set_loop_mode(lm)
         got = cd.decode_loop(dfa, steps)
         for k in ("tokens", "len", "final_state", "done"):
