@@ -270,15 +270,17 @@ CD_API cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, cons
  * If the start state is accepting every row is done with len 0.
  *
  * How it runs (cd_set_loop_mode):
- *   CD_LOOP_AUTO (default)  ONE kernel launch for the whole loop when the device supports it and
- *       B <= 32768; the CTAs stay resident and read step_logits[k] themselves.
- *       - cd_decode_loop: the rows are split into (up to 4) groups of consecutive row ids and every
- *         group is a decode loop of its own: the warp that finalises the last row of a group's step
- *         builds the group's next active list (ascending row id, i.e. the stable order of
- *         cd_compact) and publishes the step; every warp draws work from whichever group has a
- *         published step with units left, oldest step first.  While one group is between two steps
- *         the others keep the memory system busy: no launch, no counter reset, no compaction pass
- *         and no grid-wide barrier between steps.
+ *   CD_LOOP_AUTO (default)  ONE kernel launch for the whole loop -- no set-up kernel before it, no
+ *       copy after it -- when the device supports it and B <= 32768; the CTAs stay resident and read
+ *       step_logits[k] themselves.
+ *       - cd_decode_loop: rows are independent, so no row waits for another one.  The
+ *         unit of scheduling is one decoding step of one row: the warp that finalises step k of a row
+ *         publishes the row's step k + 1 (row, next state, running sum) in a device queue, from which
+ *         every warp draws pieces of row steps in order.  While some rows are between two steps
+ *         (merge, transition look-up) the others keep the memory system busy: no launch, no counter
+ *         reset, no compaction pass and no barrier between steps.  The active set never exists as a
+ *         list; the outputs are indexed by original row id, so the results are those of the stable
+ *         compaction of a6.
  *       - cd_decode_loop_limit (and cd_set_limit): a LIMIT is defined step by step over ALL rows, so
  *         the steps run in lock-step: one cooperative launch, a grid barrier after every step, the
  *         active set a bitmap over original row ids (slot i of a step = its i-th set bit).
@@ -289,18 +291,32 @@ CD_API cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, cons
  *   CD_LOOP_PER_STEP        always one launch per decoding step.
  * All three give the same tokens, lengths, states and done flags bit for bit; sum_logprob_out is
  * bit-identical between CD_LOOP_BARRIER and CD_LOOP_PER_STEP and within the stated tolerance for
- * CD_LOOP_AUTO (rows are split into work units per group, which changes the fp32 summation
- * order); each mode by itself is bitwise reproducible from run to run.
+ * CD_LOOP_AUTO (a row is split into work units by B alone, not by the number of rows still active,
+ * which changes the fp32 summation order); each mode by itself is bitwise reproducible from run to
+ * run.
  * cd_loop_trace returns, for the last loop that ran in a persistent kernel on (dfa, cuda_stream),
  * the number of decoding steps it ran (*steps_out), and for the first min(cap, 256) of them the
- * active rows and the duration in nanoseconds measured on the device (HOST arrays; with row groups
- * step k lasts from the moment its last group was published to the moment step k + 1's was;
- * *steps_out = 0 if that loop took the per-step path).  It synchronises the stream.
+ * rows that took the step and its duration in nanoseconds measured on the device (HOST arrays;
+ * without lock-step, step k lasts from the latest publication of a row's step k to the latest
+ * publication of a row's step k + 1; *steps_out = 0 if that loop took the per-step path).  It
+ * synchronises the stream.
+ *
+ * cd_decode_loop_async is cd_decode_loop without the synchronisation: it only enqueues the loop on
+ * cuda_stream and returns (CD_LOOP_AUTO, no LIMIT: exactly one kernel launch).  The outputs are valid
+ * once the stream has been synchronised; device-side failures of the loops enqueued on (dfa,
+ * cuda_stream) since the last cd_loop_sync are reported by cd_loop_sync, which synchronises the
+ * stream.  step_logits (the HOST array) may be reused as soon as the call returns.  Several loops may
+ * be enqueued back to back on one stream; loops on different streams may run concurrently.
  */
 typedef enum { CD_LOOP_AUTO = 0, CD_LOOP_PER_STEP = 1, CD_LOOP_BARRIER = 2 } cd_loop_mode;
 CD_API cd_status cd_set_loop_mode(cd_dfa_t* dfa, int32_t mode);
 CD_API cd_status cd_loop_trace(const cd_dfa_t* dfa, void* cuda_stream, int32_t cap, int64_t* t_ns_out,
                         int32_t* n_active_out, int32_t* steps_out);
+CD_API cd_status cd_decode_loop_async(const cd_dfa_t* dfa, const void* const* step_logits, cd_dtype dtype,
+                         int64_t ld_elems, int32_t B, int32_t max_steps, int32_t* tokens_out,
+                         int32_t* len_out, int32_t* final_state_out, float* sum_logprob_out,
+                         uint8_t* done_out, void* cuda_stream);
+CD_API cd_status cd_loop_sync(const cd_dfa_t* dfa, void* cuda_stream);
 CD_API cd_status cd_decode_loop(const cd_dfa_t* dfa, const void* const* step_logits, cd_dtype dtype,
                          int64_t ld_elems, int32_t B, int32_t max_steps, int32_t* tokens_out,
                          int32_t* len_out, int32_t* final_state_out, float* sum_logprob_out,

@@ -21,6 +21,9 @@ from .binding import (  # noqa: F401
     compile_list,
     compile_trie,
     decode_loop,
+    decode_loop_async,
+    loop_sync,
+    PreparedLoop,
     decode_loop_cb,
     head_decode_loop_cb,
     decode_loop_host,

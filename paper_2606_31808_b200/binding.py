@@ -19,7 +19,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
     "cd_compile_dfa", "cd_build_trie", "cd_compile_trie", "cd_build_list", "cd_set_loop_mode", "cd_loop_trace", "cd_compile_list", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_set_sampling", "cd_reserve", "cd_step",
-    "cd_transition", "cd_compact", "cd_decode_loop", "cd_set_satisfying", "cd_set_limit", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_probe_read", "cd_decode_loop_cb", "cd_head_decode_loop_cb", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
+    "cd_transition", "cd_compact", "cd_decode_loop", "cd_decode_loop_async", "cd_loop_sync", "cd_set_satisfying", "cd_set_limit", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_probe_read", "cd_decode_loop_cb", "cd_head_decode_loop_cb", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
     "cd_last_error",
 )
 
@@ -363,6 +363,59 @@ def decode_loop(dfa: Dfa, step_logits: Sequence[torch.Tensor], max_steps: Option
                                 _ptr(out["tokens"]), _ptr(out["len"]), _ptr(out["final_state"]),
                                 _ptr(out["sum_logprob"]), _ptr(out["done"]), _stream(dev)))
     return out
+
+
+class PreparedLoop:
+    """The arguments of a cd_decode_loop call marshalled once: run() / enqueue() only make the C call (a decode
+    loop over a small batch lasts tens of microseconds, less than building its ctypes arguments).  The step
+    buffers, the outputs and the stream (torch's current one at construction) are fixed."""
+
+    def __init__(self, dfa: Dfa, step_logits: Sequence[torch.Tensor], max_steps: Optional[int] = None, out=None):
+        dev = dfa.device
+        max_steps = len(step_logits) if max_steps is None else max_steps
+        if max_steps > len(step_logits) or max_steps == 0:
+            raise ValueError("need 1 <= max_steps <= len(step_logits)")
+        x0 = step_logits[0]
+        B, ld, dt = x0.shape[0], x0.stride(0), _dt(x0)
+        for x in step_logits[:max_steps]:
+            if x.dim() != 2 or not x.is_cuda or x.stride(1) != 1 or x.shape[0] != B or x.stride(0) != ld or _dt(x) != dt:
+                raise TypeError("step_logits must share shape, stride and dtype")
+        self.dfa = dfa
+        self._keep = list(step_logits[:max_steps])
+        self._ptrs = (C.c_void_p * max_steps)(*[x.data_ptr() for x in self._keep])
+        self.out = _loop_outputs(B, max_steps, dev) if out is None else out
+        self._stream = _stream(dev)
+        self._args = (dfa._h, self._ptrs, C.c_int(dt), C.c_int64(ld), C.c_int32(B), C.c_int32(max_steps),
+                      _ptr(self.out["tokens"]), _ptr(self.out["len"]), _ptr(self.out["final_state"]),
+                      _ptr(self.out["sum_logprob"]), _ptr(self.out["done"]), self._stream)
+        self._run = lib().cd_decode_loop
+        self._enqueue = lib().cd_decode_loop_async
+
+    def run(self):
+        """cd_decode_loop (synchronises the stream once)."""
+        _check(self._run(*self._args))
+        return self.out
+
+    def enqueue(self):
+        """cd_decode_loop_async: enqueue only; the outputs are valid after sync()."""
+        _check(self._enqueue(*self._args))
+        return self.out
+
+    def sync(self):
+        """cd_loop_sync: synchronise the stream and report the device-side status of the loops enqueued on it."""
+        _check(lib().cd_loop_sync(self.dfa._h, self._stream))
+        return self.out
+
+
+def decode_loop_async(dfa: Dfa, step_logits: Sequence[torch.Tensor], max_steps: Optional[int] = None, out=None):
+    """cd_decode_loop_async: as decode_loop but only enqueued on torch's current stream; call loop_sync(dfa)
+    before reading the outputs."""
+    return PreparedLoop(dfa, step_logits, max_steps, out).enqueue()
+
+
+def loop_sync(dfa: Dfa):
+    """cd_loop_sync on torch's current stream."""
+    _check(lib().cd_loop_sync(dfa._h, _stream(dfa.device)))
 
 
 def head_decode_loop_host(dfa: Dfa, step_hidden_host: Sequence[torch.Tensor], W: torch.Tensor,

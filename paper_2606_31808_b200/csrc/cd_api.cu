@@ -84,8 +84,7 @@ constexpr int tune_int(const char*, int def, int, int) { return def; }
 int units_per_warp() { static const int v = tune_int("CD_UPW", cd::UNITS_PER_WARP, 1, 32); return v; }
 int tpu_max_tiles() { static const int v = tune_int("CD_TPU_MAX", cd::TPU_MAX_BYTES / STEP_TILE, 1, cd::TPU_MAX_BYTES / STEP_TILE); return v; }
 bool use_pdl() { static const int v = tune_int("CD_PDL", 1, 0, 1); return v != 0; }
-int flow_idle_ns() { static const int v = tune_int("CD_IDLE_NS", 32, 0, 100000); return v; }  // 32 / 128 / 512 ns: 648 / 660 / 675 us per c3 loop
-int flow_groups_target() { static const int v = tune_int("CD_GROUPS", 4, 1, cd::FLOW_MAX_GROUPS); return v; }
+int flow_idle_ns() { static const int v = tune_int("CD_IDLE_NS", 32, 0, 100000); return v; }  // sleep between two polls of an unpublished task
 int host_gather_mult() { static const int v = tune_int("CD_HOST_GATHER_CTAS", 4, 1, 64); return v; }  // flat from 2 to 32 (51 GB/s on PCIe Gen5 x16)
 
 // Per (handle, stream) scratch.  Operations on one stream are ordered, so one area per stream
@@ -111,13 +110,10 @@ struct StepBufs {  // sized by rows; replaced as a whole when the area grows
     unsigned long long* trace_t = nullptr;              // [LOOP_TRACE_STEPS + 1]
     int* trace_n = nullptr;                             // [LOOP_TRACE_STEPS + 1]
     unsigned long long* phase = nullptr;                // tuning builds: [LOOP_TRACE_STEPS][8]
-    // flow_kernel (row groups advancing independently)
-    unsigned long long* f_desc = nullptr;                // [FLOW_MAX_GROUPS]
-    unsigned long long* f_list[2] = {nullptr, nullptr};  // [rows + pad]
-    unsigned int* f_listf[2] = {nullptr, nullptr};
-    unsigned long long* f_res = nullptr;
-    unsigned long long* f_resf = nullptr;
-    int* f_fin = nullptr;                                // [FLOW_MAX_GROUPS]
+    // flow_kernel (row tasks)
+    int* f_q = nullptr;                                      // [8] see cd::FlowArgs
+    unsigned long long* f_trace_t[2] = {nullptr, nullptr};  // [LOOP_TRACE_STEPS + 1] each
+    int* f_trace_n[2] = {nullptr, nullptr};
 
     void release() {
         cudaFree(partials); cudaFree(tickets); cudaFree(ctrs);
@@ -125,8 +121,8 @@ struct StepBufs {  // sized by rows; replaced as a whole when the area grows
         for (int i = 0; i < 3; ++i) cudaFree(alive[i]);
         cudaFree(state_new); cudaFree(n_active); cudaFree(token); cudaFree(logprob); cudaFree(done);
         cudaFree(bar); cudaFree(trace_t); cudaFree(trace_n); cudaFree(phase);
-        cudaFree(f_desc); cudaFree(f_res); cudaFree(f_resf); cudaFree(f_fin);
-        for (int i = 0; i < 2; ++i) { cudaFree(f_list[i]); cudaFree(f_listf[i]); }
+        cudaFree(f_q);
+        for (int i = 0; i < 2; ++i) { cudaFree(f_trace_t[i]); cudaFree(f_trace_n[i]); }
         *this = StepBufs();
     }
 };
@@ -137,7 +133,11 @@ struct Scratch {
     int loop_steps_cap = 0;
     int* loop_work = nullptr;
     const void** loop_ptrs = nullptr;
-    bool trace_valid = false;  // the last loop on this stream ran in loop_kernel
+    int trace_src = 0;  // the last loop on this stream ran in: 0 step_kernel launches, 1 loop_kernel, 2 flow_kernel
+    unsigned long long* f_task = nullptr;  // flow_kernel: the task queue, [f_task_cap][4]
+    long long f_task_cap = 0;
+    int* h_status = nullptr;  // flow_kernel: [4] pinned, device-mapped host ints ([0] errors of the last loop, [1] its generation)
+    int* d_status = nullptr;  //   the same memory as the device sees it
     // host-buffer loops
     void* stage[2] = {nullptr, nullptr};
     size_t stage_bytes[2] = {0, 0};
@@ -168,7 +168,8 @@ struct Scratch {
     void release() {
         b.release();
         release_head();
-        cudaFree(loop_work); cudaFree(loop_ptrs);
+        cudaFree(loop_work); cudaFree(loop_ptrs); cudaFree(f_task);
+        if (h_status) cudaFreeHost(h_status);
         for (int i = 0; i < 2; ++i) cudaFree(stage[i]);
         cudaFree(out_i32);
         if (copy_stream) cudaStreamDestroy(copy_stream);
@@ -282,15 +283,6 @@ long long step_units_cap(const cd_dfa* d, long long n) {
     return (a > b ? a : b) + 64;
 }
 
-// flow_kernel: B rows as G groups of Bg consecutive rows (Bg a multiple of 32)
-void flow_plan(int B, int* G, int* Bg) {
-    const int gt = flow_groups_target();
-    int bg = ((B + gt - 1) / gt + 31) / 32 * 32;
-    if (bg < 32) bg = 32;
-    *Bg = bg;
-    *G = (B + bg - 1) / bg;
-}
-
 template <typename T>
 cudaError_t dev_alloc(T** p, size_t count) {
     return cudaMalloc(reinterpret_cast<void**>(p), sizeof(T) * (count ? count : 1));
@@ -299,15 +291,8 @@ cudaError_t dev_alloc(T** p, size_t count) {
 // Allocates a complete set of step buffers for `rows` rows; on failure nothing is kept.
 cd_status alloc_step_bufs(const cd_dfa* d, int rows, StepBufs* out) {
     StepBufs n;
-    long long units = step_units_cap(d, rows);
-    {   // flow_kernel: every group has a region of its own in the partial buffer
-        int G = 1, Bg = rows;
-        flow_plan(rows, &G, &Bg);
-        const long long fu = (long long)G * step_units_cap(d, Bg);
-        if (fu > units) units = fu;
-    }
+    const long long units = step_units_cap(d, rows);
     const size_t nwords = ((size_t)rows + 31) / 32;
-    const size_t frows = (size_t)rows + 32 * cd::FLOW_MAX_GROUPS;
     cudaError_t e = cudaSuccess;
     auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
     A(dev_alloc(&n.partials, (size_t)units));
@@ -327,16 +312,14 @@ cd_status alloc_step_bufs(const cd_dfa* d, int rows, StepBufs* out) {
     A(dev_alloc(&n.bar, 4));
     A(dev_alloc(&n.trace_t, (size_t)cd::LOOP_TRACE_STEPS + 1));
     A(dev_alloc(&n.trace_n, (size_t)cd::LOOP_TRACE_STEPS + 1));
-    A(dev_alloc(&n.f_desc, (size_t)cd::FLOW_MAX_GROUPS));
-    A(dev_alloc(&n.f_fin, (size_t)cd::FLOW_MAX_GROUPS));
-    A(dev_alloc(&n.f_res, frows));
-    A(dev_alloc(&n.f_resf, frows));
+    A(dev_alloc(&n.f_q, 8));
     for (int i = 0; i < 2; ++i) {
-        A(dev_alloc(&n.f_list[i], frows));
-        A(dev_alloc(&n.f_listf[i], frows));
+        A(dev_alloc(&n.f_trace_t[i], (size_t)cd::LOOP_TRACE_STEPS + 1));
+        A(dev_alloc(&n.f_trace_n[i], (size_t)cd::LOOP_TRACE_STEPS + 1));
+        if (e == cudaSuccess) e = cudaMemset(n.f_trace_t[i], 0, sizeof(unsigned long long) * ((size_t)cd::LOOP_TRACE_STEPS + 1));
+        if (e == cudaSuccess) e = cudaMemset(n.f_trace_n[i], 0, sizeof(int) * ((size_t)cd::LOOP_TRACE_STEPS + 1));
     }
-    if (e == cudaSuccess) e = cudaMemset(n.f_res, 0, sizeof(unsigned long long) * frows);   // tags start at 0
-    if (e == cudaSuccess) e = cudaMemset(n.f_resf, 0, sizeof(unsigned long long) * frows);
+    if (e == cudaSuccess) e = cudaMemset(n.f_q, 0, sizeof(int) * 8);  // (the stop word 0 is never a launch generation)
 #ifdef CD_TUNING
     A(dev_alloc(&n.phase, (size_t)cd::LOOP_TRACE_STEPS * 8));
 #endif
@@ -365,9 +348,6 @@ cd_status get_scratch(const cd_dfa* cd_, cudaStream_t stream, int rows, Scratch*
         return fail(CD_ERR_ARG, "rows (%d) * tiles per row overflows the unit index", rows);
     Scratch& s = d->scratch[stream];
     if (rows < 1) rows = 1;
-    // (the group plan of flow_kernel depends on the row count of the CALL, the partial buffer is sized for the
-    // capacity: a smaller call never needs more units per group than the capacity's plan provides -- see
-    // alloc_step_bufs; calls are checked against cap_units when they are launched)
     if (s.b.cap_rows < rows) {
         // growing: the new set is complete before the old one is touched; then wait for the work that
         // still uses the old buffers and drop them
@@ -383,7 +363,7 @@ cd_status get_scratch(const cd_dfa* cd_, cudaStream_t stream, int rows, Scratch*
         }
         s.b.release();
         s.b = fresh;
-        s.trace_valid = false;
+        s.trace_src = 0;
     }
     *out = &s;
     return CD_OK;
@@ -775,8 +755,7 @@ LimitArgs resolve_limit(const Settings& cfg, const LimitArgs& explicit_lim = Lim
 // persist: also initialise the bitmaps / states / counters of loop_kernel
 cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, int* tokens_out, int* len_out,
                            int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream,
-                           const LimitArgs& lim = LimitArgs(), int persist = 0 /*0 per step, 1 loop_kernel, 2 flow_kernel*/,
-                           int grid = 0, int dtype = CD_BF16) {
+                           const LimitArgs& lim = LimitArgs(), bool persist = false) {
     long long work = (long long)B * (max_steps > 0 ? max_steps : 1);
     long long blocks = (work + 255) / 256;
     if (blocks < 1) blocks = 1;
@@ -794,28 +773,11 @@ cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, in
     a.sat_ctr = lim.sat_ctr;
     a.limit = lim.limit;
     a.ctrs = s->b.ctrs;
-    if (persist == 1) {
+    if (persist) {
         for (int i = 0; i < 3; ++i) a.alive[i] = s->b.alive[i];
         for (int i = 0; i < 2; ++i) a.state2[i] = s->b.state2[i];
         a.work = s->loop_work;
         a.bar = s->b.bar;
-    } else if (persist == 2) {
-        flow_plan(B, &a.G, &a.Bg);
-        a.work = s->loop_work;
-        a.work_len = a.G * max_steps;
-        a.desc = s->b.f_desc;
-        a.list0 = s->b.f_list[0];
-        a.listf0 = s->b.f_listf[0];
-        a.fin = s->b.f_fin;
-        a.trace_t = s->b.trace_t;
-        a.trace_n = s->b.trace_n;
-        a.trace_len = cd::LOOP_TRACE_STEPS + 1;
-        const int T = tiles_per_row(d->dev.V, dtype);
-        for (int g = 0; g < a.G; ++g) {
-            const int ng = (g + 1) * a.Bg <= B ? a.Bg : B - g * a.Bg;
-            // unit size as if all G groups had this many rows: the groups share the warps
-            a.tpu0[g] = cd::tiles_per_unit((long long)ng * a.G, T, (long long)grid * STEP_WARPS, tpu_max_tiles(), units_per_warp());
-        }
     } else {
         a.row_ids = s->b.row_ids[0];
         a.state = s->b.state[0];
@@ -824,7 +786,7 @@ cd_status launch_loop_init(const cd_dfa* d, Scratch* s, int B, int max_steps, in
     cd::loop_init_kernel<<<(int)blocks, 256, 0, stream>>>(a);
     CU(cudaGetLastError());
     g_launches.fetch_add(1, std::memory_order_relaxed);
-    s->trace_valid = false;
+    s->trace_src = 0;
     return CD_OK;
 }
 
@@ -901,16 +863,68 @@ cd_status enqueue_persistent_loop(const cd_dfa* d, const Settings& cfg, Scratch*
     const int grid = step_grid(d, B, dtype);
     const cd_status st = dtype == CD_BF16 ? launch_loop_v<cd::DT_BF16>(a, L, grid, stream, launched)
                                           : launch_loop_v<cd::DT_F32>(a, L, grid, stream, launched);
-    if (st == CD_OK && *launched) s->trace_valid = true;
+    if (st == CD_OK && *launched) s->trace_src = 1;
     return st;
 }
 
-// The whole loop in ONE launch of flow_kernel (no LIMIT: a LIMIT is defined step by step over all rows, which
-// needs the lock-step of loop_kernel).
+cd_status get_loop_scratch(Scratch* s, int max_steps, cudaStream_t stream);
+
+// flow_kernel: tiles per unit of a B-row loop (fixed for the launch) and whether the loop fits its index ranges
+int flow_tpu(const cd_dfa* d, int B, int dtype, int grid) {
+    return cd::tiles_per_unit(B, tiles_per_row(d->dev.V, dtype), (long long)grid * STEP_WARPS, tpu_max_tiles(), units_per_warp());
+}
+constexpr long long FLOW_TASK_CAP_MAX = (256ll << 20) / 32;  // at most 256 MiB of task queue
+
+bool flow_loop_possible(const cd_dfa* d, int B, int max_steps, int dtype) {
+    const long long tasks = (long long)B * max_steps;
+    if (tasks - B > FLOW_TASK_CAP_MAX) return false;
+    const int T = tiles_per_row(d->dev.V, dtype);
+    const int tpu = flow_tpu(d, B, dtype, step_grid(d, B, dtype));
+    const long long P = (T + tpu - 1) / tpu;
+    return tasks * P + (long long)d->num_sms * STEP_WARPS * 4 < 0x7FFFFFFFLL;  // the unit counter is 32 bits wide
+}
+
+// status word of the loops (pinned, device-mapped host memory)
+cd_status get_status_word(Scratch* s) {
+    if (!s->h_status) {
+        CU(cudaHostAlloc(reinterpret_cast<void**>(&s->h_status), sizeof(int) * 4, cudaHostAllocMapped | cudaHostAllocPortable));
+        std::memset(s->h_status, 0, sizeof(int) * 4);
+        if (cudaHostGetDevicePointer(reinterpret_cast<void**>(&s->d_status), s->h_status, 0) != cudaSuccess) {
+            cudaFreeHost(s->h_status);
+            s->h_status = nullptr;
+            return fail(CD_ERR_CUDA, "mapped status word");
+        }
+    }
+    return CD_OK;
+}
+
+// task queue + status word of flow_kernel
+cd_status get_flow_scratch(Scratch* s, long long tasks, cudaStream_t stream) {
+    const cd_status st = get_status_word(s);
+    if (st != CD_OK) return st;
+    if (s->f_task_cap >= tasks) return CD_OK;
+    unsigned long long* q = nullptr;
+    const long long cap = tasks < 1024 ? 1024 : tasks;
+    if (dev_alloc(&q, (size_t)cap * 4) != cudaSuccess) return fail(CD_ERR_OOM, "task queue for %lld row steps", tasks);
+    if (cudaMemset(q, 0, sizeof(unsigned long long) * 4 * (size_t)cap) != cudaSuccess) {  // generation tags start at 0
+        cudaFree(q);
+        return fail(CD_ERR_CUDA, "task queue");
+    }
+    if (s->f_task) cudaStreamSynchronize(stream);
+    cudaFree(s->f_task);
+    s->f_task = q;
+    s->f_task_cap = cap;
+    return CD_OK;
+}
+
+// The whole loop in ONE launch of flow_kernel and nothing else: no set-up kernel, no copy afterwards (no LIMIT:
+// a LIMIT is defined step by step over all rows, which needs the lock-step of loop_kernel).
 cd_status enqueue_flow_loop(const cd_dfa* d, const Settings& cfg, Scratch* s, const void* const* step_logits,
                             cd_dtype dtype, long long ld, int B, int max_steps, int* tokens_out, int* len_out,
-                            int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream, int grid) {
-    RangeGuard range("cd decode loop (persistent kernel, row groups)");
+                            int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream) {
+    RangeGuard range("cd decode loop (persistent kernel, row tasks)");
+    cd_status st = get_flow_scratch(s, (long long)B * (max_steps - 1), stream);
+    if (st != CD_OK) return st;
     LoopExtras x;
     x.tokens = tokens_out;
     x.len = len_out;
@@ -920,32 +934,42 @@ cd_status enqueue_flow_loop(const cd_dfa* d, const Settings& cfg, Scratch* s, co
     x.max_steps = max_steps;
     cd::StepArgs a = make_step_args(d, cfg, s, dtype, ld, &x);
     a.n = B;
+    const int grid = step_grid(d, B, dtype);
     cd::FlowArgs F{};
     if (max_steps <= cd::LOOP_PARAM_STEPS) {
         for (int k = 0; k < max_steps; ++k) F.step_ptrs[k] = step_logits[k];
     } else {
+        st = get_loop_scratch(s, max_steps, stream);
+        if (st != CD_OK) return st;
         CU(cudaMemcpyAsync(s->loop_ptrs, step_logits, sizeof(void*) * (size_t)max_steps, cudaMemcpyHostToDevice, stream));
         F.step_ptrs_dev = s->loop_ptrs;
     }
     F.B = B;
-    flow_plan(B, &F.G, &F.Bg);
-    F.desc = s->b.f_desc;
+    F.tpu = flow_tpu(d, B, dtype, grid);
+    F.start = d->start;
+    F.task = s->f_task;
+    F.cap = s->f_task_cap;
+    F.q = s->b.f_q;
     for (int i = 0; i < 2; ++i) {
-        F.list[i] = s->b.f_list[i];
-        F.listf[i] = s->b.f_listf[i];
+        F.trace_t[i] = s->b.f_trace_t[i];
+        F.trace_n[i] = s->b.f_trace_n[i];
     }
-    F.res = s->b.f_res;
-    F.resf = s->b.f_resf;
-    F.fin = s->b.f_fin;
-    F.work = s->loop_work;
-    F.pcap = step_units_cap(d, F.Bg);
-    F.trace_t = s->b.trace_t;
-    F.trace_n = s->b.trace_n;
-    if ((long long)F.G * F.pcap > s->b.cap_units) return fail(CD_ERR_INTERNAL, "partial buffer too small for %d groups", F.G);
-    const cd_status st = dtype == CD_BF16 ? launch_flow_v<cd::DT_BF16>(a, F, grid, stream)
-                                          : launch_flow_v<cd::DT_F32>(a, F, grid, stream);
-    if (st == CD_OK) s->trace_valid = true;
+    F.host_status = s->d_status;
+    st = dtype == CD_BF16 ? launch_flow_v<cd::DT_BF16>(a, F, grid, stream) : launch_flow_v<cd::DT_F32>(a, F, grid, stream);
+    if (st == CD_OK) s->trace_src = 2;
     return st;
+}
+
+// End of a flow_kernel loop: the one stream synchronisation the loops promise; the kernel has put its status
+// into mapped host memory.
+cd_status finish_flow_loop(Scratch* s, cudaStream_t stream) {
+    CU(cudaStreamSynchronize(stream));
+    if (!s->h_status) return CD_OK;
+    const int err = reinterpret_cast<volatile int*>(s->h_status)[0];
+    reinterpret_cast<volatile int*>(s->h_status)[0] = 0;
+    if (err != 0)
+        return fail(CD_ERR_INTERNAL, "%d device-side consistency failures (state out of range, token missing from the CSR or a row that never finished)", err);
+    return CD_OK;
 }
 
 std::mutex& coop_mutex(int dev) {
@@ -1202,7 +1226,7 @@ cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, const int32
 static cd_status decode_loop_impl(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
                                   int32_t B, int32_t max_steps, int32_t* tokens_out, int32_t* len_out,
                                   int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out,
-                                  const LimitArgs& lim_in, void* cuda_stream) {
+                                  const LimitArgs& lim_in, void* cuda_stream, bool sync = true) {
     if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
     if (B < 0 || max_steps < 0) return fail(CD_ERR_ARG, "B / max_steps < 0");
     const Settings cfg = settings_of(d);
@@ -1225,30 +1249,26 @@ static cd_status decode_loop_impl(const cd_dfa_t* d, const void* const* step_log
     st = get_scratch(d, stream, B, &s);
     if (st != CD_OK) return st;
     bool persist = persistent_loop_possible(d, cfg, B, max_steps);
-    // no LIMIT: the barrier-free kernel (row groups advance independently); with a LIMIT, or on request, the
-    // lock-step kernel (a LIMIT is defined step by step over ALL rows)
-    const bool flow = persist && !lim.sat_ctr && cfg.loop_mode != CD_LOOP_BARRIER;
+    // no LIMIT: the barrier-free kernel (every row advances through its steps independently); with a LIMIT, or
+    // on request, the lock-step kernel (a LIMIT is defined step by step over ALL rows)
+    if (persist && !lim.sat_ctr && cfg.loop_mode != CD_LOOP_BARRIER && flow_loop_possible(d, B, max_steps, dtype)) {
+        st = enqueue_flow_loop(d, cfg, s, step_logits, dtype, ld_elems, B, max_steps, tokens_out, len_out,
+                               final_state_out, sum_logprob_out, done_out, stream);
+        if (st != CD_OK) return st;
+        return sync ? finish_flow_loop(s, stream) : CD_OK;
+    }
+    if (!sync) persist = false;  // a lock-step loop holds the device's cooperative-launch lock until it has finished
     // Two lock-step loops must never share the SMs: each waits at its grid barrier for CTAs that the other
     // one keeps from being scheduled.  Within this process they are serialised per device (the loop
     // synchronises its stream before returning anyway).
     std::unique_lock<std::mutex> coop_lock;
-    if (persist && !flow) coop_lock = std::unique_lock<std::mutex>(coop_mutex(d->device));
     if (persist) {
-        st = get_loop_scratch(s, flow ? max_steps * cd::FLOW_MAX_GROUPS : max_steps, stream);
+        coop_lock = std::unique_lock<std::mutex>(coop_mutex(d->device));
+        st = get_loop_scratch(s, max_steps, stream);
         if (st != CD_OK) return st;
-    }
-    if (flow) {
-        const int grid = step_grid(d, B, dtype);
-        st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out,
-                              stream, lim, 2, grid, dtype);
-        if (st != CD_OK) return st;
-        st = enqueue_flow_loop(d, cfg, s, step_logits, dtype, ld_elems, B, max_steps, tokens_out, len_out,
-                               final_state_out, sum_logprob_out, done_out, stream, grid);
-        if (st != CD_OK) return st;
-    } else if (persist) {
         // both forms of the set-up are cheap; the persistent one is tried first and tells whether its CTAs fit
         st = launch_loop_init(d, s, B, max_steps, tokens_out, len_out, final_state_out, sum_logprob_out, done_out,
-                              stream, lim, 1);
+                              stream, lim, true);
         if (st != CD_OK) return st;
         bool launched = false;
         st = enqueue_persistent_loop(d, cfg, s, step_logits, dtype, ld_elems, B, max_steps, tokens_out, len_out,
@@ -1267,7 +1287,40 @@ static cd_status decode_loop_impl(const cd_dfa_t* d, const void* const* step_log
                 if (st != CD_OK) return st;
             }
     }
-    return finish_loop(s, stream, persist && !flow);
+    if (!sync) {  // the loop's error count joins the status word cd_loop_sync reads
+        st = get_status_word(s);
+        if (st != CD_OK) return st;
+        cd::fold_status_kernel<<<1, 1, 0, stream>>>(s->b.ctrs, s->d_status);
+        CU(cudaGetLastError());
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        return CD_OK;
+    }
+    return finish_loop(s, stream, persist);
+}
+
+cd_status cd_decode_loop_async(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
+                               int32_t B, int32_t max_steps, int32_t* tokens_out, int32_t* len_out,
+                               int32_t* final_state_out, float* sum_logprob_out, uint8_t* done_out, void* cuda_stream) {
+    return decode_loop_impl(d, step_logits, dtype, ld_elems, B, max_steps, tokens_out, len_out, final_state_out,
+                            sum_logprob_out, done_out, LimitArgs(), cuda_stream, false);
+}
+
+cd_status cd_loop_sync(const cd_dfa_t* d, void* cuda_stream) {
+    if (!d) return fail(CD_ERR_ARG, "dfa is NULL");
+    DeviceGuard guard(d->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    cd_dfa* dm = const_cast<cd_dfa*>(d);
+    Scratch* s = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(dm->mu);
+        auto it = dm->scratch.find(stream);
+        if (it != dm->scratch.end()) s = &it->second;
+    }
+    if (!s) {
+        CU(cudaStreamSynchronize(stream));
+        return CD_OK;
+    }
+    return finish_flow_loop(s, stream);
 }
 
 cd_status cd_decode_loop(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
@@ -1289,13 +1342,20 @@ cd_status cd_loop_trace(const cd_dfa_t* d, void* cuda_stream, int32_t cap, int64
     {
         std::lock_guard<std::mutex> lk(dm->mu);
         auto it = dm->scratch.find(stream);
-        if (it != dm->scratch.end() && it->second.trace_valid) {
+        if (it != dm->scratch.end() && it->second.trace_src == 1) {
             tt = it->second.b.trace_t;
             tn = it->second.b.trace_n;
+        } else if (it != dm->scratch.end() && it->second.trace_src == 2) {
+            // flow_kernel: the buffers of the last launch are the ones the launch counter's parity no longer names
+            int par = 0;
+            CU(cudaMemcpyAsync(&par, it->second.b.f_q + 5, sizeof(int), cudaMemcpyDeviceToHost, stream));
+            CU(cudaStreamSynchronize(stream));
+            tt = it->second.b.f_trace_t[(par & 1) ^ 1];
+            tn = it->second.b.f_trace_n[(par & 1) ^ 1];
         }
     }
     *steps_out = 0;
-    if (!tt) return CD_OK;  // the last loop on this stream did not run in the persistent kernel
+    if (!tt) return CD_OK;  // the last loop on this stream did not run in a persistent kernel
     std::vector<unsigned long long> ht((size_t)cd::LOOP_TRACE_STEPS + 1);
     std::vector<int> hn((size_t)cd::LOOP_TRACE_STEPS + 1);
     CU(cudaMemcpyAsync(ht.data(), tt, sizeof(unsigned long long) * ht.size(), cudaMemcpyDeviceToHost, stream));
@@ -1304,7 +1364,7 @@ cd_status cd_loop_trace(const cd_dfa_t* d, void* cuda_stream, int32_t cap, int64
     int steps = hn[cd::LOOP_TRACE_STEPS];
     if (steps > cd::LOOP_TRACE_STEPS) steps = cd::LOOP_TRACE_STEPS;
     *steps_out = steps;
-    // (row groups: a group that finishes early stops contributing to later entries -- keep the times monotone)
+    // (row tasks: entry k is the latest publication of a task of step k -- keep the times monotone)
     for (int k = 1; k <= steps; ++k)
         if (ht[(size_t)k] < ht[(size_t)k - 1]) ht[(size_t)k] = ht[(size_t)k - 1];
     for (int k = 0; k < steps && k < cap; ++k) {

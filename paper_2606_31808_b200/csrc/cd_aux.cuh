@@ -214,16 +214,6 @@ struct LoopInitArgs {
     int* state2[2];
     int* work;
     int* bar;
-    // flow_kernel (all NULL otherwise): G groups of Bg rows; step 0 of every group is published here
-    int G, Bg, work_len;
-    unsigned long long* desc;
-    unsigned long long* list0;
-    unsigned int* listf0;
-    int* fin;
-    int tpu0[8];  // tiles per unit of step 0 of each group (cd::tiles_per_unit on the host: it depends on the grid)
-    unsigned long long* trace_t;
-    int* trace_n;
-    int trace_len;
 };
 
 __global__ void loop_init_kernel(const LoopInitArgs a) {
@@ -253,29 +243,17 @@ __global__ void loop_init_kernel(const LoopInitArgs a) {
         for (long long k = tid; k < a.max_steps; k += nth) a.work[k] = 0;
         if (tid < 3) a.bar[tid] = 0;
     }
-    if (a.desc) {
-        for (long long r = tid; r < B; r += nth) {
-            a.list0[r] = (unsigned long long)(unsigned)r | ((unsigned long long)(unsigned)a.start << 32);
-            a.listf0[r] = 0u;
-        }
-        for (long long k = tid; k < a.work_len; k += nth) a.work[k] = 0;
-        for (long long k = tid; k < a.trace_len; k += nth) {
-            a.trace_t[k] = 0ull;
-            a.trace_n[k] = (k == 0 && !none) ? B : 0;
-        }
-        if (tid < a.G) {
-            const int g = (int)tid;
-            const int ng = (g + 1) * a.Bg <= B ? a.Bg : B - g * a.Bg;
-            a.fin[g] = 0;
-            a.desc[g] = none ? ~0ull
-                             : ((unsigned long long)0u | ((unsigned long long)(unsigned)ng << 24) |
-                                ((unsigned long long)(unsigned)a.tpu0[g] << 48));
-        }
-    }
     if (tid == 0) {
         if (a.n_active) *a.n_active = none ? 0 : B;
         a.ctrs[2] = 0;
     }
+}
+
+// cd_decode_loop_async on the per-step path: the loop's error count joins the status word the host reads in
+// cd_loop_sync (pinned, device-mapped host memory).
+__global__ void fold_status_kernel(const int* __restrict__ ctrs, int* host_status) {
+    const int err = __ldcg(ctrs + 2);
+    if (err) atomicAdd_system(host_status, err);
 }
 
 // Host-buffer loop (cd_decode_loop_host) when the caller's logits are in pinned, device-mapped host

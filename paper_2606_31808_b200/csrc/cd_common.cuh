@@ -265,6 +265,12 @@ __device__ __forceinline__ unsigned long long ld_relaxed_gpu_u64(const unsigned 
     return v;
 }
 
+__device__ __forceinline__ int ld_relaxed_gpu_s32(const int* p) {
+    int v;
+    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
 // ---------------------------------------------------------------- stable compaction
 // Active-row compaction by one CTA: every thread takes 4 consecutive slots,
 // keep flags are counted per thread, prefix-summed over the warp with shuffles, over the warps

@@ -184,6 +184,8 @@ struct StepView {
     const uint32_t* s_bits;
     const int* s_pref;  // exclusive prefix of the popcounts, [nwords + 1]
     int nwords;
+    unsigned long long* trace_t;  // flow_kernel: the trace buffers of this launch
+    int* trace_n;
     unsigned long long* ph_first_fin;  // tuning builds: earliest / latest row finalisation of the step
     unsigned long long* ph_last_fin;
     unsigned long long* ph_tile;  // tuning builds: [0] earliest (complemented), [1] latest first-tile arrival over the warps
@@ -197,46 +199,49 @@ struct __align__(16) TileMeta {
     long long csr_lo;  // row_ptr[st]
     int csr_len;       // row_ptr[st + 1] - row_ptr[st]
     int lrow;          // row of the logits buffer
-    // flow_kernel: the (group, step) this tile belongs to -- a warp's ring may hold tiles of several
-    int step, n, tpu, grp;
+    // flow_kernel: the step this tile belongs to (a warp's ring may hold tiles of several) and the row's running
+    // sum of log-probs before it (fp32 bits; travels with the task)
+    int step;
+    unsigned sumbits;
+    int pad[2];
 };
 
 constexpr int MODE_STEP = 0;  // step_kernel: one launch = one step
 constexpr int MODE_LOOP = 1;  // loop_kernel: whole loop, grid barrier between steps (LIMIT loops)
 constexpr int MODE_FLOW = 2;  // flow_kernel: whole loop, row groups advance independently (no barrier)
 
-// flow_kernel (cd_decode_loop without a LIMIT): the rows are split into G groups of Bg consecutive
-// original row ids, and every group is a decode loop of its own whose steps are published one by one:
-//   desc[g]      {step:24 | n:24 | tpu:16} of the step whose units may be drawn now (DONE when the group is finished);
-//                written with release by the warp that finalised the LAST row of the previous step of the group,
-//                read with acquire by every warp before it draws a unit of that step
-//   list[k&1]    [G*Bg] {row | state << 32}: the active rows of step k of each group, ascending row id (the stable
-//                order of a6); listf[k&1] the running sum of log-probs of those rows (fp32 bits)
-//   res / resf   [G*Bg] results of the running step by slot: {tag | done << 31 | next state}, {tag | new sum bits};
-//                tag = launch generation + step, so a word is either stale or complete (as the partial slots)
-//   fin[g]       rows finalised in the running step (relaxed counter: whoever brings it to n publishes the next step)
-//   work         [G][max_steps] unit counters
-// Nothing in it waits for a warp that is not running: units are only ever drawn by running warps.
+// flow_kernel (cd_decode_loop without a LIMIT): rows are independent, so nothing makes row r
+// wait at step k for the other rows.  The unit of scheduling is a TASK = one decoding step of one row:
+//   tasks 0 .. B-1 are implicit: (row q, start state, step 0, sum 0) -- nothing is read to start them;
+//   task B + i is the i-th entry of `task`: four self-validating words {launch generation : 32 | payload : 32}
+//       [0] original row id  [1] automaton state  [2] running sum of log-probs (fp32 bits)  [3] step
+//     written (relaxed, no fence) by the warp that finalised the row's previous step, at the index it drew from
+//     q[1]; a word is either stale (older generation) or complete.
+//   Every task is split into the same P units (P fixed for the launch from B: the split of a row, hence the
+//   order of its fp32 sums, never depends on timing -- results are bitwise reproducible).  Unit u = atomicAdd on
+//   q[0]; it belongs to task u / P.  A warp whose next unit belongs to a task that is not published yet keeps
+//   consuming what its ring holds, then polls the entry (and the stop word).  Units are only ever drawn by
+//   running warps and every published task's units are drawn before any unit of a later task, so nothing waits
+//   for a warp that is not running: the launch needs no co-residency guarantee and two loops may share a device.
+//   q[2] counts the rows that left the loop (accepted, truncated at max_steps, failed); whoever brings it to B
+//   stores the launch generation into q[3], the stop word.  The last CTA to leave resets q[0..2], reports the
+//   error count q[4] to host_status (pinned, mapped host memory: no copy after the loop) and counts the launch
+//   in q[5], whose parity selects the trace buffers (the other pair is cleared for the next launch).
+// No set-up kernel: a row's outputs (len, final state, sum, done, the -1 padding of its token history) are
+// written by the warp that finalises its last step.
 struct FlowArgs {
     const void* step_ptrs[LOOP_PARAM_STEPS];
     const void* const* step_ptrs_dev;
-    int B, G, Bg;
-    unsigned long long* desc;
-    unsigned long long* list[2];
-    unsigned int* listf[2];
-    unsigned long long* res;
-    unsigned long long* resf;
-    int* fin;
-    int* work;
-    long long pcap;  // partial slots per group
-    unsigned long long* trace_t;  // [LOOP_TRACE_STEPS + 1] time at which the last group published step k; [steps] = exit
-    int* trace_n;                 // [LOOP_TRACE_STEPS] active rows of step k over all groups; [LOOP_TRACE_STEPS] = steps run
+    int B;
+    int tpu;    // tiles per unit
+    int start;  // start state
+    unsigned long long* task;  // [cap][4]
+    long long cap;             // entries of `task`
+    int* q;                    // [0] units drawn [1] tasks published [2] rows finished [3] stop word [4] errors [5] launches
+    unsigned long long* trace_t[2];  // [LOOP_TRACE_STEPS + 1] latest publication of a task of step k; [steps] = exit
+    int* trace_n[2];                 // [LOOP_TRACE_STEPS] rows that ran step k; [LOOP_TRACE_STEPS] = steps run
+    int* host_status;                // [0] errors of the loops since the host last cleared it
 };
-constexpr unsigned long long FLOW_DONE = ~0ull;
-constexpr int FLOW_MAX_GROUPS = 8;
-__host__ __device__ inline unsigned long long flow_pack(int step, int n, int tpu) {
-    return (unsigned long long)(unsigned)step | ((unsigned long long)(unsigned)n << 24) | ((unsigned long long)(unsigned)tpu << 48);
-}
 
 template <int STAGES, int TILE_BYTES>
 struct __align__(128) WarpRing {
@@ -245,7 +250,6 @@ struct __align__(128) WarpRing {
     TileMeta meta[STAGES];
     unsigned long long bar[STAGES];
     unsigned short list[SAMPLE_LIST_CAP];  // SAMPLE: positions of a tile's allowed elements, compacted
-    int want[FLOW_MAX_GROUPS];             // flow_kernel: first step of each group this warp has not seen exhausted
 };
 
 // tiles per unit for n active rows (host mirrors this in cd_api.cu: step_units_cap)
@@ -282,65 +286,19 @@ __device__ __forceinline__ int mask_rank(const DfaDev& dfa, int st, int t, int l
     return base + c;
 }
 
-// flow_kernel: every row of step `step` of group `grp` is final -- build the group's next step.  Warp-
-// cooperative.  The results of the step were stored by the rows' finalisers before their (relaxed) count,
-// so they are on their way: poll until every tag is current.  Survivors keep their order (ascending row
-// id: the stable compaction of a6).  The new step is published with a release store of its descriptor.
-template <int WARPS>
-__device__ __forceinline__ void flow_publish(const StepArgs& a, const FlowArgs& F, int grp, int step, int n, unsigned gen0,
-                                             int tiles_per_row, int tpu_max, int lane) {
-    const int kk = step + 1;
-    const unsigned long long tag = (unsigned long long)(gen0 + (unsigned)step) << 32;
-    const long long off = (long long)grp * F.Bg;
-    const unsigned long long* cur = F.list[step & 1] + off;
-    unsigned long long* nxt = F.list[kk & 1] + off;
-    unsigned int* nxtf = F.listf[kk & 1] + off;
-    int base = 0;
-    constexpr int U = 4;  // chunks of 32 slots in flight
-#pragma unroll 1
-    for (int i0 = 0; i0 < n; i0 += 32 * U) {
-        unsigned long long r[U], f[U], e[U];
-#pragma unroll
-        for (int q = 0; q < U; ++q) {
-            const int i = i0 + q * 32 + lane;
-            r[q] = f[q] = tag;
-            e[q] = 0;
-            if (i < n) {
-                e[q] = ld_relaxed_gpu_u64(cur + i);
-                int spins = 0;
-                do {
-                    r[q] = ld_relaxed_gpu_u64(F.res + off + i);
-                    f[q] = ld_relaxed_gpu_u64(F.resf + off + i);
-                } while (((r[q] ^ tag) >> 32 || (f[q] ^ tag) >> 32) && ++spins < MERGE_SPIN_LIMIT);
-            }
-        }
-#pragma unroll
-        for (int q = 0; q < U; ++q) {
-            const int i = i0 + q * 32 + lane;
-            const bool keep = (i < n) && (((unsigned)r[q] >> 31) == 0u) && !((r[q] ^ tag) >> 32);
-            const unsigned b = __ballot_sync(FULL, keep);
-            if (keep) {
-                const int p = base + __popc(b & ((1u << lane) - 1u));
-                nxt[p] = (e[q] & 0xFFFFFFFFull) | ((unsigned long long)((unsigned)r[q] & 0x7FFFFFFFu) << 32);
-                nxtf[p] = (unsigned)f[q];
-            }
-            base += __popc(b);
-        }
-    }
-    __syncwarp();
+// flow_kernel: row `rid` leaves the loop after `steps` steps -- its outputs are final.  Warp-cooperative: the
+// rest of its token history is padded with -1 (no set-up kernel did).  Whoever brings the count of finished rows
+// to B stores the stop word.
+__device__ __forceinline__ void flow_row_leaves(const StepArgs& a, const StepView& sv, const FlowArgs& F, long long rid,
+                                                int steps, int state, float sum, uint8_t done, int lane) {
+    for (int k = steps + lane; k < a.max_steps; k += 32) a.hist_tokens[rid * a.max_steps + k] = -1;
     if (lane == 0) {
-        const bool stop = (base == 0) || (kk >= a.max_steps);
-        F.fin[grp] = 0;
-        if (stop) atomicMax(F.trace_n + LOOP_TRACE_STEPS, kk);  // steps run = the most any group ran
-        if (kk <= LOOP_TRACE_STEPS) {
-            if (kk < LOOP_TRACE_STEPS) atomicAdd(F.trace_n + kk, base);
-            atomicMax(F.trace_t + kk, global_timer_ns());
-        }
-        const unsigned long long d =
-            stop ? FLOW_DONE
-                 // unit size as if all G groups had this many rows: the groups share the warps
-                 : flow_pack(kk, base, tiles_per_unit((long long)base * F.G, tiles_per_row, (long long)gridDim.x * WARPS, tpu_max, a.upw));
-        asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(F.desc + grp), "l"(d) : "memory");
+        a.hist_len[rid] = steps;
+        a.hist_final_state[rid] = state;
+        a.hist_sum_logprob[rid] = sum;
+        a.hist_done[rid] = done;
+        atomicMax(sv.trace_n + LOOP_TRACE_STEPS, steps);  // steps run = the most any row ran
+        if (atomicAdd(F.q + 2, 1) == F.B - 1) atomicExch(F.q + 3, (int)sv.gen);
     }
 }
 
@@ -348,10 +306,10 @@ __device__ __forceinline__ void flow_publish(const StepArgs& a, const FlowArgs& 
 // `gathered`: idx is the position inside the state's CSR row instead of the token id.
 // `sampled`: idx is the sampled token (position), ytok its tempered logit: logprob = (ytok - m) - log(sum).
 // MODE_LOOP: per-row arrays are indexed by the original row id (mt.lrow); surviving rows set their bit in
-// the next step's bitmap.  MODE_FLOW: the result goes to the group's result slots; returns true (in every
-// lane) if this was the last row of the group's step (the caller then publishes the next step).
+// the next step's bitmap.  MODE_FLOW: a surviving row's next step is published as a new task; a row that is
+// done, truncated or failed leaves the loop.
 template <int MODE = MODE_STEP>
-__device__ __forceinline__ bool finalize_row(const StepArgs& a, const StepView& sv, const FlowArgs* F, const TileMeta& mt,
+__device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& sv, const FlowArgs* F, const TileMeta& mt,
                                              float m, float s, int idx, int lane, bool gathered, bool sampled = false,
                                              float ytok = 0.0f) {
     float lp, lse;
@@ -362,9 +320,6 @@ __device__ __forceinline__ bool finalize_row(const StepArgs& a, const StepView& 
         csr_lo = __ldg(a.dfa.row_ptr + mt.st);
         csr_len = (int)(__ldg(a.dfa.row_ptr + mt.st + 1) - csr_lo);
     }
-    unsigned sum_prev_bits = 0;
-    if (MODE == MODE_FLOW && lane == 0)  // the row's running sum travels with its list entry (same round trip as the rank)
-        sum_prev_bits = __ldcg(F->listf[mt.step & 1] + (long long)mt.grp * F->Bg + mt.slot);
     if (m == -INFINITY) {  // every allowed logit is -inf: lowest allowed id (G6)
         lp = -INFINITY;
         lse = -INFINITY;
@@ -375,7 +330,10 @@ __device__ __forceinline__ bool finalize_row(const StepArgs& a, const StepView& 
         lse = m + L;
         pos = gathered ? idx : mask_rank(a.dfa, mt.st, idx, lane);
     }
-    int last = 0;
+    int leave = 0, ns = mt.st;
+    uint8_t dn = 1;
+    float sum = 0.0f;
+    const int step = (MODE == MODE_FLOW) ? mt.step : sv.step;
     if (lane == 0) {
         const bool in_row = (pos >= 0) && (pos < csr_len);
         const long long j = csr_lo + pos;
@@ -383,16 +341,13 @@ __device__ __forceinline__ bool finalize_row(const StepArgs& a, const StepView& 
         const int packed = in_row ? __ldg(a.dfa.next + j) : 0;  // next state | accepting << 31
         // the bitmask and the CSR describe the same set: the token found by rank must be the argmax
         const bool ok = in_row && (gathered || m == -INFINITY || token == idx);
-        int ns = mt.st;
-        uint8_t dn = 1;
         if (ok) {
             ns = packed & 0x7FFFFFFF;
             dn = (packed < 0) ? 1 : 0;
         } else {
-            atomicAdd(a.ctrs + 2, 1);
+            atomicAdd(MODE == MODE_FLOW ? F->q + 4 : a.ctrs + 2, 1);
             token = -1;
         }
-        const int step = (MODE == MODE_FLOW) ? mt.step : sv.step;
         const int slot = (MODE == MODE_STEP) ? mt.slot : mt.lrow;
         CD_PHASE_MIN(sv.ph_first_fin);
         CD_PHASE_MAX(sv.ph_last_fin);
@@ -404,29 +359,47 @@ __device__ __forceinline__ bool finalize_row(const StepArgs& a, const StepView& 
             if (a.done_out) a.done_out[slot] = dn;
         }
         if (MODE == MODE_LOOP && !dn) atomicOr(sv.alive_next + (slot >> 5), 1u << (slot & 31));
-        if (a.hist_tokens) {  // decode loop: this slot's row, original id
+        if (MODE == MODE_FLOW) {
+            const long long rid = mt.lrow;
+            a.hist_tokens[rid * a.max_steps + step] = token;
+            sum = __uint_as_float(mt.sumbits) + lp;  // step 0: 0.0f + lp
+            if (!dn && step + 1 < a.max_steps) {
+                const long long qi = atomicAdd(F->q + 1, 1);
+                if (qi < F->cap) {
+                    const unsigned long long tag = (unsigned long long)sv.gen << 32;
+                    unsigned long long* e = F->task + qi * 4;
+                    st_relaxed_gpu_u64(e + 0, tag | (unsigned)mt.lrow);
+                    st_relaxed_gpu_u64(e + 1, tag | (unsigned)ns);
+                    st_relaxed_gpu_u64(e + 2, tag | __float_as_uint(sum));
+                    st_relaxed_gpu_u64(e + 3, tag | (unsigned)(step + 1));
+                } else {
+                    atomicAdd(F->q + 4, 1);  // cannot happen: the queue holds B * (max_steps - 1) tasks
+                }
+                if (step + 1 < LOOP_TRACE_STEPS) {
+                    atomicAdd(sv.trace_n + step + 1, 1);
+                    atomicMax(sv.trace_t + step + 1, global_timer_ns());
+                }
+            } else {
+                leave = 1;
+                if (!ok) dn = 0;  // a failed row is reported undone
+            }
+        } else if (a.hist_tokens) {  // decode loop: this slot's row, original id
             const long long rid = (MODE != MODE_STEP) ? (long long)mt.lrow : (a.row_map ? (long long)__ldg(a.row_map + slot) : slot);
             a.hist_tokens[rid * a.max_steps + step] = token;
             a.hist_len[rid] = step + 1;
             a.hist_final_state[rid] = ns;
-            float sum;
-            if (MODE == MODE_FLOW) sum = (step == 0 ? 0.0f : __uint_as_float(sum_prev_bits)) + lp;
             // (written by another SM one step ago in loop_kernel: read at the L2, never from a stale L1 line)
-            else sum = __ldcg(a.hist_sum_logprob + rid) + lp;
-            a.hist_sum_logprob[rid] = sum;
+            a.hist_sum_logprob[rid] = __ldcg(a.hist_sum_logprob + rid) + lp;
             a.hist_done[rid] = ok ? dn : (uint8_t)0;
-            if (MODE != MODE_FLOW && a.sat_ctr && ok && dn && __ldg(a.satisfying + ns)) atomicAdd(a.sat_ctr, 1);
-            if (MODE == MODE_FLOW) {
-                const unsigned long long tag = (unsigned long long)(sv.gen + (unsigned)step) << 32;
-                const long long o = (long long)mt.grp * F->Bg + mt.slot;
-                st_relaxed_gpu_u64(F->res + o, tag | ((unsigned)ns & 0x7FFFFFFFu) | ((unsigned)dn << 31));
-                st_relaxed_gpu_u64(F->resf + o, tag | __float_as_uint(sum));
-                last = (atomicAdd(F->fin + mt.grp, 1) == mt.n - 1) ? 1 : 0;
-            }
+            if (a.sat_ctr && ok && dn && __ldg(a.satisfying + ns)) atomicAdd(a.sat_ctr, 1);
         }
     }
-    if (MODE == MODE_FLOW) return __shfl_sync(FULL, last, 0) != 0;
-    return false;
+    if (MODE == MODE_FLOW) {
+        leave = __shfl_sync(FULL, leave, 0);
+        if (leave)
+            flow_row_leaves(a, sv, *F, mt.lrow, step + 1, __shfl_sync(FULL, ns, 0), __shfl_sync(FULL, sum, 0),
+                            (uint8_t)__shfl_sync(FULL, (int)dn, 0), lane);
+    }
 }
 
 template <bool SAMPLE>
@@ -468,11 +441,9 @@ __device__ __forceinline__ int select_row(const StepView& sv, int i) {
 
 // The step a unit belongs to: how its rows are split and where its shared state lives.
 struct UnitCtx {
-    int n, tpu, Pd, PG, P, total_units, step, grp;
+    int n, tpu, Pd, PG, P, total_units, step;
     const unsigned char* logits;
     int* work;
-    long long pbase;  // first partial slot
-    int tbase;        // first ticket
 };
 
 template <int WARPS, int TILE_TOK, int TPU_MAX, bool GATHER>
@@ -492,8 +463,8 @@ __device__ __forceinline__ void unit_ctx_split(UnitCtx& c, const StepArgs& a, in
 // The streaming engine of a warp: issue + consume loops.
 //   MODE_STEP / MODE_LOOP: one decoding step over the slots [0, sv.n); returns when the step's units are
 //   exhausted and this warp's tiles are consumed.
-//   MODE_FLOW: the whole loop; the warp draws units from whichever group has a published step with units
-//   left (oldest step first) and returns when every group is finished.
+//   MODE_FLOW: the whole loop; the warp draws units of row tasks (see FlowArgs) and returns when every row
+//   has left the loop.
 template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER, bool SAMPLE, int MODE>
 __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv, const FlowArgs* F,
                                           WarpRing<STAGES, TILE_BYTES>& ring, RingPos& rp, const int warp, const int lane) {
@@ -515,100 +486,92 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
     const int tiles_per_row = (V + TILE_TOK - 1) / TILE_TOK;
     const int tpu_max = min(TPU_MAX, a.tpu_max);
     UnitCtx cur{};
-    bool have_step = false;   // MODE_FLOW: `cur` is a published step with units left (as far as this warp knows)
-    bool all_done = false;    // MODE_FLOW: every group is finished
+    bool all_done = false;  // MODE_FLOW: every row has left the loop
+    bool poll_pending = false;  // MODE_FLOW: poll_w / poll_stop hold the loads issued for the unit in next_u_l0
+    unsigned long long poll_w = 0;
+    int poll_stop = 0;
     if (MODE != MODE_FLOW) {
         unit_ctx_split<WARPS, TILE_TOK, TPU_MAX, GATHER>(cur, a, sv.n, tiles_per_unit(sv.n, tiles_per_row, total_warps, tpu_max, a.upw));
         cur.step = sv.step;
-        cur.grp = 0;
         cur.logits = sv.logits;
         cur.work = sv.work_ctr;
-        cur.pbase = 0;
-        cur.tbase = 0;
-        have_step = true;
     } else {
-        if (lane < FLOW_MAX_GROUPS) ring.want[lane] = 0;
-        __syncwarp();
+        unit_ctx_split<WARPS, TILE_TOK, TPU_MAX, GATHER>(cur, a, F->B, F->tpu);  // the same split for every task
+        cur.work = F->q + 0;
+        if (lane == 0) next_u_l0 = atomicAdd(cur.work, 1);
     }
     const bool ragged_row = (V % TILE_TOK) != 0;
     const uint64_t pol_stream = l2_policy_evict_first();
 
     bool exhausted = false;
     int iss_tile = 0, iss_end = 0;
-    int iss_slot = 0, iss_st = 0, iss_flags = 0, iss_len = 0, iss_row = 0;
+    int iss_slot = 0, iss_st = 0, iss_flags = 0, iss_len = 0, iss_row = 0, iss_step = 0;
+    unsigned iss_sum = 0u;
     long long iss_lo = 0;
     const unsigned char* iss_src = nullptr;  // next logits tile of the current unit
     const unsigned char* iss_msk = nullptr;  // next mask piece
     int iss_stage = rp.iss_stage, in_flight = 0;
 
-    // MODE_FLOW: look at the groups' descriptors (one per lane, acquire) and take the oldest published step
-    // this warp has not seen exhausted; false if there is none right now
-    auto acquire_step = [&]() -> bool {
-        unsigned long long d = FLOW_DONE;
-        if (lane < F->G) asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(d) : "l"(F->desc + lane) : "memory");
-        const bool done_g = (lane >= F->G) || (d == FLOW_DONE);
-        const int st_g = (int)(d & 0xFFFFFFull);
-        const bool avail = !done_g && (st_g >= ring.want[lane & (FLOW_MAX_GROUPS - 1)]);
-        if (__all_sync(FULL, done_g)) {
-            all_done = true;
-            return false;
-        }
-        int key = avail ? (st_g * FLOW_MAX_GROUPS + lane) : 0x7FFFFFFF;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) key = min(key, __shfl_xor_sync(FULL, key, o));
-        if (key == 0x7FFFFFFF) return false;
-        const int g = key & (FLOW_MAX_GROUPS - 1);
-        d = __shfl_sync(FULL, d, g);
-        const int step = (int)(d & 0xFFFFFFull), n = (int)((d >> 24) & 0xFFFFFFull), tpu = (int)(d >> 48);
-        unit_ctx_split<WARPS, TILE_TOK, TPU_MAX, GATHER>(cur, a, n, tpu);
-        cur.step = step;
-        cur.grp = g;
-        cur.logits = static_cast<const unsigned char*>(F->step_ptrs_dev ? F->step_ptrs_dev[step] : F->step_ptrs[step]);
-        cur.work = F->work + (long long)g * a.max_steps + step;
-        cur.pbase = (long long)g * F->pcap;
-        cur.tbase = g * F->Bg;
-        if (lane == 0) next_u_l0 = atomicAdd(cur.work, 1);
-        have_step = true;
-        return true;
-    };
-
     // issues one tile (or pseudo tile); false if there is nothing to issue right now
     auto issue_one = [&]() -> bool {
         while (iss_tile >= iss_end) {  // next unit (units of a gathered row beyond its pieces are skipped)
-            if (MODE == MODE_FLOW) {
-                if (!have_step && !acquire_step()) return false;
-            } else if (exhausted) {
-                return false;
-            }
+            if (MODE == MODE_FLOW ? all_done : exhausted) return false;
             const int u = __shfl_sync(FULL, next_u_l0, 0);
-            if (u >= cur.total_units) {
-                if (MODE == MODE_FLOW) {  // this step has no units left: never look at it again
-                    if (lane == 0) ring.want[cur.grp] = cur.step + 1;
-                    __syncwarp();
-                    have_step = false;
-                    continue;
-                }
-                exhausted = true;
-                return false;
-            }
-            if (lane == 0) next_u_l0 = draw_base + atomicAdd(cur.work, 1);
-            iss_slot = u / cur.P;
-            const int part = u - iss_slot * cur.P;
             long long rl;  // row of the logits buffer
+            int part;
             if (MODE == MODE_FLOW) {
-                const unsigned long long e = ld_relaxed_gpu_u64(F->list[cur.step & 1] + (long long)cur.grp * F->Bg + iss_slot);
-                rl = (long long)(unsigned)e;
-                iss_st = (int)(e >> 32);
-            } else if (MODE == MODE_LOOP) {
-                rl = select_row(sv, iss_slot);
-                // states are double-buffered by step parity: a unit drawn after its row was finalised
-                // still sees the state the row was processed in
-                iss_st = __ldcg(sv.state_cur + rl);
+                const int q = u / cur.P;
+                part = u - q * cur.P;
+                iss_step = 0;
+                iss_sum = 0u;
+                if (q < F->B) {  // implicit task: row q takes step 0 from the start state
+                    rl = q;
+                    iss_st = F->start;
+                } else {
+                    // lanes 0-3: the task's words; lane 4: the stop word (one round trip for both).  The loads are
+                    // issued here and looked at on the NEXT call: meanwhile the warp consumes a tile (or sleeps),
+                    // so a poll never stalls the consume side.
+                    const long long qi = (long long)q - F->B;
+                    const bool fresh = poll_pending && qi < F->cap && (unsigned)(poll_w >> 32) == sv.gen;
+                    const bool ready = poll_pending && __all_sync(FULL, lane >= 4 || fresh);
+                    if (!ready) {  // not published (yet)
+                        if (poll_pending && (unsigned)__shfl_sync(FULL, poll_stop, 4) == sv.gen) all_done = true;
+                        poll_w = 0;
+                        if (lane < 4 && qi < F->cap) poll_w = ld_relaxed_gpu_u64(F->task + qi * 4 + lane);
+                        if (lane == 4) poll_stop = ld_relaxed_gpu_s32(F->q + 3);
+                        poll_pending = true;
+                        return false;
+                    }
+                    poll_pending = false;
+                    const unsigned long long w = poll_w;
+                    rl = (long long)(unsigned)__shfl_sync(FULL, w, 0);
+                    iss_st = (int)(unsigned)__shfl_sync(FULL, w, 1);
+                    iss_sum = (unsigned)__shfl_sync(FULL, w, 2);
+                    iss_step = (int)(unsigned)__shfl_sync(FULL, w, 3);
+                }
+                if (lane == 0) next_u_l0 = atomicAdd(cur.work, 1);
+                iss_slot = (int)rl;
+                cur.step = iss_step;
+                cur.logits = static_cast<const unsigned char*>(F->step_ptrs_dev ? F->step_ptrs_dev[iss_step] : F->step_ptrs[iss_step]);
             } else {
-                // state[] is not written while units are in flight (next states go to state_new[])
-                iss_st = sv.state_cur[iss_slot];
-                const long long r = a.row_map ? (long long)__ldg(a.row_map + iss_slot) : (long long)iss_slot;
-                rl = a.logits_by_slot ? (long long)iss_slot : r;
+                if (u >= cur.total_units) {
+                    exhausted = true;
+                    return false;
+                }
+                if (lane == 0) next_u_l0 = draw_base + atomicAdd(cur.work, 1);
+                iss_slot = u / cur.P;
+                part = u - iss_slot * cur.P;
+                if (MODE == MODE_LOOP) {
+                    rl = select_row(sv, iss_slot);
+                    // states are double-buffered by step parity: a unit drawn after its row was finalised
+                    // still sees the state the row was processed in
+                    iss_st = __ldcg(sv.state_cur + rl);
+                } else {
+                    // state[] is not written while units are in flight (next states go to state_new[])
+                    iss_st = sv.state_cur[iss_slot];
+                    const long long r = a.row_map ? (long long)__ldg(a.row_map + iss_slot) : (long long)iss_slot;
+                    rl = a.logits_by_slot ? (long long)iss_slot : r;
+                }
             }
             iss_row = (int)rl;
             const bool bad = (iss_st < 0) || (iss_st >= a.dfa.S);
@@ -625,7 +588,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             if (bad || acc) {
                 if (lane == 0) {
                     ring.meta[iss_stage] = TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (part << 8), iss_st, 0, 0,
-                                                    iss_row, cur.step, cur.n, cur.tpu, cur.grp};
+                                                    iss_row, iss_step, iss_sum, {0, 0}};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
                 iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
@@ -637,7 +600,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 if (part >= gather_parts(iss_len, cur.PG)) continue;
                 if (lane == 0) {
                     ring.meta[iss_stage] = TileMeta{iss_slot, 0, FLAG_GATHER | FLAG_LAST | (part << 8), iss_st, iss_lo, iss_len,
-                                                    iss_row, cur.step, cur.n, cur.tpu, cur.grp};
+                                                    iss_row, iss_step, iss_sum, {0, 0}};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
                 iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
@@ -656,7 +619,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
         const uint32_t dst = smem_u32(ring.logits[iss_stage]);
         const uint32_t mdst = smem_u32(ring.mask[iss_stage]);
         const int fl = iss_flags | ((iss_tile + 1 == iss_end) ? FLAG_LAST : 0);
-        const TileMeta meta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, iss_row, cur.step, cur.n, cur.tpu, cur.grp};
+        const TileMeta meta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, iss_row, iss_step, iss_sum, {0, 0}};
         if (ragged_row && iss_tile + 1 == tiles_per_row) {
             // last tile of a row whose length is not a multiple of the tile: partial copies; the
             // < 16 trailing logits bytes go through plain loads, unused mask words are zeroed.
@@ -712,9 +675,9 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
         }
         if (in_flight == 0) {
             if (MODE != MODE_FLOW || all_done) break;
-            __nanosleep(a.idle_ns);  // nothing published right now: some group is between two steps
+            __nanosleep(a.idle_ns);  // the task of this warp's next unit is not published yet
             if (++idle_polls > FLOW_IDLE_LIMIT) {  // never on a healthy run: fail the call, do not hang
-                if (lane == 0) atomicAdd(a.ctrs + 2, 1);
+                if (lane == 0) atomicAdd(F->q + 4, 1);
                 break;
             }
             continue;
@@ -733,13 +696,9 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
         const int part = mt.flags >> 8;
         // the step this tile belongs to (MODE_FLOW: whatever the ring holds; else the step of this call)
         UnitCtx cc = cur;
-        if (MODE == MODE_FLOW) {
-            unit_ctx_split<WARPS, TILE_TOK, TPU_MAX, GATHER>(cc, a, mt.n, mt.tpu);
+        if (MODE == MODE_FLOW) {  // (the split is the same for every task)
             cc.step = mt.step;
-            cc.grp = mt.grp;
             cc.logits = static_cast<const unsigned char*>(F->step_ptrs_dev ? F->step_ptrs_dev[mt.step] : F->step_ptrs[mt.step]);
-            cc.pbase = (long long)mt.grp * F->pcap;
-            cc.tbase = mt.grp * F->Bg;
         }
         const unsigned gen = sv.gen + ((MODE == MODE_FLOW) ? (unsigned)cc.step : 0u);  // tag of the partial slots
         const unsigned long long tag = (unsigned long long)gen << 32;
@@ -748,12 +707,10 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
         auto orig_row = [&]() -> uint32_t {
             return (MODE != MODE_STEP) ? (uint32_t)mt.lrow : (uint32_t)(a.row_map ? __ldg(a.row_map + mt.slot) : mt.slot);
         };
-        bool publish = false;  // MODE_FLOW: this warp finalised the last row of (cc.grp, cc.step)
 
         if (mt.flags & (FLAG_ACCEPT | FLAG_BADSTATE)) {
             // accepted rows never advance; a state outside [0, S) is reported done
             if (part == 0) {
-                int last = 0;
                 if (lane == 0) {
                     const int slot = (MODE == MODE_STEP) ? mt.slot : mt.lrow;
                     if (MODE != MODE_FLOW) {
@@ -764,21 +721,16 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                         if (a.done_out) a.done_out[slot] = 1;
                     }
                     if (mt.flags & FLAG_BADSTATE) {
-                        atomicAdd(a.ctrs + 2, 1);
-                        if (a.hist_tokens) {  // the row leaves the loop here, undone, in the state it has
+                        atomicAdd(MODE == MODE_FLOW ? F->q + 4 : a.ctrs + 2, 1);
+                        if (MODE != MODE_FLOW && a.hist_tokens) {  // the row leaves the loop here, undone, in the state it has
                             const long long rid = orig_row();
                             a.hist_final_state[rid] = mt.st;
                             a.hist_done[rid] = 0;
                         }
                     }
-                    if (MODE == MODE_FLOW) {  // the row leaves its group
-                        const long long o = (long long)mt.grp * F->Bg + mt.slot;
-                        st_relaxed_gpu_u64(F->res + o, tag | 0x80000000u);
-                        st_relaxed_gpu_u64(F->resf + o, tag);
-                        last = (atomicAdd(F->fin + mt.grp, 1) == mt.n - 1) ? 1 : 0;
-                    }
                 }
-                if (MODE == MODE_FLOW) publish = __shfl_sync(FULL, last, 0) != 0;
+                // (flow_kernel never holds an accepting row; a row in a state outside [0, S) leaves undone)
+                if (MODE == MODE_FLOW) flow_row_leaves(a, sv, *F, mt.lrow, mt.step, mt.st, __uint_as_float(mt.sumbits), 0, lane);
             }
         } else {
             const bool gathered = GATHER && (mt.flags & FLAG_GATHER);
@@ -920,25 +872,25 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                     return __fmul_rn(xv, a.inv_tau);
                 };
                 if (np == 1) {
-                    publish = finalize_row<MODE>(a, sv, F, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
+                    finalize_row<MODE>(a, sv, F, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
                 } else {
                     // Publish from lane 1 (lane 0 is busy issuing copies): self-validating words,
                     // then a RELAXED ticket -- no fence anywhere.  The last arriver merges.
                     int t = 0;
                     if (lane == 1) {
-                        PartialSlot* ps = a.partials + (cc.pbase + (long long)mt.slot * cc.P + part);
+                        PartialSlot* ps = a.partials + ((long long)mt.slot * cc.P + part);
                         st_relaxed_gpu_u64(&ps->m, tag | (unsigned)__float_as_int(rm));
                         st_relaxed_gpu_u64(&ps->s, tag | (unsigned)__float_as_int(rs));
                         st_relaxed_gpu_u64(&ps->idx, tag | (unsigned)ri);
                         if (SAMPLE) st_relaxed_gpu_u64(&ps->pad, tag | (unsigned)__float_as_int(rk));
-                        t = atomicAdd(a.tickets + cc.tbase + mt.slot, 1);
+                        t = atomicAdd(a.tickets + mt.slot, 1);
                     }
                     t = __shfl_sync(FULL, t, 1);
                     if (t == np - 1) {
-                        if (lane == 1) a.tickets[cc.tbase + mt.slot] = 0;
+                        if (lane == 1) a.tickets[mt.slot] = 0;
                         // The other units' words were stored before their tickets, but nothing orders
                         // them: poll until every tag is current (normally the first read).
-                        const PartialSlot* base = a.partials + (cc.pbase + (long long)mt.slot * cc.P);
+                        const PartialSlot* base = a.partials + (long long)mt.slot * cc.P;
                         // Merge in slot order whoever merges (bitwise reproducible): lane q % 32 takes
                         // slot q; the own result (identical in every lane after the butterfly) stands in
                         // for slot `part`.
@@ -989,13 +941,11 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                                 online_combine(rm, rs, ri, om, os, oi);
                         }
                         warp_combine_s<SAMPLE>(rm, rs, ri, rk);
-                        publish = finalize_row<MODE>(a, sv, F, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
+                        finalize_row<MODE>(a, sv, F, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
                     }
                 }
             }
         }
-        if (MODE == MODE_FLOW && publish)
-            flow_publish<WARPS>(a, *F, cc.grp, cc.step, cc.n, sv.gen, tiles_per_row, tpu_max, lane);
         --in_flight;
         cons_stage = (cons_stage + 1 == STAGES) ? 0 : cons_stage + 1;
         cons_phase ^= (cons_stage == 0) ? 1u : 0u;
@@ -1203,12 +1153,9 @@ __global__ void __launch_bounds__(WARPS * 32, 1) loop_kernel(const StepArgs a, c
 }
 
 // ------------------------------------------------------------------ one launch = the whole loop, no barrier
-// cd_decode_loop without a LIMIT.  Every warp is an independent worker: it draws units from whichever row
-// group has a published step with units left (oldest step first, so the groups stay staggered: while one
-// group is between two steps -- last rows being merged, transition looked up, next step published -- the
-// others keep the memory system busy), and returns when every group is finished.  There is no block-wide
-// or grid-wide synchronisation after the ring set-up, and no warp ever waits for a warp that is not
-// running, so the launch needs no co-residency guarantee.
+// cd_decode_loop without a LIMIT (see FlowArgs).  Every warp is an independent worker that draws units of row
+// tasks and returns when every row has left the loop.  There is no block-wide or grid-wide synchronisation
+// after the ring set-up, no set-up kernel before the launch and no copy after it.
 template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER, bool SAMPLE = false>
 __global__ void __launch_bounds__(WARPS * 32, 1) flow_kernel(const StepArgs a, const FlowArgs F) {
     using Ring = WarpRing<STAGES, TILE_BYTES>;
@@ -1222,18 +1169,40 @@ __global__ void __launch_bounds__(WARPS * 32, 1) flow_kernel(const StepArgs a, c
     }
     __syncwarp();
     const unsigned gen0 = (unsigned)__ldcg(a.ctrs + 3);
-    if (blockIdx.x == 0 && threadIdx.x == 0) atomicMax(F.trace_t + 0, global_timer_ns());
+    const int par = __ldcg(F.q + 5) & 1;
     StepView sv{};
     sv.gen = gen0;
+    sv.trace_t = F.trace_t[par];
+    sv.trace_n = F.trace_n[par];
+    if (blockIdx.x == 0) {  // this launch's buffers were cleared by the previous one; clear the next one's
+        for (int k = threadIdx.x; k <= LOOP_TRACE_STEPS; k += WARPS * 32) {
+            F.trace_t[par ^ 1][k] = 0ull;
+            F.trace_n[par ^ 1][k] = 0;
+        }
+        if (threadIdx.x == 0) {
+            atomicMax(sv.trace_t + 0, global_timer_ns());
+            atomicAdd(sv.trace_n + 0, F.B);
+        }
+    }
     RingPos rp;
     step_body<DT, WARPS, STAGES, TILE_BYTES, GATHER, SAMPLE, MODE_FLOW>(a, sv, &F, ring, rp, warp, lane);
-    // ---------------- last CTA to leave: generation for the next launch
+    // ---------------- last CTA to leave: counters and generation for the next launch, status for the host
     __syncthreads();
     if (threadIdx.x == 0) {
         const int d = atom_add_acq_rel_gpu(a.ctrs + 1, 1);
         if (d == (int)gridDim.x - 1) {
             a.ctrs[1] = 0;
             a.ctrs[3] = (int)(gen0 + (unsigned)a.max_steps + 1u);
+            const int steps = __ldcg(sv.trace_n + LOOP_TRACE_STEPS);
+            sv.trace_t[steps < LOOP_TRACE_STEPS ? steps : LOOP_TRACE_STEPS] = global_timer_ns();
+            const int err = __ldcg(F.q + 4) + ((__ldcg(F.q + 2) == F.B) ? 0 : 1);  // every row must have left
+            F.q[0] = 0;
+            F.q[1] = 0;
+            F.q[2] = 0;
+            F.q[4] = 0;
+            F.q[5] = par ^ 1;
+            // (sticky until the host reads and clears it: cd_loop_sync reports every loop enqueued since the last one)
+            if (err) atomicAdd_system(F.host_status, err);
         }
     }
 }

@@ -385,6 +385,41 @@ def test_loop_c3_small_against_golden(cd, oracle):
     check_loop(cd, oracle, aut, [x.cuda() for x in logits], cfg.max_steps, ref=read_decode("c3_small_decode.txt"))
 
 
+def test_async_loops_back_to_back(cd, oracle):
+    """cd_decode_loop_async: three loops enqueued back to back on one stream (one kernel launch each, shared
+    scratch), one cd_loop_sync; every one matches the oracle, and the synchronous call bit for bit."""
+    cfg = wl.scaled(wl.CONFIGS["c3"], V=8192, B=300, S=64, max_steps=9)
+    aut = wl.build_automaton(cfg)
+    dfa = dev_dfa(cd, aut)
+    batches = [wl.build_step_logits(cfg, aut, device="cuda:0", batch=i) for i in range(3)]
+    preps = [cd.PreparedLoop(dfa, b) for b in batches]
+    n0 = cd.launch_count()
+    for p in preps:
+        p.enqueue()
+    launched = cd.launch_count() - n0
+    preps[0].sync()
+    assert launched == 3, launched
+    for p, b in zip(preps, batches):
+        ref = oracle.decode_loop(aut, [x.cpu() for x in b], max_steps=cfg.max_steps)
+        for k in ("tokens", "len", "final_state", "done"):
+            assert np.array_equal(p.out[k].cpu().numpy(), ref[k]), k
+        sync_out = cd.decode_loop(dfa, b)
+        for k in ("tokens", "len", "final_state", "done", "sum_logprob"):
+            assert torch.equal(sync_out[k], p.out[k]), k
+        g, r = p.out["sum_logprob"].cpu().numpy().astype(np.float64), ref["sum_logprob"]
+        fin = np.isfinite(r)
+        assert np.array_equal(np.isfinite(g), fin)
+        assert np.all(np.abs(g[fin] - r[fin]) <= np.maximum(TOL * (ref["len"] + np.abs(r))[fin], TOL))
+    # the per-step path enqueues too (LIMIT-free loops in CD_LOOP_PER_STEP mode)
+    dfa.set_loop_mode(cd.LOOP_PER_STEP)
+    q = cd.PreparedLoop(dfa, batches[1])
+    q.enqueue()
+    q.sync()
+    for k in ("tokens", "len", "final_state", "done"):
+        assert torch.equal(q.out[k], preps[1].out[k]), k
+    dfa.close()
+
+
 def test_loop_accepting_start(cd, oracle):
     aut = wl.Automaton(V=64, S=1, start=0, row_ptr=torch.tensor([0, 1]), tok=torch.tensor([1], dtype=torch.int32),
                        next=torch.tensor([0], dtype=torch.int32), accepting=torch.tensor([1], dtype=torch.uint8))
