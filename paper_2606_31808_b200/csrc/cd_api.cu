@@ -77,6 +77,10 @@ int tune_int(const char* name, int def, int lo, int hi) {
     const int v = std::atoi(e);
     return (v >= lo && v <= hi) ? v : def;
 }
+int tune_int_now(const char* name, int def) {
+    const char* e = std::getenv(name);
+    return e ? std::atoi(e) : def;
+}
 #else
 constexpr int tune_int(const char*, int def, int, int) { return def; }
 #endif
@@ -955,6 +959,12 @@ cd_status enqueue_flow_loop(const cd_dfa* d, const Settings& cfg, Scratch* s, co
         F.trace_n[i] = s->b.f_trace_n[i];
     }
     F.host_status = s->d_status;
+#ifdef CD_TUNING
+    if (const char* e = std::getenv("CD_DBG_PTR")) {  // a device buffer of the caller's, [CD_DBG_CAP][8] u64, zeroed
+        F.dbg = reinterpret_cast<unsigned long long*>(std::strtoull(e, nullptr, 0));
+        F.dbg_cap = tune_int_now("CD_DBG_CAP", 0);
+    }
+#endif
     st = dtype == CD_BF16 ? launch_flow_v<cd::DT_BF16>(a, F, grid, stream) : launch_flow_v<cd::DT_F32>(a, F, grid, stream);
     if (st == CD_OK) s->trace_src = 2;
     return st;

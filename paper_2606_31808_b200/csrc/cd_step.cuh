@@ -164,7 +164,13 @@ struct LoopArgs {
 #define CD_PHASE(L, k, i) do { if ((L).phase && (k) < LOOP_TRACE_STEPS) (L).phase[(k) * 8 + (i)] = global_timer_ns(); } while (0)
 #define CD_PHASE_MAX(ptr) do { if (ptr) atomicMax(ptr, global_timer_ns()); } while (0)
 #define CD_PHASE_MIN(ptr) do { if (ptr) atomicMax(ptr, ~global_timer_ns()); } while (0)  /* earliest = ~max(~t) */
+// flow_kernel, per task (row step): [0] published [1] ~first / [2] last unit resolved [3] last unit streamed
+// [4] merger drew the last ticket [5] merger has the partials [6] transition read [7] ~first tile landed
+#define CD_DBG_MAX(F, task, i) do { if ((F) && (F)->dbg && (task) < (F)->dbg_cap) atomicMax((F)->dbg + (long long)(task) * 8 + (i), global_timer_ns()); } while (0)
+#define CD_DBG_MIN(F, task, i) do { if ((F) && (F)->dbg && (task) < (F)->dbg_cap) atomicMax((F)->dbg + (long long)(task) * 8 + (i), ~global_timer_ns()); } while (0)
 #else
+#define CD_DBG_MAX(F, task, i) ((void)0)
+#define CD_DBG_MIN(F, task, i) ((void)0)
 #define CD_PHASE(L, k, i) ((void)0)
 #define CD_PHASE_MAX(ptr) ((void)0)
 #define CD_PHASE_MIN(ptr) ((void)0)
@@ -241,6 +247,8 @@ struct FlowArgs {
     unsigned long long* trace_t[2];  // [LOOP_TRACE_STEPS + 1] latest publication of a task of step k; [steps] = exit
     int* trace_n[2];                 // [LOOP_TRACE_STEPS] rows that ran step k; [LOOP_TRACE_STEPS] = steps run
     int* host_status;                // [0] errors of the loops since the host last cleared it
+    unsigned long long* dbg;         // tuning builds: [dbg_cap][8] per-task phase timestamps (see CD_DBG_*)
+    int dbg_cap;
 };
 
 template <int STAGES, int TILE_BYTES>
@@ -364,6 +372,7 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& 
             a.hist_tokens[rid * a.max_steps + step] = token;
             sum = __uint_as_float(mt.sumbits) + lp;  // step 0: 0.0f + lp
             if (!dn && step + 1 < a.max_steps) {
+                CD_DBG_MAX(F, mt.pad[0], 6);
                 const long long qi = atomicAdd(F->q + 1, 1);
                 if (qi < F->cap) {
                     const unsigned long long tag = (unsigned long long)sv.gen << 32;
@@ -372,6 +381,7 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& 
                     st_relaxed_gpu_u64(e + 1, tag | (unsigned)ns);
                     st_relaxed_gpu_u64(e + 2, tag | __float_as_uint(sum));
                     st_relaxed_gpu_u64(e + 3, tag | (unsigned)(step + 1));
+                    CD_DBG_MAX(F, (long long)F->B + qi, 0);
                 } else {
                     atomicAdd(F->q + 4, 1);  // cannot happen: the queue holds B * (max_steps - 1) tasks
                 }
@@ -507,6 +517,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
     int iss_tile = 0, iss_end = 0;
     int iss_slot = 0, iss_st = 0, iss_flags = 0, iss_len = 0, iss_row = 0, iss_step = 0;
     unsigned iss_sum = 0u;
+    int iss_task = 0;  // MODE_FLOW: index of the task the current unit belongs to (tuning builds: names its trace record)
     long long iss_lo = 0;
     const unsigned char* iss_src = nullptr;  // next logits tile of the current unit
     const unsigned char* iss_msk = nullptr;  // next mask piece
@@ -522,6 +533,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             if (MODE == MODE_FLOW) {
                 const int q = u / cur.P;
                 part = u - q * cur.P;
+                iss_task = q;
                 iss_step = 0;
                 iss_sum = 0u;
                 if (q < F->B) {  // implicit task: row q takes step 0 from the start state
@@ -550,6 +562,10 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                     iss_step = (int)(unsigned)__shfl_sync(FULL, w, 3);
                 }
                 if (lane == 0) next_u_l0 = atomicAdd(cur.work, 1);
+                if (lane == 0) {
+                    CD_DBG_MIN(F, q, 1);
+                    CD_DBG_MAX(F, q, 2);
+                }
                 iss_slot = (int)rl;
                 cur.step = iss_step;
                 cur.logits = static_cast<const unsigned char*>(F->step_ptrs_dev ? F->step_ptrs_dev[iss_step] : F->step_ptrs[iss_step]);
@@ -588,7 +604,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             if (bad || acc) {
                 if (lane == 0) {
                     ring.meta[iss_stage] = TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (part << 8), iss_st, 0, 0,
-                                                    iss_row, iss_step, iss_sum, {0, 0}};
+                                                    iss_row, iss_step, iss_sum, {iss_task, 0}};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
                 iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
@@ -600,7 +616,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 if (part >= gather_parts(iss_len, cur.PG)) continue;
                 if (lane == 0) {
                     ring.meta[iss_stage] = TileMeta{iss_slot, 0, FLAG_GATHER | FLAG_LAST | (part << 8), iss_st, iss_lo, iss_len,
-                                                    iss_row, iss_step, iss_sum, {0, 0}};
+                                                    iss_row, iss_step, iss_sum, {iss_task, 0}};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
                 iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
@@ -619,7 +635,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
         const uint32_t dst = smem_u32(ring.logits[iss_stage]);
         const uint32_t mdst = smem_u32(ring.mask[iss_stage]);
         const int fl = iss_flags | ((iss_tile + 1 == iss_end) ? FLAG_LAST : 0);
-        const TileMeta meta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, iss_row, iss_step, iss_sum, {0, 0}};
+        const TileMeta meta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, iss_row, iss_step, iss_sum, {iss_task, 0}};
         if (ragged_row && iss_tile + 1 == tiles_per_row) {
             // last tile of a row whose length is not a multiple of the tile: partial copies; the
             // < 16 trailing logits bytes go through plain loads, unused mask words are zeroed.
@@ -694,6 +710,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
 #endif
         const TileMeta mt = ring.meta[cons_stage];
         const int part = mt.flags >> 8;
+        if (MODE == MODE_FLOW && lane == 0 && (mt.flags & FLAG_FIRST)) CD_DBG_MIN(F, mt.pad[0], 7);
         // the step this tile belongs to (MODE_FLOW: whatever the ring holds; else the step of this call)
         UnitCtx cc = cur;
         if (MODE == MODE_FLOW) {  // (the split is the same for every task)
@@ -858,6 +875,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 }
             }
             if (mt.flags & FLAG_LAST) {
+                if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, mt.pad[0], 3);
                 float rm = m, rs = s, rk = kb;
                 int ri = idx;
                 warp_combine_s<SAMPLE>(rm, rs, ri, rk);
@@ -887,6 +905,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                     }
                     t = __shfl_sync(FULL, t, 1);
                     if (t == np - 1) {
+                        if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, mt.pad[0], 4);
                         if (lane == 1) a.tickets[mt.slot] = 0;
                         // The other units' words were stored before their tickets, but nothing orders
                         // them: poll until every tag is current (normally the first read).
@@ -941,6 +960,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                                 online_combine(rm, rs, ri, om, os, oi);
                         }
                         warp_combine_s<SAMPLE>(rm, rs, ri, rk);
+                        if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, mt.pad[0], 5);
                         finalize_row<MODE>(a, sv, F, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
                     }
                 }
