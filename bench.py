@@ -388,7 +388,7 @@ def replay_stepwise(cd, cfg, aut, dfa, logits, device, timed):
     return n_k, distinct_k, deg_k, step_ms
 
 
-def measure_loop(cd, cfg, aut, dfa, batches, device, steps, warmup, peak, verbose=False, label=""):
+def measure_loop(cd, cfg, aut, dfa, batches, device, steps, warmup, peak, verbose=False, label="", pipelined=True):
     """The decode loop of one configuration: K timed cd_decode_loop calls over the rotated resident
     batches (CUDA events on the launching stream), then the per-step picture of the persistent kernel
     from its own device-side trace (cd_loop_trace: active rows and nanoseconds per decoding step) with
@@ -401,16 +401,24 @@ def measure_loop(cd, cfg, aut, dfa, batches, device, steps, warmup, peak, verbos
         n_k, distinct_k, deg_k, _ = replay_stepwise(cd, cfg, aut, dfa, logits, device, timed=False)
         per_batch.append(dict(n=n_k, distinct=distinct_k, deg=deg_k,
                               bytes=[n * sz_logit + d * sz_mask for n, d in zip(n_k, distinct_k)]))
+    # the K loops are enqueued back to back (cd_decode_loop_async: one kernel launch each, arguments marshalled once
+    # per resident batch, every batch its own output buffers) and the stream is synchronised once at the end
+    # (cd_loop_sync, which also reports the device-side status of all K loops)
+    # (pipelined=False: cd_decode_loop, which synchronises the stream after every loop -- the lock-step kernel
+    # holds the device's cooperative-launch lock until it has finished and has no asynchronous form)
+    loops = [cd.PreparedLoop(dfa, b, max_steps=cfg.max_steps) for b in batches]
+    go = (lambda lp: lp.enqueue()) if pipelined else (lambda lp: lp.run())
     for i in range(warmup):
-        out = cd.decode_loop(dfa, batches[i % len(batches)], max_steps=cfg.max_steps, out=out)
-    torch.cuda.synchronize()
+        go(loops[i % len(loops)])
+    loops[0].sync()
     l0 = cd.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for i in range(steps):
-        out = cd.decode_loop(dfa, batches[(warmup + i) % len(batches)], max_steps=cfg.max_steps, out=out)
+        go(loops[(warmup + i) % len(loops)])
     e1.record(stream)
-    torch.cuda.synchronize()
+    loops[0].sync()
+    out = loops[(warmup + steps - 1) % len(loops)].out
     launches = cd.launch_count() - l0
     ms = e0.elapsed_time(e1) / steps
     timed = [(warmup + i) % len(batches) for i in range(steps)]
@@ -421,6 +429,7 @@ def measure_loop(cd, cfg, aut, dfa, batches, device, steps, warmup, peak, verbos
     tr_n, tr_ns = dfa.loop_trace()
     res = {
         "B": cfg.B, "max_steps": cfg.max_steps, "resident_batches": len(batches), "loops_timed": steps,
+        "loops_enqueued": "back to back (cd_decode_loop_async), one cd_loop_sync at the end" if pipelined else "cd_decode_loop (stream synchronised after every loop)",
         "rows_per_s": cfg.B / (ms * 1e-3), "ms_per_loop": ms, "row_steps_per_loop": row_steps,
         "gpu_launches_per_loop": launches / steps,
         "loop_gbs": loop_bytes / (ms * 1e-3) / 1e9,
@@ -431,7 +440,7 @@ def measure_loop(cd, cfg, aut, dfa, batches, device, steps, warmup, peak, verbos
     }
     if tr_n and tr_n == last["n"]:
         us = [t / 1e3 for t in tr_ns]
-        gbs = [b / (t * 1e-9) / 1e9 for b, t in zip(last["bytes"], tr_ns)]
+        gbs = [b / (max(t, 1) * 1e-9) / 1e9 for b, t in zip(last["bytes"], tr_ns)]  # (the device timer ticks every 256 ns)
         fixed = [u - b / (READ_RATE_GBS * 1e3) for u, b in zip(us, last["bytes"])]
         kern_us = sum(us)
         k0 = max(range(len(us)), key=lambda k: last["bytes"][k])
@@ -471,6 +480,9 @@ def per_config_section(cd, device, peak, verbose):
         dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device=device)
         dfa.reserve(cfg.B)
         res, _, _ = measure_loop(cd, cfg, aut, dfa, batches, device, k, 5, peak, verbose=verbose, label=name)
+        sy, _, _ = measure_loop(cd, cfg, aut, dfa, batches, device, k, 5, peak, pipelined=False)
+        res["sync_after_every_loop"] = {"rows_per_s": sy["rows_per_s"], "ms_per_loop": sy["ms_per_loop"],
+                                        "frac_of_measured_peak": sy["frac_of_measured_peak"]}
         # the same loops as one launch per decoding step (the round-1 structure; still what the callback / host
         # forms use) and in the lock-step persistent kernel (grid barrier per step; what a LIMIT loop runs in)
         dfa.set_loop_mode(cd.LOOP_PER_STEP)
@@ -478,7 +490,7 @@ def per_config_section(cd, device, peak, verbose):
         res["per_step_launches"] = {"rows_per_s": ps["rows_per_s"], "ms_per_loop": ps["ms_per_loop"], "loop_gbs": ps["loop_gbs"],
                                     "frac_of_measured_peak": ps["frac_of_measured_peak"]}
         dfa.set_loop_mode(cd.LOOP_BARRIER)
-        lb, _, _ = measure_loop(cd, cfg, aut, dfa, batches, device, k, 5, peak)
+        lb, _, _ = measure_loop(cd, cfg, aut, dfa, batches, device, k, 5, peak, pipelined=False)
         res["lock_step_kernel"] = {"rows_per_s": lb["rows_per_s"], "ms_per_loop": lb["ms_per_loop"],
                                    "kernel_us_per_loop": lb.get("kernel_us_per_loop"), "kernel_gbs": lb.get("kernel_gbs"),
                                    "us_per_step": lb.get("us_per_step"), "fixed_us_per_step_avg": lb.get("fixed_us_per_step_avg")}
@@ -587,12 +599,18 @@ def main():
     dfa.set_gather_max(args.gather_max)
     dfa.set_loop_mode({"auto": cd.LOOP_AUTO, "barrier": cd.LOOP_BARRIER, "per_step": cd.LOOP_PER_STEP}[args.loop_mode])
     out = None
+    # One step = one cd_decode_loop over one resident batch.  The timed loops are enqueued back to back with
+    # cd_decode_loop_async (arguments marshalled once per resident batch, every batch its own outputs); the
+    # barrier() that closes the timed region synchronises the stream and checks the device-side status of
+    # every loop (cd_loop_sync).
+    loops = [cd.PreparedLoop(dfa, b, max_steps=cfg.max_steps) for b in batches]
 
     def one_step(i):
         nonlocal out
-        out = cd.decode_loop(dfa, batches[i % len(batches)], max_steps=cfg.max_steps, out=out)
+        out = loops[i % len(loops)].enqueue()
 
     def barrier():
+        loops[0].sync()
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
@@ -661,7 +679,7 @@ def main():
         "launches_timed": args.steps if persistent else int(row_steps and sum(len(per_batch[b]["n"]) for b in timed)),
         "bytes_per_launch_avg": bytes_timed / args.steps if persistent else bytes_timed / max(1, sum(len(per_batch[b]["n"]) for b in timed)),
         "us_per_launch_avg": 1e3 * ms / args.steps if persistent else 1e3 * ms / max(1, sum(len(per_batch[b]["n"]) for b in timed)),
-        "duration_note": "CUDA events around the K timed cd_decode_loop calls / K (includes the set-up kernel and the host hand-over)",
+        "duration_note": "CUDA events around the K timed cd_decode_loop_async calls (enqueued back to back, one cd_loop_sync after them) / K",
         "read_probe_gbs": read_probe, "frac_of_read_probe": (achieved / read_probe) if read_probe else None,
         "traffic": tinfo["bytes"] if tinfo else None,
         "traffic_source": (f"committed ncu --set full capture {tinfo['profile']} (one launch; not measured in this run)"
@@ -671,7 +689,7 @@ def main():
         last = per_batch[timed[-1]]
         us = [t / 1e3 for t in tr_ns]
         kern_us = sum(us)
-        gbs = [b / (t * 1e-9) / 1e9 for b, t in zip(last["bytes"], tr_ns)]
+        gbs = [b / (max(t, 1) * 1e-9) / 1e9 for b, t in zip(last["bytes"], tr_ns)]
         roofline["device_trace"] = {
             "kernel_us_last_loop": kern_us, "kernel_gbs_last_loop": sum(last["bytes"]) / (kern_us * 1e-6) / 1e9,
             "kernel_frac_of_measured_peak": sum(last["bytes"]) / (kern_us * 1e-6) / 1e9 / peak,

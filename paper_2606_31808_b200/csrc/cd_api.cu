@@ -275,17 +275,8 @@ int step_grid(const cd_dfa* d, long long n_upper, int dtype) {
     return (int)g;
 }
 
-// Upper bound of n' * P(n') over n' <= n for the largest grid (mirrors cd::tiles_per_unit):
-// unclamped tiles-per-unit gives n'P <= upw*warps + n'; clamped at the most tiles per unit gives n' * ceil(T/tpu_max).
-long long step_units_cap(const cd_dfa* d, long long n) {
-    const int T = tiles_per_row(d->dev.V, CD_F32);  // fp32 rows have the most tiles
-    const int tpu_max = tpu_max_tiles();
-    const long long warps = (long long)d->num_sms * STEP_WARPS;
-    const long long a = warps * 32 + n;  // up to 32 units per warp
-    const long long b = n * (long long)((T + tpu_max - 1) / tpu_max + 1);
-    // small grids (few rows) use fewer warps, hence fewer units: still below a
-    return (a > b ? a : b) + 64;
-}
+// chunk results of the step kernels: MAX_CHUNKS slots per row (cd_step.cuh: canonical chunks)
+long long step_units_cap(const cd_dfa*, long long n) { return n * cd::MAX_CHUNKS + 64; }
 
 template <typename T>
 cudaError_t dev_alloc(T** p, size_t count) {
@@ -301,7 +292,7 @@ cd_status alloc_step_bufs(const cd_dfa* d, int rows, StepBufs* out) {
     auto A = [&](cudaError_t r) { if (e == cudaSuccess) e = r; };
     A(dev_alloc(&n.partials, (size_t)units));
     A(dev_alloc(&n.ctrs, 4));
-    A(dev_alloc(&n.tickets, (size_t)rows));
+    A(dev_alloc(&n.tickets, 2 * (size_t)rows));
     for (int i = 0; i < 2; ++i) {
         A(dev_alloc(&n.row_ids[i], (size_t)rows));
         A(dev_alloc(&n.state[i], (size_t)rows));
@@ -332,7 +323,7 @@ cd_status alloc_step_bufs(const cd_dfa* d, int rows, StepBufs* out) {
         const int init[4] = {0, 0, 0, 1};  // ... launches at 1
         e = cudaMemcpy(n.ctrs, init, sizeof init, cudaMemcpyHostToDevice);
     }
-    if (e == cudaSuccess) e = cudaMemset(n.tickets, 0, sizeof(int) * (size_t)rows);
+    if (e == cudaSuccess) e = cudaMemset(n.tickets, 0, sizeof(int) * 2 * (size_t)rows);
     if (e == cudaSuccess) e = cudaMemset(n.trace_n, 0, sizeof(int) * ((size_t)cd::LOOP_TRACE_STEPS + 1));
     if (e != cudaSuccess) {
         n.release();
@@ -873,19 +864,22 @@ cd_status enqueue_persistent_loop(const cd_dfa* d, const Settings& cfg, Scratch*
 
 cd_status get_loop_scratch(Scratch* s, int max_steps, cudaStream_t stream);
 
-// flow_kernel: tiles per unit of a B-row loop (fixed for the launch) and whether the loop fits its index ranges
-int flow_tpu(const cd_dfa* d, int B, int dtype, int grid) {
-    return cd::tiles_per_unit(B, tiles_per_row(d->dev.V, dtype), (long long)grid * STEP_WARPS, tpu_max_tiles(), units_per_warp());
+// flow_kernel: whether the loop fits the kernel's index ranges
+constexpr long long FLOW_RING_MAX = (512ll << 20) / (8 * cd::FLOW_ENTRY_WORDS);  // at most 512 MiB of queue
+
+// entries of the queue ring: a power of two >= 2 * B * MAX_CHUNKS (see cd::FlowArgs: B * MAX_CHUNKS suffices)
+long long flow_ring_entries(int B) {
+    long long cap = 1024;
+    while (cap < 2ll * B * cd::MAX_CHUNKS) cap <<= 1;
+    return cap;
 }
-constexpr long long FLOW_TASK_CAP_MAX = (256ll << 20) / 32;  // at most 256 MiB of task queue
 
 bool flow_loop_possible(const cd_dfa* d, int B, int max_steps, int dtype) {
-    const long long tasks = (long long)B * max_steps;
-    if (tasks - B > FLOW_TASK_CAP_MAX) return false;
-    const int T = tiles_per_row(d->dev.V, dtype);
-    const int tpu = flow_tpu(d, B, dtype, step_grid(d, B, dtype));
-    const long long P = (T + tpu - 1) / tpu;
-    return tasks * P + (long long)d->num_sms * STEP_WARPS * 4 < 0x7FFFFFFFLL;  // the unit counter is 32 bits wide
+    (void)d;
+    (void)dtype;
+    if (flow_ring_entries(B) > FLOW_RING_MAX) return false;
+    // the unit counter and the entry counter are 32 bits wide: every row step cut into MAX_CHUNKS units at worst
+    return (long long)B * max_steps * cd::MAX_CHUNKS + (long long)d->num_sms * STEP_WARPS * 4 < 0x7FFFFFFFLL;
 }
 
 // status word of the loops (pinned, device-mapped host memory)
@@ -902,22 +896,22 @@ cd_status get_status_word(Scratch* s) {
     return CD_OK;
 }
 
-// task queue + status word of flow_kernel
-cd_status get_flow_scratch(Scratch* s, long long tasks, cudaStream_t stream) {
+// queue ring + status word of flow_kernel
+cd_status get_flow_scratch(Scratch* s, long long entries, cudaStream_t stream) {
     const cd_status st = get_status_word(s);
     if (st != CD_OK) return st;
-    if (s->f_task_cap >= tasks) return CD_OK;
+    if (s->f_task_cap >= entries) return CD_OK;
     unsigned long long* q = nullptr;
-    const long long cap = tasks < 1024 ? 1024 : tasks;
-    if (dev_alloc(&q, (size_t)cap * 4) != cudaSuccess) return fail(CD_ERR_OOM, "task queue for %lld row steps", tasks);
-    if (cudaMemset(q, 0, sizeof(unsigned long long) * 4 * (size_t)cap) != cudaSuccess) {  // generation tags start at 0
+    if (dev_alloc(&q, (size_t)entries * cd::FLOW_ENTRY_WORDS) != cudaSuccess)
+        return fail(CD_ERR_OOM, "queue of %lld entries", entries);
+    if (cudaMemset(q, 0, sizeof(unsigned long long) * cd::FLOW_ENTRY_WORDS * (size_t)entries) != cudaSuccess) {  // tags start at 0
         cudaFree(q);
-        return fail(CD_ERR_CUDA, "task queue");
+        return fail(CD_ERR_CUDA, "queue");
     }
     if (s->f_task) cudaStreamSynchronize(stream);
     cudaFree(s->f_task);
     s->f_task = q;
-    s->f_task_cap = cap;
+    s->f_task_cap = entries;
     return CD_OK;
 }
 
@@ -927,7 +921,7 @@ cd_status enqueue_flow_loop(const cd_dfa* d, const Settings& cfg, Scratch* s, co
                             cd_dtype dtype, long long ld, int B, int max_steps, int* tokens_out, int* len_out,
                             int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream) {
     RangeGuard range("cd decode loop (persistent kernel, row tasks)");
-    cd_status st = get_flow_scratch(s, (long long)B * (max_steps - 1), stream);
+    cd_status st = get_flow_scratch(s, flow_ring_entries(B), stream);
     if (st != CD_OK) return st;
     LoopExtras x;
     x.tokens = tokens_out;
@@ -949,10 +943,33 @@ cd_status enqueue_flow_loop(const cd_dfa* d, const Settings& cfg, Scratch* s, co
         F.step_ptrs_dev = s->loop_ptrs;
     }
     F.B = B;
-    F.tpu = flow_tpu(d, B, dtype, grid);
     F.start = d->start;
     F.task = s->f_task;
-    F.cap = s->f_task_cap;
+    {  // the ring in use: the largest power of two the allocation holds (it only ever grows)
+        int lg = 0;
+        while ((2ll << lg) <= s->f_task_cap) ++lg;
+        F.cap_log2 = lg;
+        F.cap_mask = (unsigned)((1ll << lg) - 1);
+    }
+    {  // units a published row step is cut into (cd::FlowArgs): 64 / 32 / 16 KiB units or every chunk
+        const int T = tiles_per_row(d->dev.V, dtype), ct = cd::chunk_tiles(T), tc = cd::row_chunks(T);
+        const int W = grid * STEP_WARPS;
+        int tiles[4] = {tpu_max_tiles(), tpu_max_tiles() / 2, tpu_max_tiles() / 4, 1};
+        int th[3] = {0, -W / 2, -(W * 9) / 10};  // (c3: 530 us per loop against 538 with W/2, 0, -W/2; c2 / c4 the same)
+#ifdef CD_TUNING
+        if (const char* e = std::getenv("CD_FLOW_TILES")) std::sscanf(e, "%d,%d,%d,%d", &tiles[0], &tiles[1], &tiles[2], &tiles[3]);
+        if (const char* e = std::getenv("CD_FLOW_TH")) {  // in percent of the warps
+            int p[3] = {0, -50, -90};
+            std::sscanf(e, "%d,%d,%d", &p[0], &p[1], &p[2]);
+            for (int i = 0; i < 3; ++i) th[i] = (int)((long long)W * p[i] / 100);
+        }
+#endif
+        for (int i = 0; i < 4; ++i) {
+            const int cpu = std::max(1, tiles[i] / ct);
+            F.np_lvl[i] = (tc + cpu - 1) / cpu;
+        }
+        for (int i = 0; i < 3; ++i) F.th[i] = th[i];
+    }
     F.q = s->b.f_q;
     for (int i = 0; i < 2; ++i) {
         F.trace_t[i] = s->b.f_trace_t[i];

@@ -67,15 +67,32 @@ constexpr int TPU_MAX_BYTES = 65536;  // at most 64 KiB of logits per unit
 constexpr int UNITS_PER_WARP = 4;     // aim for >= this many units per warp when rows are few
 constexpr int GATHER_UPW = 4;         // the same for gathered rows (pieces of the CSR token list)
 
-constexpr int FLAG_FIRST = 1;   // first tile of its unit: reset the lane accumulators
-constexpr int FLAG_LAST = 2;    // last tile of its unit: reduce and publish
+// Canonical arithmetic (the same bits whatever the launch): a row is cut into CHUNKS -- chunk_tiles()
+// consecutive tiles each, at most MAX_CHUNKS per row, a function of V and the logits type only.  The result
+// of a chunk is the warp combination of the 32 lane chains over its elements (ascending token id per lane); the
+// result of a row is: lane l folds the chunk results l, l + 32 in ascending order, then the same warp
+// combination.  A UNIT (what one warp draws) is a range of whole chunks, so how a row is cut into units -- which
+// depends on the number of active rows, on the kernel and, in flow_kernel, on how busy the machine is when the
+// row's step is published -- never changes a bit of the result: logprob / lse of a row are the same from cd_step
+// on one row and from a 4096-row decode loop.  A gathered row has its own canonical pieces (gather_piece()).
+constexpr int MAX_CHUNKS = 64;
+#ifndef CD_CHUNK_TILES
+#define CD_CHUNK_TILES 1
+#endif
+constexpr int CHUNK_TILES = CD_CHUNK_TILES;
+
+constexpr int FLAG_FIRST = 1;   // first tile of its chunk: reset the lane accumulators
+constexpr int FLAG_LAST = 2;    // last tile of its chunk: reduce and publish the chunk's result
 constexpr int FLAG_ACCEPT = 4;  // pseudo tile of a slot whose state already accepts (no copy)
 constexpr int FLAG_BADSTATE = 8;
-constexpr int FLAG_GATHER = 16;  // pseudo tile of a gathered row piece (no copy)
+constexpr int FLAG_GATHER = 16;  // pseudo tile of a gathered row's unit (no copy)
+constexpr int FLAG_UEND = 32;    // last tile of its unit: take the ticket
+// TileMeta.flags: bits 8-15 = chunk index (dense tile) / part (pseudo tiles), bits 16-23 = chunks of the unit
+// (dense tile) / parts the gathered row is split into
 
-constexpr int SAMPLE_LIST_CAP = 128;  // tiles with at most this many allowed elements are compacted (SAMPLE)
+constexpr int TILE_LIST_CAP = 128;  // tiles with at most this many allowed elements are compacted across the warp
 
-constexpr int GATHER_CHUNK = 256;  // a gathered row is split into pieces of >= this many transitions
+constexpr int GATHER_CHUNK = 256;  // a gathered row is cut into pieces of >= this many transitions
 constexpr int GATHER_UNROLL = 8;   // independent gathers per lane in flight
 
 constexpr int LOOP_MAX_ROWS = 32768;     // persistent loop: rows per call (bitmap snapshot in shared memory)
@@ -84,15 +101,42 @@ constexpr int LOOP_TRACE_STEPS = 256;    // per-step (timestamp, active rows) re
 constexpr unsigned long long LOOP_SPIN_TIMEOUT_NS = 4000000000ull;  // a barrier that waits longer aborts the loop
 constexpr int FLOW_IDLE_LIMIT = 1 << 23;   // idle polls (>= 128 ns apart: > 1 s) after which a worker of flow_kernel gives up
 constexpr int MERGE_SPIN_LIMIT = 1 << 24;  // polls (>= 32 ns apart) after which a merging warp gives up
+constexpr int FLOW_ENTRY_WORDS = 8;        // 64-byte queue entries (5 words used)
 
-// number of units a gathered row of `len` transitions is split into (P = units per row of the launch)
-__host__ __device__ inline int gather_parts(int len, int P) {
-    int np = (len + GATHER_CHUNK - 1) / GATHER_CHUNK;
-    if (np < 1) np = 1;
-    return np < P ? np : P;
+// tiles per chunk / chunks per row of a row of `tiles_per_row` tiles
+__host__ __device__ inline int chunk_tiles(int tiles_per_row) {
+    const int c = (tiles_per_row + MAX_CHUNKS - 1) / MAX_CHUNKS;
+    return c < CHUNK_TILES ? CHUNK_TILES : c;
+}
+__host__ __device__ inline int row_chunks(int tiles_per_row) {
+    const int ct = chunk_tiles(tiles_per_row);
+    return (tiles_per_row + ct - 1) / ct;
+}
+// canonical pieces of a gathered row of `len` transitions: piece size (a multiple of 32) and count (<= MAX_CHUNKS)
+__host__ __device__ inline int gather_piece(int len) {
+    int p = (len + MAX_CHUNKS - 1) / MAX_CHUNKS;
+    p = (p + 31) & ~31;
+    return p < GATHER_CHUNK ? GATHER_CHUNK : p;
+}
+__host__ __device__ inline int gather_pieces(int len) {
+    const int g = gather_piece(len);
+    const int n = (len + g - 1) / g;
+    return n < 1 ? 1 : n;
+}
+// units a dense row is cut into when n rows are active (host mirrors this: cd_api.cu flow_units0)
+__host__ __device__ inline int units_per_row(long long n, int tiles_per_row, long long total_warps, int tpu_max,
+                                             int upw = UNITS_PER_WARP) {
+    const int ct = chunk_tiles(tiles_per_row);
+    const int tc = (tiles_per_row + ct - 1) / ct;
+    long long cpu = (n * tc + total_warps * upw - 1) / (total_warps * upw);  // chunks per unit
+    int cpu_max = tpu_max / ct;
+    if (cpu_max < 1) cpu_max = 1;
+    if (cpu < 1) cpu = 1;
+    if (cpu > cpu_max) cpu = cpu_max;
+    return (int)((tc + cpu - 1) / cpu);
 }
 
-// Result of one unit, readable without a fence: {gen:32 | payload:32} x 3 (+ the sampling key).
+// Result of one chunk, readable without a fence: {gen:32 | payload:32} x 3 (+ the sampling key).
 struct __align__(32) PartialSlot {
     unsigned long long m, s, idx, pad;
 };
@@ -111,8 +155,8 @@ struct StepArgs {
     float* lse_out;
     uint8_t* done_out;
     // scratch (per handle+stream)
-    PartialSlot* partials;  // [units]
-    int* tickets;           // [rows] arrivals per slot, zero between launches
+    PartialSlot* partials;  // [rows][MAX_CHUNKS]
+    int* tickets;           // [2 * rows] chunks arrived per slot (flow_kernel: per row and step parity), zero between uses
     int* ctrs;              // [0] work counter, [1] finished CTAs, [2] error count, [3] generation
     int gather_max;         // states with <= gather_max transitions are gathered (GATHER kernels; 0 = never)
     int all_gather;         // no state has more than gather_max transitions
@@ -143,7 +187,7 @@ struct StepArgs {
     // the original row for the history and the sampling noise)
     int logits_by_slot;
     int upw, tpu_max;  // unit sizing: target units per warp, most tiles per unit
-    int idle_ns;       // flow_kernel: sleep between two looks at the groups' descriptors when nothing is published
+    int idle_ns;       // flow_kernel: sleep between two looks at an unpublished queue entry
 };
 
 // Persistent loop (loop_kernel): everything that outlives a step.
@@ -164,13 +208,20 @@ struct LoopArgs {
 #define CD_PHASE(L, k, i) do { if ((L).phase && (k) < LOOP_TRACE_STEPS) (L).phase[(k) * 8 + (i)] = global_timer_ns(); } while (0)
 #define CD_PHASE_MAX(ptr) do { if (ptr) atomicMax(ptr, global_timer_ns()); } while (0)
 #define CD_PHASE_MIN(ptr) do { if (ptr) atomicMax(ptr, ~global_timer_ns()); } while (0)  /* earliest = ~max(~t) */
-// flow_kernel, per task (row step): [0] published [1] ~first / [2] last unit resolved [3] last unit streamed
-// [4] merger drew the last ticket [5] merger has the partials [6] transition read [7] ~first tile landed
-#define CD_DBG_MAX(F, task, i) do { if ((F) && (F)->dbg && (task) < (F)->dbg_cap) atomicMax((F)->dbg + (long long)(task) * 8 + (i), global_timer_ns()); } while (0)
-#define CD_DBG_MIN(F, task, i) do { if ((F) && (F)->dbg && (task) < (F)->dbg_cap) atomicMax((F)->dbg + (long long)(task) * 8 + (i), ~global_timer_ns()); } while (0)
+// flow_kernel, per row step (record row * max_steps + step): [0] published [1] ~first / [2] last unit resolved
+// [3] last unit streamed [4] merger drew the last ticket [5] merger has the chunk results [6] transition read
+// [7] ~first tile landed
+#define CD_DBG_MAX(F, rec, i) do { if ((F) && (F)->dbg && (rec) < (F)->dbg_cap) atomicMax((F)->dbg + (long long)(rec) * 16 + (i), global_timer_ns()); } while (0)
+#define CD_DBG_MIN(F, rec, i) do { if ((F) && (F)->dbg && (rec) < (F)->dbg_cap) atomicMax((F)->dbg + (long long)(rec) * 16 + (i), ~global_timer_ns()); } while (0)
+// [8..15] largest SM-clock cycle counts: [8] copy issue -> landed [9] landed -> elements done [10] chunk result + publish
+// [11] ticket -> merged [12] merged -> published
+#define CD_DBG_CYC(F, rec, i, v) do { if ((F) && (F)->dbg && (rec) < (F)->dbg_cap) atomicMax((F)->dbg + (long long)(rec) * 16 + (i), (unsigned long long)(v)); } while (0)
+#define CD_CLOCK() ((unsigned)clock64())
 #else
-#define CD_DBG_MAX(F, task, i) ((void)0)
-#define CD_DBG_MIN(F, task, i) ((void)0)
+#define CD_DBG_CYC(F, rec, i, v) ((void)0)
+#define CD_CLOCK() 0u
+#define CD_DBG_MAX(F, rec, i) ((void)0)
+#define CD_DBG_MIN(F, rec, i) ((void)0)
 #define CD_PHASE(L, k, i) ((void)0)
 #define CD_PHASE_MAX(ptr) ((void)0)
 #define CD_PHASE_MIN(ptr) ((void)0)
@@ -199,14 +250,14 @@ struct StepView {
 
 struct __align__(16) TileMeta {
     int slot;
-    int tile;   // tile index inside the row (gathered piece: unused)
-    int flags;  // FLAG_* | part << 8
+    int tile;   // tile index inside the row (pseudo tiles: unused)
+    int flags;  // FLAG_* | chunk or part << 8 | chunks of the unit or parts of the row << 16
     int st;     // automaton state of the slot
     long long csr_lo;  // row_ptr[st]
     int csr_len;       // row_ptr[st + 1] - row_ptr[st]
     int lrow;          // row of the logits buffer
     // flow_kernel: the step this tile belongs to (a warp's ring may hold tiles of several) and the row's running
-    // sum of log-probs before it (fp32 bits; travels with the task)
+    // sum of log-probs before it (fp32 bits; travels with the row)
     int step;
     unsigned sumbits;
     int pad[2];
@@ -214,21 +265,30 @@ struct __align__(16) TileMeta {
 
 constexpr int MODE_STEP = 0;  // step_kernel: one launch = one step
 constexpr int MODE_LOOP = 1;  // loop_kernel: whole loop, grid barrier between steps (LIMIT loops)
-constexpr int MODE_FLOW = 2;  // flow_kernel: whole loop, row groups advance independently (no barrier)
+constexpr int MODE_FLOW = 2;  // flow_kernel: whole loop, every row advances on its own (no barrier)
 
 // flow_kernel (cd_decode_loop without a LIMIT): rows are independent, so nothing makes row r
-// wait at step k for the other rows.  The unit of scheduling is a TASK = one decoding step of one row:
-//   tasks 0 .. B-1 are implicit: (row q, start state, step 0, sum 0) -- nothing is read to start them;
-//   task B + i is the i-th entry of `task`: four self-validating words {launch generation : 32 | payload : 32}
+// wait at step k for the other rows.  What is scheduled is a UNIT = a range of chunks of one decoding step of
+// one row, drawn in order from one counter (q[0]):
+//   units 0 .. B * P0 - 1 are implicit: unit u = part u % P0 of P0 of (row u / P0, start state, step 0, sum 0)
+//     -- nothing is read to start them;
+//   unit B * P0 + e is entry e of the queue `task` (a ring of cap = 2^cap_log2 entries of 64 bytes; entry e
+//     lives at e % cap).  Five self-validating words {tag : 32 | payload : 32}, tag = launch generation + e / cap:
 //       [0] original row id  [1] automaton state  [2] running sum of log-probs (fp32 bits)  [3] step
-//     written (relaxed, no fence) by the warp that finalised the row's previous step, at the index it drew from
-//     q[1]; a word is either stale (older generation) or complete.
-//   Every task is split into the same P units (P fixed for the launch from B: the split of a row, hence the
-//   order of its fp32 sums, never depends on timing -- results are bitwise reproducible).  Unit u = atomicAdd on
-//   q[0]; it belongs to task u / P.  A warp whose next unit belongs to a task that is not published yet keeps
-//   consuming what its ring holds, then polls the entry (and the stop word).  Units are only ever drawn by
-//   running warps and every published task's units are drawn before any unit of a later task, so nothing waits
-//   for a warp that is not running: the launch needs no co-residency guarantee and two loops may share a device.
+//       [4] part | parts << 8 (the unit is part `part` of `parts` of the row's chunks)
+//     written (relaxed, no fence) by the warp that finalised the row's previous step, at the indices it reserved
+//     with one atomicAdd on q[1]; a word is either stale (older tag) or complete.  A row has at most MAX_CHUNKS
+//     entries that are reserved and not read yet, and it reserves the entries of its next step only after every
+//     unit of this one has been read, so with cap >= B * MAX_CHUNKS an entry is never overwritten before it was read.
+//   HOW MANY units a row's next step is cut into is decided when it is published, from how busy the machine is
+//   (entries published minus units drawn): the row's full set of chunks when warps are waiting for work -- the few
+//   rows of a long tail then spread over the whole machine and a step costs one chunk's latency --, down to
+//   64 KiB units when every warp already has work queued.  The canonical arithmetic (see MAX_CHUNKS) makes the
+//   result independent of that decision, so results stay bitwise reproducible.
+//   A warp whose next unit is not published yet keeps consuming what its ring holds, then polls the entry (and
+//   the stop word).  Units are only ever drawn by running warps and every published unit is drawn before any
+//   later one, so nothing waits for a warp that is not running: the launch needs no co-residency guarantee and
+//   two loops may share a device.
 //   q[2] counts the rows that left the loop (accepted, truncated at max_steps, failed); whoever brings it to B
 //   stores the launch generation into q[3], the stop word.  The last CTA to leave resets q[0..2], reports the
 //   error count q[4] to host_status (pinned, mapped host memory: no copy after the loop) and counts the launch
@@ -239,15 +299,19 @@ struct FlowArgs {
     const void* step_ptrs[LOOP_PARAM_STEPS];
     const void* const* step_ptrs_dev;
     int B;
-    int tpu;    // tiles per unit
     int start;  // start state
-    unsigned long long* task;  // [cap][4]
-    long long cap;             // entries of `task`
-    int* q;                    // [0] units drawn [1] tasks published [2] rows finished [3] stop word [4] errors [5] launches
+    unsigned long long* task;  // [cap][FLOW_ENTRY_WORDS]
+    unsigned cap_mask;         // cap - 1
+    int cap_log2;
+    // units a published row step is cut into, by how busy the machine is: backlog (units published and not drawn
+    // yet; negative = warps waiting) >= th[i] -> np_lvl[i], below th[2] -> np_lvl[3] (every chunk a unit)
+    int np_lvl[4];
+    int th[3];
+    int* q;                    // [0] units drawn [1] entries reserved [2] rows finished [3] stop word [4] errors [5] launches
     unsigned long long* trace_t[2];  // [LOOP_TRACE_STEPS + 1] latest publication of a task of step k; [steps] = exit
     int* trace_n[2];                 // [LOOP_TRACE_STEPS] rows that ran step k; [LOOP_TRACE_STEPS] = steps run
     int* host_status;                // [0] errors of the loops since the host last cleared it
-    unsigned long long* dbg;         // tuning builds: [dbg_cap][8] per-task phase timestamps (see CD_DBG_*)
+    unsigned long long* dbg;         // tuning builds: [dbg_cap][8] phase timestamps per row step (see CD_DBG_*)
     int dbg_cap;
 };
 
@@ -257,17 +321,8 @@ struct __align__(128) WarpRing {
     unsigned char mask[STAGES][TILE_BYTES / 16];  // bf16: TILE_BYTES/2 tokens / 8; fp32 uses half
     TileMeta meta[STAGES];
     unsigned long long bar[STAGES];
-    unsigned short list[SAMPLE_LIST_CAP];  // SAMPLE: positions of a tile's allowed elements, compacted
+    unsigned short list[TILE_LIST_CAP];  // positions of a sparse tile's allowed elements, compacted
 };
-
-// tiles per unit for n active rows (host mirrors this in cd_api.cu: step_units_cap)
-__host__ __device__ inline int tiles_per_unit(long long n, int tiles_per_row, long long total_warps, int tpu_max,
-                                              int upw = UNITS_PER_WARP) {
-    long long t = (n * tiles_per_row + total_warps * upw - 1) / (total_warps * upw);
-    if (t < 1) t = 1;
-    if (t > tpu_max) t = tpu_max;
-    return (int)t;
-}
 
 template <int DT>
 __device__ __forceinline__ float tile_elem(const unsigned char* tile, int e) {
@@ -310,16 +365,17 @@ __device__ __forceinline__ void flow_row_leaves(const StepArgs& a, const StepVie
     }
 }
 
-// Row finished: (m, s, idx) is the merged result of all its units.  Warp-uniform.
+// Row finished: (m, s, idx) is the merged result of all its chunks.  Warp-uniform.
 // `gathered`: idx is the position inside the state's CSR row instead of the token id.
 // `sampled`: idx is the sampled token (position), ytok its tempered logit: logprob = (ytok - m) - log(sum).
 // MODE_LOOP: per-row arrays are indexed by the original row id (mt.lrow); surviving rows set their bit in
-// the next step's bitmap.  MODE_FLOW: a surviving row's next step is published as a new task; a row that is
-// done, truncated or failed leaves the loop.
+// the next step's bitmap.  MODE_FLOW: a surviving row's next step is published as new queue entries (q0 / q1 =
+// units drawn / entries reserved as read a moment ago: how busy the machine is); a row that is done, truncated
+// or failed leaves the loop.
 template <int MODE = MODE_STEP>
 __device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& sv, const FlowArgs* F, const TileMeta& mt,
                                              float m, float s, int idx, int lane, bool gathered, bool sampled = false,
-                                             float ytok = 0.0f) {
+                                             float ytok = 0.0f, int q0 = 0, int q1 = 0, long long units0 = 0) {
     float lp, lse;
     int pos;
     long long csr_lo = mt.csr_lo;
@@ -338,7 +394,7 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& 
         lse = m + L;
         pos = gathered ? idx : mask_rank(a.dfa, mt.st, idx, lane);
     }
-    int leave = 0, ns = mt.st;
+    int leave = 0, ns = mt.st, cont = 0;
     uint8_t dn = 1;
     float sum = 0.0f;
     const int step = (MODE == MODE_FLOW) ? mt.step : sv.step;
@@ -371,24 +427,9 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& 
             const long long rid = mt.lrow;
             a.hist_tokens[rid * a.max_steps + step] = token;
             sum = __uint_as_float(mt.sumbits) + lp;  // step 0: 0.0f + lp
+            CD_DBG_MAX(F, rid * a.max_steps + step, 6);
             if (!dn && step + 1 < a.max_steps) {
-                CD_DBG_MAX(F, mt.pad[0], 6);
-                const long long qi = atomicAdd(F->q + 1, 1);
-                if (qi < F->cap) {
-                    const unsigned long long tag = (unsigned long long)sv.gen << 32;
-                    unsigned long long* e = F->task + qi * 4;
-                    st_relaxed_gpu_u64(e + 0, tag | (unsigned)mt.lrow);
-                    st_relaxed_gpu_u64(e + 1, tag | (unsigned)ns);
-                    st_relaxed_gpu_u64(e + 2, tag | __float_as_uint(sum));
-                    st_relaxed_gpu_u64(e + 3, tag | (unsigned)(step + 1));
-                    CD_DBG_MAX(F, (long long)F->B + qi, 0);
-                } else {
-                    atomicAdd(F->q + 4, 1);  // cannot happen: the queue holds B * (max_steps - 1) tasks
-                }
-                if (step + 1 < LOOP_TRACE_STEPS) {
-                    atomicAdd(sv.trace_n + step + 1, 1);
-                    atomicMax(sv.trace_t + step + 1, global_timer_ns());
-                }
+                cont = 1;
             } else {
                 leave = 1;
                 if (!ok) dn = 0;  // a failed row is reported undone
@@ -405,28 +446,50 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& 
         }
     }
     if (MODE == MODE_FLOW) {
+        cont = __shfl_sync(FULL, cont, 0);
+        ns = __shfl_sync(FULL, ns, 0);
+        sum = __shfl_sync(FULL, sum, 0);
+        if (cont) {
+            // how many units for the row's next step: all its chunks if warps are waiting for work, 64 KiB units
+            // if every warp has work queued (backlog = units published and not drawn yet)
+            const long long backlog = units0 + q1 - q0;
+            const int np = (backlog >= F->th[0]) ? F->np_lvl[0] : ((backlog >= F->th[1]) ? F->np_lvl[1] : ((backlog >= F->th[2]) ? F->np_lvl[2] : F->np_lvl[3]));
+            unsigned e0 = 0;
+            if (lane == 0) e0 = (unsigned)atomicAdd(F->q + 1, np);
+            e0 = __shfl_sync(FULL, e0, 0);
+            const unsigned w0 = (unsigned)mt.lrow, w1 = (unsigned)ns, w2 = __float_as_uint(sum), w3 = (unsigned)(step + 1);
+            for (int i = lane; i < np; i += 32) {
+                const unsigned e = e0 + (unsigned)i;
+                unsigned long long* ent = F->task + (size_t)(e & F->cap_mask) * FLOW_ENTRY_WORDS;
+                const unsigned long long tag = (unsigned long long)(sv.gen + (e >> F->cap_log2)) << 32;
+                st_relaxed_gpu_u64(ent + 0, tag | w0);
+                st_relaxed_gpu_u64(ent + 1, tag | w1);
+                st_relaxed_gpu_u64(ent + 2, tag | w2);
+                st_relaxed_gpu_u64(ent + 3, tag | w3);
+                st_relaxed_gpu_u64(ent + 4, tag | (unsigned)(i | (np << 8)));
+            }
+            if (lane == 0) {
+                CD_DBG_MAX(F, (long long)mt.lrow * a.max_steps + step + 1, 0);
+                if (step + 1 < LOOP_TRACE_STEPS) {
+                    atomicAdd(sv.trace_n + step + 1, 1);
+                    atomicMax(sv.trace_t + step + 1, global_timer_ns());
+                }
+            }
+        }
         leave = __shfl_sync(FULL, leave, 0);
         if (leave)
-            flow_row_leaves(a, sv, *F, mt.lrow, step + 1, __shfl_sync(FULL, ns, 0), __shfl_sync(FULL, sum, 0),
-                            (uint8_t)__shfl_sync(FULL, (int)dn, 0), lane);
+            flow_row_leaves(a, sv, *F, mt.lrow, step + 1, ns, sum, (uint8_t)__shfl_sync(FULL, (int)dn, 0), lane);
     }
 }
 
 template <bool SAMPLE>
 __device__ __forceinline__ void warp_combine_s(float& m, float& s, int& idx, float& kb) {
     if constexpr (!SAMPLE) {
-        warp_combine(m, s, idx);
+        warp_combine_redux(m, s, idx);
     } else {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            const float m2 = __shfl_xor_sync(FULL, m, o);
-            const float s2 = __shfl_xor_sync(FULL, s, o);
-            const int i2 = __shfl_xor_sync(FULL, idx, o);
-            const float k2 = __shfl_xor_sync(FULL, kb, o);
-            int dummy = 0;
-            online_combine(m, s, dummy, m2, s2, 0);
-            sample_combine(kb, idx, k2, i2);
-        }
+        int dummy = 0x7FFFFFFF;
+        warp_combine_redux(m, s, dummy);
+        warp_argmax_redux(kb, idx);
     }
 }
 
@@ -449,20 +512,18 @@ __device__ __forceinline__ int select_row(const StepView& sv, int i) {
     return lo * 32 + (int)__fns(sv.s_bits[lo], 0, r + 1);
 }
 
-// The step a unit belongs to: how its rows are split and where its shared state lives.
+// How the rows of a step (MODE_STEP / MODE_LOOP) or the implicit first step (MODE_FLOW) are cut into units.
 struct UnitCtx {
-    int n, tpu, Pd, PG, P, total_units, step;
+    int n, Pd, PG, P, total_units, step;
     const unsigned char* logits;
     int* work;
 };
 
-template <int WARPS, int TILE_TOK, int TPU_MAX, bool GATHER>
-__device__ __forceinline__ void unit_ctx_split(UnitCtx& c, const StepArgs& a, int n, int tpu) {
+template <int WARPS, bool GATHER>
+__device__ __forceinline__ void unit_ctx_split(UnitCtx& c, const StepArgs& a, int n, int tiles_per_row, int tpu_max) {
     const int total_warps = gridDim.x * WARPS;
-    const int tiles_per_row = (a.dfa.V + TILE_TOK - 1) / TILE_TOK;
     c.n = n;
-    c.tpu = tpu;
-    c.Pd = (tiles_per_row + tpu - 1) / tpu;  // units per row of a dense scan
+    c.Pd = units_per_row(n, tiles_per_row, total_warps, tpu_max, a.upw);  // units per row of a dense scan
     // a gathered row is split only as far as needed to give every warp a few units
     c.PG = GATHER ? max(1, min(c.Pd, (total_warps * GATHER_UPW) / max(n, 1))) : c.Pd;
     // units per row of this step; if every state is gathered no unit is drawn in vain
@@ -473,8 +534,7 @@ __device__ __forceinline__ void unit_ctx_split(UnitCtx& c, const StepArgs& a, in
 // The streaming engine of a warp: issue + consume loops.
 //   MODE_STEP / MODE_LOOP: one decoding step over the slots [0, sv.n); returns when the step's units are
 //   exhausted and this warp's tiles are consumed.
-//   MODE_FLOW: the whole loop; the warp draws units of row tasks (see FlowArgs) and returns when every row
-//   has left the loop.
+//   MODE_FLOW: the whole loop; the warp draws units (see FlowArgs) and returns when every row has left the loop.
 template <int DT, int WARPS, int STAGES, int TILE_BYTES, bool GATHER, bool SAMPLE, int MODE>
 __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv, const FlowArgs* F,
                                           WarpRing<STAGES, TILE_BYTES>& ring, RingPos& rp, const int warp, const int lane) {
@@ -488,25 +548,29 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
     // ---------------- issue side (warp-uniform state)
     // MODE_STEP / MODE_LOOP: the first unit of a warp is its global warp id (no atomic on the start-up
     // chain); later units come from the work counter, which therefore starts at 0 = unit `total_warps`.
-    // MODE_FLOW: every unit is drawn from its step's counter.
+    // MODE_FLOW: every unit is drawn from the counter.
     const int total_warps = gridDim.x * WARPS;
     const int draw_base = (MODE == MODE_FLOW) ? 0 : total_warps;
     int next_u_l0 = blockIdx.x * WARPS + warp;  // prefetched unit id, valid in lane 0
     const int V = a.dfa.V;
     const int tiles_per_row = (V + TILE_TOK - 1) / TILE_TOK;
+    const int CT = chunk_tiles(tiles_per_row);              // tiles per chunk
+    const int Tc = (tiles_per_row + CT - 1) / CT;           // chunks per row
     const int tpu_max = min(TPU_MAX, a.tpu_max);
     UnitCtx cur{};
-    bool all_done = false;  // MODE_FLOW: every row has left the loop
+    bool all_done = false;      // MODE_FLOW: every row has left the loop
     bool poll_pending = false;  // MODE_FLOW: poll_w / poll_stop hold the loads issued for the unit in next_u_l0
     unsigned long long poll_w = 0;
     int poll_stop = 0;
+    long long units0 = 0;  // MODE_FLOW: implicit units (the first step of every row)
     if (MODE != MODE_FLOW) {
-        unit_ctx_split<WARPS, TILE_TOK, TPU_MAX, GATHER>(cur, a, sv.n, tiles_per_unit(sv.n, tiles_per_row, total_warps, tpu_max, a.upw));
+        unit_ctx_split<WARPS, GATHER>(cur, a, sv.n, tiles_per_row, tpu_max);
         cur.step = sv.step;
         cur.logits = sv.logits;
         cur.work = sv.work_ctr;
     } else {
-        unit_ctx_split<WARPS, TILE_TOK, TPU_MAX, GATHER>(cur, a, F->B, F->tpu);  // the same split for every task
+        unit_ctx_split<WARPS, GATHER>(cur, a, F->B, tiles_per_row, tpu_max);
+        units0 = (long long)F->B * cur.P;
         cur.work = F->q + 0;
         if (lane == 0) next_u_l0 = atomicAdd(cur.work, 1);
     }
@@ -514,10 +578,9 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
     const uint64_t pol_stream = l2_policy_evict_first();
 
     bool exhausted = false;
-    int iss_tile = 0, iss_end = 0;
-    int iss_slot = 0, iss_st = 0, iss_flags = 0, iss_len = 0, iss_row = 0, iss_step = 0;
+    int iss_tile = 0, iss_end = 0, iss_in_chunk = 0, iss_nch = 0;
+    int iss_slot = 0, iss_st = 0, iss_len = 0, iss_row = 0, iss_step = 0;
     unsigned iss_sum = 0u;
-    int iss_task = 0;  // MODE_FLOW: index of the task the current unit belongs to (tuning builds: names its trace record)
     long long iss_lo = 0;
     const unsigned char* iss_src = nullptr;  // next logits tile of the current unit
     const unsigned char* iss_msk = nullptr;  // next mask piece
@@ -529,28 +592,29 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             if (MODE == MODE_FLOW ? all_done : exhausted) return false;
             const int u = __shfl_sync(FULL, next_u_l0, 0);
             long long rl;  // row of the logits buffer
-            int part;
+            int part, np;  // this unit is part `part` of `np` of its row
             if (MODE == MODE_FLOW) {
-                const int q = u / cur.P;
-                part = u - q * cur.P;
-                iss_task = q;
                 iss_step = 0;
                 iss_sum = 0u;
-                if (q < F->B) {  // implicit task: row q takes step 0 from the start state
+                if (u < units0) {  // implicit unit: row u / P takes step 0 from the start state
+                    const int q = u / cur.P;
+                    part = u - q * cur.P;
+                    np = cur.P;
                     rl = q;
                     iss_st = F->start;
                 } else {
-                    // lanes 0-3: the task's words; lane 4: the stop word (one round trip for both).  The loads are
+                    // lanes 0-4: the entry's words; lane 5: the stop word (one round trip for both).  The loads are
                     // issued here and looked at on the NEXT call: meanwhile the warp consumes a tile (or sleeps),
                     // so a poll never stalls the consume side.
-                    const long long qi = (long long)q - F->B;
-                    const bool fresh = poll_pending && qi < F->cap && (unsigned)(poll_w >> 32) == sv.gen;
-                    const bool ready = poll_pending && __all_sync(FULL, lane >= 4 || fresh);
+                    const unsigned e = (unsigned)((long long)u - units0);
+                    const unsigned expect = sv.gen + (e >> F->cap_log2);
+                    const bool fresh = poll_pending && (unsigned)(poll_w >> 32) == expect;
+                    const bool ready = poll_pending && __all_sync(FULL, lane >= 5 || fresh);
                     if (!ready) {  // not published (yet)
-                        if (poll_pending && (unsigned)__shfl_sync(FULL, poll_stop, 4) == sv.gen) all_done = true;
+                        if (poll_pending && (unsigned)__shfl_sync(FULL, poll_stop, 5) == sv.gen) all_done = true;
                         poll_w = 0;
-                        if (lane < 4 && qi < F->cap) poll_w = ld_relaxed_gpu_u64(F->task + qi * 4 + lane);
-                        if (lane == 4) poll_stop = ld_relaxed_gpu_s32(F->q + 3);
+                        if (lane < 5) poll_w = ld_relaxed_gpu_u64(F->task + (size_t)(e & F->cap_mask) * FLOW_ENTRY_WORDS + lane);
+                        if (lane == 5) poll_stop = ld_relaxed_gpu_s32(F->q + 3);
                         poll_pending = true;
                         return false;
                     }
@@ -560,11 +624,17 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                     iss_st = (int)(unsigned)__shfl_sync(FULL, w, 1);
                     iss_sum = (unsigned)__shfl_sync(FULL, w, 2);
                     iss_step = (int)(unsigned)__shfl_sync(FULL, w, 3);
+                    const unsigned pn = (unsigned)__shfl_sync(FULL, w, 4);
+                    part = (int)(pn & 0xFFu);
+                    np = (int)((pn >> 8) & 0xFFu);
                 }
+                // (drawing the next unit only when the last tile of this one is issued -- so that the warps that have
+                // waited longest, not the ones that just took work, hold the next ids -- was tried: the draw and the
+                // poll then sit in front of every unit's first copy; c4 lost 2 %, the tail gained nothing)
                 if (lane == 0) next_u_l0 = atomicAdd(cur.work, 1);
                 if (lane == 0) {
-                    CD_DBG_MIN(F, q, 1);
-                    CD_DBG_MAX(F, q, 2);
+                    CD_DBG_MIN(F, rl * a.max_steps + iss_step, 1);
+                    CD_DBG_MAX(F, rl * a.max_steps + iss_step, 2);
                 }
                 iss_slot = (int)rl;
                 cur.step = iss_step;
@@ -577,6 +647,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 if (lane == 0) next_u_l0 = draw_base + atomicAdd(cur.work, 1);
                 iss_slot = u / cur.P;
                 part = u - iss_slot * cur.P;
+                np = cur.P;
                 if (MODE == MODE_LOOP) {
                     rl = select_row(sv, iss_slot);
                     // states are double-buffered by step parity: a unit drawn after its row was finalised
@@ -604,7 +675,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             if (bad || acc) {
                 if (lane == 0) {
                     ring.meta[iss_stage] = TileMeta{iss_slot, 0, (bad ? FLAG_BADSTATE : FLAG_ACCEPT) | (part << 8), iss_st, 0, 0,
-                                                    iss_row, iss_step, iss_sum, {iss_task, 0}};
+                                                    iss_row, iss_step, iss_sum, {0, 0}};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
                 iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
@@ -613,10 +684,12 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 return true;
             }
             if (GATHER && iss_len <= a.gather_max) {
-                if (part >= gather_parts(iss_len, cur.PG)) continue;
+                // a gathered row is cut into at most as many units as it has canonical pieces
+                const int parts = min(gather_pieces(iss_len), (MODE == MODE_FLOW) ? np : cur.PG);
+                if (part >= parts) continue;
                 if (lane == 0) {
-                    ring.meta[iss_stage] = TileMeta{iss_slot, 0, FLAG_GATHER | FLAG_LAST | (part << 8), iss_st, iss_lo, iss_len,
-                                                    iss_row, iss_step, iss_sum, {iss_task, 0}};
+                    ring.meta[iss_stage] = TileMeta{iss_slot, 0, FLAG_GATHER | (part << 8) | (parts << 16), iss_st, iss_lo, iss_len,
+                                                    iss_row, iss_step, iss_sum, {0, 0}};
                     mbar_arrive(smem_u32(&ring.bar[iss_stage]));
                 }
                 iss_stage = (iss_stage + 1 == STAGES) ? 0 : iss_stage + 1;
@@ -624,18 +697,24 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 iss_tile = iss_end = 0;
                 return true;
             }
-            iss_tile = part * cur.tpu;
-            iss_end = min(iss_tile + cur.tpu, tiles_per_row);
+            // dense: chunks [Tc * part / np, Tc * (part + 1) / np)
+            const int c0 = (int)(((long long)Tc * part) / np), c1 = (int)(((long long)Tc * (part + 1)) / np);
+            iss_nch = c1 - c0;
+            iss_tile = c0 * CT;
+            iss_end = min(c1 * CT, tiles_per_row);
+            iss_in_chunk = 0;
             iss_src = cur.logits + rl * a.ld_bytes + (long long)iss_tile * TILE_BYTES;
             iss_msk = reinterpret_cast<const unsigned char*>(a.dfa.mask + (long long)iss_st * a.dfa.Wpad) +
                       (long long)iss_tile * MASK_BYTES;
-            iss_flags = (part << 8) | FLAG_FIRST;
         }
         const uint32_t bar = smem_u32(&ring.bar[iss_stage]);
         const uint32_t dst = smem_u32(ring.logits[iss_stage]);
         const uint32_t mdst = smem_u32(ring.mask[iss_stage]);
-        const int fl = iss_flags | ((iss_tile + 1 == iss_end) ? FLAG_LAST : 0);
-        const TileMeta meta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, iss_row, iss_step, iss_sum, {iss_task, 0}};
+        const bool chunk_ends = (iss_in_chunk + 1 == CT) || (iss_tile + 1 == tiles_per_row);
+        const int chunk = (CT == 1) ? iss_tile : iss_tile / CT;
+        const int fl = ((iss_in_chunk == 0) ? FLAG_FIRST : 0) | (chunk_ends ? FLAG_LAST : 0) |
+                       ((iss_tile + 1 == iss_end) ? FLAG_UEND : 0) | (chunk << 8) | (iss_nch << 16);
+        const TileMeta meta{iss_slot, iss_tile, fl, iss_st, iss_lo, iss_len, iss_row, iss_step, iss_sum, {0, (int)CD_CLOCK()}};
         if (ragged_row && iss_tile + 1 == tiles_per_row) {
             // last tile of a row whose length is not a multiple of the tile: partial copies; the
             // < 16 trailing logits bytes go through plain loads, unused mask words are zeroed.
@@ -666,7 +745,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             bulk_g2s_hint(dst, iss_src, TILE_BYTES, bar, pol_stream);
             bulk_g2s(mdst, iss_msk, MASK_BYTES, bar);
         }
-        iss_flags &= ~FLAG_FIRST;
+        iss_in_chunk = chunk_ends ? 0 : iss_in_chunk + 1;
         iss_src += TILE_BYTES;
         iss_msk += MASK_BYTES;
         ++iss_tile;
@@ -676,8 +755,40 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
     };
 
     // ---------------- consume side
-    float m = -INFINITY, s = 0.0f, kb = -INFINITY;  // kb: best perturbed key (SAMPLE); idx then is its token
-    int idx = 0x7FFFFFFF;
+    // NC independent chains per lane (greedy: one per mask word of a tile, so that a lone warp is not bound by
+    // the latency of one dependent chain of online updates; sampling keeps one): chain j of lane l sees the
+    // elements of word j * 32 + l of every tile of the chunk, in ascending token id
+    constexpr int NC = SAMPLE ? 1 : WPL;
+    float am[NC], as[NC];
+    int ai[NC];
+    float kb = -INFINITY;  // best perturbed key (SAMPLE); ai[0] then is its token
+    bool many_chains = false;  // warp-uniform: a chain other than chain 0 was fed since the last reset
+    auto reset_chains = [&]() {
+        many_chains = false;
+#pragma unroll
+        for (int j = 0; j < NC; ++j) {
+            am[j] = -INFINITY;
+            as[j] = 0.0f;
+            ai[j] = 0x7FFFFFFF;
+        }
+        kb = -INFINITY;
+    };
+    // the lane's chains -> one (m, s, idx) (pairwise tree; equal maxima keep the lower token id), then the warp
+    auto chunk_result = [&](float& rm, float& rs, int& ri, float& rk) {
+        if (NC > 1 && many_chains) {  // (combining with an untouched chain changes nothing: skipping it is exact)
+#pragma unroll
+            for (int w = 1; w < NC; w <<= 1) {
+#pragma unroll
+                for (int j = 0; j + w < NC; j += 2 * w) online_combine(am[j], as[j], ai[j], am[j + w], as[j + w], ai[j + w]);
+            }
+        }
+        rm = am[0];
+        rs = as[0];
+        ri = ai[0];
+        rk = kb;
+        warp_combine_s<SAMPLE>(rm, rs, ri, rk);
+    };
+    reset_chains();
     int cons_stage = rp.cons_stage;
     uint32_t cons_phase = rp.cons_phase;
 #ifdef CD_TUNING
@@ -691,7 +802,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
         }
         if (in_flight == 0) {
             if (MODE != MODE_FLOW || all_done) break;
-            __nanosleep(a.idle_ns);  // the task of this warp's next unit is not published yet
+            __nanosleep(a.idle_ns);  // this warp's next unit is not published yet
             if (++idle_polls > FLOW_IDLE_LIMIT) {  // never on a healthy run: fail the call, do not hang
                 if (lane == 0) atomicAdd(F->q + 4, 1);
                 break;
@@ -709,25 +820,134 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
         first_tile = false;
 #endif
         const TileMeta mt = ring.meta[cons_stage];
-        const int part = mt.flags >> 8;
-        if (MODE == MODE_FLOW && lane == 0 && (mt.flags & FLAG_FIRST)) CD_DBG_MIN(F, mt.pad[0], 7);
+        const int fpart = (mt.flags >> 8) & 0xFF;   // chunk index (dense) / part (pseudo tiles)
+        const int fcnt = (mt.flags >> 16) & 0xFF;   // chunks of the unit (dense) / parts of the row (gathered)
         // the step this tile belongs to (MODE_FLOW: whatever the ring holds; else the step of this call)
-        UnitCtx cc = cur;
-        if (MODE == MODE_FLOW) {  // (the split is the same for every task)
-            cc.step = mt.step;
-            cc.logits = static_cast<const unsigned char*>(F->step_ptrs_dev ? F->step_ptrs_dev[mt.step] : F->step_ptrs[mt.step]);
-        }
-        const unsigned gen = sv.gen + ((MODE == MODE_FLOW) ? (unsigned)cc.step : 0u);  // tag of the partial slots
+        const int tstep = (MODE == MODE_FLOW) ? mt.step : cur.step;
+        const unsigned char* tlogits =
+            (MODE == MODE_FLOW) ? static_cast<const unsigned char*>(F->step_ptrs_dev ? F->step_ptrs_dev[mt.step] : F->step_ptrs[mt.step])
+                                : cur.logits;
+        const unsigned gen = sv.gen + ((MODE == MODE_FLOW) ? (unsigned)tstep : 0u);  // tag of the chunk results
         const unsigned long long tag = (unsigned long long)gen << 32;
-        const int rng_step = a.rng_step_base + cc.step;
+        const int rng_step = a.rng_step_base + tstep;
+        const long long dbg_rec = (MODE == MODE_FLOW) ? (long long)mt.lrow * a.max_steps + tstep : 0;
+        (void)dbg_rec;
         // original row id of the slot: names the history row and seeds the sampling noise
         auto orig_row = [&]() -> uint32_t {
             return (MODE != MODE_STEP) ? (uint32_t)mt.lrow : (uint32_t)(a.row_map ? __ldg(a.row_map + mt.slot) : mt.slot);
         };
+        PartialSlot* const pbase = a.partials + (long long)mt.slot * MAX_CHUNKS;
+        // lane 1 publishes the result of chunk c (lane 0 is busy issuing copies): self-validating words
+        auto publish_chunk = [&](int c, float rm, float rs, int ri, float rk) {
+            if (lane == 1) {
+                PartialSlot* ps = pbase + c;
+                st_relaxed_gpu_u64(&ps->m, tag | (unsigned)__float_as_int(rm));
+                st_relaxed_gpu_u64(&ps->s, tag | (unsigned)__float_as_int(rs));
+                st_relaxed_gpu_u64(&ps->idx, tag | (unsigned)ri);
+                if (SAMPLE) st_relaxed_gpu_u64(&ps->pad, tag | (unsigned)__float_as_int(rk));
+            }
+        };
+        // The unit is complete: `nch` of the row's `total` chunk results are published.  A RELAXED ticket counts
+        // them -- no fence anywhere; whoever completes the row merges: the other units' words were stored before
+        // their tickets but nothing orders them, so the merger polls until every tag is current (normally the
+        // first read).  Lane l folds the chunks l, l + 32, ... in ascending order, then the warp combination:
+        // the same order whoever merges and however the row was cut into units.
+        auto unit_done = [&](int nch, int total, bool gathered) {
+            int* tk = a.tickets + ((MODE == MODE_FLOW) ? (long long)mt.slot * 2 + (tstep & 1) : (long long)mt.slot);
+            bool last = true;
+            if (nch != total) {
+                int t = 0;
+                if (lane == 1) t = atomicAdd(tk, nch);
+                t = __shfl_sync(FULL, t, 1);
+                last = (t + nch == total);
+                if (last && lane == 1) *tk = 0;
+            }
+            if (!last) return;
+            if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, dbg_rec, 4);
+            const unsigned ck2 = CD_CLOCK();
+            int q0 = 0, q1 = 0;
+            if (MODE == MODE_FLOW && lane == 0) {  // how busy the machine is, for the split of the row's next step
+                q0 = ld_relaxed_gpu_s32(F->q + 0);
+                q1 = ld_relaxed_gpu_s32(F->q + 1);
+            }
+            __syncwarp();
+            float rm = -INFINITY, rs = 0.0f, rk = -INFINITY;
+            int ri = 0x7FFFFFFF;
+            constexpr int ROUNDS = MAX_CHUNKS / 32;
+            unsigned long long wm[ROUNDS], ws[ROUNDS], wi[ROUNDS], wk[ROUNDS];
+            bool ok[ROUNDS];
+#pragma unroll
+            for (int r = 0; r < ROUNDS; ++r) {  // every load of every round in flight at once
+                const int c = r * 32 + lane;
+                ok[r] = c >= total;
+                wm[r] = ws[r] = wi[r] = wk[r] = 0;
+                if (!ok[r]) {
+                    wm[r] = ld_relaxed_gpu_u64(&pbase[c].m);
+                    ws[r] = ld_relaxed_gpu_u64(&pbase[c].s);
+                    wi[r] = ld_relaxed_gpu_u64(&pbase[c].idx);
+                    if (SAMPLE) wk[r] = ld_relaxed_gpu_u64(&pbase[c].pad);
+                }
+            }
+            int spins = 0;
+            while (true) {
+                bool all_ok = true;
+#pragma unroll
+                for (int r = 0; r < ROUNDS; ++r) {
+                    if (!ok[r]) {
+                        ok[r] = ((wm[r] >> 32) == gen) && ((ws[r] >> 32) == gen) && ((wi[r] >> 32) == gen) &&
+                                (!SAMPLE || (wk[r] >> 32) == gen);
+                        if (!ok[r]) {  // a stale word: read the slot again
+                            const int c = r * 32 + lane;
+                            wm[r] = ld_relaxed_gpu_u64(&pbase[c].m);
+                            ws[r] = ld_relaxed_gpu_u64(&pbase[c].s);
+                            wi[r] = ld_relaxed_gpu_u64(&pbase[c].idx);
+                            if (SAMPLE) wk[r] = ld_relaxed_gpu_u64(&pbase[c].pad);
+                            all_ok = false;
+                        }
+                    }
+                }
+                if (__all_sync(FULL, all_ok)) break;
+                __nanosleep(32);
+                if (++spins > MERGE_SPIN_LIMIT) {  // never on a healthy run: fail the call, do not hang
+                    if (lane == 0) atomicAdd(MODE == MODE_FLOW ? F->q + 4 : a.ctrs + 2, 1);
+                    break;
+                }
+            }
+#pragma unroll
+            for (int r = 0; r < ROUNDS; ++r) {
+                if (r * 32 + lane < total) {
+                    if (SAMPLE) {
+                        int dummy = 0;
+                        online_combine(rm, rs, dummy, __int_as_float((int)(unsigned)wm[r]), __int_as_float((int)(unsigned)ws[r]), 0);
+                        sample_combine(rk, ri, __int_as_float((int)(unsigned)wk[r]), (int)(unsigned)wi[r]);
+                    } else {
+                        online_combine(rm, rs, ri, __int_as_float((int)(unsigned)wm[r]), __int_as_float((int)(unsigned)ws[r]),
+                                       (int)(unsigned)wi[r]);
+                    }
+                }
+            }
+            warp_combine_s<SAMPLE>(rm, rs, ri, rk);
+            if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, dbg_rec, 5);
+            const unsigned ck3 = CD_CLOCK();
+            if (MODE == MODE_FLOW && lane == 0) CD_DBG_CYC(F, dbg_rec, 11, ck3 - ck2);
+            // SAMPLE: the tempered logit of the sampled token is re-read from the logits row
+            float ytok = 0.0f;
+            if (SAMPLE && rm != -INFINITY) {
+                const int tokid = gathered ? __ldg(a.dfa.tok + mt.csr_lo + ri) : ri;
+                const unsigned char* rowp = tlogits + (long long)mt.lrow * a.ld_bytes;
+                const float xv = (DT == DT_BF16)
+                                     ? __uint_as_float(((uint32_t)__ldg(reinterpret_cast<const uint16_t*>(rowp) + tokid)) << 16)
+                                     : __ldg(reinterpret_cast<const float*>(rowp) + tokid);
+                ytok = __fmul_rn(xv, a.inv_tau);
+            }
+            finalize_row<MODE>(a, sv, F, mt, rm, rs, ri, lane, gathered, SAMPLE, ytok, __shfl_sync(FULL, q0, 0),
+                               __shfl_sync(FULL, q1, 0), units0);
+            if (MODE == MODE_FLOW && lane == 0) CD_DBG_CYC(F, dbg_rec, 12, CD_CLOCK() - ck3);
+        };
 
         if (mt.flags & (FLAG_ACCEPT | FLAG_BADSTATE)) {
             // accepted rows never advance; a state outside [0, S) is reported done
-            if (part == 0) {
+            if (fpart == 0) {
                 if (lane == 0) {
                     const int slot = (MODE == MODE_STEP) ? mt.slot : mt.lrow;
                     if (MODE != MODE_FLOW) {
@@ -749,22 +969,21 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 // (flow_kernel never holds an accepting row; a row in a state outside [0, S) leaves undone)
                 if (MODE == MODE_FLOW) flow_row_leaves(a, sv, *F, mt.lrow, mt.step, mt.st, __uint_as_float(mt.sumbits), 0, lane);
             }
-        } else {
-            const bool gathered = GATHER && (mt.flags & FLAG_GATHER);
-            const int np = gathered ? gather_parts(mt.csr_len, cc.PG) : cc.P;  // units this row was split into
-            if (gathered) {
-                // piece [j0, j1) of the state's CSR row: tokens read coalesced, their logits gathered
-                // with GATHER_UNROLL independent loads per lane; idx = position in the CSR row, which
-                // ascends with the token id, so "replace on strictly greater" keeps the lowest id
-                m = -INFINITY;
-                s = 0.0f;
-                kb = -INFINITY;
-                idx = 0x7FFFFFFF;
-                const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, orig_row(), (uint32_t)rng_step) : 0u;
-                const int j0 = (int)(((long long)mt.csr_len * part) / np);
-                const int j1 = (int)(((long long)mt.csr_len * (part + 1)) / np);
-                const int* tk = a.dfa.tok + mt.csr_lo;
-                const unsigned char* rowp = cc.logits + (long long)mt.lrow * a.ld_bytes;
+        } else if (GATHER && (mt.flags & FLAG_GATHER)) {
+            // unit `fpart` of `fcnt` of a gathered row: the canonical pieces [p0, p1) of the state's CSR row.  Per
+            // piece: tokens read coalesced, their logits gathered with GATHER_UNROLL independent loads per lane;
+            // idx = position in the CSR row, which ascends with the token id, so "replace on strictly greater"
+            // keeps the lowest id
+            const int npieces = gather_pieces(mt.csr_len), gp = gather_piece(mt.csr_len);
+            const int p0 = (int)(((long long)npieces * fpart) / fcnt), p1 = (int)(((long long)npieces * (fpart + 1)) / fcnt);
+            const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, orig_row(), (uint32_t)rng_step) : 0u;
+            const int* tk = a.dfa.tok + mt.csr_lo;
+            const unsigned char* rowp = tlogits + (long long)mt.lrow * a.ld_bytes;
+#pragma unroll 1
+            for (int p = p0; p < p1; ++p) {
+                reset_chains();
+                const int j0 = p * gp;
+                const int j1 = min(mt.csr_len, j0 + gp);
                 // software pipeline: the token ids of the next round are loaded while this round's
                 // logits are in flight
                 int t[GATHER_UNROLL];
@@ -794,175 +1013,125 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                     for (int u = 0; u < GATHER_UNROLL; ++u) t[u] = (jn + 32 * u < j1) ? __ldg(tk + jn + 32 * u) : -1;
 #pragma unroll
                     for (int u = 0; u < GATHER_UNROLL; ++u) {
-                        if (SAMPLE)
-                            online_update_sample(m, s, kb, idx, fmaxf(x[u], -INFINITY), tc[u], j + 32 * u, a.inv_tau, row_key);
+                        if constexpr (SAMPLE)
+                            online_update_sample(am[0], as[0], kb, ai[0], fmaxf(x[u], -INFINITY), tc[u], j + 32 * u, a.inv_tau, row_key);
                         else
-                            online_update(m, s, idx, fmaxf(x[u], -INFINITY), j + 32 * u);  // NaN -> -inf
+                            online_update(am[u % NC], as[u % NC], ai[u % NC], fmaxf(x[u], -INFINITY), j + 32 * u);  // NaN -> -inf
+                    }
+                }
+                many_chains = true;
+                float rm, rs, rk;
+                int ri;
+                chunk_result(rm, rs, ri, rk);
+                publish_chunk(p, rm, rs, ri, rk);
+            }
+            __syncwarp();
+            if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, dbg_rec, 3);
+            unit_done(p1 - p0, npieces, true);
+        } else {
+            if (MODE == MODE_FLOW && lane == 0 && (mt.flags & FLAG_FIRST)) CD_DBG_MIN(F, dbg_rec, 7);
+            const unsigned ck0 = CD_CLOCK();
+            if (MODE == MODE_FLOW && lane == 0) CD_DBG_CYC(F, dbg_rec, 8, ck0 - (unsigned)mt.pad[1]);
+            if (mt.flags & FLAG_FIRST) reset_chains();
+            const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, orig_row(), (uint32_t)rng_step) : 0u;
+            const int t0 = mt.tile * TILE_TOK;
+            const uint32_t* mw = reinterpret_cast<const uint32_t*>(ring.mask[cons_stage]);
+            const unsigned char* tile = ring.logits[cons_stage];
+            // the lane owns the tile's mask words WPL * lane .. WPL * lane + WPL - 1 (consecutive tokens; one
+            // vector load from shared memory)
+            uint32_t bits[WPL];
+            if constexpr (WPL == 4) {
+                const uint4 v = reinterpret_cast<const uint4*>(mw)[lane];
+                bits[0] = v.x; bits[1] = v.y; bits[2] = v.z; bits[3] = v.w;
+            } else if constexpr (WPL == 2) {
+                const uint2 v = reinterpret_cast<const uint2*>(mw)[lane];
+                bits[0] = v.x; bits[1] = v.y;
+            } else {
+#pragma unroll
+                for (int j = 0; j < WPL; ++j) bits[j] = mw[WPL * lane + j];
+            }
+            // Sparse tile (at most TILE_LIST_CAP allowed elements -- the normal case of a constrained step): the
+            // allowed positions are first compacted across the warp (one exclusive scan of the per-lane popcounts =
+            // ascending token order, positions written to a small shared list) and lane l then evaluates exactly the
+            // elements of rank l, l + 32, ... (ascending per lane, so "replace on strictly greater" still keeps
+            // the lowest id).  Every lane gets its fair share of the tile's allowed elements -- the bit walk below
+            // runs as long as the fullest word of any lane -- and only allowed elements cost an evaluation (with
+            // sampling: a hash and two logarithms each).
+            int cnt = 0;
+#pragma unroll
+            for (int j = 0; j < WPL; ++j) cnt += __popc(bits[j]);
+            int inc = cnt;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int up = __shfl_up_sync(FULL, inc, o);
+                if (lane >= o) inc += up;
+            }
+            const int total = __shfl_sync(FULL, inc, 31);
+            if (total <= TILE_LIST_CAP) {
+                int o = inc - cnt;
+#pragma unroll
+                for (int j = 0; j < WPL; ++j) {
+                    uint32_t b = bits[j];
+                    const int e0 = (WPL * lane + j) * 32;
+                    while (b != 0u) {
+                        ring.list[o++] = (unsigned short)(e0 + __ffs(b) - 1);
+                        b &= b - 1u;
                     }
                 }
                 __syncwarp();
+                for (int r = lane; r < total; r += 32) {
+                    const int e = ring.list[r];
+                    if constexpr (SAMPLE)
+                        online_update_sample(am[0], as[0], kb, ai[0], tile_elem<DT>(tile, e), t0 + e, t0 + e, a.inv_tau, row_key);
+                    else
+                        online_update(am[0], as[0], ai[0], tile_elem<DT>(tile, e), t0 + e);
+                }
+            } else if constexpr (SAMPLE) {
+#pragma unroll
+                for (int j = 0; j < WPL; ++j) {
+                    // warp-uniform trip count (max popcount over the lanes); idle lanes feed -inf
+                    uint32_t b = bits[j];
+                    const int e0 = (WPL * lane + j) * 32;
+                    while (__any_sync(FULL, b != 0u)) {
+                        const bool v = b != 0u;
+                        const int e = e0 + (v ? (__ffs(b) - 1) : 0);
+                        b &= b - 1u;
+                        const float x = v ? tile_elem<DT>(tile, e) : -INFINITY;
+                        online_update_sample(am[0], as[0], kb, ai[0], x, t0 + e, t0 + e, a.inv_tau, row_key);
+                    }
+                }
             } else {
-                if (mt.flags & FLAG_FIRST) {
-                    m = -INFINITY;
-                    s = 0.0f;
-                    kb = -INFINITY;
-                    idx = 0x7FFFFFFF;
-                }
-                const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, orig_row(), (uint32_t)rng_step) : 0u;
-                const int t0 = mt.tile * TILE_TOK;
-                const uint32_t* mw = reinterpret_cast<const uint32_t*>(ring.mask[cons_stage]);
-                const unsigned char* tile = ring.logits[cons_stage];
-                uint32_t bits[WPL];
+                // dense tile: the lane's WPL words advance together, one chain each: the trip count is the largest
+                // popcount of any word of the tile (warp-uniform); chains without a bit left feed -inf
+                many_chains = true;
+                uint32_t any = 0u;
 #pragma unroll
-                for (int j = 0; j < WPL; ++j) bits[j] = mw[j * 32 + lane];
-                // SAMPLE, sparse tile: the noise costs ~60 instructions per evaluation, so the allowed
-                // positions are first compacted across the warp (exclusive scan of the per-lane popcounts
-                // in (word, lane) = ascending token order, positions written to a small shared list) and
-                // each lane then evaluates exactly the elements of rank lane, lane + 32, ... (ascending per
-                // lane, so "replace on strictly greater" still keeps the lowest id).
-                bool compacted = false;
-                if constexpr (SAMPLE) {
-                    int cnt[WPL], offs[WPL], total = 0;
+                for (int j = 0; j < WPL; ++j) any |= bits[j];
+                while (__any_sync(FULL, any != 0u)) {
+                    any = 0u;
 #pragma unroll
                     for (int j = 0; j < WPL; ++j) {
-                        cnt[j] = __popc(bits[j]);
-                        int inc = cnt[j];
-#pragma unroll
-                        for (int o = 1; o < 32; o <<= 1) {
-                            const int up = __shfl_up_sync(FULL, inc, o);
-                            if (lane >= o) inc += up;
-                        }
-                        offs[j] = total + inc - cnt[j];
-                        total += __shfl_sync(FULL, inc, 31);
-                    }
-                    if (total <= SAMPLE_LIST_CAP) {
-                        compacted = true;
-#pragma unroll
-                        for (int j = 0; j < WPL; ++j) {
-                            uint32_t b = bits[j];
-                            int o = offs[j];
-                            const int e0 = (j * 32 + lane) * 32;
-                            while (b != 0u) {
-                                ring.list[o++] = (unsigned short)(e0 + __ffs(b) - 1);
-                                b &= b - 1u;
-                            }
-                        }
-                        __syncwarp();
-                        for (int r = lane; r < total; r += 32) {
-                            const int e = ring.list[r];
-                            online_update_sample(m, s, kb, idx, tile_elem<DT>(tile, e), t0 + e, t0 + e, a.inv_tau, row_key);
-                        }
-                        __syncwarp();
-                    }
-                }
-                if (!compacted) {
-#pragma unroll
-                    for (int j = 0; j < WPL; ++j) {
-                        // warp-uniform trip count (max popcount over the lanes); idle lanes feed -inf
-                        uint32_t b = bits[j];
-                        const int e0 = (j * 32 + lane) * 32;
-                        while (__any_sync(FULL, b != 0u)) {
-                            const bool v = b != 0u;
-                            const int e = e0 + (v ? (__ffs(b) - 1) : 0);
-                            b &= b - 1u;
-                            const float x = v ? tile_elem<DT>(tile, e) : -INFINITY;
-                            if (SAMPLE)
-                                online_update_sample(m, s, kb, idx, x, t0 + e, t0 + e, a.inv_tau, row_key);
-                            else
-                                online_update(m, s, idx, x, t0 + e);
-                        }
+                        const uint32_t b = bits[j];
+                        const bool v = b != 0u;
+                        const int e = (WPL * lane + j) * 32 + (v ? (__ffs(b) - 1) : 0);
+                        bits[j] = b & (b - 1u);
+                        any |= bits[j];
+                        const float x = v ? tile_elem<DT>(tile, e) : -INFINITY;
+                        online_update(am[j], as[j], ai[j], x, t0 + e);
                     }
                 }
             }
-            if (mt.flags & FLAG_LAST) {
-                if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, mt.pad[0], 3);
-                float rm = m, rs = s, rk = kb;
-                int ri = idx;
-                warp_combine_s<SAMPLE>(rm, rs, ri, rk);
-                // SAMPLE: the tempered logit of the sampled token is re-read from the logits row
-                auto sampled_y = [&](int pos) -> float {
-                    if (!SAMPLE || rm == -INFINITY) return 0.0f;
-                    const int tokid = gathered ? __ldg(a.dfa.tok + mt.csr_lo + pos) : pos;
-                    const unsigned char* rowp = cc.logits + (long long)mt.lrow * a.ld_bytes;
-                    const float xv = (DT == DT_BF16)
-                                         ? __uint_as_float(((uint32_t)__ldg(reinterpret_cast<const uint16_t*>(rowp) + tokid)) << 16)
-                                         : __ldg(reinterpret_cast<const float*>(rowp) + tokid);
-                    return __fmul_rn(xv, a.inv_tau);
-                };
-                if (np == 1) {
-                    finalize_row<MODE>(a, sv, F, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
-                } else {
-                    // Publish from lane 1 (lane 0 is busy issuing copies): self-validating words,
-                    // then a RELAXED ticket -- no fence anywhere.  The last arriver merges.
-                    int t = 0;
-                    if (lane == 1) {
-                        PartialSlot* ps = a.partials + ((long long)mt.slot * cc.P + part);
-                        st_relaxed_gpu_u64(&ps->m, tag | (unsigned)__float_as_int(rm));
-                        st_relaxed_gpu_u64(&ps->s, tag | (unsigned)__float_as_int(rs));
-                        st_relaxed_gpu_u64(&ps->idx, tag | (unsigned)ri);
-                        if (SAMPLE) st_relaxed_gpu_u64(&ps->pad, tag | (unsigned)__float_as_int(rk));
-                        t = atomicAdd(a.tickets + mt.slot, 1);
-                    }
-                    t = __shfl_sync(FULL, t, 1);
-                    if (t == np - 1) {
-                        if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, mt.pad[0], 4);
-                        if (lane == 1) a.tickets[mt.slot] = 0;
-                        // The other units' words were stored before their tickets, but nothing orders
-                        // them: poll until every tag is current (normally the first read).
-                        const PartialSlot* base = a.partials + (long long)mt.slot * cc.P;
-                        // Merge in slot order whoever merges (bitwise reproducible): lane q % 32 takes
-                        // slot q; the own result (identical in every lane after the butterfly) stands in
-                        // for slot `part`.
-                        const float om = rm, os = rs, ok_ = rk;
-                        const int oi = ri;
-                        rm = -INFINITY;
-                        rs = 0.0f;
-                        rk = -INFINITY;
-                        ri = 0x7FFFFFFF;
-                        for (int q0 = 0; q0 < np; q0 += 32) {
-                            const int q = q0 + lane;
-                            const bool want = (q < np) && (q != part);
-                            bool ok = !want;
-                            unsigned long long wm = 0, ws = 0, wi = 0, wk = 0;
-                            int spins = 0;
-                            while (true) {
-                                if (!ok) {
-                                    wm = ld_relaxed_gpu_u64(&base[q].m);
-                                    ws = ld_relaxed_gpu_u64(&base[q].s);
-                                    wi = ld_relaxed_gpu_u64(&base[q].idx);
-                                    ok = ((wm >> 32) == gen) && ((ws >> 32) == gen) && ((wi >> 32) == gen);
-                                    if (SAMPLE) {
-                                        wk = ld_relaxed_gpu_u64(&base[q].pad);
-                                        ok = ok && ((wk >> 32) == gen);
-                                    }
-                                }
-                                if (__all_sync(FULL, ok)) break;
-                                __nanosleep(32);
-                                if (++spins > MERGE_SPIN_LIMIT) {  // never on a healthy run: fail the call, do not hang
-                                    if (lane == 0) atomicAdd(a.ctrs + 2, 1);
-                                    break;
-                                }
-                            }
-                            if (SAMPLE) {
-                                int dummy = 0;
-                                if (want) {
-                                    online_combine(rm, rs, dummy, __int_as_float((int)(unsigned)wm),
-                                                   __int_as_float((int)(unsigned)ws), 0);
-                                    sample_combine(rk, ri, __int_as_float((int)(unsigned)wk), (int)(unsigned)wi);
-                                } else if (q == part) {
-                                    online_combine(rm, rs, dummy, om, os, 0);
-                                    sample_combine(rk, ri, ok_, oi);
-                                }
-                            } else if (want)
-                                online_combine(rm, rs, ri, __int_as_float((int)(unsigned)wm),
-                                               __int_as_float((int)(unsigned)ws), (int)(unsigned)wi);
-                            else if (q == part)
-                                online_combine(rm, rs, ri, om, os, oi);
-                        }
-                        warp_combine_s<SAMPLE>(rm, rs, ri, rk);
-                        if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, mt.pad[0], 5);
-                        finalize_row<MODE>(a, sv, F, mt, rm, rs, ri, lane, gathered, SAMPLE, sampled_y(ri));
-                    }
+            const unsigned ck1 = CD_CLOCK();
+            if (MODE == MODE_FLOW && lane == 0) CD_DBG_CYC(F, dbg_rec, 9, ck1 - ck0);
+            if (mt.flags & FLAG_LAST) {  // the chunk is complete
+                float rm, rs, rk;
+                int ri;
+                chunk_result(rm, rs, ri, rk);
+                publish_chunk(fpart, rm, rs, ri, rk);
+                if (MODE == MODE_FLOW && lane == 1) CD_DBG_CYC(F, dbg_rec, 10, CD_CLOCK() - ck1);
+                if (mt.flags & FLAG_UEND) {
+                    if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, dbg_rec, 3);
+                    unit_done(fcnt, Tc, false);
                 }
             }
         }

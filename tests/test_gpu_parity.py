@@ -486,7 +486,8 @@ def test_step_and_loop_are_bitwise_reproducible(cd, oracle, step_mode):
                 with torch.cuda.stream(streams[si]):
                     loops[si] = cd.decode_loop(dfa, steps)
 
-            # per loop mode the bits must repeat (the three modes split rows into units differently)
+            # the bits must repeat (since the canonical chunk arithmetic the three kernels also agree with one another:
+            # test_results_do_not_depend_on_the_batch)
             lmode = (cd.LOOP_AUTO, cd.LOOP_BARRIER, cd.LOOP_PER_STEP)[(rep // 2) % 3]
             dfa.set_loop_mode(lmode)
             threads = [threading.Thread(target=run_loop, args=(si,)) for si in range(2)]
@@ -516,6 +517,52 @@ def test_step_and_loop_are_bitwise_reproducible(cd, oracle, step_mode):
         for lmode in first_loop:
             assert np.array_equal(first_loop[lmode]["tokens"][:m].cpu().numpy(), want["tokens"]), lmode
     dfa.set_loop_mode(cd.LOOP_AUTO)
+    dfa.close()
+
+
+def test_results_do_not_depend_on_the_batch(cd, oracle, step_mode):
+    """The canonical arithmetic of cd_step.cuh: a row is cut into chunks that depend on V and the logits type only,
+    a chunk's result is a fixed function of its elements and a row's result a fixed fold of its chunks' -- so how a
+    launch cuts rows into units (which depends on the number of active rows, on the kernel and, in the row-task loop,
+    on how busy the machine is) must not change a BIT of logprob / lse.  The same rows are decoded alone, in small and
+    large batches, permuted, through cd_step and through the three loop kernels."""
+    cfg = wl.scaled(wl.CONFIGS["c4"], B=1500, S=256, max_steps=6)
+    aut = wl.build_automaton(cfg, device="cuda:0")
+    dfa = dev_dfa(cd, aut)
+    xs = wl.build_step_logits(cfg, aut, device="cuda:0")
+    live = live_states(aut, cfg.B)
+
+    def bits(t):
+        return t.view(torch.int32) if t.dtype == torch.float32 else t
+
+    # cd_step: all rows at once is the reference
+    st = torch.tensor(live, dtype=torch.int32, device="cuda:0")
+    tok0, lp0, lse0, done0 = cd.step(dfa, xs[0], st)
+    st0 = st.clone()
+    g = torch.Generator().manual_seed(5)
+    for n in (1, 2, 37, 148, 1024):
+        rows = torch.randperm(cfg.B, generator=g)[:n].to("cuda:0")
+        rm = rows.to(torch.int32)
+        st = torch.tensor(live, dtype=torch.int32, device="cuda:0")[rows].contiguous()
+        tok, lp, lse, done = cd.step(dfa, xs[0], st, row_map=rm)
+        assert torch.equal(tok, tok0[rows]) and torch.equal(st, st0[rows]) and torch.equal(done, done0[rows])
+        assert torch.equal(bits(lp), bits(lp0[rows])), ("logprob bits depend on the batch", n)
+        assert torch.equal(bits(lse), bits(lse0[rows])), ("lse bits depend on the batch", n)
+    # the loops: three kernels, whole batch and sub-batches
+    ref = None
+    for lmode in (cd.LOOP_AUTO, cd.LOOP_BARRIER, cd.LOOP_PER_STEP):
+        dfa.set_loop_mode(lmode)
+        for B in (cfg.B, 700, 3):
+            out = cd.decode_loop(dfa, [x[:B] for x in xs])
+            cur = {k: bits(v).clone() for k, v in out.items()}
+            if ref is None:
+                ref = cur
+            for k in cur:
+                assert torch.equal(cur[k], ref[k][:B]), ("loop results depend on the kernel or the batch", lmode, B, k)
+    dfa.set_loop_mode(cd.LOOP_AUTO)
+    # ... and the common result is the oracle's
+    want = oracle.decode_loop(aut, [x.cpu() for x in xs])
+    assert np.array_equal(ref["tokens"].cpu().numpy(), want["tokens"])
     dfa.close()
 
 
