@@ -274,9 +274,9 @@ CD_API cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, cons
  *       copy after it -- when the device supports it and B <= 32768; the CTAs stay resident and read
  *       step_logits[k] themselves.
  *       - cd_decode_loop: rows are independent, so no row waits for another one.  The
- *         unit of scheduling is one decoding step of one row: the warp that finalises step k of a row
- *         publishes the row's step k + 1 (row, next state, running sum) in a device queue, from which
- *         every warp draws pieces of row steps in order.  While some rows are between two steps
+ *         warp that finalises step k of a row publishes the row's step k + 1 (row, next state,
+ *         running sum; cut into 1 .. 64 work units) in a device queue, from which every warp draws
+ *         work units in order.  While some rows are between two steps
  *         (merge, transition look-up) the others keep the memory system busy: no launch, no counter
  *         reset, no compaction pass and no barrier between steps.  The active set never exists as a
  *         list; the outputs are indexed by original row id, so the results are those of the stable
@@ -289,11 +289,12 @@ CD_API cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, cons
  *       into the step kernel's last CTA.
  *   CD_LOOP_BARRIER         the lock-step persistent kernel also without a LIMIT.
  *   CD_LOOP_PER_STEP        always one launch per decoding step.
- * All three give the same tokens, lengths, states and done flags bit for bit; sum_logprob_out is
- * bit-identical between CD_LOOP_BARRIER and CD_LOOP_PER_STEP and within the stated tolerance for
- * CD_LOOP_AUTO (a row is split into work units by B alone, not by the number of rows still active,
- * which changes the fp32 summation order); each mode by itself is bitwise reproducible from run to
- * run.
+ * All three give the same outputs bit for bit, sum_logprob_out included, and from run to run: the
+ * order of a row's fp32 sums is fixed by the row alone (V and the logits type cut it into chunks
+ * whose results are folded in a fixed order), never by the batch, the kernel or timing -- in
+ * CD_LOOP_AUTO a row step is cut into more work units when warps are waiting for work and into
+ * fewer when the machine is busy, which does not change the result.  For the same reason
+ * logprob_out / lse_out of cd_step do not depend on n, row_map or the other slots of the call.
  * cd_loop_trace returns, for the last loop that ran in a persistent kernel on (dfa, cuda_stream),
  * the number of decoding steps it ran (*steps_out), and for the first min(cap, 256) of them the
  * rows that took the step and its duration in nanoseconds measured on the device (HOST arrays;
