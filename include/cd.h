@@ -393,7 +393,12 @@ CD_API cd_status cd_decode_loop_host(const cd_dfa_t* dfa, const void* const* ste
  * allowed logits as gathered dot products; the others go through a dense tcgen05
  * contraction whose epilogue applies each row's allowed-token bitmask
  * (cd_set_head_gather_max: 0 = dense for every state, > 0 = gather states with at most
- * that many transitions, -1 = automatic, the default).  Results agree with cd_step on
+ * that many transitions, -1 = automatic, the default: states with fewer than V / 300
+ * transitions are gathered, and when the remaining rows of a call together touch fewer than
+ * 0.8 V rows of W -- a late step of an early-exit loop -- they are gathered too instead of
+ * streaming all of W for a handful of rows).  A gathered row is cut into pieces of >= 128
+ * transitions, one CTA each, so a few rows of thousands of transitions still spread over
+ * the whole machine.  Results agree with cd_step on
  * exactly computed logits: token, state and done are identical whenever the best
  * allowed logit leads the runner-up by more than the fp32 accumulation error (always,
  * when the dot products are exact in fp32); logprob / lse within that error.

@@ -3,6 +3,7 @@
 // kernels of cd_step.cuh / cd_aux.cuh / cd_head.cuh / cd_dedup.cuh.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <atomic>
 #include <cstdarg>
 #include <cstdio>
@@ -161,11 +162,12 @@ struct Scratch {
     uint16_t* h_A = nullptr;      // [rows_pad, ldA]
     long long h_ldA = 0;
     cd::HeadPartial* h_partials = nullptr;
+    cd::HeadPartial* h_gpartials = nullptr;  // [rows][HG_MAX_PIECES]
     CUtensorMap h_tmA{};
 
     void release_head() {
-        cudaFree(h_flags); cudaFree(h_lists); cudaFree(h_ctr); cudaFree(h_A); cudaFree(h_partials);
-        h_flags = nullptr; h_lists = nullptr; h_ctr = nullptr; h_A = nullptr; h_partials = nullptr;
+        cudaFree(h_flags); cudaFree(h_lists); cudaFree(h_ctr); cudaFree(h_A); cudaFree(h_partials); cudaFree(h_gpartials);
+        h_flags = nullptr; h_lists = nullptr; h_ctr = nullptr; h_A = nullptr; h_partials = nullptr; h_gpartials = nullptr;
         head_rows = 0;
         head_H = 0;
     }
@@ -1620,6 +1622,7 @@ cd_status get_head_scratch(Scratch* s, int rows, int H, cudaStream_t stream) {
     A(cudaMalloc(&s->h_ctr, sizeof(int) * 4));
     A(cudaMalloc(&s->h_A, (size_t)rows_pad * (size_t)ldA * 2));
     A(cudaMalloc(&s->h_partials, sizeof(cd::HeadPartial) * (size_t)cd::head_partials_cap(rows)));
+    A(cudaMalloc(&s->h_gpartials, sizeof(cd::HeadPartial) * (size_t)rows * cd::HG_MAX_PIECES));
     if (e == cudaSuccess) e = cudaMemset(s->h_ctr, 0, sizeof(int) * 4);
     if (e == cudaSuccess) e = cudaMemset(s->h_A, 0, (size_t)rows_pad * (size_t)ldA * 2);
     cd_status st = CD_OK;
@@ -1714,6 +1717,12 @@ cd_status launch_head(const cd_dfa* d, const Settings& cfg, Scratch* s, const vo
     a.ldw = ldw;
     a.H = H;
     a.gather_max = head_gather_max_for(d, cfg);
+    a.gather_auto = (cfg.head_gather_max < 0) ? 1 : 0;
+    {  // most pieces a gathered row can have: the automatic policy may gather any state
+        const long long gdeg = a.gather_auto ? d->max_deg : std::min<long long>(d->max_deg, a.gather_max);
+        a.gp_max = cd::hg_pieces((int)std::min<long long>(gdeg, 0x7FFFFFFF));
+    }
+    a.gpartials = s->h_gpartials;
     a.not_dense = s->h_flags;
     a.not_gather = s->h_flags + s->head_rows;
     a.dense_slot = s->h_lists;
@@ -1733,7 +1742,7 @@ cd_status launch_head(const cd_dfa* d, const Settings& cfg, Scratch* s, const vo
     }
     cd::head_prepare_kernel<<<1, 1024, 0, stream>>>(a);
     CU(cudaGetLastError());
-    const bool any_gather = a.gather_max > 0 && d->min_deg_nonacc <= a.gather_max;
+    const bool any_gather = (a.gather_max > 0 && d->min_deg_nonacc <= a.gather_max) || (a.gather_auto && d->max_deg > a.gather_max);
     const bool any_dense = d->max_deg > a.gather_max;
     int launches = 1;
     if (any_gather) {
@@ -1744,10 +1753,20 @@ cd_status launch_head(const cd_dfa* d, const Settings& cfg, Scratch* s, const vo
             CU(cudaFuncSetAttribute(cd::head_gather_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
             cfg_dev = d->device;
         }
-        if (sample) cd::head_gather_kernel<true><<<n, cd::HG_WARPS * 32, smem, stream>>>(a);
-        else cd::head_gather_kernel<false><<<n, cd::HG_WARPS * 32, smem, stream>>>(a);
+        // one CTA per (row, piece), grid-stride: enough CTAs to fill the machine, never more than there are items
+        long long gblocks = (long long)n * a.gp_max;
+        if (gblocks > (long long)d->num_sms * 8) gblocks = (long long)d->num_sms * 8;
+        if (sample) cd::head_gather_kernel<true><<<(int)gblocks, cd::HG_WARPS * 32, smem, stream>>>(a);
+        else cd::head_gather_kernel<false><<<(int)gblocks, cd::HG_WARPS * 32, smem, stream>>>(a);
         CU(cudaGetLastError());
         ++launches;
+        if (a.gp_max > 1) {  // rows cut into several pieces are merged and finished here
+            const int fb = (n + 7) / 8;
+            if (sample) cd::head_gather_finish_kernel<true><<<fb, 256, 0, stream>>>(a);
+            else cd::head_gather_finish_kernel<false><<<fb, 256, 0, stream>>>(a);
+            CU(cudaGetLastError());
+            ++launches;
+        }
     }
     if (any_dense) {
         const int rows_per_block = 8;

@@ -37,7 +37,22 @@ constexpr int HD_THREADS = 192;  // warp 0 TMA, warp 1 MMA + TMEM alloc, warps 2
 constexpr int HD_TMEM_COLS = 512;
 constexpr int HD_UNITS_TARGET = 148 * 8;
 
-constexpr int HG_WARPS = 8;  // gather kernel: warps per CTA (one CTA per row)
+constexpr int HG_WARPS = 8;      // gather kernel: warps per CTA
+constexpr int HG_PIECE = 128;    // a gathered row is cut into pieces of >= this many transitions, one CTA each ...
+constexpr int HG_MAX_PIECES = 64;  // ... at most this many per row
+constexpr float HG_AUTO_FRAC = 0.8f;  // automatic policy: gather EVERY row while the W rows they touch are < 0.8 V (measured break-even on c3: ~0.9 V)
+
+// canonical pieces of a gathered row of `deg` transitions (a function of deg only: results do not depend on the batch)
+__host__ __device__ inline int hg_piece(int deg) {
+    int p = (deg + HG_MAX_PIECES - 1) / HG_MAX_PIECES;
+    p = (p + 7) & ~7;
+    return p < HG_PIECE ? HG_PIECE : p;
+}
+__host__ __device__ inline int hg_pieces(int deg) {
+    const int g = hg_piece(deg);
+    const int n = (deg + g - 1) / g;
+    return n < 1 ? 1 : n;
+}
 
 struct __align__(32) HeadPartial {
     float m, s;
@@ -119,6 +134,10 @@ struct HeadArgs {
     long long ldw;
     int H;
     int gather_max;  // states with <= gather_max transitions are gathered
+    int gather_auto; // automatic policy: when the rows above gather_max touch fewer than HG_AUTO_FRAC * V rows of W in
+                     // total (a late step of an early-exit loop), they are gathered too instead of streaming all of W
+    int gp_max;      // most pieces a gathered row of this call can have (bounds the item index)
+    HeadPartial* gpartials;  // [rows][HG_MAX_PIECES] piece results of the gathered rows cut into several pieces
     // scratch
     uint8_t* not_dense;   // [n]
     uint8_t* not_gather;  // [n]
@@ -219,6 +238,10 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 __global__ void __launch_bounds__(1024, 1) head_prepare_kernel(const HeadArgs a) {
     const StepArgs& f = a.fin;
     const int n = f.n_dev ? __ldcg(f.n_dev) : f.n;
+    __shared__ unsigned long long s_big;  // transitions of the rows above gather_max, all together
+    if (threadIdx.x == 0) s_big = 0ull;
+    __syncthreads();
+    unsigned long long big = 0ull;
     for (int i = threadIdx.x; i < n; i += blockDim.x) {
         const int st = f.state[i];
         const bool bad = (st < 0) || (st >= f.dfa.S);
@@ -232,12 +255,31 @@ __global__ void __launch_bounds__(1024, 1) head_prepare_kernel(const HeadArgs a)
             if (bad) atomicAdd(f.ctrs + 2, 1);
         } else {
             const int deg = (int)(__ldg(f.dfa.row_ptr + st + 1) - __ldg(f.dfa.row_ptr + st));
-            if (deg <= a.gather_max) ng = 0; else nd = 0;
+            if (deg <= a.gather_max) {
+                ng = 0;
+            } else {
+                nd = 0;
+                big += (unsigned long long)deg;
+            }
         }
         a.not_dense[i] = nd;
         a.not_gather[i] = ng;
     }
+    if (a.gather_auto) {  // one shared-memory atomic per warp (a 64-bit shared atomic is a CAS loop)
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) big += __shfl_xor_sync(FULL, big, o);
+        if ((threadIdx.x & 31) == 0 && big) atomicAdd(&s_big, big);
+    }
     __syncthreads();
+    // a dense step streams all V rows of W however few rows are left; gathering touches one W row per transition
+    if (a.gather_auto && s_big > 0ull && (double)s_big < (double)HG_AUTO_FRAC * (double)f.dfa.V) {
+        for (int i = threadIdx.x; i < n; i += blockDim.x)
+            if (a.not_dense[i] == 0) {
+                a.not_dense[i] = 1;
+                a.not_gather[i] = 0;
+            }
+        __syncthreads();
+    }
     block_compact(a.not_dense, nullptr, f.state, n, a.dense_slot, a.dense_state, a.hctr + 0);
     __syncthreads();
     block_compact(a.not_gather, nullptr, f.state, n, a.gather_slot, a.gather_state, a.hctr + 1);
@@ -271,9 +313,12 @@ __device__ __forceinline__ float dot8(const uint4& w, const uint4& h, float acc)
     return acc;
 }
 
-// One CTA per gathered row: the hidden row is staged in shared memory, the warps split the
-// state's CSR token list into contiguous pieces, four dot products in flight per warp; the
-// running argmax is the CSR position (ascending token id), so the transition needs no search.
+// Work item = (gathered row g, piece p of its CSR token list), one CTA each (grid-stride): the hidden row is staged
+// in shared memory, the warps split the piece into contiguous ranges, four dot products in flight per warp; the
+// running argmax is the CSR position (ascending token id), so the transition needs no search.  A row of one piece
+// (option sets, tries) is finished by its CTA; the piece results of a longer row go to gpartials and
+// head_gather_finish_kernel merges them -- a late step with a handful of rows of thousands of transitions then
+// spreads over the whole machine instead of keeping one SM per row busy.
 template <bool SAMPLE>
 __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadArgs a) {
     extern __shared__ __align__(16) unsigned char hg_smem[];
@@ -284,62 +329,72 @@ __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadAr
     const int n_gather = __ldcg(a.hctr + 1);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nv = a.H >> 3;
-    for (int g = blockIdx.x; g < n_gather; g += gridDim.x) {
+    const long long items = (long long)n_gather * a.gp_max;
+    int staged = -1;  // gathered row whose hidden row is in shared memory
+    for (long long it = blockIdx.x; it < items; it += gridDim.x) {
+        const int g = (int)(it / a.gp_max), p = (int)(it - (long long)g * a.gp_max);
         const int slot = __ldcg(a.gather_slot + g);
         const int st = __ldcg(a.gather_state + g);
-        const long long r = (f.row_map && !f.logits_by_slot) ? (long long)__ldg(f.row_map + slot) : (long long)slot;
-        const uint4* src = reinterpret_cast<const uint4*>(a.hidden + r * a.ldh);
-        __syncthreads();  // previous row's readers are done with hid / s_*
-        for (int v = threadIdx.x; v < nv; v += blockDim.x) hid[v] = __ldg(src + v);
-        __syncthreads();
         const long long lo = __ldg(f.dfa.row_ptr + st);
         const int deg = (int)(__ldg(f.dfa.row_ptr + st + 1) - lo);
-        const int j0 = (int)(((long long)deg * warp) / HG_WARPS);
-        const int j1 = (int)(((long long)deg * (warp + 1)) / HG_WARPS);
+        const int np = hg_pieces(deg);
+        if (p >= np) continue;  // (uniform over the CTA)
+        const long long r = (f.row_map && !f.logits_by_slot) ? (long long)__ldg(f.row_map + slot) : (long long)slot;
+        const uint4* src = reinterpret_cast<const uint4*>(a.hidden + r * a.ldh);
+        __syncthreads();  // previous item's readers are done with hid / s_*
+        if (staged != g) {
+            for (int v = threadIdx.x; v < nv; v += blockDim.x) hid[v] = __ldg(src + v);
+            staged = g;
+        }
+        __syncthreads();
+        const int piece = hg_piece(deg);
+        const int jlo = p * piece, jhi = min(deg, jlo + piece);
+        const int j0 = jlo + (int)(((long long)(jhi - jlo) * warp) / HG_WARPS);
+        const int j1 = jlo + (int)(((long long)(jhi - jlo) * (warp + 1)) / HG_WARPS);
         float m = -INFINITY, s = 0.0f, kb = -INFINITY, yb = -INFINITY;
         int idx = 0x7FFFFFFF;
         const uint32_t row_key =
             SAMPLE ? rng_row_key(f.seed_lo, f.seed_hi, (uint32_t)(f.row_map ? __ldg(f.row_map + slot) : slot),
                                  (uint32_t)(f.rng_step_base + f.step))
                    : 0u;
-        for (int j = j0; j < j1; j += 4) {
-            const uint4* wp[4];
-            int tq[4];
+        // two W rows at a time, each read in passes of 8 x 512 contiguous bytes per warp with every load of the pass
+        // in flight (16 independent 16-byte loads per lane): a row is fetched in one or two bursts instead of being
+        // revisited chunk by chunk -- DRAM pages are opened once
+        for (int j = j0; j < j1; j += 2) {
+            const int jb = (j + 1 < j1) ? j + 1 : j;
+            const int ta = __ldg(f.dfa.tok + lo + j), tb = __ldg(f.dfa.tok + lo + jb);
+            const uint4* wa = reinterpret_cast<const uint4*>(a.W + (long long)ta * a.ldw);
+            const uint4* wb = reinterpret_cast<const uint4*>(a.W + (long long)tb * a.ldw);
+            float acc[2] = {0.0f, 0.0f};
+            for (int v0 = lane; v0 < nv; v0 += 256) {
+                uint4 xa[8], xb[8];
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                const int jq = (j + q < j1) ? j + q : j1 - 1;
-                tq[q] = __ldg(f.dfa.tok + lo + jq);
-                wp[q] = reinterpret_cast<const uint4*>(a.W + (long long)tq[q] * a.ldw);
-            }
-            float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-            // two chunks of the four W rows per round: 8 independent 16-byte loads in flight per lane
-            int v = lane;
-            for (; v + 32 < nv; v += 64) {
-                uint4 w0[4], w1[4];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    w0[q] = __ldg(wp[q] + v);
-                    w1[q] = __ldg(wp[q] + v + 32);
+                for (int u = 0; u < 8; ++u) {
+                    const int v = v0 + 32 * u;
+                    xa[u] = (v < nv) ? __ldg(wa + v) : make_uint4(0, 0, 0, 0);
+                    xb[u] = (v < nv) ? __ldg(wb + v) : make_uint4(0, 0, 0, 0);
                 }
-                const uint4 h0 = hid[v], h1 = hid[v + 32];
 #pragma unroll
-                for (int q = 0; q < 4; ++q) acc[q] = dot8(w1[q], h1, dot8(w0[q], h0, acc[q]));
-            }
-            for (; v < nv; v += 32) {
-                const uint4 h = hid[v];
-#pragma unroll
-                for (int q = 0; q < 4; ++q) acc[q] = dot8(__ldg(wp[q] + v), h, acc[q]);
+                for (int u = 0; u < 8; ++u) {
+                    const int v = v0 + 32 * u;
+                    if (v < nv) {
+                        const uint4 h = hid[v];
+                        acc[0] = dot8(xa[u], h, acc[0]);
+                        acc[1] = dot8(xb[u], h, acc[1]);
+                    }
+                }
             }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
-#pragma unroll
-                for (int q = 0; q < 4; ++q) acc[q] += __shfl_xor_sync(FULL, acc[q], o);
+                acc[0] += __shfl_xor_sync(FULL, acc[0], o);
+                acc[1] += __shfl_xor_sync(FULL, acc[1], o);
             }
 #pragma unroll
-            for (int q = 0; q < 4; ++q)
+            for (int q = 0; q < 2; ++q)
                 if (j + q < j1) {
+                    const int tq = q ? tb : ta;
                     if (SAMPLE)
-                        head_update_sample(m, s, kb, idx, yb, fmaxf(acc[q], -INFINITY), tq[q], j + q, f.inv_tau, row_key);
+                        head_update_sample(m, s, kb, idx, yb, fmaxf(acc[q], -INFINITY), tq, j + q, f.inv_tau, row_key);
                     else
                         online_update(m, s, idx, fmaxf(acc[q], -INFINITY), j + q);  // NaN -> -inf
                 }
@@ -359,9 +414,49 @@ __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadAr
             float rk = (lane < HG_WARPS) ? s_k[lane] : -INFINITY;
             float ry = (lane < HG_WARPS) ? s_y[lane] : -INFINITY;
             head_warp_combine<SAMPLE>(rm, rs, ri, rk, ry);
-            const TileMeta mt{slot, 0, 0, st, lo, deg, 0};
-            finalize_row(f, head_view(f), nullptr, mt, rm, rs, ri, lane, true, SAMPLE, ry);
+            if (np == 1) {
+                const TileMeta mt{slot, 0, 0, st, lo, deg, 0};
+                finalize_row(f, head_view(f), nullptr, mt, rm, rs, ri, lane, true, SAMPLE, ry);
+            } else if (lane == 0) {
+                a.gpartials[(long long)g * HG_MAX_PIECES + p] = HeadPartial{rm, rs, ri, rk, ry, {0, 0, 0}};
+            }
         }
+    }
+}
+
+// Gathered rows cut into several pieces: one warp per row merges the piece results in a fixed order (lane l takes
+// the pieces l, l + 32, ascending, then the butterfly), then the CSR transition and the accept test.
+template <bool SAMPLE>
+__global__ void head_gather_finish_kernel(const HeadArgs a) {
+    const StepArgs& f = a.fin;
+    const int n_gather = __ldcg(a.hctr + 1);
+    const int lane = threadIdx.x & 31;
+    const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int nwarps = (gridDim.x * blockDim.x) >> 5;
+    for (int g = warp; g < n_gather; g += nwarps) {
+        const int slot = __ldcg(a.gather_slot + g);
+        const int st = __ldcg(a.gather_state + g);
+        const long long lo = __ldg(f.dfa.row_ptr + st);
+        const int deg = (int)(__ldg(f.dfa.row_ptr + st + 1) - lo);
+        const int np = hg_pieces(deg);
+        if (np == 1) continue;  // finished by its gather CTA
+        float m = -INFINITY, s = 0.0f, kb = -INFINITY, yb = -INFINITY;
+        int idx = 0x7FFFFFFF;
+        for (int q = lane; q < np; q += 32) {
+            const int4* pp = reinterpret_cast<const int4*>(a.gpartials + (long long)g * HG_MAX_PIECES + q);
+            const int4 p = __ldcg(pp);
+            if (SAMPLE) {
+                const int4 p2 = __ldcg(pp + 1);
+                int dummy = 0;
+                online_combine(m, s, dummy, __int_as_float(p.x), __int_as_float(p.y), 0);
+                head_sample_combine(kb, idx, yb, __int_as_float(p.w), p.z, __int_as_float(p2.x));
+            } else {
+                online_combine(m, s, idx, __int_as_float(p.x), __int_as_float(p.y), p.z);
+            }
+        }
+        head_warp_combine<SAMPLE>(m, s, idx, kb, yb);
+        const TileMeta mt{slot, 0, 0, st, lo, deg, 0};
+        finalize_row(f, head_view(f), nullptr, mt, m, s, idx, lane, true, SAMPLE, yb);
     }
 }
 

@@ -864,7 +864,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             }
             if (!last) return;
             if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, dbg_rec, 4);
-            const unsigned ck2 = CD_CLOCK();
+            [[maybe_unused]] const unsigned ck2 = CD_CLOCK();
             int q0 = 0, q1 = 0;
             if (MODE == MODE_FLOW && lane == 0) {  // how busy the machine is, for the split of the row's next step
                 q0 = ld_relaxed_gpu_s32(F->q + 0);
@@ -928,7 +928,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             }
             warp_combine_s<SAMPLE>(rm, rs, ri, rk);
             if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, dbg_rec, 5);
-            const unsigned ck3 = CD_CLOCK();
+            [[maybe_unused]] const unsigned ck3 = CD_CLOCK();
             if (MODE == MODE_FLOW && lane == 0) CD_DBG_CYC(F, dbg_rec, 11, ck3 - ck2);
             // SAMPLE: the tempered logit of the sampled token is re-read from the logits row
             float ytok = 0.0f;
@@ -1030,7 +1030,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             unit_done(p1 - p0, npieces, true);
         } else {
             if (MODE == MODE_FLOW && lane == 0 && (mt.flags & FLAG_FIRST)) CD_DBG_MIN(F, dbg_rec, 7);
-            const unsigned ck0 = CD_CLOCK();
+            [[maybe_unused]] const unsigned ck0 = CD_CLOCK();
             if (MODE == MODE_FLOW && lane == 0) CD_DBG_CYC(F, dbg_rec, 8, ck0 - (unsigned)mt.pad[1]);
             if (mt.flags & FLAG_FIRST) reset_chains();
             const uint32_t row_key = SAMPLE ? rng_row_key(a.seed_lo, a.seed_hi, orig_row(), (uint32_t)rng_step) : 0u;
@@ -1121,7 +1121,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                     }
                 }
             }
-            const unsigned ck1 = CD_CLOCK();
+            [[maybe_unused]] const unsigned ck1 = CD_CLOCK();
             if (MODE == MODE_FLOW && lane == 0) CD_DBG_CYC(F, dbg_rec, 9, ck1 - ck0);
             if (mt.flags & FLAG_LAST) {  // the chunk is complete
                 float rm, rs, rk;

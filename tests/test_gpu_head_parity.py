@@ -260,6 +260,37 @@ def test_full_size_configs(cd, oracle, full_head, kind, name, n_check):
     run_case(cd, oracle, aut, dfa, hid, W_cpu, H, states, exact=(kind == "exact"), check=check, W_dev=W_dev)
 
 
+@pytest.mark.parametrize("kind", ["exact", "gauss"])
+@pytest.mark.parametrize("n,gathered", [(14, True), (36, True), (64, False)])
+def test_late_step_of_c3_few_rows_of_big_states(cd, oracle, full_head, kind, n, gathered):
+    """A late step of an early-exit loop on c3 (V = 262144, states of ~5243 transitions): with the automatic
+    policy a handful of rows is GATHERED -- every row cut into 41 pieces over as many CTAs, merged by
+    head_gather_finish_kernel -- as long as the rows together touch fewer than 0.8 V rows of W; above, the dense
+    contraction runs.  Every row against the oracle, and the automatic result against the forced dense and forced
+    gather ones (tokens / states identical on exact inputs)."""
+    V, H, Ws = full_head
+    W_dev, W_cpu = Ws[kind]
+    cfg = wl.CONFIGS["c3"]
+    aut = wl.build_automaton(cfg)
+    deg = np.diff(np.asarray(aut.row_ptr))
+    states = live_states(aut, n, mult=7)
+    assert (float(deg[states].sum()) < 0.8 * V) == gathered  # which side of the policy this case is on
+    hid = wl.make_hidden(cfg.seed, 5, n, H, exact=(kind == "exact"))
+    dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device="cuda:0")
+    run_case(cd, oracle, aut, dfa, hid, W_cpu, H, states, exact=(kind == "exact"), W_dev=W_dev)
+    if kind == "exact":
+        res = []
+        for g in (-1, 0, 2**30):
+            dfa.set_head_gather_max(g)
+            st = torch.tensor(states, dtype=torch.int32, device="cuda:0")
+            tok, lp, lse, done = cd.head_step(dfa, hid.to("cuda:0"), W_dev, st, H=H)
+            res.append((tok.cpu(), st.cpu(), done.cpu(), lse.cpu()))
+        for r in res[1:]:
+            assert torch.equal(res[0][0], r[0]) and torch.equal(res[0][1], r[1]) and torch.equal(res[0][2], r[2])
+            assert torch.allclose(res[0][3], r[3], rtol=0, atol=2e-5)
+    dfa.close()
+
+
 # ---------------------------------------------------------------- decode loop on the head step
 @pytest.mark.parametrize("kind,V,H,B,steps", [("dfa", 3000, 128, 300, 8), ("trie", 2000, 192, 150, 5),
                                               ("dfa", 700, 64, 1, 4)])
