@@ -116,7 +116,7 @@ struct StepBufs {  // sized by rows; replaced as a whole when the area grows
     int* trace_n = nullptr;                             // [LOOP_TRACE_STEPS + 1]
     unsigned long long* phase = nullptr;                // tuning builds: [LOOP_TRACE_STEPS][8]
     // flow_kernel (row tasks)
-    int* f_q = nullptr;                                      // [8] see cd::FlowArgs
+    int* f_q = nullptr;                                      // [FQ_INTS] see cd::FlowArgs
     unsigned long long* f_trace_t[2] = {nullptr, nullptr};  // [LOOP_TRACE_STEPS + 1] each
     int* f_trace_n[2] = {nullptr, nullptr};
 
@@ -309,14 +309,14 @@ cd_status alloc_step_bufs(const cd_dfa* d, int rows, StepBufs* out) {
     A(dev_alloc(&n.bar, 4));
     A(dev_alloc(&n.trace_t, (size_t)cd::LOOP_TRACE_STEPS + 1));
     A(dev_alloc(&n.trace_n, (size_t)cd::LOOP_TRACE_STEPS + 1));
-    A(dev_alloc(&n.f_q, 8));
+    A(dev_alloc(&n.f_q, cd::FQ_INTS));
     for (int i = 0; i < 2; ++i) {
         A(dev_alloc(&n.f_trace_t[i], (size_t)cd::LOOP_TRACE_STEPS + 1));
         A(dev_alloc(&n.f_trace_n[i], (size_t)cd::LOOP_TRACE_STEPS + 1));
         if (e == cudaSuccess) e = cudaMemset(n.f_trace_t[i], 0, sizeof(unsigned long long) * ((size_t)cd::LOOP_TRACE_STEPS + 1));
         if (e == cudaSuccess) e = cudaMemset(n.f_trace_n[i], 0, sizeof(int) * ((size_t)cd::LOOP_TRACE_STEPS + 1));
     }
-    if (e == cudaSuccess) e = cudaMemset(n.f_q, 0, sizeof(int) * 8);  // (the stop word 0 is never a launch generation)
+    if (e == cudaSuccess) e = cudaMemset(n.f_q, 0, sizeof(int) * cd::FQ_INTS);  // (the stop word 0 is never a launch generation)
 #ifdef CD_TUNING
     A(dev_alloc(&n.phase, (size_t)cd::LOOP_TRACE_STEPS * 8));
 #endif
@@ -1377,7 +1377,7 @@ cd_status cd_loop_trace(const cd_dfa_t* d, void* cuda_stream, int32_t cap, int64
         } else if (it != dm->scratch.end() && it->second.trace_src == 2) {
             // flow_kernel: the buffers of the last launch are the ones the launch counter's parity no longer names
             int par = 0;
-            CU(cudaMemcpyAsync(&par, it->second.b.f_q + 5, sizeof(int), cudaMemcpyDeviceToHost, stream));
+            CU(cudaMemcpyAsync(&par, it->second.b.f_q + cd::FQ_LAUNCHES, sizeof(int), cudaMemcpyDeviceToHost, stream));
             CU(cudaStreamSynchronize(stream));
             tt = it->second.b.f_trace_t[(par & 1) ^ 1];
             tn = it->second.b.f_trace_n[(par & 1) ^ 1];

@@ -102,6 +102,10 @@ constexpr unsigned long long LOOP_SPIN_TIMEOUT_NS = 4000000000ull;  // a barrier
 constexpr int FLOW_IDLE_LIMIT = 1 << 23;   // idle polls (>= 128 ns apart: > 1 s) after which a worker of flow_kernel gives up
 constexpr int MERGE_SPIN_LIMIT = 1 << 24;  // polls (>= 32 ns apart) after which a merging warp gives up
 constexpr int FLOW_ENTRY_WORDS = 8;        // 64-byte queue entries (5 words used)
+// flow_kernel's counters, one 128-byte line each (the stop word is polled by every idle warp: kept away from the
+// lines the unit draws and the publications hit with atomics)
+constexpr int FQ_DRAWN = 0, FQ_PUBLISHED = 32, FQ_FINISHED = 64, FQ_STOP = 96, FQ_ERRORS = 128, FQ_LAUNCHES = 129;
+constexpr int FQ_INTS = 160;
 
 // tiles per chunk / chunks per row of a row of `tiles_per_row` tiles
 __host__ __device__ inline int chunk_tiles(int tiles_per_row) {
@@ -361,7 +365,7 @@ __device__ __forceinline__ void flow_row_leaves(const StepArgs& a, const StepVie
         a.hist_sum_logprob[rid] = sum;
         a.hist_done[rid] = done;
         atomicMax(sv.trace_n + LOOP_TRACE_STEPS, steps);  // steps run = the most any row ran
-        if (atomicAdd(F.q + 2, 1) == F.B - 1) atomicExch(F.q + 3, (int)sv.gen);
+        if (atomicAdd(F.q + FQ_FINISHED, 1) == F.B - 1) atomicExch(F.q + FQ_STOP, (int)sv.gen);
     }
 }
 
@@ -409,7 +413,7 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& 
             ns = packed & 0x7FFFFFFF;
             dn = (packed < 0) ? 1 : 0;
         } else {
-            atomicAdd(MODE == MODE_FLOW ? F->q + 4 : a.ctrs + 2, 1);
+            atomicAdd(MODE == MODE_FLOW ? F->q + FQ_ERRORS : a.ctrs + 2, 1);
             token = -1;
         }
         const int slot = (MODE == MODE_STEP) ? mt.slot : mt.lrow;
@@ -455,7 +459,7 @@ __device__ __forceinline__ void finalize_row(const StepArgs& a, const StepView& 
             const long long backlog = units0 + q1 - q0;
             const int np = (backlog >= F->th[0]) ? F->np_lvl[0] : ((backlog >= F->th[1]) ? F->np_lvl[1] : ((backlog >= F->th[2]) ? F->np_lvl[2] : F->np_lvl[3]));
             unsigned e0 = 0;
-            if (lane == 0) e0 = (unsigned)atomicAdd(F->q + 1, np);
+            if (lane == 0) e0 = (unsigned)atomicAdd(F->q + FQ_PUBLISHED, np);
             e0 = __shfl_sync(FULL, e0, 0);
             const unsigned w0 = (unsigned)mt.lrow, w1 = (unsigned)ns, w2 = __float_as_uint(sum), w3 = (unsigned)(step + 1);
             for (int i = lane; i < np; i += 32) {
@@ -561,7 +565,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
     bool all_done = false;      // MODE_FLOW: every row has left the loop
     bool poll_pending = false;  // MODE_FLOW: poll_w / poll_stop hold the loads issued for the unit in next_u_l0
     unsigned long long poll_w = 0;
-    int poll_stop = 0;
+    int poll_stop = 0, poll_n = 0;
     long long units0 = 0;  // MODE_FLOW: implicit units (the first step of every row)
     if (MODE != MODE_FLOW) {
         unit_ctx_split<WARPS, GATHER>(cur, a, sv.n, tiles_per_row, tpu_max);
@@ -571,7 +575,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
     } else {
         unit_ctx_split<WARPS, GATHER>(cur, a, F->B, tiles_per_row, tpu_max);
         units0 = (long long)F->B * cur.P;
-        cur.work = F->q + 0;
+        cur.work = F->q + FQ_DRAWN;
         if (lane == 0) next_u_l0 = atomicAdd(cur.work, 1);
     }
     const bool ragged_row = (V % TILE_TOK) != 0;
@@ -614,7 +618,8 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                         if (poll_pending && (unsigned)__shfl_sync(FULL, poll_stop, 5) == sv.gen) all_done = true;
                         poll_w = 0;
                         if (lane < 5) poll_w = ld_relaxed_gpu_u64(F->task + (size_t)(e & F->cap_mask) * FLOW_ENTRY_WORDS + lane);
-                        if (lane == 5) poll_stop = ld_relaxed_gpu_s32(F->q + 3);
+                        // (the stop word only every 4th look: all idle warps read that one line)
+                        if (lane == 5 && (poll_n++ & 3) == 0) poll_stop = ld_relaxed_gpu_s32(F->q + FQ_STOP);
                         poll_pending = true;
                         return false;
                     }
@@ -804,7 +809,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             if (MODE != MODE_FLOW || all_done) break;
             __nanosleep(a.idle_ns);  // this warp's next unit is not published yet
             if (++idle_polls > FLOW_IDLE_LIMIT) {  // never on a healthy run: fail the call, do not hang
-                if (lane == 0) atomicAdd(F->q + 4, 1);
+                if (lane == 0) atomicAdd(F->q + FQ_ERRORS, 1);
                 break;
             }
             continue;
@@ -867,8 +872,8 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             [[maybe_unused]] const unsigned ck2 = CD_CLOCK();
             int q0 = 0, q1 = 0;
             if (MODE == MODE_FLOW && lane == 0) {  // how busy the machine is, for the split of the row's next step
-                q0 = ld_relaxed_gpu_s32(F->q + 0);
-                q1 = ld_relaxed_gpu_s32(F->q + 1);
+                q0 = ld_relaxed_gpu_s32(F->q + FQ_DRAWN);
+                q1 = ld_relaxed_gpu_s32(F->q + FQ_PUBLISHED);
             }
             __syncwarp();
             float rm = -INFINITY, rs = 0.0f, rk = -INFINITY;
@@ -909,7 +914,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 if (__all_sync(FULL, all_ok)) break;
                 __nanosleep(32);
                 if (++spins > MERGE_SPIN_LIMIT) {  // never on a healthy run: fail the call, do not hang
-                    if (lane == 0) atomicAdd(MODE == MODE_FLOW ? F->q + 4 : a.ctrs + 2, 1);
+                    if (lane == 0) atomicAdd(MODE == MODE_FLOW ? F->q + FQ_ERRORS : a.ctrs + 2, 1);
                     break;
                 }
             }
@@ -958,7 +963,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                         if (a.done_out) a.done_out[slot] = 1;
                     }
                     if (mt.flags & FLAG_BADSTATE) {
-                        atomicAdd(MODE == MODE_FLOW ? F->q + 4 : a.ctrs + 2, 1);
+                        atomicAdd(MODE == MODE_FLOW ? F->q + FQ_ERRORS : a.ctrs + 2, 1);
                         if (MODE != MODE_FLOW && a.hist_tokens) {  // the row leaves the loop here, undone, in the state it has
                             const long long rid = orig_row();
                             a.hist_final_state[rid] = mt.st;
@@ -1358,7 +1363,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1) flow_kernel(const StepArgs a, c
     }
     __syncwarp();
     const unsigned gen0 = (unsigned)__ldcg(a.ctrs + 3);
-    const int par = __ldcg(F.q + 5) & 1;
+    const int par = __ldcg(F.q + FQ_LAUNCHES) & 1;
     StepView sv{};
     sv.gen = gen0;
     sv.trace_t = F.trace_t[par];
@@ -1384,12 +1389,12 @@ __global__ void __launch_bounds__(WARPS * 32, 1) flow_kernel(const StepArgs a, c
             a.ctrs[3] = (int)(gen0 + (unsigned)a.max_steps + 1u);
             const int steps = __ldcg(sv.trace_n + LOOP_TRACE_STEPS);
             sv.trace_t[steps < LOOP_TRACE_STEPS ? steps : LOOP_TRACE_STEPS] = global_timer_ns();
-            const int err = __ldcg(F.q + 4) + ((__ldcg(F.q + 2) == F.B) ? 0 : 1);  // every row must have left
-            F.q[0] = 0;
-            F.q[1] = 0;
-            F.q[2] = 0;
-            F.q[4] = 0;
-            F.q[5] = par ^ 1;
+            const int err = __ldcg(F.q + FQ_ERRORS) + ((__ldcg(F.q + FQ_FINISHED) == F.B) ? 0 : 1);  // every row must have left
+            F.q[FQ_DRAWN] = 0;
+            F.q[FQ_PUBLISHED] = 0;
+            F.q[FQ_FINISHED] = 0;
+            F.q[FQ_ERRORS] = 0;
+            F.q[FQ_LAUNCHES] = par ^ 1;
             // (sticky until the host reads and clears it: cd_loop_sync reports every loop enqueued since the last one)
             if (err) atomicAdd_system(F.host_status, err);
         }
