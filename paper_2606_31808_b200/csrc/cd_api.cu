@@ -90,6 +90,7 @@ int units_per_warp() { static const int v = tune_int("CD_UPW", cd::UNITS_PER_WAR
 int tpu_max_tiles() { static const int v = tune_int("CD_TPU_MAX", cd::TPU_MAX_BYTES / STEP_TILE, 1, cd::TPU_MAX_BYTES / STEP_TILE); return v; }
 bool use_pdl() { static const int v = tune_int("CD_PDL", 1, 0, 1); return v != 0; }
 int flow_idle_ns() { static const int v = tune_int("CD_IDLE_NS", 32, 0, 100000); return v; }  // sleep between two polls of an unpublished task
+bool head_pairs_enabled() { static const int v = tune_int("CD_HEAD_PAIRS", 1, 0, 1); return v != 0; }  // cta_group::2 kernel for > 128 dense rows
 int host_gather_mult() { static const int v = tune_int("CD_HOST_GATHER_CTAS", 4, 1, 64); return v; }  // flat from 2 to 32 (51 GB/s on PCIe Gen5 x16)
 
 // Per (handle, stream) scratch.  Operations on one stream are ordered, so one area per stream
@@ -227,6 +228,7 @@ struct cd_dfa {
     long long w_ld = 0;
     int w_H = 0;
     CUtensorMap w_tmap{};
+    CUtensorMap w_tmap_half{};  // the same with boxes of HD_BN / 2 rows (CTA-pair kernel: each CTA loads half a W tile)
     std::mutex mu;  // guards cfg, the weight map cache and the scratch map
     Settings cfg;
     std::map<cudaStream_t, Scratch> scratch;
@@ -1660,15 +1662,20 @@ cd_status check_head_layout(const void* hidden, long long ldh, const void* W, lo
 }
 
 // tensor map of the output embedding, cached per handle (the weights rarely change)
-cd_status head_weight_map(const cd_dfa* d, const void* W, long long ldw, int H, CUtensorMap* out) {
+cd_status head_weight_map(const cd_dfa* d, const void* W, long long ldw, int H, CUtensorMap* out, CUtensorMap* out_half) {
     cd_dfa* dm = const_cast<cd_dfa*>(d);
     std::lock_guard<std::mutex> lk(dm->mu);
     if (dm->w_ptr != W || dm->w_ld != ldw || dm->w_H != H) {
         cd_status st = make_tmap_bf16(&dm->w_tmap, W, d->dev.V, H, ldw, cd::HD_BN);
-        if (st != CD_OK) return st;
+        if (st == CD_OK) st = make_tmap_bf16(&dm->w_tmap_half, W, d->dev.V, H, ldw, cd::HD2_HALF_N);
+        if (st != CD_OK) {
+            dm->w_ptr = nullptr;
+            return st;
+        }
         dm->w_ptr = W; dm->w_ld = ldw; dm->w_H = H;
     }
     *out = dm->w_tmap;  // copied under the lock: concurrent callers may use different weights
+    *out_half = dm->w_tmap_half;
     return CD_OK;
 }
 
@@ -1735,11 +1742,14 @@ cd_status launch_head(const cd_dfa* d, const Settings& cfg, Scratch* s, const vo
     a.partials = s->h_partials;
 
     const int n = n_upper;
-    CUtensorMap tmW;
+    CUtensorMap tmW, tmWh;
     {
-        const cd_status stw = head_weight_map(d, W, ldw, H, &tmW);
+        const cd_status stw = head_weight_map(d, W, ldw, H, &tmW, &tmWh);
         if (stw != CD_OK) return stw;
     }
+    // CTA pairs (thread-block clusters of 2) for calls with more than one row tile: needs an even number of SMs in
+    // the grid and a batch that can have > 128 dense rows at all
+    a.pairs = (head_pairs_enabled() && (d->num_sms % 2) == 0 && n_upper >= cd::HD2_MIN_ROWS) ? 1 : 0;
     cd::head_prepare_kernel<<<1, 1024, 0, stream>>>(a);
     CU(cudaGetLastError());
     const bool any_gather = (a.gather_max > 0 && d->min_deg_nonacc <= a.gather_max) || (a.gather_auto && d->max_deg > a.gather_max);
@@ -1779,6 +1789,20 @@ cd_status launch_head(const cd_dfa* d, const Settings& cfg, Scratch* s, const vo
             cfg_dev2 = d->device;
         }
         const int fin_blocks = (n + rows_per_block - 1) / rows_per_block;
+        if (a.pairs) {
+            static thread_local int cfg_dev3 = -1;
+            if (cfg_dev3 != d->device) {
+                CU(cudaFuncSetAttribute(cd::head_dense2_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, cd::HD2_SMEM_BYTES));
+                CU(cudaFuncSetAttribute(cd::head_dense2_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, cd::HD2_SMEM_BYTES));
+                cfg_dev3 = d->device;
+            }
+            // (the kernel carries __cluster_dims__(2, 1, 1); each of the two dense kernels returns at once when the
+            // number of dense rows, known on the device only, puts the call in the other one's range)
+            if (sample) cd::head_dense2_kernel<true><<<d->num_sms, cd::HD_THREADS, cd::HD2_SMEM_BYTES, stream>>>(s->h_tmA, tmWh, a);
+            else cd::head_dense2_kernel<false><<<d->num_sms, cd::HD_THREADS, cd::HD2_SMEM_BYTES, stream>>>(s->h_tmA, tmWh, a);
+            CU(cudaGetLastError());
+            ++launches;
+        }
         if (sample) {
             cd::head_dense_kernel<true><<<d->num_sms, cd::HD_THREADS, cd::HD_SMEM_BYTES, stream>>>(s->h_tmA, tmW, a);
             CU(cudaGetLastError());

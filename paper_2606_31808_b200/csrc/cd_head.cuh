@@ -125,6 +125,31 @@ __host__ inline long long head_partials_cap(int n) {
     return (long long)HD_BM * (HD_UNITS_TARGET + 2 * num_m + 2);
 }
 
+// ---- CTA-pair variant of the dense contraction (head_dense2_kernel, below)
+constexpr int HD2_STAGES = 6;
+constexpr int HD2_HALF_N = HD_BN / 2;                      // W rows each CTA loads
+constexpr int HD2_B_BYTES = HD2_HALF_N * HD_BK * 2;        // 16 KiB
+constexpr int HD2_STAGE_BYTES = HD_A_BYTES + HD2_B_BYTES;  // 32 KiB
+constexpr int HD2_SMEM_BYTES = HD2_STAGES * HD2_STAGE_BYTES + 1024;
+constexpr int HD2_UNITS_TARGET = 74 * 8;
+constexpr int HD2_MIN_ROWS = HD_BM + 1;  // dense rows from which the pair kernel takes over
+
+__host__ __device__ inline HeadSched head_sched2(int n_dense, int V) {  // num_m counts PAIRS of row tiles here
+    HeadSched h;
+    h.num_m = (n_dense + 2 * HD_BM - 1) / (2 * HD_BM);
+    h.num_n = (V + HD_BN - 1) / HD_BN;
+    int nu0 = h.num_m > 0 ? (HD2_UNITS_TARGET + h.num_m - 1) / h.num_m : 1;
+    if (nu0 > h.num_n) nu0 = h.num_n;
+    if (nu0 < 1) nu0 = 1;
+    h.L = (h.num_n + nu0 - 1) / nu0;
+    h.NU = (h.num_n + h.L - 1) / h.L;
+    return h;
+}
+// partial results per dense row, whichever kernel runs the contraction
+__host__ __device__ inline int head_row_partials(int n_dense, int V, int pairs) {
+    return (pairs && n_dense >= HD2_MIN_ROWS) ? head_sched2(n_dense, V).NU : head_sched(n_dense, V).NU;
+}
+
 struct HeadArgs {
     StepArgs fin;  // dfa, outputs, sticky counters, optional loop history (see finalize_row);
                    // fin.state_new == fin.state: nothing reads state[] after head_prepare_kernel
@@ -138,6 +163,7 @@ struct HeadArgs {
                      // total (a late step of an early-exit loop), they are gathered too instead of streaming all of W
     int gp_max;      // most pieces a gathered row of this call can have (bounds the item index)
     HeadPartial* gpartials;  // [rows][HG_MAX_PIECES] piece results of the gathered rows cut into several pieces
+    int pairs;       // the CTA-pair kernel (head_dense2_kernel) is launched too and takes the calls with > 128 dense rows
     // scratch
     uint8_t* not_dense;   // [n]
     uint8_t* not_gather;  // [n]
@@ -474,6 +500,7 @@ head_dense_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     __shared__ uint32_t s_tmem;
 
     const int n_dense = __ldcg(a.hctr + 0);
+    if (a.pairs && n_dense >= HD2_MIN_ROWS) return;  // uniform: head_dense2_kernel (CTA pairs) runs this call
     const HeadSched hs = head_sched(n_dense, a.fin.dfa.V);
     if (hs.num_m == 0) return;  // uniform: nothing was allocated yet
     const int total_units = hs.num_m * hs.NU;
@@ -631,6 +658,235 @@ head_dense_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant
     if (warp == 1) tmem_dealloc(tmem, HD_TMEM_COLS);
 }
 
+// ---------------------------------------------------------------- dense, CTA pairs (cta_group::2)
+// The same contraction on pairs of SMs (thread-block cluster of 2, tcgen05.mma.cta_group::2, UMMA 256 x 256 x 16):
+// a pair owns a tile of 256 rows x 256 tokens.  Per k-block each CTA loads ITS 128 rows of A and ITS 128 tokens of
+// the W tile (32 KiB instead of 48 KiB: the tensor cores of both SMs read both halves of W), so the shared-memory
+// ring holds 6 stages instead of 4 (2.3 us of look-ahead instead of 1.5) and the L2 -> SM operand traffic drops by a
+// third.  Only the leader (cluster rank 0) issues MMAs; each CTA keeps the accumulator rows of its own 128 rows in
+// its own TMEM and runs the same masked online-softmax epilogue as head_dense_kernel.
+//   full[s]   (leader's): both producers' bytes (the TMA loads name the leader's barrier) + one arrival from each
+//   empty[s]  (own): tcgen05.commit multicast to both CTAs
+//   tfull[b]  (own): tcgen05.commit multicast;  tempty[b] (leader's): 4 epilogue warps of each CTA
+// Used when more than 128 rows are dense (two row tiles or more); head_dense_kernel keeps the single-tile case.
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// one arrival on the mbarrier at the same shared-memory offset in CTA `cta` of the cluster
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar, uint32_t cta) {
+    asm volatile(
+        "{\n\t"
+        ".reg .b32 r;\n\t"
+        "mapa.shared::cluster.u32 r, %0, %1;\n\t"
+        "mbarrier.arrive.shared::cluster.b64 _, [r];\n\t"
+        "}" ::"r"(bar),
+        "r"(cta)
+        : "memory");
+}
+constexpr uint32_t PEER_BIT_MASK = 0xFEFFFFFFu;  // clears the bit that tells the two CTAs of a pair apart: the leader's copy
+// 2-D tiled TMA load into THIS CTA's shared memory whose bytes complete on the LEADER's mbarrier
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const void* tmap, int c0, int c1, uint32_t bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(dst),
+        "l"(reinterpret_cast<uint64_t>(tmap)), "r"(c0), "r"(c1), "r"(bar & PEER_BIT_MASK)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_alloc_pair(uint32_t smem_dst, uint32_t ncols) {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc_pair(uint32_t taddr, uint32_t ncols) {
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+// one arrival on the mbarrier at this offset in BOTH CTAs once every MMA issued so far has completed
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+                 "h"((uint16_t)3)
+                 : "memory");
+}
+__device__ __forceinline__ void tc_mma_bf16_pair(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                                 uint32_t accumulate) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t"
+        "}" ::"r"(d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+template <bool SAMPLE>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(HD_THREADS, 1)
+head_dense2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmWh, const HeadArgs a) {
+    extern __shared__ __align__(1024) unsigned char hd_smem[];
+    __shared__ __align__(8) unsigned long long bar_full[HD2_STAGES], bar_empty[HD2_STAGES], bar_tfull[2], bar_tempty[2];
+    __shared__ uint32_t s_tmem;
+
+    const int n_dense = __ldcg(a.hctr + 0);
+    if (n_dense < HD2_MIN_ROWS) return;  // uniform over the grid: head_dense_kernel runs this call
+    const HeadSched hs = head_sched2(n_dense, a.fin.dfa.V);
+    const int total_units = hs.num_m * hs.NU;
+    const int num_k = (a.H + HD_BK - 1) / HD_BK;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const int cluster_id = blockIdx.x >> 1, num_clusters = gridDim.x >> 1;
+    const uint32_t tiles = (smem_u32(hd_smem) + 1023u) & ~1023u;
+
+    if (warp == 0 && lane == 0) {
+        tma_prefetch_desc(&tmA);
+        tma_prefetch_desc(&tmWh);
+#pragma unroll
+        for (int s = 0; s < HD2_STAGES; ++s) {
+            mbar_init(smem_u32(&bar_full[s]), 2);   // one arrival per producer (the peer's arrives remotely)
+            mbar_init(smem_u32(&bar_empty[s]), 1);  // tcgen05.commit, multicast
+        }
+#pragma unroll
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(smem_u32(&bar_tfull[b]), 1);
+            mbar_init(smem_u32(&bar_tempty[b]), 8);  // four epilogue warps of each CTA (leader's copy is the one waited on)
+        }
+        fence_mbar_init();
+    }
+    if (warp == 1) tmem_alloc_pair(smem_u32(&s_tmem), HD_TMEM_COLS);
+    tc_fence_before();
+    cluster_sync_all();  // barriers initialised and TMEM allocated in both CTAs before anyone signals the other
+    tc_fence_after();
+    const uint32_t tmem = s_tmem;
+
+    if (warp == 0) {
+        // ===== TMA producer (one lane, in both CTAs): its 128 rows of A, its 128 tokens of the W tile
+        if (lane == 0) {
+            int stage = 0;
+            uint32_t phase = 0;
+            for (int u = cluster_id; u < total_units; u += num_clusters) {
+                const int m_pair = u % hs.num_m, n_unit = u / hs.num_m;
+                const int nt0 = n_unit * hs.L, nt1 = min(nt0 + hs.L, hs.num_n);
+                for (int nt = nt0; nt < nt1; ++nt) {
+                    for (int kb = 0; kb < num_k; ++kb) {
+                        mbar_wait(smem_u32(&bar_empty[stage]), phase ^ 1u);
+                        const uint32_t bar = smem_u32(&bar_full[stage]);
+                        const uint32_t sa = tiles + stage * HD2_STAGE_BYTES;
+                        if (rank == 0) mbar_arrive_expect_tx(bar, 2 * HD2_STAGE_BYTES);
+                        else mbar_arrive_cluster(bar, 0);
+                        tma_load_2d_pair(sa, &tmA, kb * HD_BK, m_pair * 2 * HD_BM + (int)rank * HD_BM, bar);
+                        tma_load_2d_pair(sa + HD_A_BYTES, &tmWh, kb * HD_BK, nt * HD_BN + (int)rank * HD2_HALF_N, bar);
+                        if (++stage == HD2_STAGES) {
+                            stage = 0;
+                            phase ^= 1u;
+                        }
+                    }
+                }
+            }
+        }
+    } else if (warp == 1) {
+        // ===== MMA issuer (one lane of the leader)
+        if (lane == 0 && rank == 0) {
+            constexpr uint32_t idesc = umma_idesc_bf16(2 * HD_BM, HD_BN);
+            int stage = 0, ab = 0;
+            uint32_t phase = 0, aphase = 0;
+            for (int u = cluster_id; u < total_units; u += num_clusters) {
+                const int n_unit = u / hs.num_m;
+                const int nt0 = n_unit * hs.L, nt1 = min(nt0 + hs.L, hs.num_n);
+                for (int nt = nt0; nt < nt1; ++nt) {
+                    mbar_wait(smem_u32(&bar_tempty[ab]), aphase ^ 1u);  // both epilogues drained this buffer
+                    tc_fence_after();
+                    const uint32_t d_tmem = tmem + (uint32_t)ab * HD_BN;
+                    for (int kb = 0; kb < num_k; ++kb) {
+                        mbar_wait(smem_u32(&bar_full[stage]), phase);
+                        tc_fence_after();
+                        const uint32_t sa = tiles + stage * HD2_STAGE_BYTES;
+                        const uint64_t da = umma_desc_k_sw128(sa), db = umma_desc_k_sw128(sa + HD_A_BYTES);
+#pragma unroll
+                        for (int k = 0; k < HD_BK / HD_UK; ++k)
+                            tc_mma_bf16_pair(d_tmem, da + 2ull * k, db + 2ull * k, idesc, (kb | k) ? 1u : 0u);
+                        tc_commit_pair(smem_u32(&bar_empty[stage]));  // stage free in both CTAs once these MMAs have read it
+                        if (++stage == HD2_STAGES) {
+                            stage = 0;
+                            phase ^= 1u;
+                        }
+                    }
+                    tc_commit_pair(smem_u32(&bar_tfull[ab]));  // accumulator complete, both halves
+                    ab ^= 1;
+                    if (ab == 0) aphase ^= 1u;
+                }
+            }
+        }
+    } else {
+        // ===== epilogue (both CTAs): thread <-> accumulator row of this CTA's 128 rows
+        const int quad = warp & 3;
+        const int row_in_tile = quad * 32 + lane;
+        const DfaDev& dfa = a.fin.dfa;
+        int ab = 0;
+        uint32_t aphase = 0;
+        for (int u = cluster_id; u < total_units; u += num_clusters) {
+            const int m_pair = u % hs.num_m, n_unit = u / hs.num_m;
+            const int nt0 = n_unit * hs.L, nt1 = min(nt0 + hs.L, hs.num_n);
+            const int drow = m_pair * 2 * HD_BM + (int)rank * HD_BM + row_in_tile;
+            const bool valid = drow < n_dense;
+            const int st = valid ? __ldcg(a.dense_state + drow) : 0;
+            const uint32_t* mrow = dfa.mask + (long long)st * dfa.Wpad;
+            float m = -INFINITY, s = 0.0f, kb = -INFINITY, yb = -INFINITY;
+            int idx = 0x7FFFFFFF;
+            uint32_t row_key = 0u;
+            if (SAMPLE && valid) {
+                const int slot = __ldcg(a.dense_slot + drow);
+                row_key = rng_row_key(a.fin.seed_lo, a.fin.seed_hi,
+                                      (uint32_t)(a.fin.row_map ? __ldg(a.fin.row_map + slot) : slot),
+                                      (uint32_t)(a.fin.rng_step_base + a.fin.step));
+            }
+            for (int nt = nt0; nt < nt1; ++nt) {
+                const int n0 = nt * HD_BN;
+                uint32_t mw[8];
+                {
+                    const int w0 = n0 >> 5;
+                    uint4 lo4 = make_uint4(0, 0, 0, 0), hi4 = make_uint4(0, 0, 0, 0);
+                    if (valid && w0 + 3 < dfa.Wpad) lo4 = __ldg(reinterpret_cast<const uint4*>(mrow + w0));
+                    if (valid && w0 + 7 < dfa.Wpad) hi4 = __ldg(reinterpret_cast<const uint4*>(mrow + w0 + 4));
+                    mw[0] = lo4.x; mw[1] = lo4.y; mw[2] = lo4.z; mw[3] = lo4.w;
+                    mw[4] = hi4.x; mw[5] = hi4.y; mw[6] = hi4.z; mw[7] = hi4.w;
+                }
+                mbar_wait(smem_u32(&bar_tfull[ab]), aphase);
+                tc_fence_after();
+                const uint32_t tbase = tmem + ((uint32_t)(quad * 32) << 16) + (uint32_t)ab * HD_BN;
+#pragma unroll
+                for (int c = 0; c < HD_BN / 32; ++c) {
+                    const uint32_t bits = mw[c];
+                    if (__any_sync(FULL, bits != 0u)) {  // warp-uniform: skip columns nobody allows
+                        uint32_t v[32];
+                        tmem_ld32(tbase + c * 32, v);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int j = 0; j < 32; ++j)
+                            if ((bits >> j) & 1u) {
+                                if (SAMPLE)
+                                    head_update_sample(m, s, kb, idx, yb, fmaxf(__uint_as_float(v[j]), -INFINITY),
+                                                       n0 + c * 32 + j, n0 + c * 32 + j, a.fin.inv_tau, row_key);
+                                else
+                                    online_update(m, s, idx, fmaxf(__uint_as_float(v[j]), -INFINITY), n0 + c * 32 + j);
+                            }
+                    }
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive_cluster(smem_u32(&bar_tempty[ab]), 0);  // the leader's barrier
+                ab ^= 1;
+                if (ab == 0) aphase ^= 1u;
+            }
+            if (valid) a.partials[(long long)drow * hs.NU + n_unit] = HeadPartial{m, s, idx, kb, yb, {0, 0, 0}};
+        }
+    }
+    tc_fence_before();
+    cluster_sync_all();  // nobody leaves (or frees TMEM) while the other CTA may still read its shared memory / signal it
+    tc_fence_after();
+    if (warp == 1) tmem_dealloc_pair(tmem, HD_TMEM_COLS);
+}
+
 // ---------------------------------------------------------------- finish dense rows
 // One warp per dense row: partials merged in a fixed order (lane q % 32 takes ranges q, q + 32,
 // ... ascending, then the butterfly), then the CSR transition and the accept test.
@@ -638,7 +894,7 @@ template <bool SAMPLE>
 __global__ void head_finish_kernel(const HeadArgs a) {
     const StepArgs& f = a.fin;
     const int n_dense = __ldcg(a.hctr + 0);
-    const HeadSched hs = head_sched(n_dense, f.dfa.V);
+    const int NU = head_row_partials(n_dense, f.dfa.V, a.pairs);
     const int lane = threadIdx.x & 31;
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
     const int nwarps = (gridDim.x * blockDim.x) >> 5;
@@ -647,8 +903,8 @@ __global__ void head_finish_kernel(const HeadArgs a) {
         const int st = __ldcg(a.dense_state + d);
         float m = -INFINITY, s = 0.0f, kb = -INFINITY, yb = -INFINITY;
         int idx = 0x7FFFFFFF;
-        for (int q = lane; q < hs.NU; q += 32) {
-            const int4* pp = reinterpret_cast<const int4*>(a.partials + (long long)d * hs.NU + q);
+        for (int q = lane; q < NU; q += 32) {
+            const int4* pp = reinterpret_cast<const int4*>(a.partials + (long long)d * NU + q);
             const int4 p = __ldcg(pp);
             if (SAMPLE) {
                 const int4 p2 = __ldcg(pp + 1);
