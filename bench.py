@@ -263,6 +263,7 @@ def head_section(cd, cfg, aut, dfa, device, H, iters, warmup):
                 "note": "bytes = W rows touched (2H each), served by L2 when rows share a state; launch-latency bound at this size"}
     else:
         roof = None
+    hk = "cd::head_dense2_kernel" if n_dense > 128 else "cd::head_dense_kernel"  # which kernel ran the contraction
     head = {
         "workload": f"{cfg.name}: one cd_head_step, n={n} rows over the live states, V={V}, H={H} bf16 "
                     f"(Gemma 3 4B head shape, PAPER.md L191), {n_dense} rows dense / {n - n_dense} gathered",
@@ -270,13 +271,14 @@ def head_section(cd, cfg, aut, dfa, device, H, iters, warmup):
         "decode_loop": loop,
         "unfused_ms_per_step": ms_u, "library_gemm_ms": ms_g, "speedup_vs_unfused": ms_u / ms_f,
         "token_agreement_with_unfused_bf16_logits": agree,
-        "roofline": roof or {"bound": "tensor", "kernel": "cd::head_dense_kernel (tcgen05 128x256x64, masked online-softmax epilogue from TMEM)",
+        "roofline": roof or {"bound": "tensor", "kernel": hk + (" (CTA pairs: tcgen05 cta_group::2 256x256x16, 6-stage TMA ring, masked online-softmax epilogue from TMEM)"
+                                                               if n_dense > 128 else " (tcgen05 128x256x16, masked online-softmax epilogue from TMEM)"),
                      "achieved": ach, "peak": burst, "unit": "TFLOP/s", "frac": ach / burst if burst else None,
                      "peak_source": src, "frac_of_sustained_peak": ach / sustained if sustained else None,
                      "frac_of_nominal_2250": ach / 2250.0, "flops_per_launch": flops,
                      "note": "timed over the whole call (prepare + pack + contraction + finish), so the kernel's own rate is higher",
-                     "traffic": (ncu_traffic("cd::head_dense_kernel", cfg.name) or {}).get("bytes"),
-                     "traffic_source": (ncu_traffic("cd::head_dense_kernel", cfg.name) or {}).get("profile")},
+                     "traffic": (ncu_traffic(hk, cfg.name) or {}).get("bytes"),
+                     "traffic_source": (ncu_traffic(hk, cfg.name) or {}).get("profile")},
     }
     return head
 
