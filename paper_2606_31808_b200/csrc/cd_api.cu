@@ -565,6 +565,9 @@ cd::StepArgs make_step_args(const cd_dfa* d, const Settings& cfg, Scratch* s, cd
     a.upw = units_per_warp();
     a.tpu_max = tpu_max_tiles();
     a.idle_ns = flow_idle_ns();
+#ifdef CD_TUNING
+    a.force_p = tune_int_now("CD_FORCE_P", 0);
+#endif
     a.inv_tau = cfg.inv_tau;
     a.seed_lo = (uint32_t)(cfg.seed & 0xFFFFFFFFull);
     a.seed_hi = (uint32_t)(cfg.seed >> 32);

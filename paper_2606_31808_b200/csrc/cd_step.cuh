@@ -191,6 +191,7 @@ struct StepArgs {
     // the original row for the history and the sampling noise)
     int logits_by_slot;
     int upw, tpu_max;  // unit sizing: target units per warp, most tiles per unit
+    int force_p;       // tuning builds: > 0 = units per dense row, whatever the number of rows
     int idle_ns;       // flow_kernel: sleep between two looks at an unpublished queue entry
 };
 
@@ -528,6 +529,7 @@ __device__ __forceinline__ void unit_ctx_split(UnitCtx& c, const StepArgs& a, in
     const int total_warps = gridDim.x * WARPS;
     c.n = n;
     c.Pd = units_per_row(n, tiles_per_row, total_warps, tpu_max, a.upw);  // units per row of a dense scan
+    if (a.force_p > 0) c.Pd = min(a.force_p, row_chunks(tiles_per_row));
     // a gathered row is split only as far as needed to give every warp a few units
     c.PG = GATHER ? max(1, min(c.Pd, (total_warps * GATHER_UPW) / max(n, 1))) : c.Pd;
     // units per row of this step; if every state is gathered no unit is drawn in vain

@@ -566,6 +566,33 @@ def test_results_do_not_depend_on_the_batch(cd, oracle, step_mode):
     dfa.close()
 
 
+@pytest.mark.parametrize("V,B,steps,S", [(262144, 8, 300, 64), (2048, 3000, 300, 48)])
+def test_long_loops_wrap_the_queue_ring(cd, oracle, V, B, steps, S):
+    """Loops far longer than anything the configs need: more steps than fit the kernel's parameter block (the step
+    pointers then live in device memory), more than the 256 steps the device-side trace records, and more queue
+    entries than the ring of the row-task kernel holds -- a few rows cut into 64 units per step (V = 262144), or
+    thousands of rows of one unit each (V = 2048) -- so the ring wraps several times and its tags (launch generation +
+    wrap count) are what tells a fresh entry from the one a slot held before.  Almost no state accepts, so most rows
+    run to max_steps.  All three loop kernels against the oracle."""
+    aut = wl.make_random_dfa(91, V, S, 0.01 if V > 4096 else 0.05, 0.004)
+    dfa = dev_dfa(cd, aut)
+    nbuf = 7  # the steps cycle through 7 logits buffers (the API takes one pointer per step)
+    bufs = [wl.make_logits(91, k, B, V, 2.0, torch.bfloat16, device="cuda:0") for k in range(nbuf)]
+    xs = [bufs[k % nbuf] for k in range(steps)]
+    want = oracle.decode_loop(aut, [x.cpu() for x in bufs] * (steps // nbuf + 1), max_steps=steps)
+    assert int((want["len"] == steps).sum()) > B // 4  # long-lived rows: the loop really is long
+    for lm in (cd.LOOP_AUTO, cd.LOOP_BARRIER, cd.LOOP_PER_STEP):
+        dfa.set_loop_mode(lm)
+        for rep in range(2):  # twice: the second launch finds the ring full of the first one's entries
+            out = cd.decode_loop(dfa, xs, max_steps=steps)
+            for k in ("tokens", "len", "final_state", "done"):
+                assert np.array_equal(out[k].cpu().numpy(), want[k]), (lm, rep, k)
+            slp = out["sum_logprob"].cpu().numpy().astype(np.float64)
+            assert np.all(np.abs(slp - want["sum_logprob"]) <= TOL * (want["len"] + np.abs(want["sum_logprob"])))
+    dfa.set_loop_mode(cd.LOOP_AUTO)
+    dfa.close()
+
+
 def test_bad_state_is_reported_through_the_outputs_and_does_not_stick(cd, oracle):
     """A slot whose state is outside [0, S): cd_step cannot fail asynchronously, it reports the slot as
     done with token -1 and keeps the state; the error counter of the scratch area must not leak into the
