@@ -593,6 +593,26 @@ def test_long_loops_wrap_the_queue_ring(cd, oracle, V, B, steps, S):
     dfa.close()
 
 
+@pytest.mark.parametrize("B", [1, 2, 32768, 32769, 50000])
+def test_loop_row_count_boundaries(cd, oracle, B):
+    """One row, two rows, the most rows a persistent loop kernel takes (32768), one more and many more (those run one
+    launch per decoding step): the same results from whichever kernel the library picks, in every loop mode."""
+    cfg = wl.scaled(wl.CONFIGS["c3"], V=1024, B=B, S=16, max_steps=4, density=0.06, dtype=torch.float32)
+    aut = wl.build_automaton(cfg)
+    dfa = dev_dfa(cd, aut)
+    logits = wl.build_step_logits(cfg, aut, device="cuda:0")
+    want = oracle.decode_loop(aut, [x.cpu() for x in logits])
+    for lm in (cd.LOOP_AUTO, cd.LOOP_BARRIER, cd.LOOP_PER_STEP):
+        dfa.set_loop_mode(lm)
+        got = cd.decode_loop(dfa, logits)
+        for k in ("tokens", "len", "final_state", "done"):
+            assert np.array_equal(got[k].cpu().numpy(), want[k]), (lm, k)
+        ok, worst = close(got["sum_logprob"].cpu().numpy(), want["sum_logprob"], tol=TOL * cfg.max_steps)
+        assert ok, (lm, worst)
+    dfa.set_loop_mode(cd.LOOP_AUTO)
+    dfa.close()
+
+
 def test_bad_state_is_reported_through_the_outputs_and_does_not_stick(cd, oracle):
     """A slot whose state is outside [0, S): cd_step cannot fail asynchronously, it reports the slot as
     done with token -1 and keeps the state; the error counter of the scratch area must not leak into the
