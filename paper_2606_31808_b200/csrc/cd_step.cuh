@@ -1,5 +1,5 @@
-// cd_step.cuh -- the fused constrained step (include/cd.h cd_step) and the
-// persistent whole-loop kernel built from the same step body (cd_decode_loop).
+// cd_step.cuh -- the fused constrained step (include/cd.h cd_step) and the two
+// persistent whole-loop kernels built from the same step body (cd_decode_loop).
 //
 // Design (B200-first; the paper gives no kernel):
 //   * The step is one streaming pass over the logits, so it is HBM-bound: the job is to keep
@@ -8,44 +8,39 @@
 //     cp.async.bulk -> SASS UBLKCP) completing on per-slot mbarriers: a logits tile and the
 //     matching piece of the state's allowed-token bitmask land together.  No register staging,
 //     no block-wide barriers in the streaming phase, WARPS*STAGES*TILE_BYTES in flight per SM.
-//   * Work unit = (active slot, part of the row).  Units are handed out by one global atomic
-//     counter (dynamic balance across the 148 SMs; the two dies do not run at the same speed);
-//     the number of tiles per unit is derived on the device from the number of active rows, so
-//     the same launch shape serves a full batch and the few-rows tail of an early-exit loop
-//     without any host read of the active count.
-//   * Per tile a lane walks the set bits of its mask words (warp-uniform trip count, branch
-//     free body) and updates an online (max, sum-exp, argmax) triple; only allowed elements
-//     cost arithmetic.
-//   * Unit results of a row are merged without any fence: a unit stores its result into a slot
-//     of three 64-bit words, each carrying the launch generation in its upper half (8-byte stores
-//     are single-copy atomic, so a word is either stale or complete), then takes a RELAXED
-//     ticket.  The warp that draws the last ticket merges: it reads the other slots and re-reads
-//     any word whose tag is not current yet (the writers issued those stores before their
-//     tickets, so they are on their way; normally the first read succeeds).  A __threadfence
-//     here cost 3.8 us per unit (profiles/r1b): it waits for the bulk copies the same warp still
-//     has in flight.  Electing the merger in advance instead (the warp holding a row's last part
-//     polls until the other parts are published: no atomic at all) was tried in round 2 and
-//     dropped: a waiting warp streams nothing, and with 8 units per row an eighth of the warps
-//     wait at any time -- c4 fell from 6.8 to 6.2 TB/s (profiles/r2_merge_election.md).
+//   * Work unit = (active slot, range of whole chunks of the row).  Units are handed out by one global
+//     atomic counter (dynamic balance across the 148 SMs; the two dies do not run at the same speed).
+//   * Per tile: a sparse tile (the normal case) is compacted across the warp -- one scan of the per-lane
+//     popcounts, the allowed positions in a small shared list -- and every lane evaluates its fair share of
+//     the ALLOWED elements only, updating an online (max, sum-exp, argmax) triple; a dense tile walks the set
+//     bits of the lane's mask words as independent chains.  Warp reductions go through the redux unit.
+//   * CANONICAL CHUNKS: a row is cut into chunks (a function of V and the logits type only); a chunk's result
+//     is a fixed function of its elements, the row's a fixed fold of its chunks' results.  How a launch cuts
+//     rows into units therefore never changes a bit of logprob / lse (see MAX_CHUNKS below).
+//   * Chunk results travel through HBM without any fence: three 64-bit words, each carrying the launch
+//     generation in its upper half (8-byte stores are single-copy atomic, so a word is either stale or
+//     complete); a unit then adds its number of chunks to the row's RELAXED ticket and whoever completes the
+//     row merges, re-reading any word whose tag is not current yet (the writers issued those stores before
+//     their tickets, so they are on their way; normally the first read succeeds).  A __threadfence here cost
+//     3.8 us per unit (profiles/r1b): it waits for the bulk copies the same warp still has in flight.
 //   * The merging warp finds the chosen token's position in the state's CSR row WITHOUT searching:
 //     position = number of allowed tokens below it = rank1k[state][t >> 10] (a per-state prefix
 //     count of mask bits per 1024 tokens, built once with the automaton) + popcount of the mask
 //     words of that block below t: one round trip instead of the 2-3 of a 128-ary search, then
 //     next[] (accepting[next] rides in bit 31), the output writes and, in the decode loop, the
 //     per-row history -- while the other warps keep streaming.
-//   * step_kernel: one launch = one step.  The last CTA to finish resets the work counter, bumps
-//     the generation and (per-step decode loops: callback / host-buffer forms) performs the
-//     stable early-exit compaction.
-//   * loop_kernel: one cooperative launch = the whole decode loop (cd_decode_loop).  148 CTAs stay
+//   * step_kernel: one launch = one step (cd_step; the callback / host-buffer loops).  The last CTA to finish
+//     resets the work counter, bumps the generation and (loops) performs the stable early-exit compaction.
+//   * loop_kernel: one cooperative launch = the whole decode loop in lock-step (LIMIT loops).  148 CTAs stay
 //     resident; between decoding steps they meet at a grid barrier (one arrival atomic per CTA,
 //     the last arriver publishes the go word).  There is no compaction pass at all: the active set
 //     is a bitmap over ORIGINAL row ids (three buffers in rotation: read / being built / being
 //     cleared), finished rows simply do not set their bit for the next step, and "slot i" of a
 //     step is the i-th set bit (rank/select on a shared-memory snapshot) -- which is exactly the
-//     ascending-row-id order the stable compaction of a6 produces.  States live in two arrays
-//     indexed by original row id (read k & 1, write (k + 1) & 1).  This removes, per decoding
-//     step, a kernel launch + grid drain, the counter reset, the last-CTA compaction and the
-//     active-count hand-off.
+//     ascending-row-id order the stable compaction of a6 produces.
+//   * flow_kernel: one plain launch = the whole decode loop with NO barrier (cd_decode_loop): every row
+//     advances through its steps on its own; the warp that finalises a row's step publishes the next one as
+//     entries of a queue ring, cut into more units the idler the machine is (see FlowArgs).
 //   * Density-adaptive rows (GATHER instantiation): a row whose state has at most
 //     `gather_max` transitions is not scanned at all -- its units walk pieces of the state's CSR
 //     token list (coalesced) and gather exactly the allowed logits (one 32-byte sector each, 8
