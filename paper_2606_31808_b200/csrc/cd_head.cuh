@@ -3,17 +3,21 @@
 //
 //   head_prepare_kernel  classifies the active slots by the density of their automaton state
 //                        (accepting / gathered / dense) and builds the two work lists;
-//   head_gather_kernel   low-density states (tries, option sets): one CTA per row forms exactly
-//                        the allowed logits as gathered dot products (W rows through the CSR
-//                        token list) and finishes the row (masked logsumexp/argmax, transition);
+//   head_gather_kernel   low-density states (tries, option sets) and, in a late step of an early-exit loop,
+//                        every row (automatic policy): work item = (row, piece of >= 128 transitions of its
+//                        CSR token list), one CTA each; forms exactly the allowed logits as gathered dot
+//                        products (W rows fetched in bursts) -- a one-piece row is finished by its CTA;
+//   head_gather_finish_kernel  merges the pieces of the longer rows (masked logsumexp/argmax, transition);
 //   head_pack_kernel     copies the hidden rows of the dense slots into a contiguous A operand;
-//   head_dense_kernel    the dense contraction on the 5th-gen tensor cores: persistent,
-//                        warp-specialised (TMA producer / tcgen05.mma issuer / 4 epilogue warps),
+//   head_dense_kernel    the dense contraction on the 5th-gen tensor cores for up to 128 dense rows:
+//                        persistent, warp-specialised (TMA producer / tcgen05.mma issuer / 4 epilogue warps),
 //                        128x256 fp32 accumulators double-buffered in TMEM, operands staged by
 //                        TMA into 128B-swizzled shared memory.  The epilogue reads the
 //                        accumulator rows with tcgen05.ld and applies the allowed-token bitmask
 //                        of each row's own state to an online (max, sum-exp, argmax) -- one
 //                        partial result per (row, range of vocabulary tiles);
+//   head_dense2_kernel   the same on CTA pairs (clusters of 2, tcgen05.mma.cta_group::2, UMMA 256x256x16) for
+//                        more than 128 dense rows: each CTA loads its 128 rows of A and half of the W tile;
 //   head_finish_kernel   merges the partials of a dense row in a fixed order and does the CSR
 //                        transition + accept test.
 #pragma once
