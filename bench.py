@@ -813,6 +813,27 @@ def main():
                    "h2d_gbs": h2d * k_e2e / dt / 1e9, "host_memory": "pinned"}
             got0 = cd.decode_loop(dfa, batches[0], max_steps=cfg.max_steps)
             assert torch.equal(out_h["tokens"], got0["tokens"].cpu()), "host-buffer loop disagrees with device loop"
+            # the same with the density-adaptive step (cd_set_gather_max(-1)): when every state may be gathered the
+            # step kernel pulls only the ALLOWED logits of the active rows over the link (a 32-byte sector each)
+            if not args.no_adaptive and args.gather_max == 0:
+                dfa.set_gather_max(-1)
+                out_a = None
+                for i in range(1 + k_e2e):
+                    if i == 1:
+                        barrier()
+                        t0 = time.perf_counter()
+                    out_a = cd.decode_loop_host(dfa, host, max_steps=cfg.max_steps, out=out_a)
+                barrier()
+                dta = time.perf_counter() - t0
+                dfa.set_gather_max(0)
+                assert torch.equal(out_a["tokens"], out_h["tokens"]), "adaptive host-buffer loop disagrees with the dense one"
+                sectors = int(sum(deg_k)) * 32
+                e2e["adaptive"] = {"value": rows_per_step_all_ranks * k_e2e / dta, "unit": UNIT, "ms_per_step": 1e3 * dta / k_e2e,
+                                   "h2d_bytes_per_step": sectors, "h2d_gbs": sectors * k_e2e / dta / 1e9,
+                                   "speedup_vs_dense": dt / dta,
+                                   "note": "cd_set_gather_max(-1): same outputs; bytes = one 32-byte sector per allowed logit of "
+                                           "an active row, read by the step kernel straight from the mapped host buffers "
+                                           "(gathered only when every state has <= V / 32 transitions, else the dense path)"}
             del host
         except Exception as ex:  # e.g. not enough pinned host memory on this box
             e2e = {"value": None, "unit": UNIT, "error": str(ex)[:200]}

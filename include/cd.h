@@ -368,6 +368,13 @@ CD_API cd_status cd_set_limit(cd_dfa_t* dfa, int32_t limit, int32_t* satisfied_i
  * copy) into a compact device staging buffer kept in the (handle, stream) scratch
  * area, so a loop moves (row-steps * ld_elems * sizeof) bytes instead of
  * (steps * B * ld_elems * sizeof); copying stops as soon as no row is active.
+ * With pinned, device-mapped buffers (cudaHostAlloc / cudaHostRegister under unified
+ * addressing) nothing is read back between steps: a kernel pulls the active rows over the
+ * link.  With the density-adaptive step switched on (cd_set_gather_max != 0) and such buffers,
+ * when EVERY state of the automaton may be gathered -- at most max_transitions transitions, or,
+ * for -1 (automatic), at most V / 32 -- nothing is staged at all: the step kernel reads the
+ * allowed logits of the active rows straight from the host buffers, one 32-byte sector each
+ * (configs[4]: 42 KB per row-step instead of 512 KB).  Same outputs either way.
  */
 CD_API cd_status cd_decode_loop_host(const cd_dfa_t* dfa, const void* const* step_logits_host,
                               cd_dtype dtype, int64_t ld_elems, int32_t B, int32_t max_steps,

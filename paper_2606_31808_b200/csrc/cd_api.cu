@@ -1513,7 +1513,22 @@ cd_status cd_decode_loop_host(const cd_dfa_t* d, const void* const* step_logits_
                 dev_view[(size_t)k] = static_cast<const unsigned char*>(at.devicePointer);
             }
         }
-        if (mapped) {
+        // Density-adaptive step over PCIe (cd_set_gather_max != 0): a masked log-softmax needs only
+        // the allowed logits, and over a 51 GB/s link that is where it pays most.  When EVERY state may be
+        // gathered, the step kernel reads the allowed logits of the active rows straight from the mapped host
+        // buffer (one 32-byte sector each) and nothing is staged: configs[4] moves 42 KB per row-step instead
+        // of 512 KB.  Threshold: the caller's, or automatic = V / 32 transitions (a gathered logit costs a
+        // 32-byte sector on the link against 2 or 4 bytes per token of a full row; half the break-even).
+        const long long host_gmax = cfg.gather_max > 0 ? cfg.gather_max : (cfg.gather_max < 0 ? d->dev.V / 32 : 0);
+        if (mapped && host_gmax > 0 && d->max_deg <= host_gmax) {
+            Settings gcfg = cfg;
+            gcfg.gather_max = (int)std::min<long long>(host_gmax, 0x3FFFFFFF);
+            for (int k = 0; k < max_steps; ++k) {
+                st = enqueue_loop_step(d, gcfg, s, dev_view[(size_t)k], dtype, ld_elems, B, k, max_steps, d_tokens, d_len, d_fs,
+                                       d_slp, d_done, stream, lim, 0);
+                if (st != CD_OK) return st;
+            }
+        } else if (mapped) {
             const unsigned long long row_bytes = (unsigned long long)ld_elems * (unsigned long long)sz;
             for (int k = 0; k < max_steps; ++k) {
                 const int cur = k & 1;
