@@ -1777,15 +1777,23 @@ cd_status launch_head(const cd_dfa* d, const Settings& cfg, Scratch* s, const vo
         const size_t smem = (size_t)H * 2;
         static thread_local int cfg_dev = -1;
         if (smem > 48 * 1024 && cfg_dev != d->device) {
-            CU(cudaFuncSetAttribute(cd::head_gather_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-            CU(cudaFuncSetAttribute(cd::head_gather_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            CU(cudaFuncSetAttribute(cd::head_gather_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            CU(cudaFuncSetAttribute(cd::head_gather_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            CU(cudaFuncSetAttribute(cd::head_gather_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+            CU(cudaFuncSetAttribute(cd::head_gather_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
             cfg_dev = d->device;
         }
         // one CTA per (row, piece), grid-stride: enough CTAs to fill the machine, never more than there are items
         long long gblocks = (long long)n * a.gp_max;
         if (gblocks > (long long)d->num_sms * 8) gblocks = (long long)d->num_sms * 8;
-        if (sample) cd::head_gather_kernel<true><<<(int)gblocks, cd::HG_WARPS * 32, smem, stream>>>(a);
-        else cd::head_gather_kernel<false><<<(int)gblocks, cd::HG_WARPS * 32, smem, stream>>>(a);
+        const bool two = a.gp_max > 1;  // long rows (cut into pieces): two W rows per warp in flight
+        if (sample) {
+            if (two) cd::head_gather_kernel<true, true><<<(int)gblocks, cd::HG_WARPS * 32, smem, stream>>>(a);
+            else cd::head_gather_kernel<true, false><<<(int)gblocks, cd::HG_WARPS * 32, smem, stream>>>(a);
+        } else {
+            if (two) cd::head_gather_kernel<false, true><<<(int)gblocks, cd::HG_WARPS * 32, smem, stream>>>(a);
+            else cd::head_gather_kernel<false, false><<<(int)gblocks, cd::HG_WARPS * 32, smem, stream>>>(a);
+        }
         CU(cudaGetLastError());
         ++launches;
         if (a.gp_max > 1) {  // rows cut into several pieces are merged and finished here

@@ -349,7 +349,9 @@ __device__ __forceinline__ float dot8(const uint4& w, const uint4& h, float acc)
 // (option sets, tries) is finished by its CTA; the piece results of a longer row go to gpartials and
 // head_gather_finish_kernel merges them -- a late step with a handful of rows of thousands of transitions then
 // spreads over the whole machine instead of keeping one SM per row busy.
-template <bool SAMPLE>
+// TWO: two W rows per warp at a time (16 loads per lane in flight, 112 registers: long rows cut into pieces); else one
+// row at a time (8 loads, ~70 registers, one more CTA per SM: option sets, whose rows have a handful of transitions).
+template <bool SAMPLE, bool TWO>
 __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadArgs a) {
     extern __shared__ __align__(16) unsigned char hg_smem[];
     uint4* hid = reinterpret_cast<uint4*>(hg_smem);
@@ -387,44 +389,50 @@ __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadAr
             SAMPLE ? rng_row_key(f.seed_lo, f.seed_hi, (uint32_t)(f.row_map ? __ldg(f.row_map + slot) : slot),
                                  (uint32_t)(f.rng_step_base + f.step))
                    : 0u;
-        // two W rows at a time, each read in passes of 8 x 512 contiguous bytes per warp with every load of the pass
-        // in flight (16 independent 16-byte loads per lane): a row is fetched in one or two bursts instead of being
-        // revisited chunk by chunk -- DRAM pages are opened once
-        for (int j = j0; j < j1; j += 2) {
-            const int jb = (j + 1 < j1) ? j + 1 : j;
-            const int ta = __ldg(f.dfa.tok + lo + j), tb = __ldg(f.dfa.tok + lo + jb);
-            const uint4* wa = reinterpret_cast<const uint4*>(a.W + (long long)ta * a.ldw);
-            const uint4* wb = reinterpret_cast<const uint4*>(a.W + (long long)tb * a.ldw);
-            float acc[2] = {0.0f, 0.0f};
+        // one or two W rows at a time, each read in passes of 8 x 512 contiguous bytes per warp with every load of the
+        // pass in flight: a row is fetched in one or two bursts instead of being revisited chunk by chunk -- DRAM pages
+        // are opened once
+        constexpr int NR = TWO ? 2 : 1;
+        for (int j = j0; j < j1; j += NR) {
+            int tk[NR];
+            const uint4* wr[NR];
+#pragma unroll
+            for (int q = 0; q < NR; ++q) {
+                const int jq = (j + q < j1) ? j + q : j;
+                tk[q] = __ldg(f.dfa.tok + lo + jq);
+                wr[q] = reinterpret_cast<const uint4*>(a.W + (long long)tk[q] * a.ldw);
+            }
+            float acc[NR];
+#pragma unroll
+            for (int q = 0; q < NR; ++q) acc[q] = 0.0f;
             for (int v0 = lane; v0 < nv; v0 += 256) {
-                uint4 xa[8], xb[8];
+                uint4 x[NR][8];
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
                     const int v = v0 + 32 * u;
-                    xa[u] = (v < nv) ? __ldg(wa + v) : make_uint4(0, 0, 0, 0);
-                    xb[u] = (v < nv) ? __ldg(wb + v) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+                    for (int q = 0; q < NR; ++q) x[q][u] = (v < nv) ? __ldg(wr[q] + v) : make_uint4(0, 0, 0, 0);
                 }
 #pragma unroll
                 for (int u = 0; u < 8; ++u) {
                     const int v = v0 + 32 * u;
                     if (v < nv) {
                         const uint4 h = hid[v];
-                        acc[0] = dot8(xa[u], h, acc[0]);
-                        acc[1] = dot8(xb[u], h, acc[1]);
+#pragma unroll
+                        for (int q = 0; q < NR; ++q) acc[q] = dot8(x[q][u], h, acc[q]);
                     }
                 }
             }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
-                acc[0] += __shfl_xor_sync(FULL, acc[0], o);
-                acc[1] += __shfl_xor_sync(FULL, acc[1], o);
+#pragma unroll
+                for (int q = 0; q < NR; ++q) acc[q] += __shfl_xor_sync(FULL, acc[q], o);
             }
 #pragma unroll
-            for (int q = 0; q < 2; ++q)
+            for (int q = 0; q < NR; ++q)
                 if (j + q < j1) {
-                    const int tq = q ? tb : ta;
                     if (SAMPLE)
-                        head_update_sample(m, s, kb, idx, yb, fmaxf(acc[q], -INFINITY), tq, j + q, f.inv_tau, row_key);
+                        head_update_sample(m, s, kb, idx, yb, fmaxf(acc[q], -INFINITY), tk[q], j + q, f.inv_tau, row_key);
                     else
                         online_update(m, s, idx, fmaxf(acc[q], -INFINITY), j + q);  // NaN -> -inf
                 }
