@@ -502,8 +502,20 @@ cd_status launch_flow_t(const cd::StepArgs& a, const cd::FlowArgs& F, int grid, 
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         configured_dev = dev;
     }
-    kern<<<grid, STEP_WARPS * 32, smem, stream>>>(a, F);
-    CU(cudaGetLastError());
+    // programmatic stream serialization (as launch_step_t): back-to-back loops of small batches (cd_decode_loop_async)
+    // do not pay the launch latency between two kernels; the kernel waits (griddepcontrol.wait) before it touches
+    // global memory, so whatever produced the logits has completed and flushed
+    cudaLaunchConfig_t lc{};
+    lc.gridDim = dim3((unsigned)grid);
+    lc.blockDim = dim3((unsigned)(STEP_WARPS * 32));
+    lc.dynamicSmemBytes = smem;
+    lc.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = use_pdl() ? 1 : 0;
+    lc.attrs = at;
+    lc.numAttrs = 1;
+    CU(cudaLaunchKernelEx(&lc, kern, a, F));
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return CD_OK;
 }

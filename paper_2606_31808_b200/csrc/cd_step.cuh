@@ -1359,6 +1359,10 @@ __global__ void __launch_bounds__(WARPS * 32, 1) flow_kernel(const StepArgs a, c
         fence_mbar_init();
     }
     __syncwarp();
+    // Programmatic dependent launch (see step_kernel): this grid may be scheduled while the previous kernel of the
+    // stream drains; nothing here reads or writes global memory before that kernel has completed and flushed.
+    pdl_launch_dependents();
+    pdl_wait();
     const unsigned gen0 = (unsigned)__ldcg(a.ctrs + 3);
     const int par = __ldcg(F.q + FQ_LAUNCHES) & 1;
     StepView sv{};
