@@ -99,8 +99,11 @@ constexpr int MERGE_SPIN_LIMIT = 1 << 24;  // polls (>= 32 ns apart) after which
 constexpr int FLOW_ENTRY_WORDS = 8;        // 64-byte queue entries (5 words used)
 // flow_kernel's counters, one 128-byte line each (the stop word is polled by every idle warp: kept away from the
 // lines the unit draws and the publications hit with atomics)
-constexpr int FQ_DRAWN = 0, FQ_PUBLISHED = 32, FQ_FINISHED = 64, FQ_STOP = 96, FQ_ERRORS = 128, FQ_LAUNCHES = 129;
-constexpr int FQ_INTS = 160;
+constexpr int FQ_DRAWN = 0, FQ_PUBLISHED = 32, FQ_FINISHED = 64, FQ_ERRORS = 96, FQ_LAUNCHES = 97, FQ_STOP = 128;
+// the stop word exists in FQ_STOP_COPIES lines (warp w reads copy w % FQ_STOP_COPIES): every idle warp can look at it
+// on every poll without 1,700 warps reading one line
+constexpr int FQ_STOP_COPIES = 64;
+constexpr int FQ_INTS = FQ_STOP + 32 * FQ_STOP_COPIES;
 
 // tiles per chunk / chunks per row of a row of `tiles_per_row` tiles
 __host__ __device__ inline int chunk_tiles(int tiles_per_row) {
@@ -361,8 +364,11 @@ __device__ __forceinline__ void flow_row_leaves(const StepArgs& a, const StepVie
         a.hist_sum_logprob[rid] = sum;
         a.hist_done[rid] = done;
         atomicMax(sv.trace_n + LOOP_TRACE_STEPS, steps);  // steps run = the most any row ran
-        if (atomicAdd(F.q + FQ_FINISHED, 1) == F.B - 1) atomicExch(F.q + FQ_STOP, (int)sv.gen);
     }
+    int last = 0;
+    if (lane == 0) last = (atomicAdd(F.q + FQ_FINISHED, 1) == F.B - 1) ? 1 : 0;
+    if (__shfl_sync(FULL, last, 0))  // the loop is over: every copy of the stop word
+        for (int i = lane; i < FQ_STOP_COPIES; i += 32) atomicExch(F.q + FQ_STOP + 32 * i, (int)sv.gen);
 }
 
 // Row finished: (m, s, idx) is the merged result of all its chunks.  Warp-uniform.
@@ -547,11 +553,10 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
     static_assert(WPL >= 1 && TILE_TOK % 1024 == 0, "tile must hold a multiple of 32 mask words");
 
     // ---------------- issue side (warp-uniform state)
-    // MODE_STEP / MODE_LOOP: the first unit of a warp is its global warp id (no atomic on the start-up
-    // chain); later units come from the work counter, which therefore starts at 0 = unit `total_warps`.
-    // MODE_FLOW: every unit is drawn from the counter.
+    // The first unit of a warp is its global warp id (no atomic on the start-up chain: 1,776 warps drawing from one
+    // address at once); later units come from the work counter, which therefore starts at 0 = unit `total_warps`.
     const int total_warps = gridDim.x * WARPS;
-    const int draw_base = (MODE == MODE_FLOW) ? 0 : total_warps;
+    const int draw_base = total_warps;
     int next_u_l0 = blockIdx.x * WARPS + warp;  // prefetched unit id, valid in lane 0
     const int V = a.dfa.V;
     const int tiles_per_row = (V + TILE_TOK - 1) / TILE_TOK;
@@ -562,7 +567,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
     bool all_done = false;      // MODE_FLOW: every row has left the loop
     bool poll_pending = false;  // MODE_FLOW: poll_w / poll_stop hold the loads issued for the unit in next_u_l0
     unsigned long long poll_w = 0;
-    int poll_stop = 0, poll_n = 0;
+    int poll_stop = 0;
     long long units0 = 0;  // MODE_FLOW: implicit units (the first step of every row)
     if (MODE != MODE_FLOW) {
         unit_ctx_split<WARPS, GATHER>(cur, a, sv.n, tiles_per_row, tpu_max);
@@ -573,7 +578,6 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
         unit_ctx_split<WARPS, GATHER>(cur, a, F->B, tiles_per_row, tpu_max);
         units0 = (long long)F->B * cur.P;
         cur.work = F->q + FQ_DRAWN;
-        if (lane == 0) next_u_l0 = atomicAdd(cur.work, 1);
     }
     const bool ragged_row = (V % TILE_TOK) != 0;
     const uint64_t pol_stream = l2_policy_evict_first();
@@ -615,8 +619,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                         if (poll_pending && (unsigned)__shfl_sync(FULL, poll_stop, 5) == sv.gen) all_done = true;
                         poll_w = 0;
                         if (lane < 5) poll_w = ld_relaxed_gpu_u64(F->task + (size_t)(e & F->cap_mask) * FLOW_ENTRY_WORDS + lane);
-                        // (the stop word only every 4th look: all idle warps read that one line)
-                        if (lane == 5 && (poll_n++ & 3) == 0) poll_stop = ld_relaxed_gpu_s32(F->q + FQ_STOP);
+                        if (lane == 5) poll_stop = ld_relaxed_gpu_s32(F->q + FQ_STOP + 32 * ((blockIdx.x * WARPS + warp) % FQ_STOP_COPIES));
                         poll_pending = true;
                         return false;
                     }
@@ -633,7 +636,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 // (drawing the next unit only when the last tile of this one is issued -- so that the warps that have
                 // waited longest, not the ones that just took work, hold the next ids -- was tried: the draw and the
                 // poll then sit in front of every unit's first copy; c4 lost 2 %, the tail gained nothing)
-                if (lane == 0) next_u_l0 = atomicAdd(cur.work, 1);
+                if (lane == 0) next_u_l0 = draw_base + atomicAdd(cur.work, 1);
                 if (lane == 0) {
                     CD_DBG_MIN(F, rl * a.max_steps + iss_step, 1);
                     CD_DBG_MAX(F, rl * a.max_steps + iss_step, 2);
@@ -869,7 +872,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
             [[maybe_unused]] const unsigned ck2 = CD_CLOCK();
             int q0 = 0, q1 = 0;
             if (MODE == MODE_FLOW && lane == 0) {  // how busy the machine is, for the split of the row's next step
-                q0 = ld_relaxed_gpu_s32(F->q + FQ_DRAWN);
+                q0 = ld_relaxed_gpu_s32(F->q + FQ_DRAWN) + (int)(gridDim.x * WARPS);  // (+ the static first units)
                 q1 = ld_relaxed_gpu_s32(F->q + FQ_PUBLISHED);
             }
             __syncwarp();
