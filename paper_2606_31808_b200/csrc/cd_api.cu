@@ -13,6 +13,7 @@
 #include <mutex>
 #include <new>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/cd.h"
@@ -1640,6 +1641,24 @@ cd_status make_tmap_bf16(CUtensorMap* out, const void* base, long long rows, lon
     return CD_OK;
 }
 
+// Launch with programmatic stream serialization (as launch_step_t): the kernels of an LM-head step are short and
+// many (prepare, gather, gather finish, pack, two contractions of which one returns at once, finish, loop tail);
+// each begins with griddepcontrol.wait, so the next one's launch overlaps the running one instead of following it.
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t stream, Args&&... args) {
+    cudaLaunchConfig_t lc{};
+    lc.gridDim = dim3(grid);
+    lc.blockDim = dim3(block);
+    lc.dynamicSmemBytes = smem;
+    lc.stream = stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = use_pdl() ? 1 : 0;
+    lc.attrs = at;
+    lc.numAttrs = 1;
+    return cudaLaunchKernelEx(&lc, kern, std::forward<Args>(args)...);
+}
+
 cd_status get_head_scratch(Scratch* s, int rows, int H, cudaStream_t stream) {
     if (s->head_rows >= rows && s->head_H == H) return CD_OK;  // the A tensor map is built for exactly H columns
     if (s->head_rows > 0) CU(cudaStreamSynchronize(stream));
@@ -1780,7 +1799,7 @@ cd_status launch_head(const cd_dfa* d, const Settings& cfg, Scratch* s, const vo
     // CTA pairs (thread-block clusters of 2) for calls with more than one row tile: needs an even number of SMs in
     // the grid and a batch that can have > 128 dense rows at all
     a.pairs = (head_pairs_enabled() && (d->num_sms % 2) == 0 && n_upper >= cd::HD2_MIN_ROWS) ? 1 : 0;
-    cd::head_prepare_kernel<<<1, 1024, 0, stream>>>(a);
+    CU(launch_pdl(cd::head_prepare_kernel, (unsigned)(1), (unsigned)(1024), (size_t)(0), stream, a));
     CU(cudaGetLastError());
     const bool any_gather = (a.gather_max > 0 && d->min_deg_nonacc <= a.gather_max) || (a.gather_auto && d->max_deg > a.gather_max);
     const bool any_dense = d->max_deg > a.gather_max;
@@ -1800,25 +1819,25 @@ cd_status launch_head(const cd_dfa* d, const Settings& cfg, Scratch* s, const vo
         if (gblocks > (long long)d->num_sms * 8) gblocks = (long long)d->num_sms * 8;
         const bool two = a.gp_max > 1;  // long rows (cut into pieces): two W rows per warp in flight
         if (sample) {
-            if (two) cd::head_gather_kernel<true, true><<<(int)gblocks, cd::HG_WARPS * 32, smem, stream>>>(a);
-            else cd::head_gather_kernel<true, false><<<(int)gblocks, cd::HG_WARPS * 32, smem, stream>>>(a);
+            if (two) CU(launch_pdl(cd::head_gather_kernel<true, true>, (unsigned)((int)gblocks), (unsigned)(cd::HG_WARPS * 32), (size_t)(smem), stream, a));
+            else CU(launch_pdl(cd::head_gather_kernel<true, false>, (unsigned)((int)gblocks), (unsigned)(cd::HG_WARPS * 32), (size_t)(smem), stream, a));
         } else {
-            if (two) cd::head_gather_kernel<false, true><<<(int)gblocks, cd::HG_WARPS * 32, smem, stream>>>(a);
-            else cd::head_gather_kernel<false, false><<<(int)gblocks, cd::HG_WARPS * 32, smem, stream>>>(a);
+            if (two) CU(launch_pdl(cd::head_gather_kernel<false, true>, (unsigned)((int)gblocks), (unsigned)(cd::HG_WARPS * 32), (size_t)(smem), stream, a));
+            else CU(launch_pdl(cd::head_gather_kernel<false, false>, (unsigned)((int)gblocks), (unsigned)(cd::HG_WARPS * 32), (size_t)(smem), stream, a));
         }
         CU(cudaGetLastError());
         ++launches;
         if (a.gp_max > 1) {  // rows cut into several pieces are merged and finished here
             const int fb = (n + 7) / 8;
-            if (sample) cd::head_gather_finish_kernel<true><<<fb, 256, 0, stream>>>(a);
-            else cd::head_gather_finish_kernel<false><<<fb, 256, 0, stream>>>(a);
+            if (sample) CU(launch_pdl(cd::head_gather_finish_kernel<true>, (unsigned)(fb), (unsigned)(256), (size_t)(0), stream, a));
+            else CU(launch_pdl(cd::head_gather_finish_kernel<false>, (unsigned)(fb), (unsigned)(256), (size_t)(0), stream, a));
             CU(cudaGetLastError());
             ++launches;
         }
     }
     if (any_dense) {
         const int rows_per_block = 8;
-        cd::head_pack_kernel<<<(n + rows_per_block - 1) / rows_per_block, rows_per_block * 32, 0, stream>>>(a);
+        CU(launch_pdl(cd::head_pack_kernel, (unsigned)((n + rows_per_block - 1) / rows_per_block), (unsigned)(rows_per_block * 32), (size_t)(0), stream, a));
         CU(cudaGetLastError());
         static thread_local int cfg_dev2 = -1;
         if (cfg_dev2 != d->device) {
@@ -1836,25 +1855,25 @@ cd_status launch_head(const cd_dfa* d, const Settings& cfg, Scratch* s, const vo
             }
             // (the kernel carries __cluster_dims__(2, 1, 1); each of the two dense kernels returns at once when the
             // number of dense rows, known on the device only, puts the call in the other one's range)
-            if (sample) cd::head_dense2_kernel<true><<<d->num_sms, cd::HD_THREADS, cd::HD2_SMEM_BYTES, stream>>>(s->h_tmA, tmWh, a);
-            else cd::head_dense2_kernel<false><<<d->num_sms, cd::HD_THREADS, cd::HD2_SMEM_BYTES, stream>>>(s->h_tmA, tmWh, a);
+            if (sample) CU(launch_pdl(cd::head_dense2_kernel<true>, (unsigned)(d->num_sms), (unsigned)(cd::HD_THREADS), (size_t)(cd::HD2_SMEM_BYTES), stream, s->h_tmA, tmWh, a));
+            else CU(launch_pdl(cd::head_dense2_kernel<false>, (unsigned)(d->num_sms), (unsigned)(cd::HD_THREADS), (size_t)(cd::HD2_SMEM_BYTES), stream, s->h_tmA, tmWh, a));
             CU(cudaGetLastError());
             ++launches;
         }
         if (sample) {
-            cd::head_dense_kernel<true><<<d->num_sms, cd::HD_THREADS, cd::HD_SMEM_BYTES, stream>>>(s->h_tmA, tmW, a);
+            CU(launch_pdl(cd::head_dense_kernel<true>, (unsigned)(d->num_sms), (unsigned)(cd::HD_THREADS), (size_t)(cd::HD_SMEM_BYTES), stream, s->h_tmA, tmW, a));
             CU(cudaGetLastError());
-            cd::head_finish_kernel<true><<<fin_blocks, rows_per_block * 32, 0, stream>>>(a);
+            CU(launch_pdl(cd::head_finish_kernel<true>, (unsigned)(fin_blocks), (unsigned)(rows_per_block * 32), (size_t)(0), stream, a));
         } else {
-            cd::head_dense_kernel<false><<<d->num_sms, cd::HD_THREADS, cd::HD_SMEM_BYTES, stream>>>(s->h_tmA, tmW, a);
+            CU(launch_pdl(cd::head_dense_kernel<false>, (unsigned)(d->num_sms), (unsigned)(cd::HD_THREADS), (size_t)(cd::HD_SMEM_BYTES), stream, s->h_tmA, tmW, a));
             CU(cudaGetLastError());
-            cd::head_finish_kernel<false><<<fin_blocks, rows_per_block * 32, 0, stream>>>(a);
+            CU(launch_pdl(cd::head_finish_kernel<false>, (unsigned)(fin_blocks), (unsigned)(rows_per_block * 32), (size_t)(0), stream, a));
         }
         CU(cudaGetLastError());
         launches += 3;
     }
     if (x) {
-        cd::head_loop_tail_kernel<<<1, 1024, 0, stream>>>(a);
+        CU(launch_pdl(cd::head_loop_tail_kernel, (unsigned)(1), (unsigned)(1024), (size_t)(0), stream, a));
         CU(cudaGetLastError());
         ++launches;
     }

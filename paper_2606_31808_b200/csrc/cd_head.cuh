@@ -266,6 +266,8 @@ __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.
 // here; the others go to the gather list (state has <= gather_max
 // transitions) or to the dense list, both in slot order.
 __global__ void __launch_bounds__(1024, 1) head_prepare_kernel(const HeadArgs a) {
+    pdl_launch_dependents();  // launched with programmatic stream serialization: the next kernel may be scheduled,
+    pdl_wait();               // and nothing of this one touches global memory before its predecessor has completed
     const StepArgs& f = a.fin;
     const int n = f.n_dev ? __ldcg(f.n_dev) : f.n;
     __shared__ unsigned long long s_big;  // transitions of the rows above gather_max, all together
@@ -318,6 +320,8 @@ __global__ void __launch_bounds__(1024, 1) head_prepare_kernel(const HeadArgs a)
 // ---------------------------------------------------------------- pack: dense rows -> A
 // One warp per dense row, 16-byte copies (H % 8 == 0, rows 16-byte aligned).
 __global__ void head_pack_kernel(const HeadArgs a) {
+    pdl_launch_dependents();  // launched with programmatic stream serialization: the next kernel may be scheduled,
+    pdl_wait();               // and nothing of this one touches global memory before its predecessor has completed
     const int n_dense = __ldcg(a.hctr + 0);
     const int lane = threadIdx.x & 31;
     const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -353,6 +357,8 @@ __device__ __forceinline__ float dot8(const uint4& w, const uint4& h, float acc)
 // row at a time (8 loads, ~70 registers, one more CTA per SM: option sets, whose rows have a handful of transitions).
 template <bool SAMPLE, bool TWO>
 __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadArgs a) {
+    pdl_launch_dependents();  // launched with programmatic stream serialization: the next kernel may be scheduled,
+    pdl_wait();               // and nothing of this one touches global memory before its predecessor has completed
     extern __shared__ __align__(16) unsigned char hg_smem[];
     uint4* hid = reinterpret_cast<uint4*>(hg_smem);
     __shared__ float s_m[HG_WARPS], s_s[HG_WARPS], s_k[HG_WARPS], s_y[HG_WARPS];
@@ -466,6 +472,8 @@ __global__ void __launch_bounds__(HG_WARPS * 32) head_gather_kernel(const HeadAr
 // the pieces l, l + 32, ascending, then the butterfly), then the CSR transition and the accept test.
 template <bool SAMPLE>
 __global__ void head_gather_finish_kernel(const HeadArgs a) {
+    pdl_launch_dependents();  // launched with programmatic stream serialization: the next kernel may be scheduled,
+    pdl_wait();               // and nothing of this one touches global memory before its predecessor has completed
     const StepArgs& f = a.fin;
     const int n_gather = __ldcg(a.hctr + 1);
     const int lane = threadIdx.x & 31;
@@ -507,6 +515,8 @@ __global__ void head_gather_finish_kernel(const HeadArgs a) {
 template <bool SAMPLE>
 __global__ void __launch_bounds__(HD_THREADS, 1)
 head_dense_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmW, const HeadArgs a) {
+    pdl_launch_dependents();  // launched with programmatic stream serialization: the next kernel may be scheduled,
+    pdl_wait();               // and nothing of this one touches global memory before its predecessor has completed
     extern __shared__ __align__(1024) unsigned char hd_smem[];
     __shared__ __align__(8) unsigned long long bar_full[HD_STAGES], bar_empty[HD_STAGES], bar_tfull[2], bar_tempty[2];
     __shared__ uint32_t s_tmem;
@@ -736,6 +746,8 @@ __device__ __forceinline__ void tc_mma_bf16_pair(uint32_t d_tmem, uint64_t a_des
 template <bool SAMPLE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(HD_THREADS, 1)
 head_dense2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmWh, const HeadArgs a) {
+    pdl_launch_dependents();  // launched with programmatic stream serialization: the next kernel may be scheduled,
+    pdl_wait();               // and nothing of this one touches global memory before its predecessor has completed
     extern __shared__ __align__(1024) unsigned char hd_smem[];
     __shared__ __align__(8) unsigned long long bar_full[HD2_STAGES], bar_empty[HD2_STAGES], bar_tfull[2], bar_tempty[2];
     __shared__ uint32_t s_tmem;
@@ -904,6 +916,8 @@ head_dense2_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constan
 // ... ascending, then the butterfly), then the CSR transition and the accept test.
 template <bool SAMPLE>
 __global__ void head_finish_kernel(const HeadArgs a) {
+    pdl_launch_dependents();  // launched with programmatic stream serialization: the next kernel may be scheduled,
+    pdl_wait();               // and nothing of this one touches global memory before its predecessor has completed
     const StepArgs& f = a.fin;
     const int n_dense = __ldcg(a.hctr + 0);
     const int NU = head_row_partials(n_dense, f.dfa.V, a.pairs);
@@ -938,6 +952,8 @@ __global__ void head_finish_kernel(const HeadArgs a) {
 // ---------------------------------------------------------------- decode loop: compaction
 // Last kernel of a loop step: stable early-exit compaction of the active list.
 __global__ void __launch_bounds__(1024, 1) head_loop_tail_kernel(const HeadArgs a) {
+    pdl_launch_dependents();  // launched with programmatic stream serialization: the next kernel may be scheduled,
+    pdl_wait();               // and nothing of this one touches global memory before its predecessor has completed
     const StepArgs& f = a.fin;
     const int n = f.n_dev ? __ldcg(f.n_dev) : f.n;
     block_compact(f.done_out, f.row_map, f.state, n, f.cmp_row_ids_out, f.cmp_state_out, f.cmp_n_out);
