@@ -113,7 +113,7 @@ struct StepBufs {  // sized by rows; replaced as a whole when the area grows
     // persistent loop
     uint32_t* alive[3] = {nullptr, nullptr, nullptr};  // [ceil(rows / 32)] each
     int* state2[2] = {nullptr, nullptr};                // [rows] each
-    int* bar = nullptr;                                 // [4]
+    int* bar = nullptr;                                 // [LB_INTS]
     unsigned long long* trace_t = nullptr;              // [LOOP_TRACE_STEPS + 1]
     int* trace_n = nullptr;                             // [LOOP_TRACE_STEPS + 1]
     unsigned long long* phase = nullptr;                // tuning builds: [LOOP_TRACE_STEPS][8]
@@ -309,7 +309,7 @@ cd_status alloc_step_bufs(const cd_dfa* d, int rows, StepBufs* out) {
     A(dev_alloc(&n.token, (size_t)rows));
     A(dev_alloc(&n.logprob, (size_t)rows));
     A(dev_alloc(&n.done, (size_t)rows));
-    A(dev_alloc(&n.bar, 4));
+    A(dev_alloc(&n.bar, cd::LB_INTS));
     A(dev_alloc(&n.trace_t, (size_t)cd::LOOP_TRACE_STEPS + 1));
     A(dev_alloc(&n.trace_n, (size_t)cd::LOOP_TRACE_STEPS + 1));
     A(dev_alloc(&n.f_q, cd::FQ_INTS));
@@ -1112,7 +1112,7 @@ cd_status finish_loop(Scratch* s, cudaStream_t stream, bool persistent) {
     int h[4] = {0, 0, 0, 0};
     int hb[4] = {0, 0, 0, 0};
     CU(cudaMemcpyAsync(h, s->b.ctrs, sizeof h, cudaMemcpyDeviceToHost, stream));
-    if (persistent) CU(cudaMemcpyAsync(hb, s->b.bar, sizeof hb, cudaMemcpyDeviceToHost, stream));
+    if (persistent) CU(cudaMemcpyAsync(hb + 2, s->b.bar + cd::LB_ABORT, sizeof(int), cudaMemcpyDeviceToHost, stream));
     CU(cudaStreamSynchronize(stream));
     if (hb[2] != 0)
         return fail(CD_ERR_INTERNAL, "the persistent loop kernel timed out at a grid barrier (device shared with a kernel that never ends?)");

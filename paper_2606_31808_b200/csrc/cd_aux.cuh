@@ -241,7 +241,7 @@ __global__ void loop_init_kernel(const LoopInitArgs a) {
             a.alive[2][w] = 0u;
         }
         for (long long k = tid; k < a.max_steps; k += nth) a.work[k] = 0;
-        if (tid < 3) a.bar[tid] = 0;
+        if (tid < 3) a.bar[tid * 32] = 0;  // arrivals, go word, abort flag (cd_step.cuh LB_*)
     }
     if (tid == 0) {
         if (a.n_active) *a.n_active = none ? 0 : B;

@@ -96,6 +96,9 @@ constexpr int LOOP_TRACE_STEPS = 256;    // per-step (timestamp, active rows) re
 constexpr unsigned long long LOOP_SPIN_TIMEOUT_NS = 4000000000ull;  // a barrier that waits longer aborts the loop
 constexpr int FLOW_IDLE_LIMIT = 1 << 23;   // idle polls (>= 128 ns apart: > 1 s) after which a worker of flow_kernel gives up
 constexpr int MERGE_SPIN_LIMIT = 1 << 24;  // polls (>= 32 ns apart) after which a merging warp gives up
+// loop_kernel's barrier words, one 128-byte line each (the go word and the abort flag are polled by every CTA while
+// the arrivals are counted with atomics)
+constexpr int LB_ARRIVE = 0, LB_GO = 32, LB_ABORT = 64, LB_INTS = 96;
 constexpr int FLOW_ENTRY_WORDS = 8;        // 64-byte queue entries (5 words used)
 // flow_kernel's counters, one 128-byte line each (the stop word is polled by every idle warp: kept away from the
 // lines the unit draws and the publications hit with atomics)
@@ -201,7 +204,7 @@ struct LoopArgs {
     uint32_t* alive[3];  // [nwords] active-row bitmaps in rotation: step k reads k % 3, builds (k + 1) % 3, clears (k + 2) % 3
     int* state2[2];      // [B] states by original row id: step k reads k & 1, writes (k + 1) & 1
     int* work;           // [max_steps] per-step work counters (zeroed by loop_init)
-    int* bar;            // [0] arrivals, [1] go word: (steps completed) | stop << 30, [2] abort flag
+    int* bar;            // [LB_INTS]: arrivals, go word: (steps completed) | stop << 30, abort flag -- one 128-byte line each
     unsigned long long* trace_t;  // [LOOP_TRACE_STEPS + 1] globaltimer at the start of every step, then at exit
     int* trace_n;                 // [LOOP_TRACE_STEPS] active rows of every step, [LOOP_TRACE_STEPS] = steps run
     unsigned long long* phase;    // tuning builds (-DCD_TUNING): [LOOP_TRACE_STEPS][8] phase timestamps of every step
@@ -1227,14 +1230,14 @@ __device__ __forceinline__ int loop_barrier(const LoopArgs& L, int k1, const int
         const int old = atom_add_acq_rel_gpu(L.bar + 0, 1);
         if (old == k1 * (int)gridDim.x - 1) {
             const int stop = (sat_ctr && __ldcg(sat_ctr) >= limit) ? 1 : 0;
-            st_release_gpu_s32(L.bar + 1, k1 | (stop << 30));
+            st_release_gpu_s32(L.bar + LB_GO, k1 | (stop << 30));
         }
         int v;
         const unsigned long long t0 = global_timer_ns();
-        while (((v = ld_acquire_gpu_s32(L.bar + 1)) & 0x3FFFFFFF) < k1) {
-            if (ld_acquire_gpu_s32(L.bar + 2) != 0) { v = k1 | (1 << 30); break; }
+        while (((v = ld_acquire_gpu_s32(L.bar + LB_GO)) & 0x3FFFFFFF) < k1) {
+            if (ld_acquire_gpu_s32(L.bar + LB_ABORT) != 0) { v = k1 | (1 << 30); break; }
             if (global_timer_ns() - t0 > LOOP_SPIN_TIMEOUT_NS) {  // never on a healthy device: fail, do not hang
-                atomicExch(L.bar + 2, 1);
+                atomicExch(L.bar + LB_ABORT, 1);
                 v = k1 | (1 << 30);
                 break;
             }
