@@ -281,7 +281,16 @@ int step_grid(const cd_dfa* d, long long n_upper, int dtype) {
 }
 
 // chunk results of the step kernels: MAX_CHUNKS slots per row (cd_step.cuh: canonical chunks)
-long long step_units_cap(const cd_dfa*, long long n) { return n * cd::MAX_CHUNKS + 64; }
+// = the most chunks (fp32 rows have the most tiles) or gathered pieces (any state may be gathered: cd_set_gather_max)
+// a row of this automaton can have; a function of the automaton alone, so every launch on the handle agrees on it
+int partial_stride(const cd_dfa* d) {
+    const int chunks = cd::row_chunks(tiles_per_row(d->dev.V, CD_F32));
+    // (gather_pieces is not monotone beyond MAX_CHUNKS * GATHER_CHUNK transitions: bound it)
+    const long long p256 = (d->max_deg + cd::GATHER_CHUNK - 1) / cd::GATHER_CHUNK;
+    const int pieces = (int)std::max<long long>(1, std::min<long long>(p256, cd::MAX_CHUNKS));
+    return std::max(chunks, pieces);
+}
+long long step_units_cap(const cd_dfa* d, long long n) { return n * partial_stride(d) + 64; }
 
 template <typename T>
 cudaError_t dev_alloc(T** p, size_t count) {
@@ -571,6 +580,7 @@ cd::StepArgs make_step_args(const cd_dfa* d, const Settings& cfg, Scratch* s, cd
     a.ld_bytes = ld * (dtype == CD_BF16 ? 2 : 4);
     a.state_new = s->b.state_new;
     a.partials = s->b.partials;
+    a.pstride = partial_stride(d);
     a.tickets = s->b.tickets;
     a.ctrs = s->b.ctrs;
     a.gather_max = gather_max_for(d, cfg, dtype);

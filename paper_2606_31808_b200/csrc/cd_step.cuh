@@ -160,7 +160,8 @@ struct StepArgs {
     float* lse_out;
     uint8_t* done_out;
     // scratch (per handle+stream)
-    PartialSlot* partials;  // [rows][MAX_CHUNKS]
+    PartialSlot* partials;  // [rows][pstride]
+    int pstride;            // chunk-result slots per row: the most chunks / gathered pieces a row of this automaton can have
     int* tickets;           // [2 * rows] chunks arrived per slot (flow_kernel: per row and step parity), zero between uses
     int* ctrs;              // [0] work counter, [1] finished CTAs, [2] error count, [3] generation
     int gather_max;         // states with <= gather_max transitions are gathered (GATHER kernels; 0 = never)
@@ -844,7 +845,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
         auto orig_row = [&]() -> uint32_t {
             return (MODE != MODE_STEP) ? (uint32_t)mt.lrow : (uint32_t)(a.row_map ? __ldg(a.row_map + mt.slot) : mt.slot);
         };
-        PartialSlot* const pbase = a.partials + (long long)mt.slot * MAX_CHUNKS;
+        PartialSlot* const pbase = a.partials + (long long)mt.slot * a.pstride;
         // lane 1 publishes the result of chunk c (lane 0 is busy issuing copies): self-validating words
         auto publish_chunk = [&](int c, float rm, float rs, int ri, float rk) {
             if (lane == 1) {
