@@ -897,17 +897,17 @@ cd_status get_loop_scratch(Scratch* s, int max_steps, cudaStream_t stream);
 // flow_kernel: whether the loop fits the kernel's index ranges
 constexpr long long FLOW_RING_MAX = (512ll << 20) / (8 * cd::FLOW_ENTRY_WORDS);  // at most 512 MiB of queue
 
-// entries of the queue ring: a power of two >= 2 * B * MAX_CHUNKS (see cd::FlowArgs: B * MAX_CHUNKS suffices)
-long long flow_ring_entries(int B) {
+// entries of the queue ring: a power of two >= 2 * B * (chunks per row): a row step is cut into at most that many units
+// (see cd::FlowArgs: B * chunks suffices)
+long long flow_ring_entries(const cd_dfa* d, int B, int dtype) {
+    const long long tc = cd::row_chunks(tiles_per_row(d->dev.V, dtype));
     long long cap = 1024;
-    while (cap < 2ll * B * cd::MAX_CHUNKS) cap <<= 1;
+    while (cap < 2ll * B * tc) cap <<= 1;
     return cap;
 }
 
 bool flow_loop_possible(const cd_dfa* d, int B, int max_steps, int dtype) {
-    (void)d;
-    (void)dtype;
-    if (flow_ring_entries(B) > FLOW_RING_MAX) return false;
+    if (flow_ring_entries(d, B, dtype) > FLOW_RING_MAX) return false;
     // the unit counter and the entry counter are 32 bits wide: every row step cut into MAX_CHUNKS units at worst
     return (long long)B * max_steps * cd::MAX_CHUNKS + (long long)d->num_sms * STEP_WARPS * 4 < 0x7FFFFFFFLL;
 }
@@ -951,7 +951,7 @@ cd_status enqueue_flow_loop(const cd_dfa* d, const Settings& cfg, Scratch* s, co
                             cd_dtype dtype, long long ld, int B, int max_steps, int* tokens_out, int* len_out,
                             int* final_state_out, float* sum_logprob_out, uint8_t* done_out, cudaStream_t stream) {
     RangeGuard range("cd decode loop (persistent kernel, row tasks)");
-    cd_status st = get_flow_scratch(s, flow_ring_entries(B), stream);
+    cd_status st = get_flow_scratch(s, flow_ring_entries(d, B, dtype), stream);
     if (st != CD_OK) return st;
     LoopExtras x;
     x.tokens = tokens_out;
