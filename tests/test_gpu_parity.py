@@ -756,6 +756,26 @@ def test_host_buffer_loop_matches_device_loop(cd, oracle):
     dfa.close()
 
 
+def test_host_buffer_loop_gathers_over_the_link_in_automatic_mode(cd, oracle):
+    """cd_decode_loop_host with cd_set_gather_max(-1) and pinned, mapped buffers: every state of this automaton has fewer
+    than V / 32 transitions, so the step kernel reads the allowed logits straight from host memory (nothing is staged);
+    with pageable buffers the same call stages the active rows.  Both against the oracle."""
+    cfg = wl.scaled(wl.CONFIGS["c3"], V=30000, B=300, S=64, max_steps=8)
+    aut = wl.build_automaton(cfg)
+    assert int(torch.diff(torch.as_tensor(aut.row_ptr)).max()) <= cfg.V // 32
+    logits = wl.build_step_logits(cfg, aut, device="cuda:0")
+    want = oracle.decode_loop(aut, [x.cpu() for x in logits])
+    dfa = cd.compile_dfa(aut.V, aut.S, aut.start, aut.row_ptr, aut.tok, aut.next, aut.accepting, device="cuda:0")
+    dfa.set_gather_max(-1)
+    for host in ([x.cpu().pin_memory() for x in logits], [x.cpu() for x in logits]):
+        got = cd.decode_loop_host(dfa, host, max_steps=cfg.max_steps)
+        for k in ("tokens", "len", "final_state", "done"):
+            assert np.array_equal(got[k].numpy(), want[k]), k
+        ok, worst = close(got["sum_logprob"].numpy(), want["sum_logprob"], tol=TOL * cfg.max_steps)
+        assert ok, worst
+    dfa.close()
+
+
 def test_trie_sugar_equals_explicit_csr(cd, oracle):
     cfg = wl.scaled(wl.CONFIGS["c2"], V=20000, B=200, K=30)
     aut = wl.build_automaton(cfg)
