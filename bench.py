@@ -81,7 +81,7 @@ def parse_args():
                          "sharded B/N rows per rank (SURVEY 8(e): contiguous row ranges, no collective)")
     ap.add_argument("--no-per-config", action="store_true", help="skip the c1-c3 block (per_config)")
     ap.add_argument("--loop-mode", default="auto", choices=["auto", "barrier", "per_step"],
-                    help="auto: cd_decode_loop as ONE persistent kernel, row groups advancing independently (default); "
+                    help="auto: cd_decode_loop as ONE persistent kernel, every row advancing on its own (default); "
                          "barrier: the lock-step persistent kernel; per_step: one launch per decoding step")
     return ap.parse_args()
 
@@ -447,7 +447,7 @@ def measure_loop(cd, cfg, aut, dfa, batches, device, steps, warmup, peak, verbos
         kern_us = sum(us)
         k0 = max(range(len(us)), key=lambda k: last["bytes"][k])
         res.update({
-            "kernel": "cd::flow_kernel (one launch per loop; row groups advance independently, no grid barrier)",
+            "kernel": "cd::flow_kernel (one launch per loop; every row advances on its own, no grid barrier)",
             "kernel_us_per_loop": kern_us,
             "kernel_gbs": sum(last["bytes"]) / (kern_us * 1e-6) / 1e9,
             "kernel_frac_of_measured_peak": sum(last["bytes"]) / (kern_us * 1e-6) / 1e9 / peak,
@@ -457,8 +457,8 @@ def measure_loop(cd, cfg, aut, dfa, batches, device, steps, warmup, peak, verbos
             "us_per_step": [round(u, 2) for u in us],
             "gbs_per_step": [round(g, 0) for g in gbs],
             "fixed_us_per_step_avg": sum(fixed) / len(fixed),
-            "fixed_cost_note": f"step time minus its bytes at the kernel's pure-read rate ({READ_RATE_GBS:.0f} GB/s); with row "
-                               "groups a step lasts from the publication of its last group to that of the next step's, so "
+            "fixed_cost_note": f"step time minus its bytes at the kernel's pure-read rate ({READ_RATE_GBS:.0f} GB/s); rows advance on "
+                               "their own: a step lasts from the last publication of a row's step k to that of a row's step k + 1, so "
                                "the first step carries the pipeline fill and single steps can come out below their byte time",
         })
         if verbose:
@@ -673,7 +673,7 @@ def main():
     roofline = {
         "bound": "hbm",
         "kernel": (kname + " (persistent: the whole decode loop in one launch; per row and step: fused mask read + masked "
-                   "logsumexp/argmax + transition; " + ("row groups advance independently, no barrier)" if args.loop_mode == "auto"
+                   "logsumexp/argmax + transition; " + ("every row advances on its own, no barrier)" if args.loop_mode == "auto"
                                                         else "grid barrier between steps)")) if persistent else
                   "cd::step_kernel (fused mask + masked logsumexp/argmax + CSR transition), one launch per decoding step",
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
