@@ -256,6 +256,49 @@ CD_API cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, cons
                      void* cuda_stream);
 
 /*
+ * cd_compact for callers that must not allocate device memory while they decode.
+ *
+ * Who that is.  This library usually shares its GPU with the LM server that produces the
+ * logits, and such a server claims nearly all of HBM for weights and KV cache when it starts
+ * (the paper's set-up runs a quantised model on one 16 GB card).
+ * A query engine that decodes next to it has three reasons not to ask the driver for memory
+ * per call: the request can fail with out-of-memory although the work needs a few KB; the
+ * plain allocator synchronises the whole device, stalling the server's streams; and the
+ * stream-ordered allocator that cd_compact uses for long lists needs a memory pool, which some
+ * deployments switch off or cap (a pool owned by the engine's own caching allocator, MPS
+ * clients with a pinned memory limit, processes running under a fixed cgroup-style HBM
+ * budget).  For them the multi-CTA scan of cd_compact exists in a form whose only scratch --
+ * one 64-bit word per 4096-slot chunk plus a ticket -- lives in a fixed array inside the
+ * library image: CD_COMPACT_NOALLOC_MAX_N / 4096 + 1 words = 32,776 bytes, held by every GPU
+ * on which the library is loaded until the process exits.
+ *
+ * Same arguments, same result as cd_compact (a6: stable partition keeping done[i] == 0; the
+ * first *n_active_out entries of row_ids_out / state_out are written; DEVICE pointers, all on
+ * one device, the one n_active_out lives on).  This call never calls cudaMalloc, cudaFree,
+ * their Async forms or any library routine that allocates: one cudaMemsetAsync over the words
+ * it is about to use (they keep the previous call's values and must start at zero) and one
+ * kernel launch, both on cuda_stream.
+ *
+ * Limits and rules that cd_compact does not have:
+ *   - n <= CD_COMPACT_NOALLOC_MAX_N (2^24 slots).  A longer list is refused with CD_ERR_ARG and
+ *     a message naming the limit; nothing is launched.  Split the list or call cd_compact.
+ *   - There is ONE array per GPU and every call on that GPU uses it.  Two calls whose kernels
+ *     may run at the same time (different streams, different host threads, two handles --
+ *     the array belongs to the library, not to an automaton) race on it and return garbage
+ *     or spin: keep calls on one stream, or order them with events.  Calls on different
+ *     GPUs do not interact.
+ *   - The first call on each GPU resolves the array's device address (cudaGetSymbolAddress,
+ *     with that GPU current; this is also when a lazily loaded CUDA module is brought onto the
+ *     device).  Make that first call during set-up, outside any stream capture; a call with
+ *     n = 0 is enough.
+ * Errors: CD_ERR_ARG (as cd_compact, plus n above the limit), CD_ERR_CUDA.
+ */
+#define CD_COMPACT_NOALLOC_MAX_N (1 << 24)
+CD_API cd_status cd_compact_noalloc(const uint8_t* done, const int32_t* row_ids_in, const int32_t* state_in,
+                             int32_t n, int32_t* row_ids_out, int32_t* state_out, int32_t* n_active_out,
+                             void* cuda_stream);
+
+/*
  * The whole loop: every row starts in the start state; for
  * k = 0 .. max_steps-1 the active rows take one cd_step on step_logits[k]
  * (DEVICE pointers in a HOST array; each [B, ld_elems], indexed by ORIGINAL row

@@ -16,6 +16,8 @@ from .binding import (  # noqa: F401
     CdError,
     Dfa,
     compact,
+    compact_noalloc,
+    COMPACT_NOALLOC_MAX_N,
     build_list,
     compile_dfa,
     compile_list,

@@ -19,7 +19,7 @@ STATUS = {0: "CD_OK", 1: "CD_ERR_ARG", 2: "CD_ERR_AUTOMATON", 3: "CD_ERR_DEAD_ST
 # every symbol include/cd.h declares (tests check the .so exports each of them)
 SYMBOLS = (
     "cd_compile_dfa", "cd_build_trie", "cd_compile_trie", "cd_build_list", "cd_set_loop_mode", "cd_loop_trace", "cd_compile_list", "cd_free_dfa", "cd_dfa_info", "cd_set_gather_max", "cd_set_sampling", "cd_reserve", "cd_step",
-    "cd_transition", "cd_compact", "cd_decode_loop", "cd_decode_loop_async", "cd_loop_sync", "cd_set_satisfying", "cd_set_limit", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_probe_read", "cd_decode_loop_cb", "cd_head_decode_loop_cb", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
+    "cd_transition", "cd_compact", "cd_compact_noalloc", "cd_decode_loop", "cd_decode_loop_async", "cd_loop_sync", "cd_set_satisfying", "cd_set_limit", "cd_decode_loop_limit", "cd_decode_loop_host", "cd_set_head_gather_max", "cd_head_step", "cd_head_decode_loop", "cd_head_decode_loop_host", "cd_probe_read", "cd_decode_loop_cb", "cd_head_decode_loop_cb", "cd_dedup", "cd_join_results", "cd_filter_rows", "cd_launch_count",
     "cd_last_error",
 )
 
@@ -317,6 +317,33 @@ def compact(done: torch.Tensor, row_ids: Optional[torch.Tensor] = None, state: O
     with torch.cuda.device(dev):
         _check(lib().cd_compact(_ptr(done), _ptr(row_ids), _ptr(state), C.c_int32(n), _ptr(ro), _ptr(so), _ptr(na),
                                 _stream(dev)))
+    return ro, so, na
+
+
+COMPACT_NOALLOC_MAX_N = 1 << 24
+
+
+def compact_noalloc(done: torch.Tensor, row_ids: Optional[torch.Tensor], state: Optional[torch.Tensor], out,
+                    n: Optional[int] = None):
+    """cd_compact_noalloc: `compact` for processes that may not allocate device memory while they
+    decode -- an engine living beside an LM server that has reserved almost all of HBM, or one
+    whose stream-ordered memory pool is disabled or capped.  The scan's scratch is a fixed 32 KB
+    array inside libcd.so, so the library allocates nothing; for the same reason this wrapper
+    allocates nothing either: `out` = (row_ids_out i32[>= n], state_out i32[>= n] or None,
+    n_active i32[1]) is required and returned.  At most COMPACT_NOALLOC_MAX_N slots per call
+    (CdError with code CD_ERR_ARG above that).  All calls on a GPU share the array: keep them
+    on one stream.  Make the first call on each GPU during set-up, before any stream capture."""
+    dev = done.device
+    _dev_tensor(done, torch.uint8, "done", dev)
+    n = done.numel() if n is None else n
+    if row_ids is not None:
+        _dev_tensor(row_ids, torch.int32, "row_ids", dev)
+    if state is not None:
+        _dev_tensor(state, torch.int32, "state", dev)
+    ro, so, na = out
+    with torch.cuda.device(dev):
+        _check(lib().cd_compact_noalloc(_ptr(done), _ptr(row_ids), _ptr(state), C.c_int32(n), _ptr(ro), _ptr(so),
+                                        _ptr(na), _stream(dev)))
     return ro, so, na
 
 

@@ -1116,6 +1116,54 @@ cd_status launch_compact(const uint8_t* done, const int* row_ids_in, const int* 
     return CD_OK;
 }
 
+// ---- cd_compact_noalloc (include/cd.h): the look-back compaction with its chunk words in the library image.
+// A caller that shares the GPU with an LM server holding nearly all of HBM, or that runs without a usable
+// memory pool, cannot afford launch_compact's cudaMallocAsync; this array is the scratch it gets instead.
+// One word per 4096-slot chunk + the ticket word behind the words in use: 4097 x 8 = 32,776 bytes on every
+// GPU that loads the library, until the process exits.  Shared by all calls on a GPU (see the header).
+constexpr int NOALLOC_MAX_CHUNKS = CD_COMPACT_NOALLOC_MAX_N / cd::SCAN_CHUNK;
+static_assert(CD_COMPACT_NOALLOC_MAX_N % cd::SCAN_CHUNK == 0, "the limit is a whole number of chunks");
+static __device__ __align__(256) unsigned long long g_noalloc_tiles[NOALLOC_MAX_CHUNKS + 1];
+
+// In host code `g_noalloc_tiles` is only a handle for the runtime, not an address a kernel may use: the
+// device address is asked for once per GPU, with that GPU current, and kept.  No allocation afterwards.
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mu;
+unsigned long long* g_noalloc_addr[NOALLOC_MAX_DEVICES] = {};
+
+cd_status noalloc_tiles_of(int dev, unsigned long long** out) {  // `dev` is the current device
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) return fail(CD_ERR_ARG, "cd_compact_noalloc: device ordinal %d not supported", dev);
+    std::lock_guard<std::mutex> lk(g_noalloc_mu);
+    if (!g_noalloc_addr[dev]) {
+        void* p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_noalloc_tiles));
+        if (!p) return fail(CD_ERR_CUDA, "cd_compact_noalloc: no device address for the scratch array on device %d", dev);
+        g_noalloc_addr[dev] = static_cast<unsigned long long*>(p);
+    }
+    *out = g_noalloc_addr[dev];
+    return CD_OK;
+}
+
+cd_status launch_compact_noalloc(const uint8_t* done, const int* row_ids_in, const int* state_in, int n, int* row_ids_out,
+                                 int* state_out, int* n_out, cudaStream_t stream) {
+    int dev = 0;
+    cd_status st = device_of(n_out, &dev);
+    if (st != CD_OK) return st;
+    DeviceGuard guard(dev);
+    if (!guard.ok) return fail(CD_ERR_CUDA, "cd_compact_noalloc: cannot make device %d current", dev);
+    unsigned long long* tile = nullptr;
+    st = noalloc_tiles_of(dev, &tile);
+    if (st != CD_OK) return st;
+    const int chunks = n > 0 ? (n + cd::SCAN_CHUNK - 1) / cd::SCAN_CHUNK : 1;
+    // the words of this call (chunk states + ticket) still hold the last call's prefixes: back to zero, in stream order
+    CU(cudaMemsetAsync(tile, 0, sizeof(unsigned long long) * ((size_t)chunks + 1), stream));
+    cd::compact_lookback_kernel<<<chunks, 1024, 0, stream>>>(done, row_ids_in, state_in, n, row_ids_out, state_out, n_out,
+                                                            nullptr, tile, reinterpret_cast<int*>(tile + chunks));
+    CU(cudaGetLastError());
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    return CD_OK;
+}
+
 // End of every loop: one read of the error counter (and of the persistent loop's abort flag) and the one
 // stream synchronisation the loops promise.
 cd_status finish_loop(Scratch* s, cudaStream_t stream, bool persistent) {
@@ -1278,6 +1326,20 @@ cd_status cd_compact(const uint8_t* done, const int32_t* row_ids_in, const int32
     if (n > 0 && state_in && !state_out) return fail(CD_ERR_ARG, "state_in given without state_out");
     return launch_compact(done, row_ids_in, state_in, n, row_ids_out, state_out, n_active_out, nullptr,
                           static_cast<cudaStream_t>(cuda_stream));
+}
+
+// cd_compact without any allocation: the scan's chunk words are the library's own fixed array (see above and cd.h).
+cd_status cd_compact_noalloc(const uint8_t* done, const int32_t* row_ids_in, const int32_t* state_in, int32_t n,
+                             int32_t* row_ids_out, int32_t* state_out, int32_t* n_active_out, void* cuda_stream) {
+    if (n < 0) return fail(CD_ERR_ARG, "n < 0");
+    if (n > CD_COMPACT_NOALLOC_MAX_N)
+        return fail(CD_ERR_ARG, "cd_compact_noalloc: n = %d is above the fixed scratch of this entry point (at most %d slots per call); "
+                    "split the list or use cd_compact", (int)n, (int)CD_COMPACT_NOALLOC_MAX_N);
+    if (!n_active_out) return fail(CD_ERR_ARG, "n_active_out is NULL");
+    if (n > 0 && (!done || !row_ids_out)) return fail(CD_ERR_ARG, "NULL pointer");
+    if (n > 0 && state_in && !state_out) return fail(CD_ERR_ARG, "state_in given without state_out");
+    return launch_compact_noalloc(done, row_ids_in, state_in, n, row_ids_out, state_out, n_active_out,
+                                  static_cast<cudaStream_t>(cuda_stream));
 }
 
 static cd_status decode_loop_impl(const cd_dfa_t* d, const void* const* step_logits, cd_dtype dtype, int64_t ld_elems,
