@@ -12,6 +12,7 @@ from .oracle_cd import (  # noqa: F401
     dedup,
     det_logf,
     gumbel,
+    fmix32,
     sample_decode_loop,
     sample_step,
     filter_rows,

@@ -487,7 +487,8 @@ int orc_filter_rows(const int32_t *final_state, const uint8_t *done, const int32
  * Outputs: logprob = log softmax(y)[t*] = (y_t* - m) - log(sum), lse = m + log(sum), with
  * sum = sum_{t in A} exp(y_t - m) accumulated in double as in O2.
  */
-static uint32_t orc_fmix32(uint32_t h)
+/* murmur3's 32-bit finalizer (public domain; exported so that a test can hold it against the published vectors) */
+uint32_t orc_fmix32(uint32_t h)
 {
     h ^= h >> 16;
     h *= 0x85EBCA6Bu;

@@ -68,6 +68,8 @@ def _load():
         _lib.orc_sample_decode_loop.restype = C.c_int
         _lib.orc_det_logf.restype = C.c_float
         _lib.orc_det_logf.argtypes = [C.c_float]
+        _lib.orc_fmix32.restype = C.c_uint32
+        _lib.orc_fmix32.argtypes = [C.c_uint32]
         _lib.orc_gumbel.restype = C.c_float
         _lib.orc_gumbel.argtypes = [C.c_uint32] * 5
         _lib.orc_join_results.restype = C.c_int
@@ -321,6 +323,11 @@ def filter_rows(final_state, done, satisfying, row_ids=None):
 def det_logf(x: float) -> float:
     """The fp32 logarithm of the sampling definition (O10)."""
     return float(_load().orc_det_logf(C.c_float(x)))
+
+
+def fmix32(h: int) -> int:
+    """The 32-bit mixing function of the counter-based generator (O10)."""
+    return int(_load().orc_fmix32(h & 0xFFFFFFFF))
 
 
 def gumbel(seed: int, row: int, step: int, tok: int) -> float:

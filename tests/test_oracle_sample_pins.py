@@ -114,3 +114,60 @@ def test_sampled_loop_replays_as_steps_and_list_filter(oracle):
     assert np.array_equal(got["tokens"], want_tok) and np.array_equal(got["len"], want_len)
     assert np.allclose(got["sum_logprob"], want_slp, rtol=0, atol=1e-12)
     assert want_len.max() > 1
+
+
+# ---------------------------------------------------------------- the integer side of the generator, from outside
+# MurmurHash3_x86_32 of the EMPTY key is fmix32(seed) (no blocks, no tail, length 0), so the reference vectors
+# that every murmur3 port is verified with pin the finalizer itself:
+#   murmur3_32("", seed 0) = 0x00000000, ("", seed 1) = 0x514E28B7, ("", seed 0xFFFFFFFF) = 0x81F16F39
+MURMUR3_EMPTY_KEY = [(0x00000000, 0x00000000), (0x00000001, 0x514E28B7), (0xFFFFFFFF, 0x81F16F39)]
+
+
+def test_fmix32_against_murmur3_published_vectors(oracle):
+    for seed, want in MURMUR3_EMPTY_KEY:
+        assert oracle.fmix32(seed) == want, (hex(seed), hex(oracle.fmix32(seed)), hex(want))
+    # a bijection on 32-bit words (xorshifts and odd multipliers): no two of many inputs collide
+    xs = np.random.default_rng(5).integers(0, 2**32, size=20000, dtype=np.uint64)
+    assert len({oracle.fmix32(int(x)) for x in set(xs.tolist())}) == len(set(xs.tolist()))
+    # avalanche: flipping one input bit flips about half of the output bits
+    flips = [bin(oracle.fmix32(int(x)) ^ oracle.fmix32(int(x) ^ (1 << b))).count("1") for x in xs[:300] for b in range(32)]
+    assert 15.0 < np.mean(flips) < 17.0 and min(flips) >= 1
+
+
+AXES = ["seed_lo", "seed_hi", "row", "step", "tok"]
+
+
+def _g(oracle, seed_lo=0x9ABCDEF0, seed_hi=0x12345678, row=1234, step=7, tok=4321):
+    return oracle.gumbel((seed_hi << 32) | seed_lo, row, step, tok)
+
+
+@pytest.mark.parametrize("axis", AXES)
+def test_noise_depends_on_every_input_varied_alone(oracle, axis):
+    """A generator that dropped (or merely truncated) one of its five inputs would return a constant, or a short
+    cycle, along that axis.  4096 consecutive values of the axis and 4096 values with only a high bit pattern
+    changing: all distinct uniforms, uniformly spread, and neighbours uncorrelated."""
+    n = 4096
+    for vals in (range(n), [(i * 0x00100001) & 0xFFFFFFFF for i in range(n)], [(i << 20) & 0xFFFFFFFF for i in range(n)]):
+        g = np.array([_g(oracle, **{axis: int(v)}) for v in vals])
+        u = np.exp(-np.exp(-g))
+        assert len(np.unique(g)) > 0.995 * n, (axis, len(np.unique(g)))  # (24-bit uniforms: a few birthdays at most)
+        hist, _ = np.histogram(u, bins=16, range=(0.0, 1.0))
+        chi2 = float(((hist - n / 16) ** 2 / (n / 16)).sum())
+        assert chi2 < 45.0, (axis, chi2)  # 15 degrees of freedom: P(chi2 > 45) ~ 8e-5
+        c = np.corrcoef(u[:-1], u[1:])[0, 1]
+        assert abs(c) < 0.08, (axis, c)  # 5 sigma of 1 / sqrt(n)
+
+
+def test_noise_streams_of_different_inputs_are_unrelated(oracle):
+    """Two axes never alias: the stream over tokens of (row r, step k) is uncorrelated with the one of (row r + 1,
+    step k), (row r, step k + 1), of the swapped pair (row k, step r), and of a seed differing in its high or low
+    word only."""
+    n = 4096
+    def stream(**kw):
+        return np.exp(-np.exp(-np.array([_g(oracle, tok=t, **kw) for t in range(n)])))
+    base = stream(row=10, step=3)
+    others = [stream(row=11, step=3), stream(row=10, step=4), stream(row=3, step=10),
+              stream(row=10, step=3, seed_hi=0x12345679), stream(row=10, step=3, seed_lo=0x9ABCDEF1)]
+    for o in others:
+        assert not np.array_equal(o, base)
+        assert abs(np.corrcoef(base, o)[0, 1]) < 0.08
