@@ -542,21 +542,47 @@ def run_reference(args, rank):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "logits_dtype": str(cfg.dtype).replace("torch.", ""),
         "data": "synthetic", "config": {"workload": cfg.desc, "sample": sample},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "host_cores": os.cpu_count(), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "row_steps_per_s": row_steps * args.steps / total,
     }
     print(json.dumps(line), flush=True)
 
 
+def launcher_command(args_gpus: int, argv, master_port: int = 0):
+    """`python bench.py --gpus N` with N > 1 outside torchrun: the command that starts N ranks of this same
+    script on this node (one rank per GPU over NCCL; rendezvous on 127.0.0.1, the hostname may not resolve)."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args_gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(master_port or 29500 + os.getpid() % 2000)]
+    return cmd + [os.path.abspath(__file__)] + list(argv)
+
+
+def check_gpus(requested: int, visible: int):
+    """A request for more GPUs than the node shows is an error, never a silent 1-GPU run."""
+    if requested < 1:
+        raise SystemExit(f"bench.py: --gpus {requested}: need at least one GPU")
+    if requested > visible:
+        raise SystemExit(f"bench.py: --gpus {requested} requested but only {visible} CUDA device(s) are visible on this "
+                         "node; refusing to report a smaller run under that label")
+
+
 def main():
     args = parse_args()
+    if args.impl != "reference" and "WORLD_SIZE" not in os.environ:
+        check_gpus(args.gpus, torch.cuda.device_count() if torch.cuda.is_available() else 0)
+        if args.gpus > 1:  # start the ranks ourselves: the line then reports n_gpus = the ranks that ran
+            env = dict(os.environ)
+            env.setdefault("NCCL_DEBUG", "INFO")  # the communicator's rank count is in the log (stderr)
+            env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+            raise SystemExit(subprocess.call(launcher_command(args.gpus, sys.argv[1:]), env=env))
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if args.impl == "reference":
         run_reference(args, rank)
         return
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started {world} rank(s); they must agree")
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
     import paper_2606_31808_b200 as cd
@@ -854,7 +880,7 @@ def main():
             if time.perf_counter() - t0 > 12.0 or reps >= 400:
                 break
         dt = time.perf_counter() - t0
-        cpu = {"value": R * reps / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+        cpu = {"value": R * reps / dt, "unit": UNIT, "cores": 1, "host_cores": os.cpu_count(), "kind": "oracle",
                "sample": f"rows [0,{R}) of one {cfg.name} batch, all {cfg.max_steps} steps, {reps} passes, "
                          f"{int(res['n_active_hist'].sum())} row-steps per pass (D2H copy excluded)",
                "row_steps_per_s": int(res["n_active_hist"].sum()) * reps / dt}
@@ -885,7 +911,9 @@ def main():
             "vs_baseline": None, "dtype": "f32", "logits_dtype": "bf16" if cfg.dtype == torch.bfloat16 else "f32",
             "data": "synthetic",
             "config": {
-                "workload": f"{cfg.name}: {cfg.desc}; one step = cd_decode_loop over one batch of B={cfg.B} rows",
+                "workload": f"{cfg.name}: {cfg.desc}; one step = cd_decode_loop over one batch of B={cfg.B} rows"
+                            + (f"; {len(batches)} of the table's {cfg.n_batches} batches resident per GPU, rotated over the timed steps"
+                               if getattr(cfg, "n_batches", 1) > 1 else f"; {len(batches)} seeded batches resident, rotated"),
                 "B": cfg.B, "V": cfg.V, "max_steps": cfg.max_steps, "S": aut.S, "nnz": aut.nnz,
                 "resident_batches": len(batches),
                 "l2": f"inputs larger than L2: {cfg.max_steps * cfg.B * sz_logit / 2**30:.1f} GiB of logits per step, "
