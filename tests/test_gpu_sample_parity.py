@@ -160,3 +160,74 @@ def test_sampled_full_size_c4_batch(cd, oracle):
         for k in ("tokens", "len", "final_state", "done"):
             assert np.array_equal(got[k].cpu().numpy(), want[k]), (lm, k)
     dfa.close()
+
+
+# ---------------------------------------------------------------- an independent check of the sampled token
+# The oracle's O10 restates the generator and its fp32 logarithm operation by operation, so bit-exact parity with it
+# does not by itself rule out a mistake both sides share.  Here the decision is recomputed a third way: the uniform
+# u of (seed, row, step, token) from a numpy statement of the counter hash (held against murmur3's published
+# finalizer vectors below), g = -log(-log u) with libm in float64, t* = argmax over the allowed set of y_t + g_t.
+# Wherever the winner leads the runner-up by more than the fp32 error of the kernel's y + g (the logarithm's 3e-7
+# relative error twice over, |g| <= 17, one rounding of the sum: < 1e-5) the GPU token must be that argmax.
+def _np_fmix32(h):
+    h = h.astype(np.uint64)
+    h ^= h >> np.uint64(16)
+    h = (h * np.uint64(0x85EBCA6B)) & np.uint64(0xFFFFFFFF)
+    h ^= h >> np.uint64(13)
+    h = (h * np.uint64(0xC2B2AE35)) & np.uint64(0xFFFFFFFF)
+    h ^= h >> np.uint64(16)
+    return h
+
+
+def _np_uniform(seed, row, step, toks):
+    M = np.uint64(0xFFFFFFFF)
+    lo, hi = np.uint64(seed & 0xFFFFFFFF), np.uint64(seed >> 32)
+    h = _np_fmix32(np.array([lo ^ ((np.uint64(row) * np.uint64(0x9E3779B1)) & M)]))
+    rk = _np_fmix32(h ^ ((np.uint64(step) * np.uint64(0x85EBCA77)) & M) ^ hi)
+    t = toks.astype(np.uint64)
+    hh = _np_fmix32((_np_fmix32(rk ^ ((t * np.uint64(0xC2B2AE3D)) & M)) + np.uint64(0x27D4EB2F)) & M)
+    return (2.0 * (hh >> np.uint64(9)).astype(np.float64) + 1.0) * 2.0**-24
+
+
+def test_numpy_generator_is_the_published_finalizer_and_the_oracles_uniform(oracle):
+    got = _np_fmix32(np.array([0, 1, 0xFFFFFFFF], dtype=np.uint64)).tolist()
+    assert got == [0x00000000, 0x514E28B7, 0x81F16F39]  # murmur3_32 of the empty key, seeds 0, 1, 0xFFFFFFFF
+    toks = np.arange(0, 3000, 7)
+    u = _np_uniform(0x1234567890ABCDEF, 77, 5, toks)
+    g = np.array([oracle.gumbel(0x1234567890ABCDEF, 77, 5, int(t)) for t in toks])
+    assert np.all(np.abs(-np.log(-np.log(u)) - g) <= 1e-5)
+
+
+@pytest.mark.parametrize("V,S,n,density,dtype,T", [
+    (40000, 12, 70, 0.05, torch.bfloat16, 0.7),
+    (262144, 16, 24, 0.02, torch.bfloat16, 1.3),
+    (5000, 5, 300, 1.0, torch.float32, 2.0),
+])
+def test_sampled_token_is_the_float64_gumbel_argmax(cd, mode, V, S, n, density, dtype, T):
+    seed, step = 0x0FEDCBA987654321, 9
+    aut = wl.make_random_dfa(52, V, S, density, 0.2)
+    dfa = dev_dfa(cd, aut, mode)
+    dfa.set_sampling(T, seed=seed, step_base=step)
+    x = wl.make_logits(52, 0, n + 10, V, 2.0, dtype)
+    states = live_states(aut, n)
+    row_map = [(i * 7 + 3) % (n + 10) for i in range(n)]
+    st_d = torch.tensor(states, dtype=torch.int32, device="cuda:0")
+    tok, _, _, _ = cd.step(dfa, x.to("cuda:0"), st_d, row_map=torch.tensor(row_map, dtype=torch.int32, device="cuda:0"))
+    tok = tok.cpu().numpy()
+    rp, tk = np.asarray(aut.row_ptr), np.asarray(aut.tok)
+    inv_T = np.float32(1.0) / np.float32(T)
+    decided = 0
+    for i in range(n):
+        A = tk[rp[states[i]]:rp[states[i] + 1]].astype(np.int64)
+        y = (x[row_map[i]].float().numpy()[A] * inv_T).astype(np.float64)  # y_t = fl32(x_t * fl32(1 / T))
+        score = y - np.log(-np.log(_np_uniform(seed, row_map[i], step, A)))
+        order = np.argsort(-score, kind="stable")
+        lead = score[order[0]] - score[order[1]] if A.size > 1 else np.inf
+        assert int(tok[i]) in set(A.tolist())
+        if lead > 1e-5 * max(1.0, abs(score[order[0]])):
+            decided += 1
+            assert int(tok[i]) == int(A[order[0]]), (i, int(tok[i]), int(A[order[0]]), lead)
+        else:  # a near tie: either of the two leaders
+            assert int(tok[i]) in (int(A[order[0]]), int(A[order[1]]))
+    assert decided >= 0.95 * n  # the check is not vacuous
+    dfa.close()
