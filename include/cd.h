@@ -45,6 +45,14 @@
  *     handle: two streams that need different settings use two handles (or
  *     order their calls).  cd_set_satisfying overwrites the device copy of the
  *     set in place: do not call it while a loop that uses a LIMIT is running;
+ *   - whole-loop kernels (cd_decode_loop, cd_decode_loop_async) occupy every SM and
+ *     finish only once each of their thread blocks has run, so two of them never
+ *     overlap on one GPU: launched on different streams of one process they run one
+ *     after the other (the library orders them; the first time a second stream is
+ *     used for a loop on a GPU costs one device synchronisation).  Two PROCESSES
+ *     that run loops on the same GPU at the same time are not ordered by anything
+ *     and can stall each other until the loop gives up with CD_ERR_INTERNAL: give
+ *     each process its own GPU, or use the per-step mode (cd_set_loop_mode);
  *   - logits rows start 16-byte aligned: the base pointer is 16-byte aligned
  *     and ld_elems * sizeof(element) is a multiple of 16; ld_elems >= V.
  *   - there is no CPU fallback: without a CUDA device every call fails with
@@ -338,24 +346,18 @@ CD_API cd_status cd_compact_noalloc(const uint8_t* done, const int32_t* row_ids_
  * CD_LOOP_AUTO a row step is cut into more work units when warps are waiting for work and into
  * fewer when the machine is busy, which does not change the result.  For the same reason
  * logprob_out / lse_out of cd_step do not depend on n, row_map or the other slots of the call.
- * cd_loop_trace returns, for the last loop that ran in a persistent kernel on (dfa, cuda_stream),
- * the number of decoding steps it ran (*steps_out), and for the first min(cap, 256) of them the
- * rows that took the step and its duration in nanoseconds measured on the device (HOST arrays;
- * without lock-step, step k lasts from the latest publication of a row's step k to the latest
- * publication of a row's step k + 1; *steps_out = 0 if that loop took the per-step path).  It
- * synchronises the stream.
+ * (Per-step timings of the last persistent loop: cd_loop_trace in cd_diag.h.)
  *
  * cd_decode_loop_async is cd_decode_loop without the synchronisation: it only enqueues the loop on
  * cuda_stream and returns (CD_LOOP_AUTO, no LIMIT: exactly one kernel launch).  The outputs are valid
  * once the stream has been synchronised; device-side failures of the loops enqueued on (dfa,
  * cuda_stream) since the last cd_loop_sync are reported by cd_loop_sync, which synchronises the
  * stream.  step_logits (the HOST array) may be reused as soon as the call returns.  Several loops may
- * be enqueued back to back on one stream; loops on different streams may run concurrently.
+ * be enqueued back to back on one stream; loops enqueued on different streams run one after the other
+ * (see Conventions: a whole-loop kernel occupies the GPU).
  */
 typedef enum { CD_LOOP_AUTO = 0, CD_LOOP_PER_STEP = 1, CD_LOOP_BARRIER = 2 } cd_loop_mode;
 CD_API cd_status cd_set_loop_mode(cd_dfa_t* dfa, int32_t mode);
-CD_API cd_status cd_loop_trace(const cd_dfa_t* dfa, void* cuda_stream, int32_t cap, int64_t* t_ns_out,
-                        int32_t* n_active_out, int32_t* steps_out);
 CD_API cd_status cd_decode_loop_async(const cd_dfa_t* dfa, const void* const* step_logits, cd_dtype dtype,
                          int64_t ld_elems, int32_t B, int32_t max_steps, int32_t* tokens_out,
                          int32_t* len_out, int32_t* final_state_out, float* sum_logprob_out,
@@ -525,17 +527,6 @@ CD_API cd_status cd_head_decode_loop_host(const cd_dfa_t* dfa, const void* const
                                    void* cuda_stream);
 
 /*
- * Measurement aid for the roofline: streams `bytes` (>= 8192, rounded down to
- * 8 KiB tiles) of the DEVICE buffer `buf` (16-byte aligned) through the copy machinery of the
- * step kernel -- per-warp rings of 1-D bulk async copies, 12 warps x 2 stages x 8 KiB per SM --
- * with no arithmetic, `iters` times after 2 warm-up launches, and writes the average duration
- * of one pass in milliseconds to *ms_out (HOST float).  bytes / time is what a pure-read
- * kernel of this shape reaches on this GPU; bench.py reports it beside the measured copy
- * peak.  Synchronises the stream.
- */
-CD_API cd_status cd_probe_read(const void* buf, int64_t bytes, int32_t iters, float* ms_out, void* cuda_stream);
-
-/*
  * Callback forms of the loops ("how a real LM forward would plug in").  Before
  * decoding step k the library calls, on the calling host thread,
  *     next_logits(user, k, d_row_ids, d_n_active, n_upper, &logits, &ld_elems, &by_slot)
@@ -561,10 +552,6 @@ CD_API cd_status cd_head_decode_loop_cb(const cd_dfa_t* dfa, cd_next_hidden_fn n
                                  int64_t ldw_elems, int32_t H, int32_t B, int32_t max_steps,
                                  int32_t* tokens_out, int32_t* len_out, int32_t* final_state_out,
                                  float* sum_logprob_out, uint8_t* done_out, void* cuda_stream);
-
-/* Number of kernel launches this library has enqueued from the calling thread's
-   process so far (monotone; used by bench.py to report gpu_launches). */
-CD_API int64_t cd_launch_count(void);
 
 /* Message of the last failure on the calling thread ("" if none). */
 CD_API const char* cd_last_error(void);

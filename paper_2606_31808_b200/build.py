@@ -20,7 +20,7 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libcd.so")
 SOURCES = [os.path.join(CSRC, "cd_api.cu")]
 DEPS = [os.path.join(CSRC, f) for f in ("cd_api.cu", "cd_step.cuh", "cd_head.cuh", "cd_dedup.cuh", "cd_types.hpp", "cd_aux.cuh", "cd_common.cuh")] + [
-    os.path.join(ROOT, "include", "cd.h")
+    os.path.join(ROOT, "include", "cd.h"), os.path.join(ROOT, "include", "cd_diag.h")
 ]
 
 NVCC_FLAGS = [

@@ -17,6 +17,7 @@
 #include <vector>
 
 #include "../../include/cd.h"
+#include "../../include/cd_diag.h"
 #include "cd_aux.cuh"
 #include "cd_common.cuh"
 #include "cd_step.cuh"
@@ -373,6 +374,13 @@ cd_status get_scratch(const cd_dfa* cd_, cudaStream_t stream, int rows, Scratch*
         s.b.release();
         s.b = fresh;
         s.trace_src = 0;
+        // The fresh counters restart the launch generation at 1, and flow_kernel's queue ring is tagged with
+        // generations: entries left by earlier loops would read as already published.  The stream is idle here
+        // (synchronised above if anything ever ran on these buffers): drop the ring, get_flow_scratch makes a
+        // zeroed one.
+        cudaFree(s.f_task);
+        s.f_task = nullptr;
+        s.f_task_cap = 0;
     }
     *out = &s;
     return CD_OK;
@@ -499,8 +507,8 @@ cd_status launch_loop_v(const cd::StepArgs& a, const cd::LoopArgs& L, int grid, 
     return launch_loop_t<DT>(a, L, grid, stream, fits);
 }
 
-// Persistent loop without a barrier (flow_kernel): a plain launch -- no warp of it ever waits for a warp that
-// is not running, so it needs no co-residency guarantee.
+// Persistent loop without a barrier (flow_kernel): a plain launch.  Its CTAs need not be resident together, but each
+// of them must get to run (a warp's first unit is its global id): see FlowOrder for what that asks of the host.
 template <int DT, bool GATHER = false, bool SAMPLE = false>
 cd_status launch_flow_t(const cd::StepArgs& a, const cd::FlowArgs& F, int grid, cudaStream_t stream) {
     auto kern = cd::flow_kernel<DT, STEP_WARPS, STEP_STAGES, STEP_TILE, GATHER, SAMPLE>;
@@ -894,6 +902,22 @@ cd_status enqueue_persistent_loop(const cd_dfa* d, const Settings& cfg, Scratch*
 
 cd_status get_loop_scratch(Scratch* s, int max_steps, cudaStream_t stream);
 
+// Order of flow_kernel launches on one device across the streams of this process.  While the process has used a
+// single stream for these loops nothing is added: stream order does it, and back-to-back loops keep their
+// programmatic overlap.  When a second stream shows up the device is synchronised once; from then on every launch
+// records an event and a launch on another stream waits for the one before it.  Loops of OTHER PROCESSES on the
+// same GPU are not covered: they can starve each other into the idle timeout (CD_ERR_INTERNAL), see cd.h.
+struct FlowOrder {
+    std::mutex mu;
+    cudaStream_t last = nullptr;
+    bool any = false, multi = false, ev_recorded = false;
+    cudaEvent_t ev = nullptr;
+};
+FlowOrder& flow_order(int dev) {
+    static FlowOrder o[64];
+    return o[dev & 63];
+}
+
 // flow_kernel: whether the loop fits the kernel's index ranges
 constexpr long long FLOW_RING_MAX = (512ll << 20) / (8 * cd::FLOW_ENTRY_WORDS);  // at most 512 MiB of queue
 
@@ -1012,9 +1036,37 @@ cd_status enqueue_flow_loop(const cd_dfa* d, const Settings& cfg, Scratch* s, co
         F.dbg_cap = tune_int_now("CD_DBG_CAP", 0);
     }
 #endif
-    st = dtype == CD_BF16 ? launch_flow_v<cd::DT_BF16>(a, F, grid, stream) : launch_flow_v<cd::DT_F32>(a, F, grid, stream);
+    {
+        // flow_kernel hands every warp its first unit by global warp id, so a launch ends only once ALL of its CTAs
+        // have run.  Two launches on two streams could each hold part of the SMs and wait for the rest until the
+        // idle timeout; launches on a device are therefore ordered across the streams of this process (FlowOrder).
+        FlowOrder& fo = flow_order(d->device);
+        std::lock_guard<std::mutex> lk(fo.mu);
+        if (fo.any && fo.last != stream) {
+            if (!fo.multi) {  // the second stream this process uses for these loops: from now on launches leave an event
+                CU(cudaDeviceSynchronize());
+                CU(cudaEventCreateWithFlags(&fo.ev, cudaEventDisableTiming));
+                fo.multi = true;
+            } else if (fo.ev_recorded) {
+                CU(cudaStreamWaitEvent(stream, fo.ev, 0));
+            }
+        }
+        st = dtype == CD_BF16 ? launch_flow_v<cd::DT_BF16>(a, F, grid, stream) : launch_flow_v<cd::DT_F32>(a, F, grid, stream);
+        if (st == CD_OK) {
+            if (fo.multi && cudaEventRecord(fo.ev, stream) == cudaSuccess) fo.ev_recorded = true;
+            fo.last = stream;
+            fo.any = true;
+        }
+    }
     if (st == CD_OK) s->trace_src = 2;
     return st;
+}
+
+// A loop that gave up (a row that never finished, a merge that timed out) leaves the tickets of its unfinished row
+// steps non-zero; the next loop on this scratch would count from them and merge too early.  Back to zero, in
+// stream order, before anything else runs on these buffers.
+void clear_tickets(Scratch* s, cudaStream_t stream) {
+    if (s->b.tickets) cudaMemsetAsync(s->b.tickets, 0, sizeof(int) * 2 * (size_t)s->b.cap_rows, stream);
 }
 
 // End of a flow_kernel loop: the one stream synchronisation the loops promise; the kernel has put its status
@@ -1024,6 +1076,7 @@ cd_status finish_flow_loop(Scratch* s, cudaStream_t stream) {
     if (!s->h_status) return CD_OK;
     const int err = reinterpret_cast<volatile int*>(s->h_status)[0];
     reinterpret_cast<volatile int*>(s->h_status)[0] = 0;
+    if (err != 0) clear_tickets(s, stream);
     if (err != 0)
         return fail(CD_ERR_INTERNAL, "%d device-side consistency failures (state out of range, token missing from the CSR or a row that never finished)", err);
     return CD_OK;
@@ -1172,6 +1225,7 @@ cd_status finish_loop(Scratch* s, cudaStream_t stream, bool persistent) {
     CU(cudaMemcpyAsync(h, s->b.ctrs, sizeof h, cudaMemcpyDeviceToHost, stream));
     if (persistent) CU(cudaMemcpyAsync(hb + 2, s->b.bar + cd::LB_ABORT, sizeof(int), cudaMemcpyDeviceToHost, stream));
     CU(cudaStreamSynchronize(stream));
+    if (hb[2] != 0 || h[2] != 0) clear_tickets(s, stream);
     if (hb[2] != 0)
         return fail(CD_ERR_INTERNAL, "the persistent loop kernel timed out at a grid barrier (device shared with a kernel that never ends?)");
     if (h[2] != 0)
@@ -1456,24 +1510,33 @@ cd_status cd_loop_trace(const cd_dfa_t* d, void* cuda_stream, int32_t cap, int64
     DeviceGuard guard(d->device);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     cd_dfa* dm = const_cast<cd_dfa*>(d);
+    *steps_out = 0;
     const unsigned long long* tt = nullptr;
     const int* tn = nullptr;
-    {
+    const int* f_q = nullptr;  // flow_kernel: which of its two buffer pairs is told by the launch counter's parity
+    const unsigned long long* ftt[2] = {nullptr, nullptr};
+    const int* ftn[2] = {nullptr, nullptr};
+    {  // only the pointers are taken under the handle's lock: other threads using the handle do not wait for this stream
         std::lock_guard<std::mutex> lk(dm->mu);
         auto it = dm->scratch.find(stream);
         if (it != dm->scratch.end() && it->second.trace_src == 1) {
             tt = it->second.b.trace_t;
             tn = it->second.b.trace_n;
         } else if (it != dm->scratch.end() && it->second.trace_src == 2) {
-            // flow_kernel: the buffers of the last launch are the ones the launch counter's parity no longer names
-            int par = 0;
-            CU(cudaMemcpyAsync(&par, it->second.b.f_q + cd::FQ_LAUNCHES, sizeof(int), cudaMemcpyDeviceToHost, stream));
-            CU(cudaStreamSynchronize(stream));
-            tt = it->second.b.f_trace_t[(par & 1) ^ 1];
-            tn = it->second.b.f_trace_n[(par & 1) ^ 1];
+            f_q = it->second.b.f_q;
+            for (int i = 0; i < 2; ++i) {
+                ftt[i] = it->second.b.f_trace_t[i];
+                ftn[i] = it->second.b.f_trace_n[i];
+            }
         }
     }
-    *steps_out = 0;
+    if (f_q) {  // the buffers of the last launch are the ones the launch counter's parity no longer names
+        int par = 0;
+        CU(cudaMemcpyAsync(&par, f_q + cd::FQ_LAUNCHES, sizeof(int), cudaMemcpyDeviceToHost, stream));
+        CU(cudaStreamSynchronize(stream));
+        tt = ftt[(par & 1) ^ 1];
+        tn = ftn[(par & 1) ^ 1];
+    }
     if (!tt) return CD_OK;  // the last loop on this stream did not run in a persistent kernel
     std::vector<unsigned long long> ht((size_t)cd::LOOP_TRACE_STEPS + 1);
     std::vector<int> hn((size_t)cd::LOOP_TRACE_STEPS + 1);
@@ -2251,9 +2314,15 @@ cd_status cd_join_results(const int32_t* rep, int32_t N, int32_t max_steps, cons
     if (st != CD_OK) return st;
     DeviceGuard guard(dev);
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    cd::join_kernel<<<grid_for((long long)N * (max_steps > 0 ? max_steps : 1), 256), 256, 0, stream>>>(
+    int vec_lanes = 0;  // lanes per token row on the 16-byte path (cd_dedup.cuh), 0 = element-wise copy
+    if (tokens_out && max_steps > 0 && max_steps % 4 == 0 && ((reinterpret_cast<uintptr_t>(tokens_out) | reinterpret_cast<uintptr_t>(tokens_d)) & 15) == 0) {
+        vec_lanes = 1;
+        while (vec_lanes < 32 && vec_lanes < max_steps / 4) vec_lanes <<= 1;
+    }
+    const long long threads = vec_lanes ? (long long)N * vec_lanes : (long long)N * (max_steps > 0 ? max_steps : 1);
+    cd::join_kernel<<<grid_for(threads, 256), 256, 0, stream>>>(
         rep, N, max_steps, tokens_d, len_d, final_state_d, sum_logprob_d, done_d, max_steps > 0 ? tokens_out : nullptr,
-        len_out, final_state_out, sum_logprob_out, done_out);
+        len_out, final_state_out, sum_logprob_out, done_out, vec_lanes);
     CU(cudaGetLastError());
     g_launches.fetch_add(1, std::memory_order_relaxed);
     return CD_OK;

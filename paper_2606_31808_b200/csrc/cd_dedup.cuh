@@ -82,9 +82,30 @@ __global__ void dedup_rep_kernel(const int* __restrict__ first, const int* __res
 __global__ void join_kernel(const int* __restrict__ rep, int N, int max_steps, const int* __restrict__ tokens_d,
                             const int* __restrict__ len_d, const int* __restrict__ fs_d, const float* __restrict__ slp_d,
                             const uint8_t* __restrict__ done_d, int* __restrict__ tokens, int* __restrict__ len,
-                            int* __restrict__ fs, float* __restrict__ slp, uint8_t* __restrict__ done) {
+                            int* __restrict__ fs, float* __restrict__ slp, uint8_t* __restrict__ done, int vec_lanes) {
     const long long nth = (long long)gridDim.x * blockDim.x;
     const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (vec_lanes > 0) {
+        // token rows of whole 16-byte vectors (max_steps % 4 == 0, both arrays 16-byte aligned): a group of vec_lanes
+        // lanes (a power of two <= 32) per row -- rep[i] is read once per row (one broadcast load per group), the
+        // history moves as int4, the group's first lane carries the row's scalar results
+        const int vpr = max_steps >> 2;
+        const int sub = (int)(tid & (vec_lanes - 1));
+        const int sh = __ffs(vec_lanes) - 1;  // (no 64-bit division on the index path)
+        for (long long i = tid >> sh; i < N; i += nth >> sh) {
+            const int r = rep[i];
+            if (sub == 0) {
+                if (len) len[i] = len_d[r];
+                if (fs) fs[i] = fs_d[r];
+                if (slp) slp[i] = slp_d[r];
+                if (done) done[i] = done_d[r];
+            }
+            const int4* __restrict__ src = reinterpret_cast<const int4*>(tokens_d + (long long)r * max_steps);
+            int4* __restrict__ dst = reinterpret_cast<int4*>(tokens + i * max_steps);
+            for (int k = sub; k < vpr; k += vec_lanes) dst[k] = __ldg(src + k);
+        }
+        return;
+    }
     for (long long i = tid; i < N; i += nth) {
         const int r = rep[i];
         if (len) len[i] = len_d[r];

@@ -286,16 +286,24 @@ constexpr int MODE_FLOW = 2;  // flow_kernel: whole loop, every row advances on 
 //     written (relaxed, no fence) by the warp that finalised the row's previous step, at the indices it reserved
 //     with one atomicAdd on q[1]; a word is either stale (older tag) or complete.  A row has at most MAX_CHUNKS
 //     entries that are reserved and not read yet, and it reserves the entries of its next step only after every
-//     unit of this one has been read, so with cap >= B * MAX_CHUNKS an entry is never overwritten before it was read.
+//     unit of this one has been read, so with cap >= B * MAX_CHUNKS at most cap entries are UNREAD at any time.
+//     That bounds their number, not the span of indices they cover: a warp holds the id of its next unit while it
+//     finishes the current one, and if the other rows meanwhile publish a full ring of entries (cap is 2 * B * chunks,
+//     at least 1024: possible only for a handful of rows running hundreds of steps past a stalled warp) the slot is
+//     rewritten with a later tag before that warp reads it.  The tag check turns this into a reader that never
+//     sees its tag -- the idle timeout ends the loop with CD_ERR_INTERNAL -- never into a wrong result.
 //   HOW MANY units a row's next step is cut into is decided when it is published, from how busy the machine is
 //   (entries published minus units drawn): the row's full set of chunks when warps are waiting for work -- the few
 //   rows of a long tail then spread over the whole machine and a step costs one chunk's latency --, down to
 //   64 KiB units when every warp already has work queued.  The canonical arithmetic (see MAX_CHUNKS) makes the
 //   result independent of that decision, so results stay bitwise reproducible.
 //   A warp whose next unit is not published yet keeps consuming what its ring holds, then polls the entry (and
-//   the stop word).  Units are only ever drawn by running warps and every published unit is drawn before any
-//   later one, so nothing waits for a warp that is not running: the launch needs no co-residency guarantee and
-//   two loops may share a device.
+//   the stop word).  Units taken from the counter are only ever drawn by running warps and every published unit is
+//   drawn before any later one.  The FIRST unit of a warp is not drawn: it is the warp's global id (see step_body),
+//   so the rows of step 0 are started only once every CTA of the launch has run -- the launch needs all its CTAs to
+//   get an SM eventually.  A kernel that ends frees them; ANOTHER flow loop does not end before its own CTAs all
+//   ran, so two of them on one device could hold each other up until the idle timeout.  The host orders these
+//   launches across the streams of a process (cd_api.cu FlowOrder); loops of different processes are not covered.
 //   q[2] counts the rows that left the loop (accepted, truncated at max_steps, failed); whoever brings it to B
 //   stores the launch generation into q[3], the stop word.  The last CTA to leave resets q[0..2], reports the
 //   error count q[4] to host_status (pinned, mapped host memory: no copy after the loop) and counts the launch
@@ -869,7 +877,7 @@ __device__ __forceinline__ void step_body(const StepArgs& a, const StepView& sv,
                 if (lane == 1) t = atomicAdd(tk, nch);
                 t = __shfl_sync(FULL, t, 1);
                 last = (t + nch == total);
-                if (last && lane == 1) *tk = 0;
+                if (last && lane == 1) atomicExch(tk, 0);  // (an atomic like the adds it is ordered with, not a plain store)
             }
             if (!last) return;
             if (MODE == MODE_FLOW && lane == 0) CD_DBG_MAX(F, dbg_rec, 4);

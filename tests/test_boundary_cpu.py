@@ -16,7 +16,8 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _header_symbols():
-    text = open(os.path.join(ROOT, "include", "cd.h")).read()
+    inc = os.path.join(ROOT, "include")  # cd.h: the decoding contract; cd_diag.h: measurement aids of the same library
+    text = "".join(open(os.path.join(inc, f)).read() for f in sorted(os.listdir(inc)) if f.endswith(".h"))
     return sorted(set(re.findall(r"CD_API[^;(]*?\b(cd_\w+)\s*\(", text)))
 
 

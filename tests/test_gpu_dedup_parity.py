@@ -109,3 +109,32 @@ def test_filter_rows_matches_oracle(cd, oracle, N):
         want = oracle.filter_rows(fs, dn, sat, row_ids=row_ids)
         assert int(no) == want.size
         assert np.array_equal(ro[: int(no)].cpu().numpy(), want)
+
+
+@pytest.mark.parametrize("max_steps", [1, 4, 6, 8, 16, 20, 132, 256])
+@pytest.mark.parametrize("N,D", [(1, 1), (33, 5), (70001, 977)])
+def test_join_copies_token_rows_of_every_width(cd, oracle, max_steps, N, D):
+    """LEFT JOIN back for histories of any length: rows of whole 16-byte vectors move as int4 with a
+    group of lanes per row (max_steps % 4 == 0: 1, 2, 4 ... 32 lanes), the others element by element; same result
+    as the oracle's O9, bit for bit, including an unaligned view of the history (element-wise path again)."""
+    rng = np.random.default_rng(max_steps * 1000 + N)
+    res_d = {
+        "tokens": torch.tensor(rng.integers(-1, 262144, size=(D, max_steps)).astype(np.int32), device="cuda:0"),
+        "len": torch.tensor(rng.integers(0, max_steps + 1, size=D).astype(np.int32), device="cuda:0"),
+        "final_state": torch.tensor(rng.integers(0, 4096, size=D).astype(np.int32), device="cuda:0"),
+        "sum_logprob": torch.tensor(rng.normal(size=D).astype(np.float32), device="cuda:0"),
+        "done": torch.tensor(rng.integers(0, 2, size=D).astype(np.uint8), device="cuda:0"),
+    }
+    rep = torch.tensor(rng.integers(0, D, size=N).astype(np.int32), device="cuda:0")
+    want = oracle.join_results(rep.cpu().numpy(), {k: v.cpu().numpy() for k, v in res_d.items()})
+    got = cd.join_results(rep, res_d)
+    torch.cuda.synchronize()
+    for k in ("tokens", "len", "final_state", "done"):
+        assert np.array_equal(got[k].cpu().numpy(), want[k]), k
+    assert np.array_equal(got["sum_logprob"].cpu().numpy(), want["sum_logprob"].astype(np.float32))
+    # the same history at an address that is not a multiple of 16 bytes
+    flat = torch.empty(D * max_steps + 1, dtype=torch.int32, device="cuda:0")
+    shifted = flat[1:].view(D, max_steps)
+    shifted.copy_(res_d["tokens"])
+    got2 = cd.join_results(rep, dict(res_d, tokens=shifted))
+    assert np.array_equal(got2["tokens"].cpu().numpy(), want["tokens"])
