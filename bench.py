@@ -323,7 +323,7 @@ def dedup_section(cd, device, iters, warmup):
             "join_ms": ms_j, "join_rows_per_s": N / (ms_j * 1e-3), "join_gbs": b_j / (ms_j * 1e-3) / 1e9,
             "join_frac_of_hbm_peak": b_j / (ms_j * 1e-3) / 1e9 / peak,
             "lm_calls_saved": f"{N - D} of {N} generations (factor {N / D:.0f})",
-            "note": "dedup is bound by hash-table atomics and the one-CTA stable scan, not by bytes; both are "
+            "note": "dedup is bound by hash-table atomics (2 per key onto few hot words: profiles/r3a_dedup_join.md), not by bytes; both are "
                     "negligible next to the decode loop they remove (256 batches x ~4 ms)"}
 
 
